@@ -1,0 +1,180 @@
+/*
+ * gsrq.h -- C ABI of libgsrq: the GSRQ residual-quantization encoder (weighted
+ * Gain-Shape K-means codebook fit + per-stage encode) and the stand-alone decode,
+ * hand-written CUDA for NVIDIA B200 (sm_100a).
+ *
+ * Citations are to the paper text, /root/reference/PAPER.md ("PAPER.md:<line>" plus
+ * section / equation / algorithm), and to DESIGN.md for the readings taken where the
+ * paper is silent.
+ *
+ * Conventions (all entry points)
+ *   - Every pointer is a DEVICE pointer owned by the caller, except: the small structs
+ *     (gsrq_view, gsrq_codebook -- host structs holding device pointers), `stats`
+ *     (host), and the *_host entry points at the bottom, which say so.
+ *   - The library allocates nothing that outlives a call; scratch comes from the
+ *     caller's `workspace` (>= gsrq_workspace_bytes(), 256-byte aligned).
+ *   - Calls are asynchronous on `stream`.  The only implied synchronisation is the
+ *     copy of `stats` to the host in gsrq_fit_stage (skipped when stats == NULL).
+ *   - Return value: GSRQ_OK (0) or a negative gsrq_status; never throws, never
+ *     aborts.  After an error the outputs are unspecified; gsrq_last_error() returns a
+ *     thread-local message.
+ *   - Same inputs => bit-identical outputs on every run (no floating-point atomics).
+ *   - There is no CPU fallback: without a CUDA device every compute entry point
+ *     returns GSRQ_ECUDA.
+ *
+ * Notation: a KV tensor of G heads x T tokens x hd
+ * channels is split into M = hd/d sub-vectors ("rows") of dimension d per (head,
+ * token) (Product Quantization); row i = t*M + m of head g is kv[g][t][m*d..m*d+d).
+ * Each head g and residual stage s has one codebook of K centroids
+ * mu_k = g_k * s_k, g_k >= 0, ||s_k|| = 1 (Eq. 3).  A code is the index k (uint8).
+ */
+#ifndef GSRQ_H_
+#define GSRQ_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GSRQ_MAX_ITERS 128 /* PAPER.md:479 "setting the maximum iteration to around 100 is sufficient" */
+#define GSRQ_MAX_K 256     /* codes are one byte; PAPER.md:250 uses K = 256 throughout */
+#define GSRQ_MAX_STAGES 32 /* PAPER.md:252 R = 32 for 2 BPA */
+
+typedef enum {
+  GSRQ_OK = 0,
+  GSRQ_EINVAL = -1,       /* bad shape / alignment / K > 256 / hd % d != 0 / NULL pointer */
+  GSRQ_EUNSUPPORTED = -2, /* valid request this build has no kernel for (d not in {8,16,32}) */
+  GSRQ_EWORKSPACE = -3,   /* workspace too small or misaligned */
+  GSRQ_ECUDA = -4,        /* CUDA runtime error (message in gsrq_last_error) */
+  GSRQ_EDEGENERATE = -5   /* a group has fewer than K distinct non-zero fit rows (init impossible) */
+} gsrq_status;
+
+enum { GSRQ_F32 = 0, GSRQ_BF16 = 1 };
+
+/* Strided view of one layer's K or V cache.  Innermost hd elements are contiguous.
+ * [G][T][hd] -> stride_g = T*hd, stride_t = hd;  [T][G][hd] -> stride_g = hd, stride_t = G*hd. */
+typedef struct {
+  int32_t dtype;    /* GSRQ_F32 or GSRQ_BF16 */
+  int32_t G;        /* codebook groups = KV heads */
+  int64_t T;        /* tokens (batch folded in) */
+  int32_t hd, d;    /* head_dim and sub-vector dim; hd % d == 0 */
+  int64_t stride_g; /* in elements */
+  int64_t stride_t; /* in elements */
+} gsrq_view;
+
+/* Codebooks of all stages (device arrays, caller-owned):
+ * shapes [G][S][K][d] fp32 unit-norm, gains [G][S][K] fp32 >= 0  (Eq. 3). */
+typedef struct {
+  int32_t K, S;
+  float *shapes;
+  float *gains;
+} gsrq_codebook;
+
+/* Per-group statistics of one gsrq_fit_stage call (host struct; pass an array of G). */
+typedef struct {
+  int32_t iters_run;     /* Lloyd iterations executed before Alg. 1 l.15-16 broke (<= iters) */
+  int32_t n_empty_last;  /* empty clusters at the last update (kept unchanged) */
+  int64_t n_changed_last;
+  int64_t n_refined;     /* rows whose arg-max went through the exact fp64 re-score */
+  double wdist_after_assign[GSRQ_MAX_ITERS]; /* J_t = sum_i w_i ||r_i - g s||^2 after iteration t's assignment */
+  int64_t n_changed[GSRQ_MAX_ITERS];         /* rows whose assignment changed at iteration t */
+} gsrq_fit_stats;
+
+/* Scratch size for any call on this view with these parameters.
+ * n_fit_tokens = 0 means "fit on all T tokens".  Host function, no CUDA calls. */
+size_t gsrq_workspace_bytes(const gsrq_view *view, int K, int S, int64_t n_fit_tokens);
+
+/*
+ * Fit the codebook of residual stage `stage` with weighted GSKM.
+ *   Algorithm 1 with per-sample weights (reading c-W):
+ *   init: K seeded distinct non-zero fit rows, normalised (Alg. 1 l.1; reading c-I), gains by
+ *   Eq. 8 under the max-projection assignment (l.2); then up to `iters` iterations of
+ *   assignment  k_i = argmax_k (2 g_k r_i.s_k - g_k^2), lowest k on ties   (Eq. 5)
+ *   update      s_k = normalize(sum w_i y_i), y_i = r_i/(||r_i|| + 1e-12)   (Eq. 6-7)
+ *               g_k = max(0, sum w_i r_i.s_k / sum w_i) with the new s_k    (Eq. 8)
+ *   with the safeguards of PAPER.md:178 (empty cluster and near-zero direction keep the old
+ *   value) and the early exit of Alg. 1 l.15-16.
+ * kv       : the tensor described by `view` (read-only).
+ * w        : [.][T] fp32 per-token weights, row of group g at w + g*w_stride_g (0 = shared);
+ *            NULL = uniform.  A sub-vector inherits its token's weight.
+ * fit_tokens: [G][n_fit] int64 sorted token ids the codebook is fitted on; NULL = all T
+ *            tokens (then n_fit is ignored).
+ * cb       : stages < `stage` are read (only when residual == NULL and stage > 0),
+ *            stage `stage` is written.
+ * residual : [G][T*M][d] fp32 residual after stage-1 (gsrq_encode's residual_out), or NULL:
+ *            stage 0 reads kv; stage > 0 re-derives the residual from kv and cb.
+ * seed     : selects the initial rows (splitmix64 stream, reading c-I).
+ * stats    : HOST array of G structs or NULL.  When given, the call synchronises `stream`
+ *            and returns GSRQ_EDEGENERATE if any group could not be initialised.
+ */
+int gsrq_fit_stage(const void *kv, const gsrq_view *view, const float *w, int64_t w_stride_g,
+                   const int64_t *fit_tokens, int64_t n_fit, gsrq_codebook *cb, int stage,
+                   const float *residual, int iters, uint64_t seed, gsrq_fit_stats *stats,
+                   void *workspace, size_t workspace_bytes, void *stream);
+
+/*
+ * Encode stages [stage_begin, stage_end) with fixed codebooks (RQ):
+ *   for s: a = argmax_k (2 g_k r.s_k - g_k^2) (Eq. 5); code = a; r <- fl32(r - fl32(g_a s_a)).
+ * codes       : [S][G][T*M] uint8, stage-major planes (a prefix of stages decodes alone,
+ *               PAPER.md:25).  Planes in range are written; when stage_begin > 0 the
+ *               planes < stage_begin are READ to rebuild the residual from kv.
+ * residual_out: [G][T*M][d] fp32 residual after stage_end-1, or NULL.
+ */
+int gsrq_encode(const void *kv, const gsrq_view *view, const gsrq_codebook *cb, int stage_begin,
+                int stage_end, uint8_t *codes, float *residual_out, void *workspace,
+                size_t workspace_bytes, void *stream);
+
+/*
+ * Decode the first n_stages stages (PAPER.md:56  x ~= sum_l C_l[i_l]; prefix PAPER.md:25):
+ *   xhat = ((c0[a0] + c1[a1]) + ...) in fp32, stage order, c_k = fl32(g_k s_k); one
+ *   round-to-nearest-even cast to out_view->dtype (reading c-D).
+ * kv_out is written through out_view (same striding rules as the input view).
+ */
+int gsrq_decode(const uint8_t *codes, const gsrq_codebook *cb, int n_stages, void *kv_out,
+                const gsrq_view *out_view, void *stream);
+
+/* ---- step-wise entry points (the lock-step parity protocol of DESIGN.md section 6) ---- */
+
+/* One assignment pass over ALL T*M rows of every group against stage `stage` of cb.
+ * rows come from `residual` ([G][T*M][d] fp32) when non-NULL, else from kv.
+ * mode 0: Eq. 5 score; mode 1: plain projection r.s_k (the init assignment, reading c-I).
+ * idx_out: [G][T*M] uint8. */
+int gsrq_assign(const void *kv, const gsrq_view *view, const float *residual,
+                const gsrq_codebook *cb, int stage, int mode, uint8_t *idx_out, void *workspace,
+                size_t workspace_bytes, void *stream);
+
+/* One update (Eq. 6-8 weighted + safeguards) of stage `stage` of cb from a GIVEN assignment
+ * idx [G][T*M] over all rows.  shapes_too = 0 updates gains only (Alg. 1 l.2). */
+int gsrq_update(const void *kv, const gsrq_view *view, const float *residual, const float *w,
+                int64_t w_stride_g, const uint8_t *idx, gsrq_codebook *cb, int stage,
+                int shapes_too, void *workspace, size_t workspace_bytes, void *stream);
+
+/* The K initial row ids gsrq_fit_stage would draw (local fit-row indices), ids_out [G][K] int64. */
+int gsrq_init_ids(const void *kv, const gsrq_view *view, const float *residual,
+                  const int64_t *fit_tokens, int64_t n_fit, int K, int stage, uint64_t seed,
+                  int64_t *ids_out, void *workspace, size_t workspace_bytes, void *stream);
+
+/* ---- host-buffer convenience (end-to-end measurement: H2D + kernels + D2H inside) ---- */
+
+/* gsrq_encode on HOST buffers: kv_host and codes_host are host pointers (pinned or pageable);
+ * cb holds DEVICE codebooks.  Allocates device scratch for the duration of the call, copies
+ * kv in, encodes [0,S), copies all S code planes out, synchronises. */
+int gsrq_encode_host(const void *kv_host, const gsrq_view *view, const gsrq_codebook *cb,
+                     uint8_t *codes_host);
+
+/* gsrq_decode on HOST buffers: codes_host in, kv_out_host out (contiguous per out_view). */
+int gsrq_decode_host(const uint8_t *codes_host, const gsrq_codebook *cb, int n_stages,
+                     void *kv_out_host, const gsrq_view *out_view);
+
+/* Thread-local message of the last error returned on this thread ("" if none). */
+const char *gsrq_last_error(void);
+
+/* Library version string, e.g. "gsrq-b200 0.1 (sm_100a)". */
+const char *gsrq_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GSRQ_H_ */

@@ -1,0 +1,157 @@
+"""Thin ctypes binding over libgsrq (include/gsrq.h): argument marshalling only.
+
+Functions carry the C names.  Tensors are torch CUDA tensors used purely as device
+memory; the current torch CUDA stream is passed as the stream.  There is no fallback:
+if the library is not built, or a call fails, this raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+import torch
+
+from . import build as _build
+
+GSRQ_MAX_ITERS = 128
+GSRQ_F32, GSRQ_BF16 = 0, 1
+_STATUS = {0: "GSRQ_OK", -1: "GSRQ_EINVAL", -2: "GSRQ_EUNSUPPORTED", -3: "GSRQ_EWORKSPACE",
+           -4: "GSRQ_ECUDA", -5: "GSRQ_EDEGENERATE"}
+
+
+class GsrqError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"{_STATUS.get(code, code)}: {msg}")
+        self.code = code
+
+
+class gsrq_view(C.Structure):
+    _fields_ = [("dtype", C.c_int32), ("G", C.c_int32), ("T", C.c_int64), ("hd", C.c_int32), ("d", C.c_int32),
+                ("stride_g", C.c_int64), ("stride_t", C.c_int64)]
+
+
+class gsrq_codebook(C.Structure):
+    _fields_ = [("K", C.c_int32), ("S", C.c_int32), ("shapes", C.c_void_p), ("gains", C.c_void_p)]
+
+
+class gsrq_fit_stats(C.Structure):
+    _fields_ = [("iters_run", C.c_int32), ("n_empty_last", C.c_int32), ("n_changed_last", C.c_int64),
+                ("n_refined", C.c_int64), ("wdist_after_assign", C.c_double * GSRQ_MAX_ITERS),
+                ("n_changed", C.c_int64 * GSRQ_MAX_ITERS)]
+
+
+_lib = None
+EXPORTS = ["gsrq_workspace_bytes", "gsrq_fit_stage", "gsrq_encode", "gsrq_decode", "gsrq_assign", "gsrq_update",
+           "gsrq_init_ids", "gsrq_encode_host", "gsrq_decode_host", "gsrq_last_error", "gsrq_version"]
+
+
+def lib_path() -> Path:
+    return _build.LIB
+
+
+def lib():
+    """Load libgsrq.so (built in-tree by paper_2607_01065_b200.build). Fails loudly if absent."""
+    global _lib
+    if _lib is None:
+        p = lib_path()
+        if not p.exists():
+            raise ImportError(f"{p} is not built: run `python -c 'import __graft_entry__ as g; g.build()'`")
+        _lib = C.CDLL(str(p))
+        _lib.gsrq_workspace_bytes.restype = C.c_size_t
+        _lib.gsrq_last_error.restype = C.c_char_p
+        _lib.gsrq_version.restype = C.c_char_p
+    return _lib
+
+
+def _check(rc):
+    if rc != 0:
+        raise GsrqError(rc, lib().gsrq_last_error().decode())
+
+
+def _ptr(t):
+    return C.c_void_p(t.data_ptr()) if t is not None else C.c_void_p(0)
+
+
+def _stream():
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def view_of(x: torch.Tensor, d: int, head_inner: bool = False) -> gsrq_view:
+    """View for a [G][T][hd] tensor (or [T][G][hd] when head_inner)."""
+    dt = {torch.float32: GSRQ_F32, torch.bfloat16: GSRQ_BF16}[x.dtype]
+    if head_inner:
+        T, G, hd = x.shape
+        sg, st = x.stride(1), x.stride(0)
+    else:
+        G, T, hd = x.shape
+        sg, st = x.stride(0), x.stride(1)
+    assert x.stride(2) == 1
+    return gsrq_view(dt, G, T, hd, d, sg, st)
+
+
+def codebook_of(shapes: torch.Tensor, gains: torch.Tensor) -> gsrq_codebook:
+    """shapes [G][S][K][d] fp32, gains [G][S][K] fp32, contiguous CUDA tensors."""
+    assert shapes.is_contiguous() and gains.is_contiguous() and shapes.dtype == torch.float32
+    return gsrq_codebook(shapes.shape[2], shapes.shape[1], shapes.data_ptr(), gains.data_ptr())
+
+
+def gsrq_version() -> str:
+    return lib().gsrq_version().decode()
+
+
+def gsrq_workspace_bytes(view: gsrq_view, K: int, S: int, n_fit_tokens: int = 0) -> int:
+    n = lib().gsrq_workspace_bytes(C.byref(view), K, S, C.c_int64(n_fit_tokens))
+    if n == 0:
+        raise GsrqError(-1, lib().gsrq_last_error().decode())
+    return n
+
+
+def workspace(view: gsrq_view, K: int, S: int, n_fit_tokens: int = 0, device="cuda") -> torch.Tensor:
+    return torch.empty(gsrq_workspace_bytes(view, K, S, n_fit_tokens), dtype=torch.uint8, device=device)
+
+
+def gsrq_fit_stage(kv, view, w, w_stride_g, fit_tokens, cb, stage, residual, iters, seed, ws, want_stats=True):
+    G = view.G
+    stats = (gsrq_fit_stats * G)() if want_stats else None
+    n_fit = 0 if fit_tokens is None else fit_tokens.shape[1]
+    rc = lib().gsrq_fit_stage(_ptr(kv), C.byref(view), _ptr(w), C.c_int64(w_stride_g), _ptr(fit_tokens),
+                              C.c_int64(n_fit), C.byref(cb), stage, _ptr(residual), iters, C.c_uint64(seed),
+                              stats, _ptr(ws), C.c_size_t(ws.numel()), _stream())
+    _check(rc)
+    return stats
+
+
+def gsrq_encode(kv, view, cb, stage_begin, stage_end, codes, residual_out, ws):
+    _check(lib().gsrq_encode(_ptr(kv), C.byref(view), C.byref(cb), stage_begin, stage_end, _ptr(codes),
+                             _ptr(residual_out), _ptr(ws), C.c_size_t(ws.numel()), _stream()))
+
+
+def gsrq_decode(codes, cb, n_stages, kv_out, out_view):
+    _check(lib().gsrq_decode(_ptr(codes), C.byref(cb), n_stages, _ptr(kv_out), C.byref(out_view), _stream()))
+
+
+def gsrq_assign(kv, view, residual, cb, stage, mode, idx_out, ws):
+    _check(lib().gsrq_assign(_ptr(kv), C.byref(view), _ptr(residual), C.byref(cb), stage, mode, _ptr(idx_out),
+                             _ptr(ws), C.c_size_t(ws.numel()), _stream()))
+
+
+def gsrq_update(kv, view, residual, w, w_stride_g, idx, cb, stage, shapes_too, ws):
+    _check(lib().gsrq_update(_ptr(kv), C.byref(view), _ptr(residual), _ptr(w), C.c_int64(w_stride_g), _ptr(idx),
+                             C.byref(cb), stage, int(shapes_too), _ptr(ws), C.c_size_t(ws.numel()), _stream()))
+
+
+def gsrq_init_ids(kv, view, residual, fit_tokens, K, stage, seed, ids_out, ws):
+    n_fit = 0 if fit_tokens is None else fit_tokens.shape[1]
+    _check(lib().gsrq_init_ids(_ptr(kv), C.byref(view), _ptr(residual), _ptr(fit_tokens), C.c_int64(n_fit), K, stage,
+                               C.c_uint64(seed), _ptr(ids_out), _ptr(ws), C.c_size_t(ws.numel()), _stream()))
+
+
+def gsrq_encode_host(kv_host: torch.Tensor, view, cb, codes_host: torch.Tensor):
+    """kv_host / codes_host are HOST tensors (pinned or pageable); copies happen inside the call."""
+    assert not kv_host.is_cuda and not codes_host.is_cuda
+    _check(lib().gsrq_encode_host(_ptr(kv_host), C.byref(view), C.byref(cb), _ptr(codes_host)))
+
+
+def gsrq_decode_host(codes_host: torch.Tensor, cb, n_stages, kv_out_host: torch.Tensor, out_view):
+    assert not kv_out_host.is_cuda and not codes_host.is_cuda
+    _check(lib().gsrq_decode_host(_ptr(codes_host), C.byref(cb), n_stages, _ptr(kv_out_host), C.byref(out_view)))

@@ -1,0 +1,420 @@
+// gsrq_lib.cu -- host side of libgsrq: argument checks, workspace plan, kernel launches.
+// Every step of the path runs in the kernels under csrc/; this file only orchestrates.
+#include <stdarg.h>
+#include <string.h>
+
+#include "gsrq_common.cuh"
+#include "k_codec.cuh"
+#include "k_prep.cuh"
+#include "k_reduce.cuh"
+#include "k_score.cuh"
+
+namespace gsrq {
+
+static_assert(sizeof(gsrq_view) == 40 && sizeof(gsrq_codebook) == 24 && sizeof(gsrq_fit_stats) == 24 + 16 * GSRQ_MAX_ITERS, "ABI layout");
+static thread_local char g_err[512] = "";
+
+void set_error(const char *fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+}
+
+static inline size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
+struct Plan {
+  long long nf_tok, Nf, Nall, C;
+  int M;
+  size_t off_Rf, off_rinv, off_wt, off_idx, off_list, off_part, off_st, off_cnt, off_ids, off_etot, total;
+};
+
+constexpr int kNumCounters = 256;
+
+static Plan make_plan(const gsrq_view *v, int K, int S, long long n_fit_tokens) {
+  (void)S;
+  Plan p;
+  p.M = v->hd / v->d;
+  p.nf_tok = (n_fit_tokens > 0) ? n_fit_tokens : v->T;
+  p.Nf = p.nf_tok * p.M;
+  p.Nall = v->T * p.M;
+  p.C = (p.Nf + kChunkRows - 1) / kChunkRows;
+  size_t o = 0;
+  p.off_Rf = o;   o += align_up((size_t)v->G * p.Nf * v->d * sizeof(float));
+  p.off_rinv = o; o += align_up((size_t)v->G * p.Nf * sizeof(double));
+  p.off_wt = o;   o += align_up((size_t)v->G * p.nf_tok * sizeof(float));
+  p.off_idx = o;  o += align_up((size_t)v->G * p.Nf);
+  p.off_list = o; o += align_up((size_t)v->G * p.Nall * sizeof(uint32_t));
+  p.off_part = o; o += align_up((size_t)v->G * p.C * K * (2 * v->d + 2) * sizeof(double));
+  p.off_st = o;   o += align_up((size_t)v->G * sizeof(DevStats));
+  p.off_cnt = o;  o += align_up(kNumCounters * sizeof(unsigned int));
+  p.off_ids = o;  o += align_up((size_t)v->G * GSRQ_MAX_K * sizeof(long long));
+  p.off_etot = o; o += align_up((size_t)v->G * sizeof(double));
+  p.total = o;
+  return p;
+}
+
+static int check_view(const gsrq_view *v, int K, int S) {
+  if (!v) { set_error("view is NULL"); return GSRQ_EINVAL; }
+  if (v->dtype != GSRQ_F32 && v->dtype != GSRQ_BF16) { set_error("view.dtype must be GSRQ_F32 or GSRQ_BF16"); return GSRQ_EINVAL; }
+  if (v->G <= 0 || v->T <= 0 || v->hd <= 0 || v->d <= 0 || v->hd % v->d) { set_error("bad view shape (G=%d T=%lld hd=%d d=%d)", v->G, (long long)v->T, v->hd, v->d); return GSRQ_EINVAL; }
+  if (K <= 0 || K > GSRQ_MAX_K) { set_error("K must be in [1, %d], got %d", GSRQ_MAX_K, K); return GSRQ_EINVAL; }
+  if (S <= 0 || S > GSRQ_MAX_STAGES) { set_error("S must be in [1, %d], got %d", GSRQ_MAX_STAGES, S); return GSRQ_EINVAL; }
+  if (v->d != 8 && v->d != 16 && v->d != 32) { set_error("d = %d: this build has kernels for d in {8, 16, 32}", v->d); return GSRQ_EUNSUPPORTED; }
+  const int al = (v->dtype == GSRQ_BF16) ? 8 : 4;  // 16-byte vector loads
+  if (v->stride_g % al || v->stride_t % al) { set_error("strides must be multiples of %d elements (16-byte loads)", al); return GSRQ_EINVAL; }
+  if ((long long)v->G * v->T * (v->hd / v->d) >= (1LL << 32)) { set_error("G*T*M must be < 2^32"); return GSRQ_EINVAL; }
+  return GSRQ_OK;
+}
+
+static int check_ws(const void *ws, size_t bytes, const Plan &p) {
+  if (!ws || ((uintptr_t)ws & 255)) { set_error("workspace must be non-NULL and 256-byte aligned"); return GSRQ_EWORKSPACE; }
+  if (bytes < p.total) { set_error("workspace too small: %zu < %zu bytes", bytes, p.total); return GSRQ_EWORKSPACE; }
+  return GSRQ_OK;
+}
+
+static RowSrc make_src(const void *kv, const gsrq_view *v, const float *rows, long long rows_per_group) {
+  RowSrc s;
+  s.kv = kv; s.rows = rows; s.dtype = v->dtype; s.M = v->hd / v->d; s.d = v->d;
+  s.stride_g = v->stride_g; s.stride_t = v->stride_t; s.rows_per_group = rows_per_group;
+  return s;
+}
+
+#define DISPATCH_D(d, ...)                          \
+  do {                                              \
+    if ((d) == 8) { constexpr int D = 8; __VA_ARGS__; }   \
+    else if ((d) == 16) { constexpr int D = 16; __VA_ARGS__; } \
+    else { constexpr int D = 32; __VA_ARGS__; }     \
+  } while (0)
+
+// One filter + refine pass (assignment or multi-stage encode) described by `p`.
+static int run_encode(EncParams p, int G, int d, cudaStream_t stream) {
+  constexpr int RPT = 2;
+  const size_t smem = ((size_t)p.K * d + p.K + 4) * sizeof(float);
+  dim3 grid((unsigned)((p.N + 256 * RPT - 1) / (256 * RPT)), (unsigned)G);
+  DISPATCH_D(d, (k_encode<D, RPT><<<grid, 256, smem, stream>>>(p)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  DISPATCH_D(d, (k_encode_refine<D><<<296, 256, 0, stream>>>(p)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  return GSRQ_OK;
+}
+
+static int run_reduce_renorm(const Plan &pl, const gsrq_view *v, int K, char *ws, const uint8_t *idx, float *shapes_st,
+                             float *gains_st, long long cb_stride_g, DevStats *st, int lloyd, int t, cudaStream_t stream) {
+  const int d = v->d;
+  const float *Rf = (const float *)(ws + pl.off_Rf);
+  const double *rinv = (const double *)(ws + pl.off_rinv);
+  const float *wt = (const float *)(ws + pl.off_wt);
+  double *part = (double *)(ws + pl.off_part);
+  const double *etot = (const double *)(ws + pl.off_etot);
+  const size_t smem = (size_t)K * kBmWords * 4 + (size_t)(kReduceThreads / 32) * kChunkRows * 2;
+  dim3 grid((unsigned)pl.C, (unsigned)v->G);
+  DISPATCH_D(d, {
+    GSRQ_CUDA_CHECK(cudaFuncSetAttribute(k_reduce<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_reduce<D><<<grid, kReduceThreads, smem, stream>>>(Rf, rinv, wt, idx, pl.Nf, pl.M, K, part, st);
+  });
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  DISPATCH_D(d, (k_renorm<D><<<v->G, 256, 0, stream>>>(part, (int)pl.C, K, shapes_st, gains_st, cb_stride_g, etot, st, lloyd, t)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  return GSRQ_OK;
+}
+
+// Gather the fit rows (deriving the stage's residual when needed) and the per-row constants.
+static int prepare_rows(const Plan &pl, const void *kv, const gsrq_view *v, const float *w, long long w_stride_g,
+                        const long long *fit_tokens, const gsrq_codebook *cb, int stage, const float *residual, char *ws,
+                        cudaStream_t stream) {
+  const int d = v->d, G = v->G;
+  float *Rf = (float *)(ws + pl.off_Rf);
+  double *rinv = (double *)(ws + pl.off_rinv);
+  float *wt = (float *)(ws + pl.off_wt);
+  RowSrc src = make_src(kv, v, residual, pl.Nall);
+  dim3 grid((unsigned)((pl.Nf + 255) / 256), (unsigned)G);
+  DISPATCH_D(d, (k_gather<D><<<grid, 256, 0, stream>>>(src, w, w_stride_g, fit_tokens, pl.nf_tok, Rf, nullptr, wt)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  if (!residual && stage > 0) {  // r = x - sum_{s<stage} c^(s)[a^(s)], in place on the compact rows
+    EncParams p{};
+    p.src = make_src(nullptr, v, Rf, pl.Nf);
+    p.N = pl.Nf; p.shapes = cb->shapes; p.gains = cb->gains; p.S = cb->S; p.K = cb->K;
+    p.s_begin = 0; p.s_end = stage; p.s_base = 0; p.mode = 0; p.subtract = 1;
+    p.codes = nullptr; p.code_stride_s = 0; p.res_out = Rf; p.st = nullptr; p.slot = 0;
+    p.list = (uint32_t *)(ws + pl.off_list);
+    p.list_cnt = (unsigned int *)(ws + pl.off_cnt) + (kNumCounters - 1);
+    int rc = run_encode(p, G, d, stream);
+    if (rc) return rc;
+  }
+  const long long n_rows = (long long)G * pl.Nf;
+  DISPATCH_D(d, (k_rinv<D><<<(unsigned)((n_rows + 255) / 256), 256, 0, stream>>>(Rf, n_rows, rinv)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  DISPATCH_D(d, (k_energy<D><<<G, 1024, 0, stream>>>(Rf, wt, pl.Nf, pl.M, (double *)(ws + pl.off_etot))));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  return GSRQ_OK;
+}
+
+}  // namespace gsrq
+
+using namespace gsrq;
+
+extern "C" {
+
+const char *gsrq_last_error(void) { return g_err; }
+const char *gsrq_version(void) { return "gsrq-b200 0.1 (sm_100a)"; }
+
+size_t gsrq_workspace_bytes(const gsrq_view *view, int K, int S, int64_t n_fit_tokens) {
+  if (check_view(view, K, S) != GSRQ_OK) return 0;
+  if (n_fit_tokens < 0 || n_fit_tokens > view->T) return 0;
+  return make_plan(view, K, S, n_fit_tokens).total;
+}
+
+int gsrq_fit_stage(const void *kv, const gsrq_view *view, const float *w, int64_t w_stride_g, const int64_t *fit_tokens,
+                   int64_t n_fit, gsrq_codebook *cb, int stage, const float *residual, int iters, uint64_t seed,
+                   gsrq_fit_stats *stats, void *workspace, size_t workspace_bytes, void *stream_) {
+  cudaStream_t stream = (cudaStream_t)stream_;
+  if (!kv || !cb || !cb->shapes || !cb->gains) { set_error("NULL kv / codebook"); return GSRQ_EINVAL; }
+  int rc = check_view(view, cb->K, cb->S);
+  if (rc) return rc;
+  if (stage < 0 || stage >= cb->S) { set_error("stage %d out of [0, %d)", stage, cb->S); return GSRQ_EINVAL; }
+  if (iters < 0 || iters > GSRQ_MAX_ITERS) { set_error("iters must be in [0, %d]", GSRQ_MAX_ITERS); return GSRQ_EINVAL; }
+  if (fit_tokens && (n_fit <= 0 || n_fit > view->T)) { set_error("n_fit out of range"); return GSRQ_EINVAL; }
+  const Plan pl = make_plan(view, cb->K, cb->S, fit_tokens ? n_fit : 0);
+  if (pl.Nf < cb->K) { set_error("fewer fit rows (%lld) than codewords (%d)", pl.Nf, cb->K); return GSRQ_EDEGENERATE; }
+  rc = check_ws(workspace, workspace_bytes, pl);
+  if (rc) return rc;
+  char *ws = (char *)workspace;
+  const int G = view->G, d = view->d, K = cb->K;
+  DevStats *st = (DevStats *)(ws + pl.off_st);
+  unsigned int *cnt = (unsigned int *)(ws + pl.off_cnt);
+  uint8_t *idx = (uint8_t *)(ws + pl.off_idx);
+  long long *ids = (long long *)(ws + pl.off_ids);
+  float *Rf = (float *)(ws + pl.off_Rf);
+  GSRQ_CUDA_CHECK(cudaMemsetAsync(st, 0, (size_t)G * sizeof(DevStats), stream));
+  GSRQ_CUDA_CHECK(cudaMemsetAsync(cnt, 0, kNumCounters * sizeof(unsigned int), stream));
+  GSRQ_CUDA_CHECK(cudaMemsetAsync(idx, 0, (size_t)G * pl.Nf, stream));
+  rc = prepare_rows(pl, kv, view, w, w_stride_g, (const long long *)fit_tokens, cb, stage, residual, ws, stream);
+  if (rc) return rc;
+
+  float *shapes_st = cb->shapes + (size_t)stage * K * d;
+  float *gains_st = cb->gains + (size_t)stage * K;
+  const long long cb_stride_g = (long long)cb->S * K;
+  DISPATCH_D(d, (k_init_ids<D><<<G, 512, 0, stream>>>(Rf, pl.Nf, K, G, stage, seed, ids, st)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  DISPATCH_D(d, (k_init_shapes<D><<<G, 256, 0, stream>>>(Rf, pl.Nf, K, ids, shapes_st, gains_st, cb_stride_g)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+
+  EncParams p{};
+  p.src = make_src(nullptr, view, Rf, pl.Nf);
+  p.N = pl.Nf; p.shapes = cb->shapes; p.gains = cb->gains; p.S = cb->S; p.K = K;
+  p.subtract = 0;
+  p.codes = idx; p.code_stride_s = 0; p.res_out = nullptr; p.st = st;
+  p.list = (uint32_t *)(ws + pl.off_list);
+  // t = 0 is Alg. 1 l.2: gains by Eq. 8 under the max-projection assignment (reading c-I)
+  rc = 0;
+  for (int t = 0; t <= iters && rc == 0; ++t) {
+    EncParams a = p;
+    a.mode = (t == 0) ? 1 : 0;
+    a.slot = t;
+    a.list_cnt = cnt + t;
+    // score only stage `stage` on the prepared rows: present it to the kernel as a 1-stage pass
+    a.shapes = shapes_st; a.gains = gains_st;
+    a.s_begin = 0; a.s_end = 1; a.s_base = 0;
+    rc = run_encode(a, G, d, stream);
+    if (rc) break;
+    rc = run_reduce_renorm(pl, view, K, ws, idx, shapes_st, gains_st, cb_stride_g, st, t > 0, t, stream);
+  }
+  if (rc) return rc;
+  if (stats) {
+    DevStats *h = (DevStats *)malloc((size_t)G * sizeof(DevStats));
+    if (!h) { set_error("out of host memory"); return GSRQ_ECUDA; }
+    cudaError_t e = cudaMemcpyAsync(h, st, (size_t)G * sizeof(DevStats), cudaMemcpyDeviceToHost, stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+    if (e != cudaSuccess) { free(h); set_error("stats copy failed: %s", cudaGetErrorString(e)); return GSRQ_ECUDA; }
+    int degenerate = 0;
+    for (int g = 0; g < G; ++g) {
+      gsrq_fit_stats *o = stats + g;
+      memset(o, 0, sizeof(*o));
+      o->iters_run = h[g].iters_run;
+      o->n_empty_last = h[g].n_empty;
+      o->n_refined = h[g].refined;
+      for (int t = 1; t <= h[g].iters_run; ++t) {
+        o->wdist_after_assign[t - 1] = h[g].J[t];
+        o->n_changed[t - 1] = h[g].changed[t];
+      }
+      o->n_changed_last = h[g].iters_run ? h[g].changed[h[g].iters_run] : 0;
+      degenerate |= (h[g].err != 0);
+    }
+    free(h);
+    if (degenerate) { set_error("a group has fewer than K distinct non-zero fit rows"); return GSRQ_EDEGENERATE; }
+  }
+  return GSRQ_OK;
+}
+
+
+int gsrq_encode(const void *kv, const gsrq_view *view, const gsrq_codebook *cb, int stage_begin, int stage_end,
+                uint8_t *codes, float *residual_out, void *workspace, size_t workspace_bytes, void *stream_) {
+  cudaStream_t stream = (cudaStream_t)stream_;
+  if (!kv || !cb || !cb->shapes || !cb->gains || !codes) { set_error("NULL kv / codebook / codes"); return GSRQ_EINVAL; }
+  int rc = check_view(view, cb->K, cb->S);
+  if (rc) return rc;
+  if (stage_begin < 0 || stage_end > cb->S || stage_begin >= stage_end) { set_error("bad stage range [%d, %d)", stage_begin, stage_end); return GSRQ_EINVAL; }
+  const Plan pl = make_plan(view, cb->K, cb->S, 0);
+  rc = check_ws(workspace, workspace_bytes, pl);
+  if (rc) return rc;
+  char *ws = (char *)workspace;
+  unsigned int *cnt = (unsigned int *)(ws + pl.off_cnt);
+  GSRQ_CUDA_CHECK(cudaMemsetAsync(cnt, 0, sizeof(unsigned int), stream));
+  EncParams p{};
+  p.src = make_src(kv, view, nullptr, 0);
+  p.N = pl.Nall; p.shapes = cb->shapes; p.gains = cb->gains; p.S = cb->S; p.K = cb->K;
+  p.s_begin = stage_begin; p.s_end = stage_end; p.s_base = 0; p.mode = 0; p.subtract = 1;
+  p.codes = codes; p.code_stride_s = (long long)view->G * pl.Nall; p.res_out = residual_out;
+  p.st = nullptr; p.slot = 0; p.list = (uint32_t *)(ws + pl.off_list); p.list_cnt = cnt;
+  return run_encode(p, view->G, view->d, stream);
+}
+
+int gsrq_decode(const uint8_t *codes, const gsrq_codebook *cb, int n_stages, void *kv_out, const gsrq_view *out_view,
+                void *stream_) {
+  cudaStream_t stream = (cudaStream_t)stream_;
+  if (!codes || !cb || !cb->shapes || !cb->gains || !kv_out) { set_error("NULL codes / codebook / output"); return GSRQ_EINVAL; }
+  int rc = check_view(out_view, cb->K, cb->S);
+  if (rc) return rc;
+  if (n_stages < 0 || n_stages > cb->S) { set_error("n_stages %d out of [0, %d]", n_stages, cb->S); return GSRQ_EINVAL; }
+  const int d = out_view->d;
+  DecParams p{};
+  p.codes = codes; p.shapes = cb->shapes; p.gains = cb->gains; p.S = cb->S; p.K = cb->K; p.G = out_view->G;
+  p.n_stages = n_stages; p.M = out_view->hd / d; p.N = out_view->T * p.M; p.out = kv_out; p.dtype = out_view->dtype;
+  p.stride_g = out_view->stride_g; p.stride_t = out_view->stride_t;
+  const size_t smem = (size_t)n_stages * cb->K * d * sizeof(float);
+  const bool use_smem = smem <= 200 * 1024;
+  // enough CTAs to fill the machine a few times, but few enough that the table load amortises
+  long long rows_per_cta = 8192;
+  while (rows_per_cta > 1024 && (p.N + rows_per_cta - 1) / rows_per_cta * out_view->G < 4 * 148) rows_per_cta /= 2;
+  p.rows_per_cta = rows_per_cta;
+  dim3 grid((unsigned)((p.N + rows_per_cta - 1) / rows_per_cta), (unsigned)out_view->G);
+  if (use_smem) {
+    DISPATCH_D(d, {
+      GSRQ_CUDA_CHECK(cudaFuncSetAttribute(k_decode<D, true, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(200 * 1024)));
+      k_decode<D, true, 4><<<grid, 256, smem, stream>>>(p);
+    });
+  } else {
+    DISPATCH_D(d, (k_decode<D, false, 4><<<grid, 256, 0, stream>>>(p)));
+  }
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  return GSRQ_OK;
+}
+
+int gsrq_assign(const void *kv, const gsrq_view *view, const float *residual, const gsrq_codebook *cb, int stage, int mode,
+                uint8_t *idx_out, void *workspace, size_t workspace_bytes, void *stream_) {
+  cudaStream_t stream = (cudaStream_t)stream_;
+  if ((!kv && !residual) || !cb || !cb->shapes || !cb->gains || !idx_out) { set_error("NULL input"); return GSRQ_EINVAL; }
+  int rc = check_view(view, cb->K, cb->S);
+  if (rc) return rc;
+  if (stage < 0 || stage >= cb->S || (mode != 0 && mode != 1)) { set_error("bad stage / mode"); return GSRQ_EINVAL; }
+  const Plan pl = make_plan(view, cb->K, cb->S, 0);
+  rc = check_ws(workspace, workspace_bytes, pl);
+  if (rc) return rc;
+  char *ws = (char *)workspace;
+  unsigned int *cnt = (unsigned int *)(ws + pl.off_cnt);
+  GSRQ_CUDA_CHECK(cudaMemsetAsync(cnt, 0, sizeof(unsigned int), stream));
+  EncParams p{};
+  p.src = make_src(kv, view, residual, pl.Nall);
+  p.N = pl.Nall; p.S = cb->S; p.K = cb->K;
+  p.shapes = cb->shapes + (size_t)stage * cb->K * view->d;
+  p.gains = cb->gains + (size_t)stage * cb->K;
+  p.s_begin = 0; p.s_end = 1; p.s_base = 0; p.mode = mode; p.subtract = 0;
+  p.codes = idx_out; p.code_stride_s = 0; p.res_out = nullptr; p.st = nullptr; p.slot = 0;
+  p.list = (uint32_t *)(ws + pl.off_list); p.list_cnt = cnt;
+  return run_encode(p, view->G, view->d, stream);
+}
+
+int gsrq_update(const void *kv, const gsrq_view *view, const float *residual, const float *w, int64_t w_stride_g,
+                const uint8_t *idx, gsrq_codebook *cb, int stage, int shapes_too, void *workspace, size_t workspace_bytes,
+                void *stream_) {
+  cudaStream_t stream = (cudaStream_t)stream_;
+  if ((!kv && !residual) || !cb || !cb->shapes || !cb->gains || !idx) { set_error("NULL input"); return GSRQ_EINVAL; }
+  int rc = check_view(view, cb->K, cb->S);
+  if (rc) return rc;
+  if (stage < 0 || stage >= cb->S) { set_error("bad stage"); return GSRQ_EINVAL; }
+  const Plan pl = make_plan(view, cb->K, cb->S, 0);
+  rc = check_ws(workspace, workspace_bytes, pl);
+  if (rc) return rc;
+  char *ws = (char *)workspace;
+  DevStats *st = (DevStats *)(ws + pl.off_st);
+  GSRQ_CUDA_CHECK(cudaMemsetAsync(st, 0, (size_t)view->G * sizeof(DevStats), stream));
+  // rows = residual when given, else kv as is (the caller states which stage's rows these are)
+  rc = prepare_rows(pl, kv, view, w, w_stride_g, nullptr, cb, 0, residual, ws, stream);
+  if (rc) return rc;
+  return run_reduce_renorm(pl, view, cb->K, ws, idx, cb->shapes + (size_t)stage * cb->K * view->d,
+                           cb->gains + (size_t)stage * cb->K, (long long)cb->S * cb->K, st, shapes_too ? 1 : 0, 1, stream);
+}
+
+int gsrq_init_ids(const void *kv, const gsrq_view *view, const float *residual, const int64_t *fit_tokens, int64_t n_fit,
+                  int K, int stage, uint64_t seed, int64_t *ids_out, void *workspace, size_t workspace_bytes, void *stream_) {
+  cudaStream_t stream = (cudaStream_t)stream_;
+  if ((!kv && !residual) || !ids_out) { set_error("NULL input"); return GSRQ_EINVAL; }
+  int rc = check_view(view, K, 1);
+  if (rc) return rc;
+  if (fit_tokens && (n_fit <= 0 || n_fit > view->T)) { set_error("n_fit out of range"); return GSRQ_EINVAL; }
+  const Plan pl = make_plan(view, K, 1, fit_tokens ? n_fit : 0);
+  if (pl.Nf < K) { set_error("fewer fit rows than codewords"); return GSRQ_EDEGENERATE; }
+  rc = check_ws(workspace, workspace_bytes, pl);
+  if (rc) return rc;
+  char *ws = (char *)workspace;
+  DevStats *st = (DevStats *)(ws + pl.off_st);
+  GSRQ_CUDA_CHECK(cudaMemsetAsync(st, 0, (size_t)view->G * sizeof(DevStats), stream));
+  rc = prepare_rows(pl, kv, view, nullptr, 0, (const long long *)fit_tokens, nullptr, 0, residual, ws, stream);
+  if (rc) return rc;
+  const int d = view->d;
+  DISPATCH_D(d, (k_init_ids<D><<<view->G, 512, 0, stream>>>((const float *)(ws + pl.off_Rf), pl.Nf, K, view->G, stage, seed,
+                                                              (long long *)ids_out, st)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  return GSRQ_OK;
+}
+
+int gsrq_encode_host(const void *kv_host, const gsrq_view *view, const gsrq_codebook *cb, uint8_t *codes_host) {
+  if (!kv_host || !cb || !codes_host) { set_error("NULL input"); return GSRQ_EINVAL; }
+  int rc = check_view(view, cb->K, cb->S);
+  if (rc) return rc;
+  // host buffer must be one dense block covering the view
+  const size_t esz = view->dtype == GSRQ_BF16 ? 2 : 4;
+  const size_t n_el = (size_t)view->G * view->T * view->hd;
+  const size_t n_codes = (size_t)cb->S * view->G * view->T * (view->hd / view->d);
+  const size_t wsb = gsrq_workspace_bytes(view, cb->K, cb->S, 0);
+  void *d_kv = nullptr, *d_codes = nullptr, *d_ws = nullptr;
+  cudaStream_t stream = nullptr;
+  cudaError_t e = cudaMalloc(&d_kv, n_el * esz);
+  if (e == cudaSuccess) e = cudaMalloc(&d_codes, n_codes);
+  if (e == cudaSuccess) e = cudaMalloc(&d_ws, wsb);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(d_kv, kv_host, n_el * esz, cudaMemcpyHostToDevice, stream);
+  if (e == cudaSuccess) {
+    rc = gsrq_encode(d_kv, view, cb, 0, cb->S, (uint8_t *)d_codes, nullptr, d_ws, wsb, stream);
+    if (rc == GSRQ_OK) e = cudaMemcpyAsync(codes_host, d_codes, n_codes, cudaMemcpyDeviceToHost, stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+  }
+  cudaFree(d_kv); cudaFree(d_codes); cudaFree(d_ws);
+  if (e != cudaSuccess) { set_error("gsrq_encode_host: %s", cudaGetErrorString(e)); return GSRQ_ECUDA; }
+  return rc;
+}
+
+int gsrq_decode_host(const uint8_t *codes_host, const gsrq_codebook *cb, int n_stages, void *kv_out_host,
+                     const gsrq_view *out_view) {
+  if (!codes_host || !cb || !kv_out_host) { set_error("NULL input"); return GSRQ_EINVAL; }
+  int rc = check_view(out_view, cb->K, cb->S);
+  if (rc) return rc;
+  const size_t esz = out_view->dtype == GSRQ_BF16 ? 2 : 4;
+  const size_t n_el = (size_t)out_view->G * out_view->T * out_view->hd;
+  const size_t n_codes = (size_t)cb->S * out_view->G * out_view->T * (out_view->hd / out_view->d);
+  void *d_kv = nullptr, *d_codes = nullptr;
+  cudaStream_t stream = nullptr;
+  cudaError_t e = cudaMalloc(&d_kv, n_el * esz);
+  if (e == cudaSuccess) e = cudaMalloc(&d_codes, n_codes);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(d_codes, codes_host, n_codes, cudaMemcpyHostToDevice, stream);
+  if (e == cudaSuccess) {
+    rc = gsrq_decode((const uint8_t *)d_codes, cb, n_stages, d_kv, out_view, stream);
+    if (rc == GSRQ_OK) e = cudaMemcpyAsync(kv_out_host, d_kv, n_el * esz, cudaMemcpyDeviceToHost, stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+  }
+  cudaFree(d_kv); cudaFree(d_codes);
+  if (e != cudaSuccess) { set_error("gsrq_decode_host: %s", cudaGetErrorString(e)); return GSRQ_ECUDA; }
+  return rc;
+}
+
+}  // extern "C"

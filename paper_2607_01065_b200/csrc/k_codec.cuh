@@ -1,0 +1,101 @@
+// k_codec.cuh -- decode: xhat_i = ((c0[a0_i] + c1[a1_i]) + ...) in fp32, stage order, one
+// RN-even cast to the output dtype (prefix of stages PAPER.md:25; reading c-D).
+// HBM-bound: reads S bytes and writes 2d (bf16) bytes per sub-vector.  The scaled codeword
+// tables c^(s)[K][D] = fl32(g_k s_k) live in shared memory; D/4 lanes cooperate on a row so
+// that every store instruction of a warp covers one contiguous 256-byte span (bf16).
+#pragma once
+#include "gsrq_common.cuh"
+
+namespace gsrq {
+
+struct DecParams {
+  const uint8_t *codes;  // [S][G][N]
+  const float *shapes;   // [G][S][K][D]
+  const float *gains;    // [G][S][K]
+  int S, K, G;
+  int n_stages;
+  long long N;           // rows per group = T*M
+  int M;
+  void *out;
+  int dtype;
+  long long stride_g, stride_t;
+  long long rows_per_cta;
+};
+
+__device__ __forceinline__ uint32_t pack_bf16x2(float a, float b) {
+  const __nv_bfloat16 lo = __float2bfloat16_rn(a), hi = __float2bfloat16_rn(b);
+  return (uint32_t)__bfloat16_as_ushort(lo) | ((uint32_t)__bfloat16_as_ushort(hi) << 16);
+}
+
+// grid = (ceil(N / rows_per_cta), G), block = 256, dynamic smem = n_stages*K*D*4 (SMEM) or 0.
+template <int D, bool SMEM, int U>
+__global__ void __launch_bounds__(256) k_decode(DecParams p) {
+  extern __shared__ __align__(16) float tab[];
+  constexpr int LPR = D / 4;      // lanes per row
+  constexpr int RPI = 256 / LPR;  // rows per CTA iteration
+  const int g = blockIdx.y;
+  if (SMEM) {
+    for (int e = threadIdx.x; e < p.n_stages * p.K * D; e += 256) {
+      const int s = e / (p.K * D), r = e - s * p.K * D;
+      const long long cb = ((long long)g * p.S + s) * p.K;
+      tab[e] = __fmul_rn(p.gains[cb + r / D], p.shapes[cb * D + r]);
+    }
+    __syncthreads();
+  }
+  const int sub = threadIdx.x % LPR, rl = threadIdx.x / LPR;
+  const long long r0 = (long long)blockIdx.x * p.rows_per_cta;
+  const long long r1 = min(p.N, r0 + p.rows_per_cta);
+  for (long long ib = r0 + rl; ib < r1; ib += (long long)RPI * U) {
+    int code[U][GSRQ_MAX_STAGES > 8 ? 8 : GSRQ_MAX_STAGES];
+    float4 acc[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) acc[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int s0 = 0; s0 < p.n_stages; s0 += 8) {
+      const int ns = min(8, p.n_stages - s0);
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const long long i = ib + (long long)u * RPI;
+#pragma unroll
+        for (int s = 0; s < 8; ++s)
+          code[u][s] = (s < ns && i < r1) ? p.codes[((long long)(s0 + s) * p.G + g) * p.N + i] : 0;
+      }
+#pragma unroll
+      for (int s = 0; s < 8; ++s) {
+        if (s >= ns) break;
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+          float4 c;
+          if (SMEM) {
+            c = *reinterpret_cast<const float4 *>(tab + ((s0 + s) * p.K + code[u][s]) * D + sub * 4);
+          } else {
+            const long long cb = ((long long)g * p.S + s0 + s) * p.K + code[u][s];
+            const float gk = p.gains[cb];
+            const float4 sv = *reinterpret_cast<const float4 *>(p.shapes + cb * D + sub * 4);
+            c = make_float4(__fmul_rn(gk, sv.x), __fmul_rn(gk, sv.y), __fmul_rn(gk, sv.z), __fmul_rn(gk, sv.w));
+          }
+          if (s0 + s == 0) acc[u] = c;
+          else {
+            acc[u].x = __fadd_rn(acc[u].x, c.x); acc[u].y = __fadd_rn(acc[u].y, c.y);
+            acc[u].z = __fadd_rn(acc[u].z, c.z); acc[u].w = __fadd_rn(acc[u].w, c.w);
+          }
+        }
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const long long i = ib + (long long)u * RPI;
+      if (i >= r1) continue;
+      const long long tok = i / p.M;
+      const int m = (int)(i - tok * p.M);
+      const long long off = (long long)g * p.stride_g + tok * p.stride_t + (long long)m * D + sub * 4;
+      if (p.dtype == GSRQ_BF16) {
+        uint2 v = make_uint2(pack_bf16x2(acc[u].x, acc[u].y), pack_bf16x2(acc[u].z, acc[u].w));
+        *reinterpret_cast<uint2 *>(reinterpret_cast<uint16_t *>(p.out) + off) = v;
+      } else {
+        *reinterpret_cast<float4 *>(reinterpret_cast<float *>(p.out) + off) = acc[u];
+      }
+    }
+  }
+}
+
+}  // namespace gsrq

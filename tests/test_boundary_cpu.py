@@ -1,0 +1,69 @@
+"""CPU-side checks of the C-ABI boundary: the library loads, exports every symbol the header
+declares, sizes workspaces, and rejects bad arguments before touching CUDA."""
+import ctypes as C
+import re
+from pathlib import Path
+
+import pytest
+
+ROOT = Path(__file__).resolve().parent.parent
+
+
+@pytest.fixture(scope="module")
+def B():
+    import __graft_entry__ as ge
+    ge.build()
+    from paper_2607_01065_b200 import binding
+    return binding
+
+
+def test_every_declared_symbol_is_exported(B):
+    hdr = (ROOT / "include" / "gsrq.h").read_text()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    names = set(re.findall(r"\b(gsrq_[a-z_0-9]+)\s*\(", hdr))
+    assert {"gsrq_fit_stage", "gsrq_encode", "gsrq_decode", "gsrq_workspace_bytes"} <= names
+    lib = B.lib()
+    for n in names:
+        assert hasattr(lib, n), n
+    assert set(B.EXPORTS) == names
+    assert "sm_100a" in B.gsrq_version()
+
+
+def test_struct_layout_matches_header(B):
+    assert C.sizeof(B.gsrq_view) == 40
+    assert C.sizeof(B.gsrq_codebook) == 24
+    assert C.sizeof(B.gsrq_fit_stats) == 24 + 8 * 128 + 8 * 128
+
+
+def test_workspace_bytes_and_argument_errors(B):
+    v = B.gsrq_view(B.GSRQ_BF16, 8, 4096, 128, 16, 4096 * 128, 128)
+    n_all = B.gsrq_workspace_bytes(v, 256, 2, 0)
+    n_fit = B.gsrq_workspace_bytes(v, 256, 2, 512)
+    assert n_all > n_fit > 8 * 4096 * 8 * 4      # the flagged-row list alone
+    assert n_all % 256 == 0
+    for bad in [B.gsrq_view(B.GSRQ_BF16, 8, 4096, 128, 24, 4096 * 128, 128),    # hd % d
+                B.gsrq_view(7, 8, 4096, 128, 16, 4096 * 128, 128),              # dtype
+                B.gsrq_view(B.GSRQ_BF16, 8, 4096, 128, 16, 4096 * 128 + 1, 128)]:  # alignment
+        with pytest.raises(B.GsrqError) as e:
+            B.gsrq_workspace_bytes(bad, 256, 2, 0)
+        assert e.value.code == -1
+    with pytest.raises(B.GsrqError):
+        B.gsrq_workspace_bytes(v, 257, 2, 0)
+    lib = B.lib()
+    v64 = B.gsrq_view(B.GSRQ_BF16, 8, 4096, 128, 64, 4096 * 128, 128)
+    assert lib.gsrq_workspace_bytes(C.byref(v64), 256, 2, C.c_int64(0)) == 0
+    assert b"d = 64" in lib.gsrq_last_error()
+    # compute entry points validate before any CUDA call: NULL pointers -> GSRQ_EINVAL
+    cb = B.gsrq_codebook(256, 2, None, None)
+    rc = lib.gsrq_encode(None, C.byref(v), C.byref(cb), 0, 2, None, None, None, C.c_size_t(0), None)
+    assert rc == -1
+    rc = lib.gsrq_decode(None, C.byref(cb), 2, None, C.byref(v), None)
+    assert rc == -1
+
+
+def test_product_path_does_not_reach_the_oracle():
+    """The CUDA path and its binding must not import or link anything under oracle/."""
+    for p in (ROOT / "paper_2607_01065_b200").rglob("*"):
+        if p.suffix in {".py", ".cu", ".cuh", ".h"}:
+            txt = p.read_text()
+            assert not re.search(r"(import\s+oracle|from\s+oracle|#include[^\n]*oracle|gsrq_oracle|oracle/build)", txt), p
