@@ -1,0 +1,276 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line per run (see DESIGN.md section 7 for what each key means).
+
+A "step" is one pass of the whole hot path over one synthetic layer tensor of BASELINE.json
+config 1 (8 KV heads x 4096 tokens x 128, bf16, d=16, K=256, S=2, 20 iterations/stage):
+for each stage: gsrq_fit_stage -> gsrq_encode of that stage (residual carried); then gsrq_decode.
+value = KV vectors (token x head) through the whole step per second, summed over ranks.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--cfg 1|2]
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+import torch
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+from paper_2607_01065_b200 import inputs  # noqa: E402
+
+METRIC = "gsrq_fit_encode_decode_kv_vectors_per_s"
+UNIT = "KV vectors/s"
+
+
+def peaks():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        d = json.loads(p.read_text())
+        return dict(hbm_gbs=d["hbm_gbs"], bf16_tflops=d["bf16_tflops"], bf16_tflops_sustained=d["bf16_tflops_sustained"],
+                    source="MEASURED_PEAKS.json")
+    return dict(hbm_gbs=6650.0, bf16_tflops=1590.0, bf16_tflops_sustained=1400.0, source="fallback (B200_PROFILING.md)")
+
+
+class ClockSampler(threading.Thread):
+    """Samples nvidia-smi clocks / throttle reasons every 200 ms while the timed region runs."""
+
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.stop_flag, self.proc = index, [], False, None
+
+    def run(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "200"], stdout=subprocess.PIPE, text=True)
+            for line in self.proc.stdout:
+                self.samples.append([t.strip() for t in line.split(",")])
+                if self.stop_flag:
+                    break
+        except Exception:
+            pass
+
+    def finish(self):
+        self.stop_flag = True
+        if self.proc:
+            self.proc.terminate()
+        sm = [float(s[0]) for s in self.samples if s and s[0].replace(".", "").isdigit()]
+        mx = [float(s[1]) for s in self.samples if len(s) > 1 and s[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[i] for s in self.samples if len(s) >= 6 for i in range(4) if s[2 + i].lower().startswith("active")})
+        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None, reasons=reasons,
+                    samples=len(sm))
+
+
+def oracle_step(x, w, c):
+    """The CPU oracle doing the same step (fit + encode every stage, then decode)."""
+    from oracle import gsrq_oracle as o
+    out = o.gsrq_fit_encode(x, w, c.d, c.K, c.S, c.iters, seed=0)
+    o.decode(out["codes"], out["shapes"], out["gains"], c.hd, bf16=(c.dtype == "bf16"))
+    return out
+
+
+def run_reference(args, c):
+    """--impl reference: the oracle as it stands on the host cores, same config / metric."""
+    from oracle import gsrq_oracle as o
+    o.build()
+    dd = inputs.make(c.cfg)
+    x, w = dd["x"], dd["w"]
+    for _ in range(min(args.warmup, 1)):
+        oracle_step(x[:1], w, c)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_step(x, w, c)
+    dt = (time.perf_counter() - t0) / args.steps
+    val = c.G * c.T / dt
+    line = dict(metric=METRIC, value=val, unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
+                ms_per_step=dt * 1e3, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64",
+                data="synthetic", impl="reference",
+                config=dict(workload=f"cfg{c.cfg}:{c.name}", G=c.G, T=c.T, hd=c.hd, d=c.d, K=c.K, S=c.S, iters=c.iters),
+                cpu_baseline=dict(value=val, unit=UNIT, cores=o.n_threads(), kind="oracle",
+                                  sample=f"whole cfg{c.cfg} step (all {c.G} heads), {args.steps} step(s)"),
+                e2e=dict(value=val, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--cfg", type=int, default=1, choices=[1, 2])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    c = inputs.CONFIGS[args.cfg]
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+
+    if args.impl == "reference":
+        if rank == 0:
+            run_reference(args, c)
+        return
+
+    import __graft_entry__ as ge
+    from paper_2607_01065_b200 import binding as B
+    if rank == 0:
+        ge.build()
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        dist.barrier()
+    torch.cuda.set_device(local)
+    B.lib()
+
+    # ---- inputs (replicas: rank r works on its own layer; rank 0 is the documented seeds) ----
+    kind = c.kinds[0]
+    gen = inputs.k_like if kind == "k" else inputs.v_like
+    x_np = gen(c.G, c.T, c.hd, inputs.seed_of(c.cfg, kind) + 100 * rank)
+    w_np = inputs.token_weights(c.T, inputs.seed_of(c.cfg, "w") + 100 * rank)
+    x_host = torch.from_numpy(x_np).to(torch.bfloat16).pin_memory()
+    w_host = torch.from_numpy(w_np).pin_memory()
+    x = x_host.cuda()
+    w = w_host.cuda()
+    view = B.view_of(x, c.d)
+    G, T, hd, d, K, S = c.G, c.T, c.hd, c.d, c.K, c.S
+    M = hd // d
+    shapes = torch.zeros(G, S, K, d, device="cuda")
+    gains = torch.zeros(G, S, K, device="cuda")
+    cb = B.codebook_of(shapes, gains)
+    ws = B.workspace(view, K, S, 0)
+    codes = torch.zeros(S, G, T * M, dtype=torch.uint8, device="cuda")
+    residual = torch.zeros(G, T * M, d, device="cuda")
+    out = torch.zeros_like(x)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+
+    def step():
+        for s in range(S):
+            B.gsrq_fit_stage(x, view, w, 0, None, cb, s, residual if s else None, c.iters, 0, ws, want_stats=False)
+            B.gsrq_encode(x, view, cb, s, s + 1, codes, residual, ws)
+        B.gsrq_decode(codes, cb, S, out, view)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    l0 = B.gsrq_launch_count()
+    evs = []
+    for _ in range(args.steps):
+        flush.fill_(1)                      # evict the previous step's data from L2 (not timed)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); step(); b.record()
+        evs.append((a, b))
+    barrier()
+    launches = B.gsrq_launch_count() - l0
+    ms = sum(a.elapsed_time(b) for a, b in evs)
+    tt = torch.tensor([ms], device="cuda", dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    ms = float(tt.item())
+    ms_per_step = ms / args.steps
+    value = world * G * T / (ms_per_step * 1e-3)
+
+    # ---- per-kernel device time, measured live with CUDA events around every launch ----
+    B.gsrq_profile_enable(True)
+    for _ in range(2):
+        step()
+    torch.cuda.synchronize()
+    prof = B.gsrq_profile_read()
+    B.gsrq_profile_enable(False)
+    # decode alone (cold L2) for the decode GB/s figure
+    dts = []
+    for _ in range(5):
+        flush.fill_(1)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); B.gsrq_decode(codes, cb, S, out, view); b.record()
+        torch.cuda.synchronize()
+        dts.append(a.elapsed_time(b))
+    dec_ms = float(np.median(dts))
+    dec_bytes = G * T * M * S + G * T * hd * 2
+    ets = []
+    for _ in range(5):
+        flush.fill_(1)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); B.gsrq_encode(x, view, cb, 0, S, codes, None, ws); b.record()
+        torch.cuda.synchronize()
+        ets.append(a.elapsed_time(b))
+    enc_ms = float(np.median(ets))
+
+    # ---- end to end through the host-buffer C-ABI call: H2D + fit + encode + decode + D2H ----
+    sh_h = torch.empty(G, S, K, d).pin_memory(); ga_h = torch.empty(G, S, K).pin_memory()
+    co_h = torch.empty(S, G, T * M, dtype=torch.uint8).pin_memory(); out_h = torch.empty_like(x_host).pin_memory()
+    for _ in range(2):
+        B.gsrq_pipeline_host(x_host, view, w_host, K, S, c.iters, 0, sh_h, ga_h, co_h, out_h)
+    barrier()
+    t0 = time.perf_counter()
+    n_e2e = max(3, args.steps // 2)
+    for _ in range(n_e2e):
+        B.gsrq_pipeline_host(x_host, view, w_host, K, S, c.iters, 0, sh_h, ga_h, co_h, out_h)
+    barrier()
+    e2e_s = (time.perf_counter() - t0) / n_e2e
+    te = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_val = world * G * T / float(te.item())
+    h2d = x_host.numel() * 2 + w_host.numel() * 4
+    d2h = sh_h.numel() * 4 + ga_h.numel() * 4 + co_h.numel() + out_h.numel() * 2
+    clocks = sampler.finish()
+
+    if rank != 0:
+        return
+    pk = peaks()
+    # dominant kernel = the scoring filter; algorithmic work = 2*K*d flops per sub-vector per scoring pass
+    sc_ms, sc_n = prof["score"]
+    rows_per_launch = G * T * M
+    flops_per_launch = 2.0 * K * d * rows_per_launch
+    achieved_tf = flops_per_launch / (sc_ms / max(sc_n, 1) * 1e-3) / 1e12
+    tot_ms = sum(v[0] for v in prof.values())
+    roofline = dict(bound="tensor", kernel="k_encode (scoring filter + arg-max)", achieved=achieved_tf,
+                    peak=pk["bf16_tflops_sustained"], unit="TFLOP/s", frac=achieved_tf / pk["bf16_tflops_sustained"],
+                    traffic=None, peak_source=pk["source"] + " (sustained bf16: kernel timed inside a long step)",
+                    ms_per_launch=sc_ms / max(sc_n, 1), launches=sc_n, share_of_step=sc_ms / tot_ms if tot_ms else None,
+                    by_class={k: dict(ms=v[0] / 2, launches=v[1] // 2) for k, v in prof.items()})
+    line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
+                ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="bf16 in, fp32/fp64 arithmetic",
+                data="synthetic", impl="ours",
+                config=dict(workload=f"cfg{c.cfg}:{c.name}", G=G, T=T, hd=hd, d=d, K=K, S=S, iters=c.iters,
+                            l2="flushed between steps (256 MiB write, untimed)", parallelism="replicas"),
+                clocks=clocks, gpu_launches=int(launches),
+                e2e=dict(value=e2e_val, unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h,
+                         call="gsrq_pipeline_host"),
+                roofline=roofline,
+                encode=dict(kv_vectors_per_s=G * T / (enc_ms * 1e-3), ms=enc_ms, stages=S,
+                            tensor_frac=(2.0 * K * d * rows_per_launch * S / (enc_ms * 1e-3) / 1e12) / pk["bf16_tflops"]),
+                decode=dict(gb_per_s=dec_bytes / (dec_ms * 1e-3) / 1e9, ms=dec_ms, bytes=dec_bytes,
+                            hbm_frac=dec_bytes / (dec_ms * 1e-3) / 1e9 / pk["hbm_gbs"]))
+    if not args.no_cpu_baseline:
+        from oracle import gsrq_oracle as o
+        t0 = time.perf_counter()
+        oracle_step(x_np, w_np, c)
+        dt = time.perf_counter() - t0
+        line["cpu_baseline"] = dict(value=G * T / dt, unit=UNIT, cores=o.n_threads(), kind="oracle",
+                                    sample=f"whole cfg{c.cfg} step once ({dt:.1f} s)")
+    print(json.dumps(line))
+
+
+if __name__ == "__main__":
+    main()

@@ -168,6 +168,28 @@ int gsrq_encode_host(const void *kv_host, const gsrq_view *view, const gsrq_code
 int gsrq_decode_host(const uint8_t *codes_host, const gsrq_codebook *cb, int n_stages,
                      void *kv_out_host, const gsrq_view *out_view);
 
+/* The whole hot path on HOST buffers, as one call (the end-to-end measurement): copies kv_host
+ * (dense, laid out as `view` says) and w_host ([T] or NULL) to the device, then for each stage
+ * s < S: gsrq_fit_stage (all tokens, `iters`, `seed`) + gsrq_encode of that stage; then, when
+ * kv_out_host != NULL, gsrq_decode of all S stages; copies shapes [G][S][K][d], gains [G][S][K],
+ * codes [S][G][T*M] (and the decoded tensor) back to the host and synchronises.  Device scratch
+ * is taken from the stream-ordered allocator for the duration of the call. */
+int gsrq_pipeline_host(const void *kv_host, const gsrq_view *view, const float *w_host, int K, int S,
+                       int iters, uint64_t seed, float *shapes_host, float *gains_host,
+                       uint8_t *codes_host, void *kv_out_host);
+
+/* ---- measurement hooks (host functions) ---- */
+
+#define GSRQ_N_KERNEL_CLASSES 6 /* 0 prep, 1 score (filter), 2 refine, 3 reduce, 4 renorm, 5 decode */
+
+/* When on, every kernel launch of this library is bracketed by a CUDA event pair on its stream. */
+void gsrq_profile_enable(int on);
+/* Synchronise the recorded events; per kernel class return summed device ms and launch counts
+ * since the last read (arrays of GSRQ_N_KERNEL_CLASSES, either may be NULL); clears the record. */
+int gsrq_profile_read(double *ms_by_class, int64_t *launches_by_class);
+/* Kernels launched by this library in this process so far. */
+int64_t gsrq_launch_count(void);
+
 /* Thread-local message of the last error returned on this thread ("" if none). */
 const char *gsrq_last_error(void);
 

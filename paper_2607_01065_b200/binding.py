@@ -42,7 +42,8 @@ class gsrq_fit_stats(C.Structure):
 
 _lib = None
 EXPORTS = ["gsrq_workspace_bytes", "gsrq_fit_stage", "gsrq_encode", "gsrq_decode", "gsrq_assign", "gsrq_update",
-           "gsrq_init_ids", "gsrq_encode_host", "gsrq_decode_host", "gsrq_last_error", "gsrq_version"]
+           "gsrq_init_ids", "gsrq_encode_host", "gsrq_decode_host", "gsrq_pipeline_host", "gsrq_profile_enable",
+           "gsrq_profile_read", "gsrq_launch_count", "gsrq_last_error", "gsrq_version"]
 
 
 def lib_path() -> Path:
@@ -60,6 +61,7 @@ def lib():
         _lib.gsrq_workspace_bytes.restype = C.c_size_t
         _lib.gsrq_last_error.restype = C.c_char_p
         _lib.gsrq_version.restype = C.c_char_p
+        _lib.gsrq_launch_count.restype = C.c_int64
     return _lib
 
 
@@ -155,3 +157,30 @@ def gsrq_encode_host(kv_host: torch.Tensor, view, cb, codes_host: torch.Tensor):
 def gsrq_decode_host(codes_host: torch.Tensor, cb, n_stages, kv_out_host: torch.Tensor, out_view):
     assert not kv_out_host.is_cuda and not codes_host.is_cuda
     _check(lib().gsrq_decode_host(_ptr(codes_host), C.byref(cb), n_stages, _ptr(kv_out_host), C.byref(out_view)))
+
+
+def gsrq_pipeline_host(kv_host, view, w_host, K, S, iters, seed, shapes_host, gains_host, codes_host, kv_out_host):
+    """All arguments are HOST tensors; H2D, fit + encode (+ decode), D2H and the sync happen inside."""
+    for t in (kv_host, w_host, shapes_host, gains_host, codes_host, kv_out_host):
+        assert t is None or not t.is_cuda
+    _check(lib().gsrq_pipeline_host(_ptr(kv_host), C.byref(view), _ptr(w_host), K, S, iters, C.c_uint64(seed),
+                                    _ptr(shapes_host), _ptr(gains_host), _ptr(codes_host), _ptr(kv_out_host)))
+
+
+KERNEL_CLASSES = ["prep", "score", "refine", "reduce", "renorm", "decode"]
+
+
+def gsrq_profile_enable(on: bool):
+    lib().gsrq_profile_enable(int(on))
+
+
+def gsrq_profile_read():
+    """Per kernel class: (summed device ms, launches) since the last read."""
+    ms = (C.c_double * 6)()
+    n = (C.c_int64 * 6)()
+    _check(lib().gsrq_profile_read(ms, n))
+    return {k: (ms[i], n[i]) for i, k in enumerate(KERNEL_CLASSES)}
+
+
+def gsrq_launch_count() -> int:
+    return int(lib().gsrq_launch_count())

@@ -3,6 +3,9 @@
 #include <stdarg.h>
 #include <string.h>
 
+#include <mutex>
+#include <vector>
+
 #include "gsrq_common.cuh"
 #include "k_codec.cuh"
 #include "k_prep.cuh"
@@ -20,6 +23,34 @@ void set_error(const char *fmt, ...) {
   vsnprintf(g_err, sizeof(g_err), fmt, ap);
   va_end(ap);
 }
+
+
+// ---- launch accounting / optional per-kernel CUDA-event timing (gsrq_profile_*) ----
+enum { kClsPrep = 0, kClsScore = 1, kClsRefine = 2, kClsReduce = 3, kClsRenorm = 4, kClsDecode = 5, kNumCls = 6 };
+struct ProfRec { int cls; cudaEvent_t a, b; };
+static std::mutex g_prof_mu;
+static std::vector<ProfRec> g_prof_recs;
+static bool g_prof_on = false;
+static long long g_launches[kNumCls] = {0, 0, 0, 0, 0, 0};
+
+struct ProfScope {
+  cudaStream_t stream;
+  cudaEvent_t b = nullptr;
+  ProfScope(int cls, cudaStream_t s) : stream(s) {
+    std::lock_guard<std::mutex> lk(g_prof_mu);
+    g_launches[cls]++;
+    if (g_prof_on) {
+      ProfRec r{cls, nullptr, nullptr};
+      if (cudaEventCreate(&r.a) == cudaSuccess && cudaEventCreate(&r.b) == cudaSuccess) {
+        cudaEventRecord(r.a, stream);
+        b = r.b;
+        g_prof_recs.push_back(r);
+      }
+    }
+  }
+  ~ProfScope() { if (b) cudaEventRecord(b, stream); }
+};
+#define LAUNCH(cls, stream, ...) do { gsrq::ProfScope _ps(cls, stream); __VA_ARGS__; } while (0)
 
 static inline size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
@@ -92,9 +123,9 @@ static int run_encode(EncParams p, int G, int d, cudaStream_t stream) {
   constexpr int RPT = 2;
   const size_t smem = ((size_t)p.K * d + p.K + 4) * sizeof(float);
   dim3 grid((unsigned)((p.N + 256 * RPT - 1) / (256 * RPT)), (unsigned)G);
-  DISPATCH_D(d, (k_encode<D, RPT><<<grid, 256, smem, stream>>>(p)));
+  LAUNCH(kClsScore, stream, DISPATCH_D(d, (k_encode<D, RPT><<<grid, 256, smem, stream>>>(p))));
   GSRQ_CUDA_CHECK(cudaGetLastError());
-  DISPATCH_D(d, (k_encode_refine<D><<<296, 256, 0, stream>>>(p)));
+  LAUNCH(kClsRefine, stream, DISPATCH_D(d, (k_encode_refine<D><<<296, 256, 0, stream>>>(p))));
   GSRQ_CUDA_CHECK(cudaGetLastError());
   return GSRQ_OK;
 }
@@ -111,10 +142,10 @@ static int run_reduce_renorm(const Plan &pl, const gsrq_view *v, int K, char *ws
   dim3 grid((unsigned)pl.C, (unsigned)v->G);
   DISPATCH_D(d, {
     GSRQ_CUDA_CHECK(cudaFuncSetAttribute(k_reduce<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_reduce<D><<<grid, kReduceThreads, smem, stream>>>(Rf, rinv, wt, idx, pl.Nf, pl.M, K, part, st);
+    LAUNCH(kClsReduce, stream, (k_reduce<D><<<grid, kReduceThreads, smem, stream>>>(Rf, rinv, wt, idx, pl.Nf, pl.M, K, part, st)));
   });
   GSRQ_CUDA_CHECK(cudaGetLastError());
-  DISPATCH_D(d, (k_renorm<D><<<v->G, 256, 0, stream>>>(part, (int)pl.C, K, shapes_st, gains_st, cb_stride_g, etot, st, lloyd, t)));
+  LAUNCH(kClsRenorm, stream, DISPATCH_D(d, (k_renorm<D><<<v->G, 256, 0, stream>>>(part, (int)pl.C, K, shapes_st, gains_st, cb_stride_g, etot, st, lloyd, t))));
   GSRQ_CUDA_CHECK(cudaGetLastError());
   return GSRQ_OK;
 }
@@ -129,7 +160,7 @@ static int prepare_rows(const Plan &pl, const void *kv, const gsrq_view *v, cons
   float *wt = (float *)(ws + pl.off_wt);
   RowSrc src = make_src(kv, v, residual, pl.Nall);
   dim3 grid((unsigned)((pl.Nf + 255) / 256), (unsigned)G);
-  DISPATCH_D(d, (k_gather<D><<<grid, 256, 0, stream>>>(src, w, w_stride_g, fit_tokens, pl.nf_tok, Rf, nullptr, wt)));
+  LAUNCH(kClsPrep, stream, DISPATCH_D(d, (k_gather<D><<<grid, 256, 0, stream>>>(src, w, w_stride_g, fit_tokens, pl.nf_tok, Rf, nullptr, wt))));
   GSRQ_CUDA_CHECK(cudaGetLastError());
   if (!residual && stage > 0) {  // r = x - sum_{s<stage} c^(s)[a^(s)], in place on the compact rows
     EncParams p{};
@@ -143,9 +174,9 @@ static int prepare_rows(const Plan &pl, const void *kv, const gsrq_view *v, cons
     if (rc) return rc;
   }
   const long long n_rows = (long long)G * pl.Nf;
-  DISPATCH_D(d, (k_rinv<D><<<(unsigned)((n_rows + 255) / 256), 256, 0, stream>>>(Rf, n_rows, rinv)));
+  LAUNCH(kClsPrep, stream, DISPATCH_D(d, (k_rinv<D><<<(unsigned)((n_rows + 255) / 256), 256, 0, stream>>>(Rf, n_rows, rinv))));
   GSRQ_CUDA_CHECK(cudaGetLastError());
-  DISPATCH_D(d, (k_energy<D><<<G, 1024, 0, stream>>>(Rf, wt, pl.Nf, pl.M, (double *)(ws + pl.off_etot))));
+  LAUNCH(kClsPrep, stream, DISPATCH_D(d, (k_energy<D><<<G, 1024, 0, stream>>>(Rf, wt, pl.Nf, pl.M, (double *)(ws + pl.off_etot)))));
   GSRQ_CUDA_CHECK(cudaGetLastError());
   return GSRQ_OK;
 }
@@ -195,9 +226,9 @@ int gsrq_fit_stage(const void *kv, const gsrq_view *view, const float *w, int64_
   float *shapes_st = cb->shapes + (size_t)stage * K * d;
   float *gains_st = cb->gains + (size_t)stage * K;
   const long long cb_stride_g = (long long)cb->S * K;
-  DISPATCH_D(d, (k_init_ids<D><<<G, 512, 0, stream>>>(Rf, pl.Nf, K, G, stage, seed, ids, st)));
+  LAUNCH(kClsPrep, stream, DISPATCH_D(d, (k_init_ids<D><<<G, 512, 0, stream>>>(Rf, pl.Nf, K, G, stage, seed, ids, st))));
   GSRQ_CUDA_CHECK(cudaGetLastError());
-  DISPATCH_D(d, (k_init_shapes<D><<<G, 256, 0, stream>>>(Rf, pl.Nf, K, ids, shapes_st, gains_st, cb_stride_g)));
+  LAUNCH(kClsPrep, stream, DISPATCH_D(d, (k_init_shapes<D><<<G, 256, 0, stream>>>(Rf, pl.Nf, K, ids, shapes_st, gains_st, cb_stride_g))));
   GSRQ_CUDA_CHECK(cudaGetLastError());
 
   EncParams p{};
@@ -292,10 +323,10 @@ int gsrq_decode(const uint8_t *codes, const gsrq_codebook *cb, int n_stages, voi
   if (use_smem) {
     DISPATCH_D(d, {
       GSRQ_CUDA_CHECK(cudaFuncSetAttribute(k_decode<D, true, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(200 * 1024)));
-      k_decode<D, true, 4><<<grid, 256, smem, stream>>>(p);
+      LAUNCH(kClsDecode, stream, (k_decode<D, true, 4><<<grid, 256, smem, stream>>>(p)));
     });
   } else {
-    DISPATCH_D(d, (k_decode<D, false, 4><<<grid, 256, 0, stream>>>(p)));
+    LAUNCH(kClsDecode, stream, DISPATCH_D(d, (k_decode<D, false, 4><<<grid, 256, 0, stream>>>(p))));
   }
   GSRQ_CUDA_CHECK(cudaGetLastError());
   return GSRQ_OK;
@@ -363,8 +394,8 @@ int gsrq_init_ids(const void *kv, const gsrq_view *view, const float *residual, 
   rc = prepare_rows(pl, kv, view, nullptr, 0, (const long long *)fit_tokens, nullptr, 0, residual, ws, stream);
   if (rc) return rc;
   const int d = view->d;
-  DISPATCH_D(d, (k_init_ids<D><<<view->G, 512, 0, stream>>>((const float *)(ws + pl.off_Rf), pl.Nf, K, view->G, stage, seed,
-                                                              (long long *)ids_out, st)));
+  LAUNCH(kClsPrep, stream, DISPATCH_D(d, (k_init_ids<D><<<view->G, 512, 0, stream>>>((const float *)(ws + pl.off_Rf), pl.Nf, K, view->G,
+                                                                                     stage, seed, (long long *)ids_out, st))));
   GSRQ_CUDA_CHECK(cudaGetLastError());
   return GSRQ_OK;
 }
@@ -415,6 +446,82 @@ int gsrq_decode_host(const uint8_t *codes_host, const gsrq_codebook *cb, int n_s
   cudaFree(d_kv); cudaFree(d_codes);
   if (e != cudaSuccess) { set_error("gsrq_decode_host: %s", cudaGetErrorString(e)); return GSRQ_ECUDA; }
   return rc;
+}
+
+
+int gsrq_pipeline_host(const void *kv_host, const gsrq_view *view, const float *w_host, int K, int S, int iters,
+                       uint64_t seed, float *shapes_host, float *gains_host, uint8_t *codes_host, void *kv_out_host) {
+  if (!kv_host || !shapes_host || !gains_host || !codes_host) { set_error("NULL input"); return GSRQ_EINVAL; }
+  int rc = check_view(view, K, S);
+  if (rc) return rc;
+  const int G = view->G, d = view->d, M = view->hd / d;
+  const size_t esz = view->dtype == GSRQ_BF16 ? 2 : 4;
+  const size_t kv_bytes = (size_t)G * view->T * view->hd * esz;
+  const size_t n_rows = (size_t)G * view->T * M;
+  const size_t sh_bytes = (size_t)G * S * K * d * 4, ga_bytes = (size_t)G * S * K * 4;
+  const size_t wsb = gsrq_workspace_bytes(view, K, S, 0);
+  cudaStream_t stream = nullptr;
+  char *base = nullptr;
+  size_t off[8], o = 0;
+  const size_t sizes[8] = {kv_bytes, (size_t)view->T * 4, sh_bytes, ga_bytes, n_rows * S, n_rows * d * 4, wsb, kv_bytes};
+  for (int i = 0; i < 8; ++i) { off[i] = o; o += align_up(sizes[i]); }
+  cudaError_t e = cudaMallocAsync((void **)&base, o, stream);
+  if (e != cudaSuccess) { set_error("gsrq_pipeline_host: %s", cudaGetErrorString(e)); return GSRQ_ECUDA; }
+  void *d_kv = base + off[0];
+  float *d_w = w_host ? (float *)(base + off[1]) : nullptr;
+  gsrq_codebook cb{K, S, (float *)(base + off[2]), (float *)(base + off[3])};
+  uint8_t *d_codes = (uint8_t *)(base + off[4]);
+  float *d_res = (float *)(base + off[5]);
+  void *d_ws = base + off[6], *d_out = base + off[7];
+  e = cudaMemcpyAsync(d_kv, kv_host, kv_bytes, cudaMemcpyHostToDevice, stream);
+  if (e == cudaSuccess && w_host) e = cudaMemcpyAsync(d_w, w_host, (size_t)view->T * 4, cudaMemcpyHostToDevice, stream);
+  for (int s = 0; s < S && rc == GSRQ_OK && e == cudaSuccess; ++s) {
+    rc = gsrq_fit_stage(d_kv, view, d_w, 0, nullptr, 0, &cb, s, s ? d_res : nullptr, iters, seed, nullptr, d_ws, wsb, stream);
+    if (rc == GSRQ_OK) rc = gsrq_encode(d_kv, view, &cb, s, s + 1, d_codes, d_res, d_ws, wsb, stream);
+  }
+  if (rc == GSRQ_OK && e == cudaSuccess && kv_out_host) {
+    rc = gsrq_decode(d_codes, &cb, S, d_out, view, stream);
+    if (rc == GSRQ_OK) e = cudaMemcpyAsync(kv_out_host, d_out, kv_bytes, cudaMemcpyDeviceToHost, stream);
+  }
+  if (rc == GSRQ_OK && e == cudaSuccess) e = cudaMemcpyAsync(shapes_host, cb.shapes, sh_bytes, cudaMemcpyDeviceToHost, stream);
+  if (rc == GSRQ_OK && e == cudaSuccess) e = cudaMemcpyAsync(gains_host, cb.gains, ga_bytes, cudaMemcpyDeviceToHost, stream);
+  if (rc == GSRQ_OK && e == cudaSuccess) e = cudaMemcpyAsync(codes_host, d_codes, n_rows * S, cudaMemcpyDeviceToHost, stream);
+  cudaFreeAsync(base, stream);
+  cudaError_t e2 = cudaStreamSynchronize(stream);
+  if (e == cudaSuccess) e = e2;
+  if (e != cudaSuccess) { set_error("gsrq_pipeline_host: %s", cudaGetErrorString(e)); return GSRQ_ECUDA; }
+  return rc;
+}
+
+void gsrq_profile_enable(int on) {
+  std::lock_guard<std::mutex> lk(g_prof_mu);
+  g_prof_on = on != 0;
+}
+
+int gsrq_profile_read(double *ms_by_class, int64_t *launches_by_class) {
+  std::vector<ProfRec> recs;
+  {
+    std::lock_guard<std::mutex> lk(g_prof_mu);
+    recs.swap(g_prof_recs);
+  }
+  for (int c = 0; c < kNumCls; ++c) { if (ms_by_class) ms_by_class[c] = 0.0; if (launches_by_class) launches_by_class[c] = 0; }
+  int rc = GSRQ_OK;
+  for (auto &r : recs) {
+    float ms = 0.f;
+    cudaError_t e = cudaEventSynchronize(r.b);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, r.a, r.b);
+    if (e != cudaSuccess) { set_error("profile read: %s", cudaGetErrorString(e)); rc = GSRQ_ECUDA; }
+    else { if (ms_by_class) ms_by_class[r.cls] += ms; if (launches_by_class) launches_by_class[r.cls] += 1; }
+    cudaEventDestroy(r.a); cudaEventDestroy(r.b);
+  }
+  return rc;
+}
+
+int64_t gsrq_launch_count(void) {
+  std::lock_guard<std::mutex> lk(g_prof_mu);
+  long long n = 0;
+  for (int c = 0; c < kNumCls; ++c) n += g_launches[c];
+  return n;
 }
 
 }  // extern "C"
