@@ -83,7 +83,8 @@ typedef struct {
 } gsrq_fit_stats;
 
 /* Scratch size for any call on this view with these parameters.
- * n_fit_tokens = 0 means "fit on all T tokens".  Host function, no CUDA calls. */
+ * n_fit_tokens > 0: size of the fit subset; 0: "fit on all T tokens"; < 0: no fit at all
+ * (gsrq_encode / gsrq_decode only).  Host function, no CUDA calls. */
 size_t gsrq_workspace_bytes(const gsrq_view *view, int K, int S, int64_t n_fit_tokens);
 
 /*
@@ -144,6 +145,13 @@ int gsrq_decode(const uint8_t *codes, const gsrq_codebook *cb, int n_stages, voi
 int gsrq_assign(const void *kv, const gsrq_view *view, const float *residual,
                 const gsrq_codebook *cb, int stage, int mode, uint8_t *idx_out, void *workspace,
                 size_t workspace_bytes, void *stream);
+
+/* Test hook: gsrq_assign through the tensor-core filter (d == 16 only) that also dumps the raw
+ * filter scores, scores_out [G][T*M][256] fp32 (column k >= K holds -3e38).  Used to validate the
+ * filter's error bound E_i against exact arithmetic. */
+int gsrq_debug_scores(const void *kv, const gsrq_view *view, const float *residual,
+                      const gsrq_codebook *cb, int stage, int mode, float *scores_out,
+                      uint8_t *idx_out, void *workspace, size_t workspace_bytes, void *stream);
 
 /* One update (Eq. 6-8 weighted + safeguards) of stage `stage` of cb from a GIVEN assignment
  * idx [G][T*M] over all rows.  shapes_too = 0 updates gains only (Alg. 1 l.2). */

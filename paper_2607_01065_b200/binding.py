@@ -42,7 +42,7 @@ class gsrq_fit_stats(C.Structure):
 
 _lib = None
 EXPORTS = ["gsrq_workspace_bytes", "gsrq_fit_stage", "gsrq_encode", "gsrq_decode", "gsrq_assign", "gsrq_update",
-           "gsrq_init_ids", "gsrq_encode_host", "gsrq_decode_host", "gsrq_pipeline_host", "gsrq_profile_enable",
+           "gsrq_init_ids", "gsrq_debug_scores", "gsrq_encode_host", "gsrq_decode_host", "gsrq_pipeline_host", "gsrq_profile_enable",
            "gsrq_profile_read", "gsrq_launch_count", "gsrq_last_error", "gsrq_version"]
 
 
@@ -135,6 +135,11 @@ def gsrq_decode(codes, cb, n_stages, kv_out, out_view):
 def gsrq_assign(kv, view, residual, cb, stage, mode, idx_out, ws):
     _check(lib().gsrq_assign(_ptr(kv), C.byref(view), _ptr(residual), C.byref(cb), stage, mode, _ptr(idx_out),
                              _ptr(ws), C.c_size_t(ws.numel()), _stream()))
+
+
+def gsrq_debug_scores(kv, view, residual, cb, stage, mode, scores_out, idx_out, ws):
+    _check(lib().gsrq_debug_scores(_ptr(kv), C.byref(view), _ptr(residual), C.byref(cb), stage, mode, _ptr(scores_out),
+                                   _ptr(idx_out), _ptr(ws), C.c_size_t(ws.numel()), _stream()))
 
 
 def gsrq_update(kv, view, residual, w, w_stride_g, idx, cb, stage, shapes_too, ws):

@@ -1,6 +1,7 @@
 // gsrq_lib.cu -- host side of libgsrq: argument checks, workspace plan, kernel launches.
 // Every step of the path runs in the kernels under csrc/; this file only orchestrates.
 #include <stdarg.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <mutex>
@@ -11,6 +12,7 @@
 #include "k_prep.cuh"
 #include "k_reduce.cuh"
 #include "k_score.cuh"
+#include "k_score_tc.cuh"
 
 namespace gsrq {
 
@@ -57,30 +59,41 @@ static inline size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 struct Plan {
   long long nf_tok, Nf, Nall, C;
   int M;
-  size_t off_Rf, off_rinv, off_wt, off_idx, off_list, off_part, off_st, off_cnt, off_ids, off_etot, total;
+  // [0, encode_total): what gsrq_encode / gsrq_assign-less calls need; the rest is for the fit
+  size_t off_list, off_cnt, off_st, encode_total;
+  size_t off_Rf, off_rinv, off_wt, off_idx, off_part, off_ids, off_etot;
+  size_t off_ahi, off_alo, off_rnorm, off_bimg, off_efac, total;
 };
 
 constexpr int kNumCounters = 256;
 
+// n_fit_tokens: > 0 fit subset size, 0 = fit on all tokens, < 0 = no fit (encode / decode only)
 static Plan make_plan(const gsrq_view *v, int K, int S, long long n_fit_tokens) {
   (void)S;
   Plan p;
   p.M = v->hd / v->d;
-  p.nf_tok = (n_fit_tokens > 0) ? n_fit_tokens : v->T;
+  p.nf_tok = (n_fit_tokens > 0) ? n_fit_tokens : (n_fit_tokens == 0 ? v->T : 0);
   p.Nf = p.nf_tok * p.M;
   p.Nall = v->T * p.M;
   p.C = (p.Nf + kChunkRows - 1) / kChunkRows;
   size_t o = 0;
+  p.off_list = o; o += align_up((size_t)v->G * p.Nall * sizeof(uint32_t));
+  p.off_cnt = o;  o += align_up(kNumCounters * sizeof(unsigned int));
+  p.off_st = o;   o += align_up((size_t)v->G * sizeof(DevStats));
+  p.encode_total = o;
   p.off_Rf = o;   o += align_up((size_t)v->G * p.Nf * v->d * sizeof(float));
   p.off_rinv = o; o += align_up((size_t)v->G * p.Nf * sizeof(double));
   p.off_wt = o;   o += align_up((size_t)v->G * p.nf_tok * sizeof(float));
   p.off_idx = o;  o += align_up((size_t)v->G * p.Nf);
-  p.off_list = o; o += align_up((size_t)v->G * p.Nall * sizeof(uint32_t));
   p.off_part = o; o += align_up((size_t)v->G * p.C * K * (2 * v->d + 2) * sizeof(double));
-  p.off_st = o;   o += align_up((size_t)v->G * sizeof(DevStats));
-  p.off_cnt = o;  o += align_up(kNumCounters * sizeof(unsigned int));
   p.off_ids = o;  o += align_up((size_t)v->G * GSRQ_MAX_K * sizeof(long long));
   p.off_etot = o; o += align_up((size_t)v->G * sizeof(double));
+  const bool tcp = (v->d == tc::kD);
+  p.off_ahi = o;   o += align_up(tcp ? (size_t)v->G * p.Nf * tc::kD * 2 : 0);
+  p.off_alo = o;   o += align_up(tcp ? (size_t)v->G * p.Nf * tc::kD * 2 : 0);
+  p.off_rnorm = o; o += align_up(tcp ? (size_t)v->G * p.Nf * sizeof(float) : 0);
+  p.off_bimg = o;  o += align_up(tcp ? (size_t)v->G * 3 * tc::kBImgBytes : 0);
+  p.off_efac = o;  o += align_up(tcp ? (size_t)v->G * 2 * sizeof(float) : 0);
   p.total = o;
   return p;
 }
@@ -98,9 +111,9 @@ static int check_view(const gsrq_view *v, int K, int S) {
   return GSRQ_OK;
 }
 
-static int check_ws(const void *ws, size_t bytes, const Plan &p) {
+static int check_ws(const void *ws, size_t bytes, size_t need) {
   if (!ws || ((uintptr_t)ws & 255)) { set_error("workspace must be non-NULL and 256-byte aligned"); return GSRQ_EWORKSPACE; }
-  if (bytes < p.total) { set_error("workspace too small: %zu < %zu bytes", bytes, p.total); return GSRQ_EWORKSPACE; }
+  if (bytes < need) { set_error("workspace too small: %zu < %zu bytes", bytes, need); return GSRQ_EWORKSPACE; }
   return GSRQ_OK;
 }
 
@@ -150,10 +163,85 @@ static int run_reduce_renorm(const Plan &pl, const gsrq_view *v, int K, char *ws
   return GSRQ_OK;
 }
 
+
+// ---- tensor-core scoring path (d == 16) ----
+static bool use_tc(int d) {
+  static const bool off = getenv("GSRQ_DISABLE_TC") != nullptr;
+  return d == tc::kD && !off;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn encode_tiled_fn() {
+  static EncodeTiledFn fn = []() -> EncodeTiledFn {
+    void *f = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess)
+      return nullptr;
+    return (EncodeTiledFn)f;
+  }();
+  return fn;
+}
+
+// 3-D tensor map over an operand plane [G][N][16] bf16: box = 128 rows of one group, SWIZZLE_32B,
+// out-of-range rows read as zero.
+static int make_plane_map(CUtensorMap *tm, const void *base, long long N, int G) {
+  EncodeTiledFn fn = encode_tiled_fn();
+  if (!fn) { set_error("cuTensorMapEncodeTiled entry point not available"); return GSRQ_ECUDA; }
+  const cuuint64_t dims[3] = {(cuuint64_t)tc::kD, (cuuint64_t)N, (cuuint64_t)G};
+  const cuuint64_t strides[2] = {(cuuint64_t)tc::kD * 2, (cuuint64_t)N * tc::kD * 2};
+  const cuuint32_t box[3] = {(cuuint32_t)tc::kD, (cuuint32_t)tc::kTileM, 1};
+  const cuuint32_t es[3] = {1, 1, 1};
+  CUresult r = fn(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void *>(base), dims, strides, box, es,
+                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) { set_error("cuTensorMapEncodeTiled failed (%d)", (int)r); return GSRQ_ECUDA; }
+  return GSRQ_OK;
+}
+
+// One assignment pass on the prepared fit rows with the tcgen05 filter + the exact refine.
+static int run_assign_tc(const Plan &pl, char *ws, int G, const float *shapes_st, const float *gains_st, long long cb_stride_g,
+                         int S, int K, int mode, int n_planes, uint8_t *idx, DevStats *st, int slot, unsigned int *list_cnt,
+                         float *dbg, cudaStream_t stream) {
+  uint8_t *bimg = (uint8_t *)(ws + pl.off_bimg);
+  float *efac = (float *)(ws + pl.off_efac);
+  LAUNCH(kClsRenorm, stream, (tc::k_bimg<<<G, 256, 0, stream>>>(shapes_st, gains_st, cb_stride_g, K, mode, n_planes, bimg, efac, st)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  CUtensorMap tm_hi, tm_lo;
+  int rc = make_plane_map(&tm_hi, ws + pl.off_ahi, pl.Nf, G);
+  if (rc) return rc;
+  rc = make_plane_map(&tm_lo, ws + (n_planes == 2 ? pl.off_alo : pl.off_ahi), pl.Nf, G);
+  if (rc) return rc;
+  tc::ScoreTcParams p{};
+  p.bimg = bimg; p.efac = efac; p.rnorm = (const float *)(ws + pl.off_rnorm); p.idx = idx; p.N = pl.Nf;
+  p.n_tiles = (int)((pl.Nf + tc::kTileM - 1) / tc::kTileM); p.n_planes = n_planes;
+  p.list = (uint32_t *)(ws + pl.off_list); p.list_cnt = list_cnt; p.st = st; p.slot = slot; p.dbg = dbg;
+  static int n_sm = 0;
+  if (!n_sm) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev); if (n_sm <= 0) n_sm = 148; }
+  int ctas = n_sm / G; if (ctas < 1) ctas = 1; if (ctas > p.n_tiles) ctas = p.n_tiles;
+  const size_t smem = 120 * 1024;  // > half of the SM's shared memory: one CTA (and one 512-column TMEM allocation) per SM
+  static_assert(tc::kSmemTotal <= 120 * 1024, "smem budget");
+  GSRQ_CUDA_CHECK(cudaFuncSetAttribute(tc::k_score_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  LAUNCH(kClsScore, stream, (tc::k_score_tc<<<dim3((unsigned)ctas, (unsigned)G), tc::kThreads, smem, stream>>>(tm_hi, tm_lo, p)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  // exact re-score of the flagged rows (reads the fp32 rows)
+  EncParams e{};
+  e.src.rows = (const float *)(ws + pl.off_Rf); e.src.rows_per_group = pl.Nf; e.src.M = pl.M; e.src.d = tc::kD;
+  e.N = pl.Nf; e.shapes = shapes_st; e.gains = gains_st; e.S = S; e.K = K;
+  e.s_begin = 0; e.s_end = 1; e.s_base = 0; e.mode = mode; e.subtract = 0;
+  e.codes = idx; e.code_stride_s = 0; e.res_out = nullptr; e.st = st; e.slot = slot;
+  e.list = p.list; e.list_cnt = list_cnt;
+  LAUNCH(kClsRefine, stream, (k_encode_refine<tc::kD><<<296, 256, 0, stream>>>(e)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  return GSRQ_OK;
+}
+
 // Gather the fit rows (deriving the stage's residual when needed) and the per-row constants.
 static int prepare_rows(const Plan &pl, const void *kv, const gsrq_view *v, const float *w, long long w_stride_g,
                         const long long *fit_tokens, const gsrq_codebook *cb, int stage, const float *residual, char *ws,
-                        cudaStream_t stream) {
+                        cudaStream_t stream, int n_planes = 0) {
   const int d = v->d, G = v->G;
   float *Rf = (float *)(ws + pl.off_Rf);
   double *rinv = (double *)(ws + pl.off_rinv);
@@ -174,7 +262,13 @@ static int prepare_rows(const Plan &pl, const void *kv, const gsrq_view *v, cons
     if (rc) return rc;
   }
   const long long n_rows = (long long)G * pl.Nf;
-  LAUNCH(kClsPrep, stream, DISPATCH_D(d, (k_rinv<D><<<(unsigned)((n_rows + 255) / 256), 256, 0, stream>>>(Rf, n_rows, rinv))));
+  if (n_planes > 0) {  // tensor-core path: bf16 operand planes + row norms (+ rinv) in one pass
+    LAUNCH(kClsPrep, stream, (tc::k_planes<<<(unsigned)((n_rows + 255) / 256), 256, 0, stream>>>(
+        Rf, n_rows, (__nv_bfloat16 *)(ws + pl.off_ahi), n_planes == 2 ? (__nv_bfloat16 *)(ws + pl.off_alo) : nullptr,
+        (float *)(ws + pl.off_rnorm), rinv)));
+  } else {
+    LAUNCH(kClsPrep, stream, DISPATCH_D(d, (k_rinv<D><<<(unsigned)((n_rows + 255) / 256), 256, 0, stream>>>(Rf, n_rows, rinv))));
+  }
   GSRQ_CUDA_CHECK(cudaGetLastError());
   LAUNCH(kClsPrep, stream, DISPATCH_D(d, (k_energy<D><<<G, 1024, 0, stream>>>(Rf, wt, pl.Nf, pl.M, (double *)(ws + pl.off_etot)))));
   GSRQ_CUDA_CHECK(cudaGetLastError());
@@ -192,7 +286,7 @@ const char *gsrq_version(void) { return "gsrq-b200 0.1 (sm_100a)"; }
 
 size_t gsrq_workspace_bytes(const gsrq_view *view, int K, int S, int64_t n_fit_tokens) {
   if (check_view(view, K, S) != GSRQ_OK) return 0;
-  if (n_fit_tokens < 0 || n_fit_tokens > view->T) return 0;
+  if (n_fit_tokens > view->T) { set_error("n_fit_tokens > T"); return 0; }
   return make_plan(view, K, S, n_fit_tokens).total;
 }
 
@@ -208,7 +302,7 @@ int gsrq_fit_stage(const void *kv, const gsrq_view *view, const float *w, int64_
   if (fit_tokens && (n_fit <= 0 || n_fit > view->T)) { set_error("n_fit out of range"); return GSRQ_EINVAL; }
   const Plan pl = make_plan(view, cb->K, cb->S, fit_tokens ? n_fit : 0);
   if (pl.Nf < cb->K) { set_error("fewer fit rows (%lld) than codewords (%d)", pl.Nf, cb->K); return GSRQ_EDEGENERATE; }
-  rc = check_ws(workspace, workspace_bytes, pl);
+  rc = check_ws(workspace, workspace_bytes, pl.total);
   if (rc) return rc;
   char *ws = (char *)workspace;
   const int G = view->G, d = view->d, K = cb->K;
@@ -220,7 +314,9 @@ int gsrq_fit_stage(const void *kv, const gsrq_view *view, const float *w, int64_
   GSRQ_CUDA_CHECK(cudaMemsetAsync(st, 0, (size_t)G * sizeof(DevStats), stream));
   GSRQ_CUDA_CHECK(cudaMemsetAsync(cnt, 0, kNumCounters * sizeof(unsigned int), stream));
   GSRQ_CUDA_CHECK(cudaMemsetAsync(idx, 0, (size_t)G * pl.Nf, stream));
-  rc = prepare_rows(pl, kv, view, w, w_stride_g, (const long long *)fit_tokens, cb, stage, residual, ws, stream);
+  // rows are bf16-exact only for stage 0 of a bf16 tensor; otherwise the A operand is split hi + lo
+  const int n_planes = !use_tc(d) ? 0 : ((stage == 0 && !residual && view->dtype == GSRQ_BF16) ? 1 : 2);
+  rc = prepare_rows(pl, kv, view, w, w_stride_g, (const long long *)fit_tokens, cb, stage, residual, ws, stream, n_planes);
   if (rc) return rc;
 
   float *shapes_st = cb->shapes + (size_t)stage * K * d;
@@ -247,7 +343,10 @@ int gsrq_fit_stage(const void *kv, const gsrq_view *view, const float *w, int64_
     // score only stage `stage` on the prepared rows: present it to the kernel as a 1-stage pass
     a.shapes = shapes_st; a.gains = gains_st;
     a.s_begin = 0; a.s_end = 1; a.s_base = 0;
-    rc = run_encode(a, G, d, stream);
+    if (n_planes)
+      rc = run_assign_tc(pl, ws, G, shapes_st, gains_st, cb_stride_g, cb->S, K, a.mode, n_planes, idx, st, t, cnt + t, nullptr, stream);
+    else
+      rc = run_encode(a, G, d, stream);
     if (rc) break;
     rc = run_reduce_renorm(pl, view, K, ws, idx, shapes_st, gains_st, cb_stride_g, st, t > 0, t, stream);
   }
@@ -286,8 +385,8 @@ int gsrq_encode(const void *kv, const gsrq_view *view, const gsrq_codebook *cb, 
   int rc = check_view(view, cb->K, cb->S);
   if (rc) return rc;
   if (stage_begin < 0 || stage_end > cb->S || stage_begin >= stage_end) { set_error("bad stage range [%d, %d)", stage_begin, stage_end); return GSRQ_EINVAL; }
-  const Plan pl = make_plan(view, cb->K, cb->S, 0);
-  rc = check_ws(workspace, workspace_bytes, pl);
+  const Plan pl = make_plan(view, cb->K, cb->S, -1);
+  rc = check_ws(workspace, workspace_bytes, pl.encode_total);
   if (rc) return rc;
   char *ws = (char *)workspace;
   unsigned int *cnt = (unsigned int *)(ws + pl.off_cnt);
@@ -332,28 +431,47 @@ int gsrq_decode(const uint8_t *codes, const gsrq_codebook *cb, int n_stages, voi
   return GSRQ_OK;
 }
 
-int gsrq_assign(const void *kv, const gsrq_view *view, const float *residual, const gsrq_codebook *cb, int stage, int mode,
-                uint8_t *idx_out, void *workspace, size_t workspace_bytes, void *stream_) {
-  cudaStream_t stream = (cudaStream_t)stream_;
+static int assign_all_rows(const void *kv, const gsrq_view *view, const float *residual, const gsrq_codebook *cb, int stage,
+                           int mode, uint8_t *idx_out, float *dbg, void *workspace, size_t workspace_bytes, cudaStream_t stream) {
   if ((!kv && !residual) || !cb || !cb->shapes || !cb->gains || !idx_out) { set_error("NULL input"); return GSRQ_EINVAL; }
   int rc = check_view(view, cb->K, cb->S);
   if (rc) return rc;
   if (stage < 0 || stage >= cb->S || (mode != 0 && mode != 1)) { set_error("bad stage / mode"); return GSRQ_EINVAL; }
   const Plan pl = make_plan(view, cb->K, cb->S, 0);
-  rc = check_ws(workspace, workspace_bytes, pl);
+  rc = check_ws(workspace, workspace_bytes, pl.total);
   if (rc) return rc;
   char *ws = (char *)workspace;
   unsigned int *cnt = (unsigned int *)(ws + pl.off_cnt);
   GSRQ_CUDA_CHECK(cudaMemsetAsync(cnt, 0, sizeof(unsigned int), stream));
+  const float *shapes_st = cb->shapes + (size_t)stage * cb->K * view->d;
+  const float *gains_st = cb->gains + (size_t)stage * cb->K;
+  if (use_tc(view->d)) {
+    const int n_planes = (!residual && view->dtype == GSRQ_BF16) ? 1 : 2;
+    rc = prepare_rows(pl, kv, view, nullptr, 0, nullptr, cb, 0, residual, ws, stream, n_planes);
+    if (rc) return rc;
+    return run_assign_tc(pl, ws, view->G, shapes_st, gains_st, (long long)cb->S * cb->K, cb->S, cb->K, mode, n_planes, idx_out,
+                         nullptr, 0, cnt, dbg, stream);
+  }
+  if (dbg) { set_error("score dump needs the tensor-core path (d == 16)"); return GSRQ_EUNSUPPORTED; }
   EncParams p{};
   p.src = make_src(kv, view, residual, pl.Nall);
   p.N = pl.Nall; p.S = cb->S; p.K = cb->K;
-  p.shapes = cb->shapes + (size_t)stage * cb->K * view->d;
-  p.gains = cb->gains + (size_t)stage * cb->K;
+  p.shapes = shapes_st; p.gains = gains_st;
   p.s_begin = 0; p.s_end = 1; p.s_base = 0; p.mode = mode; p.subtract = 0;
   p.codes = idx_out; p.code_stride_s = 0; p.res_out = nullptr; p.st = nullptr; p.slot = 0;
   p.list = (uint32_t *)(ws + pl.off_list); p.list_cnt = cnt;
   return run_encode(p, view->G, view->d, stream);
+}
+
+int gsrq_assign(const void *kv, const gsrq_view *view, const float *residual, const gsrq_codebook *cb, int stage, int mode,
+                uint8_t *idx_out, void *workspace, size_t workspace_bytes, void *stream_) {
+  return assign_all_rows(kv, view, residual, cb, stage, mode, idx_out, nullptr, workspace, workspace_bytes, (cudaStream_t)stream_);
+}
+
+int gsrq_debug_scores(const void *kv, const gsrq_view *view, const float *residual, const gsrq_codebook *cb, int stage, int mode,
+                      float *scores_out, uint8_t *idx_out, void *workspace, size_t workspace_bytes, void *stream_) {
+  if (!scores_out) { set_error("NULL scores_out"); return GSRQ_EINVAL; }
+  return assign_all_rows(kv, view, residual, cb, stage, mode, idx_out, scores_out, workspace, workspace_bytes, (cudaStream_t)stream_);
 }
 
 int gsrq_update(const void *kv, const gsrq_view *view, const float *residual, const float *w, int64_t w_stride_g,
@@ -365,7 +483,7 @@ int gsrq_update(const void *kv, const gsrq_view *view, const float *residual, co
   if (rc) return rc;
   if (stage < 0 || stage >= cb->S) { set_error("bad stage"); return GSRQ_EINVAL; }
   const Plan pl = make_plan(view, cb->K, cb->S, 0);
-  rc = check_ws(workspace, workspace_bytes, pl);
+  rc = check_ws(workspace, workspace_bytes, pl.total);
   if (rc) return rc;
   char *ws = (char *)workspace;
   DevStats *st = (DevStats *)(ws + pl.off_st);
@@ -386,7 +504,7 @@ int gsrq_init_ids(const void *kv, const gsrq_view *view, const float *residual, 
   if (fit_tokens && (n_fit <= 0 || n_fit > view->T)) { set_error("n_fit out of range"); return GSRQ_EINVAL; }
   const Plan pl = make_plan(view, K, 1, fit_tokens ? n_fit : 0);
   if (pl.Nf < K) { set_error("fewer fit rows than codewords"); return GSRQ_EDEGENERATE; }
-  rc = check_ws(workspace, workspace_bytes, pl);
+  rc = check_ws(workspace, workspace_bytes, pl.total);
   if (rc) return rc;
   char *ws = (char *)workspace;
   DevStats *st = (DevStats *)(ws + pl.off_st);

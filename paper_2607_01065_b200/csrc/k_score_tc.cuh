@@ -1,0 +1,371 @@
+// k_score_tc.cuh -- tcgen05 scoring + fused arg-max (the filter of DESIGN.md section 3 on the
+// 5th-gen tensor cores).  d = 16, K <= 256.
+//
+// Scores of a 128-row tile against all 256 codewords are one [128 x 16] x [16 x 256] contraction
+// per operand split, accumulated in TMEM (fp32):
+//     D  = A_hi . B_hi^T            A_hi = bf16(r)            B_hi = bf16(c'),  c' = fl32(2 g_k s_k)
+//     D += A_hi . B_lo^T            B_lo = bf16(c' - B_hi)
+//     D += A_lo . B_hi^T            A_lo = bf16(r - A_hi)     (only when r is not bf16-exact)
+//     D += A_1  . B_bias^T          A_1 = [1 1 1 0 ...],      B_bias[k] = -[b1 b2 b3 0 ...], b1+b2+b3 = fl32(g_k^2)
+// so D[i][k] ~= 2 g_k r_i.s_k - g_k^2 (Eq. 5) with a bounded error E_i, and the
+// epilogue is a pure max / arg-max: the N x K score matrix never leaves the SM.  Rows whose
+// top-2 gap is <= 2 E_i go to the exact fp64 re-score (k_encode_refine).
+//
+// Warp roles (192 threads, one CTA per SM, persistent over the tiles of one group):
+//   warp 0      TMA producer: B operand images once (cp.async.bulk), A tiles through a ring
+//               (cp.async.bulk.tensor, SWIZZLE_32B)
+//   warp 1      TMEM allocation + tcgen05.mma issue (one elected lane), tcgen05.commit
+//   warps 2-5   epilogue: tcgen05.ld of the accumulator (thread = row), hierarchical max,
+//               arg-max, near-tie flagging, code write.  Two 256-column accumulators are
+//               double-buffered so tile i's epilogue overlaps tile i+1's MMAs.
+#pragma once
+#include <cuda.h>
+
+#include "gsrq_common.cuh"
+
+namespace gsrq {
+namespace tc {
+
+constexpr int kTileM = 128, kN = 256, kD = 16;
+constexpr int kStages = 8;
+constexpr int kThreads = 192;
+constexpr uint32_t kPlaneBytes = kTileM * kD * 2;  // 4096
+constexpr uint32_t kBImgBytes = kN * kD * 2;       // 8192
+constexpr uint32_t kSmemB = 0;                                   // 3 images
+constexpr uint32_t kSmemOnes = 3 * kBImgBytes;                   // 24576
+constexpr uint32_t kSmemA = kSmemOnes + kPlaneBytes;             // 28672, ring of kStages x 2 planes
+constexpr uint32_t kSmemBar = kSmemA + kStages * 2 * kPlaneBytes;  // 94208
+constexpr uint32_t kSmemTotal = kSmemBar + 256 + 1024;           // + alignment slack
+
+struct ScoreTcParams {
+  const uint8_t *bimg;   // [G][3][8192]: B_hi, B_lo, B_bias operand images (SWIZZLE_32B K-major)
+  const float *efac;     // [G][2]: E_i = efac[0] * ||r_i|| + efac[1]
+  const float *rnorm;    // [G][N] fp32 row norms (upper bounds)
+  uint8_t *idx;          // [G][N]
+  long long N;           // rows per group
+  int n_tiles;           // tiles per group
+  int n_planes;          // 1: A_hi only; 2: A_hi + A_lo
+  uint32_t *list;
+  unsigned int *list_cnt;
+  DevStats *st;
+  int slot;
+  float *dbg;            // optional [G][N][256] raw scores (tests only)
+};
+
+// ---------------------------------------------------------------- PTX wrappers
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t.reg .pred P1;\n\t"
+      "WAIT_LOOP:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
+      "@P1 bra DONE;\n\t"
+      "bra WAIT_LOOP;\n\t"
+      "DONE:\n\t}" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+               "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap *tm, int c0, int c1, int c2, uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(dst),
+      "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void tmem_alloc(uint32_t dst_smem, uint32_t cols) {
+  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst_smem), "r"(cols) : "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t cols) {
+  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(cols) : "memory");
+}
+__device__ __forceinline__ void mma_f16(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc),
+      "r"(acc) : "memory");
+}
+__device__ __forceinline__ void mma_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+#define GSRQ_TMEM_LD16(taddr, v)                                                                                      \
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];" \
+               : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),       \
+                 "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])  \
+               : "r"(taddr) : "memory")
+
+// K-major, SWIZZLE_32B shared-memory matrix descriptor: rows are 32 B (16 bf16) wide, 8-row
+// groups are 256 B apart (SBO), the two 16-byte K chunks of a row are XOR-swizzled with bit 2
+// of the row index.  Bits: [0,14) addr>>4, [16,30) LBO>>4 (=1, unused), [32,46) SBO>>4,
+// [46,48) version = 1 (sm_100), [61,64) layout = 6 (SWIZZLE_32B).
+__device__ __forceinline__ uint64_t make_desc_sw32(uint32_t saddr) {
+  return (uint64_t)((saddr & 0x3FFFFu) >> 4) | (1ull << 16) | ((uint64_t)(256 >> 4) << 32) | (1ull << 46) | (6ull << 61);
+}
+// Instruction descriptor, kind::f16: D fp32 (bits 4-5 = 1), A bf16 (bits 7-9 = 1), B bf16 (bits 10-12 = 1),
+// both K-major (bits 15, 16 = 0), N>>3 at bits 17-22, M>>4 at bits 24-28.
+constexpr uint32_t kIdesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(kN >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
+
+// byte offset of element (row, col) of a [rows][16] bf16 tile in the SWIZZLE_32B layout
+__host__ __device__ __forceinline__ uint32_t sw32_off(int row, int col) {
+  return (uint32_t)row * 32u + ((((uint32_t)col >> 3) ^ (((uint32_t)row >> 2) & 1u)) << 4) + ((uint32_t)col & 7u) * 2u;
+}
+
+__device__ __forceinline__ float max16(const uint32_t *v) {
+  float m0 = fmaxf(fmaxf(__uint_as_float(v[0]), __uint_as_float(v[1])), __uint_as_float(v[2]));
+  float m1 = fmaxf(fmaxf(__uint_as_float(v[3]), __uint_as_float(v[4])), __uint_as_float(v[5]));
+  float m2 = fmaxf(fmaxf(__uint_as_float(v[6]), __uint_as_float(v[7])), __uint_as_float(v[8]));
+  float m3 = fmaxf(fmaxf(__uint_as_float(v[9]), __uint_as_float(v[10])), __uint_as_float(v[11]));
+  float m4 = fmaxf(fmaxf(__uint_as_float(v[12]), __uint_as_float(v[13])), __uint_as_float(v[14]));
+  m0 = fmaxf(fmaxf(m0, m1), m2);
+  m3 = fmaxf(fmaxf(m3, m4), __uint_as_float(v[15]));
+  return fmaxf(m0, m3);
+}
+
+__global__ void __launch_bounds__(kThreads, 1)
+k_score_tc(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CUtensorMap tm_lo, ScoreTcParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  const int g = blockIdx.y;
+  if (p.st && p.st[g].done) return;
+  const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  uint8_t *sgen = smem_raw + (sbase - smem_u32(smem_raw));
+  const uint32_t bar0 = sbase + kSmemBar;
+  auto full_a = [&](int s) { return bar0 + 8u * s; };
+  auto empty_a = [&](int s) { return bar0 + 8u * (kStages + s); };
+  auto tmem_full = [&](int b) { return bar0 + 8u * (2 * kStages + b); };
+  auto tmem_empty = [&](int b) { return bar0 + 8u * (2 * kStages + 2 + b); };
+  const uint32_t b_full = bar0 + 8u * (2 * kStages + 4);
+  volatile uint32_t *tmem_slot = reinterpret_cast<volatile uint32_t *>(sgen + kSmemBar + 8 * (2 * kStages + 5));
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < kStages; ++s) { mbar_init(full_a(s), 1); mbar_init(empty_a(s), 1); }
+    for (int b = 0; b < 2; ++b) { mbar_init(tmem_full(b), 1); mbar_init(tmem_empty(b), 4); }
+    mbar_init(b_full, 1);
+    fence_barrier_init();
+  }
+  // constant A_1 tile: columns 0,1,2 = 1.0 (bf16 0x3F80), rest 0
+  for (int e = threadIdx.x; e < kTileM * kD; e += kThreads) {
+    const int row = e >> 4, col = e & 15;
+    *reinterpret_cast<uint16_t *>(sgen + kSmemOnes + sw32_off(row, col)) = (col < 3) ? 0x3F80 : 0;
+  }
+  fence_proxy_async();
+  if (warp == 1) tmem_alloc(smem_u32((const void *)tmem_slot), 512);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  const int n_my = (p.n_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+
+  if (warp == 0) {
+    if (lane == 0) {
+      mbar_expect_tx(b_full, 3 * kBImgBytes);
+      bulk_g2s(sbase + kSmemB, p.bimg + (size_t)g * 3 * kBImgBytes, 3 * kBImgBytes, b_full);
+      for (int it = 0; it < n_my; ++it) {
+        const int st = it % kStages, ph = (it / kStages) & 1;
+        const int tile = blockIdx.x + it * gridDim.x;
+        mbar_wait(empty_a(st), ph ^ 1);
+        mbar_expect_tx(full_a(st), p.n_planes * kPlaneBytes);
+        tma_load_3d(sbase + kSmemA + st * 2 * kPlaneBytes, &tm_hi, 0, tile * kTileM, g, full_a(st));
+        if (p.n_planes == 2)
+          tma_load_3d(sbase + kSmemA + st * 2 * kPlaneBytes + kPlaneBytes, &tm_lo, 0, tile * kTileM, g, full_a(st));
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0) {
+      const uint64_t d_bhi = make_desc_sw32(sbase + kSmemB), d_blo = make_desc_sw32(sbase + kSmemB + kBImgBytes);
+      const uint64_t d_bias = make_desc_sw32(sbase + kSmemB + 2 * kBImgBytes), d_ones = make_desc_sw32(sbase + kSmemOnes);
+      mbar_wait(b_full, 0);
+      for (int it = 0; it < n_my; ++it) {
+        const int st = it % kStages, ph = (it / kStages) & 1;
+        const int buf = it & 1, bph = (it >> 1) & 1;
+        mbar_wait(tmem_empty(buf), bph ^ 1);
+        mbar_wait(full_a(st), ph);
+        tc_fence_after();
+        const uint32_t d = tmem_base + buf * kN;
+        const uint64_t d_ahi = make_desc_sw32(sbase + kSmemA + st * 2 * kPlaneBytes);
+        mma_f16(d, d_ahi, d_bhi, kIdesc, 0);
+        mma_f16(d, d_ahi, d_blo, kIdesc, 1);
+        if (p.n_planes == 2) mma_f16(d, make_desc_sw32(sbase + kSmemA + st * 2 * kPlaneBytes + kPlaneBytes), d_bhi, kIdesc, 1);
+        mma_f16(d, d_ones, d_bias, kIdesc, 1);
+        mma_commit(empty_a(st));
+        mma_commit(tmem_full(buf));
+      }
+    }
+  } else {
+    const int q = warp & 3;  // TMEM lane quarter this warp may access
+    const float e1 = p.efac[2 * g], e0 = p.efac[2 * g + 1];
+    unsigned int n_changed = 0;
+    for (int it = 0; it < n_my; ++it) {
+      const int buf = it & 1, bph = (it >> 1) & 1;
+      const int tile = blockIdx.x + it * gridDim.x;
+      const long long row = (long long)tile * kTileM + q * 32 + lane;
+      mbar_wait(tmem_full(buf), bph);
+      tc_fence_after();
+      const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + buf * kN;
+      // Two groupings of the 256 scores: A = 16 consecutive columns (gmA[c], c = col / 16) and
+      // B = columns with equal col % 16 (gmB[b]).  The winner is (first A group == best, first B
+      // group == best); every other column lies in another A group or another B group, so
+      // second = max(max_{c != ga} gmA[c], max_{b != gb} gmB[b]) exactly.  Pure 3-input max work.
+      float gmA[16], gmB[16];
+      uint32_t va[16], vb[16];
+      GSRQ_TMEM_LD16(taddr, va);
+#pragma unroll
+      for (int c = 0; c < 16; c += 2) {
+        tmem_wait_ld();
+        GSRQ_TMEM_LD16(taddr + (c + 1) * 16, vb);
+        gmA[c] = max16(va);
+        if (p.dbg && row < p.N)
+          for (int j = 0; j < 16; ++j) p.dbg[((long long)g * p.N + row) * kN + c * 16 + j] = __uint_as_float(va[j]);
+        float ta[16];
+#pragma unroll
+        for (int j = 0; j < 16; ++j) ta[j] = __uint_as_float(va[j]);
+        tmem_wait_ld();
+        if (c + 2 < 16) GSRQ_TMEM_LD16(taddr + (c + 2) * 16, va);
+        gmA[c + 1] = max16(vb);
+        if (p.dbg && row < p.N)
+          for (int j = 0; j < 16; ++j) p.dbg[((long long)g * p.N + row) * kN + (c + 1) * 16 + j] = __uint_as_float(vb[j]);
+#pragma unroll
+        for (int j = 0; j < 16; ++j)
+          gmB[j] = (c == 0) ? fmaxf(ta[j], __uint_as_float(vb[j])) : fmaxf(fmaxf(gmB[j], ta[j]), __uint_as_float(vb[j]));
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(tmem_empty(buf));  // accumulator drained: MMA may overwrite it
+      float best = gmA[0];
+#pragma unroll
+      for (int c = 1; c < 16; ++c) best = fmaxf(best, gmA[c]);
+      int gi = 15, ji = 15;
+#pragma unroll
+      for (int c = 14; c >= 0; --c) {
+        gi = (gmA[c] == best) ? c : gi;
+        ji = (gmB[c] == best) ? c : ji;
+      }
+      float second = -INFINITY;
+#pragma unroll
+      for (int c = 0; c < 16; ++c) {
+        second = fmaxf(second, (c == gi) ? -INFINITY : gmA[c]);
+        second = fmaxf(second, (c == ji) ? -INFINITY : gmB[c]);
+      }
+      if (row < p.N) {
+        const long long gr = (long long)g * p.N + row;
+        const float E = fmaf(e1, p.rnorm[gr], e0);
+        if (best - second <= 2.0f * E) {
+          const unsigned int pos = atomicAdd(p.list_cnt, 1u);
+          p.list[pos] = (uint32_t)gr;
+        } else {
+          const uint8_t k = (uint8_t)(gi * 16 + ji);
+          if (p.st) n_changed += (p.idx[gr] != k);
+          p.idx[gr] = k;
+        }
+      }
+    }
+    if (p.st) {
+      for (int off = 16; off; off >>= 1) n_changed += __shfl_xor_sync(0xffffffffu, n_changed, off);
+      if (lane == 0 && n_changed)
+        atomicAdd(reinterpret_cast<unsigned long long *>(&p.st[g].changed[p.slot]), (unsigned long long)n_changed);
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) tmem_dealloc(tmem_base, 512);
+}
+
+// Operand images + error factors of (group g, one stage) for k_score_tc.  grid = G, block = 256.
+//   mode 0: c' = fl32(2 fl32(g_k s_kj)), b = fl32(g_k^2);   mode 1 (projection): c' = 2 s_kj, b = 0.
+//   rows k >= K get b = 3e38 so that they can never win the arg-max.
+// efac: E = e1 ||r|| + e0,  e1 = rho * 2 g_max,  e0 = 2^-20 g_max^2.
+__global__ void __launch_bounds__(256) k_bimg(const float *__restrict__ shapes, const float *__restrict__ gains,
+                                              long long cb_stride_g, int K, int mode, int n_planes,
+                                              uint8_t *__restrict__ bimg, float *__restrict__ efac,
+                                              const DevStats *__restrict__ st) {
+  __shared__ int gmax_bits;
+  const int g = blockIdx.x, k = threadIdx.x;
+  if (st && st[g].done) return;
+  if (k == 0) gmax_bits = 0;
+  __syncthreads();
+  uint8_t *img = bimg + (size_t)g * 3 * kBImgBytes;
+  float gk = 0.f;
+  if (k < K) gk = (mode == 0) ? gains[(long long)g * cb_stride_g + k] : 1.0f;
+  const float *s = shapes + ((long long)g * cb_stride_g + k) * kD;
+#pragma unroll
+  for (int j = 0; j < kD; ++j) {
+    float c = 0.f;
+    if (k < K) c = (mode == 0) ? 2.0f * __fmul_rn(gk, s[j]) : 2.0f * s[j];
+    const __nv_bfloat16 hi = __float2bfloat16_rn(c);
+    const __nv_bfloat16 lo = __float2bfloat16_rn(__fsub_rn(c, __bfloat162float(hi)));
+    *reinterpret_cast<__nv_bfloat16 *>(img + sw32_off(k, j)) = hi;
+    *reinterpret_cast<__nv_bfloat16 *>(img + kBImgBytes + sw32_off(k, j)) = lo;
+  }
+  float b = (k < K) ? ((mode == 0) ? __fmul_rn(gk, gk) : 0.0f) : 3.0e38f;
+  const __nv_bfloat16 b1 = __float2bfloat16_rn(b);
+  const float r1 = __fsub_rn(b, __bfloat162float(b1));
+  const __nv_bfloat16 b2 = __float2bfloat16_rn(r1);
+  const __nv_bfloat16 b3 = __float2bfloat16_rn(__fsub_rn(r1, __bfloat162float(b2)));
+#pragma unroll
+  for (int j = 0; j < kD; ++j) {
+    __nv_bfloat16 v = __float2bfloat16_rn(0.f);
+    if (j == 0) v = __hneg(b1);
+    if (j == 1) v = __hneg(b2);
+    if (j == 2) v = __hneg(b3);
+    *reinterpret_cast<__nv_bfloat16 *>(img + 2 * kBImgBytes + sw32_off(k, j)) = v;
+  }
+  if (k < K && mode == 0) atomicMax(&gmax_bits, __float_as_int(fmaxf(gk, 0.f)));
+  __syncthreads();
+  if (k == 0) {
+    const float gm = (mode == 0) ? __int_as_float(gmax_bits) : 1.0f;
+    const float rho = (n_planes == 1 ? 1.5f : 4.0f) * 7.62939453125e-6f;  // x 2^-17
+    efac[2 * g] = rho * 2.0f * gm;
+    efac[2 * g + 1] = (mode == 0) ? 9.5367431640625e-7f * gm * gm : 0.0f;  // 2^-20 g_max^2
+  }
+}
+
+// fp32 rows -> bf16 operand planes (A_hi = bf16(r), A_lo = bf16(r - A_hi)), row norms, 1/(||r||+eps).
+__global__ void k_planes(const float *__restrict__ Rf, long long n_rows, __nv_bfloat16 *__restrict__ ahi,
+                         __nv_bfloat16 *__restrict__ alo, float *__restrict__ rnorm, double *__restrict__ rinv) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_rows) return;
+  float x[kD];
+  load_row_f32<kD>(Rf, i, x);
+  uint32_t h[8], l[8];
+#pragma unroll
+  for (int j = 0; j < kD; j += 2) {
+    const __nv_bfloat16 h0 = __float2bfloat16_rn(x[j]), h1 = __float2bfloat16_rn(x[j + 1]);
+    const __nv_bfloat16 l0 = __float2bfloat16_rn(__fsub_rn(x[j], __bfloat162float(h0)));
+    const __nv_bfloat16 l1 = __float2bfloat16_rn(__fsub_rn(x[j + 1], __bfloat162float(h1)));
+    h[j / 2] = (uint32_t)__bfloat16_as_ushort(h0) | ((uint32_t)__bfloat16_as_ushort(h1) << 16);
+    l[j / 2] = (uint32_t)__bfloat16_as_ushort(l0) | ((uint32_t)__bfloat16_as_ushort(l1) << 16);
+  }
+  uint4 *ph = reinterpret_cast<uint4 *>(ahi + i * kD);
+  ph[0] = make_uint4(h[0], h[1], h[2], h[3]);
+  ph[1] = make_uint4(h[4], h[5], h[6], h[7]);
+  if (alo) {
+    uint4 *pl = reinterpret_cast<uint4 *>(alo + i * kD);
+    pl[0] = make_uint4(l[0], l[1], l[2], l[3]);
+    pl[1] = make_uint4(l[4], l[5], l[6], l[7]);
+  }
+  const double n = row_norm_f64<kD>(x);
+  rnorm[i] = (float)n * 1.000001f;
+  if (rinv) rinv[i] = 1.0 / (n + kEps);
+}
+
+}  // namespace tc
+}  // namespace gsrq
