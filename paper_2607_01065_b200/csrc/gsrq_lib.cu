@@ -223,8 +223,14 @@ static int run_assign_tc(const Plan &pl, char *ws, int G, const float *shapes_st
   int ctas = n_sm / G; if (ctas < 1) ctas = 1; if (ctas > p.n_tiles) ctas = p.n_tiles;
   const size_t smem = 120 * 1024;  // > half of the SM's shared memory: one CTA (and one 512-column TMEM allocation) per SM
   static_assert(tc::kSmemTotal <= 120 * 1024, "smem budget");
-  GSRQ_CUDA_CHECK(cudaFuncSetAttribute(tc::k_score_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  LAUNCH(kClsScore, stream, (tc::k_score_tc<<<dim3((unsigned)ctas, (unsigned)G), tc::kThreads, smem, stream>>>(tm_hi, tm_lo, p)));
+  if (dbg) {
+    GSRQ_CUDA_CHECK(cudaFuncSetAttribute(tc::k_score_tc<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    LAUNCH(kClsScore, stream, (tc::k_score_tc<true><<<dim3((unsigned)ctas, (unsigned)G), tc::kThreads, smem, stream>>>(tm_hi, tm_lo, p)));
+  } else {
+    static bool attr_set = false;
+    if (!attr_set) { GSRQ_CUDA_CHECK(cudaFuncSetAttribute(tc::k_score_tc<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr_set = true; }
+    LAUNCH(kClsScore, stream, (tc::k_score_tc<false><<<dim3((unsigned)ctas, (unsigned)G), tc::kThreads, smem, stream>>>(tm_hi, tm_lo, p)));
+  }
   GSRQ_CUDA_CHECK(cudaGetLastError());
   // exact re-score of the flagged rows (reads the fp32 rows)
   EncParams e{};

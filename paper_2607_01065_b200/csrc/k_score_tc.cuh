@@ -28,7 +28,7 @@ namespace tc {
 
 constexpr int kTileM = 128, kN = 256, kD = 16;
 constexpr int kStages = 8;
-constexpr int kThreads = 192;
+constexpr int kThreads = 320;  // warp 0 TMA, warp 1 MMA, warps 2-9 epilogue (two warpgroups)
 constexpr uint32_t kPlaneBytes = kTileM * kD * 2;  // 4096
 constexpr uint32_t kBImgBytes = kN * kD * 2;       // 8192
 constexpr uint32_t kSmemB = 0;                                   // 3 images
@@ -112,6 +112,16 @@ __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.
                  "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])  \
                : "r"(taddr) : "memory")
 
+#define GSRQ_TMEM_LD32(taddr, v) \
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];" \
+               : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31]) \
+               : "r"(taddr) : "memory")
+
+#define GSRQ_TMEM_LD64(taddr, v) \
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x64.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32,%33,%34,%35,%36,%37,%38,%39,%40,%41,%42,%43,%44,%45,%46,%47,%48,%49,%50,%51,%52,%53,%54,%55,%56,%57,%58,%59,%60,%61,%62,%63}, [%64];" \
+               : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31]), "=r"(v[32]), "=r"(v[33]), "=r"(v[34]), "=r"(v[35]), "=r"(v[36]), "=r"(v[37]), "=r"(v[38]), "=r"(v[39]), "=r"(v[40]), "=r"(v[41]), "=r"(v[42]), "=r"(v[43]), "=r"(v[44]), "=r"(v[45]), "=r"(v[46]), "=r"(v[47]), "=r"(v[48]), "=r"(v[49]), "=r"(v[50]), "=r"(v[51]), "=r"(v[52]), "=r"(v[53]), "=r"(v[54]), "=r"(v[55]), "=r"(v[56]), "=r"(v[57]), "=r"(v[58]), "=r"(v[59]), "=r"(v[60]), "=r"(v[61]), "=r"(v[62]), "=r"(v[63]) \
+               : "r"(taddr) : "memory")
+
 // K-major, SWIZZLE_32B shared-memory matrix descriptor: rows are 32 B (16 bf16) wide, 8-row
 // groups are 256 B apart (SBO), the two 16-byte K chunks of a row are XOR-swizzled with bit 2
 // of the row index.  Bits: [0,14) addr>>4, [16,30) LBO>>4 (=1, unused), [32,46) SBO>>4,
@@ -139,6 +149,55 @@ __device__ __forceinline__ float max16(const uint32_t *v) {
   return fmaxf(m0, m3);
 }
 
+
+__device__ __forceinline__ float max16f(const uint32_t *v) { return max16(v); }
+
+// Running column-class maxima over 4 chunks of 16 values: gmB[j] = max over the chunks of v[16c + j].
+__device__ __forceinline__ void colmax64(const uint32_t (&v)[64], float (&gmB)[16], bool first) {
+#pragma unroll
+  for (int j = 0; j < 16; ++j) {
+    const float a = __uint_as_float(v[j]), b = __uint_as_float(v[16 + j]);
+    const float c = __uint_as_float(v[32 + j]), d = __uint_as_float(v[48 + j]);
+    if (first) gmB[j] = fmaxf(fmaxf(fmaxf(a, b), c), d);
+    else gmB[j] = fmaxf(fmaxf(fmaxf(fmaxf(gmB[j], a), b), c), d);
+  }
+}
+
+// Running column-class maxima over 2 chunks of 16 values.
+__device__ __forceinline__ void colmax32(const uint32_t (&v)[32], float (&gmB)[16], bool first) {
+#pragma unroll
+  for (int j = 0; j < 16; ++j) {
+    const float a = __uint_as_float(v[j]), b = __uint_as_float(v[16 + j]);
+    gmB[j] = first ? fmaxf(a, b) : fmaxf(fmaxf(gmB[j], a), b);
+  }
+}
+
+// Top-2 and arg-max of 16 values.  Each value first gets (15 - j) written into its 4 lowest
+// mantissa bits (a perturbation <= 2^-19 relative, accounted for in E), which makes the 16 values
+// distinct and lets the winner carry its own index.  best = max; second = max over all internal
+// nodes of a binary tournament of min(left, right) -- exact for any input, ties included.
+__device__ __forceinline__ void top2_packed16(const float (&v)[16], float &best, float &second, int &idx) {
+  float p[16];
+#pragma unroll
+  for (int j = 0; j < 16; ++j) p[j] = __uint_as_float((__float_as_uint(v[j]) & 0xFFFFFFF0u) | (uint32_t)(15 - j));
+  float a1[8], b1[8], a2[4], b2[4], a3[2], b3[2];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) { a1[i] = fmaxf(p[2 * i], p[2 * i + 1]); b1[i] = fminf(p[2 * i], p[2 * i + 1]); }
+#pragma unroll
+  for (int i = 0; i < 4; ++i) { a2[i] = fmaxf(a1[2 * i], a1[2 * i + 1]); b2[i] = fminf(a1[2 * i], a1[2 * i + 1]); }
+#pragma unroll
+  for (int i = 0; i < 2; ++i) { a3[i] = fmaxf(a2[2 * i], a2[2 * i + 1]); b3[i] = fminf(a2[2 * i], a2[2 * i + 1]); }
+  best = fmaxf(a3[0], a3[1]);
+  float s0 = fmaxf(fmaxf(b1[0], b1[1]), b1[2]);
+  float s1 = fmaxf(fmaxf(b1[3], b1[4]), b1[5]);
+  float s2 = fmaxf(fmaxf(b1[6], b1[7]), b2[0]);
+  float s3 = fmaxf(fmaxf(b2[1], b2[2]), b2[3]);
+  float s4 = fmaxf(fmaxf(b3[0], b3[1]), fminf(a3[0], a3[1]));
+  second = fmaxf(fmaxf(fmaxf(s0, s1), s2), fmaxf(s3, s4));
+  idx = 15 - (int)(__float_as_uint(best) & 15u);
+}
+
+template <bool DBG>
 __global__ void __launch_bounds__(kThreads, 1)
 k_score_tc(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CUtensorMap tm_lo, ScoreTcParams p) {
   extern __shared__ uint8_t smem_raw[];
@@ -211,69 +270,70 @@ k_score_tc(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CU
       }
     }
   } else {
-    const int q = warp & 3;  // TMEM lane quarter this warp may access
+    // Epilogue: two warpgroups; group wg owns accumulator buffer wg, i.e. the CTA's tiles it = wg, wg+2, ...
+    // so that two tiles are in flight per SM sub-partition.  Thread = row (TMEM lane).
+    const int q = warp & 3;        // TMEM lane quarter this warp may access
+    const int wg = (warp - 2) >> 2;
     const float e1 = p.efac[2 * g], e0 = p.efac[2 * g + 1];
     unsigned int n_changed = 0;
-    for (int it = 0; it < n_my; ++it) {
-      const int buf = it & 1, bph = (it >> 1) & 1;
+    for (int it = wg; it < n_my; it += 2) {
+      const int buf = wg, bph = (it >> 1) & 1;
       const int tile = blockIdx.x + it * gridDim.x;
       const long long row = (long long)tile * kTileM + q * 32 + lane;
+      const long long gr = (long long)g * p.N + row;
+      float rn = 0.f;
+      uint8_t k_old = 0;
+      if (row < p.N) { rn = p.rnorm[gr]; k_old = p.idx[gr]; }   // issued before the wait: latency hidden
       mbar_wait(tmem_full(buf), bph);
       tc_fence_after();
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + buf * kN;
       // Two groupings of the 256 scores: A = 16 consecutive columns (gmA[c], c = col / 16) and
-      // B = columns with equal col % 16 (gmB[b]).  The winner is (first A group == best, first B
-      // group == best); every other column lies in another A group or another B group, so
-      // second = max(max_{c != ga} gmA[c], max_{b != gb} gmB[b]) exactly.  Pure 3-input max work.
+      // B = columns with equal col % 16 (gmB[b]).  The winner is (arg-max A group, arg-max B
+      // group); every other column lies in another A group or another B group, so
+      // second = max(second of gmA, second of gmB).  All of it is 3-input max work.
       float gmA[16], gmB[16];
-      uint32_t va[16], vb[16];
-      GSRQ_TMEM_LD16(taddr, va);
+      uint32_t va[32], vb[32];
+      GSRQ_TMEM_LD32(taddr, va);
 #pragma unroll
-      for (int c = 0; c < 16; c += 2) {
+      for (int c = 0; c < 8; c += 2) {  // software pipeline: the load of chunk c+1 is in flight while chunk c is reduced
         tmem_wait_ld();
-        GSRQ_TMEM_LD16(taddr + (c + 1) * 16, vb);
-        gmA[c] = max16(va);
-        if (p.dbg && row < p.N)
-          for (int j = 0; j < 16; ++j) p.dbg[((long long)g * p.N + row) * kN + c * 16 + j] = __uint_as_float(va[j]);
-        float ta[16];
-#pragma unroll
-        for (int j = 0; j < 16; ++j) ta[j] = __uint_as_float(va[j]);
+        GSRQ_TMEM_LD32(taddr + (c + 1) * 32, vb);
+        gmA[2 * c] = max16(va);
+        gmA[2 * c + 1] = max16(va + 16);
+        colmax32(va, gmB, c == 0);
+        if (DBG) {
+          if (row < p.N)
+            for (int j = 0; j < 32; ++j) p.dbg[gr * kN + c * 32 + j] = __uint_as_float(va[j]);
+        }
         tmem_wait_ld();
-        if (c + 2 < 16) GSRQ_TMEM_LD16(taddr + (c + 2) * 16, va);
-        gmA[c + 1] = max16(vb);
-        if (p.dbg && row < p.N)
-          for (int j = 0; j < 16; ++j) p.dbg[((long long)g * p.N + row) * kN + (c + 1) * 16 + j] = __uint_as_float(vb[j]);
-#pragma unroll
-        for (int j = 0; j < 16; ++j)
-          gmB[j] = (c == 0) ? fmaxf(ta[j], __uint_as_float(vb[j])) : fmaxf(fmaxf(gmB[j], ta[j]), __uint_as_float(vb[j]));
+        if (c + 2 < 8) {
+          GSRQ_TMEM_LD32(taddr + (c + 2) * 32, va);
+        } else {  // accumulator drained: the MMA warp may overwrite this buffer
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(tmem_empty(buf));
+        }
+        gmA[2 * c + 2] = max16(vb);
+        gmA[2 * c + 3] = max16(vb + 16);
+        colmax32(vb, gmB, false);
+        if (DBG) {
+          if (row < p.N)
+            for (int j = 0; j < 32; ++j) p.dbg[gr * kN + (c + 1) * 32 + j] = __uint_as_float(vb[j]);
+        }
       }
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(tmem_empty(buf));  // accumulator drained: MMA may overwrite it
-      float best = gmA[0];
-#pragma unroll
-      for (int c = 1; c < 16; ++c) best = fmaxf(best, gmA[c]);
-      int gi = 15, ji = 15;
-#pragma unroll
-      for (int c = 14; c >= 0; --c) {
-        gi = (gmA[c] == best) ? c : gi;
-        ji = (gmB[c] == best) ? c : ji;
-      }
-      float second = -INFINITY;
-#pragma unroll
-      for (int c = 0; c < 16; ++c) {
-        second = fmaxf(second, (c == gi) ? -INFINITY : gmA[c]);
-        second = fmaxf(second, (c == ji) ? -INFINITY : gmB[c]);
-      }
+      float bestA, secA, bestB, secB;
+      int gi, ji;
+      top2_packed16(gmA, bestA, secA, gi);
+      top2_packed16(gmB, bestB, secB, ji);
+      const float best = fminf(bestA, bestB), second = fmaxf(secA, secB);
       if (row < p.N) {
-        const long long gr = (long long)g * p.N + row;
-        const float E = fmaf(e1, p.rnorm[gr], e0);
+        const float E = fmaf(e1, rn, e0);
         if (best - second <= 2.0f * E) {
           const unsigned int pos = atomicAdd(p.list_cnt, 1u);
           p.list[pos] = (uint32_t)gr;
         } else {
           const uint8_t k = (uint8_t)(gi * 16 + ji);
-          if (p.st) n_changed += (p.idx[gr] != k);
+          n_changed += (k_old != k);
           p.idx[gr] = k;
         }
       }
@@ -332,9 +392,9 @@ __global__ void __launch_bounds__(256) k_bimg(const float *__restrict__ shapes, 
   __syncthreads();
   if (k == 0) {
     const float gm = (mode == 0) ? __int_as_float(gmax_bits) : 1.0f;
-    const float rho = (n_planes == 1 ? 1.5f : 4.0f) * 7.62939453125e-6f;  // x 2^-17
+    const float rho = (n_planes == 1 ? 2.0f : 4.5f) * 7.62939453125e-6f;  // x 2^-17 (incl. 2^-19 index packing)
     efac[2 * g] = rho * 2.0f * gm;
-    efac[2 * g + 1] = (mode == 0) ? 9.5367431640625e-7f * gm * gm : 0.0f;  // 2^-20 g_max^2
+    efac[2 * g + 1] = (mode == 0) ? 3.814697265625e-6f * gm * gm : 0.0f;  // 2^-18 g_max^2
   }
 }
 
