@@ -172,7 +172,7 @@ def gsrq_pipeline_host(kv_host, view, w_host, K, S, iters, seed, shapes_host, ga
                                     _ptr(shapes_host), _ptr(gains_host), _ptr(codes_host), _ptr(kv_out_host)))
 
 
-KERNEL_CLASSES = ["prep", "score", "refine", "reduce", "renorm", "decode"]
+KERNEL_CLASSES = ["prep", "score", "refine", "update", "misc", "decode"]
 
 
 def gsrq_profile_enable(on: bool):

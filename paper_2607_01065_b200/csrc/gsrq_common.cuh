@@ -17,14 +17,21 @@ constexpr uint64_t kGamma = 0x9E3779B97F4A7C15ULL;
 // Device-side statistics of one group (mirrors gsrq_fit_stats; slot 0 of changed[] is the
 // init assignment, slot t the t-th Lloyd iteration).
 struct DevStats {
-  int iters_run;
-  int done;
-  int n_empty;
+  int done_iter;  // 0, or the iteration t at which Alg. 1 l.15-16 broke (kernels of passes > t skip the group)
   int err;
+  int iters_run;  // filled by k_finish
+  int pad;
   long long refined;
   long long changed[GSRQ_MAX_ITERS + 1];
-  double J[GSRQ_MAX_ITERS + 1];
+  int n_empty[GSRQ_MAX_ITERS + 1];
+  int gmax_bits[GSRQ_MAX_ITERS + 3];  // slot t: bit pattern of max_k g_k of the codebook scored at pass t
+  double J[GSRQ_MAX_ITERS + 1];       // filled by k_finish
 };
+
+// Alg. 1 l.15-16 broke at an earlier iteration: the kernels of pass t leave the group alone.
+__device__ __forceinline__ bool group_done(const DevStats *st, int g, int t) {
+  return st && st[g].done_iter != 0 && st[g].done_iter < t;
+}
 
 // Where the rows of a pass come from.  Row i of group g:
 //   src == kv  : element j at kv[g*stride_g + tok(i/M)*stride_t + (i%M)*d + j]

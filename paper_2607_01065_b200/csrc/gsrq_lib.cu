@@ -10,7 +10,7 @@
 #include "gsrq_common.cuh"
 #include "k_codec.cuh"
 #include "k_prep.cuh"
-#include "k_reduce.cuh"
+#include "k_update.cuh"
 #include "k_score.cuh"
 #include "k_score_tc.cuh"
 
@@ -28,7 +28,7 @@ void set_error(const char *fmt, ...) {
 
 
 // ---- launch accounting / optional per-kernel CUDA-event timing (gsrq_profile_*) ----
-enum { kClsPrep = 0, kClsScore = 1, kClsRefine = 2, kClsReduce = 3, kClsRenorm = 4, kClsDecode = 5, kNumCls = 6 };
+enum { kClsPrep = 0, kClsScore = 1, kClsRefine = 2, kClsUpdate = 3, kClsMisc = 4, kClsDecode = 5, kNumCls = 6 };
 struct ProfRec { int cls; cudaEvent_t a, b; };
 static std::mutex g_prof_mu;
 static std::vector<ProfRec> g_prof_recs;
@@ -57,25 +57,26 @@ struct ProfScope {
 static inline size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
 struct Plan {
-  long long nf_tok, Nf, Nall, C;
+  long long nf_tok, Nf, Nall, nE;
   int M;
-  // [0, encode_total): what gsrq_encode / gsrq_assign-less calls need; the rest is for the fit
+  // [0, encode_total): what gsrq_encode needs; the rest is for the fit
   size_t off_list, off_cnt, off_st, encode_total;
-  size_t off_Rf, off_rinv, off_wt, off_idx, off_part, off_ids, off_etot;
-  size_t off_ahi, off_alo, off_rnorm, off_bimg, off_efac, total;
+  size_t off_Rf, off_rinv, off_wt, off_idx, off_ids, off_epart, off_term;
+  size_t off_ahi, off_alo, off_rnorm, off_bimg, off_gmax, total;
 };
 
 constexpr int kNumCounters = 256;
+constexpr int kTermStride = GSRQ_MAX_ITERS + 1;
 
 // n_fit_tokens: > 0 fit subset size, 0 = fit on all tokens, < 0 = no fit (encode / decode only)
 static Plan make_plan(const gsrq_view *v, int K, int S, long long n_fit_tokens) {
-  (void)S;
+  (void)S; (void)K;
   Plan p;
   p.M = v->hd / v->d;
   p.nf_tok = (n_fit_tokens > 0) ? n_fit_tokens : (n_fit_tokens == 0 ? v->T : 0);
   p.Nf = p.nf_tok * p.M;
   p.Nall = v->T * p.M;
-  p.C = (p.Nf + kChunkRows - 1) / kChunkRows;
+  p.nE = (p.Nf + kPrepRows - 1) / kPrepRows;
   size_t o = 0;
   p.off_list = o; o += align_up((size_t)v->G * p.Nall * sizeof(uint32_t));
   p.off_cnt = o;  o += align_up(kNumCounters * sizeof(unsigned int));
@@ -85,15 +86,15 @@ static Plan make_plan(const gsrq_view *v, int K, int S, long long n_fit_tokens) 
   p.off_rinv = o; o += align_up((size_t)v->G * p.Nf * sizeof(double));
   p.off_wt = o;   o += align_up((size_t)v->G * p.nf_tok * sizeof(float));
   p.off_idx = o;  o += align_up((size_t)v->G * p.Nf);
-  p.off_part = o; o += align_up((size_t)v->G * p.C * K * (2 * v->d + 2) * sizeof(double));
   p.off_ids = o;  o += align_up((size_t)v->G * GSRQ_MAX_K * sizeof(long long));
-  p.off_etot = o; o += align_up((size_t)v->G * sizeof(double));
+  p.off_epart = o; o += align_up((size_t)v->G * p.nE * sizeof(double));
+  p.off_term = o; o += align_up(p.Nf ? (size_t)v->G * kTermStride * 256 * sizeof(double) : 0);
   const bool tcp = (v->d == tc::kD);
   p.off_ahi = o;   o += align_up(tcp ? (size_t)v->G * p.Nf * tc::kD * 2 : 0);
   p.off_alo = o;   o += align_up(tcp ? (size_t)v->G * p.Nf * tc::kD * 2 : 0);
   p.off_rnorm = o; o += align_up(tcp ? (size_t)v->G * p.Nf * sizeof(float) : 0);
   p.off_bimg = o;  o += align_up(tcp ? (size_t)v->G * 3 * tc::kBImgBytes : 0);
-  p.off_efac = o;  o += align_up(tcp ? (size_t)v->G * 2 * sizeof(float) : 0);
+  p.off_gmax = o;  o += align_up(tcp ? (size_t)v->G * sizeof(int) : 0);
   p.total = o;
   return p;
 }
@@ -143,22 +144,21 @@ static int run_encode(EncParams p, int G, int d, cudaStream_t stream) {
   return GSRQ_OK;
 }
 
-static int run_reduce_renorm(const Plan &pl, const gsrq_view *v, int K, char *ws, const uint8_t *idx, float *shapes_st,
-                             float *gains_st, long long cb_stride_g, DevStats *st, int lloyd, int t, cudaStream_t stream) {
+// One update (reduction + Eq. 7 / Eq. 8 + operand images) of the stage slice from the assignment `idx`.
+static int run_update(const Plan &pl, const gsrq_view *v, int K, char *ws, const uint8_t *idx, float *shapes_st,
+                      float *gains_st, long long cb_stride_g, DevStats *st, int lloyd, int t, bool images, cudaStream_t stream) {
   const int d = v->d;
-  const float *Rf = (const float *)(ws + pl.off_Rf);
-  const double *rinv = (const double *)(ws + pl.off_rinv);
-  const float *wt = (const float *)(ws + pl.off_wt);
-  double *part = (double *)(ws + pl.off_part);
-  const double *etot = (const double *)(ws + pl.off_etot);
-  const size_t smem = (size_t)K * kBmWords * 4 + (size_t)(kReduceThreads / 32) * kChunkRows * 2;
-  dim3 grid((unsigned)pl.C, (unsigned)v->G);
+  UpdParams u{};
+  u.Rf = (const float *)(ws + pl.off_Rf); u.rinv = (const double *)(ws + pl.off_rinv); u.wt = (const float *)(ws + pl.off_wt);
+  u.idx = idx; u.Nf = pl.Nf; u.M = pl.M; u.K = K; u.shapes = shapes_st; u.gains = gains_st; u.cb_stride_g = cb_stride_g;
+  u.st = st; u.term = st ? (double *)(ws + pl.off_term) : nullptr; u.term_stride = kTermStride; u.lloyd = lloyd; u.t = t;
+  u.bimg = images ? (uint8_t *)(ws + pl.off_bimg) : nullptr;
+  dim3 grid((unsigned)((K + kCPC - 1) / kCPC), (unsigned)v->G);
   DISPATCH_D(d, {
-    GSRQ_CUDA_CHECK(cudaFuncSetAttribute(k_reduce<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    LAUNCH(kClsReduce, stream, (k_reduce<D><<<grid, kReduceThreads, smem, stream>>>(Rf, rinv, wt, idx, pl.Nf, pl.M, K, part, st)));
+    static bool attr_set = false;
+    if (!attr_set) { GSRQ_CUDA_CHECK(cudaFuncSetAttribute(k_update<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)upd_smem_bytes<D>())); attr_set = true; }
+    LAUNCH(kClsUpdate, stream, (k_update<D><<<grid, kUpdThreads, upd_smem_bytes<D>(), stream>>>(u)));
   });
-  GSRQ_CUDA_CHECK(cudaGetLastError());
-  LAUNCH(kClsRenorm, stream, DISPATCH_D(d, (k_renorm<D><<<v->G, 256, 0, stream>>>(part, (int)pl.C, K, shapes_st, gains_st, cb_stride_g, etot, st, lloyd, t))));
   GSRQ_CUDA_CHECK(cudaGetLastError());
   return GSRQ_OK;
 }
@@ -201,23 +201,25 @@ static int make_plane_map(CUtensorMap *tm, const void *base, long long N, int G)
   return GSRQ_OK;
 }
 
-// One assignment pass on the prepared fit rows with the tcgen05 filter + the exact refine.
-static int run_assign_tc(const Plan &pl, char *ws, int G, const float *shapes_st, const float *gains_st, long long cb_stride_g,
-                         int S, int K, int mode, int n_planes, uint8_t *idx, DevStats *st, int slot, unsigned int *list_cnt,
-                         float *dbg, cudaStream_t stream) {
-  uint8_t *bimg = (uint8_t *)(ws + pl.off_bimg);
-  float *efac = (float *)(ws + pl.off_efac);
-  LAUNCH(kClsRenorm, stream, (tc::k_bimg<<<G, 256, 0, stream>>>(shapes_st, gains_st, cb_stride_g, K, mode, n_planes, bimg, efac, st)));
-  GSRQ_CUDA_CHECK(cudaGetLastError());
-  CUtensorMap tm_hi, tm_lo;
-  int rc = make_plane_map(&tm_hi, ws + pl.off_ahi, pl.Nf, G);
+struct TcMaps { CUtensorMap hi, lo; };
+
+static int make_tc_maps(TcMaps *m, const Plan &pl, char *ws, int G, int n_planes) {
+  int rc = make_plane_map(&m->hi, ws + pl.off_ahi, pl.Nf, G);
   if (rc) return rc;
-  rc = make_plane_map(&tm_lo, ws + (n_planes == 2 ? pl.off_alo : pl.off_ahi), pl.Nf, G);
-  if (rc) return rc;
+  return make_plane_map(&m->lo, ws + (n_planes == 2 ? pl.off_alo : pl.off_ahi), pl.Nf, G);
+}
+
+// One assignment pass on the prepared fit rows: tcgen05 filter with the exact refine inside.
+// The operand images (and max gain at gmax) of the scored codebook must already be in the workspace.
+static int run_assign_tc(const Plan &pl, char *ws, const TcMaps &maps, int G, const float *shapes_st, const float *gains_st,
+                         long long cb_stride_g, int K, int mode, int n_planes, uint8_t *idx, DevStats *st, int slot,
+                         const int *gmax, long long gmax_stride, float *dbg, cudaStream_t stream) {
   tc::ScoreTcParams p{};
-  p.bimg = bimg; p.efac = efac; p.rnorm = (const float *)(ws + pl.off_rnorm); p.idx = idx; p.N = pl.Nf;
-  p.n_tiles = (int)((pl.Nf + tc::kTileM - 1) / tc::kTileM); p.n_planes = n_planes;
-  p.list = (uint32_t *)(ws + pl.off_list); p.list_cnt = list_cnt; p.st = st; p.slot = slot; p.dbg = dbg;
+  p.bimg = (const uint8_t *)(ws + pl.off_bimg); p.gmax = gmax; p.gmax_stride = gmax_stride;
+  p.rnorm = (const float *)(ws + pl.off_rnorm); p.rows = (const float *)(ws + pl.off_Rf);
+  p.shapes = shapes_st; p.gains = gains_st; p.cb_stride_g = cb_stride_g; p.idx = idx; p.N = pl.Nf;
+  p.n_tiles = (int)((pl.Nf + tc::kTileM - 1) / tc::kTileM); p.n_planes = n_planes; p.K = K; p.mode = mode;
+  p.st = st; p.slot = slot; p.dbg = dbg;
   static int n_sm = 0;
   if (!n_sm) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev); if (n_sm <= 0) n_sm = 148; }
   int ctas = n_sm / G; if (ctas < 1) ctas = 1; if (ctas > p.n_tiles) ctas = p.n_tiles;
@@ -225,60 +227,54 @@ static int run_assign_tc(const Plan &pl, char *ws, int G, const float *shapes_st
   static_assert(tc::kSmemTotal <= 120 * 1024, "smem budget");
   if (dbg) {
     GSRQ_CUDA_CHECK(cudaFuncSetAttribute(tc::k_score_tc<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    LAUNCH(kClsScore, stream, (tc::k_score_tc<true><<<dim3((unsigned)ctas, (unsigned)G), tc::kThreads, smem, stream>>>(tm_hi, tm_lo, p)));
+    LAUNCH(kClsScore, stream, (tc::k_score_tc<true><<<dim3((unsigned)ctas, (unsigned)G), tc::kThreads, smem, stream>>>(maps.hi, maps.lo, p)));
   } else {
     static bool attr_set = false;
     if (!attr_set) { GSRQ_CUDA_CHECK(cudaFuncSetAttribute(tc::k_score_tc<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr_set = true; }
-    LAUNCH(kClsScore, stream, (tc::k_score_tc<false><<<dim3((unsigned)ctas, (unsigned)G), tc::kThreads, smem, stream>>>(tm_hi, tm_lo, p)));
+    LAUNCH(kClsScore, stream, (tc::k_score_tc<false><<<dim3((unsigned)ctas, (unsigned)G), tc::kThreads, smem, stream>>>(maps.hi, maps.lo, p)));
   }
-  GSRQ_CUDA_CHECK(cudaGetLastError());
-  // exact re-score of the flagged rows (reads the fp32 rows)
-  EncParams e{};
-  e.src.rows = (const float *)(ws + pl.off_Rf); e.src.rows_per_group = pl.Nf; e.src.M = pl.M; e.src.d = tc::kD;
-  e.N = pl.Nf; e.shapes = shapes_st; e.gains = gains_st; e.S = S; e.K = K;
-  e.s_begin = 0; e.s_end = 1; e.s_base = 0; e.mode = mode; e.subtract = 0;
-  e.codes = idx; e.code_stride_s = 0; e.res_out = nullptr; e.st = st; e.slot = slot;
-  e.list = p.list; e.list_cnt = list_cnt;
-  LAUNCH(kClsRefine, stream, (k_encode_refine<tc::kD><<<296, 256, 0, stream>>>(e)));
   GSRQ_CUDA_CHECK(cudaGetLastError());
   return GSRQ_OK;
 }
 
-// Gather the fit rows (deriving the stage's residual when needed) and the per-row constants.
+static int launch_prep(const Plan &pl, const gsrq_view *v, const RowSrc &src, const float *w, long long w_stride_g,
+                       const long long *fit_tokens, char *ws, bool consts, int n_planes, cudaStream_t stream) {
+  PrepParams q{};
+  q.src = src; q.w = w; q.w_stride_g = w_stride_g; q.fit_tokens = fit_tokens; q.nf_tok = pl.nf_tok;
+  q.Rf = (float *)(ws + pl.off_Rf); q.rinv = (double *)(ws + pl.off_rinv); q.wt = (float *)(ws + pl.off_wt);
+  q.epart = consts ? (double *)(ws + pl.off_epart) : nullptr;
+  q.ahi = (consts && n_planes > 0) ? (__nv_bfloat16 *)(ws + pl.off_ahi) : nullptr;
+  q.alo = (consts && n_planes == 2) ? (__nv_bfloat16 *)(ws + pl.off_alo) : nullptr;
+  q.rnorm = (consts && n_planes > 0) ? (float *)(ws + pl.off_rnorm) : nullptr;
+  dim3 grid((unsigned)pl.nE, (unsigned)v->G);
+  const int d = v->d;
+  LAUNCH(kClsPrep, stream, DISPATCH_D(d, (k_prep_rows<D><<<grid, 256, 0, stream>>>(q))));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  return GSRQ_OK;
+}
+
+// Gather the fit rows (deriving the stage's residual when needed) with their per-row constants,
+// operand planes (n_planes > 0) and energy partials.
 static int prepare_rows(const Plan &pl, const void *kv, const gsrq_view *v, const float *w, long long w_stride_g,
                         const long long *fit_tokens, const gsrq_codebook *cb, int stage, const float *residual, char *ws,
                         cudaStream_t stream, int n_planes = 0) {
   const int d = v->d, G = v->G;
   float *Rf = (float *)(ws + pl.off_Rf);
-  double *rinv = (double *)(ws + pl.off_rinv);
-  float *wt = (float *)(ws + pl.off_wt);
-  RowSrc src = make_src(kv, v, residual, pl.Nall);
-  dim3 grid((unsigned)((pl.Nf + 255) / 256), (unsigned)G);
-  LAUNCH(kClsPrep, stream, DISPATCH_D(d, (k_gather<D><<<grid, 256, 0, stream>>>(src, w, w_stride_g, fit_tokens, pl.nf_tok, Rf, nullptr, wt))));
-  GSRQ_CUDA_CHECK(cudaGetLastError());
-  if (!residual && stage > 0) {  // r = x - sum_{s<stage} c^(s)[a^(s)], in place on the compact rows
-    EncParams p{};
-    p.src = make_src(nullptr, v, Rf, pl.Nf);
-    p.N = pl.Nf; p.shapes = cb->shapes; p.gains = cb->gains; p.S = cb->S; p.K = cb->K;
-    p.s_begin = 0; p.s_end = stage; p.s_base = 0; p.mode = 0; p.subtract = 1;
-    p.codes = nullptr; p.code_stride_s = 0; p.res_out = Rf; p.st = nullptr; p.slot = 0;
-    p.list = (uint32_t *)(ws + pl.off_list);
-    p.list_cnt = (unsigned int *)(ws + pl.off_cnt) + (kNumCounters - 1);
-    int rc = run_encode(p, G, d, stream);
-    if (rc) return rc;
-  }
-  const long long n_rows = (long long)G * pl.Nf;
-  if (n_planes > 0) {  // tensor-core path: bf16 operand planes + row norms (+ rinv) in one pass
-    LAUNCH(kClsPrep, stream, (tc::k_planes<<<(unsigned)((n_rows + 255) / 256), 256, 0, stream>>>(
-        Rf, n_rows, (__nv_bfloat16 *)(ws + pl.off_ahi), n_planes == 2 ? (__nv_bfloat16 *)(ws + pl.off_alo) : nullptr,
-        (float *)(ws + pl.off_rnorm), rinv)));
-  } else {
-    LAUNCH(kClsPrep, stream, DISPATCH_D(d, (k_rinv<D><<<(unsigned)((n_rows + 255) / 256), 256, 0, stream>>>(Rf, n_rows, rinv))));
-  }
-  GSRQ_CUDA_CHECK(cudaGetLastError());
-  LAUNCH(kClsPrep, stream, DISPATCH_D(d, (k_energy<D><<<G, 1024, 0, stream>>>(Rf, wt, pl.Nf, pl.M, (double *)(ws + pl.off_etot)))));
-  GSRQ_CUDA_CHECK(cudaGetLastError());
-  return GSRQ_OK;
+  const bool derive = (!residual && stage > 0);
+  int rc = launch_prep(pl, v, make_src(kv, v, residual, pl.Nall), w, w_stride_g, fit_tokens, ws, !derive, n_planes, stream);
+  if (rc || !derive) return rc;
+  // r = x - sum_{s<stage} c^(s)[a^(s)], in place on the compact rows; then the constants of the residual rows
+  EncParams p{};
+  p.src = make_src(nullptr, v, Rf, pl.Nf);
+  p.N = pl.Nf; p.shapes = cb->shapes; p.gains = cb->gains; p.S = cb->S; p.K = cb->K;
+  p.s_begin = 0; p.s_end = stage; p.s_base = 0; p.mode = 0; p.subtract = 1;
+  p.codes = nullptr; p.code_stride_s = 0; p.res_out = Rf; p.st = nullptr; p.slot = 0;
+  p.list = (uint32_t *)(ws + pl.off_list);
+  p.list_cnt = (unsigned int *)(ws + pl.off_cnt) + (kNumCounters - 1);
+  rc = run_encode(p, G, d, stream);
+  if (rc) return rc;
+  return launch_prep(pl, v, make_src(nullptr, v, Rf, pl.Nf), (const float *)(ws + pl.off_wt), pl.nf_tok, nullptr, ws, true,
+                     n_planes, stream);
 }
 
 }  // namespace gsrq
@@ -328,35 +324,40 @@ int gsrq_fit_stage(const void *kv, const gsrq_view *view, const float *w, int64_
   float *shapes_st = cb->shapes + (size_t)stage * K * d;
   float *gains_st = cb->gains + (size_t)stage * K;
   const long long cb_stride_g = (long long)cb->S * K;
-  LAUNCH(kClsPrep, stream, DISPATCH_D(d, (k_init_ids<D><<<G, 512, 0, stream>>>(Rf, pl.Nf, K, G, stage, seed, ids, st))));
+  uint8_t *bimg = n_planes ? (uint8_t *)(ws + pl.off_bimg) : nullptr;
+  LAUNCH(kClsPrep, stream, DISPATCH_D(d, (k_init_ids<D><<<G, 512, 0, stream>>>(Rf, pl.Nf, K, G, stage, seed, ids, st, shapes_st, gains_st,
+                                                                              cb_stride_g, bimg))));
   GSRQ_CUDA_CHECK(cudaGetLastError());
-  LAUNCH(kClsPrep, stream, DISPATCH_D(d, (k_init_shapes<D><<<G, 256, 0, stream>>>(Rf, pl.Nf, K, ids, shapes_st, gains_st, cb_stride_g))));
-  GSRQ_CUDA_CHECK(cudaGetLastError());
+  TcMaps maps;
+  if (n_planes) { rc = make_tc_maps(&maps, pl, ws, G, n_planes); if (rc) return rc; }
 
   EncParams p{};
   p.src = make_src(nullptr, view, Rf, pl.Nf);
-  p.N = pl.Nf; p.shapes = cb->shapes; p.gains = cb->gains; p.S = cb->S; p.K = K;
+  p.N = pl.Nf; p.S = cb->S; p.K = K;
   p.subtract = 0;
   p.codes = idx; p.code_stride_s = 0; p.res_out = nullptr; p.st = st;
   p.list = (uint32_t *)(ws + pl.off_list);
-  // t = 0 is Alg. 1 l.2: gains by Eq. 8 under the max-projection assignment (reading c-I)
-  rc = 0;
+  // score only stage `stage` on the prepared rows: present it to the kernels as a 1-stage pass
+  p.shapes = shapes_st; p.gains = gains_st; p.s_begin = 0; p.s_end = 1; p.s_base = 0;
+  // t = 0 is Alg. 1 l.2: gains by Eq. 8 under the max-projection assignment (reading c-I);
+  // t >= 1 are the Lloyd iterations.  Two launches per pass: assignment, then the fused update.
   for (int t = 0; t <= iters && rc == 0; ++t) {
-    EncParams a = p;
-    a.mode = (t == 0) ? 1 : 0;
-    a.slot = t;
-    a.list_cnt = cnt + t;
-    // score only stage `stage` on the prepared rows: present it to the kernel as a 1-stage pass
-    a.shapes = shapes_st; a.gains = gains_st;
-    a.s_begin = 0; a.s_end = 1; a.s_base = 0;
-    if (n_planes)
-      rc = run_assign_tc(pl, ws, G, shapes_st, gains_st, cb_stride_g, cb->S, K, a.mode, n_planes, idx, st, t, cnt + t, nullptr, stream);
-    else
+    const int mode = (t == 0) ? 1 : 0;
+    if (n_planes) {
+      rc = run_assign_tc(pl, ws, maps, G, shapes_st, gains_st, cb_stride_g, K, mode, n_planes, idx, st, t, &st[0].gmax_bits[t],
+                         (long long)(sizeof(DevStats) / sizeof(int)), nullptr, stream);
+    } else {
+      EncParams a = p;
+      a.mode = mode; a.slot = t; a.list_cnt = cnt + t;
       rc = run_encode(a, G, d, stream);
+    }
     if (rc) break;
-    rc = run_reduce_renorm(pl, view, K, ws, idx, shapes_st, gains_st, cb_stride_g, st, t > 0, t, stream);
+    rc = run_update(pl, view, K, ws, idx, shapes_st, gains_st, cb_stride_g, st, t > 0, t, n_planes != 0, stream);
   }
   if (rc) return rc;
+  LAUNCH(kClsMisc, stream, (k_finish<<<G, 160, 0, stream>>>(st, (const double *)(ws + pl.off_term), kTermStride, K,
+                                                            (const double *)(ws + pl.off_epart), (int)pl.nE, iters)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
   if (stats) {
     DevStats *h = (DevStats *)malloc((size_t)G * sizeof(DevStats));
     if (!h) { set_error("out of host memory"); return GSRQ_ECUDA; }
@@ -368,12 +369,12 @@ int gsrq_fit_stage(const void *kv, const gsrq_view *view, const float *w, int64_
       gsrq_fit_stats *o = stats + g;
       memset(o, 0, sizeof(*o));
       o->iters_run = h[g].iters_run;
-      o->n_empty_last = h[g].n_empty;
       o->n_refined = h[g].refined;
       for (int t = 1; t <= h[g].iters_run; ++t) {
         o->wdist_after_assign[t - 1] = h[g].J[t];
         o->n_changed[t - 1] = h[g].changed[t];
       }
+      o->n_empty_last = h[g].n_empty[h[g].iters_run];
       o->n_changed_last = h[g].iters_run ? h[g].changed[h[g].iters_run] : 0;
       degenerate |= (h[g].err != 0);
     }
@@ -455,8 +456,16 @@ static int assign_all_rows(const void *kv, const gsrq_view *view, const float *r
     const int n_planes = (!residual && view->dtype == GSRQ_BF16) ? 1 : 2;
     rc = prepare_rows(pl, kv, view, nullptr, 0, nullptr, cb, 0, residual, ws, stream, n_planes);
     if (rc) return rc;
-    return run_assign_tc(pl, ws, view->G, shapes_st, gains_st, (long long)cb->S * cb->K, cb->S, cb->K, mode, n_planes, idx_out,
-                         nullptr, 0, cnt, dbg, stream);
+    const long long cb_stride_g = (long long)cb->S * cb->K;
+    int *gmax = (int *)(ws + pl.off_gmax);
+    LAUNCH(kClsMisc, stream, (tc::k_bimg<<<view->G, 256, 0, stream>>>(shapes_st, gains_st, cb_stride_g, cb->K, mode,
+                                                                      (uint8_t *)(ws + pl.off_bimg), gmax)));
+    GSRQ_CUDA_CHECK(cudaGetLastError());
+    TcMaps maps;
+    rc = make_tc_maps(&maps, pl, ws, view->G, n_planes);
+    if (rc) return rc;
+    return run_assign_tc(pl, ws, maps, view->G, shapes_st, gains_st, cb_stride_g, cb->K, mode, n_planes, idx_out, nullptr, 0, gmax, 1,
+                         dbg, stream);
   }
   if (dbg) { set_error("score dump needs the tensor-core path (d == 16)"); return GSRQ_EUNSUPPORTED; }
   EncParams p{};
@@ -497,8 +506,8 @@ int gsrq_update(const void *kv, const gsrq_view *view, const float *residual, co
   // rows = residual when given, else kv as is (the caller states which stage's rows these are)
   rc = prepare_rows(pl, kv, view, w, w_stride_g, nullptr, cb, 0, residual, ws, stream);
   if (rc) return rc;
-  return run_reduce_renorm(pl, view, cb->K, ws, idx, cb->shapes + (size_t)stage * cb->K * view->d,
-                           cb->gains + (size_t)stage * cb->K, (long long)cb->S * cb->K, st, shapes_too ? 1 : 0, 1, stream);
+  return run_update(pl, view, cb->K, ws, idx, cb->shapes + (size_t)stage * cb->K * view->d,
+                    cb->gains + (size_t)stage * cb->K, (long long)cb->S * cb->K, nullptr, shapes_too ? 1 : 0, 1, false, stream);
 }
 
 int gsrq_init_ids(const void *kv, const gsrq_view *view, const float *residual, const int64_t *fit_tokens, int64_t n_fit,
@@ -519,7 +528,8 @@ int gsrq_init_ids(const void *kv, const gsrq_view *view, const float *residual, 
   if (rc) return rc;
   const int d = view->d;
   LAUNCH(kClsPrep, stream, DISPATCH_D(d, (k_init_ids<D><<<view->G, 512, 0, stream>>>((const float *)(ws + pl.off_Rf), pl.Nf, K, view->G,
-                                                                                     stage, seed, (long long *)ids_out, st))));
+                                                                                     stage, seed, (long long *)ids_out, st, nullptr,
+                                                                                     nullptr, 0, nullptr))));
   GSRQ_CUDA_CHECK(cudaGetLastError());
   return GSRQ_OK;
 }

@@ -1,64 +1,100 @@
-// k_prep.cuh -- per-stage preparation kernels: gather the fit rows, per-row 1/(||r||+eps),
-// weighted energy, seeded initial rows (Alg. 1 l.1; reading c-I).
+// k_prep.cuh -- per-stage preparation kernels: gather the fit rows with their per-row constants,
+// operand planes and weighted energy; seeded initial rows and shapes (Alg. 1 l.1; reading c-I).
 #pragma once
 #include "gsrq_common.cuh"
+#include "k_update.cuh"
 
 namespace gsrq {
 
-// Gather the fit rows of every group into a compact fp32 buffer Rf [G][Nf][D] and compute
-// rinv[g][i] = 1 / (||r_i|| + eps) in fp64 (Eq. 6 with the safeguard of PAPER.md:178) and the
-// compact per-fit-token weights wt [G][nf_tok].
-template <int D>
-__global__ void k_gather(RowSrc src, const float *__restrict__ w, long long w_stride_g,
-                         const long long *__restrict__ fit_tokens, long long nf_tok,
-                         float *__restrict__ Rf, double *__restrict__ rinv, float *__restrict__ wt) {
-  const int g = blockIdx.y;
-  const long long Nf = nf_tok * src.M;
-  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= Nf) return;
-  const long long tl = i / src.M;
-  const int m = (int)(i - tl * src.M);
-  const long long tok = fit_tokens ? fit_tokens[(long long)g * nf_tok + tl] : tl;
-  float x[D];
-  if (src.rows) load_row_f32<D>(src.rows, (long long)g * src.rows_per_group + tok * src.M + m, x);
-  else load_row_kv<D>(src.kv, src.dtype, (long long)g * src.stride_g + tok * src.stride_t + (long long)m * D, x);
-  store_row_f32<D>(Rf, (long long)g * Nf + i, x);
-  if (rinv) rinv[(long long)g * Nf + i] = 1.0 / (row_norm_f64<D>(x) + kEps);
-  if (wt && m == 0) wt[(long long)g * nf_tok + tl] = w ? w[(long long)g * w_stride_g + tok] : 1.0f;
-}
+constexpr int kPrepRows = 1024;  // rows per CTA of k_prep_rows (256 threads x 4)
 
-// Etot[g] = sum_i w_i ||r_i||^2 in fp64, fixed order (thread-strided partials + smem tree):
-// the constant of Eq. 4 that turns sum of scores into the distortion J.
+struct PrepParams {
+  RowSrc src;
+  const float *w;              // [.][T] per-token weights or nullptr (uniform)
+  long long w_stride_g;
+  const long long *fit_tokens; // [G][nf_tok] or nullptr
+  long long nf_tok;
+  float *Rf;                   // [G][Nf][D] compact fp32 rows (out; may alias src.rows)
+  double *rinv;                // [G][Nf] 1/(||r||+eps)  (Eq. 6 with the safeguard of PAPER.md:178)
+  float *wt;                   // [G][nf_tok] compact per-fit-token weights (out)
+  double *epart;               // [G][gridDim.x] partial sums of w_i ||r_i||^2 (Eq. 4's constant), or nullptr
+  __nv_bfloat16 *ahi, *alo;    // [G][Nf][16] bf16 operand planes of the tensor-core filter (D == 16), or nullptr
+  float *rnorm;                // [G][Nf] fp32 upper bound of ||r_i||, or nullptr
+};
+
+// One pass over the fit rows of every group: gather (through fit_tokens) into the compact fp32
+// buffer, per-row constants, operand planes A_hi = bf16(r), A_lo = bf16(r - A_hi), and the CTA's
+// partial of the weighted energy (fixed order: 4 rows per thread in row order, then a tree).
+// grid = (ceil(Nf / kPrepRows), G), block = 256.
 template <int D>
-__global__ void __launch_bounds__(1024) k_energy(const float *__restrict__ Rf, const float *__restrict__ wt,
-                                                 long long Nf, int M, double *__restrict__ Etot) {
-  __shared__ double sh[1024];
-  const int g = blockIdx.x;
-  double acc = 0.0;
-  for (long long i = threadIdx.x; i < Nf; i += 1024) {
+__global__ void __launch_bounds__(256) k_prep_rows(PrepParams p) {
+  __shared__ double sh[256];
+  const int g = blockIdx.y;
+  const long long Nf = p.nf_tok * p.src.M;
+  double e = 0.0;
+#pragma unroll
+  for (int u = 0; u < kPrepRows / 256; ++u) {
+    const long long i = (long long)blockIdx.x * kPrepRows + u * 256 + threadIdx.x;
+    if (i >= Nf) continue;
+    const long long tl = i / p.src.M;
+    const int m = (int)(i - tl * p.src.M);
+    const long long tok = p.fit_tokens ? p.fit_tokens[(long long)g * p.nf_tok + tl] : tl;
     float x[D];
-    load_row_f32<D>(Rf, (long long)g * Nf + i, x);
+    if (p.src.rows) load_row_f32<D>(p.src.rows, (long long)g * p.src.rows_per_group + tok * p.src.M + m, x);
+    else load_row_kv<D>(p.src.kv, p.src.dtype, (long long)g * p.src.stride_g + tok * p.src.stride_t + (long long)m * D, x);
+    const long long gi = (long long)g * Nf + i;
+    store_row_f32<D>(p.Rf, gi, x);
+    const float wv = p.w ? p.w[(long long)g * p.w_stride_g + tok] : 1.0f;
+    if (m == 0) p.wt[(long long)g * p.nf_tok + tl] = wv;
     double n2 = 0.0;
 #pragma unroll
-    for (int j = 0; j < D; ++j) n2 += (double)x[j] * (double)x[j];
-    acc += (double)wt[(long long)g * (Nf / M) + i / M] * n2;
+    for (int j = 0; j < D; ++j) n2 = __dadd_rn(n2, __dmul_rn((double)x[j], (double)x[j]));
+    const double n = sqrt(n2);
+    p.rinv[gi] = 1.0 / (n + kEps);
+    e += (double)wv * n2;
+    if (p.rnorm) p.rnorm[gi] = (float)n * 1.000001f;
+    if (D == 16 && p.ahi) {
+      uint32_t h[8], l[8];
+#pragma unroll
+      for (int j = 0; j < 16; j += 2) {
+        const __nv_bfloat16 h0 = __float2bfloat16_rn(x[j]), h1 = __float2bfloat16_rn(x[j + 1]);
+        const __nv_bfloat16 l0 = __float2bfloat16_rn(__fsub_rn(x[j], __bfloat162float(h0)));
+        const __nv_bfloat16 l1 = __float2bfloat16_rn(__fsub_rn(x[j + 1], __bfloat162float(h1)));
+        h[j / 2] = (uint32_t)__bfloat16_as_ushort(h0) | ((uint32_t)__bfloat16_as_ushort(h1) << 16);
+        l[j / 2] = (uint32_t)__bfloat16_as_ushort(l0) | ((uint32_t)__bfloat16_as_ushort(l1) << 16);
+      }
+      uint4 *ph = reinterpret_cast<uint4 *>(p.ahi + gi * 16);
+      ph[0] = make_uint4(h[0], h[1], h[2], h[3]);
+      ph[1] = make_uint4(h[4], h[5], h[6], h[7]);
+      if (p.alo) {
+        uint4 *pl = reinterpret_cast<uint4 *>(p.alo + gi * 16);
+        pl[0] = make_uint4(l[0], l[1], l[2], l[3]);
+        pl[1] = make_uint4(l[4], l[5], l[6], l[7]);
+      }
+    }
   }
-  sh[threadIdx.x] = acc;
+  if (!p.epart) return;
+  sh[threadIdx.x] = e;
   __syncthreads();
-  for (int s = 512; s > 0; s >>= 1) {
+  for (int s = 128; s > 0; s >>= 1) {
     if ((int)threadIdx.x < s) sh[threadIdx.x] += sh[threadIdx.x + s];
     __syncthreads();
   }
-  if (threadIdx.x == 0) Etot[g] = sh[0];
+  if (threadIdx.x == 0) p.epart[(long long)g * gridDim.x + blockIdx.x] = sh[0];
 }
 
 // Seeded initial rows.  Candidate n of group g is splitmix64(seed_g)[n] mod Nf; a candidate is
 // accepted iff its row is non-zero and its value did not occur earlier in the stream; the first
 // K accepted are the initial rows (same rule as "skip if already chosen or zero norm").
-// One block of 512 threads per group evaluates 512 candidates per batch.
+// One block of 512 threads per group evaluates 512 candidates per batch.  When shapes != nullptr
+// the block goes on to Alg. 1 l.1: s_k = fl32(r / ||r||) (fp64 division) for the chosen rows, g_k = 0
+// (set by the first gain update), and, when bimg != nullptr (D == 16), the projection-mode operand
+// images of all 256 rows for the first scoring pass.
 template <int D>
 __global__ void __launch_bounds__(512) k_init_ids(const float *__restrict__ Rf, long long Nf, int K, int G, int stage,
-                                                  uint64_t seed, long long *__restrict__ ids, DevStats *__restrict__ st) {
+                                                  uint64_t seed, long long *__restrict__ ids, DevStats *__restrict__ st,
+                                                  float *__restrict__ shapes, float *__restrict__ gains,
+                                                  long long cb_stride_g, uint8_t *__restrict__ bimg) {
   __shared__ long long cand[512];
   __shared__ int ok[512];
   __shared__ int scan[512];
@@ -110,21 +146,24 @@ __global__ void __launch_bounds__(512) k_init_ids(const float *__restrict__ Rf, 
   } else {
     for (int k = t; k < K; k += 512) ids[(long long)g * K + k] = chosen[k];
   }
-}
-
-// s_k = fl32(r / ||r||) in fp64 for the K chosen rows; g_k = 0 (set by the first gain update).
-template <int D>
-__global__ void k_init_shapes(const float *__restrict__ Rf, long long Nf, int K, const long long *__restrict__ ids,
-                              float *__restrict__ shapes, float *__restrict__ gains, long long cb_stride_g) {
-  const int g = blockIdx.x;
-  for (int k = threadIdx.x; k < K; k += blockDim.x) {
-    float x[D];
-    load_row_f32<D>(Rf, (long long)g * Nf + ids[(long long)g * K + k], x);
-    const double n = row_norm_f64<D>(x);
-    float *s = shapes + (long long)g * cb_stride_g * D + (long long)k * D;
+  if (!shapes) return;
+  for (int k = t; k < GSRQ_MAX_K; k += 512) {
+    float sv[D];
 #pragma unroll
-    for (int j = 0; j < D; ++j) s[j] = (n > 0.0) ? (float)((double)x[j] / n) : 0.0f;
-    gains[(long long)g * cb_stride_g + k] = 0.0f;
+    for (int j = 0; j < D; ++j) sv[j] = 0.0f;
+    if (k < K) {
+      float x[D];
+      load_row_f32<D>(Rf, (long long)g * Nf + (k < n_chosen ? chosen[k] : 0), x);
+      const double n = row_norm_f64<D>(x);
+#pragma unroll
+      for (int j = 0; j < D; ++j) sv[j] = (n > 0.0) ? (float)((double)x[j] / n) : 0.0f;
+      store_row_f32<D>(shapes + (long long)g * cb_stride_g * D, k, sv);
+      gains[(long long)g * cb_stride_g + k] = 0.0f;
+    }
+    if (D == 16 && bimg) {
+#pragma unroll
+      for (int j = 0; j < D; ++j) write_bimg_elem(bimg + (size_t)g * 3 * kBImgBytesU, k, j, 1.0f, sv[j], 1, k >= K);
+    }
   }
 }
 

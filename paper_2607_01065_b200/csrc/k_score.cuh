@@ -108,7 +108,7 @@ __global__ void __launch_bounds__(256) k_encode(EncParams p) {
   float *e_sh = b_sh + p.K;
   int *gmax_bits = reinterpret_cast<int *>(e_sh + 2);
   const int g = blockIdx.y;
-  if (p.st && p.st[g].done) return;
+  if (group_done(p.st, g, p.slot)) return;
   const long long i0 = (long long)blockIdx.x * (256 * RPT) + threadIdx.x;
   float x[RPT][D];
   bool live[RPT];

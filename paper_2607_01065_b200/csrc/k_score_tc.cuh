@@ -9,19 +9,21 @@
 //     D += A_1  . B_bias^T          A_1 = [1 1 1 0 ...],      B_bias[k] = -[b1 b2 b3 0 ...], b1+b2+b3 = fl32(g_k^2)
 // so D[i][k] ~= 2 g_k r_i.s_k - g_k^2 (Eq. 5) with a bounded error E_i, and the
 // epilogue is a pure max / arg-max: the N x K score matrix never leaves the SM.  Rows whose
-// top-2 gap is <= 2 E_i go to the exact fp64 re-score (k_encode_refine).
+// top-2 gap is <= 2 E_i (about 1e-4 of them) are re-scored on the spot, by their epilogue warp,
+// in fp64 with the definition's operation order (refine_row_warp).
 //
 // Warp roles (192 threads, one CTA per SM, persistent over the tiles of one group):
 //   warp 0      TMA producer: B operand images once (cp.async.bulk), A tiles through a ring
 //               (cp.async.bulk.tensor, SWIZZLE_32B)
 //   warp 1      TMEM allocation + tcgen05.mma issue (one elected lane), tcgen05.commit
-//   warps 2-5   epilogue: tcgen05.ld of the accumulator (thread = row), hierarchical max,
-//               arg-max, near-tie flagging, code write.  Two 256-column accumulators are
-//               double-buffered so tile i's epilogue overlaps tile i+1's MMAs.
+//   warps 2-9   epilogue (two warpgroups, one per 256-column accumulator): tcgen05.ld of the
+//               accumulator (thread = row), hierarchical max, arg-max, near-tie refine, code
+//               write.  Tile i's epilogue overlaps tile i+1's MMAs.
 #pragma once
 #include <cuda.h>
 
 #include "gsrq_common.cuh"
+#include "k_update.cuh"
 
 namespace gsrq {
 namespace tc {
@@ -39,16 +41,21 @@ constexpr uint32_t kSmemTotal = kSmemBar + 256 + 1024;           // + alignment 
 
 struct ScoreTcParams {
   const uint8_t *bimg;   // [G][3][8192]: B_hi, B_lo, B_bias operand images (SWIZZLE_32B K-major)
-  const float *efac;     // [G][2]: E_i = efac[0] * ||r_i|| + efac[1]
+  const int *gmax;       // bit pattern of max_k g_k of group g at gmax[g * gmax_stride] (mode 0)
+  long long gmax_stride;
   const float *rnorm;    // [G][N] fp32 row norms (upper bounds)
+  const float *rows;     // [G][N][16] fp32 rows (exact path)
+  const float *shapes;   // stage slice; codeword k of group g at shapes + (g*cb_stride_g + k)*16
+  const float *gains;
+  long long cb_stride_g;
   uint8_t *idx;          // [G][N]
   long long N;           // rows per group
   int n_tiles;           // tiles per group
   int n_planes;          // 1: A_hi only; 2: A_hi + A_lo
-  uint32_t *list;
-  unsigned int *list_cnt;
+  int K;
+  int mode;              // 0: Eq. 5 score; 1: plain projection
   DevStats *st;
-  int slot;
+  int slot;              // pass index t
   float *dbg;            // optional [G][N][256] raw scores (tests only)
 };
 
@@ -133,11 +140,6 @@ __device__ __forceinline__ uint64_t make_desc_sw32(uint32_t saddr) {
 // both K-major (bits 15, 16 = 0), N>>3 at bits 17-22, M>>4 at bits 24-28.
 constexpr uint32_t kIdesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(kN >> 3) << 17) | ((uint32_t)(kTileM >> 4) << 24);
 
-// byte offset of element (row, col) of a [rows][16] bf16 tile in the SWIZZLE_32B layout
-__host__ __device__ __forceinline__ uint32_t sw32_off(int row, int col) {
-  return (uint32_t)row * 32u + ((((uint32_t)col >> 3) ^ (((uint32_t)row >> 2) & 1u)) << 4) + ((uint32_t)col & 7u) * 2u;
-}
-
 __device__ __forceinline__ float max16(const uint32_t *v) {
   float m0 = fmaxf(fmaxf(__uint_as_float(v[0]), __uint_as_float(v[1])), __uint_as_float(v[2]));
   float m1 = fmaxf(fmaxf(__uint_as_float(v[3]), __uint_as_float(v[4])), __uint_as_float(v[5]));
@@ -197,12 +199,50 @@ __device__ __forceinline__ void top2_packed16(const float (&v)[16], float &best,
   idx = 15 - (int)(__float_as_uint(best) & 15u);
 }
 
+// Exact path for one row, run by a whole warp: fp64, dot product summed in element order without
+// FMA contraction, score = (2 g)(r.s) - g g -- the definition's own operation order; lowest k wins ties.
+// Only the columns of the 16-column groups in `gmask` are candidates: a column whose filter score is
+// below best - 2E cannot be the exact arg-max, and every other column lies in a group whose maximum
+// is >= best - 2E.  Two groups (one per half-warp) are scored per round.
+__device__ __noinline__ int refine_row_warp(const float *__restrict__ x_row, const float *__restrict__ sh,
+                                            const float *__restrict__ ga, int K, int mode, int lane, uint32_t gmask) {
+  float x[kD];
+  load_row_f32<kD>(x_row, 0, x);
+  double best = -INFINITY;
+  int bi = 0x7fffffff;
+  while (gmask) {
+    const int c0 = __ffs(gmask) - 1;
+    gmask &= gmask - 1;
+    int c1 = -1;
+    if (gmask) { c1 = __ffs(gmask) - 1; gmask &= gmask - 1; }
+    const int c = (lane < 16) ? c0 : c1;
+    const int kk = 16 * c + (lane & 15);
+    if (c >= 0 && kk < K) {
+      double dot = 0.0;
+#pragma unroll
+      for (int j = 0; j < kD; ++j) dot = __dadd_rn(dot, __dmul_rn((double)x[j], (double)sh[kk * kD + j]));
+      double sc = dot;
+      if (mode == 0) {
+        const double gk = (double)ga[kk];
+        sc = __dsub_rn(__dmul_rn(__dmul_rn(2.0, gk), dot), __dmul_rn(gk, gk));
+      }
+      if (sc > best || (sc == best && kk < bi)) { best = sc; bi = kk; }
+    }
+  }
+  for (int off = 16; off; off >>= 1) {
+    const double ob = __shfl_xor_sync(0xffffffffu, best, off);
+    const int oi = __shfl_xor_sync(0xffffffffu, bi, off);
+    if (ob > best || (ob == best && oi < bi)) { best = ob; bi = oi; }
+  }
+  return (bi == 0x7fffffff) ? 0 : bi;
+}
+
 template <bool DBG>
 __global__ void __launch_bounds__(kThreads, 1)
 k_score_tc(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CUtensorMap tm_lo, ScoreTcParams p) {
   extern __shared__ uint8_t smem_raw[];
   const int g = blockIdx.y;
-  if (p.st && p.st[g].done) return;
+  if (group_done(p.st, g, p.slot)) return;
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
   uint8_t *sgen = smem_raw + (sbase - smem_u32(smem_raw));
   const uint32_t bar0 = sbase + kSmemBar;
@@ -274,8 +314,13 @@ k_score_tc(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CU
     // so that two tiles are in flight per SM sub-partition.  Thread = row (TMEM lane).
     const int q = warp & 3;        // TMEM lane quarter this warp may access
     const int wg = (warp - 2) >> 2;
-    const float e1 = p.efac[2 * g], e0 = p.efac[2 * g + 1];
-    unsigned int n_changed = 0;
+    // E_i = e1 ||r_i|| + e0,  e1 = rho 2^-17 (2 g_max),  e0 = 2^-18 g_max^2
+    const float gm = (p.mode == 0) ? __int_as_float(p.gmax[(long long)g * p.gmax_stride]) : 1.0f;
+    const float e1 = (p.n_planes == 1 ? 2.0f : 4.5f) * 7.62939453125e-6f * 2.0f * gm;
+    const float e0 = (p.mode == 0) ? 3.814697265625e-6f * gm * gm : 0.0f;
+    const float *sh_g = p.shapes + (long long)g * p.cb_stride_g * kD;
+    const float *ga_g = p.gains + (long long)g * p.cb_stride_g;
+    unsigned int n_changed = 0, n_refined = 0;
     for (int it = wg; it < n_my; it += 2) {
       const int buf = wg, bph = (it >> 1) & 1;
       const int tile = blockIdx.x + it * gridDim.x;
@@ -326,22 +371,34 @@ k_score_tc(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CU
       top2_packed16(gmA, bestA, secA, gi);
       top2_packed16(gmB, bestB, secB, ji);
       const float best = fminf(bestA, bestB), second = fmaxf(secA, secB);
-      if (row < p.N) {
-        const float E = fmaf(e1, rn, e0);
-        if (best - second <= 2.0f * E) {
-          const unsigned int pos = atomicAdd(p.list_cnt, 1u);
-          p.list[pos] = (uint32_t)gr;
-        } else {
-          const uint8_t k = (uint8_t)(gi * 16 + ji);
-          n_changed += (k_old != k);
-          p.idx[gr] = k;
+      int k_new = gi * 16 + ji;
+      const float E2 = 2.0f * fmaf(e1, rn, e0);
+      const bool flag = (row < p.N) && (best - second <= E2);
+      unsigned int m = __ballot_sync(0xffffffffu, flag);
+      n_refined += __popc(m);
+      if (m) {  // ambiguous rows: the exact path decides among the groups within 2E of the best
+        uint32_t gmask = 0;
+#pragma unroll
+        for (int c = 0; c < 16; ++c) gmask |= (gmA[c] >= best - E2) ? (1u << c) : 0u;
+        while (m) {
+          const int l = __ffs(m) - 1;
+          m &= m - 1;
+          const long long gr_l = (long long)g * p.N + (long long)tile * kTileM + q * 32 + l;
+          const int k = refine_row_warp(p.rows + gr_l * kD, sh_g, ga_g, p.K, p.mode, lane, __shfl_sync(0xffffffffu, gmask, l));
+          if (lane == l) k_new = k;
         }
+      }
+      if (row < p.N) {
+        n_changed += (k_old != (uint8_t)k_new);
+        p.idx[gr] = (uint8_t)k_new;
       }
     }
     if (p.st) {
       for (int off = 16; off; off >>= 1) n_changed += __shfl_xor_sync(0xffffffffu, n_changed, off);
       if (lane == 0 && n_changed)
         atomicAdd(reinterpret_cast<unsigned long long *>(&p.st[g].changed[p.slot]), (unsigned long long)n_changed);
+      if (lane == 0 && n_refined)
+        atomicAdd(reinterpret_cast<unsigned long long *>(&p.st[g].refined), (unsigned long long)n_refined);
     }
   }
   tc_fence_before();
@@ -349,82 +406,23 @@ k_score_tc(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CU
   if (warp == 1) tmem_dealloc(tmem_base, 512);
 }
 
-// Operand images + error factors of (group g, one stage) for k_score_tc.  grid = G, block = 256.
-//   mode 0: c' = fl32(2 fl32(g_k s_kj)), b = fl32(g_k^2);   mode 1 (projection): c' = 2 s_kj, b = 0.
-//   rows k >= K get b = 3e38 so that they can never win the arg-max.
-// efac: E = e1 ||r|| + e0,  e1 = rho * 2 g_max,  e0 = 2^-20 g_max^2.
+// Operand images and max gain of (group g, one stage) for a stand-alone scoring pass (gsrq_assign;
+// inside a fit the update kernel writes them).  grid = G, block = 256 (thread = codeword row).
 __global__ void __launch_bounds__(256) k_bimg(const float *__restrict__ shapes, const float *__restrict__ gains,
-                                              long long cb_stride_g, int K, int mode, int n_planes,
-                                              uint8_t *__restrict__ bimg, float *__restrict__ efac,
-                                              const DevStats *__restrict__ st) {
+                                              long long cb_stride_g, int K, int mode, uint8_t *__restrict__ bimg,
+                                              int *__restrict__ gmax) {
   __shared__ int gmax_bits;
   const int g = blockIdx.x, k = threadIdx.x;
-  if (st && st[g].done) return;
   if (k == 0) gmax_bits = 0;
   __syncthreads();
-  uint8_t *img = bimg + (size_t)g * 3 * kBImgBytes;
-  float gk = 0.f;
-  if (k < K) gk = (mode == 0) ? gains[(long long)g * cb_stride_g + k] : 1.0f;
+  const float gk = (k < K && mode == 0) ? gains[(long long)g * cb_stride_g + k] : 1.0f;
   const float *s = shapes + ((long long)g * cb_stride_g + k) * kD;
 #pragma unroll
-  for (int j = 0; j < kD; ++j) {
-    float c = 0.f;
-    if (k < K) c = (mode == 0) ? 2.0f * __fmul_rn(gk, s[j]) : 2.0f * s[j];
-    const __nv_bfloat16 hi = __float2bfloat16_rn(c);
-    const __nv_bfloat16 lo = __float2bfloat16_rn(__fsub_rn(c, __bfloat162float(hi)));
-    *reinterpret_cast<__nv_bfloat16 *>(img + sw32_off(k, j)) = hi;
-    *reinterpret_cast<__nv_bfloat16 *>(img + kBImgBytes + sw32_off(k, j)) = lo;
-  }
-  float b = (k < K) ? ((mode == 0) ? __fmul_rn(gk, gk) : 0.0f) : 3.0e38f;
-  const __nv_bfloat16 b1 = __float2bfloat16_rn(b);
-  const float r1 = __fsub_rn(b, __bfloat162float(b1));
-  const __nv_bfloat16 b2 = __float2bfloat16_rn(r1);
-  const __nv_bfloat16 b3 = __float2bfloat16_rn(__fsub_rn(r1, __bfloat162float(b2)));
-#pragma unroll
-  for (int j = 0; j < kD; ++j) {
-    __nv_bfloat16 v = __float2bfloat16_rn(0.f);
-    if (j == 0) v = __hneg(b1);
-    if (j == 1) v = __hneg(b2);
-    if (j == 2) v = __hneg(b3);
-    *reinterpret_cast<__nv_bfloat16 *>(img + 2 * kBImgBytes + sw32_off(k, j)) = v;
-  }
+  for (int j = 0; j < kD; ++j)
+    write_bimg_elem(bimg + (size_t)g * 3 * kBImgBytes, k, j, gk, (k < K) ? s[j] : 0.0f, mode, k >= K);
   if (k < K && mode == 0) atomicMax(&gmax_bits, __float_as_int(fmaxf(gk, 0.f)));
   __syncthreads();
-  if (k == 0) {
-    const float gm = (mode == 0) ? __int_as_float(gmax_bits) : 1.0f;
-    const float rho = (n_planes == 1 ? 2.0f : 4.5f) * 7.62939453125e-6f;  // x 2^-17 (incl. 2^-19 index packing)
-    efac[2 * g] = rho * 2.0f * gm;
-    efac[2 * g + 1] = (mode == 0) ? 3.814697265625e-6f * gm * gm : 0.0f;  // 2^-18 g_max^2
-  }
-}
-
-// fp32 rows -> bf16 operand planes (A_hi = bf16(r), A_lo = bf16(r - A_hi)), row norms, 1/(||r||+eps).
-__global__ void k_planes(const float *__restrict__ Rf, long long n_rows, __nv_bfloat16 *__restrict__ ahi,
-                         __nv_bfloat16 *__restrict__ alo, float *__restrict__ rnorm, double *__restrict__ rinv) {
-  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n_rows) return;
-  float x[kD];
-  load_row_f32<kD>(Rf, i, x);
-  uint32_t h[8], l[8];
-#pragma unroll
-  for (int j = 0; j < kD; j += 2) {
-    const __nv_bfloat16 h0 = __float2bfloat16_rn(x[j]), h1 = __float2bfloat16_rn(x[j + 1]);
-    const __nv_bfloat16 l0 = __float2bfloat16_rn(__fsub_rn(x[j], __bfloat162float(h0)));
-    const __nv_bfloat16 l1 = __float2bfloat16_rn(__fsub_rn(x[j + 1], __bfloat162float(h1)));
-    h[j / 2] = (uint32_t)__bfloat16_as_ushort(h0) | ((uint32_t)__bfloat16_as_ushort(h1) << 16);
-    l[j / 2] = (uint32_t)__bfloat16_as_ushort(l0) | ((uint32_t)__bfloat16_as_ushort(l1) << 16);
-  }
-  uint4 *ph = reinterpret_cast<uint4 *>(ahi + i * kD);
-  ph[0] = make_uint4(h[0], h[1], h[2], h[3]);
-  ph[1] = make_uint4(h[4], h[5], h[6], h[7]);
-  if (alo) {
-    uint4 *pl = reinterpret_cast<uint4 *>(alo + i * kD);
-    pl[0] = make_uint4(l[0], l[1], l[2], l[3]);
-    pl[1] = make_uint4(l[4], l[5], l[6], l[7]);
-  }
-  const double n = row_norm_f64<kD>(x);
-  rnorm[i] = (float)n * 1.000001f;
-  if (rinv) rinv[i] = 1.0 / (n + kEps);
+  if (k == 0) gmax[g] = gmax_bits;
 }
 
 }  // namespace tc

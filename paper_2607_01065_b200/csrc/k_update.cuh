@@ -1,0 +1,311 @@
+// k_update.cuh -- deterministic segmented weighted centroid reduction (sums of Eq. 6-8),
+// codeword renormalisation (Eq. 7, Eq. 8, safeguards of PAPER.md:178) and the tensor-core
+// operand images of the updated codewords, in ONE "cluster-owner" kernel.
+//
+// Per cluster k the update needs  cnt_k, W_k = sum w_i, A_k = sum w_i r_i, B_k = sum w_i y_i,
+// y_i = r_i/(||r_i||+eps).  A CTA owns kCPC consecutive clusters of one group: it scans the
+// group's assignment bytes in passes, compacts the rows of its clusters into an ascending list
+// (a stable counting sort: integer work only), stages those rows in shared memory with one
+// wave of independent loads, and one warp per cluster adds them up in fp64 in ascending row
+// order -- the definition's own order, so A_k, W_k are bit-identical to a sequential fp64 loop
+// and B_k differs only by the rounding of w_i/(||r_i||+eps).  No
+// floating-point atomics, no cross-CTA partials: bit-identical run to run.  The same CTA then applies
+// Eq. 7 / Eq. 8 to its clusters, stores s_k, g_k, the per-cluster term of J (Eq. 4 summed over
+// the cluster), the cluster's rows of the B operand images for the next scoring pass, and
+// max g (integer atomicMax on the bit pattern: order-independent).
+#pragma once
+#include "gsrq_common.cuh"
+
+namespace gsrq {
+
+constexpr int kCPC = 16;            // clusters per CTA = warps per CTA (warp c sums cluster k0 + c)
+constexpr int kUpdThreads = 512;
+constexpr int kPassRows = 16384;    // rows scanned per pass (32 per thread)
+constexpr int kRoundRows = 1024;    // rows staged in shared memory per round
+
+struct UpdParams {
+  const float *Rf;        // [G][Nf][D] fp32 rows
+  const double *rinv;     // [G][Nf]   1/(||r||+eps)
+  const float *wt;        // [G][Nf/M] per-fit-token weights
+  const uint8_t *idx;     // [G][Nf]
+  long long Nf;
+  int M, K;
+  float *shapes;          // stage slice: shapes + (g*cb_stride_g + k)*D
+  float *gains;
+  long long cb_stride_g;
+  DevStats *st;           // may be nullptr (step-wise gsrq_update)
+  double *term;           // [G][term_stride][256] or nullptr
+  int term_stride;
+  int lloyd;              // 0: gains only (Alg. 1 l.2); 1: shapes + gains
+  int t;                  // pass index (slot of changed[], n_empty[], gmax_bits[t+1])
+  uint8_t *bimg;          // [G][3][8192] operand images (D == 16 only) or nullptr
+};
+
+// byte offset of element (row, col) of a [rows][16] bf16 tile in the SWIZZLE_32B K-major layout
+__host__ __device__ __forceinline__ uint32_t sw32_off(int row, int col) {
+  return (uint32_t)row * 32u + ((((uint32_t)col >> 3) ^ (((uint32_t)row >> 2) & 1u)) << 4) + ((uint32_t)col & 7u) * 2u;
+}
+constexpr uint32_t kBImgBytesU = 256 * 16 * 2;
+
+// Write row k of the three operand images (B_hi, B_lo, B_bias) for codeword (gk, s[0..16)):
+//   mode 0: c' = fl32(2 fl32(g_k s_kj)), b = fl32(g_k^2);   mode 1 (projection): c' = 2 s_kj, b = 0;
+//   dead rows (k >= K) get c' = 0, b = 3e38 so that they can never win the arg-max.
+__device__ __forceinline__ void write_bimg_elem(uint8_t *img, int k, int j, float gk, float sj, int mode, bool dead) {
+  float c = 0.f;
+  if (!dead) c = (mode == 0) ? 2.0f * __fmul_rn(gk, sj) : 2.0f * sj;
+  const __nv_bfloat16 hi = __float2bfloat16_rn(c);
+  const __nv_bfloat16 lo = __float2bfloat16_rn(__fsub_rn(c, __bfloat162float(hi)));
+  *reinterpret_cast<__nv_bfloat16 *>(img + sw32_off(k, j)) = hi;
+  *reinterpret_cast<__nv_bfloat16 *>(img + kBImgBytesU + sw32_off(k, j)) = lo;
+  const float b = dead ? 3.0e38f : ((mode == 0) ? __fmul_rn(gk, gk) : 0.0f);
+  const __nv_bfloat16 b1 = __float2bfloat16_rn(b);
+  const float r1 = __fsub_rn(b, __bfloat162float(b1));
+  const __nv_bfloat16 b2 = __float2bfloat16_rn(r1);
+  const __nv_bfloat16 b3 = __float2bfloat16_rn(__fsub_rn(r1, __bfloat162float(b2)));
+  __nv_bfloat16 v = __float2bfloat16_rn(0.f);
+  if (j == 0) v = __hneg(b1);
+  if (j == 1) v = __hneg(b2);
+  if (j == 2) v = __hneg(b3);
+  *reinterpret_cast<__nv_bfloat16 *>(img + 2 * kBImgBytesU + sw32_off(k, j)) = v;
+}
+
+// 4 assignment bytes of rows [r, r+4) of one group; rows >= Nf read as `miss`.
+__device__ __forceinline__ uint32_t load_idx_word(const uint8_t *ig, long long r, long long Nf, bool aligned, uint32_t miss) {
+  if (aligned && r + 4 <= Nf) return *reinterpret_cast<const uint32_t *>(ig + r);
+  uint32_t w = 0;
+#pragma unroll
+  for (int b = 0; b < 4; ++b) {
+    const uint32_t v = (r + b < Nf) ? (uint32_t)ig[r + b] : miss;
+    w |= v << (8 * b);
+  }
+  return w;
+}
+
+template <int D>
+constexpr size_t upd_smem_bytes() {
+  constexpr int P = 2 * D + 2;
+  return sizeof(double) * (kRoundRows + kCPC * P) + sizeof(float) * (kRoundRows * D + kRoundRows) +
+         sizeof(int) * (kCPC + 4) + sizeof(uint16_t) * (kPassRows + kCPC * kUpdThreads) + kPassRows;
+}
+
+// grid = (ceil(K / kCPC), G), block = kUpdThreads, dynamic smem = upd_smem_bytes<D>().
+template <int D>
+__global__ void __launch_bounds__(kUpdThreads) k_update(UpdParams p) {
+  extern __shared__ __align__(16) uint8_t upd_sm[];
+  constexpr int P = 2 * D + 2;
+  constexpr int Q = (2 * D + 31) / 32;
+  constexpr int LPR = D / 4;
+  static_assert(kCPC * 32 == kUpdThreads && kPassRows == 32 * kUpdThreads, "thread mapping");
+  double *cbbuf = reinterpret_cast<double *>(upd_sm);       // [kRoundRows]  w_i / (||r_i|| + eps)
+  double *fin = cbbuf + kRoundRows;                         // [kCPC][P]
+  float *xbuf = reinterpret_cast<float *>(fin + kCPC * P);  // [kRoundRows][D]
+  float *wbuf = xbuf + kRoundRows * D;                      // [kRoundRows]
+  int *ctot = reinterpret_cast<int *>(wbuf + kRoundRows);   // [kCPC] (+4 pad)
+  uint16_t *list = reinterpret_cast<uint16_t *>(ctot + kCPC + 4);  // [kPassRows] rows of the pass, by (cluster, row)
+  uint16_t *cntb = list + kPassRows;                        // [kCPC][kUpdThreads] per-thread counts -> prefixes
+  uint8_t *idxb = reinterpret_cast<uint8_t *>(cntb + kCPC * kUpdThreads);  // [kPassRows] assignment bytes of the pass
+
+  const int g = blockIdx.y, k0 = blockIdx.x * kCPC;
+  if (group_done(p.st, g, p.t)) return;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const uint8_t *ig = p.idx + (long long)g * p.Nf;
+  const bool aligned = (reinterpret_cast<uintptr_t>(ig) & 3) == 0;
+  const uint32_t pat = (uint32_t)(k0 & 0xF0) * 0x01010101u;
+  const uint32_t miss = (uint32_t)((k0 ^ 0x80) & 0xFF);  // a byte outside [k0, k0 + 16)
+  const float *rows = p.Rf + (long long)g * p.Nf * D;
+  const double *ri = p.rinv + (long long)g * p.Nf;
+  const float *wg = p.wt + (long long)g * (p.Nf / p.M);
+  const unsigned int Mu = (unsigned int)p.M;
+
+  double s[Q];  // warp c, lane e: element e (+32q) of [A | B] of cluster k0 + c
+#pragma unroll
+  for (int q = 0; q < Q; ++q) s[q] = 0.0;
+  double Wk = 0.0;
+  long long cntk = 0;
+  for (long long pb = 0; pb < p.Nf; pb += kPassRows) {
+    // ---- walk 1: my 32 assignment bytes -> hit mask, per-(cluster, thread) counts ----
+    uint32_t m = 0;
+    const long long r0 = pb + 32 * tid;
+#pragma unroll
+    for (int wi = 0; wi < 8; ++wi) {
+      const uint32_t w = (r0 + 4 * wi < p.Nf) ? load_idx_word(ig, r0 + 4 * wi, p.Nf, aligned, miss) : miss * 0x01010101u;
+      reinterpret_cast<uint32_t *>(idxb)[8 * tid + wi] = w;
+      uint32_t h = __vcmpeq4(w & 0xF0F0F0F0u, pat) & 0x08040201u;  // bits 0, 9, 18, 27 <- bytes 0..3 hit
+      h = (h | (h >> 8) | (h >> 16) | (h >> 24)) & 0xFu;
+      m |= h << (4 * wi);
+    }
+#pragma unroll
+    for (int c = 0; c < kCPC; ++c) cntb[c * kUpdThreads + tid] = 0;
+    for (uint32_t mm = m; mm; mm &= mm - 1) {
+      const int r = __ffs(mm) - 1;
+      const int c = idxb[32 * tid + r] & (kCPC - 1);
+      cntb[c * kUpdThreads + tid] += 1;
+    }
+    __syncthreads();
+    // ---- warp c: exclusive prefix of cluster c's counts over the 512 threads (integers) ----
+    {
+      uint16_t *row = cntb + warp * kUpdThreads + 16 * lane;
+      uint4 v0 = reinterpret_cast<uint4 *>(row)[0], v1 = reinterpret_cast<uint4 *>(row)[1];
+      uint32_t u[8] = {v0.x, v0.y, v0.z, v0.w, v1.x, v1.y, v1.z, v1.w};
+      int run = 0;
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {  // two 16-bit counts per word -> their exclusive prefixes
+        const int a = (int)(u[i] & 0xFFFFu), b = (int)(u[i] >> 16);
+        u[i] = (uint32_t)run | ((uint32_t)(run + a) << 16);
+        run += a + b;
+      }
+      int incl = run;
+#pragma unroll
+      for (int off = 1; off < 32; off <<= 1) {
+        const int v = __shfl_up_sync(0xffffffffu, incl, off);
+        if (lane >= off) incl += v;
+      }
+      const uint32_t base2 = (uint32_t)(incl - run) * 0x00010001u;
+#pragma unroll
+      for (int i = 0; i < 8; ++i) u[i] += base2;
+      reinterpret_cast<uint4 *>(row)[0] = make_uint4(u[0], u[1], u[2], u[3]);
+      reinterpret_cast<uint4 *>(row)[1] = make_uint4(u[4], u[5], u[6], u[7]);
+      if (lane == 31) ctot[warp] = incl;
+    }
+    __syncthreads();
+    // ---- walk 2: stable scatter of my hits, ordered by (cluster, row) ----
+    int cbase[kCPC + 1];
+    cbase[0] = 0;
+#pragma unroll
+    for (int c = 0; c < kCPC; ++c) cbase[c + 1] = cbase[c] + ctot[c];
+    const int total = cbase[kCPC];
+    for (uint32_t mm = m; mm; mm &= mm - 1) {
+      const int r = __ffs(mm) - 1;
+      const int c = idxb[32 * tid + r] & (kCPC - 1);
+      int base = 0;
+#pragma unroll
+      for (int c2 = 0; c2 < kCPC; ++c2) base = (c2 == c) ? cbase[c2] : base;
+      const int pos = base + (int)cntb[c * kUpdThreads + tid];
+      cntb[c * kUpdThreads + tid] += 1;
+      list[pos] = (uint16_t)(32 * tid + r);
+    }
+    int seg0 = 0, seg1 = 0;
+#pragma unroll
+    for (int c2 = 0; c2 < kCPC; ++c2)
+      if (c2 == warp) { seg0 = cbase[c2]; seg1 = cbase[c2 + 1]; }
+    __syncthreads();
+    for (int lo = 0; lo < total; lo += kRoundRows) {
+      const int n = min(kRoundRows, total - lo);
+      // ---- stage the round's rows: one wave of independent 16-byte loads ----
+      for (int it = tid; it < n * LPR; it += kUpdThreads) {
+        const int e = it / LPR, q = it - e * LPR;
+        const long long row = pb + list[lo + e];
+        const float4 v = *reinterpret_cast<const float4 *>(rows + row * D + 4 * q);
+        *reinterpret_cast<float4 *>(xbuf + e * D + 4 * q) = v;
+        if (q == 0) {
+          const float wv = wg[(unsigned int)row / Mu];
+          wbuf[e] = wv;
+          cbbuf[e] = (double)wv * ri[row];
+        }
+      }
+      __syncthreads();
+      // ---- warp c adds cluster c's rows of this round in list (= ascending row) order ----
+      const int a = max(seg0, lo), b = min(seg1, lo + n);
+      for (int pos = a; pos < b; ++pos) {
+        const int e = pos - lo;
+        const double wv = (double)wbuf[e], cb = cbbuf[e];
+        Wk += wv;
+#pragma unroll
+        for (int q = 0; q < Q; ++q) {
+          const int el = lane + 32 * q;
+          if (el < 2 * D) s[q] += ((el >= D) ? cb : wv) * (double)xbuf[e * D + (el % D)];
+        }
+      }
+      if (a < b) cntk += b - a;
+      __syncthreads();
+    }
+  }
+  {
+    double *out = fin + warp * P;
+#pragma unroll
+    for (int q = 0; q < Q; ++q) {
+      const int el = lane + 32 * q;
+      if (el < 2 * D) out[el] = s[q];
+    }
+    if (lane == 0) { out[2 * D] = Wk; out[2 * D + 1] = (double)cntk; }
+  }
+  __syncwarp();
+  // ---- Eq. 7 / Eq. 8 for my clusters: warp c, lane j (every lane evaluates the scalar chain) ----
+  if (warp < kCPC && k0 + warp < p.K) {
+    const int k = k0 + warp;
+    const double *f = fin + warp * P;
+    float *s = p.shapes + ((long long)g * p.cb_stride_g + k) * D;
+    float *gp = p.gains + (long long)g * p.cb_stride_g + k;
+    const double W = f[2 * D], cnt = f[2 * D + 1];
+    const float g_old_f = *gp;
+    const double g_old = (double)g_old_f;
+    float sn[D];
+#pragma unroll
+    for (int j = 0; j < D; ++j) sn[j] = s[j];
+    __syncwarp();  // every lane holds the old shape before any lane overwrites it
+    double proj_old = 0.0;
+#pragma unroll
+    for (int j = 0; j < D; ++j) proj_old += f[j] * (double)sn[j];
+    const double tk = 2.0 * g_old * proj_old - W * g_old * g_old;  // sum over the cluster of (2 g r.s - g^2) w
+    float g_new = g_old_f;
+    bool new_shape = false;
+    if (cnt != 0.0 && W > 0.0) {
+      if (p.lloyd) {
+        double bn2 = 0.0;
+#pragma unroll
+        for (int j = 0; j < D; ++j) bn2 = __dadd_rn(bn2, __dmul_rn(f[D + j], f[D + j]));
+        const double bn = sqrt(bn2);
+        if (bn / W > kDelta) {
+          new_shape = true;
+#pragma unroll
+          for (int j = 0; j < D; ++j) sn[j] = (float)(f[D + j] / bn);
+        }
+      }
+      double proj = 0.0;
+#pragma unroll
+      for (int j = 0; j < D; ++j) proj = __dadd_rn(proj, __dmul_rn(f[j], (double)sn[j]));
+      const double gk = proj / W;
+      g_new = (float)(gk > 0.0 ? gk : 0.0);
+    }
+    float mine = 0.f;
+#pragma unroll
+    for (int j = 0; j < D; ++j) if (j == lane) mine = sn[j];
+    if (lane < D && new_shape) s[lane] = mine;
+    if (D == 16 && p.bimg && lane < 16)
+      write_bimg_elem(p.bimg + (size_t)g * 3 * kBImgBytesU, k, lane, g_new, mine, 0, false);
+    if (lane == 0) {
+      *gp = g_new;
+      if (p.lloyd && p.term) p.term[((long long)g * p.term_stride + p.t) * 256 + k] = tk;
+      if (p.st) {
+        atomicMax(&p.st[g].gmax_bits[p.t + 1], __float_as_int(g_new));
+        if (cnt == 0.0) atomicAdd(&p.st[g].n_empty[p.t], 1);
+      }
+    }
+  }
+  // Alg. 1 l.15-16: assignments unchanged -> this was the last iteration of the group
+  if (p.st && p.lloyd && p.t > 1 && blockIdx.x == 0 && tid == 0 && p.st[g].changed[p.t] == 0) p.st[g].done_iter = p.t;
+}
+
+// Per-group wrap-up of a fit: iters_run, Etot = sum of the energy partials (fixed order) and
+// J_t = Etot - sum_k term_t[k] (Eq. 4 summed over rows; k in ascending order).  grid = G, block = 160.
+__global__ void __launch_bounds__(160) k_finish(DevStats *__restrict__ st, const double *__restrict__ term, int term_stride,
+                                                int K, const double *__restrict__ epart, int n_epart, int iters) {
+  __shared__ double etot;
+  const int g = blockIdx.x, t = threadIdx.x;
+  if (t == 0) {
+    double e = 0.0;
+    for (int c = 0; c < n_epart; ++c) e += epart[(long long)g * n_epart + c];
+    etot = e;
+    st[g].iters_run = st[g].done_iter ? st[g].done_iter : iters;
+  }
+  __syncthreads();
+  const int n = st[g].done_iter ? st[g].done_iter : iters;
+  if (t >= 1 && t <= n) {
+    const double *tm = term + ((long long)g * term_stride + t) * 256;
+    double sum = 0.0;
+    for (int k = 0; k < K; ++k) sum += tm[k];
+    st[g].J[t] = etot - sum;
+  }
+}
+
+}  // namespace gsrq
