@@ -37,7 +37,9 @@ constexpr uint32_t kSmemB = 0;                                   // 3 images
 constexpr uint32_t kSmemOnes = 3 * kBImgBytes;                   // 24576
 constexpr uint32_t kSmemA = kSmemOnes + kPlaneBytes;             // 28672, ring of kStages x 2 planes
 constexpr uint32_t kSmemBar = kSmemA + kStages * 2 * kPlaneBytes;  // 94208
-constexpr uint32_t kSmemTotal = kSmemBar + 256 + 1024;           // + alignment slack
+constexpr int kQCap = 512;                                       // deferred exact re-scores per CTA
+constexpr uint32_t kSmemQ = kSmemBar + 256;                      // kQCap x {row, gmask | k_old << 16}, then the counter
+constexpr uint32_t kSmemTotal = kSmemQ + kQCap * 8 + 16 + 1024;  // + alignment slack
 
 struct ScoreTcParams {
   const uint8_t *bimg;   // [G][3][8192]: B_hi, B_lo, B_bias operand images (SWIZZLE_32B K-major)
@@ -252,12 +254,15 @@ k_score_tc(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CU
   auto tmem_empty = [&](int b) { return bar0 + 8u * (2 * kStages + 2 + b); };
   const uint32_t b_full = bar0 + 8u * (2 * kStages + 4);
   volatile uint32_t *tmem_slot = reinterpret_cast<volatile uint32_t *>(sgen + kSmemBar + 8 * (2 * kStages + 5));
+  uint2 *queue = reinterpret_cast<uint2 *>(sgen + kSmemQ);
+  unsigned int *qcnt = reinterpret_cast<unsigned int *>(sgen + kSmemQ + kQCap * 8);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < kStages; ++s) { mbar_init(full_a(s), 1); mbar_init(empty_a(s), 1); }
     for (int b = 0; b < 2; ++b) { mbar_init(tmem_full(b), 1); mbar_init(tmem_empty(b), 4); }
     mbar_init(b_full, 1);
+    *qcnt = 0;
     fence_barrier_init();
   }
   // constant A_1 tile: columns 0,1,2 = 1.0 (bf16 0x3F80), rest 0
@@ -376,21 +381,45 @@ k_score_tc(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CU
       const bool flag = (row < p.N) && (best - second <= E2);
       unsigned int m = __ballot_sync(0xffffffffu, flag);
       n_refined += __popc(m);
-      if (m) {  // ambiguous rows: the exact path decides among the groups within 2E of the best
+      if (m) {  // ambiguous rows: the exact path decides among the groups within 2E of the best.
+        // They are queued and re-scored after the CTA's last tile by all epilogue warps at once, so that
+        // a re-score never stalls the accumulator pipeline; a full queue falls back to doing it here.
         uint32_t gmask = 0;
 #pragma unroll
         for (int c = 0; c < 16; ++c) gmask |= (gmA[c] >= best - E2) ? (1u << c) : 0u;
-        while (m) {
-          const int l = __ffs(m) - 1;
-          m &= m - 1;
+        bool queued = false;
+        if (flag) {
+          const unsigned int pos = atomicAdd(qcnt, 1u);
+          queued = pos < (unsigned int)kQCap;
+          if (queued) queue[pos] = make_uint2((uint32_t)row, gmask | ((uint32_t)k_old << 16));
+        }
+        unsigned int mo = __ballot_sync(0xffffffffu, flag && !queued);
+        while (mo) {
+          const int l = __ffs(mo) - 1;
+          mo &= mo - 1;
           const long long gr_l = (long long)g * p.N + (long long)tile * kTileM + q * 32 + l;
           const int k = refine_row_warp(p.rows + gr_l * kD, sh_g, ga_g, p.K, p.mode, lane, __shfl_sync(0xffffffffu, gmask, l));
           if (lane == l) k_new = k;
         }
+        if (queued) k_new = -1;  // written by the deferred pass
       }
-      if (row < p.N) {
+      if (row < p.N && k_new >= 0) {
         n_changed += (k_old != (uint8_t)k_new);
         p.idx[gr] = (uint8_t)k_new;
+      }
+    }
+    // deferred exact re-scores: entry e is taken by epilogue warp e % 8
+    asm volatile("bar.sync 1, 256;" ::: "memory");
+    {
+      const unsigned int nq = min(*qcnt, (unsigned int)kQCap);
+      for (unsigned int e = (unsigned int)(warp - 2); e < nq; e += 8) {
+        const uint2 en = queue[e];
+        const long long gr_e = (long long)g * p.N + en.x;
+        const int k = refine_row_warp(p.rows + gr_e * kD, sh_g, ga_g, p.K, p.mode, lane, en.y & 0xFFFFu);
+        if (lane == 0) {
+          n_changed += ((en.y >> 16) != (uint32_t)k);
+          p.idx[gr_e] = (uint8_t)k;
+        }
       }
     }
     if (p.st) {

@@ -84,7 +84,7 @@ __device__ __forceinline__ uint32_t load_idx_word(const uint8_t *ig, long long r
 template <int D>
 constexpr size_t upd_smem_bytes() {
   constexpr int P = 2 * D + 2;
-  return sizeof(double) * (kRoundRows + kCPC * P) + sizeof(float) * (kRoundRows * D + kRoundRows) +
+  return sizeof(double) * (2 * kRoundRows + kCPC * P) + sizeof(float) * (kRoundRows * D) +
          sizeof(int) * (kCPC + 4) + sizeof(uint16_t) * (kPassRows + kCPC * kUpdThreads) + kPassRows;
 }
 
@@ -96,11 +96,10 @@ __global__ void __launch_bounds__(kUpdThreads) k_update(UpdParams p) {
   constexpr int Q = (2 * D + 31) / 32;
   constexpr int LPR = D / 4;
   static_assert(kCPC * 32 == kUpdThreads && kPassRows == 32 * kUpdThreads, "thread mapping");
-  double *cbbuf = reinterpret_cast<double *>(upd_sm);       // [kRoundRows]  w_i / (||r_i|| + eps)
-  double *fin = cbbuf + kRoundRows;                         // [kCPC][P]
+  double *coef = reinterpret_cast<double *>(upd_sm);        // [kRoundRows][2]  { w_i, w_i / (||r_i|| + eps) }
+  double *fin = coef + 2 * kRoundRows;                      // [kCPC][P]
   float *xbuf = reinterpret_cast<float *>(fin + kCPC * P);  // [kRoundRows][D]
-  float *wbuf = xbuf + kRoundRows * D;                      // [kRoundRows]
-  int *ctot = reinterpret_cast<int *>(wbuf + kRoundRows);   // [kCPC] (+4 pad)
+  int *ctot = reinterpret_cast<int *>(xbuf + kRoundRows * D);  // [kCPC] (+4 pad)
   uint16_t *list = reinterpret_cast<uint16_t *>(ctot + kCPC + 4);  // [kPassRows] rows of the pass, by (cluster, row)
   uint16_t *cntb = list + kPassRows;                        // [kCPC][kUpdThreads] per-thread counts -> prefixes
   uint8_t *idxb = reinterpret_cast<uint8_t *>(cntb + kCPC * kUpdThreads);  // [kPassRows] assignment bytes of the pass
@@ -116,10 +115,16 @@ __global__ void __launch_bounds__(kUpdThreads) k_update(UpdParams p) {
   const double *ri = p.rinv + (long long)g * p.Nf;
   const float *wg = p.wt + (long long)g * (p.Nf / p.M);
   const unsigned int Mu = (unsigned int)p.M;
+  const int msh = ((Mu & (Mu - 1)) == 0) ? (31 - __clz((int)Mu)) : -1;  // M is a power of two: shift
 
   double s[Q];  // warp c, lane e: element e (+32q) of [A | B] of cluster k0 + c
+  int isB[Q], col[Q];
+  bool live[Q];
 #pragma unroll
-  for (int q = 0; q < Q; ++q) s[q] = 0.0;
+  for (int q = 0; q < Q; ++q) {
+    const int el = lane + 32 * q;
+    s[q] = 0.0; live[q] = el < 2 * D; isB[q] = (el >= D) ? 1 : 0; col[q] = el % D;
+  }
   double Wk = 0.0;
   long long cntk = 0;
   for (long long pb = 0; pb < p.Nf; pb += kPassRows) {
@@ -191,29 +196,65 @@ __global__ void __launch_bounds__(kUpdThreads) k_update(UpdParams p) {
     __syncthreads();
     for (int lo = 0; lo < total; lo += kRoundRows) {
       const int n = min(kRoundRows, total - lo);
-      // ---- stage the round's rows: one wave of independent 16-byte loads ----
-      for (int it = tid; it < n * LPR; it += kUpdThreads) {
-        const int e = it / LPR, q = it - e * LPR;
-        const long long row = pb + list[lo + e];
-        const float4 v = *reinterpret_cast<const float4 *>(rows + row * D + 4 * q);
-        *reinterpret_cast<float4 *>(xbuf + e * D + 4 * q) = v;
-        if (q == 0) {
-          const float wv = wg[(unsigned int)row / Mu];
-          wbuf[e] = wv;
-          cbbuf[e] = (double)wv * ri[row];
+      // ---- stage the round's rows: every load of the round is issued before the first store ----
+      {
+        constexpr int GI = kRoundRows * LPR / kUpdThreads;  // items per thread; q is the same for all of them
+        const int q = tid % LPR;
+        float4 v[GI];
+        float wv[GI];
+        double rv[GI];
+#pragma unroll
+        for (int u = 0; u < GI; ++u) {
+          const int e = (tid + u * kUpdThreads) / LPR;
+          if (e < n) {
+            const long long row = pb + list[lo + e];
+            v[u] = __ldg(reinterpret_cast<const float4 *>(rows + row * D + 4 * q));
+            if (q == 0) {
+              const unsigned int tok = (msh >= 0) ? ((unsigned int)row >> msh) : ((unsigned int)row / Mu);
+              wv[u] = __ldg(wg + tok);
+              rv[u] = __ldg(ri + row);
+            }
+          }
+        }
+#pragma unroll
+        for (int u = 0; u < GI; ++u) {
+          const int e = (tid + u * kUpdThreads) / LPR;
+          if (e < n) {
+            *reinterpret_cast<float4 *>(xbuf + e * D + 4 * q) = v[u];
+            if (q == 0) *reinterpret_cast<double2 *>(coef + 2 * e) = make_double2((double)wv[u], (double)wv[u] * rv[u]);
+          }
         }
       }
       __syncthreads();
       // ---- warp c adds cluster c's rows of this round in list (= ascending row) order ----
       const int a = max(seg0, lo), b = min(seg1, lo + n);
-      for (int pos = a; pos < b; ++pos) {
+      int pos = a;
+      for (; pos + 4 <= b; pos += 4) {  // loads of 4 rows in flight; the adds stay in list order
+        double cf[4][Q];
+        float xv[4][Q];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int e = pos + u - lo;
+#pragma unroll
+          for (int q = 0; q < Q; ++q) {
+            cf[u][q] = live[q] ? coef[2 * e + isB[q]] : 0.0;
+            xv[u][q] = live[q] ? xbuf[e * D + col[q]] : 0.0f;
+          }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          Wk += cf[u][0];  // lane 0 is an A lane: its coefficient is w_i
+#pragma unroll
+          for (int q = 0; q < Q; ++q) s[q] += cf[u][q] * (double)xv[u][q];
+        }
+      }
+      for (; pos < b; ++pos) {
         const int e = pos - lo;
-        const double wv = (double)wbuf[e], cb = cbbuf[e];
-        Wk += wv;
 #pragma unroll
         for (int q = 0; q < Q; ++q) {
-          const int el = lane + 32 * q;
-          if (el < 2 * D) s[q] += ((el >= D) ? cb : wv) * (double)xbuf[e * D + (el % D)];
+          const double cf = live[q] ? coef[2 * e + isB[q]] : 0.0;
+          if (q == 0) Wk += cf;
+          s[q] += cf * (double)(live[q] ? xbuf[e * D + col[q]] : 0.0f);
         }
       }
       if (a < b) cntk += b - a;
@@ -257,8 +298,11 @@ __global__ void __launch_bounds__(kUpdThreads) k_update(UpdParams p) {
         const double bn = sqrt(bn2);
         if (bn / W > kDelta) {
           new_shape = true;
+          float *sx = reinterpret_cast<float *>(xbuf) + warp * D;  // xbuf is free now: exchange the new shape
+          if (lane < D) sx[lane] = (float)(f[D + lane] / bn);
+          __syncwarp();
 #pragma unroll
-          for (int j = 0; j < D; ++j) sn[j] = (float)(f[D + j] / bn);
+          for (int j = 0; j < D; ++j) sn[j] = sx[j];
         }
       }
       double proj = 0.0;
