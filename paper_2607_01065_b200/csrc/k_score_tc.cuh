@@ -39,7 +39,8 @@ constexpr uint32_t kSmemA = kSmemOnes + kPlaneBytes;             // 28672, ring 
 constexpr uint32_t kSmemBar = kSmemA + kStages * 2 * kPlaneBytes;  // 94208
 constexpr int kQCap = 512;                                       // deferred exact re-scores per CTA
 constexpr uint32_t kSmemQ = kSmemBar + 256;                      // kQCap x {row, gmask | k_old << 16}, then the counter
-constexpr uint32_t kSmemTotal = kSmemQ + kQCap * 8 + 16 + 1024;  // + alignment slack
+constexpr uint32_t kSmemSh = kSmemQ + kQCap * 8 + 16;             // fp32 shapes [256][16] + gains [256] of the group (exact path)
+constexpr uint32_t kSmemTotal = kSmemSh + kN * kD * 4 + kN * 4 + 1024;  // + alignment slack
 
 struct ScoreTcParams {
   const uint8_t *bimg;   // [G][3][8192]: B_hi, B_lo, B_bias operand images (SWIZZLE_32B K-major)
@@ -323,8 +324,16 @@ k_score_tc(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CU
     const float gm = (p.mode == 0) ? __int_as_float(p.gmax[(long long)g * p.gmax_stride]) : 1.0f;
     const float e1 = (p.n_planes == 1 ? 2.0f : 4.5f) * 7.62939453125e-6f * 2.0f * gm;
     const float e0 = (p.mode == 0) ? 3.814697265625e-6f * gm * gm : 0.0f;
-    const float *sh_g = p.shapes + (long long)g * p.cb_stride_g * kD;
-    const float *ga_g = p.gains + (long long)g * p.cb_stride_g;
+    // the exact path reads the group's fp32 codebook from shared memory: staged here, while the first tile is in flight
+    float *sh_g = reinterpret_cast<float *>(sgen + kSmemSh);
+    float *ga_g = sh_g + kN * kD;
+    {
+      const int et = threadIdx.x - 64;  // 0..255
+      const float4 *src = reinterpret_cast<const float4 *>(p.shapes + (long long)g * p.cb_stride_g * kD);
+      for (int e = et; e < p.K * (kD / 4); e += 256) reinterpret_cast<float4 *>(sh_g)[e] = __ldg(src + e);
+      if (et < p.K) ga_g[et] = __ldg(p.gains + (long long)g * p.cb_stride_g + et);
+      asm volatile("bar.sync 1, 256;" ::: "memory");
+    }
     unsigned int n_changed = 0, n_refined = 0;
     for (int it = wg; it < n_my; it += 2) {
       const int buf = wg, bph = (it >> 1) & 1;

@@ -109,6 +109,7 @@ __global__ void __launch_bounds__(kUpdThreads) k_update(UpdParams p) {
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const uint8_t *ig = p.idx + (long long)g * p.Nf;
   const bool aligned = (reinterpret_cast<uintptr_t>(ig) & 3) == 0;
+  const bool aligned16 = (reinterpret_cast<uintptr_t>(ig) & 15) == 0;
   const uint32_t pat = (uint32_t)(k0 & 0xF0) * 0x01010101u;
   const uint32_t miss = (uint32_t)((k0 ^ 0x80) & 0xFF);  // a byte outside [k0, k0 + 16)
   const float *rows = p.Rf + (long long)g * p.Nf * D;
@@ -130,14 +131,31 @@ __global__ void __launch_bounds__(kUpdThreads) k_update(UpdParams p) {
   for (long long pb = 0; pb < p.Nf; pb += kPassRows) {
     // ---- walk 1: my 32 assignment bytes -> hit mask, per-(cluster, thread) counts ----
     uint32_t m = 0;
-    const long long r0 = pb + 32 * tid;
+    {
+      // the warp stages its 1024 bytes with coalesced 16-byte loads, then each thread takes its 32 rows
+      const long long wb = pb + 1024 * warp;
+      uint4 *stage = reinterpret_cast<uint4 *>(idxb + 1024 * warp);
+      if (aligned16 && wb + 1024 <= p.Nf) {
+        const uint4 *src = reinterpret_cast<const uint4 *>(ig + wb);
+        const uint4 v0 = __ldg(src + lane), v1 = __ldg(src + 32 + lane);
+        stage[lane] = v0;
+        stage[32 + lane] = v1;
+      } else {
+        const long long r0 = wb + 32 * lane;
 #pragma unroll
-    for (int wi = 0; wi < 8; ++wi) {
-      const uint32_t w = (r0 + 4 * wi < p.Nf) ? load_idx_word(ig, r0 + 4 * wi, p.Nf, aligned, miss) : miss * 0x01010101u;
-      reinterpret_cast<uint32_t *>(idxb)[8 * tid + wi] = w;
-      uint32_t h = __vcmpeq4(w & 0xF0F0F0F0u, pat) & 0x08040201u;  // bits 0, 9, 18, 27 <- bytes 0..3 hit
-      h = (h | (h >> 8) | (h >> 16) | (h >> 24)) & 0xFu;
-      m |= h << (4 * wi);
+        for (int wi = 0; wi < 8; ++wi)
+          reinterpret_cast<uint32_t *>(idxb)[8 * tid + wi] =
+              (r0 + 4 * wi < p.Nf) ? load_idx_word(ig, r0 + 4 * wi, p.Nf, aligned, miss) : miss * 0x01010101u;
+      }
+      __syncwarp();
+      const uint4 a0 = stage[2 * lane], a1 = stage[2 * lane + 1];
+      const uint32_t w[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
+#pragma unroll
+      for (int wi = 0; wi < 8; ++wi) {
+        uint32_t h = __vcmpeq4(w[wi] & 0xF0F0F0F0u, pat) & 0x08040201u;  // bits 0, 9, 18, 27 <- bytes 0..3 hit
+        h = (h | (h >> 8) | (h >> 16) | (h >> 24)) & 0xFu;
+        m |= h << (4 * wi);
+      }
     }
 #pragma unroll
     for (int c = 0; c < kCPC; ++c) cntb[c * kUpdThreads + tid] = 0;
