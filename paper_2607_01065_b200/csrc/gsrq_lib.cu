@@ -13,6 +13,7 @@
 #include "k_update.cuh"
 #include "k_score.cuh"
 #include "k_score_tc.cuh"
+#include "k_encode_tc.cuh"
 
 namespace gsrq {
 
@@ -60,7 +61,7 @@ struct Plan {
   long long nf_tok, Nf, Nall, nE;
   int M;
   // [0, encode_total): what gsrq_encode needs; the rest is for the fit
-  size_t off_list, off_cnt, off_st, encode_total;
+  size_t off_list, off_cnt, off_st, off_ebimg, off_egmax, encode_total;
   size_t off_Rf, off_rinv, off_wt, off_idx, off_ids, off_epart, off_term;
   size_t off_ahi, off_alo, off_rnorm, off_bimg, off_gmax, total;
 };
@@ -81,6 +82,8 @@ static Plan make_plan(const gsrq_view *v, int K, int S, long long n_fit_tokens) 
   p.off_list = o; o += align_up((size_t)v->G * p.Nall * sizeof(uint32_t));
   p.off_cnt = o;  o += align_up(kNumCounters * sizeof(unsigned int));
   p.off_st = o;   o += align_up((size_t)v->G * sizeof(DevStats));
+  p.off_ebimg = o; o += align_up(v->d == tc::kD ? (size_t)v->G * tc::kEncMaxS * 3 * tc::kBImgBytes : 0);
+  p.off_egmax = o; o += align_up(v->d == tc::kD ? (size_t)v->G * tc::kEncMaxS * sizeof(int) : 0);
   p.encode_total = o;
   p.off_Rf = o;   o += align_up((size_t)v->G * p.Nf * v->d * sizeof(float));
   p.off_rinv = o; o += align_up((size_t)v->G * p.Nf * sizeof(double));
@@ -277,6 +280,50 @@ static int prepare_rows(const Plan &pl, const void *kv, const gsrq_view *v, cons
                      n_planes, stream);
 }
 
+// ---- fused tensor-core encode (d == 16, bf16 input, stages [0, n) with n <= kEncMaxS) ----
+static bool can_encode_tc(const void *kv, const gsrq_view *v, int stage_begin, int stage_end) {
+  const int M = v->hd / v->d;
+  return use_tc(v->d) && v->dtype == GSRQ_BF16 && stage_begin == 0 && stage_end <= tc::kEncMaxS && M <= tc::kTileM &&
+         (M & (M - 1)) == 0 && ((uintptr_t)kv & 15) == 0 && v->T < (1LL << 31);
+}
+
+
+static int run_encode_tc(const void *kv, const gsrq_view *v, const gsrq_codebook *cb, int n_stages, uint8_t *codes,
+                         float *residual_out, const Plan &pl, char *ws, unsigned int *list_cnt, cudaStream_t stream) {
+  const int G = v->G, M = pl.M, tpt = tc::kTileM / M;
+  EncodeTiledFn fn = encode_tiled_fn();
+  if (!fn) { set_error("cuTensorMapEncodeTiled entry point not available"); return GSRQ_ECUDA; }
+  // dims {16, M, T, G} (or {16, M, G, T} when the head stride is the smaller one); strides in bytes
+  const bool head_inner = v->stride_g < v->stride_t;
+  CUtensorMap tm;
+  const cuuint64_t dims[4] = {(cuuint64_t)tc::kD, (cuuint64_t)M, (cuuint64_t)(head_inner ? G : v->T), (cuuint64_t)(head_inner ? v->T : G)};
+  const cuuint64_t strides[3] = {(cuuint64_t)tc::kD * 2, (cuuint64_t)(head_inner ? v->stride_g : v->stride_t) * 2,
+                                 (cuuint64_t)(head_inner ? v->stride_t : v->stride_g) * 2};
+  const cuuint32_t box[4] = {(cuuint32_t)tc::kD, (cuuint32_t)M, (cuuint32_t)(head_inner ? 1 : tpt), (cuuint32_t)(head_inner ? tpt : 1)};
+  const cuuint32_t es[4] = {1, 1, 1, 1};
+  CUresult r = fn(&tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void *>(kv), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                  CU_TENSOR_MAP_SWIZZLE_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) { set_error("cuTensorMapEncodeTiled (kv) failed (%d)", (int)r); return GSRQ_ECUDA; }
+  uint8_t *bimg = (uint8_t *)(ws + pl.off_ebimg);
+  int *gmax = (int *)(ws + pl.off_egmax);
+  LAUNCH(kClsMisc, stream, (tc::k_bimg<<<G * n_stages, 256, 0, stream>>>(cb->shapes, cb->gains, (long long)cb->S * cb->K, n_stages, cb->K, 0, bimg, gmax)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  tc::EncTcParams p{};
+  p.bimg = bimg; p.gmax = gmax; p.shapes = cb->shapes; p.gains = cb->gains; p.S = cb->S; p.K = cb->K; p.n_stages = n_stages;
+  p.codes = codes; p.code_stride_s = (long long)G * pl.Nall; p.res_out = residual_out; p.N = pl.Nall;
+  p.n_tiles = (int)((v->T + tpt - 1) / tpt);
+  p.list = (uint32_t *)(ws + pl.off_list); p.list_cnt = list_cnt;
+  static int n_sm = 0;
+  if (!n_sm) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev); if (n_sm <= 0) n_sm = 148; }
+  int ctas = n_sm / G; if (ctas < 1) ctas = 1; if (ctas > p.n_tiles) ctas = p.n_tiles;
+  const size_t smem = tc::kEncSmemTotal;
+  static bool attr_set = false;
+  if (!attr_set) { GSRQ_CUDA_CHECK(cudaFuncSetAttribute(tc::k_encode_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr_set = true; }
+  LAUNCH(kClsScore, stream, (tc::k_encode_tc<<<dim3((unsigned)ctas, (unsigned)G), tc::kThreads, smem, stream>>>(tm, p, tpt, head_inner ? 1 : 0)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  return GSRQ_OK;
+}
+
 }  // namespace gsrq
 
 using namespace gsrq;
@@ -404,6 +451,15 @@ int gsrq_encode(const void *kv, const gsrq_view *view, const gsrq_codebook *cb, 
   p.s_begin = stage_begin; p.s_end = stage_end; p.s_base = 0; p.mode = 0; p.subtract = 1;
   p.codes = codes; p.code_stride_s = (long long)view->G * pl.Nall; p.res_out = residual_out;
   p.st = nullptr; p.slot = 0; p.list = (uint32_t *)(ws + pl.off_list); p.list_cnt = cnt;
+  if (can_encode_tc(kv, view, stage_begin, stage_end)) {
+    // tensor-core filter over all stages; rows it cannot decide go to the exact path below
+    rc = run_encode_tc(kv, view, cb, stage_end, codes, residual_out, pl, ws, cnt, stream);
+    if (rc) return rc;
+    const int d = view->d;
+    LAUNCH(kClsRefine, stream, DISPATCH_D(d, (k_encode_refine<D><<<296, 256, 0, stream>>>(p))));
+    GSRQ_CUDA_CHECK(cudaGetLastError());
+    return GSRQ_OK;
+  }
   return run_encode(p, view->G, view->d, stream);
 }
 
@@ -458,7 +514,7 @@ static int assign_all_rows(const void *kv, const gsrq_view *view, const float *r
     if (rc) return rc;
     const long long cb_stride_g = (long long)cb->S * cb->K;
     int *gmax = (int *)(ws + pl.off_gmax);
-    LAUNCH(kClsMisc, stream, (tc::k_bimg<<<view->G, 256, 0, stream>>>(shapes_st, gains_st, cb_stride_g, cb->K, mode,
+    LAUNCH(kClsMisc, stream, (tc::k_bimg<<<view->G, 256, 0, stream>>>(shapes_st, gains_st, cb_stride_g, 1, cb->K, mode,
                                                                       (uint8_t *)(ws + pl.off_bimg), gmax)));
     GSRQ_CUDA_CHECK(cudaGetLastError());
     TcMaps maps;

@@ -202,6 +202,51 @@ __device__ __forceinline__ void top2_packed16(const float (&v)[16], float &best,
   idx = 15 - (int)(__float_as_uint(best) & 15u);
 }
 
+// Arg-max and runner-up of the 256 fp32 scores of one accumulator row (thread = TMEM lane).
+// Two groupings of the 256 scores: A = 16 consecutive columns (gmA[c], c = col / 16) and
+// B = columns with equal col % 16 (gmB[b]).  The winner is (arg-max A group gi, arg-max B
+// group ji); every other column lies in another A group or another B group, so
+// second = max(second of gmA, second of gmB).  All of it is 3-input max work.  The accumulator is
+// read with software-pipelined tcgen05.ld (chunk c+1 in flight while chunk c is reduced);
+// on_drained() runs as soon as the last chunk is in registers.
+template <bool DBG, typename F>
+__device__ __forceinline__ void tile_argmax(uint32_t taddr, float (&gmA)[16], float &best, float &second, int &gi, int &ji,
+                                            float *dbg_row, F on_drained) {
+  float gmB[16];
+  uint32_t va[32], vb[32];
+  GSRQ_TMEM_LD32(taddr, va);
+#pragma unroll
+  for (int c = 0; c < 8; c += 2) {
+    tmem_wait_ld();
+    GSRQ_TMEM_LD32(taddr + (c + 1) * 32, vb);
+    gmA[2 * c] = max16(va);
+    gmA[2 * c + 1] = max16(va + 16);
+    colmax32(va, gmB, c == 0);
+    if (DBG) {
+      if (dbg_row)
+        for (int j = 0; j < 32; ++j) dbg_row[c * 32 + j] = __uint_as_float(va[j]);
+    }
+    tmem_wait_ld();
+    if (c + 2 < 8) {
+      GSRQ_TMEM_LD32(taddr + (c + 2) * 32, va);
+    } else {
+      on_drained();
+    }
+    gmA[2 * c + 2] = max16(vb);
+    gmA[2 * c + 3] = max16(vb + 16);
+    colmax32(vb, gmB, false);
+    if (DBG) {
+      if (dbg_row)
+        for (int j = 0; j < 32; ++j) dbg_row[(c + 1) * 32 + j] = __uint_as_float(vb[j]);
+    }
+  }
+  float bestA, secA, bestB, secB;
+  top2_packed16(gmA, bestA, secA, gi);
+  top2_packed16(gmB, bestB, secB, ji);
+  best = fminf(bestA, bestB);
+  second = fmaxf(secA, secB);
+}
+
 // Exact path for one row, run by a whole warp: fp64, dot product summed in element order without
 // FMA contraction, score = (2 g)(r.s) - g g -- the definition's own operation order; lowest k wins ties.
 // Only the columns of the 16-column groups in `gmask` are candidates: a column whose filter score is
@@ -346,45 +391,13 @@ k_score_tc(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CU
       mbar_wait(tmem_full(buf), bph);
       tc_fence_after();
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + buf * kN;
-      // Two groupings of the 256 scores: A = 16 consecutive columns (gmA[c], c = col / 16) and
-      // B = columns with equal col % 16 (gmB[b]).  The winner is (arg-max A group, arg-max B
-      // group); every other column lies in another A group or another B group, so
-      // second = max(second of gmA, second of gmB).  All of it is 3-input max work.
-      float gmA[16], gmB[16];
-      uint32_t va[32], vb[32];
-      GSRQ_TMEM_LD32(taddr, va);
-#pragma unroll
-      for (int c = 0; c < 8; c += 2) {  // software pipeline: the load of chunk c+1 is in flight while chunk c is reduced
-        tmem_wait_ld();
-        GSRQ_TMEM_LD32(taddr + (c + 1) * 32, vb);
-        gmA[2 * c] = max16(va);
-        gmA[2 * c + 1] = max16(va + 16);
-        colmax32(va, gmB, c == 0);
-        if (DBG) {
-          if (row < p.N)
-            for (int j = 0; j < 32; ++j) p.dbg[gr * kN + c * 32 + j] = __uint_as_float(va[j]);
-        }
-        tmem_wait_ld();
-        if (c + 2 < 8) {
-          GSRQ_TMEM_LD32(taddr + (c + 2) * 32, va);
-        } else {  // accumulator drained: the MMA warp may overwrite this buffer
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive(tmem_empty(buf));
-        }
-        gmA[2 * c + 2] = max16(vb);
-        gmA[2 * c + 3] = max16(vb + 16);
-        colmax32(vb, gmB, false);
-        if (DBG) {
-          if (row < p.N)
-            for (int j = 0; j < 32; ++j) p.dbg[gr * kN + (c + 1) * 32 + j] = __uint_as_float(vb[j]);
-        }
-      }
-      float bestA, secA, bestB, secB;
+      float gmA[16], best, second;
       int gi, ji;
-      top2_packed16(gmA, bestA, secA, gi);
-      top2_packed16(gmB, bestB, secB, ji);
-      const float best = fminf(bestA, bestB), second = fmaxf(secA, secB);
+      tile_argmax<DBG>(taddr, gmA, best, second, gi, ji, (DBG && row < p.N) ? p.dbg + gr * kN : nullptr, [&]() {
+        tc_fence_before();  // accumulator drained: the MMA warp may overwrite this buffer
+        __syncwarp();
+        if (lane == 0) mbar_arrive(tmem_empty(buf));
+      });
       int k_new = gi * 16 + ji;
       const float E2 = 2.0f * fmaf(e1, rn, e0);
       const bool flag = (row < p.N) && (best - second <= E2);
@@ -444,23 +457,26 @@ k_score_tc(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CU
   if (warp == 1) tmem_dealloc(tmem_base, 512);
 }
 
-// Operand images and max gain of (group g, one stage) for a stand-alone scoring pass (gsrq_assign;
-// inside a fit the update kernel writes them).  grid = G, block = 256 (thread = codeword row).
+// Operand images and max gain of (group g, stage s) for block b = g * n_stages + s; codeword k of that
+// block is at index g * group_stride + s * K + k of shapes / gains.  Used by the stand-alone passes
+// (gsrq_assign: n_stages = 1 on a stage slice; gsrq_encode: all stages); inside a fit the update kernel
+// writes the images.  grid = G * n_stages, block = 256 (thread = codeword row).
 __global__ void __launch_bounds__(256) k_bimg(const float *__restrict__ shapes, const float *__restrict__ gains,
-                                              long long cb_stride_g, int K, int mode, uint8_t *__restrict__ bimg,
-                                              int *__restrict__ gmax) {
+                                              long long group_stride, int n_stages, int K, int mode,
+                                              uint8_t *__restrict__ bimg, int *__restrict__ gmax) {
   __shared__ int gmax_bits;
-  const int g = blockIdx.x, k = threadIdx.x;
+  const int b = blockIdx.x, k = threadIdx.x;
+  const long long base = (long long)(b / n_stages) * group_stride + (long long)(b % n_stages) * K;
   if (k == 0) gmax_bits = 0;
   __syncthreads();
-  const float gk = (k < K && mode == 0) ? gains[(long long)g * cb_stride_g + k] : 1.0f;
-  const float *s = shapes + ((long long)g * cb_stride_g + k) * kD;
+  const float gk = (k < K && mode == 0) ? gains[base + k] : 1.0f;
+  const float *s = shapes + (base + k) * kD;
 #pragma unroll
   for (int j = 0; j < kD; ++j)
-    write_bimg_elem(bimg + (size_t)g * 3 * kBImgBytes, k, j, gk, (k < K) ? s[j] : 0.0f, mode, k >= K);
+    write_bimg_elem(bimg + (size_t)b * 3 * kBImgBytes, k, j, gk, (k < K) ? s[j] : 0.0f, mode, k >= K);
   if (k < K && mode == 0) atomicMax(&gmax_bits, __float_as_int(fmaxf(gk, 0.f)));
   __syncthreads();
-  if (k == 0) gmax[g] = gmax_bits;
+  if (k == 0) gmax[b] = gmax_bits;
 }
 
 }  // namespace tc
