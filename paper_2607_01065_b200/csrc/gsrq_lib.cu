@@ -475,13 +475,49 @@ int gsrq_decode(const uint8_t *codes, const gsrq_codebook *cb, int n_stages, voi
   p.codes = codes; p.shapes = cb->shapes; p.gains = cb->gains; p.S = cb->S; p.K = cb->K; p.G = out_view->G;
   p.n_stages = n_stages; p.M = out_view->hd / d; p.N = out_view->T * p.M; p.out = kv_out; p.dtype = out_view->dtype;
   p.stride_g = out_view->stride_g; p.stride_t = out_view->stride_t;
+  p.row_begin = 0;
+  // bandwidth path: full 256-row chunks (d == 16, 1..4 stages, 16-byte aligned code planes)
+  if (d == 16 && n_stages >= 1 && n_stages <= 4 && p.N % 16 == 0 && p.N >= 256 && ((uintptr_t)codes & 15) == 0) {
+    const long long n_chunks = p.N / 256;
+    const bool dense = out_view->stride_t == out_view->hd;
+    static int n_sm = 0;
+    if (!n_sm) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev); if (n_sm <= 0) n_sm = 148; }
+    const size_t smem = (size_t)n_stages * kDecTabBytes;
+    int per_sm = (int)((227 * 1024) / (smem + 1024));  // CTAs that fit on one SM (shared memory; 40 registers x 512 threads)
+    if (per_sm > 2) per_sm = 2;  // measured: a third CTA per SM lowers the achieved bandwidth
+    if (per_sm < 1) per_sm = 1;
+    long long ctas = (per_sm * n_sm + out_view->G - 1) / out_view->G;
+    const long long need = (n_chunks + kDecThreads / 32 - 1) / (kDecThreads / 32);
+    if (ctas > need) ctas = need;
+    dim3 grid((unsigned)ctas, (unsigned)out_view->G);
+#define GSRQ_DEC_FAST(NS, DENSE)                                                                                          \
+  do {                                                                                                                    \
+    GSRQ_CUDA_CHECK(cudaFuncSetAttribute(k_decode_fast<NS, DENSE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+    LAUNCH(kClsDecode, stream, (k_decode_fast<NS, DENSE><<<grid, kDecThreads, smem, stream>>>(p, n_chunks)));                \
+  } while (0)
+    switch (n_stages * 2 + (dense ? 1 : 0)) {
+      case 2: GSRQ_DEC_FAST(1, false); break;
+      case 3: GSRQ_DEC_FAST(1, true); break;
+      case 4: GSRQ_DEC_FAST(2, false); break;
+      case 5: GSRQ_DEC_FAST(2, true); break;
+      case 6: GSRQ_DEC_FAST(3, false); break;
+      case 7: GSRQ_DEC_FAST(3, true); break;
+      case 8: GSRQ_DEC_FAST(4, false); break;
+      default: GSRQ_DEC_FAST(4, true); break;
+    }
+#undef GSRQ_DEC_FAST
+    GSRQ_CUDA_CHECK(cudaGetLastError());
+    p.row_begin = n_chunks * 256;
+    if (p.row_begin == p.N) return GSRQ_OK;
+  }
   const size_t smem = (size_t)n_stages * cb->K * d * sizeof(float);
   const bool use_smem = smem <= 200 * 1024;
   // enough CTAs to fill the machine a few times, but few enough that the table load amortises
+  const long long n_rows = p.N - p.row_begin;
   long long rows_per_cta = 8192;
-  while (rows_per_cta > 1024 && (p.N + rows_per_cta - 1) / rows_per_cta * out_view->G < 4 * 148) rows_per_cta /= 2;
+  while (rows_per_cta > 1024 && (n_rows + rows_per_cta - 1) / rows_per_cta * out_view->G < 4 * 148) rows_per_cta /= 2;
   p.rows_per_cta = rows_per_cta;
-  dim3 grid((unsigned)((p.N + rows_per_cta - 1) / rows_per_cta), (unsigned)out_view->G);
+  dim3 grid((unsigned)((n_rows + rows_per_cta - 1) / rows_per_cta), (unsigned)out_view->G);
   if (use_smem) {
     DISPATCH_D(d, {
       GSRQ_CUDA_CHECK(cudaFuncSetAttribute(k_decode<D, true, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(200 * 1024)));
@@ -667,7 +703,9 @@ int gsrq_pipeline_host(const void *kv_host, const gsrq_view *view, const float *
   if (e == cudaSuccess && w_host) e = cudaMemcpyAsync(d_w, w_host, (size_t)view->T * 4, cudaMemcpyHostToDevice, stream);
   for (int s = 0; s < S && rc == GSRQ_OK && e == cudaSuccess; ++s) {
     rc = gsrq_fit_stage(d_kv, view, d_w, 0, nullptr, 0, &cb, s, s ? d_res : nullptr, iters, seed, nullptr, d_ws, wsb, stream);
-    if (rc == GSRQ_OK) rc = gsrq_encode(d_kv, view, &cb, s, s + 1, d_codes, d_res, d_ws, wsb, stream);
+    // the fused tensor-core encode restarts from stage 0 (cheap); otherwise only stage s is encoded
+    const int sb = can_encode_tc(d_kv, view, 0, s + 1) ? 0 : s;
+    if (rc == GSRQ_OK) rc = gsrq_encode(d_kv, view, &cb, sb, s + 1, d_codes, (s + 1 < S) ? d_res : nullptr, d_ws, wsb, stream);
   }
   if (rc == GSRQ_OK && e == cudaSuccess && kv_out_host) {
     rc = gsrq_decode(d_codes, &cb, S, d_out, view, stream);

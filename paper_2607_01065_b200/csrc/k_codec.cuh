@@ -20,6 +20,7 @@ struct DecParams {
   int dtype;
   long long stride_g, stride_t;
   long long rows_per_cta;
+  long long row_begin;   // generic kernel: first row it decodes (the tail after the fast kernel's chunks)
 };
 
 __device__ __forceinline__ uint32_t pack_bf16x2(float a, float b) {
@@ -43,7 +44,7 @@ __global__ void __launch_bounds__(256) k_decode(DecParams p) {
     __syncthreads();
   }
   const int sub = threadIdx.x % LPR, rl = threadIdx.x / LPR;
-  const long long r0 = (long long)blockIdx.x * p.rows_per_cta;
+  const long long r0 = p.row_begin + (long long)blockIdx.x * p.rows_per_cta;
   const long long r1 = min(p.N, r0 + p.rows_per_cta);
   for (long long ib = r0 + rl; ib < r1; ib += (long long)RPI * U) {
     int code[U][GSRQ_MAX_STAGES > 8 ? 8 : GSRQ_MAX_STAGES];
@@ -93,6 +94,86 @@ __global__ void __launch_bounds__(256) k_decode(DecParams p) {
         *reinterpret_cast<uint2 *>(reinterpret_cast<uint16_t *>(p.out) + off) = v;
       } else {
         *reinterpret_cast<float4 *>(reinterpret_cast<float *>(p.out) + off) = acc[u];
+      }
+    }
+  }
+}
+
+// ---- bandwidth path (D = 16, NS <= 4 stages, N % 16 == 0): full chunks of 256 rows ----
+// HBM traffic is NS code bytes in and 32 (bf16) / 64 (fp32) bytes out per row; the per-row work
+// that has to keep up with it is the table gather, NS x 64 bytes of shared-memory reads per row,
+// so the table layout is what decides the speed.  Each codeword row is stored twice, as
+// 128 bytes [c0 c1 c2 c3 | c0 c1 c2 c3] (16-byte chunks), and lane l reads the chunk at byte
+// (l % 8) * 16 of its codeword's row: the 8 lanes of an LDS.128 phase always hit the 8 distinct
+// 16-byte bank groups, whatever the codes are -- no bank conflicts for any data.
+// Mapping: a warp owns 256 consecutive rows and decodes 8 consecutive rows per iteration, 4 lanes
+// (one 4-element quarter each) per row.
+constexpr int kDecThreads = 512;
+constexpr int kDecTabBytes = 256 * 128;  // per stage
+
+template <int NS, bool DENSE>
+__global__ void __launch_bounds__(kDecThreads) k_decode_fast(DecParams p, long long n_chunks) {
+  extern __shared__ __align__(16) float tab[];
+  const int g = blockIdx.y;
+  for (int e = threadIdx.x; e < NS * p.K * 16; e += kDecThreads) {
+    const int s = e / (p.K * 16), r = e - s * p.K * 16, k = r >> 4, j = r & 15;
+    const long long cb = ((long long)g * p.S + s) * p.K + k;
+    const float v = __fmul_rn(p.gains[cb], p.shapes[cb * 16 + j]);
+    float *row = tab + ((size_t)s * 256 + k) * 32;
+    row[j] = v;
+    row[16 + j] = v;
+  }
+  __syncthreads();
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int slot = lane >> 2, c4 = lane & 3;
+  const float *tl = tab + (lane & 7) * 4;
+  const int msh = ((p.M & (p.M - 1)) == 0) ? (31 - __clz(p.M)) : -1;
+  const long long ch0 = (long long)blockIdx.x * (kDecThreads / 32) + warp, chs = (long long)gridDim.x * (kDecThreads / 32);
+  // lane l holds the 8 code bytes of rows 8l..8l+7 of the chunk (one coalesced 256-byte load per stage),
+  // loaded one chunk ahead; iteration u decodes rows 8u..8u+7 (slot = row within the 8), whose codes
+  // sit in lane u: two shuffles per stage.  Every store instruction writes 256 contiguous bytes (bf16).
+  uint2 nx[NS];
+  if (ch0 < n_chunks) {
+#pragma unroll
+    for (int s = 0; s < NS; ++s)
+      nx[s] = __ldcs(reinterpret_cast<const uint2 *>(p.codes + ((long long)s * p.G + g) * p.N + ch0 * 256) + lane);
+  }
+  for (long long ch = ch0; ch < n_chunks; ch += chs) {
+    uint2 cw[NS];
+#pragma unroll
+    for (int s = 0; s < NS; ++s) cw[s] = nx[s];
+    if (ch + chs < n_chunks) {
+#pragma unroll
+      for (int s = 0; s < NS; ++s)
+        nx[s] = __ldcs(reinterpret_cast<const uint2 *>(p.codes + ((long long)s * p.G + g) * p.N + (ch + chs) * 256) + lane);
+    }
+#pragma unroll 8
+    for (int u = 0; u < 32; ++u) {
+      float4 acc;
+#pragma unroll
+      for (int s = 0; s < NS; ++s) {
+        const uint32_t lo = __shfl_sync(0xffffffffu, cw[s].x, u), hi = __shfl_sync(0xffffffffu, cw[s].y, u);
+        const uint32_t k = (((slot & 4) ? hi : lo) >> (8 * (slot & 3))) & 0xFFu;
+        const float4 c = *reinterpret_cast<const float4 *>(tl + ((size_t)s * 256 + k) * 32);
+        if (s == 0) acc = c;
+        else {
+          acc.x = __fadd_rn(acc.x, c.x); acc.y = __fadd_rn(acc.y, c.y);
+          acc.z = __fadd_rn(acc.z, c.z); acc.w = __fadd_rn(acc.w, c.w);
+        }
+      }
+      const long long i = ch * 256 + u * 8 + slot;
+      long long off;
+      if (DENSE) {
+        off = (long long)g * p.stride_g + i * 16 + c4 * 4;
+      } else {
+        const long long tok = (msh >= 0) ? (i >> msh) : (i / p.M);
+        off = (long long)g * p.stride_g + tok * p.stride_t + (i - tok * p.M) * 16 + c4 * 4;
+      }
+      if (p.dtype == GSRQ_BF16) {
+        __stcs(reinterpret_cast<uint2 *>(reinterpret_cast<uint16_t *>(p.out) + off),
+               make_uint2(pack_bf16x2(acc.x, acc.y), pack_bf16x2(acc.z, acc.w)));
+      } else {
+        __stcs(reinterpret_cast<float4 *>(reinterpret_cast<float *>(p.out) + off), acc);
       }
     }
   }
