@@ -3,10 +3,14 @@
 
 A "step" is one pass of the whole hot path over one synthetic layer tensor of BASELINE.json
 config 1 (8 KV heads x 4096 tokens x 128, bf16, d=16, K=256, S=2, 20 iterations/stage):
-for each stage: gsrq_fit_stage -> gsrq_encode of that stage (residual carried); then gsrq_decode.
+for each stage s: gsrq_fit_stage(s) -> fused gsrq_encode of stages [0, s] (its residual feeds the
+next fit; the last one is the final encode); then gsrq_decode.
 value = KV vectors (token x head) through the whole step per second, summed over ranks.
+Unless --no-big, rank 0 also runs BASELINE.json config 4 (one 8 x 131072-token batch, head-inner
+layout, 2.1 GB): fit on a 65,536-token sample per head, full-cache encode, full-cache decode --
+the sizes at which "fraction of the HBM / tensor roofline" is physically meaningful.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--cfg 1|2]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--cfg 1|2] [--no-big]
 """
 from __future__ import annotations
 
@@ -104,6 +108,75 @@ def run_reference(args, c):
     print(json.dumps(line))
 
 
+def run_cfg4(B, pk):
+    """BASELINE.json config 4 for one tensor (K-like): batch 8 x 131072 tokens x 8 KV heads x 128, bf16, head-inner
+    layout [B*T][G][hd] (2.147 GB); d=16, K=256, S=2, 10 iterations; codebooks fitted on a seeded 65,536-token
+    sample per head, then full-cache encode and decode.  Same generator recipe as inputs.k_like, drawn on the
+    device with a seeded torch generator."""
+    c = inputs.CONFIGS[4]
+    G, hd, d, K, S, iters = c.G, c.hd, c.d, c.K, c.S, c.iters
+    T, n_fit, M = 8 * 131072, 65536, hd // d
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(inputs.seed_of(4, "k"))
+    scale = torch.exp(0.3 * torch.randn(G, hd, device="cuda", generator=gen))
+    for g in range(G):
+        scale[g, torch.randperm(hd, device="cuda", generator=gen)[:4]] *= 10.0
+    x = torch.empty(T, G, hd, dtype=torch.bfloat16, device="cuda")
+    for t0 in range(0, T, 131072):
+        x[t0:t0 + 131072] = (torch.randn(131072, G, hd, device="cuda", generator=gen) * scale).to(torch.bfloat16)
+    w = torch.exp(torch.randn(T, device="cuda", generator=gen))
+    w /= w.mean()
+    fit = torch.stack([torch.sort(torch.randperm(T, device="cuda", generator=gen)[:n_fit]).values for _ in range(G)]).contiguous()
+    view = B.view_of(x, d, head_inner=True)
+    shapes = torch.zeros(G, S, K, d, device="cuda")
+    gains = torch.zeros(G, S, K, device="cuda")
+    cb = B.codebook_of(shapes, gains)
+    ws = B.workspace(view, K, S, n_fit)
+    codes = torch.zeros(S, G, T * M, dtype=torch.uint8, device="cuda")
+    out = torch.empty_like(x)
+
+    def timed(f, n=3):
+        ts = []
+        for _ in range(n):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); f(); b.record()
+            torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        return float(np.median(ts))
+
+    def fit_all():
+        for s in range(S):   # residual re-derived from kv + earlier stages on the fit rows
+            B.gsrq_fit_stage(x, view, w, 0, fit, cb, s, None, iters, 0, ws, want_stats=False)
+
+    fit_all()
+    fit_ms = timed(fit_all, 2)
+    enc = lambda: B.gsrq_encode(x, view, cb, 0, S, codes, None, ws)
+    enc()
+    enc_ms = timed(enc)
+    B.gsrq_profile_enable(True)
+    enc()
+    torch.cuda.synchronize()
+    pr = B.gsrq_profile_read()
+    B.gsrq_profile_enable(False)
+    dec = lambda: B.gsrq_decode(codes, cb, S, out, view)
+    dec()
+    dec_ms = timed(dec, 5)
+    rows = G * T * M
+    enc_tf = 2.0 * K * d * rows * S / (enc_ms * 1e-3) / 1e12
+    tc_tf = 2.0 * K * d * rows * S / (pr["encode"][0] * 1e-3) / 1e12 if pr["encode"][0] > 0 else None
+    dec_bytes = rows * S + rows * 2 * d
+    dec_gbs = dec_bytes / (dec_ms * 1e-3) / 1e9
+    # sanity: decode(encode(x)) must be closer to x than 0 is (relative residual energy < 1)
+    err = float(((out[:4096].float() - x[:4096].float()) ** 2).sum() / (x[:4096].float() ** 2).sum())
+    return dict(workload="cfg4:k-cache-8x131072x8x128 head-inner, fit on 65536-token sample/head", T=T, G=G, S=S, iters=iters,
+                bytes=x.numel() * 2, fit_ms=fit_ms,
+                encode=dict(ms=enc_ms, kv_vectors_per_s=G * T / (enc_ms * 1e-3), bound="tensor", achieved_tflops=enc_tf,
+                            frac=enc_tf / pk["bf16_tflops_sustained"], tc_kernel_ms=pr["encode"][0], tc_kernel_tflops=tc_tf,
+                            exact_path_ms=pr["refine"][0]),
+                decode=dict(ms=dec_ms, gb_per_s=dec_gbs, bound="hbm", frac=dec_gbs / pk["hbm_gbs"], bytes=dec_bytes),
+                rel_residual_energy_first_4096_tokens=err)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -112,6 +185,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cfg", type=int, default=1, choices=[1, 2])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-big", action="store_true", help="skip the config-4 (2.1 GB) encode / decode leg")
     args = ap.parse_args()
     c = inputs.CONFIGS[args.cfg]
     rank = int(os.environ.get("RANK", "0"))
@@ -158,7 +232,7 @@ def main():
     def step():
         for s in range(S):
             B.gsrq_fit_stage(x, view, w, 0, None, cb, s, residual if s else None, c.iters, 0, ws, want_stats=False)
-            B.gsrq_encode(x, view, cb, s, s + 1, codes, residual, ws)
+            B.gsrq_encode(x, view, cb, 0, s + 1, codes, residual if s + 1 < S else None, ws)
         B.gsrq_decode(codes, cb, S, out, view)
 
     def barrier():
@@ -237,18 +311,42 @@ def main():
 
     if rank != 0:
         return
+    big = None
+    if not args.no_big:
+        del flush
+        torch.cuda.empty_cache()
+        big = run_cfg4(B, peaks())
     pk = peaks()
-    # dominant kernel = the scoring filter; algorithmic work = 2*K*d flops per sub-vector per scoring pass
-    sc_ms, sc_n = prof["score"]
+    # Rooflines of the step's kernels, from the live CUDA-event brackets (two profiled steps).
+    # Algorithmic work: scoring pass 2*K*d flops per sub-vector; update kernel one read of
+    # the fp32 row + 1/(||r||+eps) + code = 4d + 9 bytes per sub-vector; decode S + 2d bytes per sub-vector.
     rows_per_launch = G * T * M
-    flops_per_launch = 2.0 * K * d * rows_per_launch
-    achieved_tf = flops_per_launch / (sc_ms / max(sc_n, 1) * 1e-3) / 1e12
     tot_ms = sum(v[0] for v in prof.values())
-    roofline = dict(bound="tensor", kernel="k_encode (scoring filter + arg-max)", achieved=achieved_tf,
-                    peak=pk["bf16_tflops_sustained"], unit="TFLOP/s", frac=achieved_tf / pk["bf16_tflops_sustained"],
-                    traffic=None, peak_source=pk["source"] + " (sustained bf16: kernel timed inside a long step)",
-                    ms_per_launch=sc_ms / max(sc_n, 1), launches=sc_n, share_of_step=sc_ms / tot_ms if tot_ms else None,
-                    by_class={k: dict(ms=v[0] / 2, launches=v[1] // 2) for k, v in prof.items()})
+
+    def kern(name, cls, bound, work_per_launch, peak, unit):
+        ms, n = prof[cls]
+        per = ms / max(n, 1)
+        ach = work_per_launch / (per * 1e-3) / (1e12 if bound == "tensor" else 1e9) if per > 0 else 0.0
+        return dict(bound=bound, kernel=name, achieved=ach, peak=peak, unit=unit, frac=ach / peak, traffic=None,
+                    ms_per_launch=per, launches=n // 2, share_of_step=ms / tot_ms if tot_ms else None)
+
+    kerns = [
+        kern("tc::k_score_tc (tcgen05 scoring + arg-max, fit passes)", "score", "tensor", 2.0 * K * d * rows_per_launch,
+             pk["bf16_tflops_sustained"], "TFLOP/s"),
+        kern("k_update (segmented fp64 reduction + Eq. 7/8)", "update", "hbm", rows_per_launch * (4.0 * d + 9.0),
+             pk["hbm_gbs"], "GB/s"),
+        kern("tc::k_encode_tc (fused S-stage encode)", "encode", "tensor", 0.0, pk["bf16_tflops_sustained"], "TFLOP/s"),
+    ]
+    # the encode class mixes [0,1) and [0,2) launches: algorithmic flops of one step's encodes / their summed time
+    enc_cls_ms = prof["encode"][0] / 2
+    if enc_cls_ms > 0:
+        ach = 2.0 * K * d * rows_per_launch * sum(range(1, S + 1)) / (enc_cls_ms * 1e-3) / 1e12
+        kerns[2].update(achieved=ach, frac=ach / pk["bf16_tflops_sustained"])
+    dom = max(kerns, key=lambda kk: kk["share_of_step"] or 0.0)
+    roofline = dict(dom)
+    roofline["peak_source"] = pk["source"] + (" (sustained bf16: kernel timed inside a long step)" if dom["bound"] == "tensor" else " (copy bandwidth)")
+    roofline["by_class"] = {k: dict(ms=v[0] / 2, launches=v[1] // 2) for k, v in prof.items()}
+    roofline["other_kernels"] = [kk for kk in kerns if kk is not dom]
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
                 ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="bf16 in, fp32/fp64 arithmetic",
                 data="synthetic", impl="ours",
@@ -262,6 +360,8 @@ def main():
                             tensor_frac=(2.0 * K * d * rows_per_launch * S / (enc_ms * 1e-3) / 1e12) / pk["bf16_tflops"]),
                 decode=dict(gb_per_s=dec_bytes / (dec_ms * 1e-3) / 1e9, ms=dec_ms, bytes=dec_bytes,
                             hbm_frac=dec_bytes / (dec_ms * 1e-3) / 1e9 / pk["hbm_gbs"]))
+    if big is not None:
+        line["cfg4"] = big
     if not args.no_cpu_baseline:
         from oracle import gsrq_oracle as o
         t0 = time.perf_counter()

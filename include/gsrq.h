@@ -188,7 +188,7 @@ int gsrq_pipeline_host(const void *kv_host, const gsrq_view *view, const float *
 
 /* ---- measurement hooks (host functions) ---- */
 
-#define GSRQ_N_KERNEL_CLASSES 6 /* 0 prep, 1 score (filter), 2 refine (CUDA-core path only), 3 update, 4 misc, 5 decode */
+#define GSRQ_N_KERNEL_CLASSES 7 /* 0 prep, 1 score (fit assignment passes; CUDA-core encode), 2 refine (exact path kernel), 3 update, 4 misc, 5 decode, 6 encode (fused tensor-core encode) */
 
 /* When on, every kernel launch of this library is bracketed by a CUDA event pair on its stream. */
 void gsrq_profile_enable(int on);

@@ -172,7 +172,7 @@ def gsrq_pipeline_host(kv_host, view, w_host, K, S, iters, seed, shapes_host, ga
                                     _ptr(shapes_host), _ptr(gains_host), _ptr(codes_host), _ptr(kv_out_host)))
 
 
-KERNEL_CLASSES = ["prep", "score", "refine", "update", "misc", "decode"]
+KERNEL_CLASSES = ["prep", "score", "refine", "update", "misc", "decode", "encode"]
 
 
 def gsrq_profile_enable(on: bool):
@@ -181,8 +181,8 @@ def gsrq_profile_enable(on: bool):
 
 def gsrq_profile_read():
     """Per kernel class: (summed device ms, launches) since the last read."""
-    ms = (C.c_double * 6)()
-    n = (C.c_int64 * 6)()
+    ms = (C.c_double * len(KERNEL_CLASSES))()
+    n = (C.c_int64 * len(KERNEL_CLASSES))()
     _check(lib().gsrq_profile_read(ms, n))
     return {k: (ms[i], n[i]) for i, k in enumerate(KERNEL_CLASSES)}
 

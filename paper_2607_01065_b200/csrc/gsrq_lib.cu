@@ -29,12 +29,12 @@ void set_error(const char *fmt, ...) {
 
 
 // ---- launch accounting / optional per-kernel CUDA-event timing (gsrq_profile_*) ----
-enum { kClsPrep = 0, kClsScore = 1, kClsRefine = 2, kClsUpdate = 3, kClsMisc = 4, kClsDecode = 5, kNumCls = 6 };
+enum { kClsPrep = 0, kClsScore = 1, kClsRefine = 2, kClsUpdate = 3, kClsMisc = 4, kClsDecode = 5, kClsEncode = 6, kNumCls = 7 };
 struct ProfRec { int cls; cudaEvent_t a, b; };
 static std::mutex g_prof_mu;
 static std::vector<ProfRec> g_prof_recs;
 static bool g_prof_on = false;
-static long long g_launches[kNumCls] = {0, 0, 0, 0, 0, 0};
+static long long g_launches[kNumCls] = {0, 0, 0, 0, 0, 0, 0};
 
 struct ProfScope {
   cudaStream_t stream;
@@ -319,7 +319,7 @@ static int run_encode_tc(const void *kv, const gsrq_view *v, const gsrq_codebook
   const size_t smem = tc::kEncSmemTotal;
   static bool attr_set = false;
   if (!attr_set) { GSRQ_CUDA_CHECK(cudaFuncSetAttribute(tc::k_encode_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr_set = true; }
-  LAUNCH(kClsScore, stream, (tc::k_encode_tc<<<dim3((unsigned)ctas, (unsigned)G), tc::kThreads, smem, stream>>>(tm, p, tpt, head_inner ? 1 : 0)));
+  LAUNCH(kClsEncode, stream, (tc::k_encode_tc<<<dim3((unsigned)ctas, (unsigned)G), tc::kThreads, smem, stream>>>(tm, p, tpt, head_inner ? 1 : 0)));
   GSRQ_CUDA_CHECK(cudaGetLastError());
   return GSRQ_OK;
 }
