@@ -79,7 +79,7 @@ static Plan make_plan(const gsrq_view *v, int K, int S, long long n_fit_tokens) 
   p.Nall = v->T * p.M;
   p.nE = (p.Nf + kPrepRows - 1) / kPrepRows;
   size_t o = 0;
-  p.off_list = o; o += align_up((size_t)v->G * p.Nall * sizeof(uint32_t));
+  p.off_list = o; o += align_up((size_t)v->G * p.Nall * sizeof(uint2));
   p.off_cnt = o;  o += align_up(kNumCounters * sizeof(unsigned int));
   p.off_st = o;   o += align_up((size_t)v->G * sizeof(DevStats));
   p.off_ebimg = o; o += align_up(v->d == tc::kD ? (size_t)v->G * tc::kEncMaxS * 3 * tc::kBImgBytes : 0);
@@ -142,7 +142,7 @@ static int run_encode(EncParams p, int G, int d, cudaStream_t stream) {
   dim3 grid((unsigned)((p.N + 256 * RPT - 1) / (256 * RPT)), (unsigned)G);
   LAUNCH(kClsScore, stream, DISPATCH_D(d, (k_encode<D, RPT><<<grid, 256, smem, stream>>>(p))));
   GSRQ_CUDA_CHECK(cudaGetLastError());
-  LAUNCH(kClsRefine, stream, DISPATCH_D(d, (k_encode_refine<D><<<296, 256, 0, stream>>>(p))));
+  LAUNCH(kClsRefine, stream, DISPATCH_D(d, (k_encode_exact<D><<<1184, 256, 0, stream>>>(p))));
   GSRQ_CUDA_CHECK(cudaGetLastError());
   return GSRQ_OK;
 }
@@ -272,7 +272,7 @@ static int prepare_rows(const Plan &pl, const void *kv, const gsrq_view *v, cons
   p.N = pl.Nf; p.shapes = cb->shapes; p.gains = cb->gains; p.S = cb->S; p.K = cb->K;
   p.s_begin = 0; p.s_end = stage; p.s_base = 0; p.mode = 0; p.subtract = 1;
   p.codes = nullptr; p.code_stride_s = 0; p.res_out = Rf; p.st = nullptr; p.slot = 0;
-  p.list = (uint32_t *)(ws + pl.off_list);
+  p.list = (uint2 *)(ws + pl.off_list);
   p.list_cnt = (unsigned int *)(ws + pl.off_cnt) + (kNumCounters - 1);
   rc = run_encode(p, G, d, stream);
   if (rc) return rc;
@@ -312,7 +312,7 @@ static int run_encode_tc(const void *kv, const gsrq_view *v, const gsrq_codebook
   p.bimg = bimg; p.gmax = gmax; p.shapes = cb->shapes; p.gains = cb->gains; p.S = cb->S; p.K = cb->K; p.n_stages = n_stages;
   p.codes = codes; p.code_stride_s = (long long)G * pl.Nall; p.res_out = residual_out; p.N = pl.Nall;
   p.n_tiles = (int)((v->T + tpt - 1) / tpt);
-  p.list = (uint32_t *)(ws + pl.off_list); p.list_cnt = list_cnt;
+  p.list = (uint2 *)(ws + pl.off_list); p.list_cnt = list_cnt;
   static int n_sm = 0;
   if (!n_sm) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev); if (n_sm <= 0) n_sm = 148; }
   int ctas = n_sm / G; if (ctas < 1) ctas = 1; if (ctas > p.n_tiles) ctas = p.n_tiles;
@@ -383,7 +383,7 @@ int gsrq_fit_stage(const void *kv, const gsrq_view *view, const float *w, int64_
   p.N = pl.Nf; p.S = cb->S; p.K = K;
   p.subtract = 0;
   p.codes = idx; p.code_stride_s = 0; p.res_out = nullptr; p.st = st;
-  p.list = (uint32_t *)(ws + pl.off_list);
+  p.list = (uint2 *)(ws + pl.off_list);
   // score only stage `stage` on the prepared rows: present it to the kernels as a 1-stage pass
   p.shapes = shapes_st; p.gains = gains_st; p.s_begin = 0; p.s_end = 1; p.s_base = 0;
   // t = 0 is Alg. 1 l.2: gains by Eq. 8 under the max-projection assignment (reading c-I);
@@ -450,13 +450,13 @@ int gsrq_encode(const void *kv, const gsrq_view *view, const gsrq_codebook *cb, 
   p.N = pl.Nall; p.shapes = cb->shapes; p.gains = cb->gains; p.S = cb->S; p.K = cb->K;
   p.s_begin = stage_begin; p.s_end = stage_end; p.s_base = 0; p.mode = 0; p.subtract = 1;
   p.codes = codes; p.code_stride_s = (long long)view->G * pl.Nall; p.res_out = residual_out;
-  p.st = nullptr; p.slot = 0; p.list = (uint32_t *)(ws + pl.off_list); p.list_cnt = cnt;
+  p.st = nullptr; p.slot = 0; p.list = (uint2 *)(ws + pl.off_list); p.list_cnt = cnt;
   if (can_encode_tc(kv, view, stage_begin, stage_end)) {
     // tensor-core filter over all stages; rows it cannot decide go to the exact path below
     rc = run_encode_tc(kv, view, cb, stage_end, codes, residual_out, pl, ws, cnt, stream);
     if (rc) return rc;
     const int d = view->d;
-    LAUNCH(kClsRefine, stream, DISPATCH_D(d, (k_encode_refine<D><<<296, 256, 0, stream>>>(p))));
+    LAUNCH(kClsRefine, stream, DISPATCH_D(d, (k_encode_exact<D><<<1184, 256, 0, stream>>>(p))));
     GSRQ_CUDA_CHECK(cudaGetLastError());
     return GSRQ_OK;
   }
@@ -566,7 +566,7 @@ static int assign_all_rows(const void *kv, const gsrq_view *view, const float *r
   p.shapes = shapes_st; p.gains = gains_st;
   p.s_begin = 0; p.s_end = 1; p.s_base = 0; p.mode = mode; p.subtract = 0;
   p.codes = idx_out; p.code_stride_s = 0; p.res_out = nullptr; p.st = nullptr; p.slot = 0;
-  p.list = (uint32_t *)(ws + pl.off_list); p.list_cnt = cnt;
+  p.list = (uint2 *)(ws + pl.off_list); p.list_cnt = cnt;
   return run_encode(p, view->G, view->d, stream);
 }
 

@@ -10,7 +10,8 @@
 //   stage s:  D = R_hi.B_hi^T + R_hi.B_lo^T + R_lo.B_hi^T + 1.B_bias^T   against stage s's images
 // The N x K score matrix and the residual between stages are never written to HBM; optionally the
 // final fp32 residual is.  A row whose top-2 gap is within the filter's error bound at any stage is
-// handed to the exact CUDA-core path (k_encode_refine), which redoes that row from stage 0.
+// handed, with its candidate codeword groups, to the exact CUDA-core path (k_encode_exact), which takes
+// the row over from that stage.
 //
 // Warp roles (320 threads, one CTA per SM, persistent over tiles of one group): warp 0 TMA producer,
 // warp 1 tcgen05.mma issue, warps 2-5 / 6-9 two epilogue warpgroups, each owning one 256-column
@@ -41,7 +42,7 @@ struct EncTcParams {
   float *res_out;          // [G][N][16] or nullptr
   long long N;             // rows per group
   int n_tiles;
-  uint32_t *list;          // rows for the exact path (g*N + i)
+  uint2 *list;             // rows for the exact path: {g*N + i, candidate-group mask | stage << 16}
   unsigned int *list_cnt;
 };
 
@@ -192,9 +193,13 @@ __global__ void __launch_bounds__(kThreads, 1) k_encode_tc(const __grid_constant
           }
         });
         const int k = gi * 16 + ji;
-        if (alive && best - second <= 2.0f * fmaf(e1, rn, e0)) {  // ambiguous: the exact path redoes this row (all stages)
+        const float E2 = 2.0f * fmaf(e1, rn, e0);
+        if (alive && best - second <= E2) {  // ambiguous: the exact path takes the row over from this stage
+          uint32_t gmask = 0;  // groups of 16 columns whose maximum is within 2E of the best: the only candidates
+#pragma unroll
+          for (int c = 0; c < 16; ++c) gmask |= (gmA[c] >= best - E2) ? (1u << c) : 0u;
           const unsigned int pos = atomicAdd(p.list_cnt, 1u);
-          p.list[pos] = (uint32_t)gr;
+          p.list[pos] = make_uint2((uint32_t)gr, gmask | ((uint32_t)s << 16));
           alive = false;
         }
         if (alive) p.codes[(long long)s * p.code_stride_s + gr] = (uint8_t)k;

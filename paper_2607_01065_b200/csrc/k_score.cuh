@@ -26,7 +26,7 @@ struct EncParams {
   float *res_out;       // [G][N][D] or nullptr (may alias src.rows)
   DevStats *st;         // nullptr outside a fit
   int slot;             // st[g].changed[slot] counts rows whose code changed
-  uint32_t *list;       // flagged rows (g*N + i)
+  uint2 *list;          // rows for the exact path: {g*N + i, candidate-group mask | first undecided stage << 16}
   unsigned int *list_cnt;
 };
 
@@ -138,7 +138,8 @@ __global__ void __launch_bounds__(256) k_encode(EncParams p) {
         const float E = fmaf(e_sh[0], sqrtf(n2) * 1.00001f, e_sh[1]);
         if (best - second <= 2.0f * E) {  // ambiguous: exact path decides this row (all stages)
           const unsigned int pos = atomicAdd(p.list_cnt, 1u);
-          p.list[pos] = (uint32_t)((long long)g * p.N + i);
+          // stages before s are decided (their codes are stored); without a code plane the row restarts from 0
+          p.list[pos] = make_uint2((uint32_t)((long long)g * p.N + i), 0xFFFFu | ((uint32_t)(p.codes ? s : 0) << 16));
           live[r] = false;
           continue;
         }
@@ -166,16 +167,58 @@ __global__ void __launch_bounds__(256) k_encode(EncParams p) {
   }
 }
 
-// Exact path: one warp per flagged row.  fp64, dot product summed in element order without
-// FMA contraction, score = (2 g) (r.s) - g g -- the definition's own operation order.
+// Exact fp64 scores of the codewords of the 16-codeword groups in `gmask` for row x; lowest k wins ties.
+// fp64, dot product summed in element order without FMA contraction, score = (2 g)(r.s) - g g: the
+// definition's own operation order.  Two groups (one per half-warp) per round.
 template <int D>
-__global__ void __launch_bounds__(256) k_encode_refine(EncParams p) {
+__device__ __forceinline__ int exact_argmax_warp(const float (&x)[D], const float *__restrict__ sh, const float *__restrict__ ga,
+                                                 int K, int mode, int lane, uint32_t gmask) {
+  double best = -INFINITY;
+  int bi = 0x7fffffff;
+  while (gmask) {
+    const int c0 = __ffs(gmask) - 1;
+    gmask &= gmask - 1;
+    int c1 = -1;
+    if (gmask) { c1 = __ffs(gmask) - 1; gmask &= gmask - 1; }
+    const int c = (lane < 16) ? c0 : c1;
+    const int kk = 16 * c + (lane & 15);
+    if (c >= 0 && kk < K) {
+      float cwv[D];
+      load_row_f32<D>(sh, kk, cwv);
+      double dot = 0.0;
+#pragma unroll
+      for (int j = 0; j < D; ++j) dot = __dadd_rn(dot, __dmul_rn((double)x[j], (double)cwv[j]));
+      double sc = dot;
+      if (mode == 0) {
+        const double gk = (double)ga[kk];
+        sc = __dsub_rn(__dmul_rn(__dmul_rn(2.0, gk), dot), __dmul_rn(gk, gk));
+      }
+      if (sc > best || (sc == best && kk < bi)) { best = sc; bi = kk; }
+    }
+  }
+  for (int off = 16; off; off >>= 1) {
+    const double ob = __shfl_xor_sync(0xffffffffu, best, off);
+    const int oi = __shfl_xor_sync(0xffffffffu, bi, off);
+    if (ob > best || (ob == best && oi < bi)) { best = ob; bi = oi; }
+  }
+  return (bi == 0x7fffffff) ? 0 : bi;
+}
+
+// Exact path: one warp per listed row.  Stages before the entry's first undecided stage s* are replayed
+// from their stored codes; stage s* is decided in fp64 among the entry's candidate groups (every
+// codeword outside them is provably not the arg-max); later stages run the fp32 filter of k_encode
+// across the warp (8 codewords per lane) and fall back to fp64 over all codewords when its top-2 gap
+// is within the error bound.  The result equals the exact-arithmetic arg-max at every stage.
+template <int D>
+__global__ void __launch_bounds__(256) k_encode_exact(EncParams p) {
   const int lane = threadIdx.x & 31;
   const unsigned int n = *p.list_cnt;
   const unsigned int warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const unsigned int nwarps = (gridDim.x * blockDim.x) >> 5;
   for (unsigned int e = warp0; e < n; e += nwarps) {
-    const long long gi = p.list[e];
+    const uint2 en = p.list[e];
+    const long long gi = en.x;
+    const int s_star = (int)(en.y >> 16);
     const int g = (int)(gi / p.N);
     const long long i = gi - (long long)g * p.N;
     float x[D];
@@ -184,30 +227,42 @@ __global__ void __launch_bounds__(256) k_encode_refine(EncParams p) {
       const float *sh = p.shapes + ((long long)g * p.S + s) * p.K * D;
       const float *ga = p.gains + ((long long)g * p.S + s) * p.K;
       int k;
-      if (s < p.s_begin) {
+      if (s < p.s_begin || s < s_star) {
         k = p.codes[(long long)(s - p.s_base) * p.code_stride_s + gi];
       } else {
-        double best = -INFINITY;
-        int bi = 0x7fffffff;
-        for (int kk = lane; kk < p.K; kk += 32) {
-          double dot = 0.0;
+        if (s == s_star) {
+          k = exact_argmax_warp<D>(x, sh, ga, p.K, p.mode, lane, en.y & 0xFFFFu);
+        } else {
+          // fp32 filter across the warp: score = fl32(2 (r.c_k) - b_k), c = fl32(g s), b = fl32(g^2)
+          float best = -INFINITY, second = -INFINITY, gmx = 0.0f;
+          int bi = 0x7fffffff;
+          for (int kk = lane; kk < p.K; kk += 32) {
+            const float gk = (p.mode == 0) ? ga[kk] : 1.0f;
+            gmx = fmaxf(gmx, gk);
+            float cwv[D];
+            load_row_f32<D>(sh, kk, cwv);
+            float dot = 0.0f;
 #pragma unroll
-          for (int j = 0; j < D; ++j) dot = __dadd_rn(dot, __dmul_rn((double)x[j], (double)sh[kk * D + j]));
-          double sc;
-          if (p.mode == 0) {
-            const double gk = (double)ga[kk];
-            sc = __dsub_rn(__dmul_rn(__dmul_rn(2.0, gk), dot), __dmul_rn(gk, gk));
-          } else {
-            sc = dot;
+            for (int j = 0; j < D; ++j) dot = fmaf(x[j], (p.mode == 0) ? __fmul_rn(gk, cwv[j]) : cwv[j], dot);
+            const float sc = fmaf(2.0f, dot, (p.mode == 0) ? -__fmul_rn(gk, gk) : 0.0f);
+            if (sc > best) { second = best; best = sc; bi = kk; }
+            else if (sc > second) second = sc;
           }
-          if (sc > best) { best = sc; bi = kk; }
+          for (int off = 16; off; off >>= 1) {
+            const float ob = __shfl_xor_sync(0xffffffffu, best, off), os = __shfl_xor_sync(0xffffffffu, second, off);
+            const int oi = __shfl_xor_sync(0xffffffffu, bi, off);
+            gmx = fmaxf(gmx, __shfl_xor_sync(0xffffffffu, gmx, off));
+            if (ob > best || (ob == best && oi < bi)) { second = fmaxf(best, os); best = ob; bi = oi; }
+            else second = fmaxf(second, ob);
+          }
+          float n2 = 0.0f;
+#pragma unroll
+          for (int j = 0; j < D; ++j) n2 = fmaf(x[j], x[j], n2);
+          const float gm = (p.mode == 0) ? gmx : 1.0f;
+          const float E = fmaf(1.05f * kU * (2 * D + 4) * gm, sqrtf(n2) * 1.00001f, (p.mode == 0) ? 1.05f * kU * 2.0f * gm * gm : 0.0f);
+          k = (bi == 0x7fffffff) ? 0 : bi;
+          if (best - second <= 2.0f * E) k = exact_argmax_warp<D>(x, sh, ga, p.K, p.mode, lane, 0xFFFFu);
         }
-        for (int off = 16; off; off >>= 1) {
-          const double ob = __shfl_xor_sync(0xffffffffu, best, off);
-          const int oi = __shfl_xor_sync(0xffffffffu, bi, off);
-          if (ob > best || (ob == best && oi < bi)) { best = ob; bi = oi; }
-        }
-        k = (bi == 0x7fffffff) ? 0 : bi;
         if (lane == 0 && p.codes) {
           uint8_t *cp = p.codes + (long long)(s - p.s_base) * p.code_stride_s + gi;
           if (p.st && *cp != (uint8_t)k)
@@ -217,8 +272,10 @@ __global__ void __launch_bounds__(256) k_encode_refine(EncParams p) {
       }
       if (p.subtract) {
         const float gk = ga[k];
+        float cwv[D];
+        load_row_f32<D>(sh, k, cwv);
 #pragma unroll
-        for (int j = 0; j < D; ++j) x[j] = __fsub_rn(x[j], __fmul_rn(gk, sh[k * D + j]));
+        for (int j = 0; j < D; ++j) x[j] = __fsub_rn(x[j], __fmul_rn(gk, cwv[j]));
       }
     }
     if (p.res_out && lane == 0) store_row_f32<D>(p.res_out, gi, x);
