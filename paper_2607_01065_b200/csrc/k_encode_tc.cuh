@@ -218,12 +218,13 @@ __global__ void __launch_bounds__(kThreads, 1) k_encode_tc(const __grid_constant
         if (s + 1 < S) {  // operand planes of the residual for the next stage
           uint32_t h[8], l[8];
 #pragma unroll
-          for (int j = 0; j < kD; j += 2) {
-            const __nv_bfloat16 h0 = __float2bfloat16_rn(r[j]), h1 = __float2bfloat16_rn(r[j + 1]);
-            const __nv_bfloat16 l0 = __float2bfloat16_rn(__fsub_rn(r[j], __bfloat162float(h0)));
-            const __nv_bfloat16 l1 = __float2bfloat16_rn(__fsub_rn(r[j + 1], __bfloat162float(h1)));
-            h[j / 2] = (uint32_t)__bfloat16_as_ushort(h0) | ((uint32_t)__bfloat16_as_ushort(h1) << 16);
-            l[j / 2] = (uint32_t)__bfloat16_as_ushort(l0) | ((uint32_t)__bfloat16_as_ushort(l1) << 16);
+          for (int j = 0; j < kD; j += 2) {  // one packed conversion per pair; the high half is re-read by masking
+            const __nv_bfloat162 hp = __floats2bfloat162_rn(r[j], r[j + 1]);
+            h[j / 2] = *reinterpret_cast<const uint32_t *>(&hp);
+            const float d0 = __fsub_rn(r[j], __uint_as_float(h[j / 2] << 16));
+            const float d1 = __fsub_rn(r[j + 1], __uint_as_float(h[j / 2] & 0xFFFF0000u));
+            const __nv_bfloat162 lp = __floats2bfloat162_rn(d0, d1);
+            l[j / 2] = *reinterpret_cast<const uint32_t *>(&lp);
           }
           uint8_t *ph_ = planes + r_in_tile * 32, *pl_ = planes + kPlaneBytes + r_in_tile * 32;
           *reinterpret_cast<uint4 *>(ph_ + (0u ^ sw)) = make_uint4(h[0], h[1], h[2], h[3]);
