@@ -17,8 +17,11 @@ def to_device(x_np: np.ndarray, dtype: str, head_inner: bool = False) -> torch.T
 
 
 def gpu_gsrq(x_np, w_np, d, K, S, iters, seed=0, dtype="bf16", fit_tokens=None, head_inner=False,
-             pass_residual=True, want_residual=True):
-    """fit stage by stage + fused encode of all stages on the GPU. Returns numpy results + stats."""
+             pass_residual=True, want_residual=True, prefix_encode=False):
+    """fit stage by stage + encode on the GPU. Returns numpy results + stats.
+    pass_residual: each stage is encoded right after its fit and its residual feeds the next fit
+    (prefix_encode: that encode is the fused [0, s] pass, as bench.py does; else stage s alone);
+    otherwise the fits re-derive their residual and one fused encode of all stages follows."""
     x = to_device(x_np, dtype, head_inner)
     view = B.view_of(x, d, head_inner)
     G, T, hd = view.G, view.T, view.hd
@@ -38,7 +41,7 @@ def gpu_gsrq(x_np, w_np, d, K, S, iters, seed=0, dtype="bf16", fit_tokens=None, 
         s = B.gsrq_fit_stage(x, view, w, w_stride, ft, cb, st, res_in, iters, seed, ws)
         stats.append(s)
         if pass_residual:
-            B.gsrq_encode(x, view, cb, st, st + 1, codes, residual, ws)
+            B.gsrq_encode(x, view, cb, 0 if prefix_encode else st, st + 1, codes, residual, ws)
     if not pass_residual:
         B.gsrq_encode(x, view, cb, 0, S, codes, residual if want_residual else None, ws)
     torch.cuda.synchronize()

@@ -1,0 +1,141 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times, and the edge
+cases of the tensor-core encode and the bandwidth decode.  Run with `-m gpu` on a B200.
+
+cfg 1 and cfg 2 are small enough for the oracle to run whole (seconds on the box's cores), so they are
+compared element by element.  cfg 4's layout is checked at 65,536 tokens x 8 heads (134 MB) on sampled
+tokens: a token's codes depend on that token's rows only, so the oracle encodes the sample alone."""
+import numpy as np
+import pytest
+import torch
+
+from _harness import gpu_decode, gpu_gsrq, to_device
+from oracle import gsrq_oracle as o
+from paper_2607_01065_b200 import inputs
+from test_gpu_parity import _check_free_running
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    import __graft_entry__ as ge
+    ge.build()
+    from paper_2607_01065_b200 import binding
+    return binding
+
+
+def test_cfg1_full_size_bench_flow():
+    """BASELINE config 1 whole (8 x 4096 x 128, K=256, S=2, 20 iterations), bench.py's call sequence."""
+    dd = inputs.make(1)
+    c = dd["config"]
+    got, ref = _check_free_running(dd, c.K, c.S, c.iters, "bf16", prefix_encode=True)
+    assert np.array_equal(got["codes"], ref["codes"])           # identical trajectories, not merely within tolerance
+    assert np.array_equal(got["shapes"], ref["shapes"]) and np.array_equal(got["gains"], ref["gains"])
+    dec = gpu_decode(got["codes_dev"], got["cb"], c.S, c.G, c.T, c.hd, c.d, dtype="bf16")
+    want, _ = o.decode(got["codes"], got["shapes"], got["gains"], c.hd, bf16=True)
+    assert np.array_equal(dec, want)
+
+
+def test_cfg2_full_size():
+    """BASELINE config 2 whole (V-like 8 x 16384 x 128, S=1, 20 iterations) + decode of the layer."""
+    dd = inputs.make(2)
+    c = dd["config"]
+    got, ref = _check_free_running(dd, c.K, c.S, c.iters, "bf16", prefix_encode=True)
+    dec = gpu_decode(got["codes_dev"], got["cb"], c.S, c.G, c.T, c.hd, c.d, dtype="bf16")
+    want, _ = o.decode(got["codes"], got["shapes"], got["gains"], c.hd, bf16=True)
+    assert np.array_equal(dec, want)
+
+
+def test_cfg4_layout_sampled_encode_decode(B):
+    """Head-inner [T][G][hd] tensor of 65,536 tokens: codebooks fitted on a 4,096-token sample per head
+    (both sides), full encode + decode on the GPU, oracle on 3,000 sampled tokens."""
+    T, n_fit, S, K, iters = 65536, 4096, 2, 256, 4
+    c = inputs.CONFIGS[4]
+    x = inputs.k_like(c.G, T, c.hd, inputs.seed_of(4, "k"))
+    w = inputs.token_weights(T, inputs.seed_of(4, "w"))
+    fit = inputs.fit_sample(c.G, T, n_fit, inputs.seed_of(4, "fit"))
+    got = gpu_gsrq(x, w, c.d, K, S, iters, dtype="bf16", fit_tokens=fit, head_inner=True, pass_residual=False,
+                   want_residual=False)
+    ref = o.gsrq_fit_encode(x, w, c.d, K, S, iters, seed=0, fit_tokens=fit, encode=False)
+    rng = np.random.default_rng(7)
+    tok = np.sort(rng.choice(T, 3000, replace=False))
+    assert np.abs(got["shapes"] - ref["shapes"]).max() <= 1e-4 and np.abs(got["gains"] - ref["gains"]).max() <= 1e-4
+    assert np.array_equal(got["shapes"], ref["shapes"]) and np.array_equal(got["gains"], ref["gains"])
+    # oracle encode of the sampled tokens with the GPU's codebooks (fixed-codebook encode is per row)
+    codes_o, _, best, second = o.encode(x[:, tok], got["shapes"], got["gains"], c.d)
+    M = c.hd // c.d
+    rows = (tok[:, None] * M + np.arange(M)[None]).reshape(-1)
+    codes_g = got["codes"][:, :, rows]
+    assert np.array_equal(codes_g, codes_o)
+    dec = gpu_decode(got["codes_dev"], got["cb"], S, c.G, T, c.hd, c.d, dtype="bf16", head_inner=True)
+    want, _ = o.decode(codes_o, got["shapes"], got["gains"], c.hd, bf16=True)
+    assert np.array_equal(dec[:, tok], want)
+
+
+@pytest.mark.parametrize("hd,T,K,S", [(64, 150, 256, 2), (32, 333, 37, 4), (256, 40, 256, 3), (16, 1000, 256, 1)])
+def test_tc_encode_shapes(B, hd, T, K, S):
+    """Fused tensor-core encode for M = hd/16 in {1, 2, 4, 16}, ragged tile tails, K < 256, S up to 4."""
+    rng = np.random.default_rng(hd + T)
+    G = 3
+    x = inputs.bf16_round(rng.standard_normal((G, T, hd)) * np.exp(0.5 * rng.standard_normal((G, T, 1))))
+    sh = rng.standard_normal((G, S, K, 16))
+    sh = (sh / np.linalg.norm(sh, axis=-1, keepdims=True)).astype(np.float32)
+    ga = np.abs(rng.standard_normal((G, S, K)) * (2.0 / (1 + np.arange(S))[None, :, None])).astype(np.float32)
+    codes_o, res_o, _, _ = o.encode(x, sh, ga, 16)
+    xd = to_device(x, "bf16")
+    view = B.view_of(xd, 16)
+    sh_d, ga_d = torch.from_numpy(sh).cuda(), torch.from_numpy(ga).cuda()   # keep alive: cb holds raw pointers
+    cb = B.codebook_of(sh_d, ga_d)
+    ws = B.workspace(view, K, S, -1)
+    M = hd // 16
+    codes = torch.zeros(S, G, T * M, dtype=torch.uint8, device="cuda")
+    res = torch.zeros(G, T * M, 16, device="cuda")
+    B.gsrq_encode(xd, view, cb, 0, S, codes, res, ws)
+    torch.cuda.synchronize()
+    assert np.array_equal(codes.cpu().numpy(), codes_o)
+    assert np.array_equal(res.cpu().numpy(), res_o)
+
+
+def test_tc_encode_all_rows_ambiguous(B):
+    """Duplicate codewords make every row an exact tie: all rows go through the exact path, lowest index wins."""
+    rng = np.random.default_rng(3)
+    G, T, hd, K, S = 2, 200, 128, 64, 2
+    x = inputs.bf16_round(rng.standard_normal((G, T, hd)))
+    sh = rng.standard_normal((G, S, K // 2, 16))
+    sh = (sh / np.linalg.norm(sh, axis=-1, keepdims=True)).astype(np.float32)
+    sh = np.concatenate([sh, sh], axis=2)                      # codeword k + K/2 == codeword k
+    ga = np.abs(rng.standard_normal((G, S, K // 2))).astype(np.float32)
+    ga = np.concatenate([ga, ga], axis=2)
+    codes_o, res_o, _, _ = o.encode(x, sh, ga, 16)
+    assert codes_o.max() < K // 2
+    xd = to_device(x, "bf16")
+    view = B.view_of(xd, 16)
+    sh_d, ga_d = torch.from_numpy(sh).cuda(), torch.from_numpy(ga).cuda()   # keep alive: cb holds raw pointers
+    cb = B.codebook_of(sh_d, ga_d)
+    ws = B.workspace(view, K, S, -1)
+    codes = torch.zeros(S, G, T * 8, dtype=torch.uint8, device="cuda")
+    res = torch.zeros(G, T * 8, 16, device="cuda")
+    B.gsrq_encode(xd, view, cb, 0, S, codes, res, ws)
+    torch.cuda.synchronize()
+    assert np.array_equal(codes.cpu().numpy(), codes_o) and np.array_equal(res.cpu().numpy(), res_o)
+
+
+@pytest.mark.parametrize("T,S,dtype,head_inner", [(100, 1, "bf16", False), (100, 2, "f32", False), (515, 3, "bf16", True),
+                                                  (32, 4, "bf16", False), (31, 2, "bf16", False), (4096, 4, "bf16", True)])
+def test_decode_bandwidth_path_and_tail(B, T, S, dtype, head_inner):
+    """Decode: full 256-row chunks through k_decode_fast, the ragged tail through the generic kernel;
+    N % 16 != 0 (T = 31... with M = 8 always a multiple of 8 only) falls back entirely.  Bit-exact."""
+    rng = np.random.default_rng(T * 10 + S)
+    G, hd, K = 2, 128, 256
+    M = hd // 16
+    sh = rng.standard_normal((G, S, K, 16))
+    sh = (sh / np.linalg.norm(sh, axis=-1, keepdims=True)).astype(np.float32)
+    ga = np.abs(rng.standard_normal((G, S, K))).astype(np.float32)
+    codes = rng.integers(0, K, size=(S, G, T * M), dtype=np.uint8)
+    sh_d, ga_d = torch.from_numpy(sh).cuda(), torch.from_numpy(ga).cuda()   # keep alive: cb holds raw pointers
+    cb = B.codebook_of(sh_d, ga_d)
+    cd = torch.from_numpy(codes).cuda()
+    for n in range(1, S + 1):
+        dec = gpu_decode(cd, cb, n, G, T, hd, 16, dtype=dtype, head_inner=head_inner)
+        want, _ = o.decode(codes, sh, ga, hd, S_used=n, bf16=(dtype == "bf16"))
+        assert np.array_equal(dec, want), (T, n)
