@@ -186,6 +186,7 @@ def main():
     ap.add_argument("--cfg", type=int, default=1, choices=[1, 2])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-big", action="store_true", help="skip the config-4 (2.1 GB) encode / decode leg")
+    ap.add_argument("--only-big", action="store_true", help="run only the config-4 leg and print its JSON (profiling aid)")
     args = ap.parse_args()
     c = inputs.CONFIGS[args.cfg]
     rank = int(os.environ.get("RANK", "0"))
@@ -207,6 +208,10 @@ def main():
         dist.barrier()
     torch.cuda.set_device(local)
     B.lib()
+    if args.only_big:
+        if rank == 0:
+            print(json.dumps(dict(impl="ours", cfg4=run_cfg4(B, peaks()))))
+        return
 
     # ---- inputs (replicas: rank r works on its own layer; rank 0 is the documented seeds) ----
     kind = c.kinds[0]
