@@ -174,8 +174,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_encode_tc(const __grid_constant
         for (int j = 0; j < kD; ++j) n2 = fmaf(r[j], r[j], n2);
         const float rn = sqrtf(n2) * 1.00001f;  // upper bound of ||r||
         const float gm = __int_as_float(p.gmax[g * S + s]);
-        const float e1 = (s == 0 ? 2.0f : 4.5f) * 7.62939453125e-6f * 2.0f * gm;
-        const float e0 = 3.814697265625e-6f * gm * gm;
+        const float rho17 = (s == 0 ? 2.0f : 4.5f) * 7.62939453125e-6f;  // rho 2^-17: one / two operand planes
         mbar_wait(tmem_full(wg), (uint32_t)((pr * S + s) & 1));
         tc_fence_after();
         if (s == 0) {  // stage-0 MMAs are done with the tile and this warp has its rows: free the ring slot
@@ -193,19 +192,17 @@ __global__ void __launch_bounds__(kThreads, 1) k_encode_tc(const __grid_constant
           }
         });
         const int k = gi * 16 + ji;
-        const float E2 = 2.0f * fmaf(e1, rn, e0);
+        const long long cw = ((long long)g * p.S + s) * p.K + min(k, p.K - 1);
+        const float gk = __ldg(p.gains + cw);
+        const float E2 = decision_margin(best, rn, gk, gm, rho17, 0);
         if (alive && best - second <= E2) {  // ambiguous: the exact path takes the row over from this stage
-          uint32_t gmask = 0;  // groups of 16 columns whose maximum is within 2E of the best: the only candidates
-#pragma unroll
-          for (int c = 0; c < 16; ++c) gmask |= (gmA[c] >= best - E2) ? (1u << c) : 0u;
+          const uint32_t gmask = candidate_groups(gmA, best, E2);  // groups of 16 columns within the margin: the only candidates
           const unsigned int pos = atomicAdd(p.list_cnt, 1u);
           p.list[pos] = make_uint2((uint32_t)gr, gmask | ((uint32_t)s << 16));
           alive = false;
         }
         if (alive) p.codes[(long long)s * p.code_stride_s + gr] = (uint8_t)k;
         // r <- fl32(r - fl32(g_k s_k)): the codeword comes from the fp32 codebook (L1-resident)
-        const long long cw = ((long long)g * p.S + s) * p.K + min(k, p.K - 1);
-        const float gk = __ldg(p.gains + cw);
         const float4 *sp = reinterpret_cast<const float4 *>(p.shapes + cw * kD);
 #pragma unroll
         for (int v = 0; v < 4; ++v) {

@@ -259,6 +259,34 @@ __device__ __forceinline__ void tile_argmax(uint32_t taddr, float (&gmA)[16], fl
   second = fmaxf(secA, secB);
 }
 
+// Decision margin of the filter for one row: best - second must exceed the sum of the error bounds of the
+// winner's score and of any competitor's score.  The bound of a score with gain g is
+//   E(g) = rho 2^-17 (2 g ||r||) + 2^-18 g^2.
+// The winner's gain g1 is known.  For a competitor, g_max would do, but it is far too pessimistic when a few
+// clusters (outlier channels) have large gains: in exact arithmetic a codeword with gain g scores at most
+// u(g) = 2 g ||r|| - g^2, which decreases for g > ||r||, so a codeword with g >= g_cap = ||r|| + sqrt(||r||^2 - B),
+// B < best - E(g1) <= exact score of the winner, is strictly below the winner whatever its shape.  Only gains
+// <= min(g_cap, g_max) matter.  rn is an upper bound of ||r||; every rounding here goes to the safe side.
+__device__ __forceinline__ float decision_margin(float best, float rn, float g1, float gmax, float rho17, int mode) {
+  if (mode != 0) return 2.0f * rho17 * 2.0f * rn + 1.0e-36f;  // projection scores: g = 1 on both sides, no g^2 term
+  const float E1 = fmaf(rho17 * 2.0f * g1, rn, 3.814697265625e-6f * g1 * g1);
+  const float B = best - E1 - 9.5367431640625e-7f * (fabsf(best) + rn * rn);
+  const float gcap = fminf(gmax, (rn + sqrtf(fmaxf(fmaf(rn, rn, -B), 0.0f))) * 1.00001f);
+  // the floor keeps exact ties (e.g. several zero-gain codewords scoring 0) ambiguous: the index bits packed into
+  // the low mantissa make tied scores differ by a few denormal ulps
+  return (E1 + fmaf(rho17 * 2.0f * gcap, rn, 3.814697265625e-6f * gcap * gcap)) * 1.00001f + 1.0e-36f;
+}
+
+// Candidate groups for the exact path: group maxima (unpacked) within the margin of the (packed) best; the packing
+// may have raised `best` by up to 2^-19 |best|, hence the extra slack.
+__device__ __forceinline__ uint32_t candidate_groups(const float (&gmA)[16], float best, float E2) {
+  const float thr = fmaf(-3.814697265625e-6f, fabsf(best), best - E2) - 1.0e-36f;
+  uint32_t gmask = 0;
+#pragma unroll
+  for (int c = 0; c < 16; ++c) gmask |= (gmA[c] >= thr) ? (1u << c) : 0u;
+  return gmask;
+}
+
 // Exact path for one row, run by a whole warp: fp64, dot product summed in element order without
 // FMA contraction, score = (2 g)(r.s) - g g -- the definition's own operation order; lowest k wins ties.
 // Only the columns of the 16-column groups in `gmask` are candidates: a column whose filter score is
@@ -377,10 +405,8 @@ k_score_tc(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CU
     // so that two tiles are in flight per SM sub-partition.  Thread = row (TMEM lane).
     const int q = warp & 3;        // TMEM lane quarter this warp may access
     const int wg = (warp - 2) >> 2;
-    // E_i = e1 ||r_i|| + e0,  e1 = rho 2^-17 (2 g_max),  e0 = 2^-18 g_max^2
     const float gm = (p.mode == 0) ? __int_as_float(p.gmax[(long long)g * p.gmax_stride]) : 1.0f;
-    const float e1 = (p.n_planes == 1 ? 2.0f : 4.5f) * 7.62939453125e-6f * 2.0f * gm;
-    const float e0 = (p.mode == 0) ? 3.814697265625e-6f * gm * gm : 0.0f;
+    const float rho17 = (p.n_planes == 1 ? 2.0f : 4.5f) * 7.62939453125e-6f;  // rho 2^-17
     // the exact path reads the group's fp32 codebook from shared memory: staged here, while the first tile is in flight
     float *sh_g = reinterpret_cast<float *>(sgen + kSmemSh);
     float *ga_g = sh_g + kN * kD;
@@ -411,16 +437,14 @@ k_score_tc(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CU
         if (lane == 0) mbar_arrive(tmem_empty(buf));
       });
       int k_new = gi * 16 + ji;
-      const float E2 = 2.0f * fmaf(e1, rn, e0);
+      const float E2 = decision_margin(best, rn, ga_g[min(k_new, p.K - 1)], gm, rho17, p.mode);
       const bool flag = (row < p.N) && (best - second <= E2);
       unsigned int m = __ballot_sync(0xffffffffu, flag);
       n_refined += __popc(m);
       if (m) {  // ambiguous rows: the exact path decides among the groups within 2E of the best.
         // They are queued and re-scored after the CTA's last tile by all epilogue warps at once, so that
         // a re-score never stalls the accumulator pipeline; a full queue falls back to doing it here.
-        uint32_t gmask = 0;
-#pragma unroll
-        for (int c = 0; c < 16; ++c) gmask |= (gmA[c] >= best - E2) ? (1u << c) : 0u;
+        const uint32_t gmask = candidate_groups(gmA, best, E2);
         bool queued = false;
         if (flag) {
           const unsigned int pos = atomicAdd(qcnt, 1u);

@@ -139,3 +139,47 @@ def test_decode_bandwidth_path_and_tail(B, T, S, dtype, head_inner):
         dec = gpu_decode(cd, cb, n, G, T, hd, 16, dtype=dtype, head_inner=head_inner)
         want, _ = o.decode(codes, sh, ga, hd, S_used=n, bf16=(dtype == "bf16"))
         assert np.array_equal(dec, want), (T, n)
+
+
+def test_decision_margin_stress(B):
+    """The filter's decision margin caps the competitor's gain by what can still beat the winner; stress it with
+    gains spread over orders of magnitude (zeros included), rows from tiny to huge norms, zero rows and
+    near-duplicate codewords, in both the 1-plane (bf16 rows) and 2-plane (fp32 residual) paths.  The result
+    must equal the exact arg-max everywhere (ties -> lowest index)."""
+    rng = np.random.default_rng(11)
+    G, T, hd, K, S = 4, 2048, 128, 256, 2
+    x = rng.standard_normal((G, T, hd)) * np.exp(1.5 * rng.standard_normal((G, T, 1)))
+    x[:, ::97] = 0.0
+    x[:, 5::211] *= 1e-3
+    x = inputs.bf16_round(x)
+    sh = rng.standard_normal((G, S, K, 16))
+    sh[:, :, 128:192] = sh[:, :, 0:64] + 1e-4 * rng.standard_normal((G, S, 64, 16))   # near-duplicates
+    sh = (sh / np.linalg.norm(sh, axis=-1, keepdims=True)).astype(np.float32)
+    ga = np.exp(2.0 * rng.standard_normal((G, S, K))).astype(np.float32)
+    ga[:, :, 128:192] = ga[:, :, 0:64]
+    ga[:, :, 7::31] = 0.0
+    codes_o, res_o, _, _ = o.encode(x, sh, ga, 16)
+    xd = to_device(x, "bf16")
+    view = B.view_of(xd, 16)
+    sh_d, ga_d = torch.from_numpy(sh).cuda(), torch.from_numpy(ga).cuda()
+    cb = B.codebook_of(sh_d, ga_d)
+    ws = B.workspace(view, K, S, 0)
+    codes = torch.zeros(S, G, T * 8, dtype=torch.uint8, device="cuda")
+    res = torch.zeros(G, T * 8, 16, device="cuda")
+    B.gsrq_encode(xd, view, cb, 0, S, codes, res, ws)          # fused tensor-core encode
+    torch.cuda.synchronize()
+    assert np.array_equal(codes.cpu().numpy(), codes_o) and np.array_equal(res.cpu().numpy(), res_o)
+    # fit-path scoring kernel: stage 0 from the bf16 rows (1 plane), stage 1 from the fp32 residual (2 planes)
+    idx = torch.zeros(G, T * 8, dtype=torch.uint8, device="cuda")
+    B.gsrq_assign(xd, view, None, cb, 0, 0, idx, ws)
+    assert np.array_equal(idx.cpu().numpy(), codes_o[0])
+    _, res0, _, _ = o.encode(x, sh, ga, 16, stage_end=1)
+    res0_d = torch.from_numpy(np.ascontiguousarray(res0)).cuda()
+    B.gsrq_assign(xd, view, res0_d, cb, 1, 0, idx, ws)
+    assert np.array_equal(idx.cpu().numpy(), codes_o[1])
+    # projection mode (Alg. 1 l.2 assignment)
+    B.gsrq_assign(xd, view, None, cb, 0, 1, idx, ws)
+    rows = o.rows_of(x, 16)
+    for g_ in range(G):
+        a, _, _ = o.assign(rows[g_], sh[g_, 0], None)
+        assert np.array_equal(idx[g_].cpu().numpy(), a.astype(np.uint8))
