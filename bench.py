@@ -177,6 +177,61 @@ def run_cfg4(B, pk):
                 rel_residual_energy_first_4096_tokens=err)
 
 
+def run_cfg3(B, pk):
+    """BASELINE.json config 3 for the K-like tensor (8 x 32768 x 128, bf16): one S=4 fit (20 iterations per stage),
+    then encode throughput and decode GB/s for S = 1..4 (prefixes of the same codebooks) and the
+    weighted distortion after each stage."""
+    c = inputs.CONFIGS[3]
+    G, T, hd, d, K, S, iters = c.G, c.T, c.hd, c.d, c.K, c.S, c.iters
+    M = hd // d
+    x = torch.from_numpy(inputs.k_like(G, T, hd, inputs.seed_of(3, "k"))).to(torch.bfloat16).cuda()
+    w = torch.from_numpy(inputs.token_weights(T, inputs.seed_of(3, "w"))).cuda()
+    view = B.view_of(x, d)
+    shapes = torch.zeros(G, S, K, d, device="cuda")
+    gains = torch.zeros(G, S, K, device="cuda")
+    cb = B.codebook_of(shapes, gains)
+    ws = B.workspace(view, K, S, 0)
+    codes = torch.zeros(S, G, T * M, dtype=torch.uint8, device="cuda")
+    residual = torch.zeros(G, T * M, d, device="cuda")
+    out = torch.empty_like(x)
+    w_rows = w.repeat_interleave(M).double()
+    e0 = float((w_rows[None] * (x.float().reshape(G, T * M, d).double() ** 2).sum(-1)).sum())
+
+    def fit_all(want_dist):
+        dist = []
+        for s in range(S):
+            B.gsrq_fit_stage(x, view, w, 0, None, cb, s, residual if s else None, iters, 0, ws, want_stats=False)
+            B.gsrq_encode(x, view, cb, 0, s + 1, codes, residual, ws)
+            if want_dist:
+                dist.append(float((w_rows[None] * (residual.double() ** 2).sum(-1)).sum()) / e0)
+        return dist
+
+    dist = fit_all(True)
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(); fit_all(False); b.record()
+    torch.cuda.synchronize()
+    fit_ms = a.elapsed_time(b)
+    rows = G * T * M
+    sweep = []
+    for n in range(1, S + 1):
+        ts, td = [], []
+        for _ in range(5):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); B.gsrq_encode(x, view, cb, 0, n, codes, None, ws); b.record()
+            torch.cuda.synchronize(); ts.append(a.elapsed_time(b))
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); B.gsrq_decode(codes, cb, n, out, view); b.record()
+            torch.cuda.synchronize(); td.append(a.elapsed_time(b))
+        em, dm = float(np.median(ts)), float(np.median(td))
+        by = rows * n + rows * 2 * d
+        sweep.append(dict(S=n, bits_per_element=n * 8.0 / d, encode_ms=em, encode_kv_vectors_per_s=G * T / (em * 1e-3),
+                          encode_tensor_frac=2.0 * K * d * rows * n / (em * 1e-3) / 1e12 / pk["bf16_tflops_sustained"],
+                          decode_ms=dm, decode_gb_per_s=by / (dm * 1e-3) / 1e9, decode_hbm_frac=by / (dm * 1e-3) / 1e9 / pk["hbm_gbs"],
+                          rel_weighted_distortion=dist[n - 1]))
+    return dict(workload="cfg3:k-cache-8x32768x128, S=4 fit, prefixes S=1..4 (67 MB: L2-resident, effective GB/s)",
+                fit_and_encode_ms=fit_ms, sweep=sweep)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -316,11 +371,13 @@ def main():
 
     if rank != 0:
         return
-    big = None
+    big = sweep3 = None
     if not args.no_big:
         del flush
         torch.cuda.empty_cache()
         big = run_cfg4(B, peaks())
+        torch.cuda.empty_cache()
+        sweep3 = run_cfg3(B, peaks())
     pk = peaks()
     # Rooflines of the step's kernels, from the live CUDA-event brackets (two profiled steps).
     # Algorithmic work: scoring pass 2*K*d flops per sub-vector; update kernel one read of
@@ -367,6 +424,7 @@ def main():
                             hbm_frac=dec_bytes / (dec_ms * 1e-3) / 1e9 / pk["hbm_gbs"]))
     if big is not None:
         line["cfg4"] = big
+        line["cfg3"] = sweep3
     if not args.no_cpu_baseline:
         from oracle import gsrq_oracle as o
         t0 = time.perf_counter()
