@@ -108,6 +108,22 @@ def run_reference(args, c):
     print(json.dumps(line))
 
 
+def rank_seed(cfg: int, what: str, rank: int) -> int:
+    """Replicas: rank r works on its own synthetic layer; rank 0 uses the documented seeds."""
+    return inputs.seed_of(cfg, what) + 100 * rank
+
+
+def whole_job_value(local_seconds: float, units_per_rank: float, world: int, device) -> tuple:
+    """Weak scaling without a data-path collective: every rank processes units_per_rank units; the job takes as
+    long as its slowest rank (MAX over ranks of the device-timed duration).  Returns (value, max_seconds)."""
+    t = torch.tensor([local_seconds], device=device, dtype=torch.float64)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    mx = float(t.item())
+    return world * units_per_rank / mx, mx
+
+
 def run_cfg4(B, pk):
     """BASELINE.json config 4 for one tensor (K-like): batch 8 x 131072 tokens x 8 KV heads x 128, bf16, head-inner
     layout [B*T][G][hd] (2.147 GB); d=16, K=256, S=2, 10 iterations; codebooks fitted on a seeded 65,536-token
@@ -271,8 +287,8 @@ def main():
     # ---- inputs (replicas: rank r works on its own layer; rank 0 is the documented seeds) ----
     kind = c.kinds[0]
     gen = inputs.k_like if kind == "k" else inputs.v_like
-    x_np = gen(c.G, c.T, c.hd, inputs.seed_of(c.cfg, kind) + 100 * rank)
-    w_np = inputs.token_weights(c.T, inputs.seed_of(c.cfg, "w") + 100 * rank)
+    x_np = gen(c.G, c.T, c.hd, rank_seed(c.cfg, kind, rank))
+    w_np = inputs.token_weights(c.T, rank_seed(c.cfg, "w", rank))
     x_host = torch.from_numpy(x_np).to(torch.bfloat16).pin_memory()
     w_host = torch.from_numpy(w_np).pin_memory()
     x = x_host.cuda()
@@ -316,12 +332,8 @@ def main():
     barrier()
     launches = B.gsrq_launch_count() - l0
     ms = sum(a.elapsed_time(b) for a, b in evs)
-    tt = torch.tensor([ms], device="cuda", dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    ms = float(tt.item())
-    ms_per_step = ms / args.steps
-    value = world * G * T / (ms_per_step * 1e-3)
+    value, max_s = whole_job_value(ms * 1e-3 / args.steps, G * T, world, "cuda")
+    ms_per_step = max_s * 1e3
 
     # ---- per-kernel device time, measured live with CUDA events around every launch ----
     B.gsrq_profile_enable(True)
@@ -361,10 +373,7 @@ def main():
         B.gsrq_pipeline_host(x_host, view, w_host, K, S, c.iters, 0, sh_h, ga_h, co_h, out_h)
     barrier()
     e2e_s = (time.perf_counter() - t0) / n_e2e
-    te = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_val = world * G * T / float(te.item())
+    e2e_val, _ = whole_job_value(e2e_s, G * T, world, "cuda")
     h2d = x_host.numel() * 2 + w_host.numel() * 4
     d2h = sh_h.numel() * 4 + ga_h.numel() * 4 + co_h.numel() + out_h.numel() * 2
     clocks = sampler.finish()
