@@ -691,6 +691,18 @@ int gsrq_pipeline_host(const void *kv_host, const gsrq_view *view, const float *
   size_t off[8], o = 0;
   const size_t sizes[8] = {kv_bytes, (size_t)view->T * 4, sh_bytes, ga_bytes, n_rows * S, n_rows * d * 4, wsb, kv_bytes};
   for (int i = 0; i < 8; ++i) { off[i] = o; o += align_up(sizes[i]); }
+  {  // keep the stream-ordered pool's memory across calls (by default it is returned to the driver at every sync)
+    static bool pool_set = false;
+    if (!pool_set) {
+      int dev = 0;
+      cudaMemPool_t pool;
+      if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+        unsigned long long keep = ~0ull;
+        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+      }
+      pool_set = true;
+    }
+  }
   cudaError_t e = cudaMallocAsync((void **)&base, o, stream);
   if (e != cudaSuccess) { set_error("gsrq_pipeline_host: %s", cudaGetErrorString(e)); return GSRQ_ECUDA; }
   void *d_kv = base + off[0];
