@@ -25,8 +25,8 @@ constexpr int kRoundRows = 1024;    // rows staged in shared memory per round
 
 struct UpdParams {
   const float *Rf;        // [G][Nf][D] fp32 rows
-  const double *rinv;     // [G][Nf]   1/(||r||+eps)
-  const float *wt;        // [G][Nf/M] per-fit-token weights
+  const double2 *coef;    // [G][Nf]   per-row {w_i, w_i/(||r_i||+eps)}
+  const float *wt;        // [G][Nf/M] per-fit-token weights (unused by the kernel; kept by the preparation)
   const uint8_t *idx;     // [G][Nf]
   long long Nf;
   int M, K;
@@ -113,10 +113,7 @@ __global__ void __launch_bounds__(kUpdThreads) k_update(UpdParams p) {
   const uint32_t pat = (uint32_t)(k0 & 0xF0) * 0x01010101u;
   const uint32_t miss = (uint32_t)((k0 ^ 0x80) & 0xFF);  // a byte outside [k0, k0 + 16)
   const float *rows = p.Rf + (long long)g * p.Nf * D;
-  const double *ri = p.rinv + (long long)g * p.Nf;
-  const float *wg = p.wt + (long long)g * (p.Nf / p.M);
-  const unsigned int Mu = (unsigned int)p.M;
-  const int msh = ((Mu & (Mu - 1)) == 0) ? (31 - __clz((int)Mu)) : -1;  // M is a power of two: shift
+  const double2 *cf_g = p.coef + (long long)g * p.Nf;
 
   double s[Q];  // warp c, lane e: element e (+32q) of [A | B] of cluster k0 + c
   int isB[Q], col[Q];
@@ -219,19 +216,14 @@ __global__ void __launch_bounds__(kUpdThreads) k_update(UpdParams p) {
         constexpr int GI = kRoundRows * LPR / kUpdThreads;  // items per thread; q is the same for all of them
         const int q = tid % LPR;
         float4 v[GI];
-        float wv[GI];
-        double rv[GI];
+        double2 cv[GI];
 #pragma unroll
         for (int u = 0; u < GI; ++u) {
           const int e = (tid + u * kUpdThreads) / LPR;
           if (e < n) {
             const long long row = pb + list[lo + e];
             v[u] = __ldg(reinterpret_cast<const float4 *>(rows + row * D + 4 * q));
-            if (q == 0) {
-              const unsigned int tok = (msh >= 0) ? ((unsigned int)row >> msh) : ((unsigned int)row / Mu);
-              wv[u] = __ldg(wg + tok);
-              rv[u] = __ldg(ri + row);
-            }
+            if (q == 0) cv[u] = __ldg(cf_g + row);
           }
         }
 #pragma unroll
@@ -239,7 +231,7 @@ __global__ void __launch_bounds__(kUpdThreads) k_update(UpdParams p) {
           const int e = (tid + u * kUpdThreads) / LPR;
           if (e < n) {
             *reinterpret_cast<float4 *>(xbuf + e * D + 4 * q) = v[u];
-            if (q == 0) *reinterpret_cast<double2 *>(coef + 2 * e) = make_double2((double)wv[u], (double)wv[u] * rv[u]);
+            if (q == 0) *reinterpret_cast<double2 *>(coef + 2 * e) = cv[u];
           }
         }
       }
