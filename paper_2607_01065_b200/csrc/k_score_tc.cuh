@@ -74,17 +74,14 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
-// try_wait with a suspend-time hint: the hardware parks the thread until the phase completes (or the hint
-// expires) instead of spinning, so that waiting producer / MMA / epilogue warps do not take issue slots from
-// the arg-max epilogue, which is issue-bound.
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   asm volatile(
       "{\n\t.reg .pred P1;\n\t"
       "WAIT_LOOP:\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1, %2;\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
       "@P1 bra DONE;\n\t"
       "bra WAIT_LOOP;\n\t"
-      "DONE:\n\t}" ::"r"(bar), "r"(parity), "r"(0x989680u) : "memory");
+      "DONE:\n\t}" ::"r"(bar), "r"(parity) : "memory");
 }
 // non-blocking probe of a phase
 __device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {
