@@ -21,7 +21,8 @@ namespace gsrq {
 constexpr int kCPC = 16;            // clusters per CTA = warps per CTA (warp c sums cluster k0 + c)
 constexpr int kUpdThreads = 512;
 constexpr int kPassRows = 16384;    // rows scanned per pass (32 per thread)
-constexpr int kRoundRows = 1024;    // rows staged in shared memory per round
+constexpr int kRoundRows = 1024;    // staged rows in shared memory: two buffers of kHalfRows
+constexpr int kHalfRows = kRoundRows / 2;
 
 struct UpdParams {
   const float *Rf;        // [G][Nf][D] fp32 rows
@@ -69,6 +70,10 @@ __device__ __forceinline__ void write_bimg_elem(uint8_t *img, int k, int j, floa
   *reinterpret_cast<__nv_bfloat16 *>(img + 2 * kBImgBytesU + sw32_off(k, j)) = v;
 }
 
+__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gsrc) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gsrc) : "memory");
+}
+
 // 4 assignment bytes of rows [r, r+4) of one group; rows >= Nf read as `miss`.
 __device__ __forceinline__ uint32_t load_idx_word(const uint8_t *ig, long long r, long long Nf, bool aligned, uint32_t miss) {
   if (aligned && r + 4 <= Nf) return *reinterpret_cast<const uint32_t *>(ig + r);
@@ -90,7 +95,7 @@ constexpr size_t upd_smem_bytes() {
 
 // grid = (ceil(K / kCPC), G), block = kUpdThreads, dynamic smem = upd_smem_bytes<D>().
 template <int D>
-__global__ void __launch_bounds__(kUpdThreads) k_update(UpdParams p) {
+__global__ void __launch_bounds__(kUpdThreads, 1) k_update(UpdParams p) {
   extern __shared__ __align__(16) uint8_t upd_sm[];
   constexpr int P = 2 * D + 2;
   constexpr int Q = (2 * D + 31) / 32;
@@ -209,33 +214,36 @@ __global__ void __launch_bounds__(kUpdThreads) k_update(UpdParams p) {
     for (int c2 = 0; c2 < kCPC; ++c2)
       if (c2 == warp) { seg0 = cbase[c2]; seg1 = cbase[c2 + 1]; }
     __syncthreads();
-    for (int lo = 0; lo < total; lo += kRoundRows) {
-      const int n = min(kRoundRows, total - lo);
-      // ---- stage the round's rows: every load of the round is issued before the first store ----
-      {
-        constexpr int GI = kRoundRows * LPR / kUpdThreads;  // items per thread; q is the same for all of them
-        const int q = tid % LPR;
-        float4 v[GI];
-        double2 cv[GI];
+    // Rounds of kHalfRows staged rows, double-buffered: the asynchronous copies of round r + 1 (rows and their
+    // coefficient pairs, 16 bytes each, global -> shared) are in flight while round r is added up.
+    auto issue = [&](int lo_r, int buf) {
+      const int n_r = min(kHalfRows, total - lo_r);
+      const int q = tid % LPR;
+      float *xb = xbuf + buf * kHalfRows * D;
+      double *cb = coef + buf * kHalfRows * 2;
 #pragma unroll
-        for (int u = 0; u < GI; ++u) {
-          const int e = (tid + u * kUpdThreads) / LPR;
-          if (e < n) {
-            const long long row = pb + list[lo + e];
-            v[u] = __ldg(reinterpret_cast<const float4 *>(rows + row * D + 4 * q));
-            if (q == 0) cv[u] = __ldg(cf_g + row);
-          }
-        }
-#pragma unroll
-        for (int u = 0; u < GI; ++u) {
-          const int e = (tid + u * kUpdThreads) / LPR;
-          if (e < n) {
-            *reinterpret_cast<float4 *>(xbuf + e * D + 4 * q) = v[u];
-            if (q == 0) *reinterpret_cast<double2 *>(coef + 2 * e) = cv[u];
-          }
+      for (int u = 0; u < kHalfRows * LPR / kUpdThreads; ++u) {
+        const int e = (tid + u * kUpdThreads) / LPR;
+        if (e < n_r) {
+          const long long row = pb + list[lo_r + e];
+          cp_async16(xb + e * D + 4 * q, rows + row * D + 4 * q);
+          if (q == 0) cp_async16(cb + 2 * e, cf_g + row);
         }
       }
+      asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    if (total > 0) issue(0, 0);
+    for (int lo = 0, rd = 0; lo < total; lo += kHalfRows, ++rd) {
+      const int n = min(kHalfRows, total - lo);
+      if (lo + kHalfRows < total) {
+        issue(lo + kHalfRows, (rd + 1) & 1);
+        asm volatile("cp.async.wait_group 1;" ::: "memory");
+      } else {
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+      }
       __syncthreads();
+      const float *xbuf_r = xbuf + (rd & 1) * kHalfRows * D;
+      const double *coef_r = coef + (rd & 1) * kHalfRows * 2;
       // ---- warp c adds cluster c's rows of this round in list (= ascending row) order ----
       const int a = max(seg0, lo), b = min(seg1, lo + n);
       int pos = a;
@@ -247,8 +255,8 @@ __global__ void __launch_bounds__(kUpdThreads) k_update(UpdParams p) {
           const int e = pos + u - lo;
 #pragma unroll
           for (int q = 0; q < Q; ++q) {
-            cf[u][q] = live[q] ? coef[2 * e + isB[q]] : 0.0;
-            xv[u][q] = live[q] ? xbuf[e * D + col[q]] : 0.0f;
+            cf[u][q] = live[q] ? coef_r[2 * e + isB[q]] : 0.0;
+            xv[u][q] = live[q] ? xbuf_r[e * D + col[q]] : 0.0f;
           }
         }
 #pragma unroll
@@ -262,9 +270,9 @@ __global__ void __launch_bounds__(kUpdThreads) k_update(UpdParams p) {
         const int e = pos - lo;
 #pragma unroll
         for (int q = 0; q < Q; ++q) {
-          const double cf = live[q] ? coef[2 * e + isB[q]] : 0.0;
+          const double cf = live[q] ? coef_r[2 * e + isB[q]] : 0.0;
           if (q == 0) Wk += cf;
-          s[q] += cf * (double)(live[q] ? xbuf[e * D + col[q]] : 0.0f);
+          s[q] += cf * (double)(live[q] ? xbuf_r[e * D + col[q]] : 0.0f);
         }
       }
       if (a < b) cntk += b - a;
