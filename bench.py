@@ -360,6 +360,19 @@ def main():
         torch.cuda.synchronize()
         ets.append(a.elapsed_time(b))
     enc_ms = float(np.median(ets))
+    # encode-on-append (PAPER.md:443 (i)): latency of quantising the newest token(s) of a batch of sequences
+    app = []
+    for n_new in (8, 16, 32):
+        chunk = x[:, :n_new]
+        cv = B.view_of(chunk, d)
+        B.gsrq_encode_append(chunk, cv, cb, S, codes, T * M, 0)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(20):
+            B.gsrq_encode_append(chunk, cv, cb, S, codes, T * M, 0)
+        b.record()
+        torch.cuda.synchronize()
+        app.append(dict(new_tokens=n_new, us_per_call=a.elapsed_time(b) * 1e3 / 20))
 
     # ---- end to end through the host-buffer C-ABI call: H2D + fit + encode + decode + D2H ----
     sh_h = torch.empty(G, S, K, d).pin_memory(); ga_h = torch.empty(G, S, K).pin_memory()
@@ -430,7 +443,8 @@ def main():
                 encode=dict(kv_vectors_per_s=G * T / (enc_ms * 1e-3), ms=enc_ms, stages=S,
                             tensor_frac=(2.0 * K * d * rows_per_launch * S / (enc_ms * 1e-3) / 1e12) / pk["bf16_tflops"]),
                 decode=dict(gb_per_s=dec_bytes / (dec_ms * 1e-3) / 1e9, ms=dec_ms, bytes=dec_bytes,
-                            hbm_frac=dec_bytes / (dec_ms * 1e-3) / 1e9 / pk["hbm_gbs"]))
+                            hbm_frac=dec_bytes / (dec_ms * 1e-3) / 1e9 / pk["hbm_gbs"]),
+                append=app)
     if big is not None:
         line["cfg4"] = big
         line["cfg3"] = sweep3

@@ -136,6 +136,17 @@ int gsrq_encode(const void *kv, const gsrq_view *view, const gsrq_codebook *cb, 
 int gsrq_decode(const uint8_t *codes, const gsrq_codebook *cb, int n_stages, void *kv_out,
                 const gsrq_view *out_view, void *stream);
 
+/*
+ * Encode-on-append (PAPER.md:443 (i): the "residual quantization ... of newly generated KV vectors" kernel of
+ * the paper's decoding loop; K = 256 codes are bytes, so bit-packing is the identity): encode the n_new tokens
+ * described by `new_view` (new_view->T = n_new; same G / hd / d / dtype rules as above) with stages [0, n_stages)
+ * of cb and store their codes at token positions [t0, t0 + n_new) of the cache's code planes:
+ *   codes[(s * G + g) * plane_rows + (t0 + t) * M + m],   plane_rows = T_cache * M   (the layout gsrq_decode reads).
+ * One small launch, no workspace; same exact arg-max as gsrq_encode (the codes are identical).
+ */
+int gsrq_encode_append(const void *kv_new, const gsrq_view *new_view, const gsrq_codebook *cb, int n_stages,
+                       uint8_t *codes, int64_t plane_rows, int64_t t0, void *stream);
+
 /* ---- step-wise entry points (the lock-step parity protocol of DESIGN.md section 6) ---- */
 
 /* One assignment pass over ALL T*M rows of every group against stage `stage` of cb.

@@ -41,7 +41,7 @@ class gsrq_fit_stats(C.Structure):
 
 
 _lib = None
-EXPORTS = ["gsrq_workspace_bytes", "gsrq_fit_stage", "gsrq_encode", "gsrq_decode", "gsrq_assign", "gsrq_update",
+EXPORTS = ["gsrq_workspace_bytes", "gsrq_fit_stage", "gsrq_encode", "gsrq_decode", "gsrq_encode_append", "gsrq_assign", "gsrq_update",
            "gsrq_init_ids", "gsrq_debug_scores", "gsrq_encode_host", "gsrq_decode_host", "gsrq_pipeline_host", "gsrq_profile_enable",
            "gsrq_profile_read", "gsrq_launch_count", "gsrq_last_error", "gsrq_version"]
 
@@ -126,6 +126,11 @@ def gsrq_fit_stage(kv, view, w, w_stride_g, fit_tokens, cb, stage, residual, ite
 def gsrq_encode(kv, view, cb, stage_begin, stage_end, codes, residual_out, ws):
     _check(lib().gsrq_encode(_ptr(kv), C.byref(view), C.byref(cb), stage_begin, stage_end, _ptr(codes),
                              _ptr(residual_out), _ptr(ws), C.c_size_t(ws.numel()), _stream()))
+
+
+def gsrq_encode_append(kv_new, new_view, cb, n_stages, codes, plane_rows, t0):
+    _check(lib().gsrq_encode_append(_ptr(kv_new), C.byref(new_view), C.byref(cb), n_stages, _ptr(codes),
+                                    C.c_int64(plane_rows), C.c_int64(t0), _stream()))
 
 
 def gsrq_decode(codes, cb, n_stages, kv_out, out_view):

@@ -530,6 +530,28 @@ int gsrq_decode(const uint8_t *codes, const gsrq_codebook *cb, int n_stages, voi
   return GSRQ_OK;
 }
 
+int gsrq_encode_append(const void *kv_new, const gsrq_view *new_view, const gsrq_codebook *cb, int n_stages, uint8_t *codes,
+                       int64_t plane_rows, int64_t t0, void *stream_) {
+  cudaStream_t stream = (cudaStream_t)stream_;
+  if (!kv_new || !cb || !cb->shapes || !cb->gains || !codes) { set_error("NULL kv / codebook / codes"); return GSRQ_EINVAL; }
+  int rc = check_view(new_view, cb->K, cb->S);
+  if (rc) return rc;
+  const int M = new_view->hd / new_view->d;
+  if (n_stages < 1 || n_stages > cb->S) { set_error("n_stages %d out of [1, %d]", n_stages, cb->S); return GSRQ_EINVAL; }
+  if (t0 < 0 || plane_rows < (t0 + new_view->T) * M) { set_error("tokens [%lld, %lld) do not fit in planes of %lld rows", (long long)t0, (long long)(t0 + new_view->T), (long long)plane_rows); return GSRQ_EINVAL; }
+  AppendParams p{};
+  p.src = make_src(kv_new, new_view, nullptr, 0);
+  p.N = new_view->T * M; p.shapes = cb->shapes; p.gains = cb->gains; p.S = cb->S; p.K = cb->K; p.n_stages = n_stages; p.G = new_view->G;
+  p.codes = codes; p.code_stride_s = (long long)new_view->G * plane_rows; p.plane_rows = plane_rows; p.row0 = t0 * M;
+  const long long rows = (long long)new_view->G * p.N;
+  long long ctas = (rows + 7) / 8;
+  if (ctas > 1184) ctas = 1184;
+  const int d = new_view->d;
+  LAUNCH(kClsEncode, stream, DISPATCH_D(d, (k_encode_append<D><<<(unsigned)ctas, 256, 0, stream>>>(p))));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  return GSRQ_OK;
+}
+
 static int assign_all_rows(const void *kv, const gsrq_view *view, const float *residual, const gsrq_codebook *cb, int stage,
                            int mode, uint8_t *idx_out, float *dbg, void *workspace, size_t workspace_bytes, cudaStream_t stream) {
   if ((!kv && !residual) || !cb || !cb->shapes || !cb->gains || !idx_out) { set_error("NULL input"); return GSRQ_EINVAL; }

@@ -204,6 +204,42 @@ __device__ __forceinline__ int exact_argmax_warp(const float (&x)[D], const floa
   return (bi == 0x7fffffff) ? 0 : bi;
 }
 
+// Exact arg-max of one row by a whole warp, cheap in the common case: fp32 filter across the warp
+// (score = fl32(2 (r.c_k) - b_k), c = fl32(g s), b = fl32(g^2); 8 codewords per lane for K = 256) with the
+// CUDA-core error bound, and fp64 over all codewords when its top-2 gap is within that bound.
+template <int D>
+__device__ __forceinline__ int warp_argmax_filtered(const float (&x)[D], const float *__restrict__ sh, const float *__restrict__ ga,
+                                                    int K, int mode, int lane) {
+  float best = -INFINITY, second = -INFINITY, gmx = 0.0f;
+  int bi = 0x7fffffff;
+  for (int kk = lane; kk < K; kk += 32) {
+    const float gk = (mode == 0) ? ga[kk] : 1.0f;
+    gmx = fmaxf(gmx, gk);
+    float cwv[D];
+    load_row_f32<D>(sh, kk, cwv);
+    float dot = 0.0f;
+#pragma unroll
+    for (int j = 0; j < D; ++j) dot = fmaf(x[j], (mode == 0) ? __fmul_rn(gk, cwv[j]) : cwv[j], dot);
+    const float sc = fmaf(2.0f, dot, (mode == 0) ? -__fmul_rn(gk, gk) : 0.0f);
+    if (sc > best) { second = best; best = sc; bi = kk; }
+    else if (sc > second) second = sc;
+  }
+  for (int off = 16; off; off >>= 1) {
+    const float ob = __shfl_xor_sync(0xffffffffu, best, off), os = __shfl_xor_sync(0xffffffffu, second, off);
+    const int oi = __shfl_xor_sync(0xffffffffu, bi, off);
+    gmx = fmaxf(gmx, __shfl_xor_sync(0xffffffffu, gmx, off));
+    if (ob > best || (ob == best && oi < bi)) { second = fmaxf(best, os); best = ob; bi = oi; }
+    else second = fmaxf(second, ob);
+  }
+  float n2 = 0.0f;
+#pragma unroll
+  for (int j = 0; j < D; ++j) n2 = fmaf(x[j], x[j], n2);
+  const float gm = (mode == 0) ? gmx : 1.0f;
+  const float E = fmaf(1.05f * kU * (2 * D + 4) * gm, sqrtf(n2) * 1.00001f, (mode == 0) ? 1.05f * kU * 2.0f * gm * gm : 0.0f);
+  if (best - second <= 2.0f * E) return exact_argmax_warp<D>(x, sh, ga, K, mode, lane, 0xFFFFu);
+  return (bi == 0x7fffffff) ? 0 : bi;
+}
+
 // Exact path: one warp per listed row.  Stages before the entry's first undecided stage s* are replayed
 // from their stored codes; stage s* is decided in fp64 among the entry's candidate groups (every
 // codeword outside them is provably not the arg-max); later stages run the fp32 filter of k_encode
@@ -233,35 +269,7 @@ __global__ void __launch_bounds__(256) k_encode_exact(EncParams p) {
         if (s == s_star) {
           k = exact_argmax_warp<D>(x, sh, ga, p.K, p.mode, lane, en.y & 0xFFFFu);
         } else {
-          // fp32 filter across the warp: score = fl32(2 (r.c_k) - b_k), c = fl32(g s), b = fl32(g^2)
-          float best = -INFINITY, second = -INFINITY, gmx = 0.0f;
-          int bi = 0x7fffffff;
-          for (int kk = lane; kk < p.K; kk += 32) {
-            const float gk = (p.mode == 0) ? ga[kk] : 1.0f;
-            gmx = fmaxf(gmx, gk);
-            float cwv[D];
-            load_row_f32<D>(sh, kk, cwv);
-            float dot = 0.0f;
-#pragma unroll
-            for (int j = 0; j < D; ++j) dot = fmaf(x[j], (p.mode == 0) ? __fmul_rn(gk, cwv[j]) : cwv[j], dot);
-            const float sc = fmaf(2.0f, dot, (p.mode == 0) ? -__fmul_rn(gk, gk) : 0.0f);
-            if (sc > best) { second = best; best = sc; bi = kk; }
-            else if (sc > second) second = sc;
-          }
-          for (int off = 16; off; off >>= 1) {
-            const float ob = __shfl_xor_sync(0xffffffffu, best, off), os = __shfl_xor_sync(0xffffffffu, second, off);
-            const int oi = __shfl_xor_sync(0xffffffffu, bi, off);
-            gmx = fmaxf(gmx, __shfl_xor_sync(0xffffffffu, gmx, off));
-            if (ob > best || (ob == best && oi < bi)) { second = fmaxf(best, os); best = ob; bi = oi; }
-            else second = fmaxf(second, ob);
-          }
-          float n2 = 0.0f;
-#pragma unroll
-          for (int j = 0; j < D; ++j) n2 = fmaf(x[j], x[j], n2);
-          const float gm = (p.mode == 0) ? gmx : 1.0f;
-          const float E = fmaf(1.05f * kU * (2 * D + 4) * gm, sqrtf(n2) * 1.00001f, (p.mode == 0) ? 1.05f * kU * 2.0f * gm * gm : 0.0f);
-          k = (bi == 0x7fffffff) ? 0 : bi;
-          if (best - second <= 2.0f * E) k = exact_argmax_warp<D>(x, sh, ga, p.K, p.mode, lane, 0xFFFFu);
+          k = warp_argmax_filtered<D>(x, sh, ga, p.K, p.mode, lane);
         }
         if (lane == 0 && p.codes) {
           uint8_t *cp = p.codes + (long long)(s - p.s_base) * p.code_stride_s + gi;
@@ -280,6 +288,42 @@ __global__ void __launch_bounds__(256) k_encode_exact(EncParams p) {
     }
     if (p.res_out && lane == 0) store_row_f32<D>(p.res_out, gi, x);
     if (p.st && lane == 0) atomicAdd(reinterpret_cast<unsigned long long *>(&p.st[g].refined), 1ull);
+  }
+}
+
+// Encode-on-append (PAPER.md:443 (i): "residual quantization ... of newly generated KV vectors"): a handful of new
+// tokens, one warp per sub-vector row, all stages with warp_argmax_filtered -- one small launch, no workspace.
+// Row i of group g of the new tokens goes to codes[s*code_stride_s + g*plane_rows + row0 + i].
+struct AppendParams {
+  RowSrc src;           // the new tokens (kv view)
+  long long N;          // new rows per group = n_new * M
+  const float *shapes;  // [G][S][K][D]
+  const float *gains;   // [G][S][K]
+  int S, K, n_stages, G;
+  uint8_t *codes;
+  long long code_stride_s, plane_rows, row0;
+};
+
+template <int D>
+__global__ void __launch_bounds__(256) k_encode_append(AppendParams p) {
+  const int lane = threadIdx.x & 31;
+  const long long total = (long long)p.G * p.N;
+  for (long long gi = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5; gi < total; gi += ((long long)gridDim.x * blockDim.x) >> 5) {
+    const int g = (int)(gi / p.N);
+    const long long i = gi - (long long)g * p.N;
+    float x[D];
+    load_src_row<D>(p.src, g, i, x);
+    for (int s = 0; s < p.n_stages; ++s) {
+      const float *sh = p.shapes + ((long long)g * p.S + s) * p.K * D;
+      const float *ga = p.gains + ((long long)g * p.S + s) * p.K;
+      const int k = warp_argmax_filtered<D>(x, sh, ga, p.K, 0, lane);
+      if (lane == 0) p.codes[(long long)s * p.code_stride_s + (long long)g * p.plane_rows + p.row0 + i] = (uint8_t)k;
+      const float gk = ga[k];
+      float cwv[D];
+      load_row_f32<D>(sh, k, cwv);
+#pragma unroll
+      for (int j = 0; j < D; ++j) x[j] = __fsub_rn(x[j], __fmul_rn(gk, cwv[j]));
+    }
   }
 }
 

@@ -183,3 +183,34 @@ def test_decision_margin_stress(B):
     for g_ in range(G):
         a, _, _ = o.assign(rows[g_], sh[g_, 0], None)
         assert np.array_equal(idx[g_].cpu().numpy(), a.astype(np.uint8))
+
+
+@pytest.mark.parametrize("dtype,hd,d,head_inner", [("bf16", 128, 16, True), ("bf16", 128, 16, False), ("f32", 64, 8, False), ("bf16", 64, 32, False)])
+def test_encode_on_append_equals_batch_encode(B, dtype, hd, d, head_inner):
+    """PAPER.md:443 (i): new tokens are quantised as they are generated.  Appending tokens 1, 3, 8, 32 at a time
+    must fill the code planes exactly as one batch encode (and as the oracle) does."""
+    rng = np.random.default_rng(5)
+    G, T, K, S = 4, 140, 200, 3
+    x = rng.standard_normal((G, T, hd)).astype(np.float32) * np.exp(0.4 * rng.standard_normal((G, T, 1))).astype(np.float32)
+    if dtype == "bf16":
+        x = inputs.bf16_round(x)
+    sh = rng.standard_normal((G, S, K, d))
+    sh = (sh / np.linalg.norm(sh, axis=-1, keepdims=True)).astype(np.float32)
+    ga = np.abs(rng.standard_normal((G, S, K)) / (1 + np.arange(S))[None, :, None]).astype(np.float32)
+    codes_o, _, _, _ = o.encode(x, sh, ga, d)
+    M = hd // d
+    xd = to_device(x, dtype, head_inner)
+    sh_d, ga_d = torch.from_numpy(sh).cuda(), torch.from_numpy(ga).cuda()
+    cb = B.codebook_of(sh_d, ga_d)
+    codes = torch.full((S, G, T * M), 255, dtype=torch.uint8, device="cuda")
+    t0 = 0
+    for n_new in [1, 3, 8, 32, 1, 64, 31]:
+        n_new = min(n_new, T - t0)
+        chunk = xd[t0:t0 + n_new] if head_inner else xd[:, t0:t0 + n_new]
+        B.gsrq_encode_append(chunk, B.view_of(chunk, d, head_inner), cb, S, codes, T * M, t0)
+        t0 += n_new
+    assert t0 == T
+    torch.cuda.synchronize()
+    assert np.array_equal(codes.cpu().numpy(), codes_o)
+    with pytest.raises(B.GsrqError):
+        B.gsrq_encode_append(chunk, B.view_of(chunk, d, head_inner), cb, S, codes, T * M, T)   # does not fit
