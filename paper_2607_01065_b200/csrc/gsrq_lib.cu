@@ -402,9 +402,11 @@ int gsrq_fit_stage(const void *kv, const gsrq_view *view, const float *w, int64_
     rc = run_update(pl, view, K, ws, idx, shapes_st, gains_st, cb_stride_g, st, t > 0, t, n_planes != 0, stream);
   }
   if (rc) return rc;
-  LAUNCH(kClsMisc, stream, (k_finish<<<G, 160, 0, stream>>>(st, (const double *)(ws + pl.off_term), kTermStride, K,
-                                                            (const double *)(ws + pl.off_epart), (int)pl.nE, iters)));
-  GSRQ_CUDA_CHECK(cudaGetLastError());
+  if (stats) {  // J_t and iters_run are only read back through `stats`
+    LAUNCH(kClsMisc, stream, (k_finish<<<G, 160, 0, stream>>>(st, (const double *)(ws + pl.off_term), kTermStride, K,
+                                                              (const double *)(ws + pl.off_epart), (int)pl.nE, iters)));
+    GSRQ_CUDA_CHECK(cudaGetLastError());
+  }
   if (stats) {
     DevStats *h = (DevStats *)malloc((size_t)G * sizeof(DevStats));
     if (!h) { set_error("out of host memory"); return GSRQ_ECUDA; }
