@@ -47,10 +47,6 @@ struct RowSrc {
   long long rows_per_group;  // of `rows`
 };
 
-struct Launch {
-  cudaStream_t stream;
-};
-
 void set_error(const char *fmt, ...);
 
 #define GSRQ_CUDA_CHECK(expr)                                                       \

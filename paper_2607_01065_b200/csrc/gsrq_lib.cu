@@ -62,7 +62,7 @@ struct Plan {
   int M;
   // [0, encode_total): what gsrq_encode needs; the rest is for the fit
   size_t off_list, off_cnt, off_st, off_ebimg, off_egmax, encode_total;
-  size_t off_Rf, off_rinv, off_wt, off_idx, off_ids, off_epart, off_term;
+  size_t off_Rf, off_coef, off_wt, off_idx, off_ids, off_epart, off_term;
   size_t off_ahi, off_alo, off_rnorm, off_bimg, off_gmax, total;
 };
 
@@ -86,7 +86,7 @@ static Plan make_plan(const gsrq_view *v, int K, int S, long long n_fit_tokens) 
   p.off_egmax = o; o += align_up(v->d == tc::kD ? (size_t)v->G * tc::kEncMaxS * sizeof(int) : 0);
   p.encode_total = o;
   p.off_Rf = o;   o += align_up((size_t)v->G * p.Nf * v->d * sizeof(float));
-  p.off_rinv = o; o += align_up((size_t)v->G * p.Nf * 2 * sizeof(double));  // per-row {w, w/(||r||+eps)}
+  p.off_coef = o; o += align_up((size_t)v->G * p.Nf * 2 * sizeof(double));  // per-row {w, w/(||r||+eps)}
   p.off_wt = o;   o += align_up((size_t)v->G * p.nf_tok * sizeof(float));
   p.off_idx = o;  o += align_up((size_t)v->G * p.Nf);
   p.off_ids = o;  o += align_up((size_t)v->G * GSRQ_MAX_K * sizeof(long long));
@@ -152,7 +152,7 @@ static int run_update(const Plan &pl, const gsrq_view *v, int K, char *ws, const
                       float *gains_st, long long cb_stride_g, DevStats *st, int lloyd, int t, bool images, cudaStream_t stream) {
   const int d = v->d;
   UpdParams u{};
-  u.Rf = (const float *)(ws + pl.off_Rf); u.coef = (const double2 *)(ws + pl.off_rinv); u.wt = (const float *)(ws + pl.off_wt);
+  u.Rf = (const float *)(ws + pl.off_Rf); u.coef = (const double2 *)(ws + pl.off_coef);
   u.idx = idx; u.Nf = pl.Nf; u.M = pl.M; u.K = K; u.shapes = shapes_st; u.gains = gains_st; u.cb_stride_g = cb_stride_g;
   u.st = st; u.term = st ? (double *)(ws + pl.off_term) : nullptr; u.term_stride = kTermStride; u.lloyd = lloyd; u.t = t;
   u.bimg = images ? (uint8_t *)(ws + pl.off_bimg) : nullptr;
@@ -244,7 +244,7 @@ static int launch_prep(const Plan &pl, const gsrq_view *v, const RowSrc &src, co
                        const long long *fit_tokens, char *ws, bool consts, int n_planes, cudaStream_t stream) {
   PrepParams q{};
   q.src = src; q.w = w; q.w_stride_g = w_stride_g; q.fit_tokens = fit_tokens; q.nf_tok = pl.nf_tok;
-  q.Rf = (float *)(ws + pl.off_Rf); q.coef = (double2 *)(ws + pl.off_rinv); q.wt = (float *)(ws + pl.off_wt);
+  q.Rf = (float *)(ws + pl.off_Rf); q.coef = (double2 *)(ws + pl.off_coef); q.wt = (float *)(ws + pl.off_wt);
   q.epart = consts ? (double *)(ws + pl.off_epart) : nullptr;
   q.ahi = (consts && n_planes > 0) ? (__nv_bfloat16 *)(ws + pl.off_ahi) : nullptr;
   q.alo = (consts && n_planes == 2) ? (__nv_bfloat16 *)(ws + pl.off_alo) : nullptr;

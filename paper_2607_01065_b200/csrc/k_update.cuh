@@ -27,7 +27,6 @@ constexpr int kHalfRows = kRoundRows / 2;
 struct UpdParams {
   const float *Rf;        // [G][Nf][D] fp32 rows
   const double2 *coef;    // [G][Nf]   per-row {w_i, w_i/(||r_i||+eps)}
-  const float *wt;        // [G][Nf/M] per-fit-token weights (unused by the kernel; kept by the preparation)
   const uint8_t *idx;     // [G][Nf]
   long long Nf;
   int M, K;
