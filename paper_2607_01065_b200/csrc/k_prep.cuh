@@ -121,8 +121,19 @@ __global__ void __launch_bounds__(512) k_init_ids(const float *__restrict__ Rf, 
     __syncthreads();
     const int nc = n_chosen;
     if (good) {
-      for (int q = 0; q < nc && good; ++q) good = (chosen[q] != c);
-      for (int q = 0; q < t && good; ++q) good = (cand[q] != c);
+      // no data-dependent exit and 8 comparisons per trip: the loads of a trip are independent, so the (in-order)
+      // thread does not pay one shared-memory latency per comparison
+      int dup = 0;
+      for (int q = 0; q < nc; ++q) dup |= (chosen[q] == c);
+      int q = 0;
+      for (; q + 8 <= t; q += 8) {
+        int d8 = 0;
+#pragma unroll
+        for (int u = 0; u < 8; ++u) d8 |= (cand[q + u] == c);
+        dup |= d8;
+      }
+      for (; q < t; ++q) dup |= (cand[q] == c);
+      good = !dup;
     }
     ok[t] = good;
     scan[t] = good;
