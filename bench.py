@@ -193,6 +193,44 @@ def run_cfg4(B, pk):
                 rel_residual_energy_first_4096_tokens=err)
 
 
+def run_cfg2(B, pk):
+    """BASELINE.json config 2: V-like 8 x 16384 x 128 (Student-t, per-token norms), d=16, K=256, S=1, 20 iterations;
+    fit + encode, and the decode of the whole layer timed (33.5 MB out: L2-resident, so GB/s is effective)."""
+    c = inputs.CONFIGS[2]
+    G, T, hd, d, K, S, iters = c.G, c.T, c.hd, c.d, c.K, c.S, c.iters
+    M = hd // d
+    x = torch.from_numpy(inputs.v_like(G, T, hd, inputs.seed_of(2, "v"))).to(torch.bfloat16).cuda()
+    w = torch.from_numpy(inputs.token_weights(T, inputs.seed_of(2, "w"))).cuda()
+    view = B.view_of(x, d)
+    shapes = torch.zeros(G, S, K, d, device="cuda")
+    gains = torch.zeros(G, S, K, device="cuda")
+    cb = B.codebook_of(shapes, gains)
+    ws = B.workspace(view, K, S, 0)
+    codes = torch.zeros(S, G, T * M, dtype=torch.uint8, device="cuda")
+    out = torch.empty_like(x)
+
+    def timed(f, n=5):
+        ts = []
+        for _ in range(n):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); f(); b.record()
+            torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        return float(np.median(ts))
+
+    fit = lambda: B.gsrq_fit_stage(x, view, w, 0, None, cb, 0, None, iters, 0, ws, want_stats=False)
+    enc = lambda: B.gsrq_encode(x, view, cb, 0, S, codes, None, ws)
+    dec = lambda: B.gsrq_decode(codes, cb, S, out, view)
+    fit(); enc(); dec()
+    fit_ms, enc_ms, dec_ms = timed(fit, 3), timed(enc), timed(dec)
+    rows = G * T * M
+    by = rows * S + rows * 2 * d
+    return dict(workload="cfg2:v-cache-8x16384x128, S=1", fit_ms=fit_ms, encode_ms=enc_ms,
+                encode_kv_vectors_per_s=G * T / (enc_ms * 1e-3),
+                encode_tensor_frac=2.0 * K * d * rows * S / (enc_ms * 1e-3) / 1e12 / pk["bf16_tflops_sustained"],
+                decode_ms=dec_ms, decode_gb_per_s=by / (dec_ms * 1e-3) / 1e9, decode_hbm_frac=by / (dec_ms * 1e-3) / 1e9 / pk["hbm_gbs"])
+
+
 def run_cfg3(B, pk):
     """BASELINE.json config 3 for the K-like tensor (8 x 32768 x 128, bf16): one S=4 fit (20 iterations per stage),
     then encode throughput and decode GB/s for S = 1..4 (prefixes of the same codebooks) and the
@@ -393,13 +431,15 @@ def main():
 
     if rank != 0:
         return
-    big = sweep3 = None
+    big = sweep3 = v2 = None
     if not args.no_big:
         del flush
         torch.cuda.empty_cache()
         big = run_cfg4(B, peaks())
         torch.cuda.empty_cache()
         sweep3 = run_cfg3(B, peaks())
+        torch.cuda.empty_cache()
+        v2 = run_cfg2(B, peaks())
     pk = peaks()
     # Rooflines of the step's kernels, from the live CUDA-event brackets (two profiled steps).
     # Algorithmic work: scoring pass 2*K*d flops per sub-vector; update kernel one read of
@@ -448,6 +488,7 @@ def main():
     if big is not None:
         line["cfg4"] = big
         line["cfg3"] = sweep3
+        line["cfg2"] = v2
     if not args.no_cpu_baseline:
         from oracle import gsrq_oracle as o
         t0 = time.perf_counter()
