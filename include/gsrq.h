@@ -108,7 +108,12 @@ size_t gsrq_workspace_bytes(const gsrq_view *view, int K, int S, int64_t n_fit_t
  *            stage 0 reads kv; stage > 0 re-derives the residual from kv and cb.
  * seed     : selects the initial rows (splitmix64 stream, reading c-I).
  * stats    : HOST array of G structs or NULL.  When given, the call synchronises `stream`
- *            and returns GSRQ_EDEGENERATE if any group could not be initialised.
+ *            and returns GSRQ_EDEGENERATE if any group could not be initialised; the per-iteration
+ *            distortions are only computed in that case.
+ * Kernels  : per pass two launches -- assignment (d == 16: tcgen05 filter with an fp64 re-score of the
+ *            ambiguous rows inside the kernel; other d: CUDA-core filter + exact kernel) and the fused
+ *            reduction / Eq. 7-8 update.  No host synchronisation inside the loop; a group whose
+ *            assignments stopped changing (Alg. 1 l.15-16) is skipped by the later passes.
  */
 int gsrq_fit_stage(const void *kv, const gsrq_view *view, const float *w, int64_t w_stride_g,
                    const int64_t *fit_tokens, int64_t n_fit, gsrq_codebook *cb, int stage,
@@ -121,7 +126,11 @@ int gsrq_fit_stage(const void *kv, const gsrq_view *view, const float *w, int64_
  * codes       : [S][G][T*M] uint8, stage-major planes (a prefix of stages decodes alone,
  *               PAPER.md:25).  Planes in range are written; when stage_begin > 0 the
  *               planes < stage_begin are READ to rebuild the residual from kv.
- * residual_out: [G][T*M][d] fp32 residual after stage_end-1, or NULL.
+ * residual_out: [G][T*M][d] fp32 residual after stage_end-1 (16-byte aligned), or NULL.
+ * Kernels     : d == 16, bf16 input, stage_begin == 0, stage_end <= 4, hd/d a power of two: one fused
+ *               tensor-core pass over all stages (the residual stays on the SM) plus the exact kernel
+ *               for the rows it could not decide; otherwise the CUDA-core filter + exact kernel.
+ *               Either way every code equals the exact-arithmetic arg-max (ties -> lowest index).
  */
 int gsrq_encode(const void *kv, const gsrq_view *view, const gsrq_codebook *cb, int stage_begin,
                 int stage_end, uint8_t *codes, float *residual_out, void *workspace,
