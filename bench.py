@@ -45,7 +45,7 @@ def peaks():
 
 
 class ClockSampler(threading.Thread):
-    """Samples nvidia-smi clocks / throttle reasons every 200 ms while the timed region runs."""
+    """Samples nvidia-smi clocks / throttle reasons every 20 ms while the timed region runs."""
 
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
@@ -57,24 +57,27 @@ class ClockSampler(threading.Thread):
     def run(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-i", str(self.index), "-lms", "200"], stdout=subprocess.PIPE, text=True)
+                                          "-i", str(self.index), "-lms", "20"], stdout=subprocess.PIPE, text=True)
             for line in self.proc.stdout:
-                self.samples.append([t.strip() for t in line.split(",")])
+                self.samples.append((time.perf_counter(), [t.strip() for t in line.split(",")]))
                 if self.stop_flag:
                     break
         except Exception:
             pass
 
-    def finish(self):
+    def finish(self, t0=None, t1=None):
+        """Median SM clock and throttle reasons over the samples taken in [t0, t1] (all samples if none fall inside)."""
         self.stop_flag = True
         if self.proc:
             self.proc.terminate()
-        sm = [float(s[0]) for s in self.samples if s and s[0].replace(".", "").isdigit()]
-        mx = [float(s[1]) for s in self.samples if len(s) > 1 and s[1].replace(".", "").isdigit()]
+        inside = [f for (t, f) in self.samples if t0 is not None and t0 <= t <= t1]
+        rows = inside if inside else [f for (_, f) in self.samples]
+        sm = [float(r[0]) for r in rows if r and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        reasons = sorted({names[i] for s in self.samples if len(s) >= 6 for i in range(4) if s[2 + i].lower().startswith("active")})
+        reasons = sorted({names[i] for r in rows if len(r) >= 6 for i in range(4) if r[2 + i].lower().startswith("active")})
         return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None, reasons=reasons,
-                    samples=len(sm))
+                    samples=len(sm), samples_in_timed_region=len(inside))
 
 
 def oracle_step(x, w, c):
@@ -355,11 +358,12 @@ def main():
             dist.barrier()
             torch.cuda.synchronize()
 
+    sampler = ClockSampler(local)
+    sampler.start()                          # nvidia-smi takes a moment to come up: start it before the warm-up
     for _ in range(max(args.warmup, 3)):
         step()
     barrier()
-    sampler = ClockSampler(local)
-    sampler.start()
+    t_region0 = time.perf_counter()
     l0 = B.gsrq_launch_count()
     evs = []
     for _ in range(args.steps):
@@ -427,7 +431,7 @@ def main():
     e2e_val, _ = whole_job_value(e2e_s, G * T, world, "cuda")
     h2d = x_host.numel() * 2 + w_host.numel() * 4
     d2h = sh_h.numel() * 4 + ga_h.numel() * 4 + co_h.numel() + out_h.numel() * 2
-    clocks = sampler.finish()
+    clocks = sampler.finish(t_region0, time.perf_counter())
 
     if rank != 0:
         return
