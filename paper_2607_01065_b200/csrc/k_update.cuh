@@ -85,11 +85,63 @@ __device__ __forceinline__ uint32_t load_idx_word(const uint8_t *ig, long long r
   return w;
 }
 
+constexpr int kBigRows = 256;  // a cluster with more rows than this in one pass is added by all warps together
+
+// Rows [x0, x1) of the staged round (positions in the pass's list; the round starts at `lo`) added in list order by
+// one warp into a partial of P = 2D + 2 values at `out` (shared memory): [A | B | W | unused].  Cold path of
+// k_update, used for clusters that hold hundreds of rows of a pass (heavy-tailed tensors).
+template <int D>
+__device__ __noinline__ void upd_add_chunk(const float *xbuf_r, const double *coef_r, int x0, int x1, int lo, int lane, double *out) {
+  constexpr int Q = (2 * D + 31) / 32;
+  double sp[Q], Wp = 0.0;
+  int isB[Q], col[Q];
+  bool live[Q];
+#pragma unroll
+  for (int q = 0; q < Q; ++q) {
+    const int el = lane + 32 * q;
+    sp[q] = 0.0; live[q] = el < 2 * D; isB[q] = (el >= D) ? 1 : 0; col[q] = el % D;
+  }
+  int pos = x0;
+  for (; pos + 4 <= x1; pos += 4) {
+    double cf[4][Q];
+    float xv[4][Q];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int e = pos + u - lo;
+#pragma unroll
+      for (int q = 0; q < Q; ++q) {
+        cf[u][q] = live[q] ? coef_r[2 * e + isB[q]] : 0.0;
+        xv[u][q] = live[q] ? xbuf_r[e * D + col[q]] : 0.0f;
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      Wp += cf[u][0];
+#pragma unroll
+      for (int q = 0; q < Q; ++q) sp[q] += cf[u][q] * (double)xv[u][q];
+    }
+  }
+  for (; pos < x1; ++pos) {
+    const int e = pos - lo;
+#pragma unroll
+    for (int q = 0; q < Q; ++q) {
+      const double cf = live[q] ? coef_r[2 * e + isB[q]] : 0.0;
+      if (q == 0) Wp += cf;
+      sp[q] += cf * (double)(live[q] ? xbuf_r[e * D + col[q]] : 0.0f);
+    }
+  }
+#pragma unroll
+  for (int q = 0; q < Q; ++q)
+    if (live[q]) out[lane + 32 * q] = sp[q];
+  if (lane == 0) out[2 * D] = Wp;
+}
+
 template <int D>
 constexpr size_t upd_smem_bytes() {
   constexpr int P = 2 * D + 2;
   return sizeof(double) * (2 * kRoundRows + kCPC * P) + sizeof(float) * (kRoundRows * D) +
-         sizeof(int) * (kCPC + 4) + sizeof(uint16_t) * (kPassRows + kCPC * kUpdThreads) + kPassRows;
+         sizeof(int) * (kCPC + 4) + sizeof(uint16_t) * (kPassRows + kCPC * kUpdThreads) + kPassRows +
+         sizeof(double) * (kUpdThreads / 32) * P + sizeof(int) * (kCPC + 4);
 }
 
 // grid = (ceil(K / kCPC), G), block = kUpdThreads, dynamic smem = upd_smem_bytes<D>().
@@ -107,6 +159,8 @@ __global__ void __launch_bounds__(kUpdThreads, 1) k_update(UpdParams p) {
   uint16_t *list = reinterpret_cast<uint16_t *>(ctot + kCPC + 4);  // [kPassRows] rows of the pass, by (cluster, row)
   uint16_t *cntb = list + kPassRows;                        // [kCPC][kUpdThreads] per-thread counts -> prefixes
   uint8_t *idxb = reinterpret_cast<uint8_t *>(cntb + kCPC * kUpdThreads);  // [kPassRows] assignment bytes of the pass
+  double *part = reinterpret_cast<double *>(idxb + kPassRows);  // [warps][P] chunk partials of a big cluster's segment
+  int *cb_s = reinterpret_cast<int *>(part + (kUpdThreads / 32) * P);  // [kCPC + 1] list offsets of the clusters; [kCPC + 1]: mask of big clusters
 
   const int g = blockIdx.y, k0 = blockIdx.x * kCPC;
   if (group_done(p.st, g, p.t)) return;
@@ -198,6 +252,13 @@ __global__ void __launch_bounds__(kUpdThreads, 1) k_update(UpdParams p) {
 #pragma unroll
     for (int c = 0; c < kCPC; ++c) cbase[c + 1] = cbase[c] + ctot[c];
     const int total = cbase[kCPC];
+    if (tid == 0) {
+      int bm = 0;
+#pragma unroll
+      for (int c = 0; c < kCPC; ++c) { cb_s[c] = cbase[c]; bm |= (cbase[c + 1] - cbase[c] > kBigRows) ? (1 << c) : 0; }
+      cb_s[kCPC] = cbase[kCPC];
+      cb_s[kCPC + 1] = bm;
+    }
     for (uint32_t mm = m; mm; mm &= mm - 1) {
       const int r = __ffs(mm) - 1;
       const int c = idxb[32 * tid + r] & (kCPC - 1);
@@ -244,7 +305,8 @@ __global__ void __launch_bounds__(kUpdThreads, 1) k_update(UpdParams p) {
       const float *xbuf_r = xbuf + (rd & 1) * kHalfRows * D;
       const double *coef_r = coef + (rd & 1) * kHalfRows * 2;
       // ---- warp c adds cluster c's rows of this round in list (= ascending row) order ----
-      const int a = max(seg0, lo), b = min(seg1, lo + n);
+      const int bigmask = cb_s[kCPC + 1];  // uniform; zero unless a cluster holds > kBigRows rows of this pass
+      const int a = max(seg0, lo), b = ((bigmask >> warp) & 1) ? a : min(seg1, lo + n);
       int pos = a;
       for (; pos + 4 <= b; pos += 4) {  // loads of 4 rows in flight; the adds stay in list order
         double cf[4][Q];
@@ -276,6 +338,34 @@ __global__ void __launch_bounds__(kUpdThreads, 1) k_update(UpdParams p) {
       }
       if (a < b) cntk += b - a;
       __syncthreads();
+      // ---- big clusters: the segment is split into one contiguous chunk per warp, added concurrently, and the chunk
+      //      partials are merged by the owner warp in warp (= list) order ----
+      for (int bmk = bigmask; bmk; bmk &= bmk - 1) {
+        const int c = __ffs(bmk) - 1;
+        const int ca = max(cb_s[c], lo), cb = min(cb_s[c + 1], lo + n);
+        if (ca >= cb) continue;
+        const int chunk = (cb - ca + kUpdThreads / 32 - 1) / (kUpdThreads / 32);
+        const int x0 = min(ca + warp * chunk, cb), x1 = min(x0 + chunk, cb);
+        upd_add_chunk<D>(xbuf_r, coef_r, x0, x1, lo, lane, part + warp * P);
+        __syncthreads();
+        if (warp == c) {
+          double pv[kUpdThreads / 32][Q], pw[kUpdThreads / 32];  // fetch first, then add in warp order
+#pragma unroll
+          for (int wq = 0; wq < kUpdThreads / 32; ++wq) {
+#pragma unroll
+            for (int q = 0; q < Q; ++q) pv[wq][q] = live[q] ? part[wq * P + lane + 32 * q] : 0.0;
+            pw[wq] = part[wq * P + 2 * D];
+          }
+#pragma unroll
+          for (int wq = 0; wq < kUpdThreads / 32; ++wq) {
+#pragma unroll
+            for (int q = 0; q < Q; ++q) s[q] += pv[wq][q];
+            Wk += pw[wq];
+          }
+          cntk += cb - ca;
+        }
+        __syncthreads();
+      }
     }
   }
   {
