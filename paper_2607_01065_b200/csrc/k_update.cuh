@@ -8,8 +8,10 @@
 // (a stable counting sort: integer work only), stages those rows in shared memory with one
 // wave of independent loads, and one warp per cluster adds them up in fp64 in ascending row
 // order -- the definition's own order, so A_k, W_k are bit-identical to a sequential fp64 loop
-// and B_k differs only by the rounding of w_i/(||r_i||+eps).  No
-// floating-point atomics, no cross-CTA partials: bit-identical run to run.  The same CTA then applies
+// and B_k differs only by the rounding of w_i/(||r_i||+eps).  A cluster that
+// holds more than kBigRows rows of a pass is instead added by all warps, one contiguous chunk each, and the
+// chunk partials are merged in chunk order (still a fixed order).  No floating-point atomics, no
+// cross-CTA partials: bit-identical run to run.  The same CTA then applies
 // Eq. 7 / Eq. 8 to its clusters, stores s_k, g_k, the per-cluster term of J (Eq. 4 summed over
 // the cluster), the cluster's rows of the B operand images for the next scoring pass, and
 // max g (integer atomicMax on the bit pattern: order-independent).
