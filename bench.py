@@ -451,11 +451,16 @@ def main():
     rows_per_launch = G * T * M
     tot_ms = sum(v[0] for v in prof.values())
 
+    # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the cfg-1 kernels from the ncu --set full
+    # captures summarised in profiles/r1_v4_ncu_full.md; None for workloads that were not captured
+    NCU_TRAFFIC = {"score": 10.09e6, "update": 21.41e6} if c.cfg == 1 else {}
+
     def kern(name, cls, bound, work_per_launch, peak, unit):
         ms, n = prof[cls]
         per = ms / max(n, 1)
         ach = work_per_launch / (per * 1e-3) / (1e12 if bound == "tensor" else 1e9) if per > 0 else 0.0
-        return dict(bound=bound, kernel=name, achieved=ach, peak=peak, unit=unit, frac=ach / peak, traffic=None,
+        return dict(bound=bound, kernel=name, achieved=ach, peak=peak, unit=unit, frac=ach / peak, traffic=NCU_TRAFFIC.get(cls),
+                    algorithmic_per_launch=work_per_launch,
                     ms_per_launch=per, launches=n // 2, share_of_step=ms / tot_ms if tot_ms else None)
 
     kerns = [
