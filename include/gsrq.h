@@ -127,9 +127,10 @@ int gsrq_fit_stage(const void *kv, const gsrq_view *view, const float *w, int64_
  *               PAPER.md:25).  Planes in range are written; when stage_begin > 0 the
  *               planes < stage_begin are READ to rebuild the residual from kv.
  * residual_out: [G][T*M][d] fp32 residual after stage_end-1 (16-byte aligned), or NULL.
- * Kernels     : d == 16, bf16 input, stage_begin == 0, stage_end <= 4, hd/d a power of two: one fused
- *               tensor-core pass over all stages (the residual stays on the SM) plus the exact kernel
- *               for the rows it could not decide; otherwise the CUDA-core filter + exact kernel.
+ * Kernels     : d == 16, stage_begin == 0, bf16 input with hd/d a power of two (or a dense fp32 tensor):
+ *               fused tensor-core passes of up to 4 stages each (the residual stays on the SM within a
+ *               pass and is carried in fp32 between passes), each followed by the exact kernel for the
+ *               rows it could not decide; otherwise the CUDA-core filter + exact kernel.
  *               Either way every code equals the exact-arithmetic arg-max (ties -> lowest index).
  */
 int gsrq_encode(const void *kv, const gsrq_view *view, const gsrq_codebook *cb, int stage_begin,

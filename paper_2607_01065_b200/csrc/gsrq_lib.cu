@@ -61,7 +61,7 @@ struct Plan {
   long long nf_tok, Nf, Nall, nE;
   int M;
   // [0, encode_total): what gsrq_encode needs; the rest is for the fit
-  size_t off_list, off_cnt, off_st, off_ebimg, off_egmax, encode_total;
+  size_t off_list, off_cnt, off_st, off_ebimg, off_egmax, off_eres, encode_total;
   size_t off_Rf, off_coef, off_wt, off_idx, off_ids, off_epart, off_term;
   size_t off_ahi, off_alo, off_rnorm, off_bimg, off_gmax, total;
 };
@@ -71,7 +71,7 @@ constexpr int kTermStride = GSRQ_MAX_ITERS + 1;
 
 // n_fit_tokens: > 0 fit subset size, 0 = fit on all tokens, < 0 = no fit (encode / decode only)
 static Plan make_plan(const gsrq_view *v, int K, int S, long long n_fit_tokens) {
-  (void)S; (void)K;
+  (void)K;
   Plan p;
   p.M = v->hd / v->d;
   p.nf_tok = (n_fit_tokens > 0) ? n_fit_tokens : (n_fit_tokens == 0 ? v->T : 0);
@@ -84,6 +84,8 @@ static Plan make_plan(const gsrq_view *v, int K, int S, long long n_fit_tokens) 
   p.off_st = o;   o += align_up((size_t)v->G * sizeof(DevStats));
   p.off_ebimg = o; o += align_up(v->d == tc::kD ? (size_t)v->G * tc::kEncMaxS * 3 * tc::kBImgBytes : 0);
   p.off_egmax = o; o += align_up(v->d == tc::kD ? (size_t)v->G * tc::kEncMaxS * sizeof(int) : 0);
+  // fp32 residual between the chained tensor-core passes of an encode with more than kEncMaxS stages
+  p.off_eres = o;  o += align_up((v->d == tc::kD && S > tc::kEncMaxS) ? (size_t)v->G * p.Nall * v->d * sizeof(float) : 0);
   p.encode_total = o;
   p.off_Rf = o;   o += align_up((size_t)v->G * p.Nf * v->d * sizeof(float));
   p.off_coef = o; o += align_up((size_t)v->G * p.Nf * 2 * sizeof(double));  // per-row {w, w/(||r||+eps)}
@@ -134,6 +136,11 @@ static RowSrc make_src(const void *kv, const gsrq_view *v, const float *rows, lo
     else if ((d) == 16) { constexpr int D = 16; __VA_ARGS__; } \
     else { constexpr int D = 32; __VA_ARGS__; }     \
   } while (0)
+
+static int run_encode_tc(const void *kv, const gsrq_view *v, const float *rows0, long long N, const gsrq_codebook *cb, int n_stages,
+                         uint8_t *codes, long long code_stride_s, float *carry, bool want_residual, const struct Plan &pl, char *ws,
+                         unsigned int *cnt_base, cudaStream_t stream);
+static bool use_tc(int d);
 
 // One filter + refine pass (assignment or multi-stage encode) described by `p`.
 static int run_encode(EncParams p, int G, int d, cudaStream_t stream) {
@@ -267,60 +274,111 @@ static int prepare_rows(const Plan &pl, const void *kv, const gsrq_view *v, cons
   int rc = launch_prep(pl, v, make_src(kv, v, residual, pl.Nall), w, w_stride_g, fit_tokens, ws, !derive, n_planes, stream);
   if (rc || !derive) return rc;
   // r = x - sum_{s<stage} c^(s)[a^(s)], in place on the compact rows; then the constants of the residual rows
-  EncParams p{};
-  p.src = make_src(nullptr, v, Rf, pl.Nf);
-  p.N = pl.Nf; p.shapes = cb->shapes; p.gains = cb->gains; p.S = cb->S; p.K = cb->K;
-  p.s_begin = 0; p.s_end = stage; p.s_base = 0; p.mode = 0; p.subtract = 1;
-  p.codes = nullptr; p.code_stride_s = 0; p.res_out = Rf; p.st = nullptr; p.slot = 0;
-  p.list = (uint2 *)(ws + pl.off_list);
-  p.list_cnt = (unsigned int *)(ws + pl.off_cnt) + (kNumCounters - 1);
-  rc = run_encode(p, G, d, stream);
-  if (rc) return rc;
+  if (use_tc(d)) {  // tensor-core passes starting from the gathered fp32 rows (no codes wanted)
+    rc = run_encode_tc(nullptr, v, Rf, pl.Nf, cb, stage, nullptr, 0, Rf, true, pl, ws, (unsigned int *)(ws + pl.off_cnt) + 200, stream);
+    if (rc) return rc;
+  } else {
+    EncParams p{};
+    p.src = make_src(nullptr, v, Rf, pl.Nf);
+    p.N = pl.Nf; p.shapes = cb->shapes; p.gains = cb->gains; p.S = cb->S; p.K = cb->K;
+    p.s_begin = 0; p.s_end = stage; p.s_base = 0; p.mode = 0; p.subtract = 1;
+    p.codes = nullptr; p.code_stride_s = 0; p.res_out = Rf; p.st = nullptr; p.slot = 0;
+    p.list = (uint2 *)(ws + pl.off_list);
+    p.list_cnt = (unsigned int *)(ws + pl.off_cnt) + (kNumCounters - 1);
+    rc = run_encode(p, G, d, stream);
+    if (rc) return rc;
+  }
   return launch_prep(pl, v, make_src(nullptr, v, Rf, pl.Nf), (const float *)(ws + pl.off_wt), pl.nf_tok, nullptr, ws, true,
                      n_planes, stream);
 }
 
-// ---- fused tensor-core encode (d == 16, bf16 input, stages [0, n) with n <= kEncMaxS) ----
-static bool can_encode_tc(const void *kv, const gsrq_view *v, int stage_begin, int stage_end) {
+// ---- fused tensor-core encode (d == 16): passes of <= kEncMaxS stages ----
+// The first pass reads a bf16 tensor straight through TMA; a dense fp32 tensor, and every later pass of a deep
+// residual quantiser, start from fp32 rows (FROM_ROWS).
+static bool can_encode_tc(const void *kv, const gsrq_view *v, int stage_begin) {
   const int M = v->hd / v->d;
-  return use_tc(v->d) && v->dtype == GSRQ_BF16 && stage_begin == 0 && stage_end <= tc::kEncMaxS && M <= tc::kTileM &&
-         (M & (M - 1)) == 0 && ((uintptr_t)kv & 15) == 0 && v->T < (1LL << 31);
+  if (!use_tc(v->d) || stage_begin != 0 || ((uintptr_t)kv & 15) || v->T >= (1LL << 31)) return false;
+  if (v->dtype == GSRQ_BF16) return M <= tc::kTileM && (M & (M - 1)) == 0;
+  return v->stride_t == v->hd && v->stride_g == v->T * v->hd;  // fp32: the tensor itself is the [G][N][16] row buffer
 }
 
-
-static int run_encode_tc(const void *kv, const gsrq_view *v, const gsrq_codebook *cb, int n_stages, uint8_t *codes,
-                         float *residual_out, const Plan &pl, char *ws, unsigned int *list_cnt, cudaStream_t stream) {
-  const int G = v->G, M = pl.M, tpt = tc::kTileM / M;
-  EncodeTiledFn fn = encode_tiled_fn();
-  if (!fn) { set_error("cuTensorMapEncodeTiled entry point not available"); return GSRQ_ECUDA; }
-  // dims {16, M, T, G} (or {16, M, G, T} when the head stride is the smaller one); strides in bytes
-  const bool head_inner = v->stride_g < v->stride_t;
+// One pass: stages [s0, s0 + ns) of cb over N rows per group.  res_in == nullptr: rows come from the bf16 tensor kv.
+static int run_encode_tc_pass(const void *kv, const gsrq_view *v, const gsrq_codebook *cb, int s0, int ns, long long N, uint8_t *codes,
+                              long long code_stride_s, const float *res_in, float *res_out, const Plan &pl, char *ws,
+                              unsigned int *list_cnt, cudaStream_t stream) {
+  const int G = v->G, M = pl.M, tpt = tc::kTileM / (res_in ? 1 : M);
   CUtensorMap tm;
-  const cuuint64_t dims[4] = {(cuuint64_t)tc::kD, (cuuint64_t)M, (cuuint64_t)(head_inner ? G : v->T), (cuuint64_t)(head_inner ? v->T : G)};
-  const cuuint64_t strides[3] = {(cuuint64_t)tc::kD * 2, (cuuint64_t)(head_inner ? v->stride_g : v->stride_t) * 2,
-                                 (cuuint64_t)(head_inner ? v->stride_t : v->stride_g) * 2};
-  const cuuint32_t box[4] = {(cuuint32_t)tc::kD, (cuuint32_t)M, (cuuint32_t)(head_inner ? 1 : tpt), (cuuint32_t)(head_inner ? tpt : 1)};
-  const cuuint32_t es[4] = {1, 1, 1, 1};
-  CUresult r = fn(&tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void *>(kv), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                  CU_TENSOR_MAP_SWIZZLE_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  if (r != CUDA_SUCCESS) { set_error("cuTensorMapEncodeTiled (kv) failed (%d)", (int)r); return GSRQ_ECUDA; }
+  memset(&tm, 0, sizeof(tm));
+  bool head_inner = false;
+  if (!res_in) {
+    EncodeTiledFn fn = encode_tiled_fn();
+    if (!fn) { set_error("cuTensorMapEncodeTiled entry point not available"); return GSRQ_ECUDA; }
+    // dims {16, M, T, G} (or {16, M, G, T} when the head stride is the smaller one); strides in bytes
+    head_inner = v->stride_g < v->stride_t;
+    const cuuint64_t dims[4] = {(cuuint64_t)tc::kD, (cuuint64_t)M, (cuuint64_t)(head_inner ? G : v->T), (cuuint64_t)(head_inner ? v->T : G)};
+    const cuuint64_t strides[3] = {(cuuint64_t)tc::kD * 2, (cuuint64_t)(head_inner ? v->stride_g : v->stride_t) * 2,
+                                   (cuuint64_t)(head_inner ? v->stride_t : v->stride_g) * 2};
+    const cuuint32_t box[4] = {(cuuint32_t)tc::kD, (cuuint32_t)M, (cuuint32_t)(head_inner ? 1 : tpt), (cuuint32_t)(head_inner ? tpt : 1)};
+    const cuuint32_t es[4] = {1, 1, 1, 1};
+    CUresult r = fn(&tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void *>(kv), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                    CU_TENSOR_MAP_SWIZZLE_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { set_error("cuTensorMapEncodeTiled (kv) failed (%d)", (int)r); return GSRQ_ECUDA; }
+  }
   uint8_t *bimg = (uint8_t *)(ws + pl.off_ebimg);
   int *gmax = (int *)(ws + pl.off_egmax);
-  LAUNCH(kClsMisc, stream, (tc::k_bimg<<<G * n_stages, 256, 0, stream>>>(cb->shapes, cb->gains, (long long)cb->S * cb->K, n_stages, cb->K, 0, bimg, gmax)));
+  LAUNCH(kClsMisc, stream, (tc::k_bimg<<<G * ns, 256, 0, stream>>>(cb->shapes + (size_t)s0 * cb->K * tc::kD, cb->gains + (size_t)s0 * cb->K,
+                                                                    (long long)cb->S * cb->K, ns, cb->K, 0, bimg, gmax)));
   GSRQ_CUDA_CHECK(cudaGetLastError());
   tc::EncTcParams p{};
-  p.bimg = bimg; p.gmax = gmax; p.shapes = cb->shapes; p.gains = cb->gains; p.S = cb->S; p.K = cb->K; p.n_stages = n_stages;
-  p.codes = codes; p.code_stride_s = (long long)G * pl.Nall; p.res_out = residual_out; p.N = pl.Nall;
-  p.n_tiles = (int)((v->T + tpt - 1) / tpt);
+  p.bimg = bimg; p.gmax = gmax; p.shapes = cb->shapes; p.gains = cb->gains; p.S = cb->S; p.K = cb->K; p.n_stages = ns; p.s0 = s0;
+  p.res_in = res_in; p.codes = codes; p.code_stride_s = code_stride_s; p.res_out = res_out; p.N = N;
+  p.n_tiles = (int)((N + tc::kTileM - 1) / tc::kTileM);
+  if (!res_in) p.n_tiles = (int)((v->T + tpt - 1) / tpt);
   p.list = (uint2 *)(ws + pl.off_list); p.list_cnt = list_cnt;
   static int n_sm = 0;
   if (!n_sm) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev); if (n_sm <= 0) n_sm = 148; }
   int ctas = n_sm / G; if (ctas < 1) ctas = 1; if (ctas > p.n_tiles) ctas = p.n_tiles;
   const size_t smem = tc::kEncSmemTotal;
   static bool attr_set = false;
-  if (!attr_set) { GSRQ_CUDA_CHECK(cudaFuncSetAttribute(tc::k_encode_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr_set = true; }
-  LAUNCH(kClsEncode, stream, (tc::k_encode_tc<<<dim3((unsigned)ctas, (unsigned)G), tc::kThreads, smem, stream>>>(tm, p, tpt, head_inner ? 1 : 0)));
+  if (!attr_set) {
+    GSRQ_CUDA_CHECK(cudaFuncSetAttribute(tc::k_encode_tc<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    GSRQ_CUDA_CHECK(cudaFuncSetAttribute(tc::k_encode_tc<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    attr_set = true;
+  }
+  if (res_in)
+    LAUNCH(kClsEncode, stream, (tc::k_encode_tc<true><<<dim3((unsigned)ctas, (unsigned)G), tc::kThreads, smem, stream>>>(tm, p, tpt, 0)));
+  else
+    LAUNCH(kClsEncode, stream, (tc::k_encode_tc<false><<<dim3((unsigned)ctas, (unsigned)G), tc::kThreads, smem, stream>>>(tm, p, tpt, head_inner ? 1 : 0)));
   GSRQ_CUDA_CHECK(cudaGetLastError());
+  return GSRQ_OK;
+}
+
+// Stages [0, n_stages) over rows (kv through view, or the fp32 rows `rows0` [G][N][16] when kv == nullptr), in passes of
+// kEncMaxS stages; after every pass the exact kernel finishes the rows the filter could not decide.  `carry` is the
+// fp32 residual buffer between passes (and the result when the caller wants the residual); may alias rows0.
+static int run_encode_tc(const void *kv, const gsrq_view *v, const float *rows0, long long N, const gsrq_codebook *cb, int n_stages,
+                         uint8_t *codes, long long code_stride_s, float *carry, bool want_residual, const Plan &pl, char *ws,
+                         unsigned int *cnt_base, cudaStream_t stream) {
+  const int d = v->d;
+  const float *cur = (kv && v->dtype == GSRQ_BF16) ? nullptr : (kv ? (const float *)kv : rows0);  // nullptr: TMA from the bf16 tensor
+  int pass = 0;
+  for (int s0 = 0; s0 < n_stages; s0 += tc::kEncMaxS, ++pass) {
+    const int ns = (n_stages - s0 < tc::kEncMaxS) ? n_stages - s0 : tc::kEncMaxS;
+    const bool last = s0 + ns == n_stages;
+    float *out = (last && !want_residual) ? nullptr : carry;
+    unsigned int *lc = cnt_base + pass;  // a fresh, zeroed counter per pass
+    int rc = run_encode_tc_pass(kv, v, cb, s0, ns, N, codes, code_stride_s, cur, out, pl, ws, lc, stream);
+    if (rc) return rc;
+    EncParams e{};
+    if (cur) e.src = make_src(nullptr, v, cur, N); else e.src = make_src(kv, v, nullptr, 0);
+    e.N = N; e.shapes = cb->shapes; e.gains = cb->gains; e.S = cb->S; e.K = cb->K;
+    e.s_first = s0; e.s_begin = s0; e.s_end = s0 + ns; e.s_base = 0; e.mode = 0; e.subtract = 1;
+    e.codes = codes; e.code_stride_s = code_stride_s; e.res_out = out; e.st = nullptr; e.slot = 0;
+    e.list = (uint2 *)(ws + pl.off_list); e.list_cnt = lc;
+    LAUNCH(kClsRefine, stream, DISPATCH_D(d, (k_encode_exact<D><<<1184, 256, 0, stream>>>(e))));
+    GSRQ_CUDA_CHECK(cudaGetLastError());
+    cur = carry;
+  }
   return GSRQ_OK;
 }
 
@@ -446,21 +504,18 @@ int gsrq_encode(const void *kv, const gsrq_view *view, const gsrq_codebook *cb, 
   if (rc) return rc;
   char *ws = (char *)workspace;
   unsigned int *cnt = (unsigned int *)(ws + pl.off_cnt);
-  GSRQ_CUDA_CHECK(cudaMemsetAsync(cnt, 0, sizeof(unsigned int), stream));
+  GSRQ_CUDA_CHECK(cudaMemsetAsync(cnt, 0, 16 * sizeof(unsigned int), stream));
   EncParams p{};
   p.src = make_src(kv, view, nullptr, 0);
   p.N = pl.Nall; p.shapes = cb->shapes; p.gains = cb->gains; p.S = cb->S; p.K = cb->K;
   p.s_begin = stage_begin; p.s_end = stage_end; p.s_base = 0; p.mode = 0; p.subtract = 1;
   p.codes = codes; p.code_stride_s = (long long)view->G * pl.Nall; p.res_out = residual_out;
   p.st = nullptr; p.slot = 0; p.list = (uint2 *)(ws + pl.off_list); p.list_cnt = cnt;
-  if (can_encode_tc(kv, view, stage_begin, stage_end)) {
-    // tensor-core filter over all stages; rows it cannot decide go to the exact path below
-    rc = run_encode_tc(kv, view, cb, stage_end, codes, residual_out, pl, ws, cnt, stream);
-    if (rc) return rc;
-    const int d = view->d;
-    LAUNCH(kClsRefine, stream, DISPATCH_D(d, (k_encode_exact<D><<<1184, 256, 0, stream>>>(p))));
-    GSRQ_CUDA_CHECK(cudaGetLastError());
-    return GSRQ_OK;
+  if (can_encode_tc(kv, view, stage_begin)) {
+    // tensor-core passes of <= 4 stages; after each, the exact kernel finishes the rows the filter could not decide
+    float *carry = residual_out ? residual_out : (float *)(ws + pl.off_eres);
+    return run_encode_tc(kv, view, nullptr, pl.Nall, cb, stage_end, codes, (long long)view->G * pl.Nall, carry, residual_out != nullptr, pl, ws,
+                         cnt, stream);
   }
   return run_encode(p, view->G, view->d, stream);
 }
@@ -740,7 +795,7 @@ int gsrq_pipeline_host(const void *kv_host, const gsrq_view *view, const float *
   for (int s = 0; s < S && rc == GSRQ_OK && e == cudaSuccess; ++s) {
     rc = gsrq_fit_stage(d_kv, view, d_w, 0, nullptr, 0, &cb, s, s ? d_res : nullptr, iters, seed, nullptr, d_ws, wsb, stream);
     // the fused tensor-core encode restarts from stage 0 (cheap); otherwise only stage s is encoded
-    const int sb = can_encode_tc(d_kv, view, 0, s + 1) ? 0 : s;
+    const int sb = can_encode_tc(d_kv, view, 0) ? 0 : s;
     if (rc == GSRQ_OK) rc = gsrq_encode(d_kv, view, &cb, sb, s + 1, d_codes, (s + 1 < S) ? d_res : nullptr, d_ws, wsb, stream);
   }
   if (rc == GSRQ_OK && e == cudaSuccess && kv_out_host) {

@@ -36,8 +36,10 @@ struct EncTcParams {
   const int *gmax;         // [G][n_stages] bit pattern of max_k g_k
   const float *shapes;     // [G][S][K][16]
   const float *gains;      // [G][S][K]
-  int S, K, n_stages;
-  uint8_t *codes;          // plane s, group g, row i at codes[s*code_stride_s + g*N + i]
+  int S, K, n_stages;      // cb->S, K, stages of this pass
+  int s0;                  // first stage of this pass (absolute index into the codebook / code planes)
+  const float *res_in;     // FROM_ROWS: [G][N][16] fp32 rows the pass starts from (may alias res_out)
+  uint8_t *codes;          // plane s, group g, row i at codes[s*code_stride_s + g*N + i]; nullptr: no codes wanted
   long long code_stride_s;
   float *res_out;          // [G][N][16] or nullptr
   long long N;             // rows per group
@@ -54,6 +56,10 @@ __device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap *tm,
 
 // tm_kv: 4-D map over the KV tensor {16 (contiguous), M, T, G} ({16, M, G, T} when head_inner), box {16, M, 128 / M, 1}, SWIZZLE_32B:
 // one box is the 128 consecutive rows (t, m) of a tile, laid out as the K-major A operand.
+// FROM_ROWS = false: stage s0 = 0 reads the bf16 rows of the KV tensor through tm_kv (exact single-plane operand).
+// FROM_ROWS = true : the pass starts from fp32 rows (a residual, or an fp32 tensor): the epilogue loads them, builds the
+//                    two operand planes itself and every stage runs the two-plane MMAs; tm_kv is unused.
+template <bool FROM_ROWS>
 __global__ void __launch_bounds__(kThreads, 1) k_encode_tc(const __grid_constant__ CUtensorMap tm_kv, EncTcParams p, int tok_per_tile,
                                                                   int head_inner) {
   extern __shared__ uint8_t smem_raw[];
@@ -95,7 +101,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_encode_tc(const __grid_constant
     if (lane == 0) {
       mbar_expect_tx(b_full, (uint32_t)S * 3 * kBImgBytes);
       bulk_g2s(sbase, p.bimg + (size_t)g * S * 3 * kBImgBytes, (uint32_t)S * 3 * kBImgBytes, b_full);
-      for (int it = 0; it < n_my; ++it) {
+      for (int it = 0; it < (FROM_ROWS ? 0 : n_my); ++it) {
         const int st = it % kEncStages, ph = (it / kEncStages) & 1;
         const int tile = blockIdx.x + it * gridDim.x;
         mbar_wait(empty_a(st), ph ^ 1);
@@ -118,7 +124,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_encode_tc(const __grid_constant
             const int it = 2 * pr + b;
             if (it >= n_my) continue;
             const uint32_t d = tmem_base + b * kN;
-            if (s == 0) {
+            if (s == 0 && !FROM_ROWS) {
               const int st = it % kEncStages, ph = (it / kEncStages) & 1;
               mbar_wait(tmem_empty(b), (pr & 1) ^ 1);
               mbar_wait(full_a(st), ph);
@@ -127,7 +133,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_encode_tc(const __grid_constant
               mma_f16(d, d_a, d_bhi, kIdesc, 0);
               mma_f16(d, d_a, d_blo, kIdesc, 1);
             } else {
-              mbar_wait(planes_ready(b), (uint32_t)((pr * (S - 1) + (s - 1)) & 1));
+              if (FROM_ROWS && s == 0) mbar_wait(tmem_empty(b), (pr & 1) ^ 1);
+              mbar_wait(planes_ready(b), FROM_ROWS ? (uint32_t)((pr * S + s) & 1) : (uint32_t)((pr * (S - 1) + (s - 1)) & 1));
               tc_fence_after();
               const uint64_t d_hi = make_desc_sw32(sbase + kEncSmemP + (2 * b) * kPlaneBytes);
               const uint64_t d_lo = make_desc_sw32(sbase + kEncSmemP + (2 * b + 1) * kPlaneBytes);
@@ -156,8 +163,36 @@ __global__ void __launch_bounds__(kThreads, 1) k_encode_tc(const __grid_constant
       const long long gr = (long long)g * p.N + row;
       bool alive = row < p.N;
       float r[kD];
+      auto publish_planes = [&]() {  // operand planes of r for the next MMAs: R_hi = bf16(r), R_lo = bf16(r - R_hi)
+        uint32_t h[8], l[8];
+#pragma unroll
+        for (int j = 0; j < kD; j += 2) {  // one packed conversion per pair; the high half is re-read by masking
+          const __nv_bfloat162 hp = __floats2bfloat162_rn(r[j], r[j + 1]);
+          h[j / 2] = *reinterpret_cast<const uint32_t *>(&hp);
+          const float d0 = __fsub_rn(r[j], __uint_as_float(h[j / 2] << 16));
+          const float d1 = __fsub_rn(r[j + 1], __uint_as_float(h[j / 2] & 0xFFFF0000u));
+          const __nv_bfloat162 lp = __floats2bfloat162_rn(d0, d1);
+          l[j / 2] = *reinterpret_cast<const uint32_t *>(&lp);
+        }
+        uint8_t *ph_ = planes + r_in_tile * 32, *pl_ = planes + kPlaneBytes + r_in_tile * 32;
+        *reinterpret_cast<uint4 *>(ph_ + (0u ^ sw)) = make_uint4(h[0], h[1], h[2], h[3]);
+        *reinterpret_cast<uint4 *>(ph_ + (16u ^ sw)) = make_uint4(h[4], h[5], h[6], h[7]);
+        *reinterpret_cast<uint4 *>(pl_ + (0u ^ sw)) = make_uint4(l[0], l[1], l[2], l[3]);
+        *reinterpret_cast<uint4 *>(pl_ + (16u ^ sw)) = make_uint4(l[4], l[5], l[6], l[7]);
+        fence_proxy_async();   // generic-proxy writes -> visible to the tensor core's async proxy
+        tc_fence_before();     // this stage's tcgen05.ld is complete before the next MMAs overwrite the accumulator
+        __syncwarp();
+        if (lane == 0) mbar_arrive(planes_ready(wg));
+      };
       for (int s = 0; s < S; ++s) {
-        if (s == 0) {  // the row itself, from the TMA-staged tile (exact bf16 -> fp32)
+        if (s == 0 && FROM_ROWS) {  // the pass starts from fp32 rows
+          if (row < p.N) load_row_f32<kD>(p.res_in, gr, r);
+          else {
+#pragma unroll
+            for (int j = 0; j < kD; ++j) r[j] = 0.0f;
+          }
+          publish_planes();
+        } else if (s == 0) {  // the row itself, from the TMA-staged tile (exact bf16 -> fp32)
           mbar_wait(full_a(st), ph);
           const uint8_t *ar = sgen + kEncSmemA + st * kPlaneBytes + r_in_tile * 32;
           const uint4 c0 = *reinterpret_cast<const uint4 *>(ar + (0u ^ sw));
@@ -174,10 +209,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_encode_tc(const __grid_constant
         for (int j = 0; j < kD; ++j) n2 = fmaf(r[j], r[j], n2);
         const float rn = sqrtf(n2) * 1.00001f;  // upper bound of ||r||
         const float gm = __int_as_float(p.gmax[g * S + s]);
-        const float rho17 = (s == 0 ? 2.0f : 4.5f) * 7.62939453125e-6f;  // rho 2^-17: one / two operand planes
+        const float rho17 = ((s == 0 && !FROM_ROWS) ? 2.0f : 4.5f) * 7.62939453125e-6f;  // rho 2^-17: one / two operand planes
         mbar_wait(tmem_full(wg), (uint32_t)((pr * S + s) & 1));
         tc_fence_after();
-        if (s == 0) {  // stage-0 MMAs are done with the tile and this warp has its rows: free the ring slot
+        if (s == 0 && !FROM_ROWS) {  // stage-0 MMAs are done with the tile and this warp has its rows: free the ring slot
           __syncwarp();
           if (lane == 0) mbar_arrive(empty_a(st));
         }
@@ -192,16 +227,18 @@ __global__ void __launch_bounds__(kThreads, 1) k_encode_tc(const __grid_constant
           }
         });
         const int k = gi * 16 + ji;
-        const long long cw = ((long long)g * p.S + s) * p.K + min(k, p.K - 1);
+        const long long cw = ((long long)g * p.S + p.s0 + s) * p.K + min(k, p.K - 1);
         const float gk = __ldg(p.gains + cw);
         const float E2 = decision_margin(best, rn, gk, gm, rho17, 0);
         if (alive && best - second <= E2) {  // ambiguous: the exact path takes the row over from this stage
           const uint32_t gmask = candidate_groups(gmA, best, E2);  // groups of 16 columns within the margin: the only candidates
           const unsigned int pos = atomicAdd(p.list_cnt, 1u);
-          p.list[pos] = make_uint2((uint32_t)gr, gmask | ((uint32_t)s << 16));
+          // without a code plane the decided stages of this pass cannot be replayed: the exact path restarts the pass
+          p.list[pos] = p.codes ? make_uint2((uint32_t)gr, gmask | ((uint32_t)(p.s0 + s) << 16))
+                                : make_uint2((uint32_t)gr, 0xFFFFu | ((uint32_t)p.s0 << 16));
           alive = false;
         }
-        if (alive) p.codes[(long long)s * p.code_stride_s + gr] = (uint8_t)k;
+        if (alive && p.codes) p.codes[(long long)(p.s0 + s) * p.code_stride_s + gr] = (uint8_t)k;
         // r <- fl32(r - fl32(g_k s_k)): the codeword comes from the fp32 codebook (L1-resident)
         const float4 *sp = reinterpret_cast<const float4 *>(p.shapes + cw * kD);
 #pragma unroll
@@ -213,25 +250,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_encode_tc(const __grid_constant
           r[4 * v + 3] = __fsub_rn(r[4 * v + 3], __fmul_rn(gk, sv.w));
         }
         if (s + 1 < S) {  // operand planes of the residual for the next stage
-          uint32_t h[8], l[8];
-#pragma unroll
-          for (int j = 0; j < kD; j += 2) {  // one packed conversion per pair; the high half is re-read by masking
-            const __nv_bfloat162 hp = __floats2bfloat162_rn(r[j], r[j + 1]);
-            h[j / 2] = *reinterpret_cast<const uint32_t *>(&hp);
-            const float d0 = __fsub_rn(r[j], __uint_as_float(h[j / 2] << 16));
-            const float d1 = __fsub_rn(r[j + 1], __uint_as_float(h[j / 2] & 0xFFFF0000u));
-            const __nv_bfloat162 lp = __floats2bfloat162_rn(d0, d1);
-            l[j / 2] = *reinterpret_cast<const uint32_t *>(&lp);
-          }
-          uint8_t *ph_ = planes + r_in_tile * 32, *pl_ = planes + kPlaneBytes + r_in_tile * 32;
-          *reinterpret_cast<uint4 *>(ph_ + (0u ^ sw)) = make_uint4(h[0], h[1], h[2], h[3]);
-          *reinterpret_cast<uint4 *>(ph_ + (16u ^ sw)) = make_uint4(h[4], h[5], h[6], h[7]);
-          *reinterpret_cast<uint4 *>(pl_ + (0u ^ sw)) = make_uint4(l[0], l[1], l[2], l[3]);
-          *reinterpret_cast<uint4 *>(pl_ + (16u ^ sw)) = make_uint4(l[4], l[5], l[6], l[7]);
-          fence_proxy_async();   // generic-proxy writes -> visible to the tensor core's async proxy
-          tc_fence_before();     // this stage's tcgen05.ld is complete before the next MMAs overwrite the accumulator
-          __syncwarp();
-          if (lane == 0) mbar_arrive(planes_ready(wg));
+          publish_planes();
         } else if (alive && p.res_out) {
           store_row_f32<kD>(p.res_out, gr, r);
         }

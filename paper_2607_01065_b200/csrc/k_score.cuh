@@ -17,6 +17,7 @@ struct EncParams {
   const float *shapes;  // [G][S][K][D]
   const float *gains;   // [G][S][K]
   int S, K;
+  int s_first;          // exact path only: first stage applied to src (src holds the residual after stage s_first - 1)
   int s_begin, s_end;   // stages scored in this pass; stages < s_begin are replayed from codes
   int s_base;           // code plane index = s - s_base
   int mode;             // 0: Eq. 5 score, 1: plain projection (init assignment, reading c-I)
@@ -259,7 +260,7 @@ __global__ void __launch_bounds__(256) k_encode_exact(EncParams p) {
     const long long i = gi - (long long)g * p.N;
     float x[D];
     load_src_row<D>(p.src, g, i, x);
-    for (int s = 0; s < p.s_end; ++s) {
+    for (int s = p.s_first; s < p.s_end; ++s) {
       const float *sh = p.shapes + ((long long)g * p.S + s) * p.K * D;
       const float *ga = p.gains + ((long long)g * p.S + s) * p.K;
       int k;

@@ -214,3 +214,35 @@ def test_encode_on_append_equals_batch_encode(B, dtype, hd, d, head_inner):
     assert np.array_equal(codes.cpu().numpy(), codes_o)
     with pytest.raises(B.GsrqError):
         B.gsrq_encode_append(chunk, B.view_of(chunk, d, head_inner), cb, S, codes, T * M, T)   # does not fit
+
+
+@pytest.mark.parametrize("S,dtype,hd,K", [(8, "bf16", 128, 256), (10, "bf16", 64, 100), (5, "f32", 128, 256), (2, "f32", 16, 64)])
+def test_tc_encode_chained_passes_and_fp32_rows(B, S, dtype, hd, K):
+    """More than 4 stages run as chained tensor-core passes through an fp32 residual (the paper's deep residual
+    quantisers: R = 12..32), and a dense fp32 tensor with d = 16 starts from fp32 rows: codes,
+    residual and decode must equal the oracle, with and without a residual output."""
+    rng = np.random.default_rng(S * 7 + hd)
+    G, T = 3, 210
+    x = rng.standard_normal((G, T, hd)) * np.exp(0.5 * rng.standard_normal((G, T, 1)))
+    x = inputs.bf16_round(x) if dtype == "bf16" else x.astype(np.float32)
+    sh = rng.standard_normal((G, S, K, 16))
+    sh = (sh / np.linalg.norm(sh, axis=-1, keepdims=True)).astype(np.float32)
+    ga = np.abs(rng.standard_normal((G, S, K)) * (2.0 / (1 + np.arange(S))[None, :, None])).astype(np.float32)
+    codes_o, res_o, _, _ = o.encode(x, sh, ga, 16)
+    xd = to_device(x, dtype)
+    view = B.view_of(xd, 16)
+    sh_d, ga_d = torch.from_numpy(sh).cuda(), torch.from_numpy(ga).cuda()
+    cb = B.codebook_of(sh_d, ga_d)
+    ws = B.workspace(view, K, S, -1)
+    M = hd // 16
+    for want_res in (True, False):
+        codes = torch.zeros(S, G, T * M, dtype=torch.uint8, device="cuda")
+        res = torch.zeros(G, T * M, 16, device="cuda") if want_res else None
+        B.gsrq_encode(xd, view, cb, 0, S, codes, res, ws)
+        torch.cuda.synchronize()
+        assert np.array_equal(codes.cpu().numpy(), codes_o), (S, want_res)
+        if want_res:
+            assert np.array_equal(res.cpu().numpy(), res_o)
+    dec = gpu_decode(codes, cb, S, G, T, hd, 16, dtype=dtype)
+    want, _ = o.decode(codes_o, sh, ga, hd, bf16=(dtype == "bf16"))
+    assert np.array_equal(dec, want)
