@@ -534,12 +534,13 @@ int gsrq_decode(const uint8_t *codes, const gsrq_codebook *cb, int n_stages, voi
   p.stride_g = out_view->stride_g; p.stride_t = out_view->stride_t;
   p.row_begin = 0;
   // bandwidth path: full 256-row chunks (d == 16, 1..4 stages, 16-byte aligned code planes)
-  if (d == 16 && n_stages >= 1 && n_stages <= 4 && p.N % 16 == 0 && p.N >= 256 && ((uintptr_t)codes & 15) == 0) {
+  if (d == 16 && n_stages >= 1 && n_stages <= kDecDeep && p.N % 16 == 0 && p.N >= 256 && ((uintptr_t)codes & 15) == 0) {
     const long long n_chunks = p.N / 256;
     const bool dense = out_view->stride_t == out_view->hd;
     static int n_sm = 0;
     if (!n_sm) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev); if (n_sm <= 0) n_sm = 148; }
-    const size_t smem = (size_t)n_stages * kDecTabBytes;
+    const bool deep = n_stages > 4;  // single-copy tables
+    const size_t smem = deep ? (size_t)n_stages * (kDecTabBytes / 2) : (size_t)n_stages * kDecTabBytes;
     int per_sm = (int)((227 * 1024) / (smem + 1024));  // CTAs that fit on one SM (shared memory; 40 registers x 512 threads)
     if (per_sm > 2) per_sm = 2;  // measured: a third CTA per SM lowers the achieved bandwidth
     if (per_sm < 1) per_sm = 1;
@@ -552,6 +553,15 @@ int gsrq_decode(const uint8_t *codes, const gsrq_codebook *cb, int n_stages, voi
     GSRQ_CUDA_CHECK(cudaFuncSetAttribute(k_decode_fast<NS, DENSE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
     LAUNCH(kClsDecode, stream, (k_decode_fast<NS, DENSE><<<grid, kDecThreads, smem, stream>>>(p, n_chunks)));                \
   } while (0)
+    if (deep) {
+      if (dense) {
+        GSRQ_CUDA_CHECK(cudaFuncSetAttribute(k_decode_fast<kDecDeep, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        LAUNCH(kClsDecode, stream, (k_decode_fast<kDecDeep, true, false><<<grid, kDecThreads, smem, stream>>>(p, n_chunks)));
+      } else {
+        GSRQ_CUDA_CHECK(cudaFuncSetAttribute(k_decode_fast<kDecDeep, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        LAUNCH(kClsDecode, stream, (k_decode_fast<kDecDeep, false, false><<<grid, kDecThreads, smem, stream>>>(p, n_chunks)));
+      }
+    } else
     switch (n_stages * 2 + (dense ? 1 : 0)) {
       case 2: GSRQ_DEC_FAST(1, false); break;
       case 3: GSRQ_DEC_FAST(1, true); break;

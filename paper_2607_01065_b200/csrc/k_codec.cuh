@@ -109,24 +109,30 @@ __global__ void __launch_bounds__(256) k_decode(DecParams p) {
 // Mapping: a warp owns 256 consecutive rows and decodes 8 consecutive rows per iteration, 4 lanes
 // (one 4-element quarter each) per row.
 constexpr int kDecThreads = 512;
-constexpr int kDecTabBytes = 256 * 128;  // per stage
+constexpr int kDecTabBytes = 256 * 128;  // per stage (duplicated rows)
+constexpr int kDecDeep = 12;             // stages of the single-copy variant (256 * 64 bytes per stage)
 
-template <int NS, bool DENSE>
+// DUP = true : NS = number of stages (1..4), duplicated table rows (128 bytes), conflict-free.
+// DUP = false: NS = kDecDeep = upper bound, p.n_stages (5..kDecDeep) stages decoded; single-copy table rows (64 bytes:
+//              two codewords of equal parity in one LDS phase conflict 2-way) so that 12 stages fit in shared memory.
+template <int NS, bool DENSE, bool DUP = true>
 __global__ void __launch_bounds__(kDecThreads) k_decode_fast(DecParams p, long long n_chunks) {
   extern __shared__ __align__(16) float tab[];
+  constexpr int RS = DUP ? 32 : 16;  // floats per table row
+  const int ns = DUP ? NS : p.n_stages;
   const int g = blockIdx.y;
-  for (int e = threadIdx.x; e < NS * p.K * 16; e += kDecThreads) {
+  for (int e = threadIdx.x; e < ns * p.K * 16; e += kDecThreads) {
     const int s = e / (p.K * 16), r = e - s * p.K * 16, k = r >> 4, j = r & 15;
     const long long cb = ((long long)g * p.S + s) * p.K + k;
     const float v = __fmul_rn(p.gains[cb], p.shapes[cb * 16 + j]);
-    float *row = tab + ((size_t)s * 256 + k) * 32;
+    float *row = tab + ((size_t)s * 256 + k) * RS;
     row[j] = v;
-    row[16 + j] = v;
+    if (DUP) row[16 + j] = v;
   }
   __syncthreads();
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int slot = lane >> 2, c4 = lane & 3;
-  const float *tl = tab + (lane & 7) * 4;
+  const float *tl = tab + (DUP ? (lane & 7) : (lane & 3)) * 4;
   const int msh = ((p.M & (p.M - 1)) == 0) ? (31 - __clz(p.M)) : -1;
   const long long ch0 = (long long)blockIdx.x * (kDecThreads / 32) + warp, chs = (long long)gridDim.x * (kDecThreads / 32);
   // lane l holds the 8 code bytes of rows 8l..8l+7 of the chunk (one coalesced 256-byte load per stage),
@@ -136,7 +142,7 @@ __global__ void __launch_bounds__(kDecThreads) k_decode_fast(DecParams p, long l
   if (ch0 < n_chunks) {
 #pragma unroll
     for (int s = 0; s < NS; ++s)
-      nx[s] = __ldcs(reinterpret_cast<const uint2 *>(p.codes + ((long long)s * p.G + g) * p.N + ch0 * 256) + lane);
+      if (s < ns) nx[s] = __ldcs(reinterpret_cast<const uint2 *>(p.codes + ((long long)s * p.G + g) * p.N + ch0 * 256) + lane);
   }
   for (long long ch = ch0; ch < n_chunks; ch += chs) {
     uint2 cw[NS];
@@ -145,16 +151,17 @@ __global__ void __launch_bounds__(kDecThreads) k_decode_fast(DecParams p, long l
     if (ch + chs < n_chunks) {
 #pragma unroll
       for (int s = 0; s < NS; ++s)
-        nx[s] = __ldcs(reinterpret_cast<const uint2 *>(p.codes + ((long long)s * p.G + g) * p.N + (ch + chs) * 256) + lane);
+        if (s < ns) nx[s] = __ldcs(reinterpret_cast<const uint2 *>(p.codes + ((long long)s * p.G + g) * p.N + (ch + chs) * 256) + lane);
     }
 #pragma unroll 8
     for (int u = 0; u < 32; ++u) {
       float4 acc;
 #pragma unroll
       for (int s = 0; s < NS; ++s) {
+        if (s >= ns) break;
         const uint32_t lo = __shfl_sync(0xffffffffu, cw[s].x, u), hi = __shfl_sync(0xffffffffu, cw[s].y, u);
         const uint32_t k = (((slot & 4) ? hi : lo) >> (8 * (slot & 3))) & 0xFFu;
-        const float4 c = *reinterpret_cast<const float4 *>(tl + ((size_t)s * 256 + k) * 32);
+        const float4 c = *reinterpret_cast<const float4 *>(tl + ((size_t)s * 256 + k) * RS);
         if (s == 0) acc = c;
         else {
           acc.x = __fadd_rn(acc.x, c.x); acc.y = __fadd_rn(acc.y, c.y);

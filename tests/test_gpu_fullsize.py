@@ -121,9 +121,11 @@ def test_tc_encode_all_rows_ambiguous(B):
 
 
 @pytest.mark.parametrize("T,S,dtype,head_inner", [(100, 1, "bf16", False), (100, 2, "f32", False), (515, 3, "bf16", True),
-                                                  (32, 4, "bf16", False), (31, 2, "bf16", False), (4096, 4, "bf16", True)])
+                                                  (32, 4, "bf16", False), (31, 2, "bf16", False), (4096, 4, "bf16", True),
+                                                  (300, 7, "bf16", True), (130, 12, "f32", False), (64, 14, "bf16", False)])
 def test_decode_bandwidth_path_and_tail(B, T, S, dtype, head_inner):
-    """Decode: full 256-row chunks through k_decode_fast, the ragged tail through the generic kernel;
+    """Decode: full 256-row chunks through k_decode_fast (1-4 stages: duplicated tables; 5-12: single-copy tables; more:
+    generic kernel), the ragged tail through the generic kernel;
     N % 16 != 0 (T = 31... with M = 8 always a multiple of 8 only) falls back entirely.  Bit-exact."""
     rng = np.random.default_rng(T * 10 + S)
     G, hd, K = 2, 128, 256
