@@ -452,8 +452,8 @@ def main():
     tot_ms = sum(v[0] for v in prof.values())
 
     # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the cfg-1 kernels from the ncu --set full
-    # captures summarised in profiles/r1_v4_ncu_full.md; None for workloads that were not captured
-    NCU_TRAFFIC = {"score": 10.09e6, "update": 21.41e6} if c.cfg == 1 else {}
+    # captures summarised in profiles/r1_v5_ncu_full.md; None for workloads that were not captured
+    NCU_TRAFFIC = {"score": 10.09e6, "update": 21.42e6} if c.cfg == 1 else {}
 
     def kern(name, cls, bound, work_per_launch, peak, unit):
         ms, n = prof[cls]
