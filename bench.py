@@ -432,6 +432,9 @@ def main():
     h2d = x_host.numel() * 2 + w_host.numel() * 4
     d2h = sh_h.numel() * 4 + ga_h.numel() * 4 + co_h.numel() + out_h.numel() * 2
     clocks = sampler.finish(t_region0, time.perf_counter())
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()      # no collective below: the remaining legs run on rank 0 alone
 
     if rank != 0:
         return
