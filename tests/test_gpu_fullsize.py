@@ -248,3 +248,92 @@ def test_tc_encode_chained_passes_and_fp32_rows(B, S, dtype, hd, K):
     dec = gpu_decode(codes, cb, S, G, T, hd, 16, dtype=dtype)
     want, _ = o.decode(codes_o, sh, ga, hd, bf16=(dtype == "bf16"))
     assert np.array_equal(dec, want)
+
+
+def _sampled_encode_decode_check(B, x_dev, view, head_inner, cb, shapes, gains, S, tok, d=16):
+    """Full-tensor encode + decode on the GPU; the oracle encodes / decodes the sampled tokens one by one with the same
+    (GPU-fitted) codebooks.  A token's codes depend on that token's rows only."""
+    G, T, hd = view.G, view.T, view.hd
+    M = hd // d
+    ws = B.workspace(view, cb.K, S, -1)
+    codes = torch.zeros(S, G, T * M, dtype=torch.uint8, device="cuda")
+    B.gsrq_encode(x_dev, view, cb, 0, S, codes, None, ws)
+    out = torch.empty_like(x_dev)
+    B.gsrq_decode(codes, cb, S, out, view)
+    torch.cuda.synchronize()
+    tok_d = torch.from_numpy(tok).cuda()
+    xs = (x_dev[tok_d].permute(1, 0, 2) if head_inner else x_dev[:, tok_d]).float().cpu().numpy()      # [G][n][hd]
+    outs = (out[tok_d].permute(1, 0, 2) if head_inner else out[:, tok_d]).float().cpu().numpy()
+    rows = (tok_d[:, None] * M + torch.arange(M, device="cuda")[None]).reshape(-1)
+    codes_s = codes[:, :, rows].cpu().numpy()
+    codes_o, res_o, _, _ = o.encode(xs, shapes, gains, d, stage_end=S)
+    assert np.array_equal(codes_s, codes_o)
+    want, _ = o.decode(codes_o, shapes, gains, hd, S_used=S, bf16=True)
+    assert np.array_equal(outs, want)
+    assert int(codes.max()) < cb.K
+    # x = (fp32) decode + residual on the sample, up to the fp32 rounding of the stage sums
+    want32, _ = o.decode(codes_o, shapes, gains, hd, S_used=S, bf16=False)
+    np.testing.assert_allclose(o.rows_of(want32, d) + res_o, o.rows_of(xs, d), atol=1e-4, rtol=1e-5)
+
+
+def test_cfg4_full_size_fit_encode_decode_sampled(B):
+    """BASELINE config 4 at its full size, as bench.py runs it: 8 x 131072 tokens x 8 heads x 128 bf16 (2.1 GB, head-inner),
+    codebooks fitted on a 65,536-token sample per head (10 iterations, S = 2), full-cache encode and decode; 2,048 sampled
+    tokens are checked against the oracle."""
+    import bench
+    c = inputs.CONFIGS[4]
+    G, hd, d, K, S, iters = c.G, c.hd, c.d, c.K, c.S, c.iters
+    T, n_fit = 8 * 131072, 65536
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(inputs.seed_of(4, "k"))
+    scale = torch.exp(0.3 * torch.randn(G, hd, device="cuda", generator=gen))
+    for g in range(G):
+        scale[g, torch.randperm(hd, device="cuda", generator=gen)[:4]] *= 10.0
+    x = torch.empty(T, G, hd, dtype=torch.bfloat16, device="cuda")
+    for t0 in range(0, T, 131072):
+        x[t0:t0 + 131072] = (torch.randn(131072, G, hd, device="cuda", generator=gen) * scale).to(torch.bfloat16)
+    w = torch.exp(torch.randn(T, device="cuda", generator=gen))
+    w /= w.mean()
+    fit = torch.stack([torch.sort(torch.randperm(T, device="cuda", generator=gen)[:n_fit]).values for _ in range(G)]).contiguous()
+    view = B.view_of(x, d, head_inner=True)
+    shapes = torch.zeros(G, S, K, d, device="cuda")
+    gains = torch.zeros(G, S, K, device="cuda")
+    cb = B.codebook_of(shapes, gains)
+    ws = B.workspace(view, K, S, n_fit)
+    stats = [B.gsrq_fit_stage(x, view, w, 0, fit, cb, s, None, iters, 0, ws) for s in range(S)]
+    del ws
+    sh, ga = shapes.cpu().numpy(), gains.cpu().numpy()
+    assert np.abs(np.linalg.norm(sh.astype(np.float64), axis=-1) - 1.0).max() <= 1e-6 and (ga >= 0).all()
+    for s in range(S):                                                   # weighted distortion on the fit set is logged per iteration
+        J = np.array(stats[s][0].wdist_after_assign[:stats[s][0].iters_run])
+        assert (np.diff(J) <= 1e-6 * J[0]).all()
+    tok = np.sort(np.random.default_rng(3).choice(T, 2048, replace=False))
+    _sampled_encode_decode_check(B, x, view, True, cb, sh, ga, S, tok)
+
+
+def test_cfg3_full_size_sweep_sampled(B):
+    """BASELINE config 3 at its full size (K-like 8 x 32768 x 128, S = 4, 20 iterations per stage): the S = 4 fit on the
+    GPU, then encode / decode for every prefix S = 1..4 checked on 1,024 sampled tokens against the oracle."""
+    c = inputs.CONFIGS[3]
+    G, T, hd, d, K, S, iters = c.G, c.T, c.hd, c.d, c.K, c.S, c.iters
+    x = torch.from_numpy(inputs.k_like(G, T, hd, inputs.seed_of(3, "k"))).to(torch.bfloat16).cuda()
+    w = torch.from_numpy(inputs.token_weights(T, inputs.seed_of(3, "w"))).cuda()
+    view = B.view_of(x, d)
+    M = hd // d
+    shapes = torch.zeros(G, S, K, d, device="cuda")
+    gains = torch.zeros(G, S, K, device="cuda")
+    cb = B.codebook_of(shapes, gains)
+    ws = B.workspace(view, K, S, 0)
+    codes = torch.zeros(S, G, T * M, dtype=torch.uint8, device="cuda")
+    residual = torch.zeros(G, T * M, d, device="cuda")
+    w_rows = w.repeat_interleave(M).double()
+    energy = [float((w_rows[None] * (x.float().reshape(G, T * M, d).double() ** 2).sum(-1)).sum())]
+    for s in range(S):
+        B.gsrq_fit_stage(x, view, w, 0, None, cb, s, residual if s else None, iters, 0, ws, want_stats=False)
+        B.gsrq_encode(x, view, cb, 0, s + 1, codes, residual, ws)
+        energy.append(float((w_rows[None] * (residual.double() ** 2).sum(-1)).sum()))
+    assert all(energy[i + 1] < energy[i] for i in range(S))              # weighted residual energy falls stage by stage (c-N)
+    sh, ga = shapes.cpu().numpy(), gains.cpu().numpy()
+    tok = np.sort(np.random.default_rng(4).choice(T, 1024, replace=False))
+    for n in range(1, S + 1):
+        _sampled_encode_decode_check(B, x, view, False, cb, sh, ga, n, tok)
