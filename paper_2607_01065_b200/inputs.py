@@ -127,3 +127,39 @@ def make(cfg: int, kind: str | None = None, T: int | None = None):
         n = min(c.n_fit_tokens, max(T // 16, 1))
         fit = fit_sample(c.G, T, n, seed_of(cfg, "fit"))
     return dict(x=x, w=w, fit_tokens=fit, config=c, kind=kind, T=T)
+
+
+def cfg4_device(kind: str = "k", T: int = 8 * 131072, n_fit: int = 65536, G: int = HEADS, hd: int = HEAD_DIM,
+                device: str = "cuda", chunk: int = 131072):
+    """BASELINE config 4 drawn ON THE DEVICE (a 2.1 GB tensor is too slow to draw with numpy): head-inner layout
+    [T][G][hd] bf16, per-token weights [T] fp32 (lognormal(0,1) / mean) and the sorted seeded fit sample [G][n_fit]
+    int64.  Same recipes as k_like / v_like / token_weights / fit_sample with a seeded torch CUDA generator
+    (seed_of(4, kind)); draws in the order: per-head statistics, tensor chunks, weights, fit sample.  The oracle is
+    given copies of the same bits (tests copy the rows they need to the host).
+      k: N(0,1) x per-channel scale exp(0.3 N(0,1)), 4 outlier channels per head x10 (fixed over batch and tokens).
+      v: Student-t(nu=4) = N(0,1) / sqrt(chi2_4 / 4), x per-(batch, token) factor exp(0.5 N(0,1)) shared by heads."""
+    gen = torch.Generator(device=device)
+    gen.manual_seed(seed_of(4, kind))
+    x = torch.empty(T, G, hd, dtype=torch.bfloat16, device=device)
+    if kind == "k":
+        scale = torch.exp(0.3 * torch.randn(G, hd, device=device, generator=gen))
+        for g in range(G):
+            scale[g, torch.randperm(hd, device=device, generator=gen)[:4]] *= 10.0
+        for t0 in range(0, T, chunk):
+            n = min(chunk, T - t0)
+            x[t0:t0 + n] = (torch.randn(n, G, hd, device=device, generator=gen) * scale).to(torch.bfloat16)
+    else:
+        for t0 in range(0, T, chunk):
+            n = min(chunk, T - t0)
+            z = torch.randn(n, G, hd, device=device, generator=gen)
+            chi = torch.zeros(n, G, hd, device=device)
+            for _ in range(4):
+                chi += torch.randn(n, G, hd, device=device, generator=gen) ** 2
+            tok = torch.exp(0.5 * torch.randn(n, 1, 1, device=device, generator=gen))
+            x[t0:t0 + n] = (z / torch.sqrt(chi / 4.0) * tok).to(torch.bfloat16)
+            del z, chi
+    w = torch.exp(torch.randn(T, device=device, generator=gen))
+    w /= w.mean()
+    fit = torch.stack([torch.sort(torch.randperm(T, device=device, generator=gen)[:n_fit]).values
+                       for _ in range(G)]).contiguous()
+    return dict(x=x, w=w, fit_tokens=fit)

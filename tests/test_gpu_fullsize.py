@@ -8,7 +8,7 @@ import numpy as np
 import pytest
 import torch
 
-from _harness import gpu_decode, gpu_gsrq, to_device
+from _harness import gpu_decode, gpu_gsrq, stats_np, to_device
 from oracle import gsrq_oracle as o
 from paper_2607_01065_b200 import inputs
 from test_gpu_parity import _check_free_running
@@ -276,25 +276,49 @@ def _sampled_encode_decode_check(B, x_dev, view, head_inner, cb, shapes, gains, 
     np.testing.assert_allclose(o.rows_of(want32, d) + res_o, o.rows_of(xs, d), atol=1e-4, rtol=1e-5)
 
 
-def test_cfg4_full_size_fit_encode_decode_sampled(B):
+def _oracle_fit_rows(rows, w_rows, K, S, iters, G):
+    """The oracle's S-stage fit on compact fit rows [G][Nf][d] (a stage's residual on the fit rows depends on those rows
+    only): Alg. 1 per group and stage, then the stage's encode to get the next residual.  Returns shapes, gains, stats."""
+    d = rows.shape[-1]
+    shapes = np.zeros((G, S, K, d), np.float32)
+    gains = np.zeros((G, S, K), np.float32)
+    stats = [[None] * S for _ in range(G)]
+    for g_ in range(G):
+        r = np.ascontiguousarray(rows[g_], dtype=np.float32)
+        for st in range(S):
+            f = o.fit_stage(r, w_rows[g_], K, iters, 0, group=g_, G=G, stage=st)
+            shapes[g_, st], gains[g_, st], stats[g_][st] = f["shapes"], f["gains"], f
+            if st + 1 < S:
+                _, r, _, _ = o.encode_stage(r, f["shapes"], f["gains"])
+    return shapes, gains, stats
+
+
+def _assert_fit_matches(got_shapes, got_gains, got_stats, ref_shapes, ref_gains, ref_stats, G, S):
+    """BASELINE criteria (b) codewords / gains within 1e-4 and (c) weighted distortion within 1e-4 relative -- here for every
+    iteration's J, plus the discrete trajectory: iterations run, rows changed per iteration, empty clusters."""
+    assert np.abs(got_shapes - ref_shapes).max() <= 1e-4
+    assert np.abs(got_gains - ref_gains).max() <= 1e-4
+    for st in range(S):
+        for g_ in range(G):
+            s_ref, s_got = ref_stats[g_][st], stats_np(got_stats[st], g_)
+            assert s_got["iters_run"] == s_ref["iters_run"], (st, g_)
+            np.testing.assert_allclose(s_got["J"], s_ref["J_assign"], rtol=1e-4)
+            assert np.array_equal(s_got["changed"], s_ref["changed"]), (st, g_)
+            assert s_got["n_empty_last"] == s_ref["n_empty_last"]
+
+
+@pytest.mark.parametrize("kind", ["k", "v"])
+def test_cfg4_full_size_fit_vs_oracle_then_sampled_encode_decode(B, kind):
     """BASELINE config 4 at its full size, as bench.py runs it: 8 x 131072 tokens x 8 heads x 128 bf16 (2.1 GB, head-inner),
-    codebooks fitted on a 65,536-token sample per head (10 iterations, S = 2), full-cache encode and decode; 2,048 sampled
-    tokens are checked against the oracle."""
-    import bench
+    K-like and V-like.  The S = 2, 10-iteration fit on the 65,536-token sample per head (524,288 fit rows per head) is
+    compared with the oracle run on the same bits (fit rows copied to the host): codebooks, per-iteration distortion,
+    iterations and changed counts.  Then the full-cache encode and decode, checked on 2,048 sampled tokens against the
+    oracle encoding them with the ORACLE's codebooks."""
     c = inputs.CONFIGS[4]
     G, hd, d, K, S, iters = c.G, c.hd, c.d, c.K, c.S, c.iters
-    T, n_fit = 8 * 131072, 65536
-    gen = torch.Generator(device="cuda")
-    gen.manual_seed(inputs.seed_of(4, "k"))
-    scale = torch.exp(0.3 * torch.randn(G, hd, device="cuda", generator=gen))
-    for g in range(G):
-        scale[g, torch.randperm(hd, device="cuda", generator=gen)[:4]] *= 10.0
-    x = torch.empty(T, G, hd, dtype=torch.bfloat16, device="cuda")
-    for t0 in range(0, T, 131072):
-        x[t0:t0 + 131072] = (torch.randn(131072, G, hd, device="cuda", generator=gen) * scale).to(torch.bfloat16)
-    w = torch.exp(torch.randn(T, device="cuda", generator=gen))
-    w /= w.mean()
-    fit = torch.stack([torch.sort(torch.randperm(T, device="cuda", generator=gen)[:n_fit]).values for _ in range(G)]).contiguous()
+    T, n_fit, M = 8 * 131072, 65536, c.hd // c.d
+    dd = inputs.cfg4_device(kind, T, n_fit)
+    x, w, fit = dd["x"], dd["w"], dd["fit_tokens"]
     view = B.view_of(x, d, head_inner=True)
     shapes = torch.zeros(G, S, K, d, device="cuda")
     gains = torch.zeros(G, S, K, device="cuda")
@@ -303,37 +327,37 @@ def test_cfg4_full_size_fit_encode_decode_sampled(B):
     stats = [B.gsrq_fit_stage(x, view, w, 0, fit, cb, s, None, iters, 0, ws) for s in range(S)]
     del ws
     sh, ga = shapes.cpu().numpy(), gains.cpu().numpy()
+    # the oracle on the same bits: the fit rows of every head, [G][n_fit * M][d], and their token weights
+    rows = torch.stack([x[fit[g_], g_] for g_ in range(G)]).float().reshape(G, n_fit * M, d).cpu().numpy()
+    w_rows = torch.stack([w[fit[g_]] for g_ in range(G)]).repeat_interleave(M, dim=1).cpu().numpy()
+    ref_sh, ref_ga, ref_stats = _oracle_fit_rows(rows, w_rows, K, S, iters, G)
+    _assert_fit_matches(sh, ga, stats, ref_sh, ref_ga, ref_stats, G, S)
+    # the shapes the fit returns are unit vectors and the gains non-negative (Eq. 3)
     assert np.abs(np.linalg.norm(sh.astype(np.float64), axis=-1) - 1.0).max() <= 1e-6 and (ga >= 0).all()
-    for s in range(S):                                                   # weighted distortion on the fit set is logged per iteration
-        J = np.array(stats[s][0].wdist_after_assign[:stats[s][0].iters_run])
-        assert (np.diff(J) <= 1e-6 * J[0]).all()
+    # full-cache encode / decode on sampled tokens, against the oracle with ITS codebooks
+    shapes.copy_(torch.from_numpy(ref_sh).cuda()); gains.copy_(torch.from_numpy(ref_ga).cuda())
     tok = np.sort(np.random.default_rng(3).choice(T, 2048, replace=False))
-    _sampled_encode_decode_check(B, x, view, True, cb, sh, ga, S, tok)
+    _sampled_encode_decode_check(B, x, view, True, cb, ref_sh, ref_ga, S, tok)
 
 
-def test_cfg3_full_size_sweep_sampled(B):
-    """BASELINE config 3 at its full size (K-like 8 x 32768 x 128, S = 4, 20 iterations per stage): the S = 4 fit on the
-    GPU, then encode / decode for every prefix S = 1..4 checked on 1,024 sampled tokens against the oracle."""
-    c = inputs.CONFIGS[3]
-    G, T, hd, d, K, S, iters = c.G, c.T, c.hd, c.d, c.K, c.S, c.iters
-    x = torch.from_numpy(inputs.k_like(G, T, hd, inputs.seed_of(3, "k"))).to(torch.bfloat16).cuda()
-    w = torch.from_numpy(inputs.token_weights(T, inputs.seed_of(3, "w"))).cuda()
-    view = B.view_of(x, d)
-    M = hd // d
-    shapes = torch.zeros(G, S, K, d, device="cuda")
-    gains = torch.zeros(G, S, K, device="cuda")
-    cb = B.codebook_of(shapes, gains)
-    ws = B.workspace(view, K, S, 0)
-    codes = torch.zeros(S, G, T * M, dtype=torch.uint8, device="cuda")
-    residual = torch.zeros(G, T * M, d, device="cuda")
-    w_rows = w.repeat_interleave(M).double()
-    energy = [float((w_rows[None] * (x.float().reshape(G, T * M, d).double() ** 2).sum(-1)).sum())]
-    for s in range(S):
-        B.gsrq_fit_stage(x, view, w, 0, None, cb, s, residual if s else None, iters, 0, ws, want_stats=False)
-        B.gsrq_encode(x, view, cb, 0, s + 1, codes, residual, ws)
-        energy.append(float((w_rows[None] * (residual.double() ** 2).sum(-1)).sum()))
-    assert all(energy[i + 1] < energy[i] for i in range(S))              # weighted residual energy falls stage by stage (c-N)
-    sh, ga = shapes.cpu().numpy(), gains.cpu().numpy()
-    tok = np.sort(np.random.default_rng(4).choice(T, 1024, replace=False))
-    for n in range(1, S + 1):
-        _sampled_encode_decode_check(B, x, view, False, cb, sh, ga, n, tok)
+@pytest.mark.parametrize("kind", ["k", "v"])
+def test_cfg3_full_size_fit_vs_oracle_and_prefix_sweep(B, kind):
+    """BASELINE config 3 at its full size (8 x 32768 x 128, K-like and V-like, S = 4, 20 iterations per stage), bench.py's
+    call sequence: the whole fit -> encode trajectory against the oracle (criteria a, b, c, per-iteration J, changed counts),
+    the decode of every prefix S = 1..4 of all 2,097,152 rows, and falling weighted residual energy (reading c-N)."""
+    dd = inputs.make(3, kind=kind)
+    c = dd["config"]
+    got, ref = _check_free_running(dd, c.K, c.S, c.iters, "bf16", prefix_encode=True)
+    M = c.hd // c.d
+    w_rows = np.repeat(dd["w"], M).astype(np.float64)
+    energy = [float((w_rows[None] * (o.rows_of(dd["x"], c.d).astype(np.float64) ** 2).sum(-1)).sum())]
+    r = o.rows_of(dd["x"], c.d).copy()
+    for st in range(c.S):
+        for g_ in range(c.G):
+            _, r[g_], _, _ = o.encode_stage(r[g_], ref["shapes"][g_, st], ref["gains"][g_, st])
+        energy.append(float((w_rows[None] * (r.astype(np.float64) ** 2).sum(-1)).sum()))
+    assert all(energy[i + 1] < energy[i] for i in range(c.S))
+    for n in range(1, c.S + 1):
+        dec = gpu_decode(got["codes_dev"], got["cb"], n, c.G, c.T, c.hd, c.d, dtype="bf16")
+        want, _ = o.decode(got["codes"], got["shapes"], got["gains"], c.hd, S_used=n, bf16=True)
+        assert np.array_equal(dec, want), n
