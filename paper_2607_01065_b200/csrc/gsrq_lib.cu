@@ -13,6 +13,7 @@
 #include "k_update.cuh"
 #include "k_score.cuh"
 #include "k_score_tc.cuh"
+#include "k_fit_tc.cuh"
 #include "k_encode_tc.cuh"
 
 namespace gsrq {
@@ -57,16 +58,29 @@ struct ProfScope {
 
 static inline size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
+// SM count of the CURRENT device (cached per device ordinal; the cache is only ever written with the same value).
+static int sm_count() {
+  static int cache[64] = {0};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return 148;
+  if (dev >= 0 && dev < 64 && cache[dev] > 0) return cache[dev];
+  int n = 0;
+  if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+  if (dev >= 0 && dev < 64) cache[dev] = n;
+  return n;
+}
+
 struct Plan {
   long long nf_tok, Nf, Nall, nE;
   int M;
   // [0, encode_total): what gsrq_encode needs; the rest is for the fit
   size_t off_list, off_cnt, off_st, off_ebimg, off_egmax, off_eres, encode_total;
   size_t off_Rf, off_coef, off_wt, off_idx, off_ids, off_epart, off_term;
-  size_t off_ahi, off_alo, off_rnorm, off_bimg, off_gmax, total;
+  size_t off_ahi, off_alo, off_rnorm, off_bimg, off_gmax, off_wn, off_part, off_bar, off_clk, total;
 };
 
 constexpr int kNumCounters = 256;
+constexpr int kMaxCtas = 256;  // upper bound of co-resident CTAs (SMs) the partial buffer is sized for
 constexpr int kTermStride = GSRQ_MAX_ITERS + 1;
 
 // n_fit_tokens: > 0 fit subset size, 0 = fit on all tokens, < 0 = no fit (encode / decode only)
@@ -100,6 +114,11 @@ static Plan make_plan(const gsrq_view *v, int K, int S, long long n_fit_tokens) 
   p.off_rnorm = o; o += align_up(tcp ? (size_t)v->G * p.Nf * sizeof(float) : 0);
   p.off_bimg = o;  o += align_up(tcp ? (size_t)v->G * 3 * tc::kBImgBytes : 0);
   p.off_gmax = o;  o += align_up(tcp ? (size_t)v->G * sizeof(int) : 0);
+  // fused fit kernel (d == 16): per-row w/(||r||+eps), per-CTA partials [G][nx][256][34] with G * nx <= kMaxCtas, group barriers
+  p.off_wn = o;    o += align_up(tcp ? (size_t)v->G * p.Nf * sizeof(double) : 0);
+  p.off_part = o;  o += align_up(tcp && p.Nf ? (size_t)(v->G > kMaxCtas ? v->G : kMaxCtas) * tc::kN * tc::kFitP * sizeof(double) : 0);
+  p.off_bar = o;   o += align_up(tcp ? (size_t)v->G * sizeof(unsigned int) : 0);
+  p.off_clk = o;   o += align_up(tcp ? (size_t)(v->G > kMaxCtas ? v->G : kMaxCtas) * 16 * sizeof(long long) : 0);
   p.total = o;
   return p;
 }
@@ -165,8 +184,7 @@ static int run_update(const Plan &pl, const gsrq_view *v, int K, char *ws, const
   u.bimg = images ? (uint8_t *)(ws + pl.off_bimg) : nullptr;
   dim3 grid((unsigned)((K + kCPC - 1) / kCPC), (unsigned)v->G);
   DISPATCH_D(d, {
-    static bool attr_set = false;
-    if (!attr_set) { GSRQ_CUDA_CHECK(cudaFuncSetAttribute(k_update<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)upd_smem_bytes<D>())); attr_set = true; }
+    GSRQ_CUDA_CHECK(cudaFuncSetAttribute(k_update<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)upd_smem_bytes<D>()));
     LAUNCH(kClsUpdate, stream, (k_update<D><<<grid, kUpdThreads, upd_smem_bytes<D>(), stream>>>(u)));
   });
   GSRQ_CUDA_CHECK(cudaGetLastError());
@@ -230,8 +248,7 @@ static int run_assign_tc(const Plan &pl, char *ws, const TcMaps &maps, int G, co
   p.shapes = shapes_st; p.gains = gains_st; p.cb_stride_g = cb_stride_g; p.idx = idx; p.N = pl.Nf;
   p.n_tiles = (int)((pl.Nf + tc::kTileM - 1) / tc::kTileM); p.n_planes = n_planes; p.K = K; p.mode = mode;
   p.st = st; p.slot = slot; p.dbg = dbg;
-  static int n_sm = 0;
-  if (!n_sm) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev); if (n_sm <= 0) n_sm = 148; }
+  const int n_sm = sm_count();
   int ctas = n_sm / G; if (ctas < 1) ctas = 1; if (ctas > p.n_tiles) ctas = p.n_tiles;
   const size_t smem = 120 * 1024;  // > half of the SM's shared memory: one CTA (and one 512-column TMEM allocation) per SM
   static_assert(tc::kSmemTotal <= 120 * 1024, "smem budget");
@@ -239,11 +256,61 @@ static int run_assign_tc(const Plan &pl, char *ws, const TcMaps &maps, int G, co
     GSRQ_CUDA_CHECK(cudaFuncSetAttribute(tc::k_score_tc<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     LAUNCH(kClsScore, stream, (tc::k_score_tc<true><<<dim3((unsigned)ctas, (unsigned)G), tc::kThreads, smem, stream>>>(maps.hi, maps.lo, p)));
   } else {
-    static bool attr_set = false;
-    if (!attr_set) { GSRQ_CUDA_CHECK(cudaFuncSetAttribute(tc::k_score_tc<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr_set = true; }
+    GSRQ_CUDA_CHECK(cudaFuncSetAttribute(tc::k_score_tc<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     LAUNCH(kClsScore, stream, (tc::k_score_tc<false><<<dim3((unsigned)ctas, (unsigned)G), tc::kThreads, smem, stream>>>(maps.hi, maps.lo, p)));
   }
   GSRQ_CUDA_CHECK(cudaGetLastError());
+  return GSRQ_OK;
+}
+
+// The fused persistent fit kernel (k_fit_tc.cuh) on the prepared fit rows: passes [t_begin, t_end] of Alg. 1 in one
+// cooperative launch, or (skip_scoring) one reduction + Eq. 7 / Eq. 8 update from the assignment already in `idx`.
+static int run_fit_tc(const Plan &pl, char *ws, const TcMaps *maps, int G, int M, float *shapes_st, float *gains_st, long long cb_stride_g,
+                      int K, int n_planes, uint8_t *idx, DevStats *st, int t_begin, int t_end, bool skip_scoring, int lloyd_override,
+                      bool images, cudaStream_t stream) {
+  tc::FitTcParams p{};
+  p.bimg = images ? (uint8_t *)(ws + pl.off_bimg) : nullptr;
+  p.shapes = shapes_st; p.gains = gains_st; p.cb_stride_g = cb_stride_g;
+  p.rnorm = (const float *)(ws + pl.off_rnorm); p.rows = (const float *)(ws + pl.off_Rf);
+  p.ahi = (const __nv_bfloat16 *)(ws + pl.off_ahi); p.wn = (const double *)(ws + pl.off_wn); p.wt = (const float *)(ws + pl.off_wt);
+  p.nf_tok = pl.nf_tok; p.M = M; p.idx = idx; p.N = pl.Nf;
+  p.n_tiles = (int)((pl.Nf + tc::kTileM - 1) / tc::kTileM); p.n_planes = n_planes; p.K = K;
+  p.t_begin = t_begin; p.t_end = t_end; p.skip_scoring = skip_scoring ? 1 : 0; p.lloyd_override = lloyd_override;
+  p.st = st; p.term = st ? (double *)(ws + pl.off_term) : nullptr; p.term_stride = kTermStride;
+  p.part = (double *)(ws + pl.off_part); p.bar = (unsigned int *)(ws + pl.off_bar);
+  GSRQ_CUDA_CHECK(cudaMemsetAsync(p.bar, 0, (size_t)G * sizeof(unsigned int), stream));
+  static const bool want_clk = getenv("GSRQ_FIT_CLOCKS") != nullptr;   // debug: per-phase cycle counts on stderr
+  if (want_clk) {
+    p.clk = (long long *)(ws + pl.off_clk);
+    GSRQ_CUDA_CHECK(cudaMemsetAsync(p.clk, 0, (size_t)(G > kMaxCtas ? G : kMaxCtas) * 16 * sizeof(long long), stream));
+  }
+  const int n_sm = sm_count();
+  int nx = n_sm / G; if (nx < 1) nx = 1; if (nx > p.n_tiles) nx = p.n_tiles;
+  if ((long long)G * nx > kMaxCtas && nx > 1) nx = kMaxCtas / G > 0 ? kMaxCtas / G : 1;
+  GSRQ_CUDA_CHECK(cudaFuncSetAttribute(tc::k_fit_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tc::kFitSmemTotal));
+  CUtensorMap zero;
+  memset(&zero, 0, sizeof(zero));
+  const CUtensorMap *hi = maps ? &maps->hi : &zero, *lo = maps ? &maps->lo : &zero;
+  void *args[3] = {(void *)hi, (void *)lo, (void *)&p};
+  const dim3 grid((unsigned)nx, (unsigned)G), block(tc::kThreads);
+  {
+    gsrq::ProfScope ps(skip_scoring ? kClsUpdate : kClsScore, stream);
+    // nx > 1: the CTAs of a group wait on one another, so they must be co-resident: cooperative launch.  nx == 1: every
+    // CTA is a group of its own (its barrier is trivially satisfied), any grid size is fine.
+    if (nx > 1) GSRQ_CUDA_CHECK(cudaLaunchCooperativeKernel((const void *)tc::k_fit_tc, grid, block, args, tc::kFitSmemTotal, stream));
+    else GSRQ_CUDA_CHECK(cudaLaunchKernel((const void *)tc::k_fit_tc, grid, block, args, tc::kFitSmemTotal, stream));
+  }
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  if (want_clk) {
+    std::vector<long long> h((size_t)G * nx * 16);
+    GSRQ_CUDA_CHECK(cudaMemcpyAsync(h.data(), p.clk, h.size() * sizeof(long long), cudaMemcpyDeviceToHost, stream));
+    GSRQ_CUDA_CHECK(cudaStreamSynchronize(stream));
+    double sum[16] = {0};
+    for (size_t c = 0; c < (size_t)G * nx; ++c) for (int q = 0; q < 16; ++q) sum[q] += (double)h[c * 16 + q];
+    const double den = (double)G * nx * (t_end - t_begin + 1);
+    fprintf(stderr, "k_fit_tc cycles per pass (mean over %d CTAs, %d passes): stage %.0f score %.0f publish %.0f bar1 %.0f merge %.0f bar2 %.0f | reduce: load %.0f bitmap %.0f wait %.0f (unused %.0f) accumulate %.0f | coef-store %.0f bitmap-rmw %.0f fetch %.0f\n",
+            G * nx, t_end - t_begin + 1, sum[0] / den, sum[1] / den, sum[2] / den, sum[3] / den, sum[4] / den, sum[5] / den, sum[6] / den, sum[7] / den, sum[8] / den, sum[9] / den, sum[10] / den, sum[11] / den, sum[12] / den, sum[13] / den);
+  }
   return GSRQ_OK;
 }
 
@@ -251,7 +318,10 @@ static int launch_prep(const Plan &pl, const gsrq_view *v, const RowSrc &src, co
                        const long long *fit_tokens, char *ws, bool consts, int n_planes, cudaStream_t stream) {
   PrepParams q{};
   q.src = src; q.w = w; q.w_stride_g = w_stride_g; q.fit_tokens = fit_tokens; q.nf_tok = pl.nf_tok;
-  q.Rf = (float *)(ws + pl.off_Rf); q.coef = (double2 *)(ws + pl.off_coef); q.wt = (float *)(ws + pl.off_wt);
+  q.Rf = (float *)(ws + pl.off_Rf); q.wt = (float *)(ws + pl.off_wt);
+  // the fused fit kernel (tensor-core path) reads w from wt and w/(||r||+eps) from wn; the cluster-owner update kernel reads pairs
+  q.coef = use_tc(v->d) ? nullptr : (double2 *)(ws + pl.off_coef);
+  q.wn = use_tc(v->d) ? (double *)(ws + pl.off_wn) : nullptr;
   q.epart = consts ? (double *)(ws + pl.off_epart) : nullptr;
   q.ahi = (consts && n_planes > 0) ? (__nv_bfloat16 *)(ws + pl.off_ahi) : nullptr;
   q.alo = (consts && n_planes == 2) ? (__nv_bfloat16 *)(ws + pl.off_alo) : nullptr;
@@ -335,16 +405,11 @@ static int run_encode_tc_pass(const void *kv, const gsrq_view *v, const gsrq_cod
   p.n_tiles = (int)((N + tc::kTileM - 1) / tc::kTileM);
   if (!res_in) p.n_tiles = (int)((v->T + tpt - 1) / tpt);
   p.list = (uint2 *)(ws + pl.off_list); p.list_cnt = list_cnt;
-  static int n_sm = 0;
-  if (!n_sm) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev); if (n_sm <= 0) n_sm = 148; }
+  const int n_sm = sm_count();
   int ctas = n_sm / G; if (ctas < 1) ctas = 1; if (ctas > p.n_tiles) ctas = p.n_tiles;
   const size_t smem = tc::kEncSmemTotal;
-  static bool attr_set = false;
-  if (!attr_set) {
-    GSRQ_CUDA_CHECK(cudaFuncSetAttribute(tc::k_encode_tc<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    GSRQ_CUDA_CHECK(cudaFuncSetAttribute(tc::k_encode_tc<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr_set = true;
-  }
+  if (res_in) GSRQ_CUDA_CHECK(cudaFuncSetAttribute(tc::k_encode_tc<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  else GSRQ_CUDA_CHECK(cudaFuncSetAttribute(tc::k_encode_tc<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   if (res_in)
     LAUNCH(kClsEncode, stream, (tc::k_encode_tc<true><<<dim3((unsigned)ctas, (unsigned)G), tc::kThreads, smem, stream>>>(tm, p, tpt, 0)));
   else
@@ -446,18 +511,16 @@ int gsrq_fit_stage(const void *kv, const gsrq_view *view, const float *w, int64_
   p.shapes = shapes_st; p.gains = gains_st; p.s_begin = 0; p.s_end = 1; p.s_base = 0;
   // t = 0 is Alg. 1 l.2: gains by Eq. 8 under the max-projection assignment (reading c-I);
   // t >= 1 are the Lloyd iterations.  Two launches per pass: assignment, then the fused update.
-  for (int t = 0; t <= iters && rc == 0; ++t) {
-    const int mode = (t == 0) ? 1 : 0;
-    if (n_planes) {
-      rc = run_assign_tc(pl, ws, maps, G, shapes_st, gains_st, cb_stride_g, K, mode, n_planes, idx, st, t, &st[0].gmax_bits[t],
-                         (long long)(sizeof(DevStats) / sizeof(int)), nullptr, stream);
-    } else {
+  if (n_planes) {  // d == 16: the whole loop is one persistent kernel (k_fit_tc.cuh)
+    rc = run_fit_tc(pl, ws, &maps, G, pl.M, shapes_st, gains_st, cb_stride_g, K, n_planes, idx, st, 0, iters, false, -1, true, stream);
+  } else {
+    for (int t = 0; t <= iters && rc == 0; ++t) {
       EncParams a = p;
-      a.mode = mode; a.slot = t; a.list_cnt = cnt + t;
+      a.mode = (t == 0) ? 1 : 0; a.slot = t; a.list_cnt = cnt + t;
       rc = run_encode(a, G, d, stream);
+      if (rc) break;
+      rc = run_update(pl, view, K, ws, idx, shapes_st, gains_st, cb_stride_g, st, t > 0, t, false, stream);
     }
-    if (rc) break;
-    rc = run_update(pl, view, K, ws, idx, shapes_st, gains_st, cb_stride_g, st, t > 0, t, n_planes != 0, stream);
   }
   if (rc) return rc;
   if (stats) {  // J_t and iters_run are only read back through `stats`
@@ -537,8 +600,7 @@ int gsrq_decode(const uint8_t *codes, const gsrq_codebook *cb, int n_stages, voi
   if (d == 16 && n_stages >= 1 && n_stages <= kDecDeep && p.N % 16 == 0 && p.N >= 256 && ((uintptr_t)codes & 15) == 0) {
     const long long n_chunks = p.N / 256;
     const bool dense = out_view->stride_t == out_view->hd;
-    static int n_sm = 0;
-    if (!n_sm) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev); if (n_sm <= 0) n_sm = 148; }
+    const int n_sm = sm_count();
     const bool deep = n_stages > 4;  // single-copy tables
     const size_t smem = deep ? (size_t)n_stages * (kDecTabBytes / 2) : (size_t)n_stages * kDecTabBytes;
     int per_sm = (int)((227 * 1024) / (smem + 1024));  // CTAs that fit on one SM (shared memory; 40 registers x 512 threads)
@@ -687,6 +749,9 @@ int gsrq_update(const void *kv, const gsrq_view *view, const float *residual, co
   // rows = residual when given, else kv as is (the caller states which stage's rows these are)
   rc = prepare_rows(pl, kv, view, w, w_stride_g, nullptr, cb, 0, residual, ws, stream);
   if (rc) return rc;
+  if (use_tc(view->d))  // the fit's own reduction / merge phases (k_fit_tc.cuh), fed with the given assignment; rows from the fp32 buffer
+    return run_fit_tc(pl, ws, nullptr, view->G, pl.M, cb->shapes + (size_t)stage * cb->K * view->d, cb->gains + (size_t)stage * cb->K,
+                      (long long)cb->S * cb->K, cb->K, 2, const_cast<uint8_t *>(idx), nullptr, 1, 1, true, shapes_too ? 1 : 0, false, stream);
   return run_update(pl, view, cb->K, ws, idx, cb->shapes + (size_t)stage * cb->K * view->d,
                     cb->gains + (size_t)stage * cb->K, (long long)cb->S * cb->K, nullptr, shapes_too ? 1 : 0, 1, false, stream);
 }

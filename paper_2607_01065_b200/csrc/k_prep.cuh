@@ -15,7 +15,8 @@ struct PrepParams {
   const long long *fit_tokens; // [G][nf_tok] or nullptr
   long long nf_tok;
   float *Rf;                   // [G][Nf][D] compact fp32 rows (out; may alias src.rows)
-  double2 *coef;               // [G][Nf] per-row {w_i, w_i/(||r_i||+eps)}  (Eq. 6 with the safeguard of PAPER.md:178)
+  double2 *coef;               // [G][Nf] per-row {w_i, w_i/(||r_i||+eps)}  (Eq. 6 with the safeguard of PAPER.md:178), or nullptr
+  double *wn;                  // [G][Nf] per-row w_i/(||r_i||+eps) alone (the fused fit kernel reads w_i from wt), or nullptr
   float *wt;                   // [G][nf_tok] compact per-fit-token weights (out)
   double *epart;               // [G][gridDim.x] partial sums of w_i ||r_i||^2 (Eq. 4's constant), or nullptr
   __nv_bfloat16 *ahi, *alo;    // [G][Nf][16] bf16 operand planes of the tensor-core filter (D == 16), or nullptr
@@ -50,7 +51,9 @@ __global__ void __launch_bounds__(256) k_prep_rows(PrepParams p) {
 #pragma unroll
     for (int j = 0; j < D; ++j) n2 = __dadd_rn(n2, __dmul_rn((double)x[j], (double)x[j]));
     const double n = sqrt(n2);
-    p.coef[gi] = make_double2((double)wv, (double)wv * (1.0 / (n + kEps)));
+    const double wnv = (double)wv * (1.0 / (n + kEps));
+    if (p.coef) p.coef[gi] = make_double2((double)wv, wnv);
+    if (p.wn) p.wn[gi] = wnv;
     e += (double)wv * n2;
     if (p.rnorm) p.rnorm[gi] = (float)n * 1.000001f;
     if (D == 16 && p.ahi) {
