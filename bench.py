@@ -1,16 +1,18 @@
 #!/usr/bin/env python
-"""bench.py -- one JSON line per run (see DESIGN.md section 7 for what each key means).
+"""bench.py -- one JSON line per run (DESIGN.md section 9 says what each key means).
 
-A "step" is one pass of the whole hot path over one synthetic layer tensor of BASELINE.json
-config 1 (8 KV heads x 4096 tokens x 128, bf16, d=16, K=256, S=2, 20 iterations/stage):
-for each stage s: gsrq_fit_stage(s) -> fused gsrq_encode of stages [0, s] (its residual feeds the
-next fit; the last one is the final encode); then gsrq_decode.
-value = KV vectors (token x head) through the whole step per second, summed over ranks.
-Unless --no-big, rank 0 also runs BASELINE.json config 4 (one 8 x 131072-token batch, head-inner
-layout, 2.1 GB): fit on a 65,536-token sample per head, full-cache encode, full-cache decode --
-the sizes at which "fraction of the HBM / tensor roofline" is physically meaningful.
+Headline workload = BASELINE.json config 4, the largest single-GPU configuration: one layer's K AND V cache,
+batch 8 x 131072 tokens x 8 KV heads x 128, bf16, head-inner layout (2.147 GB each); d=16, K=256, S=2, 10 Lloyd
+iterations; codebooks fitted on a seeded 65,536-token sample per head, then full-cache encode and full-cache decode.
+A "step" is that whole hot path for both tensors:
+    for X in (K, V): for s in 0..S-1: gsrq_fit_stage(X, stage s, fit sample) ; gsrq_encode(X, stages [0,S)) ; gsrq_decode(X)
+value = KV vectors (token x head, 2 x 8 x 1,048,576 per step) through the whole step per second, summed over ranks
+(replicas: every rank works on its own layer).  Inputs are resident in HBM and far larger than L2 (no flush needed).
+e2e is the same through gsrq_pipeline_host on pinned HOST buffers (H2D of the tensors, D2H of codes, codebooks and
+the decoded tensors inside the timed region).  Rank 0 also times BASELINE configs 1-3 and the encode-on-append
+latency as extras (>= 20 repetitions each, median and min), and the CPU oracle on a bounded sample.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--cfg 1|2] [--no-big]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-extras] [--no-cpu-baseline]
 """
 from __future__ import annotations
 
@@ -33,6 +35,8 @@ from paper_2607_01065_b200 import inputs  # noqa: E402
 
 METRIC = "gsrq_fit_encode_decode_kv_vectors_per_s"
 UNIT = "KV vectors/s"
+CFG4_T, CFG4_NFIT = 8 * 131072, 65536
+ORACLE_FIT_HEADS, ORACLE_SLICE_TOKENS = 2, 16384
 
 
 def peaks():
@@ -42,6 +46,14 @@ def peaks():
         return dict(hbm_gbs=d["hbm_gbs"], bf16_tflops=d["bf16_tflops"], bf16_tflops_sustained=d["bf16_tflops_sustained"],
                     source="MEASURED_PEAKS.json")
     return dict(hbm_gbs=6650.0, bf16_tflops=1590.0, bf16_tflops_sustained=1400.0, source="fallback (B200_PROFILING.md)")
+
+
+def workload_config():
+    """The `config` object of the JSON line: identical for both arms."""
+    c = inputs.CONFIGS[4]
+    return dict(workload=f"cfg4:{c.name} (one layer's K and V cache, head-inner)", tensors="k,v", G=c.G, T=CFG4_T, hd=c.hd,
+                d=c.d, K=c.K, S=c.S, iters=c.iters, n_fit_tokens=CFG4_NFIT,
+                l2="inputs 17x larger than L2: no flush needed", parallelism="replicas")
 
 
 class ClockSampler(threading.Thread):
@@ -80,37 +92,62 @@ class ClockSampler(threading.Thread):
                     samples=len(sm), samples_in_timed_region=len(inside))
 
 
-def oracle_step(x, w, c):
-    """The CPU oracle doing the same step (fit + encode every stage, then decode)."""
+# ------------------------------------------------------------------------------------------------ oracle (CPU) legs
+def oracle_sample_seconds(kind: str) -> dict:
+    """The CPU oracle, as it stands, on a BOUNDED sample of the cfg-4 step for one tensor kind, scaled to the whole step.
+    Sample: a numpy draw of the same recipe with 65,536 tokens x 8 heads; the S=2, 10-iteration fit of ORACLE_FIT_HEADS
+    heads on all 524,288 rows of each (= one head's fit sample), and encode + decode of all 8 heads over the first
+    ORACLE_SLICE_TOKENS tokens with those codebooks.  Whole-step estimate: fit time x 8 / heads + encode/decode time x
+    1,048,576 / slice tokens (the oracle's cost is linear in heads and in tokens)."""
     from oracle import gsrq_oracle as o
-    out = o.gsrq_fit_encode(x, w, c.d, c.K, c.S, c.iters, seed=0)
-    o.decode(out["codes"], out["shapes"], out["gains"], c.hd, bf16=(c.dtype == "bf16"))
-    return out
+    c = inputs.CONFIGS[4]
+    gen = inputs.k_like if kind == "k" else inputs.v_like
+    x = gen(c.G, CFG4_NFIT, c.hd, inputs.seed_of(4, kind))
+    w = inputs.token_weights(CFG4_NFIT, inputs.seed_of(4, "w"))
+    t0 = time.perf_counter()
+    fit = o.gsrq_fit_encode(x[:ORACLE_FIT_HEADS], w, c.d, c.K, c.S, c.iters, seed=0, encode=False)
+    t_fit = time.perf_counter() - t0
+    sh = np.concatenate([fit["shapes"]] * (c.G // ORACLE_FIT_HEADS))
+    ga = np.concatenate([fit["gains"]] * (c.G // ORACLE_FIT_HEADS))
+    t0 = time.perf_counter()
+    codes, _, _, _ = o.encode(x[:, :ORACLE_SLICE_TOKENS], sh, ga, c.d)
+    o.decode(codes, sh, ga, c.hd, bf16=True)
+    t_ed = time.perf_counter() - t0
+    full = t_fit * c.G / ORACLE_FIT_HEADS + t_ed * CFG4_T / ORACLE_SLICE_TOKENS
+    return dict(fit_s=t_fit, encode_decode_s=t_ed, whole_step_s_estimate=full)
 
 
-def run_reference(args, c):
-    """--impl reference: the oracle as it stands on the host cores, same config / metric."""
+def oracle_value(steps: int = 1):
+    """KV vectors/s of the oracle for the whole cfg-4 step (K and V), from the bounded samples; returns value, description."""
     from oracle import gsrq_oracle as o
     o.build()
-    dd = inputs.make(c.cfg)
-    x, w = dd["x"], dd["w"]
+    c = inputs.CONFIGS[4]
+    tot, cpu = 0.0, 0.0
+    for _ in range(steps):
+        for kind in ("k", "v"):
+            r = oracle_sample_seconds(kind)
+            tot += r["whole_step_s_estimate"]
+            cpu += r["fit_s"] + r["encode_decode_s"]
+    val = steps * 2 * c.G * CFG4_T / tot
+    desc = (f"per tensor (k, v): oracle fit of {ORACLE_FIT_HEADS} of 8 heads on 524,288 fit rows each + encode/decode of 8 heads x "
+            f"{ORACLE_SLICE_TOKENS} tokens, scaled linearly to 8 heads / 1,048,576 tokens; {cpu / steps:.1f} s of CPU work per step")
+    return val, tot / steps, desc, o.n_threads()
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands on the host cores, same config / metric (rank 0 only)."""
     for _ in range(min(args.warmup, 1)):
-        oracle_step(x[:1], w, c)
-    t0 = time.perf_counter()
-    for _ in range(args.steps):
-        oracle_step(x, w, c)
-    dt = (time.perf_counter() - t0) / args.steps
-    val = c.G * c.T / dt
+        oracle_sample_seconds("k")
+    val, step_s, desc, cores = oracle_value(args.steps)
     line = dict(metric=METRIC, value=val, unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
-                ms_per_step=dt * 1e3, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64",
-                data="synthetic", impl="reference",
-                config=dict(workload=f"cfg{c.cfg}:{c.name}", G=c.G, T=c.T, hd=c.hd, d=c.d, K=c.K, S=c.S, iters=c.iters),
-                cpu_baseline=dict(value=val, unit=UNIT, cores=o.n_threads(), kind="oracle",
-                                  sample=f"whole cfg{c.cfg} step (all {c.G} heads), {args.steps} step(s)"),
+                ms_per_step=step_s * 1e3, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64",
+                data="synthetic", impl="reference", config=workload_config(),
+                cpu_baseline=dict(value=val, unit=UNIT, cores=cores, kind="oracle", sample=desc),
                 e2e=dict(value=val, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
     print(json.dumps(line))
 
 
+# ------------------------------------------------------------------------------------------------ replica helpers
 def rank_seed(cfg: int, what: str, rank: int) -> int:
     """Replicas: rank r works on its own synthetic layer; rank 0 uses the documented seeds."""
     return inputs.seed_of(cfg, what) + 100 * rank
@@ -127,122 +164,31 @@ def whole_job_value(local_seconds: float, units_per_rank: float, world: int, dev
     return world * units_per_rank / mx, mx
 
 
-def run_cfg4(B, pk):
-    """BASELINE.json config 4 for one tensor (K-like): batch 8 x 131072 tokens x 8 KV heads x 128, bf16, head-inner
-    layout [B*T][G][hd] (2.147 GB); d=16, K=256, S=2, 10 iterations; codebooks fitted on a seeded 65,536-token
-    sample per head, then full-cache encode and decode.  Same generator recipe as inputs.k_like, drawn on the
-    device with a seeded torch generator."""
-    c = inputs.CONFIGS[4]
-    G, hd, d, K, S, iters = c.G, c.hd, c.d, c.K, c.S, c.iters
-    T, n_fit, M = 8 * 131072, 65536, hd // d
-    gen = torch.Generator(device="cuda")
-    gen.manual_seed(inputs.seed_of(4, "k"))
-    scale = torch.exp(0.3 * torch.randn(G, hd, device="cuda", generator=gen))
-    for g in range(G):
-        scale[g, torch.randperm(hd, device="cuda", generator=gen)[:4]] *= 10.0
-    x = torch.empty(T, G, hd, dtype=torch.bfloat16, device="cuda")
-    for t0 in range(0, T, 131072):
-        x[t0:t0 + 131072] = (torch.randn(131072, G, hd, device="cuda", generator=gen) * scale).to(torch.bfloat16)
-    w = torch.exp(torch.randn(T, device="cuda", generator=gen))
-    w /= w.mean()
-    fit = torch.stack([torch.sort(torch.randperm(T, device="cuda", generator=gen)[:n_fit]).values for _ in range(G)]).contiguous()
-    view = B.view_of(x, d, head_inner=True)
-    shapes = torch.zeros(G, S, K, d, device="cuda")
-    gains = torch.zeros(G, S, K, device="cuda")
-    cb = B.codebook_of(shapes, gains)
-    ws = B.workspace(view, K, S, n_fit)
-    codes = torch.zeros(S, G, T * M, dtype=torch.uint8, device="cuda")
-    out = torch.empty_like(x)
-
-    def timed(f, n=3):
-        ts = []
-        for _ in range(n):
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record(); f(); b.record()
-            torch.cuda.synchronize()
-            ts.append(a.elapsed_time(b))
-        return float(np.median(ts))
-
-    def fit_all():
-        for s in range(S):   # residual re-derived from kv + earlier stages on the fit rows
-            B.gsrq_fit_stage(x, view, w, 0, fit, cb, s, None, iters, 0, ws, want_stats=False)
-
-    fit_all()
-    fit_ms = timed(fit_all, 2)
-    enc = lambda: B.gsrq_encode(x, view, cb, 0, S, codes, None, ws)
-    enc()
-    enc_ms = timed(enc)
-    B.gsrq_profile_enable(True)
-    enc()
-    torch.cuda.synchronize()
-    pr = B.gsrq_profile_read()
-    B.gsrq_profile_enable(False)
-    dec = lambda: B.gsrq_decode(codes, cb, S, out, view)
-    dec()
-    dec_ms = timed(dec, 5)
-    rows = G * T * M
-    enc_tf = 2.0 * K * d * rows * S / (enc_ms * 1e-3) / 1e12
-    tc_tf = 2.0 * K * d * rows * S / (pr["encode"][0] * 1e-3) / 1e12 if pr["encode"][0] > 0 else None
-    dec_bytes = rows * S + rows * 2 * d
-    dec_gbs = dec_bytes / (dec_ms * 1e-3) / 1e9
-    # sanity: decode(encode(x)) must be closer to x than 0 is (relative residual energy < 1)
-    err = float(((out[:4096].float() - x[:4096].float()) ** 2).sum() / (x[:4096].float() ** 2).sum())
-    return dict(workload="cfg4:k-cache-8x131072x8x128 head-inner, fit on 65536-token sample/head", T=T, G=G, S=S, iters=iters,
-                bytes=x.numel() * 2, fit_ms=fit_ms,
-                encode=dict(ms=enc_ms, kv_vectors_per_s=G * T / (enc_ms * 1e-3), bound="tensor", achieved_tflops=enc_tf,
-                            frac=enc_tf / pk["bf16_tflops_sustained"], tc_kernel_ms=pr["encode"][0], tc_kernel_tflops=tc_tf,
-                            exact_path_ms=pr["refine"][0]),
-                decode=dict(ms=dec_ms, gb_per_s=dec_gbs, bound="hbm", frac=dec_gbs / pk["hbm_gbs"], bytes=dec_bytes),
-                rel_residual_energy_first_4096_tokens=err)
+def timed(f, reps=20, warm=3, flush=None):
+    """CUDA-event timing of f on the current stream: `warm` untimed calls, `reps` timed ones; (median ms, min ms)."""
+    for _ in range(warm):
+        f()
+    ts = []
+    for _ in range(reps):
+        if flush is not None:
+            flush.fill_(1)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); f(); b.record()
+        torch.cuda.synchronize()
+        ts.append(a.elapsed_time(b))
+    return float(np.median(ts)), float(np.min(ts))
 
 
-def run_cfg2(B, pk):
-    """BASELINE.json config 2: V-like 8 x 16384 x 128 (Student-t, per-token norms), d=16, K=256, S=1, 20 iterations;
-    fit + encode, and the decode of the whole layer timed (33.5 MB out: L2-resident, so GB/s is effective)."""
-    c = inputs.CONFIGS[2]
+# ------------------------------------------------------------------------------------------------ extras (rank 0)
+def run_small_cfg(B, pk, cfg, kind, flush):
+    """BASELINE configs 1 / 2 / 3 for one tensor kind (8 x T x 128 bf16, fit on all tokens, L2 flushed between repetitions):
+    the whole step (per stage: fit + fused encode [0, s]; then decode), and encode / decode for every prefix S' = 1..S."""
+    c = inputs.CONFIGS[cfg]
     G, T, hd, d, K, S, iters = c.G, c.T, c.hd, c.d, c.K, c.S, c.iters
     M = hd // d
-    x = torch.from_numpy(inputs.v_like(G, T, hd, inputs.seed_of(2, "v"))).to(torch.bfloat16).cuda()
-    w = torch.from_numpy(inputs.token_weights(T, inputs.seed_of(2, "w"))).cuda()
-    view = B.view_of(x, d)
-    shapes = torch.zeros(G, S, K, d, device="cuda")
-    gains = torch.zeros(G, S, K, device="cuda")
-    cb = B.codebook_of(shapes, gains)
-    ws = B.workspace(view, K, S, 0)
-    codes = torch.zeros(S, G, T * M, dtype=torch.uint8, device="cuda")
-    out = torch.empty_like(x)
-
-    def timed(f, n=5):
-        ts = []
-        for _ in range(n):
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record(); f(); b.record()
-            torch.cuda.synchronize()
-            ts.append(a.elapsed_time(b))
-        return float(np.median(ts))
-
-    fit = lambda: B.gsrq_fit_stage(x, view, w, 0, None, cb, 0, None, iters, 0, ws, want_stats=False)
-    enc = lambda: B.gsrq_encode(x, view, cb, 0, S, codes, None, ws)
-    dec = lambda: B.gsrq_decode(codes, cb, S, out, view)
-    fit(); enc(); dec()
-    fit_ms, enc_ms, dec_ms = timed(fit, 3), timed(enc), timed(dec)
-    rows = G * T * M
-    by = rows * S + rows * 2 * d
-    return dict(workload="cfg2:v-cache-8x16384x128, S=1", fit_ms=fit_ms, encode_ms=enc_ms,
-                encode_kv_vectors_per_s=G * T / (enc_ms * 1e-3),
-                encode_tensor_frac=2.0 * K * d * rows * S / (enc_ms * 1e-3) / 1e12 / pk["bf16_tflops_sustained"],
-                decode_ms=dec_ms, decode_gb_per_s=by / (dec_ms * 1e-3) / 1e9, decode_hbm_frac=by / (dec_ms * 1e-3) / 1e9 / pk["hbm_gbs"])
-
-
-def run_cfg3(B, pk):
-    """BASELINE.json config 3 for the K-like tensor (8 x 32768 x 128, bf16): one S=4 fit (20 iterations per stage),
-    then encode throughput and decode GB/s for S = 1..4 (prefixes of the same codebooks) and the
-    weighted distortion after each stage."""
-    c = inputs.CONFIGS[3]
-    G, T, hd, d, K, S, iters = c.G, c.T, c.hd, c.d, c.K, c.S, c.iters
-    M = hd // d
-    x = torch.from_numpy(inputs.k_like(G, T, hd, inputs.seed_of(3, "k"))).to(torch.bfloat16).cuda()
-    w = torch.from_numpy(inputs.token_weights(T, inputs.seed_of(3, "w"))).cuda()
+    gen = inputs.k_like if kind == "k" else inputs.v_like
+    x = torch.from_numpy(gen(G, T, hd, inputs.seed_of(cfg, kind))).to(torch.bfloat16).cuda()
+    w = torch.from_numpy(inputs.token_weights(T, inputs.seed_of(cfg, "w"))).cuda()
     view = B.view_of(x, d)
     shapes = torch.zeros(G, S, K, d, device="cuda")
     gains = torch.zeros(G, S, K, device="cuda")
@@ -251,63 +197,87 @@ def run_cfg3(B, pk):
     codes = torch.zeros(S, G, T * M, dtype=torch.uint8, device="cuda")
     residual = torch.zeros(G, T * M, d, device="cuda")
     out = torch.empty_like(x)
-    w_rows = w.repeat_interleave(M).double()
-    e0 = float((w_rows[None] * (x.float().reshape(G, T * M, d).double() ** 2).sum(-1)).sum())
+    rows = G * T * M
 
-    def fit_all(want_dist):
-        dist = []
+    def fit_all():
         for s in range(S):
             B.gsrq_fit_stage(x, view, w, 0, None, cb, s, residual if s else None, iters, 0, ws, want_stats=False)
-            B.gsrq_encode(x, view, cb, 0, s + 1, codes, residual, ws)
-            if want_dist:
-                dist.append(float((w_rows[None] * (residual.double() ** 2).sum(-1)).sum()) / e0)
-        return dist
+            B.gsrq_encode(x, view, cb, 0, s + 1, codes, residual if s + 1 < S else None, ws)
 
-    dist = fit_all(True)
-    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    a.record(); fit_all(False); b.record()
-    torch.cuda.synchronize()
-    fit_ms = a.elapsed_time(b)
-    rows = G * T * M
+    def step():
+        fit_all()
+        B.gsrq_decode(codes, cb, S, out, view)
+
+    step_ms, step_min = timed(step, flush=flush)
+    fit_ms, fit_min = timed(fit_all, flush=flush)
+    # weighted distortion after each stage, relative to the input's weighted energy (reading c-N)
+    w_rows = w.repeat_interleave(M).double()
+    e0 = float((w_rows[None] * (x.float().reshape(G, T * M, d).double() ** 2).sum(-1)).sum())
+    dist = []
+    for n in range(1, S + 1):
+        B.gsrq_encode(x, view, cb, 0, n, codes, residual, ws)
+        dist.append(float((w_rows[None] * (residual.double() ** 2).sum(-1)).sum()) / e0)
     sweep = []
     for n in range(1, S + 1):
-        ts, td = [], []
-        for _ in range(5):
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record(); B.gsrq_encode(x, view, cb, 0, n, codes, None, ws); b.record()
-            torch.cuda.synchronize(); ts.append(a.elapsed_time(b))
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record(); B.gsrq_decode(codes, cb, n, out, view); b.record()
-            torch.cuda.synchronize(); td.append(a.elapsed_time(b))
-        em, dm = float(np.median(ts)), float(np.median(td))
+        em, emin = timed(lambda: B.gsrq_encode(x, view, cb, 0, n, codes, None, ws), flush=flush)
+        dm, dmin = timed(lambda: B.gsrq_decode(codes, cb, n, out, view), flush=flush)
         by = rows * n + rows * 2 * d
-        sweep.append(dict(S=n, bits_per_element=n * 8.0 / d, encode_ms=em, encode_kv_vectors_per_s=G * T / (em * 1e-3),
+        sweep.append(dict(S=n, bits_per_element=n * 8.0 / d, encode_ms=em, encode_ms_min=emin,
+                          encode_kv_vectors_per_s=G * T / (em * 1e-3),
                           encode_tensor_frac=2.0 * K * d * rows * n / (em * 1e-3) / 1e12 / pk["bf16_tflops_sustained"],
-                          decode_ms=dm, decode_gb_per_s=by / (dm * 1e-3) / 1e9, decode_hbm_frac=by / (dm * 1e-3) / 1e9 / pk["hbm_gbs"],
-                          rel_weighted_distortion=dist[n - 1]))
-    return dict(workload="cfg3:k-cache-8x32768x128, S=4 fit, prefixes S=1..4 (67 MB: L2-resident, effective GB/s)",
-                fit_and_encode_ms=fit_ms, sweep=sweep)
+                          decode_ms=dm, decode_ms_min=dmin, decode_gb_per_s=by / (dm * 1e-3) / 1e9,
+                          decode_frac_of_copy_bw=by / (dm * 1e-3) / 1e9 / pk["hbm_gbs"], rel_weighted_distortion=dist[n - 1]))
+    floor_ms = (iters + 2) * S * max(2.0 * K * d * rows / (pk["bf16_tflops_sustained"] * 1e12), rows * 33.0 / (pk["hbm_gbs"] * 1e9)) * 1e3
+    return dict(workload=f"cfg{cfg}:{kind}-cache-8x{T}x128, S={S}, {iters} iterations, fit on all tokens; L2 flushed per repetition"
+                         f" ({x.numel() * 2 / 1e6:.0f} MB tensor: effective GB/s)",
+                reps=20, step_ms=step_ms, step_ms_min=step_min, kv_vectors_per_s=G * T / (step_ms * 1e-3),
+                fit_and_stage_encodes_ms=fit_ms, fit_and_stage_encodes_ms_min=fit_min,
+                fit_floor_ms=floor_ms, sweep=sweep)
 
 
+def run_append(B):
+    """Encode-on-append (PAPER.md:443 (i)): latency of quantising the newest token(s) of a batch of sequences (cfg-1 layer)."""
+    c = inputs.CONFIGS[1]
+    G, T, hd, d, K, S = c.G, c.T, c.hd, c.d, c.K, c.S
+    M = hd // d
+    x = torch.from_numpy(inputs.k_like(G, T, hd, inputs.seed_of(1, "k"))).to(torch.bfloat16).cuda()
+    gen = torch.Generator(device="cuda"); gen.manual_seed(5)
+    sh = torch.nn.functional.normalize(torch.randn(G, S, K, d, device="cuda", generator=gen), dim=-1).contiguous()
+    ga = torch.rand(G, S, K, device="cuda", generator=gen).contiguous()
+    cb = B.codebook_of(sh, ga)
+    codes = torch.zeros(S, G, T * M, dtype=torch.uint8, device="cuda")
+    app = []
+    for n_new in (8, 16, 32):
+        chunk = x[:, :n_new]
+        cv = B.view_of(chunk, d)
+
+        def f():
+            for _ in range(20):
+                B.gsrq_encode_append(chunk, cv, cb, S, codes, T * M, 0)
+
+        md, mn = timed(f, reps=20)
+        app.append(dict(new_tokens=n_new, us_per_call=md * 1e3 / 20, us_per_call_min=mn * 1e3 / 20))
+    return app
+
+
+# ------------------------------------------------------------------------------------------------ main
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--cfg", type=int, default=1, choices=[1, 2])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-big", action="store_true", help="skip the config-4 (2.1 GB) encode / decode leg")
-    ap.add_argument("--only-big", action="store_true", help="run only the config-4 leg and print its JSON (profiling aid)")
+    ap.add_argument("--no-extras", action="store_true", help="skip the config 1-3 / append legs (rank 0)")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg (profiling aid)")
     args = ap.parse_args()
-    c = inputs.CONFIGS[args.cfg]
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
 
     if args.impl == "reference":
         if rank == 0:
-            run_reference(args, c)
+            run_reference(args)
         return
 
     import __graft_entry__ as ge
@@ -320,37 +290,42 @@ def main():
         dist.barrier()
     torch.cuda.set_device(local)
     B.lib()
-    if args.only_big:
-        if rank == 0:
-            print(json.dumps(dict(impl="ours", cfg4=run_cfg4(B, peaks()))))
-        return
+    pk = peaks()
+    c = inputs.CONFIGS[4]
+    G, hd, d, K, S, iters = c.G, c.hd, c.d, c.K, c.S, c.iters
+    T, n_fit, M = CFG4_T, CFG4_NFIT, c.hd // c.d
+    rows = G * T * M
+    rows_fit = G * n_fit * M
 
-    # ---- inputs (replicas: rank r works on its own layer; rank 0 is the documented seeds) ----
-    kind = c.kinds[0]
-    gen = inputs.k_like if kind == "k" else inputs.v_like
-    x_np = gen(c.G, c.T, c.hd, rank_seed(c.cfg, kind, rank))
-    w_np = inputs.token_weights(c.T, rank_seed(c.cfg, "w", rank))
-    x_host = torch.from_numpy(x_np).to(torch.bfloat16).pin_memory()
-    w_host = torch.from_numpy(w_np).pin_memory()
-    x = x_host.cuda()
-    w = w_host.cuda()
-    view = B.view_of(x, c.d)
-    G, T, hd, d, K, S = c.G, c.T, c.hd, c.d, c.K, c.S
-    M = hd // d
-    shapes = torch.zeros(G, S, K, d, device="cuda")
-    gains = torch.zeros(G, S, K, device="cuda")
-    cb = B.codebook_of(shapes, gains)
-    ws = B.workspace(view, K, S, 0)
-    codes = torch.zeros(S, G, T * M, dtype=torch.uint8, device="cuda")
-    residual = torch.zeros(G, T * M, d, device="cuda")
-    out = torch.zeros_like(x)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+    # ---- inputs: one layer's K and V cache, drawn on the device (replicas: rank r draws its own layer) ----
+    tens = {}
+    for kind in ("k", "v"):
+        dd = inputs.cfg4_device(kind, T, n_fit, seed=rank_seed(4, kind, rank))
+        tens[kind] = dd
+    view = B.view_of(tens["k"]["x"], d, head_inner=True)
+    cbs = {}
+    for kind in ("k", "v"):
+        sh = torch.zeros(G, S, K, d, device="cuda")
+        ga = torch.zeros(G, S, K, device="cuda")
+        cbs[kind] = (B.codebook_of(sh, ga), sh, ga)
+    ws = B.workspace(view, K, S, n_fit)
+    codes = {kind: torch.zeros(S, G, T * M, dtype=torch.uint8, device="cuda") for kind in ("k", "v")}
+    out = torch.empty_like(tens["k"]["x"])
+
+    def fit(kind):
+        t = tens[kind]
+        for s in range(S):   # the stage-1 fit re-derives its residual on the fit rows from kv + the stage-0 codebook
+            B.gsrq_fit_stage(t["x"], view, t["w"], 0, t["fit_tokens"], cbs[kind][0], s, None, iters, 0, ws, want_stats=False)
+
+    def encode(kind):
+        B.gsrq_encode(tens[kind]["x"], view, cbs[kind][0], 0, S, codes[kind], None, ws)
+
+    def decode(kind):
+        B.gsrq_decode(codes[kind], cbs[kind][0], S, out, view)
 
     def step():
-        for s in range(S):
-            B.gsrq_fit_stage(x, view, w, 0, None, cb, s, residual if s else None, c.iters, 0, ws, want_stats=False)
-            B.gsrq_encode(x, view, cb, 0, s + 1, codes, residual if s + 1 < S else None, ws)
-        B.gsrq_decode(codes, cb, S, out, view)
+        for kind in ("k", "v"):
+            fit(kind); encode(kind); decode(kind)
 
     def barrier():
         torch.cuda.synchronize()
@@ -360,154 +335,144 @@ def main():
 
     sampler = ClockSampler(local)
     sampler.start()                          # nvidia-smi takes a moment to come up: start it before the warm-up
-    for _ in range(max(args.warmup, 3)):
+    warm = max(args.warmup, 3)
+    for _ in range(warm):
         step()
     barrier()
     t_region0 = time.perf_counter()
     l0 = B.gsrq_launch_count()
     evs = []
     for _ in range(args.steps):
-        flush.fill_(1)                      # evict the previous step's data from L2 (not timed)
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record(); step(); b.record()
         evs.append((a, b))
     barrier()
+    t_region1 = time.perf_counter()
     launches = B.gsrq_launch_count() - l0
     ms = sum(a.elapsed_time(b) for a, b in evs)
-    value, max_s = whole_job_value(ms * 1e-3 / args.steps, G * T, world, "cuda")
+    units = 2 * G * T
+    value, max_s = whole_job_value(ms * 1e-3 / args.steps, units, world, "cuda")
     ms_per_step = max_s * 1e3
+    clocks = sampler.finish(t_region0, t_region1)
 
-    # ---- per-kernel device time, measured live with CUDA events around every launch ----
+    # ---- per-kernel device time of one step, measured live with CUDA events around every launch ----
     B.gsrq_profile_enable(True)
-    for _ in range(2):
-        step()
+    step()
     torch.cuda.synchronize()
     prof = B.gsrq_profile_read()
     B.gsrq_profile_enable(False)
-    # decode alone (cold L2) for the decode GB/s figure
-    dts = []
-    for _ in range(5):
-        flush.fill_(1)
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record(); B.gsrq_decode(codes, cb, S, out, view); b.record()
-        torch.cuda.synchronize()
-        dts.append(a.elapsed_time(b))
-    dec_ms = float(np.median(dts))
-    dec_bytes = G * T * M * S + G * T * hd * 2
-    ets = []
-    for _ in range(5):
-        flush.fill_(1)
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record(); B.gsrq_encode(x, view, cb, 0, S, codes, None, ws); b.record()
-        torch.cuda.synchronize()
-        ets.append(a.elapsed_time(b))
-    enc_ms = float(np.median(ets))
-    # encode-on-append (PAPER.md:443 (i)): latency of quantising the newest token(s) of a batch of sequences
-    app = []
-    for n_new in (8, 16, 32):
-        chunk = x[:, :n_new]
-        cv = B.view_of(chunk, d)
-        B.gsrq_encode_append(chunk, cv, cb, S, codes, T * M, 0)
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record()
-        for _ in range(20):
-            B.gsrq_encode_append(chunk, cv, cb, S, codes, T * M, 0)
-        b.record()
-        torch.cuda.synchronize()
-        app.append(dict(new_tokens=n_new, us_per_call=a.elapsed_time(b) * 1e3 / 20))
+    # the three parts for both tensors: >= 20 repetitions, median and min
+    parts = {}
+    for kind in ("k", "v"):
+        f_md, f_mn = timed(lambda: fit(kind), reps=20, warm=1)
+        e_md, e_mn = timed(lambda: encode(kind), reps=20, warm=1)
+        d_md, d_mn = timed(lambda: decode(kind), reps=20, warm=1)
+        parts[kind] = dict(fit_ms=f_md, fit_ms_min=f_mn, encode_ms=e_md, encode_ms_min=e_mn, decode_ms=d_md, decode_ms_min=d_mn)
+    # sanity: decode(encode(x)) must be closer to x than 0 is (relative residual energy < 1), V tensor, first 4096 tokens
+    xv = tens["v"]["x"][:4096].float()
+    rel_err = float(((out[:4096].float() - xv) ** 2).sum() / (xv ** 2).sum())
 
     # ---- end to end through the host-buffer C-ABI call: H2D + fit + encode + decode + D2H ----
-    sh_h = torch.empty(G, S, K, d).pin_memory(); ga_h = torch.empty(G, S, K).pin_memory()
-    co_h = torch.empty(S, G, T * M, dtype=torch.uint8).pin_memory(); out_h = torch.empty_like(x_host).pin_memory()
-    for _ in range(2):
-        B.gsrq_pipeline_host(x_host, view, w_host, K, S, c.iters, 0, sh_h, ga_h, co_h, out_h)
-    barrier()
-    t0 = time.perf_counter()
-    n_e2e = max(3, args.steps // 2)
-    for _ in range(n_e2e):
-        B.gsrq_pipeline_host(x_host, view, w_host, K, S, c.iters, 0, sh_h, ga_h, co_h, out_h)
-    barrier()
-    e2e_s = (time.perf_counter() - t0) / n_e2e
-    e2e_val, _ = whole_job_value(e2e_s, G * T, world, "cuda")
-    h2d = x_host.numel() * 2 + w_host.numel() * 4
-    d2h = sh_h.numel() * 4 + ga_h.numel() * 4 + co_h.numel() + out_h.numel() * 2
-    clocks = sampler.finish(t_region0, time.perf_counter())
+    e2e = None
+    if not args.no_e2e:
+        host = {kind: dict(x=tens[kind]["x"].cpu().pin_memory(), w=tens[kind]["w"].cpu().pin_memory(),
+                           fit=tens[kind]["fit_tokens"].cpu().pin_memory()) for kind in ("k", "v")}
+        sh_h = torch.empty(G, S, K, d).pin_memory(); ga_h = torch.empty(G, S, K).pin_memory()
+        co_h = torch.empty(S, G, T * M, dtype=torch.uint8).pin_memory()
+        out_h = torch.empty(T, G, hd, dtype=torch.bfloat16).pin_memory()
+        del out, codes
+        torch.cuda.empty_cache()
+
+        def e2e_step():
+            for kind in ("k", "v"):
+                h = host[kind]
+                B.gsrq_pipeline_host(h["x"], view, h["w"], h["fit"], K, S, iters, 0, sh_h, ga_h, co_h, out_h)
+
+        e2e_step()
+        barrier()
+        n_e2e = max(3, args.steps // 3)
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            e2e_step()
+        barrier()
+        e2e_s = (time.perf_counter() - t0) / n_e2e
+        e2e_val, _ = whole_job_value(e2e_s, units, world, "cuda")
+        h2d = sum(h["x"].numel() * 2 + h["w"].numel() * 4 + h["fit"].numel() * 8 for h in host.values())
+        d2h = 2 * (sh_h.numel() * 4 + ga_h.numel() * 4 + co_h.numel() + out_h.numel() * 2)
+        e2e = dict(value=e2e_val, unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h, ms_per_step=e2e_s * 1e3,
+                   steps=n_e2e, call="gsrq_pipeline_host (pinned host buffers, fit_tokens given)")
+        B.gsrq_release_host_pool()
+        del host, sh_h, ga_h, co_h, out_h
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()      # no collective below: the remaining legs run on rank 0 alone
-
     if rank != 0:
         return
-    big = sweep3 = v2 = None
-    if not args.no_big:
-        del flush
-        torch.cuda.empty_cache()
-        big = run_cfg4(B, peaks())
-        torch.cuda.empty_cache()
-        sweep3 = run_cfg3(B, peaks())
-        torch.cuda.empty_cache()
-        v2 = run_cfg2(B, peaks())
-    pk = peaks()
-    # Rooflines of the step's kernels, from the live CUDA-event brackets (two profiled steps).
-    # Algorithmic work: scoring pass 2*K*d flops per sub-vector; update kernel one read of
-    # the fp32 row + 1/(||r||+eps) + code = 4d + 9 bytes per sub-vector; decode S + 2d bytes per sub-vector.
-    rows_per_launch = G * T * M
+
+    # ---- rooflines: algorithmic work per launch / live launch duration ----
     tot_ms = sum(v[0] for v in prof.values())
 
-    # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the cfg-1 kernels from the ncu --set full
-    # captures summarised in profiles/r1_v5_ncu_full.md; None for workloads that were not captured
-    NCU_TRAFFIC = {"score": 10.09e6, "update": 21.42e6} if c.cfg == 1 else {}
-
-    def kern(name, cls, bound, work_per_launch, peak, unit):
-        ms, n = prof[cls]
-        per = ms / max(n, 1)
+    def kern(name, cls, bound, work_per_launch, unit, note):
+        ms_c, n = prof[cls]
+        per = ms_c / max(n, 1)
+        peak = pk["bf16_tflops_sustained"] if bound == "tensor" else pk["hbm_gbs"]
         ach = work_per_launch / (per * 1e-3) / (1e12 if bound == "tensor" else 1e9) if per > 0 else 0.0
-        return dict(bound=bound, kernel=name, achieved=ach, peak=peak, unit=unit, frac=ach / peak, traffic=NCU_TRAFFIC.get(cls),
-                    algorithmic_per_launch=work_per_launch,
-                    ms_per_launch=per, launches=n // 2, share_of_step=ms / tot_ms if tot_ms else None)
+        return dict(bound=bound, kernel=name, achieved=ach, peak=peak, unit=unit, frac=ach / peak, traffic=None,
+                    traffic_note="dram__bytes of this kernel: see the ncu --set full summaries under profiles/ (not measured in this run)",
+                    algorithmic_per_launch=work_per_launch, ms_per_launch=per, launches=n,
+                    share_of_step=ms_c / tot_ms if tot_ms else None, note=note)
 
     kerns = [
-        kern("tc::k_score_tc (tcgen05 scoring + arg-max, fit passes)", "score", "tensor", 2.0 * K * d * rows_per_launch,
-             pk["bf16_tflops_sustained"], "TFLOP/s"),
-        kern("k_update (segmented fp64 reduction + Eq. 7/8)", "update", "hbm", rows_per_launch * (4.0 * d + 9.0),
-             pk["hbm_gbs"], "GB/s"),
-        kern("tc::k_encode_tc (fused S-stage encode)", "encode", "tensor", 0.0, pk["bf16_tflops_sustained"], "TFLOP/s"),
+        kern("tc::k_fit_tc (persistent fit: tcgen05 scoring + arg-max, fp64 reduction, merge, Eq. 7/8; all passes of a stage)", "score",
+             "tensor", 2.0 * K * d * rows_fit * (iters + 1), "TFLOP/s",
+             "8192 flops per sub-vector per pass x 4,194,304 fit rows x 11 passes per launch (one launch per stage and tensor)"),
+        kern("tc::k_encode_tc (fused S-stage encode; also the stage-1 residual derivation on the fit rows)", "encode", "tensor",
+             2.0 * K * d * (rows * S + rows_fit * 1) / 2.0, "TFLOP/s",
+             "class average over its two launches per tensor: full-cache S=2 encode (67,108,864 rows) and the 1-stage derivation on the fit rows"),
+        kern("k_decode_fast (gather + sum of S scaled codewords)", "decode", "hbm", float(rows * (S + 2 * d)), "GB/s",
+             "S + 32 bytes per sub-vector x 67,108,864 rows"),
     ]
-    # the encode class mixes [0,1) and [0,2) launches: algorithmic flops of one step's encodes / their summed time
-    enc_cls_ms = prof["encode"][0] / 2
-    if enc_cls_ms > 0:
-        ach = 2.0 * K * d * rows_per_launch * sum(range(1, S + 1)) / (enc_cls_ms * 1e-3) / 1e12
-        kerns[2].update(achieved=ach, frac=ach / pk["bf16_tflops_sustained"])
     dom = max(kerns, key=lambda kk: kk["share_of_step"] or 0.0)
     roofline = dict(dom)
-    roofline["peak_source"] = pk["source"] + (" (sustained bf16: kernel timed inside a long step)" if dom["bound"] == "tensor" else " (copy bandwidth)")
-    roofline["by_class"] = {k: dict(ms=v[0] / 2, launches=v[1] // 2) for k, v in prof.items()}
+    roofline["peak_source"] = pk["source"] + (" (sustained bf16: kernel timed inside a long step)" if dom["bound"] == "tensor"
+                                              else " (copy bandwidth)")
+    roofline["by_class_ms_per_step"] = {k: dict(ms=v[0], launches=v[1]) for k, v in prof.items()}
     roofline["other_kernels"] = [kk for kk in kerns if kk is not dom]
-    line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
-                ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="bf16 in, fp32/fp64 arithmetic",
-                data="synthetic", impl="ours",
-                config=dict(workload=f"cfg{c.cfg}:{c.name}", G=G, T=T, hd=hd, d=d, K=K, S=S, iters=c.iters,
-                            l2="flushed between steps (256 MiB write, untimed)", parallelism="replicas"),
-                clocks=clocks, gpu_launches=int(launches),
-                e2e=dict(value=e2e_val, unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h,
-                         call="gsrq_pipeline_host"),
-                roofline=roofline,
-                encode=dict(kv_vectors_per_s=G * T / (enc_ms * 1e-3), ms=enc_ms, stages=S,
-                            tensor_frac=(2.0 * K * d * rows_per_launch * S / (enc_ms * 1e-3) / 1e12) / pk["bf16_tflops"]),
-                decode=dict(gb_per_s=dec_bytes / (dec_ms * 1e-3) / 1e9, ms=dec_ms, bytes=dec_bytes,
-                            hbm_frac=dec_bytes / (dec_ms * 1e-3) / 1e9 / pk["hbm_gbs"]),
-                append=app)
-    if big is not None:
-        line["cfg4"] = big
-        line["cfg3"] = sweep3
-        line["cfg2"] = v2
+    # whole parts against their floors (per tensor)
+    fit_floor_ms = (iters + 2) * S * max(2.0 * K * d * rows_fit / (pk["bf16_tflops_sustained"] * 1e12),
+                                         rows_fit * 33.0 / (pk["hbm_gbs"] * 1e9)) * 1e3
+    enc_floor_ms = max(2.0 * K * d * rows * S / (pk["bf16_tflops_sustained"] * 1e12), rows * (2 * d + S) / (pk["hbm_gbs"] * 1e9)) * 1e3
+    dec_bytes = rows * (S + 2 * d)
+    for kind in ("k", "v"):
+        pp = parts[kind]
+        pp["fit_floor_ms"] = fit_floor_ms
+        pp["fit_frac_of_floor"] = fit_floor_ms / pp["fit_ms"]
+        pp["encode_floor_ms"] = enc_floor_ms
+        pp["encode_kv_vectors_per_s"] = G * T / (pp["encode_ms"] * 1e-3)
+        pp["encode_tensor_frac"] = 2.0 * K * d * rows * S / (pp["encode_ms"] * 1e-3) / 1e12 / pk["bf16_tflops_sustained"]
+        pp["decode_gb_per_s"] = dec_bytes / (pp["decode_ms"] * 1e-3) / 1e9
+        pp["decode_frac_of_copy_bw"] = pp["decode_gb_per_s"] / pk["hbm_gbs"]
+        pp["decode_frac_of_nominal_hbm_7700"] = pp["decode_gb_per_s"] / 7700.0
+    line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=warm,
+                ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None,
+                dtype="bf16 in, fp32/fp64 arithmetic", data="synthetic", impl="ours", config=workload_config(),
+                clocks=clocks, gpu_launches=int(launches), e2e=e2e, roofline=roofline, parts=parts,
+                rel_residual_energy_v_first_4096_tokens=rel_err)
+    if not args.no_extras:
+        del tens, ws
+        torch.cuda.empty_cache()
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+        extras = {}
+        for cfg, kinds in ((1, ("k",)), (2, ("v",)), (3, ("k", "v"))):
+            for kind in kinds:
+                extras[f"cfg{cfg}_{kind}"] = run_small_cfg(B, pk, cfg, kind, flush)
+                torch.cuda.empty_cache()
+        extras["append"] = run_append(B)
+        line["extras"] = extras
     if not args.no_cpu_baseline:
-        from oracle import gsrq_oracle as o
-        t0 = time.perf_counter()
-        oracle_step(x_np, w_np, c)
-        dt = time.perf_counter() - t0
-        line["cpu_baseline"] = dict(value=G * T / dt, unit=UNIT, cores=o.n_threads(), kind="oracle",
-                                    sample=f"whole cfg{c.cfg} step once ({dt:.1f} s)")
+        val, step_s, desc, cores = oracle_value(1)
+        line["cpu_baseline"] = dict(value=val, unit=UNIT, cores=cores, kind="oracle", sample=desc,
+                                    whole_step_s_estimate=step_s)
     print(json.dumps(line))
 
 

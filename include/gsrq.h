@@ -11,8 +11,12 @@
  *   - Every pointer is a DEVICE pointer owned by the caller, except: the small structs
  *     (gsrq_view, gsrq_codebook -- host structs holding device pointers), `stats`
  *     (host), and the *_host entry points at the bottom, which say so.
- *   - The library allocates nothing that outlives a call; scratch comes from the
- *     caller's `workspace` (>= gsrq_workspace_bytes(), 256-byte aligned).
+ *   - The device entry points allocate nothing; scratch comes from the caller's `workspace`
+ *     (>= gsrq_workspace_bytes(), 256-byte aligned).  Only the *_host entry points at the bottom
+ *     allocate: from a private, library-owned stream-ordered memory pool that is kept between
+ *     calls and released by gsrq_release_host_pool() (the process-wide default pool is not touched).
+ *   - Tensor base pointers (kv, kv_out, residual, residual_out, kv_new) must be 16-byte aligned
+ *     (vector loads / stores); a misaligned pointer returns GSRQ_EINVAL.
  *   - Calls are asynchronous on `stream`.  The only implied synchronisation is the
  *     copy of `stats` to the host in gsrq_fit_stage (skipped when stats == NULL).
  *   - Return value: GSRQ_OK (0) or a negative gsrq_status; never throws, never
@@ -52,6 +56,9 @@ typedef enum {
 } gsrq_status;
 
 enum { GSRQ_F32 = 0, GSRQ_BF16 = 1 };
+
+/* A CUDA stream (the same type as cudaStream_t / CUstream; declared here so that this header needs no CUDA header). */
+typedef struct CUstream_st *gsrq_stream_t;
 
 /* Strided view of one layer's K or V cache.  Innermost hd elements are contiguous.
  * [G][T][hd] -> stride_g = T*hd, stride_t = hd;  [T][G][hd] -> stride_g = hd, stride_t = G*hd. */
@@ -110,15 +117,16 @@ size_t gsrq_workspace_bytes(const gsrq_view *view, int K, int S, int64_t n_fit_t
  * stats    : HOST array of G structs or NULL.  When given, the call synchronises `stream`
  *            and returns GSRQ_EDEGENERATE if any group could not be initialised; the per-iteration
  *            distortions are only computed in that case.
- * Kernels  : per pass two launches -- assignment (d == 16: tcgen05 filter with an fp64 re-score of the
- *            ambiguous rows inside the kernel; other d: CUDA-core filter + exact kernel) and the fused
- *            reduction / Eq. 7-8 update.  No host synchronisation inside the loop; a group whose
- *            assignments stopped changing (Alg. 1 l.15-16) is skipped by the later passes.
+ * Kernels  : d == 16: ONE persistent cooperative kernel runs all passes (tcgen05 filter with an fp64 re-score of
+ *            the ambiguous rows, per-CTA fp64 reduction, merge + Eq. 7-8, two group barriers per pass) and
+ *            leaves the loop when a group's assignments stop changing (Alg. 1 l.15-16).  Other d: two
+ *            launches per pass (CUDA-core filter + exact kernel, cluster-owner update kernel).  No host
+ *            synchronisation inside the loop.
  */
 int gsrq_fit_stage(const void *kv, const gsrq_view *view, const float *w, int64_t w_stride_g,
                    const int64_t *fit_tokens, int64_t n_fit, gsrq_codebook *cb, int stage,
                    const float *residual, int iters, uint64_t seed, gsrq_fit_stats *stats,
-                   void *workspace, size_t workspace_bytes, void *stream);
+                   void *workspace, size_t workspace_bytes, gsrq_stream_t stream);
 
 /*
  * Encode stages [stage_begin, stage_end) with fixed codebooks (RQ):
@@ -135,7 +143,7 @@ int gsrq_fit_stage(const void *kv, const gsrq_view *view, const float *w, int64_
  */
 int gsrq_encode(const void *kv, const gsrq_view *view, const gsrq_codebook *cb, int stage_begin,
                 int stage_end, uint8_t *codes, float *residual_out, void *workspace,
-                size_t workspace_bytes, void *stream);
+                size_t workspace_bytes, gsrq_stream_t stream);
 
 /*
  * Decode the first n_stages stages (PAPER.md:56  x ~= sum_l C_l[i_l]; prefix PAPER.md:25):
@@ -144,7 +152,7 @@ int gsrq_encode(const void *kv, const gsrq_view *view, const gsrq_codebook *cb, 
  * kv_out is written through out_view (same striding rules as the input view).
  */
 int gsrq_decode(const uint8_t *codes, const gsrq_codebook *cb, int n_stages, void *kv_out,
-                const gsrq_view *out_view, void *stream);
+                const gsrq_view *out_view, gsrq_stream_t stream);
 
 /*
  * Encode-on-append (PAPER.md:443 (i): the "residual quantization ... of newly generated KV vectors" kernel of
@@ -155,7 +163,7 @@ int gsrq_decode(const uint8_t *codes, const gsrq_codebook *cb, int n_stages, voi
  * One small launch, no workspace; same exact arg-max as gsrq_encode (the codes are identical).
  */
 int gsrq_encode_append(const void *kv_new, const gsrq_view *new_view, const gsrq_codebook *cb, int n_stages,
-                       uint8_t *codes, int64_t plane_rows, int64_t t0, void *stream);
+                       uint8_t *codes, int64_t plane_rows, int64_t t0, gsrq_stream_t stream);
 
 /* ---- step-wise entry points (the lock-step parity protocol of DESIGN.md section 6) ---- */
 
@@ -165,25 +173,25 @@ int gsrq_encode_append(const void *kv_new, const gsrq_view *new_view, const gsrq
  * idx_out: [G][T*M] uint8. */
 int gsrq_assign(const void *kv, const gsrq_view *view, const float *residual,
                 const gsrq_codebook *cb, int stage, int mode, uint8_t *idx_out, void *workspace,
-                size_t workspace_bytes, void *stream);
+                size_t workspace_bytes, gsrq_stream_t stream);
 
 /* Test hook: gsrq_assign through the tensor-core filter (d == 16 only) that also dumps the raw
  * filter scores, scores_out [G][T*M][256] fp32 (column k >= K holds -3e38).  Used to validate the
  * filter's error bound E_i against exact arithmetic. */
 int gsrq_debug_scores(const void *kv, const gsrq_view *view, const float *residual,
                       const gsrq_codebook *cb, int stage, int mode, float *scores_out,
-                      uint8_t *idx_out, void *workspace, size_t workspace_bytes, void *stream);
+                      uint8_t *idx_out, void *workspace, size_t workspace_bytes, gsrq_stream_t stream);
 
 /* One update (Eq. 6-8 weighted + safeguards) of stage `stage` of cb from a GIVEN assignment
  * idx [G][T*M] over all rows.  shapes_too = 0 updates gains only (Alg. 1 l.2). */
 int gsrq_update(const void *kv, const gsrq_view *view, const float *residual, const float *w,
                 int64_t w_stride_g, const uint8_t *idx, gsrq_codebook *cb, int stage,
-                int shapes_too, void *workspace, size_t workspace_bytes, void *stream);
+                int shapes_too, void *workspace, size_t workspace_bytes, gsrq_stream_t stream);
 
 /* The K initial row ids gsrq_fit_stage would draw (local fit-row indices), ids_out [G][K] int64. */
 int gsrq_init_ids(const void *kv, const gsrq_view *view, const float *residual,
                   const int64_t *fit_tokens, int64_t n_fit, int K, int stage, uint64_t seed,
-                  int64_t *ids_out, void *workspace, size_t workspace_bytes, void *stream);
+                  int64_t *ids_out, void *workspace, size_t workspace_bytes, gsrq_stream_t stream);
 
 /* ---- host-buffer convenience (end-to-end measurement: H2D + kernels + D2H inside) ---- */
 
@@ -198,14 +206,20 @@ int gsrq_decode_host(const uint8_t *codes_host, const gsrq_codebook *cb, int n_s
                      void *kv_out_host, const gsrq_view *out_view);
 
 /* The whole hot path on HOST buffers, as one call (the end-to-end measurement): copies kv_host
- * (dense, laid out as `view` says) and w_host ([T] or NULL) to the device, then for each stage
- * s < S: gsrq_fit_stage (all tokens, `iters`, `seed`) + gsrq_encode of that stage; then, when
- * kv_out_host != NULL, gsrq_decode of all S stages; copies shapes [G][S][K][d], gains [G][S][K],
- * codes [S][G][T*M] (and the decoded tensor) back to the host and synchronises.  Device scratch
- * is taken from the stream-ordered allocator for the duration of the call. */
-int gsrq_pipeline_host(const void *kv_host, const gsrq_view *view, const float *w_host, int K, int S,
-                       int iters, uint64_t seed, float *shapes_host, float *gains_host,
+ * (dense, laid out as `view` says), w_host ([T] or NULL) and fit_tokens_host ([G][n_fit] sorted token ids,
+ * or NULL = fit on all T tokens) to the device.  Fit on all tokens: for each stage s < S gsrq_fit_stage
+ * (`iters`, `seed`) + gsrq_encode of that stage (its residual feeds the next fit).  Fit on a token subset:
+ * the S fits (each re-deriving its residual on the fit rows), then one fused gsrq_encode of all stages.  Then,
+ * when kv_out_host != NULL, gsrq_decode of all S stages; copies shapes [G][S][K][d], gains [G][S][K],
+ * codes [S][G][T*M] (and the decoded tensor) back to the host and synchronises.  Returns GSRQ_EDEGENERATE if a
+ * group could not be initialised (fewer than K distinct non-zero fit rows).  Device memory comes from the
+ * library's private pool (see the conventions at the top). */
+int gsrq_pipeline_host(const void *kv_host, const gsrq_view *view, const float *w_host, const int64_t *fit_tokens_host,
+                       int64_t n_fit, int K, int S, int iters, uint64_t seed, float *shapes_host, float *gains_host,
                        uint8_t *codes_host, void *kv_out_host);
+
+/* Free the device memory the *_host entry points keep between calls (current device). */
+void gsrq_release_host_pool(void);
 
 /* ---- measurement hooks (host functions) ---- */
 

@@ -42,7 +42,7 @@ class gsrq_fit_stats(C.Structure):
 
 _lib = None
 EXPORTS = ["gsrq_workspace_bytes", "gsrq_fit_stage", "gsrq_encode", "gsrq_decode", "gsrq_encode_append", "gsrq_assign", "gsrq_update",
-           "gsrq_init_ids", "gsrq_debug_scores", "gsrq_encode_host", "gsrq_decode_host", "gsrq_pipeline_host", "gsrq_profile_enable",
+           "gsrq_init_ids", "gsrq_debug_scores", "gsrq_encode_host", "gsrq_decode_host", "gsrq_pipeline_host", "gsrq_release_host_pool", "gsrq_profile_enable",
            "gsrq_profile_read", "gsrq_launch_count", "gsrq_last_error", "gsrq_version"]
 
 
@@ -169,12 +169,17 @@ def gsrq_decode_host(codes_host: torch.Tensor, cb, n_stages, kv_out_host: torch.
     _check(lib().gsrq_decode_host(_ptr(codes_host), C.byref(cb), n_stages, _ptr(kv_out_host), C.byref(out_view)))
 
 
-def gsrq_pipeline_host(kv_host, view, w_host, K, S, iters, seed, shapes_host, gains_host, codes_host, kv_out_host):
+def gsrq_pipeline_host(kv_host, view, w_host, fit_tokens_host, K, S, iters, seed, shapes_host, gains_host, codes_host, kv_out_host):
     """All arguments are HOST tensors; H2D, fit + encode (+ decode), D2H and the sync happen inside."""
-    for t in (kv_host, w_host, shapes_host, gains_host, codes_host, kv_out_host):
+    for t in (kv_host, w_host, fit_tokens_host, shapes_host, gains_host, codes_host, kv_out_host):
         assert t is None or not t.is_cuda
-    _check(lib().gsrq_pipeline_host(_ptr(kv_host), C.byref(view), _ptr(w_host), K, S, iters, C.c_uint64(seed),
-                                    _ptr(shapes_host), _ptr(gains_host), _ptr(codes_host), _ptr(kv_out_host)))
+    n_fit = 0 if fit_tokens_host is None else fit_tokens_host.shape[1]
+    _check(lib().gsrq_pipeline_host(_ptr(kv_host), C.byref(view), _ptr(w_host), _ptr(fit_tokens_host), C.c_int64(n_fit), K, S, iters,
+                                    C.c_uint64(seed), _ptr(shapes_host), _ptr(gains_host), _ptr(codes_host), _ptr(kv_out_host)))
+
+
+def gsrq_release_host_pool():
+    lib().gsrq_release_host_pool()
 
 
 KERNEL_CLASSES = ["prep", "score", "refine", "update", "misc", "decode", "encode"]

@@ -136,6 +136,12 @@ static int check_view(const gsrq_view *v, int K, int S) {
   return GSRQ_OK;
 }
 
+// Tensors are read / written with 16-byte vector accesses: a misaligned base would fault instead of returning an error.
+static int check_align16(const void *ptr, const char *what) {
+  if (ptr && ((uintptr_t)ptr & 15)) { set_error("%s must be 16-byte aligned", what); return GSRQ_EINVAL; }
+  return GSRQ_OK;
+}
+
 static int check_ws(const void *ws, size_t bytes, size_t need) {
   if (!ws || ((uintptr_t)ws & 255)) { set_error("workspace must be non-NULL and 256-byte aligned"); return GSRQ_EWORKSPACE; }
   if (bytes < need) { set_error("workspace too small: %zu < %zu bytes", bytes, need); return GSRQ_EWORKSPACE; }
@@ -464,7 +470,7 @@ size_t gsrq_workspace_bytes(const gsrq_view *view, int K, int S, int64_t n_fit_t
 
 int gsrq_fit_stage(const void *kv, const gsrq_view *view, const float *w, int64_t w_stride_g, const int64_t *fit_tokens,
                    int64_t n_fit, gsrq_codebook *cb, int stage, const float *residual, int iters, uint64_t seed,
-                   gsrq_fit_stats *stats, void *workspace, size_t workspace_bytes, void *stream_) {
+                   gsrq_fit_stats *stats, void *workspace, size_t workspace_bytes, gsrq_stream_t stream_) {
   cudaStream_t stream = (cudaStream_t)stream_;
   if (!kv || !cb || !cb->shapes || !cb->gains) { set_error("NULL kv / codebook"); return GSRQ_EINVAL; }
   int rc = check_view(view, cb->K, cb->S);
@@ -472,6 +478,7 @@ int gsrq_fit_stage(const void *kv, const gsrq_view *view, const float *w, int64_
   if (stage < 0 || stage >= cb->S) { set_error("stage %d out of [0, %d)", stage, cb->S); return GSRQ_EINVAL; }
   if (iters < 0 || iters > GSRQ_MAX_ITERS) { set_error("iters must be in [0, %d]", GSRQ_MAX_ITERS); return GSRQ_EINVAL; }
   if (fit_tokens && (n_fit <= 0 || n_fit > view->T)) { set_error("n_fit out of range"); return GSRQ_EINVAL; }
+  if ((rc = check_align16(kv, "kv")) || (rc = check_align16(residual, "residual"))) return rc;
   const Plan pl = make_plan(view, cb->K, cb->S, fit_tokens ? n_fit : 0);
   if (pl.Nf < cb->K) { set_error("fewer fit rows (%lld) than codewords (%d)", pl.Nf, cb->K); return GSRQ_EDEGENERATE; }
   rc = check_ws(workspace, workspace_bytes, pl.total);
@@ -534,7 +541,7 @@ int gsrq_fit_stage(const void *kv, const gsrq_view *view, const float *w, int64_
     cudaError_t e = cudaMemcpyAsync(h, st, (size_t)G * sizeof(DevStats), cudaMemcpyDeviceToHost, stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
     if (e != cudaSuccess) { free(h); set_error("stats copy failed: %s", cudaGetErrorString(e)); return GSRQ_ECUDA; }
-    int degenerate = 0;
+    int degenerate = 0, lost = 0;
     for (int g = 0; g < G; ++g) {
       gsrq_fit_stats *o = stats + g;
       memset(o, 0, sizeof(*o));
@@ -546,9 +553,11 @@ int gsrq_fit_stage(const void *kv, const gsrq_view *view, const float *w, int64_
       }
       o->n_empty_last = h[g].n_empty[h[g].iters_run];
       o->n_changed_last = h[g].iters_run ? h[g].changed[h[g].iters_run] : 0;
-      degenerate |= (h[g].err != 0);
+      degenerate |= (h[g].err == GSRQ_EDEGENERATE);
+      lost |= (h[g].err != 0 && h[g].err != GSRQ_EDEGENERATE);
     }
     free(h);
+    if (lost) { set_error("the fit kernel's group barrier timed out"); return GSRQ_ECUDA; }
     if (degenerate) { set_error("a group has fewer than K distinct non-zero fit rows"); return GSRQ_EDEGENERATE; }
   }
   return GSRQ_OK;
@@ -556,12 +565,13 @@ int gsrq_fit_stage(const void *kv, const gsrq_view *view, const float *w, int64_
 
 
 int gsrq_encode(const void *kv, const gsrq_view *view, const gsrq_codebook *cb, int stage_begin, int stage_end,
-                uint8_t *codes, float *residual_out, void *workspace, size_t workspace_bytes, void *stream_) {
+                uint8_t *codes, float *residual_out, void *workspace, size_t workspace_bytes, gsrq_stream_t stream_) {
   cudaStream_t stream = (cudaStream_t)stream_;
   if (!kv || !cb || !cb->shapes || !cb->gains || !codes) { set_error("NULL kv / codebook / codes"); return GSRQ_EINVAL; }
   int rc = check_view(view, cb->K, cb->S);
   if (rc) return rc;
   if (stage_begin < 0 || stage_end > cb->S || stage_begin >= stage_end) { set_error("bad stage range [%d, %d)", stage_begin, stage_end); return GSRQ_EINVAL; }
+  if ((rc = check_align16(kv, "kv")) || (rc = check_align16(residual_out, "residual_out"))) return rc;
   const Plan pl = make_plan(view, cb->K, cb->S, -1);
   rc = check_ws(workspace, workspace_bytes, pl.encode_total);
   if (rc) return rc;
@@ -584,12 +594,13 @@ int gsrq_encode(const void *kv, const gsrq_view *view, const gsrq_codebook *cb, 
 }
 
 int gsrq_decode(const uint8_t *codes, const gsrq_codebook *cb, int n_stages, void *kv_out, const gsrq_view *out_view,
-                void *stream_) {
+                gsrq_stream_t stream_) {
   cudaStream_t stream = (cudaStream_t)stream_;
   if (!codes || !cb || !cb->shapes || !cb->gains || !kv_out) { set_error("NULL codes / codebook / output"); return GSRQ_EINVAL; }
   int rc = check_view(out_view, cb->K, cb->S);
   if (rc) return rc;
   if (n_stages < 0 || n_stages > cb->S) { set_error("n_stages %d out of [0, %d]", n_stages, cb->S); return GSRQ_EINVAL; }
+  if ((rc = check_align16(kv_out, "kv_out"))) return rc;
   const int d = out_view->d;
   DecParams p{};
   p.codes = codes; p.shapes = cb->shapes; p.gains = cb->gains; p.S = cb->S; p.K = cb->K; p.G = out_view->G;
@@ -660,13 +671,14 @@ int gsrq_decode(const uint8_t *codes, const gsrq_codebook *cb, int n_stages, voi
 }
 
 int gsrq_encode_append(const void *kv_new, const gsrq_view *new_view, const gsrq_codebook *cb, int n_stages, uint8_t *codes,
-                       int64_t plane_rows, int64_t t0, void *stream_) {
+                       int64_t plane_rows, int64_t t0, gsrq_stream_t stream_) {
   cudaStream_t stream = (cudaStream_t)stream_;
   if (!kv_new || !cb || !cb->shapes || !cb->gains || !codes) { set_error("NULL kv / codebook / codes"); return GSRQ_EINVAL; }
   int rc = check_view(new_view, cb->K, cb->S);
   if (rc) return rc;
   const int M = new_view->hd / new_view->d;
   if (n_stages < 1 || n_stages > cb->S) { set_error("n_stages %d out of [1, %d]", n_stages, cb->S); return GSRQ_EINVAL; }
+  if ((rc = check_align16(kv_new, "kv_new"))) return rc;
   if (t0 < 0 || plane_rows < (t0 + new_view->T) * M) { set_error("tokens [%lld, %lld) do not fit in planes of %lld rows", (long long)t0, (long long)(t0 + new_view->T), (long long)plane_rows); return GSRQ_EINVAL; }
   AppendParams p{};
   p.src = make_src(kv_new, new_view, nullptr, 0);
@@ -687,6 +699,7 @@ static int assign_all_rows(const void *kv, const gsrq_view *view, const float *r
   int rc = check_view(view, cb->K, cb->S);
   if (rc) return rc;
   if (stage < 0 || stage >= cb->S || (mode != 0 && mode != 1)) { set_error("bad stage / mode"); return GSRQ_EINVAL; }
+  if ((rc = check_align16(kv, "kv")) || (rc = check_align16(residual, "residual"))) return rc;
   const Plan pl = make_plan(view, cb->K, cb->S, 0);
   rc = check_ws(workspace, workspace_bytes, pl.total);
   if (rc) return rc;
@@ -722,19 +735,19 @@ static int assign_all_rows(const void *kv, const gsrq_view *view, const float *r
 }
 
 int gsrq_assign(const void *kv, const gsrq_view *view, const float *residual, const gsrq_codebook *cb, int stage, int mode,
-                uint8_t *idx_out, void *workspace, size_t workspace_bytes, void *stream_) {
+                uint8_t *idx_out, void *workspace, size_t workspace_bytes, gsrq_stream_t stream_) {
   return assign_all_rows(kv, view, residual, cb, stage, mode, idx_out, nullptr, workspace, workspace_bytes, (cudaStream_t)stream_);
 }
 
 int gsrq_debug_scores(const void *kv, const gsrq_view *view, const float *residual, const gsrq_codebook *cb, int stage, int mode,
-                      float *scores_out, uint8_t *idx_out, void *workspace, size_t workspace_bytes, void *stream_) {
+                      float *scores_out, uint8_t *idx_out, void *workspace, size_t workspace_bytes, gsrq_stream_t stream_) {
   if (!scores_out) { set_error("NULL scores_out"); return GSRQ_EINVAL; }
   return assign_all_rows(kv, view, residual, cb, stage, mode, idx_out, scores_out, workspace, workspace_bytes, (cudaStream_t)stream_);
 }
 
 int gsrq_update(const void *kv, const gsrq_view *view, const float *residual, const float *w, int64_t w_stride_g,
                 const uint8_t *idx, gsrq_codebook *cb, int stage, int shapes_too, void *workspace, size_t workspace_bytes,
-                void *stream_) {
+                gsrq_stream_t stream_) {
   cudaStream_t stream = (cudaStream_t)stream_;
   if ((!kv && !residual) || !cb || !cb->shapes || !cb->gains || !idx) { set_error("NULL input"); return GSRQ_EINVAL; }
   int rc = check_view(view, cb->K, cb->S);
@@ -757,7 +770,7 @@ int gsrq_update(const void *kv, const gsrq_view *view, const float *residual, co
 }
 
 int gsrq_init_ids(const void *kv, const gsrq_view *view, const float *residual, const int64_t *fit_tokens, int64_t n_fit,
-                  int K, int stage, uint64_t seed, int64_t *ids_out, void *workspace, size_t workspace_bytes, void *stream_) {
+                  int K, int stage, uint64_t seed, int64_t *ids_out, void *workspace, size_t workspace_bytes, gsrq_stream_t stream_) {
   cudaStream_t stream = (cudaStream_t)stream_;
   if ((!kv && !residual) || !ids_out) { set_error("NULL input"); return GSRQ_EINVAL; }
   int rc = check_view(view, K, 1);
@@ -829,62 +842,109 @@ int gsrq_decode_host(const uint8_t *codes_host, const gsrq_codebook *cb, int n_s
 }
 
 
-int gsrq_pipeline_host(const void *kv_host, const gsrq_view *view, const float *w_host, int K, int S, int iters,
-                       uint64_t seed, float *shapes_host, float *gains_host, uint8_t *codes_host, void *kv_out_host) {
+// ---- the *_host entry points' private stream-ordered pool (one per device, kept between calls) ----
+static std::mutex g_pool_mu;
+static cudaMemPool_t g_pools[64] = {nullptr};
+
+static cudaMemPool_t host_pool() {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
+  std::lock_guard<std::mutex> lk(g_pool_mu);
+  if (!g_pools[dev]) {
+    cudaMemPoolProps props;
+    memset(&props, 0, sizeof(props));
+    props.allocType = cudaMemAllocationTypePinned;
+    props.handleTypes = cudaMemHandleTypeNone;
+    props.location.type = cudaMemLocationTypeDevice;
+    props.location.id = dev;
+    cudaMemPool_t pool = nullptr;
+    if (cudaMemPoolCreate(&pool, &props) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    unsigned long long keep = ~0ull;   // keep the memory between calls (gsrq_release_host_pool() returns it)
+    cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    g_pools[dev] = pool;
+  }
+  return g_pools[dev];
+}
+
+__global__ void k_collect_err(const DevStats *__restrict__ st, int G, int *__restrict__ err_accum) {
+  for (int g = threadIdx.x; g < G; g += blockDim.x)
+    if (st[g].err) atomicMin(err_accum, st[g].err);   // error codes are negative: keep the lowest
+}
+
+int gsrq_pipeline_host(const void *kv_host, const gsrq_view *view, const float *w_host, const int64_t *fit_tokens_host,
+                       int64_t n_fit, int K, int S, int iters, uint64_t seed, float *shapes_host, float *gains_host,
+                       uint8_t *codes_host, void *kv_out_host) {
   if (!kv_host || !shapes_host || !gains_host || !codes_host) { set_error("NULL input"); return GSRQ_EINVAL; }
   int rc = check_view(view, K, S);
   if (rc) return rc;
+  if (fit_tokens_host && (n_fit <= 0 || n_fit > view->T)) { set_error("n_fit out of range"); return GSRQ_EINVAL; }
   const int G = view->G, d = view->d, M = view->hd / d;
   const size_t esz = view->dtype == GSRQ_BF16 ? 2 : 4;
   const size_t kv_bytes = (size_t)G * view->T * view->hd * esz;
   const size_t n_rows = (size_t)G * view->T * M;
   const size_t sh_bytes = (size_t)G * S * K * d * 4, ga_bytes = (size_t)G * S * K * 4;
-  const size_t wsb = gsrq_workspace_bytes(view, K, S, 0);
+  const size_t ft_bytes = fit_tokens_host ? (size_t)G * n_fit * sizeof(int64_t) : 0;
+  const size_t wsb = gsrq_workspace_bytes(view, K, S, fit_tokens_host ? n_fit : 0);
+  const bool per_stage = !fit_tokens_host;   // fit on all tokens: encode each stage after its fit, its residual feeds the next fit
   cudaStream_t stream = nullptr;
+  cudaMemPool_t pool = host_pool();
+  if (!pool) { set_error("gsrq_pipeline_host: could not create the device memory pool"); return GSRQ_ECUDA; }
   char *base = nullptr;
-  size_t off[8], o = 0;
-  const size_t sizes[8] = {kv_bytes, (size_t)view->T * 4, sh_bytes, ga_bytes, n_rows * S, n_rows * d * 4, wsb, kv_bytes};
-  for (int i = 0; i < 8; ++i) { off[i] = o; o += align_up(sizes[i]); }
-  {  // keep the stream-ordered pool's memory across calls (by default it is returned to the driver at every sync)
-    static bool pool_set = false;
-    if (!pool_set) {
-      int dev = 0;
-      cudaMemPool_t pool;
-      if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
-        unsigned long long keep = ~0ull;
-        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
-      }
-      pool_set = true;
-    }
-  }
-  cudaError_t e = cudaMallocAsync((void **)&base, o, stream);
+  size_t off[10], o = 0;
+  const size_t sizes[10] = {kv_bytes, (size_t)view->T * 4, sh_bytes, ga_bytes, n_rows * S, per_stage ? n_rows * d * 4 : 0, wsb,
+                            kv_out_host ? kv_bytes : 0, ft_bytes, 256};
+  for (int i = 0; i < 10; ++i) { off[i] = o; o += align_up(sizes[i]); }
+  cudaError_t e = cudaMallocFromPoolAsync((void **)&base, o, pool, stream);
   if (e != cudaSuccess) { set_error("gsrq_pipeline_host: %s", cudaGetErrorString(e)); return GSRQ_ECUDA; }
   void *d_kv = base + off[0];
   float *d_w = w_host ? (float *)(base + off[1]) : nullptr;
   gsrq_codebook cb{K, S, (float *)(base + off[2]), (float *)(base + off[3])};
   uint8_t *d_codes = (uint8_t *)(base + off[4]);
-  float *d_res = (float *)(base + off[5]);
+  float *d_res = per_stage ? (float *)(base + off[5]) : nullptr;
   void *d_ws = base + off[6], *d_out = base + off[7];
+  int64_t *d_ft = fit_tokens_host ? (int64_t *)(base + off[8]) : nullptr;
+  int *d_err = (int *)(base + off[9]);
+  const Plan pl = make_plan(view, K, S, fit_tokens_host ? n_fit : 0);
   e = cudaMemcpyAsync(d_kv, kv_host, kv_bytes, cudaMemcpyHostToDevice, stream);
   if (e == cudaSuccess && w_host) e = cudaMemcpyAsync(d_w, w_host, (size_t)view->T * 4, cudaMemcpyHostToDevice, stream);
+  if (e == cudaSuccess && d_ft) e = cudaMemcpyAsync(d_ft, fit_tokens_host, ft_bytes, cudaMemcpyHostToDevice, stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(d_err, 0, sizeof(int), stream);
   for (int s = 0; s < S && rc == GSRQ_OK && e == cudaSuccess; ++s) {
-    rc = gsrq_fit_stage(d_kv, view, d_w, 0, nullptr, 0, &cb, s, s ? d_res : nullptr, iters, seed, nullptr, d_ws, wsb, stream);
-    // the fused tensor-core encode restarts from stage 0 (cheap); otherwise only stage s is encoded
-    const int sb = can_encode_tc(d_kv, view, 0) ? 0 : s;
-    if (rc == GSRQ_OK) rc = gsrq_encode(d_kv, view, &cb, sb, s + 1, d_codes, (s + 1 < S) ? d_res : nullptr, d_ws, wsb, stream);
+    rc = gsrq_fit_stage(d_kv, view, d_w, 0, d_ft, n_fit, &cb, s, (per_stage && s) ? d_res : nullptr, iters, seed, nullptr, d_ws, wsb, stream);
+    if (rc == GSRQ_OK) {   // remember a failed initialisation (the stage's statistics are reset by the next fit)
+      k_collect_err<<<1, 128, 0, stream>>>((const DevStats *)((char *)d_ws + pl.off_st), G, d_err);
+      e = cudaGetLastError();
+    }
+    if (per_stage && rc == GSRQ_OK && e == cudaSuccess) {
+      // the fused tensor-core encode restarts from stage 0 (cheap); otherwise only stage s is encoded
+      const int sb = can_encode_tc(d_kv, view, 0) ? 0 : s;
+      rc = gsrq_encode(d_kv, view, &cb, sb, s + 1, d_codes, (s + 1 < S) ? d_res : nullptr, d_ws, wsb, stream);
+    }
   }
+  if (!per_stage && rc == GSRQ_OK && e == cudaSuccess) rc = gsrq_encode(d_kv, view, &cb, 0, S, d_codes, nullptr, d_ws, wsb, stream);
   if (rc == GSRQ_OK && e == cudaSuccess && kv_out_host) {
     rc = gsrq_decode(d_codes, &cb, S, d_out, view, stream);
     if (rc == GSRQ_OK) e = cudaMemcpyAsync(kv_out_host, d_out, kv_bytes, cudaMemcpyDeviceToHost, stream);
   }
+  int h_err = 0;
   if (rc == GSRQ_OK && e == cudaSuccess) e = cudaMemcpyAsync(shapes_host, cb.shapes, sh_bytes, cudaMemcpyDeviceToHost, stream);
   if (rc == GSRQ_OK && e == cudaSuccess) e = cudaMemcpyAsync(gains_host, cb.gains, ga_bytes, cudaMemcpyDeviceToHost, stream);
   if (rc == GSRQ_OK && e == cudaSuccess) e = cudaMemcpyAsync(codes_host, d_codes, n_rows * S, cudaMemcpyDeviceToHost, stream);
+  if (rc == GSRQ_OK && e == cudaSuccess) e = cudaMemcpyAsync(&h_err, d_err, sizeof(int), cudaMemcpyDeviceToHost, stream);
   cudaFreeAsync(base, stream);
   cudaError_t e2 = cudaStreamSynchronize(stream);
   if (e == cudaSuccess) e = e2;
   if (e != cudaSuccess) { set_error("gsrq_pipeline_host: %s", cudaGetErrorString(e)); return GSRQ_ECUDA; }
+  if (rc == GSRQ_OK && h_err == GSRQ_EDEGENERATE) { set_error("a group has fewer than K distinct non-zero fit rows"); return GSRQ_EDEGENERATE; }
+  if (rc == GSRQ_OK && h_err != 0) { set_error("the fit kernel's group barrier timed out"); return GSRQ_ECUDA; }
   return rc;
+}
+
+void gsrq_release_host_pool(void) {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return;
+  std::lock_guard<std::mutex> lk(g_pool_mu);
+  if (g_pools[dev]) { cudaMemPoolDestroy(g_pools[dev]); g_pools[dev] = nullptr; }
 }
 
 void gsrq_profile_enable(int on) {

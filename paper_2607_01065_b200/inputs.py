@@ -130,16 +130,16 @@ def make(cfg: int, kind: str | None = None, T: int | None = None):
 
 
 def cfg4_device(kind: str = "k", T: int = 8 * 131072, n_fit: int = 65536, G: int = HEADS, hd: int = HEAD_DIM,
-                device: str = "cuda", chunk: int = 131072):
+                device: str = "cuda", chunk: int = 131072, seed: int | None = None):
     """BASELINE config 4 drawn ON THE DEVICE (a 2.1 GB tensor is too slow to draw with numpy): head-inner layout
     [T][G][hd] bf16, per-token weights [T] fp32 (lognormal(0,1) / mean) and the sorted seeded fit sample [G][n_fit]
     int64.  Same recipes as k_like / v_like / token_weights / fit_sample with a seeded torch CUDA generator
-    (seed_of(4, kind)); draws in the order: per-head statistics, tensor chunks, weights, fit sample.  The oracle is
+    (seed_of(4, kind) unless `seed` is given); draws in the order: per-head statistics, tensor chunks, weights, fit sample.  The oracle is
     given copies of the same bits (tests copy the rows they need to the host).
       k: N(0,1) x per-channel scale exp(0.3 N(0,1)), 4 outlier channels per head x10 (fixed over batch and tokens).
       v: Student-t(nu=4) = N(0,1) / sqrt(chi2_4 / 4), x per-(batch, token) factor exp(0.5 N(0,1)) shared by heads."""
     gen = torch.Generator(device=device)
-    gen.manual_seed(seed_of(4, kind))
+    gen.manual_seed(seed_of(4, kind) if seed is None else seed)
     x = torch.empty(T, G, hd, dtype=torch.bfloat16, device=device)
     if kind == "k":
         scale = torch.exp(0.3 * torch.randn(G, hd, device=device, generator=gen))
