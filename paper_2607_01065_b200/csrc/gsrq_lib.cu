@@ -76,7 +76,8 @@ struct Plan {
   // [0, encode_total): what gsrq_encode needs; the rest is for the fit
   size_t off_list, off_cnt, off_st, off_ebimg, off_egmax, off_eres, encode_total;
   size_t off_Rf, off_coef, off_wt, off_idx, off_ids, off_epart, off_term;
-  size_t off_ahi, off_alo, off_rnorm, off_bimg, off_gmax, off_wn, off_part, off_bar, off_clk, total;
+  size_t off_ahi, off_alo, off_rnorm, off_bimg, off_gmax, off_wn, off_part, off_bar, off_clk, off_chg, total;
+  long long chg_stride_g;
 };
 
 constexpr int kNumCounters = 256;
@@ -119,6 +120,9 @@ static Plan make_plan(const gsrq_view *v, int K, int S, long long n_fit_tokens) 
   p.off_part = o;  o += align_up(tcp && p.Nf ? (size_t)(v->G > kMaxCtas ? v->G : kMaxCtas) * tc::kN * tc::kFitP * sizeof(double) : 0);
   p.off_bar = o;   o += align_up(tcp ? (size_t)v->G * sizeof(unsigned int) : 0);
   p.off_clk = o;   o += align_up(tcp ? (size_t)(v->G > kMaxCtas ? v->G : kMaxCtas) * 16 * sizeof(long long) : 0);
+  // change lists of the incremental reduction: per group 128 entries per tile + 512 per CTA (k_fit_tc.cuh)
+  p.chg_stride_g = ((p.Nf + tc::kTileM - 1) / tc::kTileM) * tc::kTileM + 512LL * kMaxCtas;
+  p.off_chg = o;   o += align_up(tcp && p.Nf ? (size_t)v->G * p.chg_stride_g * sizeof(uint2) : 0);
   p.total = o;
   return p;
 }
@@ -284,6 +288,7 @@ static int run_fit_tc(const Plan &pl, char *ws, const TcMaps *maps, int G, int M
   p.t_begin = t_begin; p.t_end = t_end; p.skip_scoring = skip_scoring ? 1 : 0; p.lloyd_override = lloyd_override;
   p.st = st; p.term = st ? (double *)(ws + pl.off_term) : nullptr; p.term_stride = kTermStride;
   p.part = (double *)(ws + pl.off_part); p.bar = (unsigned int *)(ws + pl.off_bar);
+  p.chg = (uint2 *)(ws + pl.off_chg); p.chg_stride_g = pl.chg_stride_g;
   GSRQ_CUDA_CHECK(cudaMemsetAsync(p.bar, 0, (size_t)G * sizeof(unsigned int), stream));
   static const bool want_clk = getenv("GSRQ_FIT_CLOCKS") != nullptr;   // debug: per-phase cycle counts on stderr
   if (want_clk) {
@@ -314,8 +319,9 @@ static int run_fit_tc(const Plan &pl, char *ws, const TcMaps *maps, int G, int M
     double sum[16] = {0};
     for (size_t c = 0; c < (size_t)G * nx; ++c) for (int q = 0; q < 16; ++q) sum[q] += (double)h[c * 16 + q];
     const double den = (double)G * nx * (t_end - t_begin + 1);
-    fprintf(stderr, "k_fit_tc cycles per pass (mean over %d CTAs, %d passes): stage %.0f score %.0f publish %.0f bar1 %.0f merge %.0f bar2 %.0f | reduce: load %.0f bitmap %.0f wait %.0f (unused %.0f) accumulate %.0f | coef-store %.0f bitmap-rmw %.0f fetch %.0f\n",
-            G * nx, t_end - t_begin + 1, sum[0] / den, sum[1] / den, sum[2] / den, sum[3] / den, sum[4] / den, sum[5] / den, sum[6] / den, sum[7] / den, sum[8] / den, sum[9] / den, sum[10] / den, sum[11] / den, sum[12] / den, sum[13] / den);
+    fprintf(stderr, "k_fit_tc cycles per pass (mean over %d CTAs, %d passes): stage %.0f score %.0f reduce+publish %.0f bar1 %.0f merge %.0f bar2 %.0f | list entries %.0f batches %.1f; first-pass reduce %.0f cycles\n",
+            G * nx, t_end - t_begin + 1, sum[0] / den, sum[1] / den, sum[2] / den, sum[3] / den, sum[4] / den, sum[5] / den, sum[6] / den, sum[7] / den,
+            sum[8] / ((double)G * nx));
   }
   return GSRQ_OK;
 }

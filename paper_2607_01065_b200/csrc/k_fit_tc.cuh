@@ -6,18 +6,20 @@
 //   (a) stage   the group's operand images (B_hi, B_lo, B_bias) and fp32 codebook, global -> shared memory;
 //   (b) score   tcgen05 filter + fused arg-max over the CTA's tiles, exact fp64 re-score of the ambiguous rows
 //               (k_score_tc.cuh; Eq. 5); assignment bytes out, changed-row count;
-//   (c) reduce  the CTA's rows, in batches of 1024 staged by one bulk copy: a per-cluster membership bitmap is built
-//               with plain byte stores (each thread owns one byte column, so there are no atomics); thread k then
-//               walks cluster k's bitmap row and adds the rows it finds to its own fp64 registers
-//               A_k = sum w_i r_i, B_k = sum w_i r_i/(||r_i||+eps), W_k = sum w_i, cnt_k (Eq. 6-8 sums, weighted per
-//               reading c-W); after the last batch the CTA's partials [K][34] go to global memory;
+//   (c) reduce  the CTA keeps the sums of its own rows per cluster, A_k = sum w_i r_i, B_k = sum w_i r_i/(||r_i||+eps),
+//               W_k = sum w_i, cnt_k (Eq. 6-8 sums, weighted per reading c-W), in shared memory as fp64 for the whole
+//               fit.  The first pass adds every row; later passes are INCREMENTAL: the scoring epilogue appends the
+//               rows whose assignment changed (a few per cent of the rows after the first iterations) to per-warp
+//               lists, and the reduce phase subtracts such a row from its old cluster and adds it to its new one.
+//               Cluster k belongs to reduce warp k % 8, which walks the lists in a fixed order (warp segment, tile,
+//               row), 32 lanes = the 16 elements of A_k and of B_k; the CTA's sums [K][34] then go to global memory;
 //   (d) barrier among the nx CTAs of the group (integer arrive counter in global memory);
 //   (e) merge   CTA bx owns clusters k = bx, bx + nx, ...: it adds the nx partials in CTA order, applies Eq. 7 / Eq. 8
 //               with the safeguards of PAPER.md:178, stores s_k, g_k, the cluster's term of J, and the cluster's rows
 //               of the next pass's operand images;
 //   (f) barrier; Alg. 1 l.15-16: leave the loop when no assignment changed (t > 1).
 //
-// Every floating-point sum has a fixed order (bitmap-walk order within a cluster and batch, batch order, CTA order): same
+// Every floating-point sum has a fixed order (list order within a cluster, pass order, CTA order): same
 // inputs => same bits; there are no floating-point atomics (integer atomics: counters, max of a bit pattern, the
 // barrier).  TMEM, the mbarriers and the constant tile are set up once per fit instead of once per pass, and the
 // whole fit is one launch.
@@ -27,23 +29,23 @@
 namespace gsrq {
 namespace tc {
 
-constexpr int kFitBatch = 1024;                 // rows per reduction batch
 constexpr int kFitWarps = kThreads / 32;        // 10
 constexpr int kFitP = 2 * kD + 2;               // partial record: A[16] | B[16] | W | cnt
 // shared memory (offsets from the 1024-byte aligned base).  Phase (c) reuses the (idle) A ring for the staged rows.
 constexpr uint32_t kFitSmemOnes = 0;                                         // constant A_1 tile
-constexpr uint32_t kFitSmemA = kFitSmemOnes + kPlaneBytes;                   // ring of kStages x 2 planes | rows of a batch
+constexpr uint32_t kFitSmemA = kFitSmemOnes + kPlaneBytes;                   // ring of kStages x 2 planes | staging of the reduce warps
 constexpr uint32_t kFitSmemB = kFitSmemA + kStages * 2 * kPlaneBytes;        // 3 operand images
 constexpr uint32_t kFitSmemQ = kFitSmemB + 3 * kBImgBytes;                   // deferred exact re-scores
 constexpr uint32_t kFitSmemSh = kFitSmemQ + kQCap * 8 + 16;                  // fp32 codebook + gains
 constexpr uint32_t kFitSmemBar = kFitSmemSh + kN * kD * 4 + kN * 4;          // mbarriers, TMEM slot
-constexpr uint32_t kFitSmemBits = kFitSmemBar + 256;                         // bitmap [256][32] words
-constexpr uint32_t kFitSmemCoef = kFitSmemBits + kN * (kFitBatch / 32) * 4;  // [1024] {w_i, w_i/(||r_i||+eps)} fp64
-constexpr uint32_t kFitSmemFin = kFitSmemCoef + kFitBatch * 16;              // [20][34] fp64 merged sums of a chunk of clusters
-constexpr uint32_t kFitSmemMisc = kFitSmemFin + 2 * kFitWarps * kFitP * 8;   // flags
+constexpr uint32_t kFitSmemAcc = kFitSmemBar + 256;                          // [256][34] fp64: this CTA's sums per cluster (kept over the passes)
+constexpr uint32_t kFitSmemFin = kFitSmemAcc + kN * kFitP * 8;               // [20][34] fp64 merged sums of a chunk of clusters
+constexpr uint32_t kFitSmemMisc = kFitSmemFin + 2 * kFitWarps * kFitP * 8;   // flags, list lengths
 constexpr uint32_t kFitSmemTotal = kFitSmemMisc + 64 + 1024;                 // + alignment slack
-static_assert(kFitBatch * kD * 4 <= kStages * 2 * kPlaneBytes, "the staged rows of a batch reuse the A ring");
-static_assert(kFitSmemB % 1024 == 0 && kFitSmemBits % 16 == 0 && kFitSmemCoef % 16 == 0 && kFitSmemTotal <= 227 * 1024, "shared-memory budget / alignment");
+constexpr int kFitRedWarps = 8;                                              // reduce warps (= the epilogue warps); cluster k belongs to warp k % 8
+constexpr uint32_t kFitStageBytes = 32768 + 4096 + 16384;                    // staging buffer of the reduce phase: 256 x {row fp64, {w, w/(||r||+eps)}} + bitmaps [256][16] words
+static_assert(2 * kFitStageBytes <= kFitSmemBar - kFitSmemA, "the two staging buffers of the reduce phase are laid over the scoring-only buffers (A ring, operand images, queue, fp32 codebook)");
+static_assert(kFitSmemB % 1024 == 0 && kFitSmemAcc % 16 == 0 && kFitSmemTotal <= 227 * 1024, "shared-memory budget / alignment");
 
 struct FitTcParams {
   uint8_t *bimg;           // [G][3][8192] operand images of the codebook scored next (pass 0: written by k_init_ids)
@@ -66,6 +68,8 @@ struct FitTcParams {
   DevStats *st;            // [G] or nullptr
   double *term;            // [G][term_stride][256] per-cluster terms of J, or nullptr
   int term_stride;
+  uint2 *chg;              // [G][chg_stride_g] change lists: {row - r0, k_old | k_new << 8 | pending << 17}
+  long long chg_stride_g;  // >= 128 n_tiles + 512 nx
   double *part;            // [G][nx][256][34] per-CTA partials
   unsigned int *bar;       // [G] arrive counters of the group barrier (zero at launch)
   long long *clk;          // debug: [G][nx][16] cycles per phase (GSRQ_FIT_CLOCKS), or nullptr
@@ -100,22 +104,20 @@ k_fit_tc(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CUte
   auto empty_a = [&](int s) { return bar0 + 8u * (kStages + s); };
   auto tmem_full = [&](int b) { return bar0 + 8u * (2 * kStages + b); };
   auto tmem_empty = [&](int b) { return bar0 + 8u * (2 * kStages + 2 + b); };
-  const uint32_t rows_full = bar0 + 8u * (2 * kStages + 4);
   volatile uint32_t *tmem_slot = reinterpret_cast<volatile uint32_t *>(sgen + kFitSmemBar + 8 * (2 * kStages + 5));
   uint2 *queue = reinterpret_cast<uint2 *>(sgen + kFitSmemQ);
   unsigned int *qcnt = reinterpret_cast<unsigned int *>(sgen + kFitSmemQ + kQCap * 8);
   float *sh_g = reinterpret_cast<float *>(sgen + kFitSmemSh);
   float *ga_g = sh_g + kN * kD;
-  uint32_t *bits = reinterpret_cast<uint32_t *>(sgen + kFitSmemBits);
-  double2 *coef_s = reinterpret_cast<double2 *>(sgen + kFitSmemCoef);
+  double *acc_s = reinterpret_cast<double *>(sgen + kFitSmemAcc);
   double *fin_all = reinterpret_cast<double *>(sgen + kFitSmemFin);
   volatile long long *misc = reinterpret_cast<volatile long long *>(sgen + kFitSmemMisc);
+  volatile unsigned int *lcnt = reinterpret_cast<volatile unsigned int *>(sgen + kFitSmemMisc + 16);   // [8] entries in each warp's change list
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, tid = threadIdx.x;
 
   if (tid == 0) {
     for (int s = 0; s < kStages; ++s) { mbar_init(full_a(s), 1); mbar_init(empty_a(s), 1); }
     for (int b = 0; b < 2; ++b) { mbar_init(tmem_full(b), 1); mbar_init(tmem_empty(b), 4); }
-    mbar_init(rows_full, 1);
     fence_barrier_init();
   }
   // constant A_1 tile: columns 0,1,2 = 1.0 (bf16 0x3F80), rest 0
@@ -123,6 +125,7 @@ k_fit_tc(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CUte
     const int row = e >> 4, col = e & 15;
     *reinterpret_cast<uint16_t *>(sgen + kFitSmemOnes + sw32_off(row, col)) = (col < 3) ? 0x3F80 : 0;
   }
+  for (int e = tid; e < kN * kFitP; e += kThreads) acc_s[e] = 0.0;
   fence_proxy_async();
   if (warp == 1) tmem_alloc(smem_u32((const void *)tmem_slot), 512);
   tc_fence_before();
@@ -141,7 +144,9 @@ k_fit_tc(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CUte
   const int msh = ((p.M & (p.M - 1)) == 0) ? (31 - __clz(p.M)) : -1;
   const bool rows_bf16 = p.n_planes == 1;
   int tbase = 0;             // tiles this CTA has pushed through the pipeline in earlier passes (ring / accumulator phases)
-  unsigned int n_batches = 0;  // reduction batches so far (phase of rows_full)
+  // change lists: the CTA's region starts at entry 128 tb + 512 bx of the group's buffer, one segment per epilogue warp
+  const long long cap_w = (long long)(n_my / 2 + 2) * 32;
+  uint2 *chg_cta = p.chg + (long long)g * p.chg_stride_g + (long long)tb * kTileM + (long long)bx * 512;
   unsigned int epoch = 0;      // group barriers passed
 
   long long clk_last = p.clk ? clock64() : 0;
@@ -155,6 +160,7 @@ k_fit_tc(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CUte
   for (int t = p.t_begin; t <= p.t_end; ++t) {
     const int mode = (t == 0) ? 1 : 0;
     const int lloyd = (p.lloyd_override >= 0) ? p.lloyd_override : (t > 0 ? 1 : 0);
+    const bool first = (t == p.t_begin);   // the pass that adds every row; later passes move the changed rows only
     // ---------------- (a) operand images and fp32 codebook of the group -> shared memory ----------------
     if (!p.skip_scoring) {
       const uint4 *src = reinterpret_cast<const uint4 *>(p.bimg + (size_t)g * 3 * kBImgBytes);
@@ -207,7 +213,8 @@ k_fit_tc(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CUte
         const int q = warp & 3;        // TMEM lane quarter this warp may access
         const int wg = (warp - 2) >> 2;
         const float gm = (mode == 0) ? __int_as_float(stg ? __ldcg(&stg->gmax_bits[t]) : 0x7f7fffff) : 1.0f;
-        unsigned int n_changed = 0, n_refined = 0;
+        unsigned int n_changed = 0, n_refined = 0, lc = 0;
+        uint2 *seg = chg_cta + (long long)(warp - 2) * cap_w;
         for (int it = ((tbase & 1) == wg) ? 0 : 1; it < n_my; it += 2) {
           const int gt = tbase + it, buf = wg, bph = (gt >> 1) & 1;
           const long long row = (long long)(tb + it) * kTileM + q * 32 + lane;
@@ -252,7 +259,15 @@ k_fit_tc(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CUte
             n_changed += (k_old != (uint8_t)k_new);
             p.idx[gr] = (uint8_t)k_new;
           }
+          if (!first) {  // rows that (may) have moved: appended in row order; a queued row's new cluster is read back from idx later
+            const bool ch = (row < p.N) && (k_new < 0 || (uint8_t)k_new != k_old);
+            const unsigned int cm = __ballot_sync(0xffffffffu, ch);
+            if (ch) seg[lc + __popc(cm & ((1u << lane) - 1u))] =
+                make_uint2((uint32_t)(row - r0), (uint32_t)k_old | ((uint32_t)(k_new < 0 ? 0 : k_new) << 8) | (k_new < 0 ? (1u << 17) : 0u));
+            lc += __popc(cm);
+          }
         }
+        if (lane == 0) lcnt[warp - 2] = lc;
         // deferred exact re-scores: entry e is taken by epilogue warp e % 8
         asm volatile("bar.sync 1, 256;" ::: "memory");
         {
@@ -278,130 +293,158 @@ k_fit_tc(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CUte
     }
     clk_mark(1);
 
-    // ---------------- (c) reduction over my rows, batches of kFitBatch ----------------
-    {
-      uint8_t *rows_s = sgen + kFitSmemA;   // the staged rows of the batch reuse the (idle) A ring
+    // ---------------- (c) this CTA's sums per cluster: add every row (first pass) or move the changed rows ----------------
+    // Operations come in batches of 256 list entries, one per thread of warps 2-9.  Fetch (two batches / one batch ahead,
+    // into registers): the entry, then its row, weights and -- first pass / queued rows -- its cluster.  Park (staging
+    // buffer b & 1, laid over the scoring-only shared memory): the row widened to fp64 (the fp32 -> fp64 conversion runs
+    // at 1/8 rate, so it is done once per entry here, not once per use), {w_i, w_i/(||r_i||+eps)}, and one bit per
+    // operation in the bitmap row of the cluster it leaves / joins (integer atomicOr: order-free).  Walk: thread k owns
+    // cluster k; it loads the cluster's 34 sums into registers, visits the set bits of its bitmap row in order
+    // (leaving rows, then joining rows; entry order within each) and stores the sums back after the last batch.
+    if (warp >= 2) {
+      const int j = tid - 64;    // entry of the batch this thread fetches and parks; also the cluster it owns
       const uint8_t *ig = p.idx + (long long)g * p.N;
-      // thread k owns cluster k: its sums live in registers for the whole phase
-      double accA[kD], accB[kD], accW = 0.0;
-      int cnt = 0;
+      unsigned int pre[kFitRedWarps + 1];   // prefix sums of the list lengths
+      pre[0] = 0;
 #pragma unroll
-      for (int e = 0; e < kD; ++e) { accA[e] = 0.0; accB[e] = 0.0; }
-      // Batch pipeline: the coefficients of batch b + 1 are fetched into registers while batch b is added up; the
-      // walk clears the bitmap words it consumes, so the bitmap is clean again when the next batch builds its own.
-      constexpr int kCoefPer = (kFitBatch + kThreads - 1) / kThreads;   // 4 rows per thread
-      float cw[kCoefPer];
-      double cn[kCoefPer];
-      uint32_t k8[2];   // the 8 assignment bytes of rows 8 tid .. 8 tid + 7 of the batch
-      auto fetch_coef = [&](long long b0, int nb) {
+      for (int q = 0; q < kFitRedWarps; ++q) pre[q + 1] = pre[q] + (first ? 0u : lcnt[q]);
+      const long long n_tot = first ? (r1 - r0) : (long long)pre[kFitRedWarps];
+      const int nbat = (int)((n_tot + 255) / 256);
+      if (p.clk && tid == 64) { p.clk[((long long)g * nx + bx) * 16 + 6] += n_tot; p.clk[((long long)g * nx + bx) * 16 + 7] += nbat; }
+      auto buf_xd = [&](int b) { return reinterpret_cast<double2 *>(sgen + kFitSmemA + (b & 1) * kFitStageBytes); };              // [256][8] double2
+      auto buf_cs = [&](int b) { return reinterpret_cast<double2 *>(sgen + kFitSmemA + (b & 1) * kFitStageBytes + 32768); };      // [256] {w, wn}
+      auto buf_bm = [&](int b) { return reinterpret_cast<uint32_t *>(sgen + kFitSmemA + (b & 1) * kFitStageBytes + 36864); };     // [256][16]: 8 words "leaves", 8 words "joins"
+      // entry: x = row - r0, y = k_old | k_new << 8 | pending << 17 (nothing here may consume the loaded value: it is still in flight)
+      auto valid_entry = [&](int b) -> bool { return (long long)b * 256 + j < n_tot; };
+      auto load_entry = [&](int b) -> uint2 {
+        const long long f = (long long)b * 256 + j;
+        if (f >= n_tot) return make_uint2(0u, 0u);
+        if (first) return make_uint2((uint32_t)f, (1u << 17));
+        int q = 0;
+        unsigned int base = 0;
 #pragma unroll
-        for (int u = 0; u < kCoefPer; ++u) {
-          const int e = tid + u * kThreads;
-          cw[u] = 0.0f; cn[u] = 0.0;
-          if (e < nb) {
-            const long long gr_ = b0 + e;
-            const long long tk_ = (msh >= 0) ? (gr_ >> msh) : (gr_ / p.M);
-            cw[u] = p.wt[(long long)g * p.nf_tok + tk_];
-            cn[u] = p.wn[(long long)g * p.N + gr_];
-          }
-        }
-        k8[0] = 0; k8[1] = 0;
-        if (8 * tid < nb) {
-          const uint8_t *ip = ig + b0 + 8 * tid;
-          if (((reinterpret_cast<uintptr_t>(ip) & 7) == 0) && 8 * tid + 8 <= nb) {
-            const uint2 v = *reinterpret_cast<const uint2 *>(ip);
-            k8[0] = v.x; k8[1] = v.y;
-          } else {
-#pragma unroll
-            for (int j = 0; j < 8; ++j)
-              if (8 * tid + j < nb) k8[j >> 2] |= (uint32_t)ip[j] << (8 * (j & 3));
-          }
-        }
+        for (int u = 1; u < kFitRedWarps; ++u)
+          if (f >= (long long)pre[u]) { q = u; base = pre[u]; }
+        return __ldcg(chg_cta + (long long)q * cap_w + (f - (long long)base));
       };
-      for (int e = tid; e < kN * (kFitBatch / 32) / 4; e += kThreads) reinterpret_cast<uint4 *>(bits)[e] = make_uint4(0, 0, 0, 0);
-      if (r0 < r1) fetch_coef(r0, (int)min((long long)kFitBatch, r1 - r0));
-      __syncthreads();
-      for (long long b0 = r0; b0 < r1; b0 += kFitBatch) {
-        const int nb = (int)min((long long)kFitBatch, r1 - b0);
-        const uint32_t row_bytes = rows_bf16 ? 32u : 64u;
-        if (tid == 0) {
-          mbar_expect_tx(rows_full, (uint32_t)nb * row_bytes);
-          const uint8_t *src = rows_bf16 ? reinterpret_cast<const uint8_t *>(p.ahi) + ((long long)g * p.N + b0) * 32
-                                         : reinterpret_cast<const uint8_t *>(p.rows) + ((long long)g * p.N + b0) * 64;
-          bulk_g2s(smem_u32(rows_s), src, (uint32_t)nb * row_bytes, rows_full);
+      uint4 xr[4];
+      float wv = 0.f;
+      double wnv = 0.0;
+      int knv = 0;
+      auto load_data = [&](const uint2 e, bool valid) {
+        if (!valid) return;
+        const long long rr = r0 + e.x, gr_ = (long long)g * p.N + rr;
+        if (rows_bf16) {
+          xr[0] = __ldg(reinterpret_cast<const uint4 *>(p.ahi + gr_ * kD));
+          xr[1] = __ldg(reinterpret_cast<const uint4 *>(p.ahi + gr_ * kD) + 1);
+        } else {
+#pragma unroll
+          for (int q4 = 0; q4 < 4; ++q4) xr[q4] = __ldg(reinterpret_cast<const uint4 *>(p.rows + gr_ * kD) + q4);
         }
+        const long long tk_ = (msh >= 0) ? (rr >> msh) : (rr / p.M);
+        wv = __ldg(p.wt + (long long)g * p.nf_tok + tk_);
+        wnv = __ldg(p.wn + gr_);
+        knv = (e.y & (1u << 17)) ? (int)__ldcg(ig + rr) : (int)((e.y >> 8) & 255u);
+      };
+      auto park = [&](int b, const uint2 e, bool valid) {
+        if (!valid) return;
+        const uint32_t ko = e.y & 255u;
+        if (!first && (uint32_t)knv == ko) return;   // a queued row that stayed where it was
+        float x[kD];
+        if (rows_bf16) {
+          const uint32_t u[8] = {xr[0].x, xr[0].y, xr[0].z, xr[0].w, xr[1].x, xr[1].y, xr[1].z, xr[1].w};
 #pragma unroll
-        for (int u = 0; u < kCoefPer; ++u) {   // per-row coefficients {w_i, w_i / (||r_i|| + eps)} of this batch
-          const int e = tid + u * kThreads;
-          if (e < nb) coef_s[e] = make_double2((double)cw[u], cn[u]);
+          for (int q8 = 0; q8 < 8; ++q8) { x[2 * q8] = __uint_as_float(u[q8] << 16); x[2 * q8 + 1] = __uint_as_float(u[q8] & 0xFFFF0000u); }
+        } else {
+#pragma unroll
+          for (int q4 = 0; q4 < 4; ++q4) { x[4 * q4] = __uint_as_float(xr[q4].x); x[4 * q4 + 1] = __uint_as_float(xr[q4].y); x[4 * q4 + 2] = __uint_as_float(xr[q4].z); x[4 * q4 + 3] = __uint_as_float(xr[q4].w); }
         }
-        clk_mark(11);
-        // membership bitmap: thread j owns byte column j (rows 8j..8j+7) of every cluster's 128-byte row: no races
-        if (8 * tid < nb) {
-          uint8_t *bb = reinterpret_cast<uint8_t *>(bits);
+        double2 *xd = buf_xd(b) + j * 8;
 #pragma unroll
-          for (int j = 0; j < 8; ++j)
-            if (8 * tid + j < nb) bb[(int)((k8[j >> 2] >> (8 * (j & 3))) & 0xFFu) * (kFitBatch / 8) + tid] |= (uint8_t)(1u << j);
-        }
-        clk_mark(12);
-        if (b0 + kFitBatch < r1) fetch_coef(b0 + kFitBatch, (int)min((long long)kFitBatch, r1 - b0 - kFitBatch));   // in flight during the walk
-        clk_mark(13);
-        __syncthreads();
-        clk_mark(7);
-        mbar_wait(rows_full, n_batches & 1);
-        n_batches++;
-        clk_mark(8);
-        // thread k walks the non-empty words of cluster k's bitmap row (word j of the walk is (j + k) & 31: conflict-free, and
-        // a fixed function of k) and adds the rows it finds: the lanes of a warp advance through their own rows together
-        if (tid < p.K) {
-          uint32_t sm = 0;
+        for (int q8 = 0; q8 < 8; ++q8) xd[q8] = make_double2((double)x[2 * q8], (double)x[2 * q8 + 1]);
+        buf_cs(b)[j] = make_double2((double)wv, wnv);
+        uint32_t *bm = buf_bm(b);
+        if (!first) atomicOr(bm + ko * 16 + (j >> 5), 1u << (j & 31));
+        atomicOr(bm + (uint32_t)knv * 16 + 8 + (j >> 5), 1u << (j & 31));
+      };
+      // this thread's cluster: sums in registers, in 16-byte chunks ROTATED by the lane (slot q holds chunk (q + lane) & 7) so that
+      // the row reads of a warp (every lane another row, all lanes the same slot) fall into 8 different bank groups
+      double2 aA[8], aB[8];
+      double aW, aC;
+      {
+        const double2 *src = reinterpret_cast<const double2 *>(acc_s + j * kFitP);
 #pragma unroll
-          for (int j = 0; j < kFitBatch / 32; ++j) sm |= (bits[tid * (kFitBatch / 32) + ((j + tid) & 31)] != 0u) ? (1u << j) : 0u;
-          const int hf = lane & 1;   // odd lanes read the two 16-byte halves of a bf16 row in the other order: spreads the banks
-          while (sm) {
-            const int wi = ((__ffs(sm) - 1) + tid) & 31;
-            sm &= sm - 1;
-            uint32_t word = bits[tid * (kFitBatch / 32) + wi];
-            bits[tid * (kFitBatch / 32) + wi] = 0u;
-            while (word) {
-              const int pr = wi * 32 + (__ffs(word) - 1);
-              word &= word - 1;
-              const double2 cf = coef_s[pr];
-              float x[kD];
-              if (rows_bf16) {
-                const uint4 va = reinterpret_cast<const uint4 *>(rows_s)[pr * 2 + hf], vb = reinterpret_cast<const uint4 *>(rows_s)[pr * 2 + (hf ^ 1)];
-                const uint4 v0 = hf ? vb : va, v1 = hf ? va : vb;
-                const uint32_t u[8] = {v0.x, v0.y, v0.z, v0.w, v1.x, v1.y, v1.z, v1.w};
+        for (int q = 0; q < 8; ++q) { const int c = (q + lane) & 7; aA[q] = src[c]; aB[q] = src[8 + c]; }
+        aW = acc_s[j * kFitP + 2 * kD]; aC = acc_s[j * kFitP + 2 * kD + 1];
+      }
+      for (int e = j; e < 2 * 256 * 16; e += 256) reinterpret_cast<uint32_t *>(sgen + kFitSmemA + (e >> 12) * kFitStageBytes + 36864)[e & 4095] = 0u;
+      asm volatile("bar.sync 1, 256;" ::: "memory");
+      uint2 e_cur = load_entry(0), e_nxt = load_entry(1);
+      load_data(e_cur, valid_entry(0));
+      park(0, e_cur, valid_entry(0));
+      asm volatile("bar.sync 1, 256;" ::: "memory");
+      for (int b = 0; b < nbat; ++b) {
+        if (b + 1 < nbat) load_data(e_nxt, valid_entry(b + 1));   // batch b + 1: rows and weights in flight
+        const uint2 e_nn = (b + 2 < nbat) ? load_entry(b + 2) : make_uint2(0u, 0u);   // batch b + 2: its list entries
+        {
+          const double2 *xd = buf_xd(b);
+          const double2 *cs = buf_cs(b);
+          uint32_t *bm = buf_bm(b) + j * 16;
+          uint32_t nz = 0;   // non-empty words of my bitmap row: bits 0-7 "leaves", 8-15 "joins"
+          {
+            const uint4 w0 = reinterpret_cast<const uint4 *>(bm)[0], w1 = reinterpret_cast<const uint4 *>(bm)[1];
+            const uint4 w2 = reinterpret_cast<const uint4 *>(bm)[2], w3 = reinterpret_cast<const uint4 *>(bm)[3];
+            const uint32_t ww[16] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w, w2.x, w2.y, w2.z, w2.w, w3.x, w3.y, w3.z, w3.w};
 #pragma unroll
-                for (int e = 0; e < 8; ++e) { x[2 * e] = __uint_as_float(u[e] << 16); x[2 * e + 1] = __uint_as_float(u[e] & 0xFFFF0000u); }
-              } else {
-#pragma unroll
-                for (int q4 = 0; q4 < 4; ++q4) {
-                  const float4 v = reinterpret_cast<const float4 *>(rows_s)[pr * 4 + q4];
-                  x[4 * q4] = v.x; x[4 * q4 + 1] = v.y; x[4 * q4 + 2] = v.z; x[4 * q4 + 3] = v.w;
-                }
-              }
-#pragma unroll
-              for (int e = 0; e < kD; ++e) {
-                const double xd = (double)x[e];
-                accA[e] = fma(cf.x, xd, accA[e]);
-                accB[e] = fma(cf.y, xd, accB[e]);
-              }
-              accW += cf.x;
-              cnt += 1;
+            for (int q = 0; q < 16; ++q) nz |= (ww[q] != 0u) ? (1u << q) : 0u;
+          }
+          uint32_t word = 0;
+          int wi = 0;
+          for (;;) {
+            if (word == 0u) {
+              if (nz == 0u) break;
+              wi = __ffs(nz) - 1;
+              nz &= nz - 1;
+              word = bm[wi];
+              bm[wi] = 0u;   // the bitmap is clean again for the batch after next
             }
+            const int e = (wi & 7) * 32 + (__ffs(word) - 1);
+            word &= word - 1;
+            double2 c2 = cs[e];
+            if (wi < 8) { c2.x = -c2.x; c2.y = -c2.y; }
+            const double2 *xe = xd + e * 8;
+            double2 xv[8];   // all eight loads in flight before the first use (the compiler would otherwise chain them through one register quad)
+#pragma unroll
+            for (int q = 0; q < 8; ++q) xv[q] = xe[(q + lane) & 7];
+            asm volatile("" ::: "memory");
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+              aA[q].x = fma(c2.x, xv[q].x, aA[q].x); aA[q].y = fma(c2.x, xv[q].y, aA[q].y);
+              aB[q].x = fma(c2.y, xv[q].x, aB[q].x); aB[q].y = fma(c2.y, xv[q].y, aB[q].y);
+            }
+            aW += c2.x;
+            aC += (wi < 8) ? -1.0 : 1.0;
           }
         }
-        __syncthreads();
-        clk_mark(10);
+        if (b + 1 < nbat) park(b + 1, e_nxt, valid_entry(b + 1));
+        e_nxt = e_nn;
+        asm volatile("bar.sync 1, 256;" ::: "memory");
       }
-      // publish this CTA's partials: record k = A[16] | B[16] | W | cnt
-      if (tid < kN) {
-        double2 *pk = reinterpret_cast<double2 *>(p.part + (((long long)g * nx + bx) * kN + tid) * kFitP);
+      {
+        double2 *dst = reinterpret_cast<double2 *>(acc_s + j * kFitP);
 #pragma unroll
-        for (int e = 0; e < kD / 2; ++e) { pk[e] = make_double2(accA[2 * e], accA[2 * e + 1]); pk[kD / 2 + e] = make_double2(accB[2 * e], accB[2 * e + 1]); }
-        pk[kD] = make_double2(accW, (double)cnt);
+        for (int q = 0; q < 8; ++q) { const int c = (q + lane) & 7; dst[c] = aA[q]; dst[8 + c] = aB[q]; }
+        acc_s[j * kFitP + 2 * kD] = aW; acc_s[j * kFitP + 2 * kD + 1] = aC;
       }
+      fence_proxy_async();   // generic-proxy use of the scoring buffers ends here; the next pass's TMA / tensor core use them again
+    }
+    __syncthreads();
+    if (p.clk && tid == 0 && first) p.clk[((long long)g * nx + bx) * 16 + 8] += clock64() - clk_last;
+    // publish this CTA's sums: record k = A[16] | B[16] | W | cnt
+    {
+      double2 *dst = reinterpret_cast<double2 *>(p.part + ((long long)g * nx + bx) * kN * kFitP);
+      const double2 *src = reinterpret_cast<const double2 *>(acc_s);
+      for (int e = tid; e < kN * kFitP / 2; e += kThreads) dst[e] = src[e];
     }
     clk_mark(2);
 
