@@ -15,6 +15,8 @@
 #include "k_score_tc.cuh"
 #include "k_fit_tc.cuh"
 #include "k_encode_tc.cuh"
+#include "k_wide.cuh"
+#include "k_score_tc_wide.cuh"
 
 namespace gsrq {
 
@@ -127,13 +129,15 @@ static Plan make_plan(const gsrq_view *v, int K, int S, long long n_fit_tokens) 
   return p;
 }
 
+static inline bool is_wide(int d) { return d == 64 || d == 128 || d == 256; }   // the paper's operating points (k_wide.cuh)
+
 static int check_view(const gsrq_view *v, int K, int S) {
   if (!v) { set_error("view is NULL"); return GSRQ_EINVAL; }
   if (v->dtype != GSRQ_F32 && v->dtype != GSRQ_BF16) { set_error("view.dtype must be GSRQ_F32 or GSRQ_BF16"); return GSRQ_EINVAL; }
   if (v->G <= 0 || v->T <= 0 || v->hd <= 0 || v->d <= 0 || v->hd % v->d) { set_error("bad view shape (G=%d T=%lld hd=%d d=%d)", v->G, (long long)v->T, v->hd, v->d); return GSRQ_EINVAL; }
   if (K <= 0 || K > GSRQ_MAX_K) { set_error("K must be in [1, %d], got %d", GSRQ_MAX_K, K); return GSRQ_EINVAL; }
   if (S <= 0 || S > GSRQ_MAX_STAGES) { set_error("S must be in [1, %d], got %d", GSRQ_MAX_STAGES, S); return GSRQ_EINVAL; }
-  if (v->d != 8 && v->d != 16 && v->d != 32) { set_error("d = %d: this build has kernels for d in {8, 16, 32}", v->d); return GSRQ_EUNSUPPORTED; }
+  if (v->d != 8 && v->d != 16 && v->d != 32 && !is_wide(v->d)) { set_error("d = %d: this build has kernels for d in {8, 16, 32, 64, 128, 256}", v->d); return GSRQ_EUNSUPPORTED; }
   const int al = (v->dtype == GSRQ_BF16) ? 8 : 4;  // 16-byte vector loads
   if (v->stride_g % al || v->stride_t % al) { set_error("strides must be multiples of %d elements (16-byte loads)", al); return GSRQ_EINVAL; }
   if ((long long)v->G * v->T * (v->hd / v->d) >= (1LL << 32)) { set_error("G*T*M must be < 2^32"); return GSRQ_EINVAL; }
@@ -459,9 +463,301 @@ static int run_encode_tc(const void *kv, const gsrq_view *v, const float *rows0,
   return GSRQ_OK;
 }
 
+
+// ======================================================================================================================
+// Wide sub-vectors (d = 64 / 128 / 256): exact fp64 kernels (k_wide.cuh) with the tcgen05 filter
+// (k_score_tc_wide.cuh) in front of the assignment for d = 64 / 128.  One launch per step, stage by stage (unfused).
+// ======================================================================================================================
+struct WPlan {
+  long long nf_tok, Nf, Nall, R, nE;   // R = rows the row-sized buffers hold
+  int M;
+  size_t off_st, off_cnt, off_rows, off_wt, off_wn, off_rnorm, off_idx, off_ids, off_epart, off_term, off_ahi, off_alo, off_bimg, off_gmax,
+      off_list, total;
+};
+
+static bool wide_tc(int d) { return (d == 64 || d == 128) && use_tc(tc::kD); }
+
+static WPlan make_wplan(const gsrq_view *v, long long n_fit_tokens) {
+  WPlan p;
+  p.M = v->hd / v->d;
+  p.nf_tok = (n_fit_tokens > 0) ? n_fit_tokens : (n_fit_tokens == 0 ? v->T : 0);
+  p.Nf = p.nf_tok * p.M;
+  p.Nall = v->T * p.M;
+  p.R = p.Nall;
+  p.nE = (p.R + 7) / 8;
+  const size_t G = (size_t)v->G, R = (size_t)p.R, d = (size_t)v->d;
+  const bool tcp = wide_tc(v->d);
+  size_t o = 0;
+  p.off_st = o;    o += align_up(G * sizeof(DevStats));
+  p.off_cnt = o;   o += align_up(kNumCounters * sizeof(unsigned int));
+  p.off_rows = o;  o += align_up(G * R * d * sizeof(float));
+  p.off_wt = o;    o += align_up(G * (size_t)v->T * sizeof(float));
+  p.off_wn = o;    o += align_up(G * R * sizeof(double));
+  p.off_rnorm = o; o += align_up(G * R * sizeof(float));
+  p.off_idx = o;   o += align_up(G * R);
+  p.off_ids = o;   o += align_up(G * GSRQ_MAX_K * sizeof(long long));
+  p.off_epart = o; o += align_up(G * (size_t)p.nE * sizeof(double));
+  p.off_term = o;  o += align_up(G * kTermStride * 256 * sizeof(double));
+  p.off_ahi = o;   o += align_up(tcp ? G * R * d * 2 : 0);
+  p.off_alo = o;   o += align_up(tcp ? G * R * d * 2 : 0);
+  p.off_bimg = o;  o += align_up(tcp ? G * (size_t)tc::wide_bimg_bytes<2>() : 0);
+  p.off_gmax = o;  o += align_up(G * sizeof(int));
+  p.off_list = o;  o += align_up(G * R * sizeof(uint32_t));
+  p.total = o;
+  return p;
+}
+
+static int make_wide_map(CUtensorMap *tm, const void *base, long long N, int G, int d) {
+  EncodeTiledFn fn = encode_tiled_fn();
+  if (!fn) { set_error("cuTensorMapEncodeTiled entry point not available"); return GSRQ_ECUDA; }
+  const cuuint64_t dims[3] = {(cuuint64_t)d, (cuuint64_t)N, (cuuint64_t)G};
+  const cuuint64_t strides[2] = {(cuuint64_t)d * 2, (cuuint64_t)N * d * 2};
+  const cuuint32_t box[3] = {64, (cuuint32_t)tc::kTileM, 1};
+  const cuuint32_t es[3] = {1, 1, 1};
+  CUresult r = fn(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void *>(base), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                  CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) { set_error("cuTensorMapEncodeTiled (wide plane) failed (%d)", (int)r); return GSRQ_ECUDA; }
+  return GSRQ_OK;
+}
+
+// gather (through fit_tokens) + per-row constants (+ operand planes) of N = nf_tok * M rows per group into the plan's row buffer
+static int wide_prep(const WPlan &pl, const gsrq_view *v, const RowSrc &src, const float *w, long long w_stride_g, const long long *fit_tokens,
+                     long long nf_tok, char *ws, bool planes, bool two_planes, bool energy, float *rows_out, cudaStream_t stream) {
+  wide::WPrepParams q{};
+  q.src = src; q.w = w; q.w_stride_g = w_stride_g; q.fit_tokens = fit_tokens; q.nf_tok = nf_tok;
+  q.Rf = rows_out; q.wt = (float *)(ws + pl.off_wt); q.wn = (double *)(ws + pl.off_wn);
+  q.rnorm = (float *)(ws + pl.off_rnorm);
+  q.epart = energy ? (double *)(ws + pl.off_epart) : nullptr;
+  q.ahi = planes ? (__nv_bfloat16 *)(ws + pl.off_ahi) : nullptr;
+  q.alo = (planes && two_planes) ? (__nv_bfloat16 *)(ws + pl.off_alo) : nullptr;
+  const long long N = nf_tok * src.M;
+  dim3 grid((unsigned)((N + 7) / 8), (unsigned)v->G);
+  LAUNCH(kClsPrep, stream, (wide::k_wide_prep<<<grid, 256, 0, stream>>>(q)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  return GSRQ_OK;
+}
+
+// One assignment pass over N rows per group (rows fp32 [G][N][d]) against a stage slice: tcgen05 filter + exact kernel on the
+// undecided rows (d = 64 / 128 with operand planes prepared), or the exact kernel on every row.
+static int wide_assign(const WPlan &pl, const gsrq_view *v, char *ws, const float *rows, long long N, const float *shapes_st, const float *gains_st,
+                       long long cb_stride_g, int K, int mode, bool use_filter, int n_planes, uint8_t *idx, DevStats *st, int slot,
+                       unsigned int *list_cnt, float *dbg, cudaStream_t stream) {
+  const int G = v->G, d = v->d;
+  wide::WAssignParams a{};
+  a.rows = rows; a.N = N; a.d = d; a.K = K; a.mode = mode; a.shapes = shapes_st; a.gains = gains_st; a.cb_stride_g = cb_stride_g;
+  a.idx = idx; a.idx16 = 0; a.st = st; a.slot = slot;
+  const size_t smem = wide::wide_assign_smem(d);
+  GSRQ_CUDA_CHECK(cudaFuncSetAttribute(wide::k_wide_assign, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  if (!use_filter) {
+    dim3 grid((unsigned)((N + wide::kWaRows - 1) / wide::kWaRows), (unsigned)G);
+    LAUNCH(kClsRefine, stream, (wide::k_wide_assign<<<grid, 256, smem, stream>>>(a)));
+    GSRQ_CUDA_CHECK(cudaGetLastError());
+    return GSRQ_OK;
+  }
+  uint8_t *bimg = (uint8_t *)(ws + pl.off_bimg);
+  int *gmax = (int *)(ws + pl.off_gmax);
+  uint32_t *list = (uint32_t *)(ws + pl.off_list);
+  GSRQ_CUDA_CHECK(cudaMemsetAsync(list_cnt, 0, sizeof(unsigned int), stream));
+  CUtensorMap tmh, tml;
+  int rc = make_wide_map(&tmh, ws + pl.off_ahi, N, G, d);
+  if (rc) return rc;
+  rc = make_wide_map(&tml, ws + (n_planes == 2 ? pl.off_alo : pl.off_ahi), N, G, d);
+  if (rc) return rc;
+  tc::ScoreWideParams p{};
+  p.bimg = bimg; p.gmax = gmax; p.rnorm = (const float *)(ws + pl.off_rnorm); p.gains = gains_st; p.cb_stride_g = cb_stride_g;
+  p.idx = idx; p.N = N; p.n_tiles = (int)((N + tc::kTileM - 1) / tc::kTileM); p.n_planes = n_planes; p.K = K; p.mode = (mode == wide::kModeProj) ? 1 : 0;
+  p.st = st; p.slot = slot; p.list = list; p.list_cnt = list_cnt; p.dbg = dbg;
+  const int n_sm = sm_count();
+  int ctas = n_sm / G; if (ctas < 1) ctas = 1; if (ctas > p.n_tiles) ctas = p.n_tiles;
+  const dim3 grid((unsigned)ctas, (unsigned)G);
+#define GSRQ_WIDE_TC(KB, DBG)                                                                                                                   \
+  do {                                                                                                                                          \
+    LAUNCH(kClsMisc, stream, (tc::k_bimg_wide<KB><<<G, 256, 0, stream>>>(shapes_st, gains_st, cb_stride_g, K, p.mode, bimg, gmax)));              \
+    GSRQ_CUDA_CHECK(cudaGetLastError());                                                                                                        \
+    GSRQ_CUDA_CHECK(cudaFuncSetAttribute(tc::k_score_tc_wide<KB, DBG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tc::WideSmem<KB>::kTotal)); \
+    LAUNCH(kClsScore, stream, (tc::k_score_tc_wide<KB, DBG><<<grid, tc::kThreads, tc::WideSmem<KB>::kTotal, stream>>>(tmh, tml, p)));             \
+  } while (0)
+  if (d == 128) { if (dbg) GSRQ_WIDE_TC(2, true); else GSRQ_WIDE_TC(2, false); }
+  else { if (dbg) GSRQ_WIDE_TC(1, true); else GSRQ_WIDE_TC(1, false); }
+#undef GSRQ_WIDE_TC
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  a.list = list; a.list_cnt = list_cnt;
+  // the list length is only known on the device: enough tiles for every row, most of them exit at once
+  dim3 gridl((unsigned)(((long long)G * N + wide::kWaRows - 1) / wide::kWaRows), 1);
+  LAUNCH(kClsRefine, stream, (wide::k_wide_assign<<<gridl, 256, smem, stream>>>(a)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  return GSRQ_OK;
+}
+
+static int wide_subtract(const WPlan &pl, const gsrq_view *v, char *ws, float *rows, long long N, const float *shapes_st, const float *gains_st,
+                         long long cb_stride_g, int K, const uint8_t *idx, uint8_t *codes, bool planes, cudaStream_t stream) {
+  wide::WSubParams q{};
+  q.rows = rows; q.N = N; q.d = v->d; q.K = K; q.shapes = shapes_st; q.gains = gains_st; q.cb_stride_g = cb_stride_g; q.idx = idx; q.codes = codes;
+  q.ahi = planes ? (__nv_bfloat16 *)(ws + pl.off_ahi) : nullptr; q.alo = planes ? (__nv_bfloat16 *)(ws + pl.off_alo) : nullptr;
+  q.rnorm = planes ? (float *)(ws + pl.off_rnorm) : nullptr;
+  dim3 grid((unsigned)((N + 7) / 8), (unsigned)v->G);
+  LAUNCH(kClsEncode, stream, (wide::k_wide_subtract<<<grid, 256, 0, stream>>>(q)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  return GSRQ_OK;
+}
+
+static int wide_update(const WPlan &pl, const gsrq_view *v, char *ws, const float *rows, long long N, long long nf_tok, const uint8_t *idx,
+                       float *shapes_st, float *gains_st, long long cb_stride_g, int K, int mode, DevStats *st, int t, cudaStream_t stream) {
+  wide::WUpdateParams u{};
+  u.rows = rows; u.wn = (const double *)(ws + pl.off_wn); u.wt = (const float *)(ws + pl.off_wt); u.nf_tok = nf_tok; u.M = pl.M;
+  u.idx = idx; u.idx16 = 0; u.N = N; u.d = v->d; u.K = K; u.shapes = shapes_st; u.gains = gains_st; u.cb_stride_g = cb_stride_g; u.mode = mode;
+  u.st = st; u.term = st ? (double *)(ws + pl.off_term) : nullptr; u.term_stride = kTermStride; u.term_k = 256; u.t = t; u.gmax = nullptr;
+  LAUNCH(kClsUpdate, stream, (wide::k_wide_update<<<dim3((unsigned)K, (unsigned)v->G), 256, 0, stream>>>(u)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  return GSRQ_OK;
+}
+
+// rows of the fit (gathered through fit_tokens; the stage's residual derived from kv + earlier stages when not given)
+static int wide_fit_rows(const WPlan &pl, const void *kv, const gsrq_view *v, const float *w, long long w_stride_g, const long long *fit_tokens,
+                         const gsrq_codebook *cb, int stage, const float *residual, char *ws, bool planes, int n_planes, cudaStream_t stream) {
+  float *Rf = (float *)(ws + pl.off_rows);
+  const bool derive = (!residual && stage > 0);
+  const int K = cb ? cb->K : 0, d = v->d;
+  int rc = wide_prep(pl, v, make_src(kv, v, residual, pl.Nall), w, w_stride_g, fit_tokens, pl.nf_tok, ws, planes && !derive, n_planes == 2, !derive, Rf, stream);
+  if (rc || !derive) return rc;
+  uint8_t *idx = (uint8_t *)(ws + pl.off_idx);
+  unsigned int *cnt = (unsigned int *)(ws + pl.off_cnt);
+  for (int s = 0; s < stage; ++s) {   // r = x - sum_{s < stage} c^(s)[a^(s)] on the compact rows, stage by stage (exact kernel: no planes yet)
+    const float *sh = cb->shapes + (size_t)s * K * d, *ga = cb->gains + (size_t)s * K;
+    rc = wide_assign(pl, v, ws, Rf, pl.Nf, sh, ga, (long long)cb->S * K, K, wide::kModeGskm, false, 2, idx, nullptr, 0, cnt + 200 + s, nullptr, stream);
+    if (rc) return rc;
+    rc = wide_subtract(pl, v, ws, Rf, pl.Nf, sh, ga, (long long)cb->S * K, K, idx, nullptr, false, stream);
+    if (rc) return rc;
+  }
+  GSRQ_CUDA_CHECK(cudaMemsetAsync(idx, 0, (size_t)v->G * pl.Nf, stream));
+  // per-row constants of the residual rows; weights come from the compact per-fit-token array written by the first pass
+  wide::WPrepParams q{};
+  q.src = make_src(nullptr, v, Rf, pl.Nf); q.w = (const float *)(ws + pl.off_wt); q.w_stride_g = pl.nf_tok; q.fit_tokens = nullptr; q.nf_tok = pl.nf_tok;
+  q.Rf = Rf; q.wt = (float *)(ws + pl.off_wt); q.wn = (double *)(ws + pl.off_wn); q.rnorm = (float *)(ws + pl.off_rnorm);
+  q.epart = (double *)(ws + pl.off_epart);
+  q.ahi = planes ? (__nv_bfloat16 *)(ws + pl.off_ahi) : nullptr; q.alo = (planes && n_planes == 2) ? (__nv_bfloat16 *)(ws + pl.off_alo) : nullptr;
+  dim3 grid((unsigned)((pl.Nf + 7) / 8), (unsigned)v->G);
+  LAUNCH(kClsPrep, stream, (wide::k_wide_prep<<<grid, 256, 0, stream>>>(q)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  return GSRQ_OK;
+}
+
+static int fit_stage_wide(const void *kv, const gsrq_view *view, const float *w, int64_t w_stride_g, const int64_t *fit_tokens, int64_t n_fit,
+                          gsrq_codebook *cb, int stage, const float *residual, int iters, uint64_t seed, gsrq_fit_stats *stats, void *workspace,
+                          size_t workspace_bytes, cudaStream_t stream) {
+  const WPlan pl = make_wplan(view, fit_tokens ? n_fit : 0);
+  if (pl.Nf < cb->K) { set_error("fewer fit rows (%lld) than codewords (%d)", pl.Nf, cb->K); return GSRQ_EDEGENERATE; }
+  int rc = check_ws(workspace, workspace_bytes, pl.total);
+  if (rc) return rc;
+  char *ws = (char *)workspace;
+  const int G = view->G, d = view->d, K = cb->K;
+  DevStats *st = (DevStats *)(ws + pl.off_st);
+  unsigned int *cnt = (unsigned int *)(ws + pl.off_cnt);
+  uint8_t *idx = (uint8_t *)(ws + pl.off_idx);
+  float *Rf = (float *)(ws + pl.off_rows);
+  GSRQ_CUDA_CHECK(cudaMemsetAsync(st, 0, (size_t)G * sizeof(DevStats), stream));
+  GSRQ_CUDA_CHECK(cudaMemsetAsync(cnt, 0, kNumCounters * sizeof(unsigned int), stream));
+  GSRQ_CUDA_CHECK(cudaMemsetAsync(idx, 0, (size_t)G * pl.Nf, stream));
+  const bool filter = wide_tc(d);
+  const int n_planes = (stage == 0 && !residual && view->dtype == GSRQ_BF16) ? 1 : 2;
+  rc = wide_fit_rows(pl, kv, view, w, w_stride_g, (const long long *)fit_tokens, cb, stage, residual, ws, filter, n_planes, stream);
+  if (rc) return rc;
+  float *shapes_st = cb->shapes + (size_t)stage * K * d;
+  float *gains_st = cb->gains + (size_t)stage * K;
+  const long long cb_stride_g = (long long)cb->S * K;
+  LAUNCH(kClsPrep, stream, (wide::k_wide_init<<<G, 512, (size_t)K * sizeof(long long), stream>>>(Rf, pl.Nf, d, K, G, stage, seed, (long long *)(ws + pl.off_ids), st,
+                                                                                                shapes_st, gains_st, cb_stride_g, 0)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  for (int t = 0; t <= iters; ++t) {   // t = 0: Alg. 1 l.2 (gains under the max-projection assignment); t >= 1: Lloyd iterations
+    rc = wide_assign(pl, view, ws, Rf, pl.Nf, shapes_st, gains_st, cb_stride_g, K, t == 0 ? wide::kModeProj : wide::kModeGskm, filter, n_planes, idx, st, t,
+                     cnt + (t % 128), nullptr, stream);
+    if (rc) return rc;
+    rc = wide_update(pl, view, ws, Rf, pl.Nf, pl.nf_tok, idx, shapes_st, gains_st, cb_stride_g, K, t > 0 ? 1 : 0, st, t, stream);
+    if (rc) return rc;
+    LAUNCH(kClsMisc, stream, (wide::k_wide_converged<<<(G + 255) / 256, 256, 0, stream>>>(st, G, t)));
+    GSRQ_CUDA_CHECK(cudaGetLastError());
+  }
+  if (!stats) return GSRQ_OK;
+  LAUNCH(kClsMisc, stream, (k_finish<<<G, 160, 0, stream>>>(st, (const double *)(ws + pl.off_term), kTermStride, K, (const double *)(ws + pl.off_epart),
+                                                            (int)((pl.Nf + 7) / 8), iters)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  return GSRQ_OK;   // the caller copies the statistics
+}
+
+static int encode_wide(const void *kv, const gsrq_view *view, const gsrq_codebook *cb, int stage_begin, int stage_end, uint8_t *codes,
+                       float *residual_out, void *workspace, size_t workspace_bytes, cudaStream_t stream) {
+  const WPlan pl = make_wplan(view, -1);
+  int rc = check_ws(workspace, workspace_bytes, pl.total);
+  if (rc) return rc;
+  char *ws = (char *)workspace;
+  const int G = view->G, d = view->d, K = cb->K;
+  const long long N = pl.Nall, cb_stride_g = (long long)cb->S * K;
+  unsigned int *cnt = (unsigned int *)(ws + pl.off_cnt);
+  float *R = residual_out ? residual_out : (float *)(ws + pl.off_rows);
+  const bool filter = wide_tc(d);
+  // the working residual: all rows of kv as fp32 (+ the bf16-exact operand plane when stage 0 is scored by the filter)
+  rc = wide_prep(pl, view, make_src(kv, view, nullptr, 0), nullptr, 0, nullptr, view->T, ws, filter && stage_begin == 0, view->dtype != GSRQ_BF16, false, R, stream);
+  if (rc) return rc;
+  for (int s = 0; s < stage_end; ++s) {
+    const float *sh = cb->shapes + (size_t)s * K * d, *ga = cb->gains + (size_t)s * K;
+    uint8_t *plane = codes + (size_t)s * G * N;
+    if (s >= stage_begin) {
+      const int n_planes = (s == 0 && view->dtype == GSRQ_BF16) ? 1 : 2;
+      rc = wide_assign(pl, view, ws, R, N, sh, ga, cb_stride_g, K, wide::kModeGskm, filter, n_planes, plane, nullptr, 0, cnt + 1 + (s % 64), nullptr, stream);
+      if (rc) return rc;
+    }
+    const bool need_res = (s + 1 < stage_end) || residual_out;
+    if (!need_res) break;
+    // planes of the new residual only when the next stage is scored by the filter
+    rc = wide_subtract(pl, view, ws, R, N, sh, ga, cb_stride_g, K, plane, nullptr, filter && s + 1 < stage_end && s + 1 >= stage_begin, stream);
+    if (rc) return rc;
+  }
+  return GSRQ_OK;
+}
+
+static int decode_wide(const uint8_t *codes, const gsrq_codebook *cb, int n_stages, void *kv_out, const gsrq_view *ov, cudaStream_t stream) {
+  wide::WDecParams p{};
+  p.codes = codes; p.shapes = cb->shapes; p.gains = cb->gains; p.S = cb->S; p.K = cb->K; p.G = ov->G; p.n_stages = n_stages; p.d = ov->d;
+  p.M = ov->hd / ov->d; p.N = ov->T * p.M; p.out = kv_out; p.dtype = ov->dtype; p.stride_g = ov->stride_g; p.stride_t = ov->stride_t;
+  dim3 grid((unsigned)((p.N + 7) / 8), (unsigned)ov->G);
+  LAUNCH(kClsDecode, stream, (wide::k_wide_decode<<<grid, 256, 0, stream>>>(p)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  return GSRQ_OK;
+}
+
 }  // namespace gsrq
 
 using namespace gsrq;
+
+// Copy the device statistics of a fit to the caller's host structs (synchronises the stream).
+static int copy_fit_stats(const DevStats *st, int G, gsrq_fit_stats *stats, cudaStream_t stream) {
+  {
+    DevStats *h = (DevStats *)malloc((size_t)G * sizeof(DevStats));
+    if (!h) { set_error("out of host memory"); return GSRQ_ECUDA; }
+    cudaError_t e = cudaMemcpyAsync(h, st, (size_t)G * sizeof(DevStats), cudaMemcpyDeviceToHost, stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+    if (e != cudaSuccess) { free(h); set_error("stats copy failed: %s", cudaGetErrorString(e)); return GSRQ_ECUDA; }
+    int degenerate = 0, lost = 0;
+    for (int g = 0; g < G; ++g) {
+      gsrq_fit_stats *o = stats + g;
+      memset(o, 0, sizeof(*o));
+      o->iters_run = h[g].iters_run;
+      o->n_refined = h[g].refined;
+      for (int t = 1; t <= h[g].iters_run; ++t) {
+        o->wdist_after_assign[t - 1] = h[g].J[t];
+        o->n_changed[t - 1] = h[g].changed[t];
+      }
+      o->n_empty_last = h[g].n_empty[h[g].iters_run];
+      o->n_changed_last = h[g].iters_run ? h[g].changed[h[g].iters_run] : 0;
+      degenerate |= (h[g].err == GSRQ_EDEGENERATE);
+      lost |= (h[g].err != 0 && h[g].err != GSRQ_EDEGENERATE);
+    }
+    free(h);
+    if (lost) { set_error("the fit kernel's group barrier timed out"); return GSRQ_ECUDA; }
+    if (degenerate) { set_error("a group has fewer than K distinct non-zero fit rows"); return GSRQ_EDEGENERATE; }
+  }
+  return GSRQ_OK;
+}
 
 extern "C" {
 
@@ -471,6 +767,7 @@ const char *gsrq_version(void) { return "gsrq-b200 0.1 (sm_100a)"; }
 size_t gsrq_workspace_bytes(const gsrq_view *view, int K, int S, int64_t n_fit_tokens) {
   if (check_view(view, K, S) != GSRQ_OK) return 0;
   if (n_fit_tokens > view->T) { set_error("n_fit_tokens > T"); return 0; }
+  if (is_wide(view->d)) return make_wplan(view, n_fit_tokens).total;
   return make_plan(view, K, S, n_fit_tokens).total;
 }
 
@@ -485,6 +782,11 @@ int gsrq_fit_stage(const void *kv, const gsrq_view *view, const float *w, int64_
   if (iters < 0 || iters > GSRQ_MAX_ITERS) { set_error("iters must be in [0, %d]", GSRQ_MAX_ITERS); return GSRQ_EINVAL; }
   if (fit_tokens && (n_fit <= 0 || n_fit > view->T)) { set_error("n_fit out of range"); return GSRQ_EINVAL; }
   if ((rc = check_align16(kv, "kv")) || (rc = check_align16(residual, "residual"))) return rc;
+  if (is_wide(view->d)) {
+    rc = fit_stage_wide(kv, view, w, w_stride_g, fit_tokens, n_fit, cb, stage, residual, iters, seed, stats, workspace, workspace_bytes, stream);
+    if (rc || !stats) return rc;
+    return copy_fit_stats((const DevStats *)((char *)workspace + make_wplan(view, fit_tokens ? n_fit : 0).off_st), view->G, stats, stream);
+  }
   const Plan pl = make_plan(view, cb->K, cb->S, fit_tokens ? n_fit : 0);
   if (pl.Nf < cb->K) { set_error("fewer fit rows (%lld) than codewords (%d)", pl.Nf, cb->K); return GSRQ_EDEGENERATE; }
   rc = check_ws(workspace, workspace_bytes, pl.total);
@@ -541,31 +843,7 @@ int gsrq_fit_stage(const void *kv, const gsrq_view *view, const float *w, int64_
                                                               (const double *)(ws + pl.off_epart), (int)pl.nE, iters)));
     GSRQ_CUDA_CHECK(cudaGetLastError());
   }
-  if (stats) {
-    DevStats *h = (DevStats *)malloc((size_t)G * sizeof(DevStats));
-    if (!h) { set_error("out of host memory"); return GSRQ_ECUDA; }
-    cudaError_t e = cudaMemcpyAsync(h, st, (size_t)G * sizeof(DevStats), cudaMemcpyDeviceToHost, stream);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
-    if (e != cudaSuccess) { free(h); set_error("stats copy failed: %s", cudaGetErrorString(e)); return GSRQ_ECUDA; }
-    int degenerate = 0, lost = 0;
-    for (int g = 0; g < G; ++g) {
-      gsrq_fit_stats *o = stats + g;
-      memset(o, 0, sizeof(*o));
-      o->iters_run = h[g].iters_run;
-      o->n_refined = h[g].refined;
-      for (int t = 1; t <= h[g].iters_run; ++t) {
-        o->wdist_after_assign[t - 1] = h[g].J[t];
-        o->n_changed[t - 1] = h[g].changed[t];
-      }
-      o->n_empty_last = h[g].n_empty[h[g].iters_run];
-      o->n_changed_last = h[g].iters_run ? h[g].changed[h[g].iters_run] : 0;
-      degenerate |= (h[g].err == GSRQ_EDEGENERATE);
-      lost |= (h[g].err != 0 && h[g].err != GSRQ_EDEGENERATE);
-    }
-    free(h);
-    if (lost) { set_error("the fit kernel's group barrier timed out"); return GSRQ_ECUDA; }
-    if (degenerate) { set_error("a group has fewer than K distinct non-zero fit rows"); return GSRQ_EDEGENERATE; }
-  }
+  if (stats) return copy_fit_stats(st, G, stats, stream);
   return GSRQ_OK;
 }
 
@@ -578,6 +856,7 @@ int gsrq_encode(const void *kv, const gsrq_view *view, const gsrq_codebook *cb, 
   if (rc) return rc;
   if (stage_begin < 0 || stage_end > cb->S || stage_begin >= stage_end) { set_error("bad stage range [%d, %d)", stage_begin, stage_end); return GSRQ_EINVAL; }
   if ((rc = check_align16(kv, "kv")) || (rc = check_align16(residual_out, "residual_out"))) return rc;
+  if (is_wide(view->d)) return encode_wide(kv, view, cb, stage_begin, stage_end, codes, residual_out, workspace, workspace_bytes, stream);
   const Plan pl = make_plan(view, cb->K, cb->S, -1);
   rc = check_ws(workspace, workspace_bytes, pl.encode_total);
   if (rc) return rc;
@@ -607,6 +886,7 @@ int gsrq_decode(const uint8_t *codes, const gsrq_codebook *cb, int n_stages, voi
   if (rc) return rc;
   if (n_stages < 0 || n_stages > cb->S) { set_error("n_stages %d out of [0, %d]", n_stages, cb->S); return GSRQ_EINVAL; }
   if ((rc = check_align16(kv_out, "kv_out"))) return rc;
+  if (is_wide(out_view->d)) return decode_wide(codes, cb, n_stages, kv_out, out_view, stream);
   const int d = out_view->d;
   DecParams p{};
   p.codes = codes; p.shapes = cb->shapes; p.gains = cb->gains; p.S = cb->S; p.K = cb->K; p.G = out_view->G;
@@ -682,6 +962,7 @@ int gsrq_encode_append(const void *kv_new, const gsrq_view *new_view, const gsrq
   if (!kv_new || !cb || !cb->shapes || !cb->gains || !codes) { set_error("NULL kv / codebook / codes"); return GSRQ_EINVAL; }
   int rc = check_view(new_view, cb->K, cb->S);
   if (rc) return rc;
+  if (is_wide(new_view->d)) { set_error("gsrq_encode_append: d = %d is not supported (use gsrq_encode)", new_view->d); return GSRQ_EUNSUPPORTED; }
   const int M = new_view->hd / new_view->d;
   if (n_stages < 1 || n_stages > cb->S) { set_error("n_stages %d out of [1, %d]", n_stages, cb->S); return GSRQ_EINVAL; }
   if ((rc = check_align16(kv_new, "kv_new"))) return rc;
@@ -706,6 +987,20 @@ static int assign_all_rows(const void *kv, const gsrq_view *view, const float *r
   if (rc) return rc;
   if (stage < 0 || stage >= cb->S || (mode != 0 && mode != 1)) { set_error("bad stage / mode"); return GSRQ_EINVAL; }
   if ((rc = check_align16(kv, "kv")) || (rc = check_align16(residual, "residual"))) return rc;
+  if (is_wide(view->d)) {
+    const WPlan wp = make_wplan(view, 0);
+    rc = check_ws(workspace, workspace_bytes, wp.total);
+    if (rc) return rc;
+    char *wsw = (char *)workspace;
+    const bool filter = wide_tc(view->d);
+    if (dbg && !filter) { set_error("score dump needs the tensor-core path (d == 16, 64, 128)"); return GSRQ_EUNSUPPORTED; }
+    const int n_planes = (!residual && view->dtype == GSRQ_BF16) ? 1 : 2;
+    float *Rf = (float *)(wsw + wp.off_rows);
+    rc = wide_prep(wp, view, make_src(kv, view, residual, wp.Nall), nullptr, 0, nullptr, view->T, wsw, filter, n_planes == 2, false, Rf, stream);
+    if (rc) return rc;
+    return wide_assign(wp, view, wsw, Rf, wp.Nall, cb->shapes + (size_t)stage * cb->K * view->d, cb->gains + (size_t)stage * cb->K, (long long)cb->S * cb->K,
+                       cb->K, mode == 1 ? wide::kModeProj : wide::kModeGskm, filter, n_planes, idx_out, nullptr, 0, (unsigned int *)(wsw + wp.off_cnt), dbg, stream);
+  }
   const Plan pl = make_plan(view, cb->K, cb->S, 0);
   rc = check_ws(workspace, workspace_bytes, pl.total);
   if (rc) return rc;
@@ -759,6 +1054,17 @@ int gsrq_update(const void *kv, const gsrq_view *view, const float *residual, co
   int rc = check_view(view, cb->K, cb->S);
   if (rc) return rc;
   if (stage < 0 || stage >= cb->S) { set_error("bad stage"); return GSRQ_EINVAL; }
+  if (is_wide(view->d)) {
+    const WPlan wp = make_wplan(view, 0);
+    rc = check_ws(workspace, workspace_bytes, wp.total);
+    if (rc) return rc;
+    char *wsw = (char *)workspace;
+    float *Rf = (float *)(wsw + wp.off_rows);
+    rc = wide_prep(wp, view, make_src(kv, view, residual, wp.Nall), w, w_stride_g, nullptr, view->T, wsw, false, false, false, Rf, stream);
+    if (rc) return rc;
+    return wide_update(wp, view, wsw, Rf, wp.Nall, view->T, idx, cb->shapes + (size_t)stage * cb->K * view->d, cb->gains + (size_t)stage * cb->K,
+                       (long long)cb->S * cb->K, cb->K, shapes_too ? 1 : 0, nullptr, 1, stream);
+  }
   const Plan pl = make_plan(view, cb->K, cb->S, 0);
   rc = check_ws(workspace, workspace_bytes, pl.total);
   if (rc) return rc;
@@ -782,6 +1088,22 @@ int gsrq_init_ids(const void *kv, const gsrq_view *view, const float *residual, 
   int rc = check_view(view, K, 1);
   if (rc) return rc;
   if (fit_tokens && (n_fit <= 0 || n_fit > view->T)) { set_error("n_fit out of range"); return GSRQ_EINVAL; }
+  if (is_wide(view->d)) {
+    const WPlan wp = make_wplan(view, fit_tokens ? n_fit : 0);
+    if (wp.Nf < K) { set_error("fewer fit rows than codewords"); return GSRQ_EDEGENERATE; }
+    rc = check_ws(workspace, workspace_bytes, wp.total);
+    if (rc) return rc;
+    char *wsw = (char *)workspace;
+    DevStats *stw = (DevStats *)(wsw + wp.off_st);
+    GSRQ_CUDA_CHECK(cudaMemsetAsync(stw, 0, (size_t)view->G * sizeof(DevStats), stream));
+    float *Rf = (float *)(wsw + wp.off_rows);
+    rc = wide_prep(wp, view, make_src(kv, view, residual, wp.Nall), nullptr, 0, (const long long *)fit_tokens, wp.nf_tok, wsw, false, false, false, Rf, stream);
+    if (rc) return rc;
+    LAUNCH(kClsPrep, stream, (wide::k_wide_init<<<view->G, 512, (size_t)K * sizeof(long long), stream>>>(Rf, wp.Nf, view->d, K, view->G, stage, seed, (long long *)ids_out, stw,
+                                                                                                      nullptr, nullptr, 0, 0)));
+    GSRQ_CUDA_CHECK(cudaGetLastError());
+    return GSRQ_OK;
+  }
   const Plan pl = make_plan(view, K, 1, fit_tokens ? n_fit : 0);
   if (pl.Nf < K) { set_error("fewer fit rows than codewords"); return GSRQ_EDEGENERATE; }
   rc = check_ws(workspace, workspace_bytes, pl.total);
@@ -918,7 +1240,8 @@ int gsrq_pipeline_host(const void *kv_host, const gsrq_view *view, const float *
   for (int s = 0; s < S && rc == GSRQ_OK && e == cudaSuccess; ++s) {
     rc = gsrq_fit_stage(d_kv, view, d_w, 0, d_ft, n_fit, &cb, s, (per_stage && s) ? d_res : nullptr, iters, seed, nullptr, d_ws, wsb, stream);
     if (rc == GSRQ_OK) {   // remember a failed initialisation (the stage's statistics are reset by the next fit)
-      k_collect_err<<<1, 128, 0, stream>>>((const DevStats *)((char *)d_ws + pl.off_st), G, d_err);
+      const size_t off_st = is_wide(d) ? make_wplan(view, fit_tokens_host ? n_fit : 0).off_st : pl.off_st;
+      k_collect_err<<<1, 128, 0, stream>>>((const DevStats *)((char *)d_ws + off_st), G, d_err);
       e = cudaGetLastError();
     }
     if (per_stage && rc == GSRQ_OK && e == cudaSuccess) {

@@ -1,0 +1,567 @@
+// k_wide.cuh -- the paper's own operating points: wide sub-vectors d = 64 / 128 / 256 (D = 128 with
+// R = 32 / 16 / 12 stages, D = 256 with R = 12; K = 256), and the textbook weighted K-means (KM) baseline of the Fig. 4
+// comparison (PAPER.md:60-85 section 4, :202-212) with up to 4096 centroids.  These kernels are exact by construction:
+//   k_wide_prep     gather the fit rows (warp per row), row norms in fp64, weights, bf16 operand planes for the
+//                   tensor-core filter (k_score_tc_wide.cuh)
+//   k_wide_init     seeded initial rows (Alg. 1 l.1; reading c-I), any d
+//   k_wide_assign   arg-max of Eq. 5 (or the plain projection, or the KM distance) in fp64 with the definition's own
+//                   operation order, for all rows or for the rows a filter could not decide
+//   k_wide_update   weighted cluster sums in fp64 in ascending row order (one CTA per cluster), Eq. 7 / Eq. 8 with the
+//                   safeguards of PAPER.md:178, or the KM centroid (weighted mean)
+//   k_wide_subtract r <- fl32(r - fl32(g_k s_k)) and the code byte (RQ); operand planes of the new residual
+//   k_wide_decode   xhat = sum of the stages' codewords in fp32 stage order (reading c-D)
+// No floating-point atomics; every sum has a fixed order.
+#pragma once
+#include "gsrq_common.cuh"
+
+namespace gsrq {
+namespace wide {
+
+constexpr int kMaxD = 256;
+constexpr int kMaxK = 4096;
+
+enum { kModeGskm = 0, kModeProj = 1, kModeKm = 2 };   // scoring rule of k_wide_assign
+
+// ---------------------------------------------------------------------------------------------------- prep
+struct WPrepParams {
+  RowSrc src;                  // kv (strided, bf16 / fp32) or fp32 rows [G][rows_per_group][d]
+  const float *w;              // [.][T] per-token weights or nullptr
+  long long w_stride_g;
+  const long long *fit_tokens; // [G][nf_tok] or nullptr
+  long long nf_tok;
+  float *Rf;                   // [G][Nf][d] compact fp32 rows (out; may alias src.rows when there is no gather)
+  float *wt;                   // [G][nf_tok]
+  double *wn;                  // [G][Nf] w_i / (||r_i|| + eps)
+  float *rnorm;                // [G][Nf] upper bound of ||r_i|| (fp32) or nullptr
+  double *epart;               // [G][gridDim.x] partials of sum w_i ||r_i||^2, or nullptr
+  __nv_bfloat16 *ahi, *alo;    // [G][Nf][d] bf16 operand planes or nullptr
+};
+
+// warp per row, 8 rows per CTA.  grid = (ceil(Nf / 8), G), block = 256.
+__global__ void __launch_bounds__(256) k_wide_prep(WPrepParams p) {
+  __shared__ double esh[8];
+  const int g = blockIdx.y, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int d = p.src.d;
+  const long long Nf = p.nf_tok * p.src.M;
+  const long long i = (long long)blockIdx.x * 8 + warp;
+  double e = 0.0;
+  if (i < Nf) {
+    const long long tl = i / p.src.M;
+    const int m = (int)(i - tl * p.src.M);
+    const long long tok = p.fit_tokens ? p.fit_tokens[(long long)g * p.nf_tok + tl] : tl;
+    const long long gi = (long long)g * Nf + i;
+    double n2 = 0.0;
+    for (int e0 = lane * 4; e0 < d; e0 += 128) {
+      float x[4];
+      if (p.src.rows) {
+        const float4 v = *reinterpret_cast<const float4 *>(p.src.rows + ((long long)g * p.src.rows_per_group + tok * p.src.M + m) * d + e0);
+        x[0] = v.x; x[1] = v.y; x[2] = v.z; x[3] = v.w;
+      } else if (p.src.dtype == GSRQ_BF16) {
+        const uint2 v = *reinterpret_cast<const uint2 *>(reinterpret_cast<const uint16_t *>(p.src.kv) + (long long)g * p.src.stride_g + tok * p.src.stride_t + (long long)m * d + e0);
+        x[0] = __uint_as_float(v.x << 16); x[1] = __uint_as_float(v.x & 0xFFFF0000u);
+        x[2] = __uint_as_float(v.y << 16); x[3] = __uint_as_float(v.y & 0xFFFF0000u);
+      } else {
+        const float4 v = *reinterpret_cast<const float4 *>(reinterpret_cast<const float *>(p.src.kv) + (long long)g * p.src.stride_g + tok * p.src.stride_t + (long long)m * d + e0);
+        x[0] = v.x; x[1] = v.y; x[2] = v.z; x[3] = v.w;
+      }
+      *reinterpret_cast<float4 *>(p.Rf + gi * d + e0) = make_float4(x[0], x[1], x[2], x[3]);
+#pragma unroll
+      for (int u = 0; u < 4; ++u) n2 = __dadd_rn(n2, __dmul_rn((double)x[u], (double)x[u]));
+      if (p.ahi) {
+        uint32_t h[2], l[2];
+#pragma unroll
+        for (int u = 0; u < 4; u += 2) {
+          const __nv_bfloat16 h0 = __float2bfloat16_rn(x[u]), h1 = __float2bfloat16_rn(x[u + 1]);
+          const __nv_bfloat16 l0 = __float2bfloat16_rn(__fsub_rn(x[u], __bfloat162float(h0)));
+          const __nv_bfloat16 l1 = __float2bfloat16_rn(__fsub_rn(x[u + 1], __bfloat162float(h1)));
+          h[u / 2] = (uint32_t)__bfloat16_as_ushort(h0) | ((uint32_t)__bfloat16_as_ushort(h1) << 16);
+          l[u / 2] = (uint32_t)__bfloat16_as_ushort(l0) | ((uint32_t)__bfloat16_as_ushort(l1) << 16);
+        }
+        *reinterpret_cast<uint2 *>(p.ahi + gi * d + e0) = make_uint2(h[0], h[1]);
+        if (p.alo) *reinterpret_cast<uint2 *>(p.alo + gi * d + e0) = make_uint2(l[0], l[1]);
+      }
+    }
+    for (int off = 16; off; off >>= 1) n2 += __shfl_xor_sync(0xffffffffu, n2, off);   // fixed tree: every lane ends with the same sum
+    const double n = sqrt(n2);
+    const float wv = p.w ? p.w[(long long)g * p.w_stride_g + tok] : 1.0f;
+    if (lane == 0) {
+      if (m == 0) p.wt[(long long)g * p.nf_tok + tl] = wv;
+      p.wn[gi] = (double)wv * (1.0 / (n + kEps));
+      if (p.rnorm) p.rnorm[gi] = (float)n * 1.000001f;
+    }
+    e = (double)wv * n2;
+  }
+  if (!p.epart) return;
+  if (lane == 0) esh[warp] = e;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double s = 0.0;
+    for (int q = 0; q < 8; ++q) s += esh[q];
+    p.epart[(long long)g * gridDim.x + blockIdx.x] = s;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------- init
+// Same candidate stream and acceptance rule as k_init_ids (k_prep.cuh), for any d.  grid = G, block = 512.
+// shapes == nullptr: ids only.  km: the initial centroids are the chosen rows themselves (not normalised), gains = 1.
+__global__ void __launch_bounds__(512) k_wide_init(const float *__restrict__ Rf, long long Nf, int d, int K, int G, int stage,
+                                                   uint64_t seed, long long *__restrict__ ids, DevStats *__restrict__ st,
+                                                   float *__restrict__ shapes, float *__restrict__ gains, long long cb_stride_g, int km) {
+  __shared__ long long cand[512];
+  __shared__ int ok[512];
+  __shared__ int scan[512];
+  __shared__ int n_chosen;
+  extern __shared__ long long chosen[];   // [K]
+  const int g = blockIdx.x, t = threadIdx.x;
+  const uint64_t sg = seed ^ (kGamma * (uint64_t)(1 + g + G * stage));
+  if (t == 0) n_chosen = 0;
+  __syncthreads();
+  const long long limit = 64LL * K + 4096;
+  for (long long base = 0; base < limit; base += 512) {
+    const long long n = base + t;
+    const long long c = (long long)(splitmix64_at(sg, (uint64_t)n) % (uint64_t)Nf);
+    int good = n < limit;
+    if (good) {
+      const float *x = Rf + ((long long)g * Nf + c) * d;
+      bool nz = false;
+      for (int j = 0; j < d; ++j) nz |= (x[j] != 0.0f);
+      good = nz;
+    }
+    cand[t] = c;
+    __syncthreads();
+    const int nc = n_chosen;
+    if (good) {
+      int dup = 0;
+      for (int q = 0; q < nc; ++q) dup |= (chosen[q] == c);
+      for (int q = 0; q < t; ++q) dup |= (cand[q] == c);
+      good = !dup;
+    }
+    ok[t] = good;
+    scan[t] = good;
+    __syncthreads();
+    for (int off = 1; off < 512; off <<= 1) {
+      const int v = (t >= off) ? scan[t - off] : 0;
+      __syncthreads();
+      scan[t] += v;
+      __syncthreads();
+    }
+    const int pos = nc + scan[t] - ok[t];
+    if (ok[t] && pos < K) chosen[pos] = c;
+    __syncthreads();
+    if (t == 0) n_chosen = min(K, nc + scan[511]);
+    __syncthreads();
+    if (n_chosen >= K) break;
+  }
+  const bool degenerate = n_chosen < K;
+  if (degenerate && t == 0) st[g].err = GSRQ_EDEGENERATE;
+  for (int k = t; k < K; k += 512) ids[(long long)g * K + k] = (k < n_chosen) ? chosen[k] : 0;
+  if (!shapes) return;
+  for (int k = t; k < K; k += 512) {
+    const float *x = Rf + ((long long)g * Nf + (k < n_chosen ? chosen[k] : 0)) * d;
+    float *s = shapes + ((long long)g * cb_stride_g + k) * d;
+    double n2 = 0.0;
+    for (int j = 0; j < d; ++j) n2 = __dadd_rn(n2, __dmul_rn((double)x[j], (double)x[j]));
+    const double n = sqrt(n2);
+    for (int j = 0; j < d; ++j) s[j] = km ? x[j] : ((n > 0.0) ? (float)((double)x[j] / n) : 0.0f);
+    gains[(long long)g * cb_stride_g + k] = km ? 1.0f : 0.0f;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------- assign
+struct WAssignParams {
+  const float *rows;      // [G][N][d] fp32
+  long long N;
+  int d, K, mode;         // kModeGskm / kModeProj / kModeKm
+  const float *shapes;    // stage slice: codeword k of group g at shapes + (g*cb_stride_g + k)*d   (KM: the centroid itself)
+  const float *gains;
+  long long cb_stride_g;
+  void *idx;              // [G][N] uint8 (idx16 == 0) or uint16
+  int idx16;
+  const uint32_t *list;   // rows to score: {g*N + i}, or nullptr = every row
+  const unsigned int *list_cnt;
+  DevStats *st;           // changed[slot] += rows whose assignment changed (nullptr: not counted)
+  int slot;
+  double *best_out;       // optional [G][N] best score (tests)
+};
+
+constexpr int kWaRows = 32, kWaCw = 32;   // tile: 32 rows x chunks of 32 codewords; block = 256
+
+__host__ __device__ inline size_t wide_assign_smem(int d) { return ((size_t)kWaRows * (d + 1) + (size_t)kWaCw * d) * sizeof(double) + kWaRows * 8 * 16; }
+
+// Exact arg-max, the oracle's arithmetic: dot = sum_j x_j s_kj in element order, products and sums rounded separately
+// (no FMA contraction); score = (2 g) dot - g g; lowest k wins ties (reading c-T).  KM: dist = sum_j (x_j - mu_kj)^2 in
+// element order, arg-MIN, lowest k on ties.  Thread (r = tid % 32, q = tid / 32) scores row r against codewords
+// 4 q .. 4 q + 3 of every 32-codeword chunk (ascending k), then the 8 threads of a row are merged in ascending q.
+// grid = (ceil(n_rows / 32), G or 1 with a list), block = 256, dynamic smem = wide_assign_smem(d).
+__global__ void __launch_bounds__(256) k_wide_assign(WAssignParams p) {
+  extern __shared__ __align__(16) double wsm[];
+  const int d = p.d;
+  double *xs = wsm;                       // [32][d + 1]
+  double *cw = xs + kWaRows * (d + 1);    // [32][d]
+  double *mb = cw + kWaCw * d;            // [32][8] best scores
+  int *mk = reinterpret_cast<int *>(mb + kWaRows * 8);   // [32][8] best indices
+  const int tid = threadIdx.x, r = tid & 31, q = tid >> 5;
+  long long n_rows = p.N;
+  int g = blockIdx.y;
+  if (p.list) n_rows = (long long)*p.list_cnt;
+  else if (group_done(p.st, g, p.slot)) return;
+  const long long t0 = (long long)blockIdx.x * kWaRows;
+  if (t0 >= n_rows) return;
+  // global row of my tile row (list mode: rows of any group)
+  long long grow = -1;
+  if (t0 + r < n_rows) grow = p.list ? (long long)p.list[t0 + r] : (long long)g * p.N + t0 + r;
+  // stage the tile's rows as fp64: warp q converts rows q, q + 8, ...
+  for (int rr = q; rr < kWaRows; rr += 8) {
+    const long long gr = (t0 + rr < n_rows) ? (p.list ? (long long)p.list[t0 + rr] : (long long)g * p.N + t0 + rr) : -1;
+    for (int j = r; j < d; j += 32) xs[rr * (d + 1) + j] = (gr >= 0) ? (double)p.rows[gr * d + j] : 0.0;
+  }
+  const int my_g = (grow >= 0) ? (int)(grow / p.N) : 0;   // list mode: the row's group
+  // list mode mixes groups in one tile: each thread reads codewords of ITS row's group, so the codeword chunk in shared
+  // memory is only used when the whole tile is one group
+  bool uniform = !p.list;
+  if (p.list) {
+    const int g0 = (int)((long long)p.list[t0] / p.N);
+    const int g1 = (int)((long long)p.list[min(t0 + kWaRows, n_rows) - 1] / p.N);   // the list is not sorted: check every row
+    int same = (grow < 0) || (my_g == g0);
+    same = __syncthreads_and(same);
+    uniform = same && (g0 == g1);
+    g = g0;
+  }
+  double best = (p.mode == kModeKm) ? INFINITY : -INFINITY;
+  int bk = 0x7fffffff;
+  __syncthreads();
+  for (int k0 = 0; k0 < p.K; k0 += kWaCw) {
+    if (uniform) {
+      __syncthreads();
+      for (int e = tid; e < kWaCw * d; e += 256) {
+        const int kk = k0 + e / d;
+        cw[e] = (kk < p.K) ? (double)p.shapes[((long long)g * p.cb_stride_g + kk) * d + (e % d)] : 0.0;
+      }
+      __syncthreads();
+    }
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};
+    const double *xr = xs + r * (d + 1);
+    if (uniform) {
+      const double *c0 = cw + (4 * q) * d;
+      for (int j = 0; j < d; ++j) {
+        const double x = xr[j];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const double c = c0[u * d + j];
+          if (p.mode == kModeKm) { const double e = __dsub_rn(x, c); acc[u] = __dadd_rn(acc[u], __dmul_rn(e, e)); }
+          else acc[u] = __dadd_rn(acc[u], __dmul_rn(x, c));
+        }
+      }
+    } else if (grow >= 0) {
+      for (int u = 0; u < 4; ++u) {
+        const int kk = k0 + 4 * q + u;
+        if (kk >= p.K) break;
+        const float *c0 = p.shapes + ((long long)my_g * p.cb_stride_g + kk) * d;
+        double a = 0.0;
+        for (int j = 0; j < d; ++j) {
+          const double x = xr[j], c = (double)c0[j];
+          if (p.mode == kModeKm) { const double e = __dsub_rn(x, c); a = __dadd_rn(a, __dmul_rn(e, e)); }
+          else a = __dadd_rn(a, __dmul_rn(x, c));
+        }
+        acc[u] = a;
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int kk = k0 + 4 * q + u;
+      if (kk >= p.K) continue;
+      double sc = acc[u];
+      if (p.mode == kModeGskm) {
+        const double gk = (double)p.gains[(long long)(uniform ? g : my_g) * p.cb_stride_g + kk];
+        sc = __dsub_rn(__dmul_rn(__dmul_rn(2.0, gk), acc[u]), __dmul_rn(gk, gk));
+      }
+      const bool better = (p.mode == kModeKm) ? (sc < best) : (sc > best);
+      if (better) { best = sc; bk = kk; }   // ascending k within the thread: strict comparison keeps the lowest index
+    }
+  }
+  mb[r * 8 + q] = best;
+  mk[r * 8 + q] = bk;
+  __syncthreads();
+  if (q == 0 && grow >= 0) {
+    double b = mb[r * 8];
+    int k = mk[r * 8];
+    for (int u = 1; u < 8; ++u) {
+      const double ob = mb[r * 8 + u];
+      const int ok_ = mk[r * 8 + u];
+      const bool better = (p.mode == kModeKm) ? (ob < b) : (ob > b);
+      if (better || (ob == b && ok_ < k)) { b = ob; k = ok_; }
+    }
+    if (k == 0x7fffffff) k = 0;
+    int old;
+    if (p.idx16) { uint16_t *ip = reinterpret_cast<uint16_t *>(p.idx) + grow; old = *ip; *ip = (uint16_t)k; }
+    else { uint8_t *ip = reinterpret_cast<uint8_t *>(p.idx) + grow; old = *ip; *ip = (uint8_t)k; }
+    if (p.best_out) p.best_out[grow] = b;
+    if (p.st && old != k) atomicAdd(reinterpret_cast<unsigned long long *>(&p.st[(int)(grow / p.N)].changed[p.slot]), 1ull);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------- update
+struct WUpdateParams {
+  const float *rows;      // [G][N][d]
+  const double *wn;       // [G][N]
+  const float *wt;        // [G][nf_tok]
+  long long nf_tok;
+  int M;
+  const void *idx;        // [G][N] uint8 / uint16
+  int idx16;
+  long long N;
+  int d, K;
+  float *shapes, *gains;  // stage slice
+  long long cb_stride_g;
+  int mode;               // 0: gains only (Alg. 1 l.2); 1: shapes + gains (Eq. 7, Eq. 8); 2: KM centroid = weighted mean
+  DevStats *st;           // or nullptr
+  double *term;           // [G][term_stride][term_k] per-cluster terms of J, or nullptr
+  int term_stride, term_k;
+  int t;
+  int *gmax;              // optional [G]: bit pattern of max_k g_k after this update (atomicMax on an int), for the tensor-core filter
+};
+
+// One CTA per (cluster, group): scan the group's assignment, collect the cluster's rows in ascending order, add them up in
+// fp64 in that order (thread = element: A_e for e < d, B_e for the next d values), then Eq. 7 / Eq. 8.
+// grid = (K, G), block = 256.
+__global__ void __launch_bounds__(256) k_wide_update(WUpdateParams p) {
+  __shared__ long long rowq[4096];
+  __shared__ int wcnt[8];
+  __shared__ double fin[2 * kMaxD + 2];
+  __shared__ double red[256];
+  const int k = blockIdx.x, g = blockIdx.y, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  if (group_done(p.st, g, p.t)) return;
+  const int d = p.d;
+  const int nq = (2 * d + 255) / 256;   // values per thread
+  double acc[2] = {0.0, 0.0};
+  double accW = 0.0;
+  long long cnt = 0;
+  const float *rows_g = p.rows + (long long)g * p.N * d;
+  for (long long c0 = 0; c0 < p.N; c0 += 4096) {
+    // ordered compaction of the matching rows of [c0, c0 + 4096): thread t looks at rows c0 + 16 t .. + 15
+    int my[16], nm = 0;
+    const long long b0 = c0 + 16LL * tid;
+#pragma unroll
+    for (int u = 0; u < 16; ++u) {
+      const long long i = b0 + u;
+      int v = -1;
+      if (i < p.N) v = p.idx16 ? (int)reinterpret_cast<const uint16_t *>(p.idx)[(long long)g * p.N + i] : (int)reinterpret_cast<const uint8_t *>(p.idx)[(long long)g * p.N + i];
+      my[u] = (v == k);
+      nm += my[u];
+    }
+    int incl = nm;
+    for (int off = 1; off < 32; off <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, off); if (lane >= off) incl += v; }
+    if (lane == 31) wcnt[warp] = incl;
+    __syncthreads();
+    int base = 0, total = 0;
+    for (int w8 = 0; w8 < 8; ++w8) { if (w8 < warp) base += wcnt[w8]; total += wcnt[w8]; }
+    int pos = base + incl - nm;
+#pragma unroll
+    for (int u = 0; u < 16; ++u) if (my[u]) rowq[pos++] = b0 + u;
+    __syncthreads();
+    // add the rows in order; 4 rows in flight
+    for (int r0 = 0; r0 < total; r0 += 4) {
+      float xv[4][2];
+      double cf[4][2];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        if (r0 + u < total) {
+          const long long i = rowq[r0 + u];
+          const double wv = (double)__ldg(p.wt + (long long)g * p.nf_tok + i / p.M), wnv = __ldg(p.wn + (long long)g * p.N + i);
+#pragma unroll
+          for (int q = 0; q < 2; ++q) {
+            const int v = tid + 256 * q;
+            xv[u][q] = (q < nq && v < 2 * d) ? __ldg(rows_g + i * d + (v < d ? v : v - d)) : 0.0f;
+            cf[u][q] = (v < d) ? wv : wnv;
+          }
+          if (tid == 0) accW += wv;
+        } else {
+#pragma unroll
+          for (int q = 0; q < 2; ++q) { xv[u][q] = 0.0f; cf[u][q] = 0.0; }
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u)
+#pragma unroll
+        for (int q = 0; q < 2; ++q) acc[q] = fma(cf[u][q], (double)xv[u][q], acc[q]);
+    }
+    cnt += total;
+    __syncthreads();
+  }
+#pragma unroll
+  for (int q = 0; q < 2; ++q) { const int v = tid + 256 * q; if (q < nq && v < 2 * d) fin[v] = acc[q]; }
+  if (tid == 0) { fin[2 * d] = accW; fin[2 * d + 1] = (double)cnt; }
+  __syncthreads();
+  // block-wide sums in a fixed tree order
+  auto block_sum = [&](double v) -> double {
+    red[tid] = v;
+    __syncthreads();
+    for (int s = 128; s > 0; s >>= 1) { if (tid < s) red[tid] += red[tid + s]; __syncthreads(); }
+    const double r = red[0];
+    __syncthreads();
+    return r;
+  };
+  float *s = p.shapes + ((long long)g * p.cb_stride_g + k) * d;
+  float *gp = p.gains + (long long)g * p.cb_stride_g + k;
+  const double W = fin[2 * d];
+  const float g_old_f = *gp;
+  const double g_old = (double)g_old_f;
+  const int e = tid;   // element handled in the tail (d <= 256)
+  const float s_old = (e < d) ? s[e] : 0.0f;
+  if (p.mode == 2) {   // KM: centroid = weighted mean; empty cluster keeps its centroid
+    const double mu_old2 = block_sum((e < d) ? (double)s_old * (double)s_old : 0.0);
+    const double dot_old = block_sum((e < d) ? fin[e] * (double)s_old : 0.0);
+    if (tid == 0 && p.term) p.term[((long long)g * p.term_stride + p.t) * p.term_k + k] = 2.0 * dot_old - W * mu_old2;   // sum over the cluster of w (2 x.mu - ||mu||^2)
+    if (cnt != 0 && W > 0.0 && e < d) s[e] = (float)(fin[e] / W);
+    if (tid == 0 && p.st && cnt == 0) atomicAdd(&p.st[g].n_empty[p.t], 1);
+    return;
+  }
+  const double proj_old = block_sum((e < d) ? fin[e] * (double)s_old : 0.0);
+  const double tk = 2.0 * g_old * proj_old - W * g_old * g_old;
+  float g_new = g_old_f;
+  float s_new = s_old;
+  if (cnt != 0 && W > 0.0) {
+    if (p.mode == 1) {
+      const double bn2 = block_sum((e < d) ? fin[d + e] * fin[d + e] : 0.0);
+      const double bn = sqrt(bn2);
+      if (bn / W > kDelta && e < d) s_new = (float)(fin[d + e] / bn);
+    }
+    const double proj = block_sum((e < d) ? fin[e] * (double)s_new : 0.0);
+    const double gk = proj / W;
+    g_new = (float)(gk > 0.0 ? gk : 0.0);
+  }
+  if (e < d) s[e] = s_new;
+  if (tid == 0) {
+    *gp = g_new;
+    if (p.mode == 1 && p.term) p.term[((long long)g * p.term_stride + p.t) * p.term_k + k] = tk;
+    if (p.gmax) atomicMax(p.gmax + g, __float_as_int(g_new));
+    if (p.st) {
+      atomicMax(&p.st[g].gmax_bits[p.t + 1], __float_as_int(g_new));
+      if (cnt == 0) atomicAdd(&p.st[g].n_empty[p.t], 1);
+    }
+  }
+}
+
+// Alg. 1 l.15-16 after pass t: assignments unchanged -> the group is done.  grid = 1, block = G (<= 1024).
+__global__ void k_wide_converged(DevStats *st, int G, int t) {
+  const int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g < G && t > 1 && st[g].done_iter == 0 && st[g].changed[t] == 0) st[g].done_iter = t;
+}
+
+// ---------------------------------------------------------------------------------------------------- subtract / decode
+struct WSubParams {
+  float *rows;            // [G][N][d] residual, updated in place
+  long long N;
+  int d, K;
+  const float *shapes;    // stage slice
+  const float *gains;
+  long long cb_stride_g;
+  const uint8_t *idx;     // [G][N]
+  uint8_t *codes;         // code plane of this stage [G][N] (may be idx itself) or nullptr
+  __nv_bfloat16 *ahi, *alo;   // operand planes of the NEW residual, or nullptr
+  float *rnorm;
+};
+
+// r <- fl32(r - fl32(g_k s_k)), element-wise, no contraction (reading c-P).  warp per row; grid = (ceil(N / 8), G).
+__global__ void __launch_bounds__(256) k_wide_subtract(WSubParams p) {
+  const int g = blockIdx.y, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const long long i = (long long)blockIdx.x * 8 + warp;
+  if (i >= p.N) return;
+  const long long gi = (long long)g * p.N + i;
+  const int k = p.idx[gi];
+  if (p.codes && lane == 0) p.codes[gi] = (uint8_t)k;
+  const float gk = p.gains[(long long)g * p.cb_stride_g + k];
+  const float *s = p.shapes + ((long long)g * p.cb_stride_g + k) * p.d;
+  double n2 = 0.0;
+  for (int e0 = lane * 4; e0 < p.d; e0 += 128) {
+    float4 r = *reinterpret_cast<float4 *>(p.rows + gi * p.d + e0);
+    const float4 sv = *reinterpret_cast<const float4 *>(s + e0);
+    r.x = __fsub_rn(r.x, __fmul_rn(gk, sv.x)); r.y = __fsub_rn(r.y, __fmul_rn(gk, sv.y));
+    r.z = __fsub_rn(r.z, __fmul_rn(gk, sv.z)); r.w = __fsub_rn(r.w, __fmul_rn(gk, sv.w));
+    *reinterpret_cast<float4 *>(p.rows + gi * p.d + e0) = r;
+    if (p.ahi) {
+      const float x[4] = {r.x, r.y, r.z, r.w};
+      uint32_t h[2], l[2];
+#pragma unroll
+      for (int u = 0; u < 4; u += 2) {
+        const __nv_bfloat16 h0 = __float2bfloat16_rn(x[u]), h1 = __float2bfloat16_rn(x[u + 1]);
+        const __nv_bfloat16 l0 = __float2bfloat16_rn(__fsub_rn(x[u], __bfloat162float(h0)));
+        const __nv_bfloat16 l1 = __float2bfloat16_rn(__fsub_rn(x[u + 1], __bfloat162float(h1)));
+        h[u / 2] = (uint32_t)__bfloat16_as_ushort(h0) | ((uint32_t)__bfloat16_as_ushort(h1) << 16);
+        l[u / 2] = (uint32_t)__bfloat16_as_ushort(l0) | ((uint32_t)__bfloat16_as_ushort(l1) << 16);
+      }
+      *reinterpret_cast<uint2 *>(p.ahi + gi * p.d + e0) = make_uint2(h[0], h[1]);
+      *reinterpret_cast<uint2 *>(p.alo + gi * p.d + e0) = make_uint2(l[0], l[1]);
+      n2 += (double)r.x * r.x + (double)r.y * r.y + (double)r.z * r.z + (double)r.w * r.w;
+    }
+  }
+  if (p.rnorm) {
+    for (int off = 16; off; off >>= 1) n2 += __shfl_xor_sync(0xffffffffu, n2, off);
+    if (lane == 0) p.rnorm[gi] = (float)sqrt(n2) * 1.000001f;
+  }
+}
+
+struct WDecParams {
+  const uint8_t *codes;   // [S][G][N]
+  const float *shapes;    // [G][S][K][d]
+  const float *gains;     // [G][S][K]
+  int S, K, G, n_stages, d, M;
+  long long N;
+  void *out;
+  int dtype;
+  long long stride_g, stride_t;
+};
+
+// xhat = ((c0 + c1) + ...) fp32 in stage order, one RN-even cast.  warp per row (the codeword rows are 4 d bytes wide and
+// come from L2: S x 256 x d x 4 bytes per group do not fit in shared memory).  grid = (ceil(N / 8), G), block = 256.
+__global__ void __launch_bounds__(256) k_wide_decode(WDecParams p) {
+  const int g = blockIdx.y, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const long long i = (long long)blockIdx.x * 8 + warp;
+  if (i >= p.N) return;
+  const long long tok = i / p.M;
+  const int m = (int)(i - tok * p.M);
+  const long long off = (long long)g * p.stride_g + tok * p.stride_t + (long long)m * p.d;
+  for (int e0 = lane * 4; e0 < p.d; e0 += 128) {
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int s = 0; s < p.n_stages; ++s) {
+      const int k = p.codes[((long long)s * p.G + g) * p.N + i];
+      const long long cb = ((long long)g * p.S + s) * p.K + k;
+      const float gk = __ldg(p.gains + cb);
+      const float4 sv = __ldg(reinterpret_cast<const float4 *>(p.shapes + cb * p.d + e0));
+      const float4 c = make_float4(__fmul_rn(gk, sv.x), __fmul_rn(gk, sv.y), __fmul_rn(gk, sv.z), __fmul_rn(gk, sv.w));
+      if (s == 0) acc = c;
+      else { acc.x = __fadd_rn(acc.x, c.x); acc.y = __fadd_rn(acc.y, c.y); acc.z = __fadd_rn(acc.z, c.z); acc.w = __fadd_rn(acc.w, c.w); }
+    }
+    if (p.dtype == GSRQ_BF16) {
+      const __nv_bfloat16 b0 = __float2bfloat16_rn(acc.x), b1 = __float2bfloat16_rn(acc.y), b2 = __float2bfloat16_rn(acc.z), b3 = __float2bfloat16_rn(acc.w);
+      *reinterpret_cast<uint2 *>(reinterpret_cast<uint16_t *>(p.out) + off + e0) =
+          make_uint2((uint32_t)__bfloat16_as_ushort(b0) | ((uint32_t)__bfloat16_as_ushort(b1) << 16),
+                     (uint32_t)__bfloat16_as_ushort(b2) | ((uint32_t)__bfloat16_as_ushort(b3) << 16));
+    } else {
+      *reinterpret_cast<float4 *>(reinterpret_cast<float *>(p.out) + off + e0) = acc;
+    }
+  }
+}
+
+// Gather kv rows of ALL tokens into compact fp32 rows (the encode's working residual).  warp per row.
+__global__ void __launch_bounds__(256) k_wide_gather(RowSrc src, long long N, float *__restrict__ out) {
+  const int g = blockIdx.y, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const long long i = (long long)blockIdx.x * 8 + warp;
+  if (i >= N) return;
+  const int d = src.d;
+  const long long tok = i / src.M;
+  const int m = (int)(i - tok * src.M);
+  for (int e0 = lane * 4; e0 < d; e0 += 128) {
+    float4 v;
+    if (src.dtype == GSRQ_BF16) {
+      const uint2 u = *reinterpret_cast<const uint2 *>(reinterpret_cast<const uint16_t *>(src.kv) + (long long)g * src.stride_g + tok * src.stride_t + (long long)m * d + e0);
+      v = make_float4(__uint_as_float(u.x << 16), __uint_as_float(u.x & 0xFFFF0000u), __uint_as_float(u.y << 16), __uint_as_float(u.y & 0xFFFF0000u));
+    } else {
+      v = *reinterpret_cast<const float4 *>(reinterpret_cast<const float *>(src.kv) + (long long)g * src.stride_g + tok * src.stride_t + (long long)m * d + e0);
+    }
+    *reinterpret_cast<float4 *>(out + ((long long)g * N + i) * d + e0) = v;
+  }
+}
+
+}  // namespace wide
+}  // namespace gsrq
