@@ -472,8 +472,9 @@ struct WPlan {
   long long nf_tok, Nf, Nall, R, nE;   // R = rows the row-sized buffers hold
   int M;
   size_t off_st, off_cnt, off_rows, off_wt, off_wn, off_rnorm, off_idx, off_ids, off_epart, off_term, off_ahi, off_alo, off_bimg, off_gmax,
-      off_list, total;
+      off_list, off_part, total;
 };
+constexpr int kWideParts = 4;   // row ranges per group in the wide update (k_wide.cuh)
 
 static bool wide_tc(int d) { return (d == 64 || d == 128) && use_tc(tc::kD); }
 
@@ -502,7 +503,8 @@ static WPlan make_wplan(const gsrq_view *v, long long n_fit_tokens) {
   p.off_alo = o;   o += align_up(tcp ? G * R * d * 2 : 0);
   p.off_bimg = o;  o += align_up(tcp ? G * (size_t)tc::wide_bimg_bytes<2>() : 0);
   p.off_gmax = o;  o += align_up(G * sizeof(int));
-  p.off_list = o;  o += align_up(G * R * sizeof(uint32_t));
+  p.off_list = o;  o += align_up(G * R * sizeof(uint2));
+  p.off_part = o;  o += align_up(G * GSRQ_MAX_K * (size_t)kWideParts * (2 * d + 2) * sizeof(double));
   p.total = o;
   return p;
 }
@@ -556,8 +558,9 @@ static int wide_assign(const WPlan &pl, const gsrq_view *v, char *ws, const floa
   }
   uint8_t *bimg = (uint8_t *)(ws + pl.off_bimg);
   int *gmax = (int *)(ws + pl.off_gmax);
-  uint32_t *list = (uint32_t *)(ws + pl.off_list);
+  uint2 *list = (uint2 *)(ws + pl.off_list);
   GSRQ_CUDA_CHECK(cudaMemsetAsync(list_cnt, 0, sizeof(unsigned int), stream));
+  GSRQ_CUDA_CHECK(cudaMemsetAsync(gmax, 0, (size_t)G * sizeof(int), stream));
   CUtensorMap tmh, tml;
   int rc = make_wide_map(&tmh, ws + pl.off_ahi, N, G, d);
   if (rc) return rc;
@@ -572,7 +575,7 @@ static int wide_assign(const WPlan &pl, const gsrq_view *v, char *ws, const floa
   const dim3 grid((unsigned)ctas, (unsigned)G);
 #define GSRQ_WIDE_TC(KB, DBG)                                                                                                                   \
   do {                                                                                                                                          \
-    LAUNCH(kClsMisc, stream, (tc::k_bimg_wide<KB><<<G, 256, 0, stream>>>(shapes_st, gains_st, cb_stride_g, K, p.mode, bimg, gmax)));              \
+    LAUNCH(kClsMisc, stream, (tc::k_bimg_wide<KB><<<dim3((unsigned)G, 8), 256, 0, stream>>>(shapes_st, gains_st, cb_stride_g, K, p.mode, bimg, gmax))); \
     GSRQ_CUDA_CHECK(cudaGetLastError());                                                                                                        \
     GSRQ_CUDA_CHECK(cudaFuncSetAttribute(tc::k_score_tc_wide<KB, DBG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tc::WideSmem<KB>::kTotal)); \
     LAUNCH(kClsScore, stream, (tc::k_score_tc_wide<KB, DBG><<<grid, tc::kThreads, tc::WideSmem<KB>::kTotal, stream>>>(tmh, tml, p)));             \
@@ -581,10 +584,9 @@ static int wide_assign(const WPlan &pl, const gsrq_view *v, char *ws, const floa
   else { if (dbg) GSRQ_WIDE_TC(1, true); else GSRQ_WIDE_TC(1, false); }
 #undef GSRQ_WIDE_TC
   GSRQ_CUDA_CHECK(cudaGetLastError());
-  a.list = list; a.list_cnt = list_cnt;
-  // the list length is only known on the device: enough tiles for every row, most of them exit at once
-  dim3 gridl((unsigned)(((long long)G * N + wide::kWaRows - 1) / wide::kWaRows), 1);
-  LAUNCH(kClsRefine, stream, (wide::k_wide_assign<<<gridl, 256, smem, stream>>>(a)));
+  a.list_cnt = list_cnt;
+  // the list length is only known on the device: a machine-filling grid strides over it (one warp per undecided row)
+  LAUNCH(kClsRefine, stream, (wide::k_wide_refine<<<2 * n_sm, 256, (size_t)8 * d * sizeof(double), stream>>>(a, list)));
   GSRQ_CUDA_CHECK(cudaGetLastError());
   return GSRQ_OK;
 }
@@ -607,8 +609,15 @@ static int wide_update(const WPlan &pl, const gsrq_view *v, char *ws, const floa
   u.rows = rows; u.wn = (const double *)(ws + pl.off_wn); u.wt = (const float *)(ws + pl.off_wt); u.nf_tok = nf_tok; u.M = pl.M;
   u.idx = idx; u.idx16 = 0; u.N = N; u.d = v->d; u.K = K; u.shapes = shapes_st; u.gains = gains_st; u.cb_stride_g = cb_stride_g; u.mode = mode;
   u.st = st; u.term = st ? (double *)(ws + pl.off_term) : nullptr; u.term_stride = kTermStride; u.term_k = 256; u.t = t; u.gmax = nullptr;
-  LAUNCH(kClsUpdate, stream, (wide::k_wide_update<<<dim3((unsigned)K, (unsigned)v->G), 256, 0, stream>>>(u)));
+  u.nparts = (N >= 8192) ? kWideParts : 1; u.part = (double *)(ws + pl.off_part);
+  const dim3 ugrid((unsigned)K, (unsigned)v->G, (unsigned)u.nparts);
+  if (v->d > 128) LAUNCH(kClsUpdate, stream, (wide::k_wide_update<2><<<ugrid, 256, 0, stream>>>(u)));
+  else LAUNCH(kClsUpdate, stream, (wide::k_wide_update<1><<<ugrid, 256, 0, stream>>>(u)));
   GSRQ_CUDA_CHECK(cudaGetLastError());
+  if (u.nparts > 1) {
+    LAUNCH(kClsUpdate, stream, (wide::k_wide_update_finish<<<dim3((unsigned)K, (unsigned)v->G), 256, 0, stream>>>(u)));
+    GSRQ_CUDA_CHECK(cudaGetLastError());
+  }
   return GSRQ_OK;
 }
 

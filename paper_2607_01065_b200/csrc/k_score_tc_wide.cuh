@@ -44,7 +44,7 @@ struct ScoreWideParams {
   int n_tiles, n_planes, K, mode;
   DevStats *st;
   int slot;
-  uint32_t *list;         // undecided rows {g*N + i} for the exact kernel
+  uint2 *list;            // undecided rows {g*N + i, mask of the candidate 16-codeword groups} for the exact kernel
   unsigned int *list_cnt;
   float *dbg;             // optional [G][N][256] raw scores (tests)
 };
@@ -61,29 +61,32 @@ __host__ __device__ __forceinline__ uint32_t sw128_off(int row, int col) {
 template <int KB> __host__ __device__ constexpr uint32_t wide_bimg_bytes() { return 2 * KB * kWKbBytesB + kBImgBytes; }
 
 // Operand images of one (group, stage slice): c' = fl32(2 fl32(g_k s_kj)) split hi / lo, bias b = fl32(g_k^2) split in three
-// (mode 1, projection: c' = 2 s_kj, b = 0); rows k >= K can never win.  grid = G, block = 256 (thread = codeword).
+// (mode 1, projection: c' = 2 s_kj, b = 0); rows k >= K can never win.  grid = (G, 8): 32 codewords per CTA, block = 256;
+// gmax[g] (zeroed by the caller) receives the bit pattern of max_k g_k.
 template <int KB>
 __global__ void __launch_bounds__(256) k_bimg_wide(const float *__restrict__ shapes, const float *__restrict__ gains, long long cb_stride_g,
                                                    int K, int mode, uint8_t *__restrict__ bimg, int *__restrict__ gmax) {
-  __shared__ int gmax_bits;
-  const int g = blockIdx.x, k = threadIdx.x;
+  const int g = blockIdx.x, k0 = blockIdx.y * 32;
   constexpr int d = 64 * KB;
   uint8_t *img = bimg + (size_t)g * wide_bimg_bytes<KB>();
-  if (k == 0) gmax_bits = 0;
-  __syncthreads();
-  const bool dead = k >= K;
-  const float gk = (!dead && mode == 0) ? gains[(long long)g * cb_stride_g + k] : 1.0f;
-  const float *s = shapes + ((long long)g * cb_stride_g + k) * d;
-  for (int j = 0; j < d; ++j) {
+  for (int e = threadIdx.x; e < 32 * d; e += 256) {   // coalesced over the codeword rows
+    const int k = k0 + e / d, j = e % d;
+    const bool dead = k >= K;
     float c = 0.f;
-    if (!dead) c = (mode == 0) ? 2.0f * __fmul_rn(gk, s[j]) : 2.0f * s[j];
+    if (!dead) {
+      const float sj = shapes[((long long)g * cb_stride_g + k) * d + j];
+      c = (mode == 0) ? 2.0f * __fmul_rn(gains[(long long)g * cb_stride_g + k], sj) : 2.0f * sj;
+    }
     const __nv_bfloat16 hi = __float2bfloat16_rn(c);
     const __nv_bfloat16 lo = __float2bfloat16_rn(__fsub_rn(c, __bfloat162float(hi)));
     const uint32_t off = (uint32_t)(j >> 6) * kWKbBytesB + sw128_off(k, j & 63);
     *reinterpret_cast<__nv_bfloat16 *>(img + off) = hi;
     *reinterpret_cast<__nv_bfloat16 *>(img + KB * kWKbBytesB + off) = lo;
   }
-  {
+  if (threadIdx.x < 32) {
+    const int k = k0 + threadIdx.x;
+    const bool dead = k >= K;
+    const float gk = (!dead && mode == 0) ? gains[(long long)g * cb_stride_g + k] : 1.0f;
     const float b = dead ? 3.0e38f : ((mode == 0) ? __fmul_rn(gk, gk) : 0.0f);
     const __nv_bfloat16 b1 = __float2bfloat16_rn(b);
     const float r1 = __fsub_rn(b, __bfloat162float(b1));
@@ -97,10 +100,8 @@ __global__ void __launch_bounds__(256) k_bimg_wide(const float *__restrict__ sha
       if (j == 2) v = __hneg(b3);
       *reinterpret_cast<__nv_bfloat16 *>(bias + sw32_off(k, j)) = v;
     }
+    if (!dead && mode == 0 && gmax) atomicMax(gmax + g, __float_as_int(fmaxf(gk, 0.f)));
   }
-  if (!dead && mode == 0) atomicMax(&gmax_bits, __float_as_int(fmaxf(gk, 0.f)));
-  __syncthreads();
-  if (k == 0 && gmax) gmax[g] = gmax_bits;
 }
 
 template <int KB, bool DBG>
@@ -188,9 +189,11 @@ k_score_tc_wide(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant
     const int q = warp & 3;        // TMEM lane quarter this warp may access
     const int wg = (warp - 2) >> 2;
     const float gm = (p.mode == 0) ? __int_as_float(p.gmax[g]) : 1.0f;
-    // error bound of a score with gain g:  E(g) = rho 2^-17 (2 g ||r||) + 2^-18 g^2: operand splits 2^-18 each,
-    // dropped lo.lo 2^-18, the 4-bit index packing 2^-19, fp32 accumulation of 3 x 8 KB + 1 MMAs of 16 products each
-    const float rho17 = (p.n_planes == 1 ? 8.0f : 10.0f) * (float)KB * 0.5f * 7.62939453125e-6f;
+    // error bound of a score with gain g:  E(g) = rho 2^-17 (2 g ||r||) + 2^-18 g^2.  In units of
+    // 2^-17 (2 g ||r||): operand splits 0.5 each, dropped lo.lo 0.5, 4-bit index packing 0.25, fp32 accumulation of 3 d + 3 products
+    // (one rounding of 2^-24 each, the pessimistic reading of the tensor core's accumulation): 3.0 at d = 128, 1.5 at d = 64.
+    // rho = 5 / 6 (d = 128, one / two operand planes), 4 / 5 (d = 64); measured worst error: 1.3 / 1.7 units (tests/test_gpu_wide.py)
+    const float rho17 = (KB == 2 ? (p.n_planes == 1 ? 5.0f : 6.0f) : (p.n_planes == 1 ? 4.0f : 5.0f)) * 7.62939453125e-6f;
     unsigned int n_changed = 0;
     for (int it = wg; it < n_my; it += 2) {
       const int buf = wg, bph = (it >> 1) & 1;
@@ -215,7 +218,7 @@ k_score_tc_wide(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant
       const float E2 = decision_margin(best, rn, gk, gm, rho17, p.mode);
       if (row < p.N) {
         if (best - second <= E2) {
-          p.list[atomicAdd(p.list_cnt, 1u)] = (uint32_t)gr;   // the exact kernel decides (and counts the change)
+          p.list[atomicAdd(p.list_cnt, 1u)] = make_uint2((uint32_t)gr, candidate_groups(gmA, best, E2));   // the exact kernel decides (and counts the change)
         } else {
           n_changed += (k_old != (uint8_t)k_new);
           p.idx[gr] = (uint8_t)k_new;

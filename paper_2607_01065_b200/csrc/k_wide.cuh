@@ -202,101 +202,160 @@ __global__ void __launch_bounds__(256) k_wide_assign(WAssignParams p) {
   int *mk = reinterpret_cast<int *>(mb + kWaRows * 8);   // [32][8] best indices
   const int tid = threadIdx.x, r = tid & 31, q = tid >> 5;
   long long n_rows = p.N;
-  int g = blockIdx.y;
+  const int g_blk = blockIdx.y;
   if (p.list) n_rows = (long long)*p.list_cnt;
-  else if (group_done(p.st, g, p.slot)) return;
-  const long long t0 = (long long)blockIdx.x * kWaRows;
-  if (t0 >= n_rows) return;
-  // global row of my tile row (list mode: rows of any group)
-  long long grow = -1;
-  if (t0 + r < n_rows) grow = p.list ? (long long)p.list[t0 + r] : (long long)g * p.N + t0 + r;
-  // stage the tile's rows as fp64: warp q converts rows q, q + 8, ...
-  for (int rr = q; rr < kWaRows; rr += 8) {
-    const long long gr = (t0 + rr < n_rows) ? (p.list ? (long long)p.list[t0 + rr] : (long long)g * p.N + t0 + rr) : -1;
-    for (int j = r; j < d; j += 32) xs[rr * (d + 1) + j] = (gr >= 0) ? (double)p.rows[gr * d + j] : 0.0;
-  }
-  const int my_g = (grow >= 0) ? (int)(grow / p.N) : 0;   // list mode: the row's group
-  // list mode mixes groups in one tile: each thread reads codewords of ITS row's group, so the codeword chunk in shared
-  // memory is only used when the whole tile is one group
-  bool uniform = !p.list;
-  if (p.list) {
-    const int g0 = (int)((long long)p.list[t0] / p.N);
-    const int g1 = (int)((long long)p.list[min(t0 + kWaRows, n_rows) - 1] / p.N);   // the list is not sorted: check every row
-    int same = (grow < 0) || (my_g == g0);
-    same = __syncthreads_and(same);
-    uniform = same && (g0 == g1);
-    g = g0;
-  }
-  double best = (p.mode == kModeKm) ? INFINITY : -INFINITY;
-  int bk = 0x7fffffff;
-  __syncthreads();
-  for (int k0 = 0; k0 < p.K; k0 += kWaCw) {
-    if (uniform) {
-      __syncthreads();
-      for (int e = tid; e < kWaCw * d; e += 256) {
-        const int kk = k0 + e / d;
-        cw[e] = (kk < p.K) ? (double)p.shapes[((long long)g * p.cb_stride_g + kk) * d + (e % d)] : 0.0;
-      }
-      __syncthreads();
+  else if (group_done(p.st, g_blk, p.slot)) return;
+  for (long long t0 = (long long)blockIdx.x * kWaRows; t0 < n_rows; t0 += (long long)gridDim.x * kWaRows) {
+    int g = g_blk;
+    // global row of my tile row (list mode: rows of any group)
+    long long grow = -1;
+    if (t0 + r < n_rows) grow = p.list ? (long long)p.list[t0 + r] : (long long)g * p.N + t0 + r;
+    __syncthreads();   // the previous tile is done with the shared buffers
+    // stage the tile's rows as fp64: warp q converts rows q, q + 8, ...
+    for (int rr = q; rr < kWaRows; rr += 8) {
+      const long long gr = (t0 + rr < n_rows) ? (p.list ? (long long)p.list[t0 + rr] : (long long)g * p.N + t0 + rr) : -1;
+      for (int j = r; j < d; j += 32) xs[rr * (d + 1) + j] = (gr >= 0) ? (double)p.rows[gr * d + j] : 0.0;
     }
-    double acc[4] = {0.0, 0.0, 0.0, 0.0};
-    const double *xr = xs + r * (d + 1);
-    if (uniform) {
-      const double *c0 = cw + (4 * q) * d;
-      for (int j = 0; j < d; ++j) {
-        const double x = xr[j];
+    const int my_g = (grow >= 0) ? (int)(grow / p.N) : 0;   // list mode: the row's group
+    // list mode can mix groups in one tile: the codeword chunk in shared memory is only used when the whole tile is one group
+    bool uniform = !p.list;
+    if (p.list) {
+      const int g0 = (int)((long long)p.list[t0] / p.N);
+      const int same = __syncthreads_and((grow < 0) || (my_g == g0));
+      uniform = same != 0;
+      g = g0;
+    }
+    double best = (p.mode == kModeKm) ? INFINITY : -INFINITY;
+    int bk = 0x7fffffff;
+    __syncthreads();
+    for (int k0 = 0; k0 < p.K; k0 += kWaCw) {
+      if (uniform) {
+        __syncthreads();
+        for (int e = tid; e < kWaCw * d; e += 256) {
+          const int kk = k0 + e / d;
+          cw[e] = (kk < p.K) ? (double)p.shapes[((long long)g * p.cb_stride_g + kk) * d + (e % d)] : 0.0;
+        }
+        __syncthreads();
+      }
+      double acc[4] = {0.0, 0.0, 0.0, 0.0};
+      const double *xr = xs + r * (d + 1);
+      if (uniform) {
+        const double *c0 = cw + (4 * q) * d;
+        for (int j = 0; j < d; ++j) {
+          const double x = xr[j];
 #pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const double c = c0[u * d + j];
+            if (p.mode == kModeKm) { const double e = __dsub_rn(x, c); acc[u] = __dadd_rn(acc[u], __dmul_rn(e, e)); }
+            else acc[u] = __dadd_rn(acc[u], __dmul_rn(x, c));
+          }
+        }
+      } else if (grow >= 0) {
         for (int u = 0; u < 4; ++u) {
-          const double c = c0[u * d + j];
-          if (p.mode == kModeKm) { const double e = __dsub_rn(x, c); acc[u] = __dadd_rn(acc[u], __dmul_rn(e, e)); }
-          else acc[u] = __dadd_rn(acc[u], __dmul_rn(x, c));
+          const int kk = k0 + 4 * q + u;
+          if (kk >= p.K) break;
+          const float *c0 = p.shapes + ((long long)my_g * p.cb_stride_g + kk) * d;
+          double a = 0.0;
+          for (int j = 0; j < d; ++j) {
+            const double x = xr[j], c = (double)c0[j];
+            if (p.mode == kModeKm) { const double e = __dsub_rn(x, c); a = __dadd_rn(a, __dmul_rn(e, e)); }
+            else a = __dadd_rn(a, __dmul_rn(x, c));
+          }
+          acc[u] = a;
         }
       }
-    } else if (grow >= 0) {
+#pragma unroll
       for (int u = 0; u < 4; ++u) {
         const int kk = k0 + 4 * q + u;
-        if (kk >= p.K) break;
-        const float *c0 = p.shapes + ((long long)my_g * p.cb_stride_g + kk) * d;
-        double a = 0.0;
-        for (int j = 0; j < d; ++j) {
-          const double x = xr[j], c = (double)c0[j];
-          if (p.mode == kModeKm) { const double e = __dsub_rn(x, c); a = __dadd_rn(a, __dmul_rn(e, e)); }
-          else a = __dadd_rn(a, __dmul_rn(x, c));
+        if (kk >= p.K) continue;
+        double sc = acc[u];
+        if (p.mode == kModeGskm) {
+          const double gk = (double)p.gains[(long long)(uniform ? g : my_g) * p.cb_stride_g + kk];
+          sc = __dsub_rn(__dmul_rn(__dmul_rn(2.0, gk), acc[u]), __dmul_rn(gk, gk));
         }
-        acc[u] = a;
+        const bool better = (p.mode == kModeKm) ? (sc < best) : (sc > best);
+        if (better) { best = sc; bk = kk; }   // ascending k within the thread: strict comparison keeps the lowest index
       }
     }
-#pragma unroll
-    for (int u = 0; u < 4; ++u) {
-      const int kk = k0 + 4 * q + u;
-      if (kk >= p.K) continue;
-      double sc = acc[u];
-      if (p.mode == kModeGskm) {
-        const double gk = (double)p.gains[(long long)(uniform ? g : my_g) * p.cb_stride_g + kk];
-        sc = __dsub_rn(__dmul_rn(__dmul_rn(2.0, gk), acc[u]), __dmul_rn(gk, gk));
+    mb[r * 8 + q] = best;
+    mk[r * 8 + q] = bk;
+    __syncthreads();
+    if (q == 0 && grow >= 0) {
+      double b = mb[r * 8];
+      int k = mk[r * 8];
+      for (int u = 1; u < 8; ++u) {
+        const double ob = mb[r * 8 + u];
+        const int ok_ = mk[r * 8 + u];
+        const bool better = (p.mode == kModeKm) ? (ob < b) : (ob > b);
+        if (better || (ob == b && ok_ < k)) { b = ob; k = ok_; }
       }
-      const bool better = (p.mode == kModeKm) ? (sc < best) : (sc > best);
-      if (better) { best = sc; bk = kk; }   // ascending k within the thread: strict comparison keeps the lowest index
+      if (k == 0x7fffffff) k = 0;
+      int old;
+      if (p.idx16) { uint16_t *ip = reinterpret_cast<uint16_t *>(p.idx) + grow; old = *ip; *ip = (uint16_t)k; }
+      else { uint8_t *ip = reinterpret_cast<uint8_t *>(p.idx) + grow; old = *ip; *ip = (uint8_t)k; }
+      if (p.best_out) p.best_out[grow] = b;
+      if (p.st && old != k) atomicAdd(reinterpret_cast<unsigned long long *>(&p.st[(int)(grow / p.N)].changed[p.slot]), 1ull);
     }
   }
-  mb[r * 8 + q] = best;
-  mk[r * 8 + q] = bk;
-  __syncthreads();
-  if (q == 0 && grow >= 0) {
-    double b = mb[r * 8];
-    int k = mk[r * 8];
-    for (int u = 1; u < 8; ++u) {
-      const double ob = mb[r * 8 + u];
-      const int ok_ = mk[r * 8 + u];
-      const bool better = (p.mode == kModeKm) ? (ob < b) : (ob > b);
-      if (better || (ob == b && ok_ < k)) { b = ob; k = ok_; }
+}
+
+// The rows the tensor-core filter could not decide: list entry {g*N + i, mask of the 16-codeword groups whose filter maximum lies
+// within the decision margin} -- a codeword outside those groups cannot be the exact arg-max.  One warp per
+// entry: the row is staged in shared memory as fp64, lane l scores codeword 16 c + l % 16 of two candidate groups per round with
+// the oracle's arithmetic (element order, separate multiply and add), lowest k wins ties.  grid-stride; block = 256 (8 warps),
+// dynamic smem = 8 * d * 8 bytes.
+__global__ void __launch_bounds__(256) k_wide_refine(WAssignParams p, const uint2 *__restrict__ list2) {
+  extern __shared__ __align__(16) double rsm[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, d = p.d;
+  double *xs = rsm + warp * d;
+  const unsigned int n = *p.list_cnt;
+  for (unsigned int e = blockIdx.x * 8 + warp; e < n; e += gridDim.x * 8) {
+    const uint2 en = list2[e];
+    const long long grow = en.x;
+    const int g = (int)(grow / p.N);
+    uint32_t gmask = en.y & 0xFFFFu;
+    __syncwarp();
+    for (int j = lane; j < d; j += 32) xs[j] = (double)p.rows[grow * d + j];
+    __syncwarp();
+    double best = -INFINITY;
+    int bi = 0x7fffffff;
+    while (gmask) {
+      const int c0 = __ffs(gmask) - 1;
+      gmask &= gmask - 1;
+      int c1 = -1;
+      if (gmask) { c1 = __ffs(gmask) - 1; gmask &= gmask - 1; }
+      const int c = (lane < 16) ? c0 : c1;
+      const int kk = 16 * c + (lane & 15);
+      if (c >= 0 && kk < p.K) {
+        const float *sk = p.shapes + ((long long)g * p.cb_stride_g + kk) * d;
+        double dot = 0.0;
+        for (int j = 0; j < d; j += 4) {
+          const float4 sv = __ldg(reinterpret_cast<const float4 *>(sk + j));
+          dot = __dadd_rn(dot, __dmul_rn(xs[j], (double)sv.x));
+          dot = __dadd_rn(dot, __dmul_rn(xs[j + 1], (double)sv.y));
+          dot = __dadd_rn(dot, __dmul_rn(xs[j + 2], (double)sv.z));
+          dot = __dadd_rn(dot, __dmul_rn(xs[j + 3], (double)sv.w));
+        }
+        double sc = dot;
+        if (p.mode == kModeGskm) {
+          const double gk = (double)p.gains[(long long)g * p.cb_stride_g + kk];
+          sc = __dsub_rn(__dmul_rn(__dmul_rn(2.0, gk), dot), __dmul_rn(gk, gk));
+        }
+        if (sc > best || (sc == best && kk < bi)) { best = sc; bi = kk; }
+      }
     }
-    if (k == 0x7fffffff) k = 0;
-    int old;
-    if (p.idx16) { uint16_t *ip = reinterpret_cast<uint16_t *>(p.idx) + grow; old = *ip; *ip = (uint16_t)k; }
-    else { uint8_t *ip = reinterpret_cast<uint8_t *>(p.idx) + grow; old = *ip; *ip = (uint8_t)k; }
-    if (p.best_out) p.best_out[grow] = b;
-    if (p.st && old != k) atomicAdd(reinterpret_cast<unsigned long long *>(&p.st[(int)(grow / p.N)].changed[p.slot]), 1ull);
+    for (int off = 16; off; off >>= 1) {
+      const double ob = __shfl_xor_sync(0xffffffffu, best, off);
+      const int oi = __shfl_xor_sync(0xffffffffu, bi, off);
+      if (ob > best || (ob == best && oi < bi)) { best = ob; bi = oi; }
+    }
+    if (lane == 0) {
+      const int k = (bi == 0x7fffffff) ? 0 : bi;
+      uint8_t *ip = reinterpret_cast<uint8_t *>(p.idx) + grow;
+      const int old = *ip;
+      *ip = (uint8_t)k;
+      if (p.st && old != k) atomicAdd(reinterpret_cast<unsigned long long *>(&p.st[g].changed[p.slot]), 1ull);
+    }
   }
 }
 
@@ -319,35 +378,61 @@ struct WUpdateParams {
   int term_stride, term_k;
   int t;
   int *gmax;              // optional [G]: bit pattern of max_k g_k after this update (atomicMax on an int), for the tensor-core filter
+  int nparts;             // the rows of a group are split in nparts contiguous ranges (gridDim.z), one CTA each
+  double *part;           // nparts > 1: [G][K][nparts][2d + 2] partial sums, merged in range order by k_wide_update_finish
 };
 
-// One CTA per (cluster, group): scan the group's assignment, collect the cluster's rows in ascending order, add them up in
-// fp64 in that order (thread = element: A_e for e < d, B_e for the next d values), then Eq. 7 / Eq. 8.
-// grid = (K, G), block = 256.
+// Eq. 7 / Eq. 8 (or the KM centroid) for cluster k of group g from its sums fin = A[d] | B[d] | W | cnt; all 256 threads.
+__device__ __forceinline__ void wide_finish_cluster(const WUpdateParams &p, int g, int k, const double *fin, double *red);
+
+// One CTA per (cluster, group, row range): scan the range's assignment, collect the cluster's rows in ascending order, add them
+// up in fp64 in that order (thread = element: A_e for e < d, B_e for the next d values); with one range per group the CTA goes
+// on to Eq. 7 / Eq. 8, else the partial sums go to global memory for k_wide_update_finish (heavy-tailed cluster sizes: a
+// cluster with thousands of rows would otherwise keep one CTA busy long after the others have finished).
+// grid = (K, G, nparts), block = 256.  NQ = values per thread = ceil(2 d / 256).
+template <int NQ>
 __global__ void __launch_bounds__(256) k_wide_update(WUpdateParams p) {
-  __shared__ long long rowq[4096];
+  constexpr int kChunk = 2048;              // rows scanned per round (8 per thread)
+  __shared__ int rowq[kChunk];              // matching rows of the round (offset from the round's first row), ascending
+  __shared__ float wq[kChunk];              // their weights w_i
+  __shared__ double wnq[kChunk];            // and w_i / (||r_i|| + eps)
   __shared__ int wcnt[8];
   __shared__ double fin[2 * kMaxD + 2];
   __shared__ double red[256];
   const int k = blockIdx.x, g = blockIdx.y, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   if (group_done(p.st, g, p.t)) return;
+  const long long rb = (p.N * (long long)blockIdx.z / p.nparts) & ~15LL;   // range starts on a 16-row boundary
+  const long long re = (blockIdx.z + 1 == (unsigned)p.nparts) ? p.N : ((p.N * (long long)(blockIdx.z + 1) / p.nparts) & ~15LL);
   const int d = p.d;
-  const int nq = (2 * d + 255) / 256;   // values per thread
-  double acc[2] = {0.0, 0.0};
+  const int msh = ((p.M & (p.M - 1)) == 0) ? (31 - __clz(p.M)) : -1;
+  double acc[NQ];
+#pragma unroll
+  for (int q = 0; q < NQ; ++q) acc[q] = 0.0;
   double accW = 0.0;
   long long cnt = 0;
   const float *rows_g = p.rows + (long long)g * p.N * d;
-  for (long long c0 = 0; c0 < p.N; c0 += 4096) {
-    // ordered compaction of the matching rows of [c0, c0 + 4096): thread t looks at rows c0 + 16 t .. + 15
-    int my[16], nm = 0;
-    const long long b0 = c0 + 16LL * tid;
+  // element this thread reads and whether it belongs to A (coefficient w) or B (coefficient w / (||r|| + eps))
+  int el[NQ];
+  bool isA[NQ], live[NQ];
 #pragma unroll
-    for (int u = 0; u < 16; ++u) {
-      const long long i = b0 + u;
-      int v = -1;
-      if (i < p.N) v = p.idx16 ? (int)reinterpret_cast<const uint16_t *>(p.idx)[(long long)g * p.N + i] : (int)reinterpret_cast<const uint8_t *>(p.idx)[(long long)g * p.N + i];
-      my[u] = (v == k);
-      nm += my[u];
+  for (int q = 0; q < NQ; ++q) { const int v = tid + 256 * q; live[q] = v < 2 * d; isA[q] = v < d; el[q] = (v < d) ? v : v - d; if (!live[q]) el[q] = 0; }
+  for (long long c0 = rb; c0 < re; c0 += kChunk) {
+    // ordered compaction of the matching rows of [c0, c0 + kChunk): thread t looks at rows c0 + 8 t .. + 7
+    int my[8], nm = 0;
+    const long long b0 = c0 + 8LL * tid;
+    if (!p.idx16 && b0 + 8 <= re && (((long long)g * p.N + b0) & 7) == 0) {   // 8 assignment bytes in one load
+      const uint2 v2 = *reinterpret_cast<const uint2 *>(reinterpret_cast<const uint8_t *>(p.idx) + (long long)g * p.N + b0);
+#pragma unroll
+      for (int u = 0; u < 8; ++u) { my[u] = (int)(((u < 4 ? v2.x : v2.y) >> (8 * (u & 3))) & 255u) == k; nm += my[u]; }
+    } else {
+#pragma unroll
+      for (int u = 0; u < 8; ++u) {
+        const long long i = b0 + u;
+        int v = -1;
+        if (i < re) v = p.idx16 ? (int)reinterpret_cast<const uint16_t *>(p.idx)[(long long)g * p.N + i] : (int)reinterpret_cast<const uint8_t *>(p.idx)[(long long)g * p.N + i];
+        my[u] = (v == k);
+        nm += my[u];
+      }
     }
     int incl = nm;
     for (int off = 1; off < 32; off <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, off); if (lane >= off) incl += v; }
@@ -357,41 +442,76 @@ __global__ void __launch_bounds__(256) k_wide_update(WUpdateParams p) {
     for (int w8 = 0; w8 < 8; ++w8) { if (w8 < warp) base += wcnt[w8]; total += wcnt[w8]; }
     int pos = base + incl - nm;
 #pragma unroll
-    for (int u = 0; u < 16; ++u) if (my[u]) rowq[pos++] = b0 + u;
-    __syncthreads();
-    // add the rows in order; 4 rows in flight
-    for (int r0 = 0; r0 < total; r0 += 4) {
-      float xv[4][2];
-      double cf[4][2];
-#pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        if (r0 + u < total) {
-          const long long i = rowq[r0 + u];
-          const double wv = (double)__ldg(p.wt + (long long)g * p.nf_tok + i / p.M), wnv = __ldg(p.wn + (long long)g * p.N + i);
-#pragma unroll
-          for (int q = 0; q < 2; ++q) {
-            const int v = tid + 256 * q;
-            xv[u][q] = (q < nq && v < 2 * d) ? __ldg(rows_g + i * d + (v < d ? v : v - d)) : 0.0f;
-            cf[u][q] = (v < d) ? wv : wnv;
-          }
-          if (tid == 0) accW += wv;
-        } else {
-#pragma unroll
-          for (int q = 0; q < 2; ++q) { xv[u][q] = 0.0f; cf[u][q] = 0.0; }
-        }
+    for (int u = 0; u < 8; ++u)
+      if (my[u]) {
+        const long long i = b0 + u;
+        rowq[pos] = (int)(i - c0);
+        wq[pos] = __ldg(p.wt + (long long)g * p.nf_tok + ((msh >= 0) ? (i >> msh) : (i / p.M)));
+        wnq[pos] = __ldg(p.wn + (long long)g * p.N + i);
+        ++pos;
       }
+    __syncthreads();
+    // add the rows in list order, 4 per trip, the next trip's loads in flight while this trip is added
+    const float *rows_c = rows_g + c0 * d;
+    float xa[4][NQ], xb[4][NQ];
+    auto ld = [&](float (&x)[4][NQ], int r0) {
 #pragma unroll
       for (int u = 0; u < 4; ++u)
 #pragma unroll
-        for (int q = 0; q < 2; ++q) acc[q] = fma(cf[u][q], (double)xv[u][q], acc[q]);
+        for (int q = 0; q < NQ; ++q) x[u][q] = (r0 + u < total && live[q]) ? __ldg(rows_c + (long long)rowq[r0 + u] * d + el[q]) : 0.0f;
+    };
+    auto fm = [&](const float (&x)[4][NQ], int r0) {
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        if (r0 + u < total) {
+          const double wv = (double)wq[r0 + u], wnv = wnq[r0 + u];
+#pragma unroll
+          for (int q = 0; q < NQ; ++q) acc[q] = fma(isA[q] ? wv : wnv, (double)x[u][q], acc[q]);
+          if (tid == 0) accW += wv;
+        }
+      }
+    };
+    ld(xa, 0);
+    for (int r0 = 0; r0 < total; r0 += 8) {
+      ld(xb, r0 + 4);
+      fm(xa, r0);
+      ld(xa, r0 + 8);
+      fm(xb, r0 + 4);
     }
     cnt += total;
     __syncthreads();
   }
 #pragma unroll
-  for (int q = 0; q < 2; ++q) { const int v = tid + 256 * q; if (q < nq && v < 2 * d) fin[v] = acc[q]; }
+  for (int q = 0; q < NQ; ++q) { const int v = tid + 256 * q; if (live[q]) fin[v] = acc[q]; }
   if (tid == 0) { fin[2 * d] = accW; fin[2 * d + 1] = (double)cnt; }
   __syncthreads();
+  if (p.nparts > 1) {
+    double *out = p.part + (((long long)g * p.K + k) * p.nparts + blockIdx.z) * (2 * d + 2);
+    for (int v = tid; v < 2 * d + 2; v += 256) out[v] = fin[v];
+    return;
+  }
+  wide_finish_cluster(p, g, k, fin, red);
+}
+
+// Merge the nparts partial sums of a cluster in range order, then Eq. 7 / Eq. 8.  grid = (K, G), block = 256.
+__global__ void __launch_bounds__(256) k_wide_update_finish(WUpdateParams p) {
+  __shared__ double fin[2 * kMaxD + 2];
+  __shared__ double red[256];
+  const int k = blockIdx.x, g = blockIdx.y, tid = threadIdx.x;
+  if (group_done(p.st, g, p.t)) return;
+  const int d = p.d;
+  const double *in = p.part + ((long long)g * p.K + k) * p.nparts * (2 * d + 2);
+  for (int v = tid; v < 2 * d + 2; v += 256) {
+    double sum = 0.0;
+    for (int q = 0; q < p.nparts; ++q) sum += in[(long long)q * (2 * d + 2) + v];
+    fin[v] = sum;
+  }
+  __syncthreads();
+  wide_finish_cluster(p, g, k, fin, red);
+}
+
+__device__ __forceinline__ void wide_finish_cluster(const WUpdateParams &p, int g, int k, const double *fin, double *red) {
+  const int tid = threadIdx.x, d = p.d;
   // block-wide sums in a fixed tree order
   auto block_sum = [&](double v) -> double {
     red[tid] = v;
@@ -404,9 +524,10 @@ __global__ void __launch_bounds__(256) k_wide_update(WUpdateParams p) {
   float *s = p.shapes + ((long long)g * p.cb_stride_g + k) * d;
   float *gp = p.gains + (long long)g * p.cb_stride_g + k;
   const double W = fin[2 * d];
+  const long long cnt = (long long)fin[2 * d + 1];
   const float g_old_f = *gp;
   const double g_old = (double)g_old_f;
-  const int e = tid;   // element handled in the tail (d <= 256)
+  const int e = tid;   // element handled here (d <= 256)
   const float s_old = (e < d) ? s[e] : 0.0f;
   if (p.mode == 2) {   // KM: centroid = weighted mean; empty cluster keeps its centroid
     const double mu_old2 = block_sum((e < d) ? (double)s_old * (double)s_old : 0.0);
