@@ -21,17 +21,18 @@ import numpy as np
 
 _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "gsrq_oracle.c"
+_SRC_KM = _HERE / "km_oracle.c"      # K-means baseline + quality metrics (section 6.1)
 _SO = _HERE / "build" / "libgsrq_oracle.so"
 _lib = None
 
 
 def build(force: bool = False) -> Path:
     """Compile the oracle with gcc (no fast-math, no FMA contraction)."""
-    if force or not _SO.exists() or _SO.stat().st_mtime < _SRC.stat().st_mtime:
+    if force or not _SO.exists() or _SO.stat().st_mtime < max(_SRC.stat().st_mtime, _SRC_KM.stat().st_mtime):
         _SO.parent.mkdir(exist_ok=True)
         tmp = _SO.with_suffix(f".tmp{os.getpid()}.so")
         cmd = ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off",
-               "-fno-fast-math", "-o", str(tmp), str(_SRC), "-lm"]
+               "-fno-fast-math", "-o", str(tmp), str(_SRC), str(_SRC_KM), "-lm"]
         subprocess.run(cmd, check=True)
         os.replace(tmp, _SO)
     return _SO
@@ -42,6 +43,7 @@ def lib():
     if _lib is None:
         _lib = C.CDLL(str(build()))
         _lib.gsrq_oracle_wdist.restype = C.c_double
+        _lib.km_oracle_wdist.restype = C.c_double
         _lib.gsrq_oracle_splitmix64_next.restype = C.c_uint64
     return _lib
 
@@ -256,3 +258,49 @@ def decode(codes, shapes, gains, hd, S_used=None, bf16=True):
         return out, None
     bits = f32_to_bf16_bits(out)
     return bf16_bits_to_f32(bits), bits
+
+
+# ---- K-means baseline and quality metrics (oracle/km_oracle.c; section 6.1, :200-212) ----
+def km_assign(x, mu):
+    """argmin_k ||x_i - mu_k||^2, lowest k on ties. Returns idx, squared distance."""
+    x, mu = _f32(x), _f32(mu)
+    N, d = x.shape
+    idx = np.zeros(N, dtype=np.int32)
+    best = np.zeros(N, dtype=np.float64)
+    lib().km_oracle_assign(_p(x, C.c_float), C.c_int64(N), d, _p(mu, C.c_float), mu.shape[0], _p(idx, C.c_int32), _p(best, C.c_double))
+    return idx, best
+
+
+def km_update(x, w, idx, mu):
+    """mu_k = weighted mean of the cluster (empty cluster keeps mu_k). Returns new mu, n_empty."""
+    x, mu = _f32(x), _f32(mu).copy()
+    w = _f32(w) if w is not None else None
+    idx = np.ascontiguousarray(idx, dtype=np.int32)
+    ne = lib().km_oracle_update(_p(x, C.c_float), _p(w, C.c_float), C.c_int64(x.shape[0]), x.shape[1], _p(idx, C.c_int32), mu.shape[0], _p(mu, C.c_float))
+    return mu, int(ne)
+
+
+def km_fit(x, w, K, iters, seed):
+    """Lloyd K-means from K seeded distinct rows. Returns a dict."""
+    x = _f32(x)
+    w = _f32(w) if w is not None else None
+    N, d = x.shape
+    mu = np.zeros((K, d), dtype=np.float32)
+    idx = np.zeros(N, dtype=np.int32)
+    J = np.full(max(iters, 1), np.nan, dtype=np.float64)
+    ch = np.full(max(iters, 1), -1, dtype=np.int64)
+    it, ne = C.c_int32(0), C.c_int32(0)
+    rc = lib().km_oracle_fit(_p(x, C.c_float), _p(w, C.c_float), C.c_int64(N), d, K, iters, C.c_uint64(seed), _p(mu, C.c_float),
+                             _p(idx, C.c_int32), _p(J, C.c_double), _p(ch, C.c_int64), C.byref(it), C.byref(ne))
+    if rc != 0:
+        raise ValueError("degenerate input: fewer than K distinct non-zero rows")
+    return dict(mu=mu, idx_last=idx, J_assign=J[:it.value], changed=ch[:it.value], iters_run=it.value, n_empty_last=ne.value)
+
+
+def metrics(x, proto, idx):
+    """MSE, gain error, cosine similarity, shrinkage ratio of the reconstruction xhat_i = proto[idx_i]."""
+    x, proto = _f32(x), _f32(proto)
+    idx = np.ascontiguousarray(idx, dtype=np.int32)
+    out = np.zeros(4, dtype=np.float64)
+    lib().km_oracle_metrics(_p(x, C.c_float), C.c_int64(x.shape[0]), x.shape[1], _p(proto, C.c_float), _p(idx, C.c_int32), _p(out, C.c_double))
+    return dict(mse=float(out[0]), gain_err=float(out[1]), cosine=float(out[2]), shrinkage=float(out[3]))
