@@ -49,7 +49,7 @@ extern "C" {
 typedef enum {
   GSRQ_OK = 0,
   GSRQ_EINVAL = -1,       /* bad shape / alignment / K > 256 / hd % d != 0 / NULL pointer */
-  GSRQ_EUNSUPPORTED = -2, /* valid request this build has no kernel for (d not in {8,16,32}) */
+  GSRQ_EUNSUPPORTED = -2, /* valid request this build has no kernel for (d not in {8,16,32,64,128,256}) */
   GSRQ_EWORKSPACE = -3,   /* workspace too small or misaligned */
   GSRQ_ECUDA = -4,        /* CUDA runtime error (message in gsrq_last_error) */
   GSRQ_EDEGENERATE = -5   /* a group has fewer than K distinct non-zero fit rows (init impossible) */
@@ -192,6 +192,34 @@ int gsrq_update(const void *kv, const gsrq_view *view, const float *residual, co
 int gsrq_init_ids(const void *kv, const gsrq_view *view, const float *residual,
                   const int64_t *fit_tokens, int64_t n_fit, int K, int stage, uint64_t seed,
                   int64_t *ids_out, void *workspace, size_t workspace_bytes, gsrq_stream_t stream);
+
+/* ---- stand-alone clustering of fp32 rows: GSKM against the K-means baseline (section 6.1, :200-212; section 4, :60-85) ---- */
+
+/* Scratch for the three calls below (host function, no CUDA calls); 0 on bad arguments. */
+size_t gsrq_cluster_workspace_bytes(int64_t N, int d, int K);
+
+/*
+ * Learn a codebook of K prototypes on x [N][d] fp32 (device, 16-byte aligned; d a multiple of 4, d <= 256; K <= 4096), one group:
+ *   method 0: weighted GSKM, Algorithm 1 exactly as gsrq_fit_stage runs it (seeded init, Eq. 5 / 7 / 8, safeguards, early exit);
+ *   method 1: standard weighted K-means "KM" (l2 assignment, arithmetic-mean centroid; Lloyd iterations from the
+ *             same K seeded rows; ties -> lowest index; an empty cluster keeps its centroid).
+ * w: [N] fp32 per-row weights or NULL.  Out: shapes [K][d], gains [K] (KM: shapes holds the centroids mu_k, gains = 1), idx_out [N]
+ * uint16 = the assignment of the last iteration run, stats (host, one struct, or NULL; when given the call synchronises).
+ * Every assignment is the exact arg-max / arg-min (fp64, the definition's operation order); sums in fp64, fixed order.
+ */
+int gsrq_cluster_fit(const float *x, const float *w, int64_t N, int d, int K, int iters, uint64_t seed, int method, float *shapes,
+                     float *gains, uint16_t *idx_out, gsrq_fit_stats *stats, void *workspace, size_t workspace_bytes,
+                     gsrq_stream_t stream);
+
+/* One assignment of every row against a given codebook (method as above): idx_out [N] uint16. */
+int gsrq_cluster_assign(const float *x, int64_t N, int d, int K, int method, const float *shapes, const float *gains,
+                        uint16_t *idx_out, gsrq_stream_t stream);
+
+/* Quality of the reconstruction xhat_i = prototype of idx_i (KM: mu_k; GSKM: fl32(g_k s_k)), PAPER.md:202 and :85:
+ * out_host[0] = MSE = E||x - xhat||^2, [1] = gain error E| ||x|| - ||xhat|| |, [2] = cosine similarity E cos(x, xhat),
+ * [3] = shrinkage ratio E||xhat||^2 / E||x||^2.  out_host is a HOST array of 4 doubles; the call synchronises. */
+int gsrq_cluster_metrics(const float *x, int64_t N, int d, int K, int method, const float *shapes, const float *gains,
+                         const uint16_t *idx, double *out_host, void *workspace, size_t workspace_bytes, gsrq_stream_t stream);
 
 /* ---- host-buffer convenience (end-to-end measurement: H2D + kernels + D2H inside) ---- */
 

@@ -41,7 +41,7 @@ class gsrq_fit_stats(C.Structure):
 
 
 _lib = None
-EXPORTS = ["gsrq_workspace_bytes", "gsrq_fit_stage", "gsrq_encode", "gsrq_decode", "gsrq_encode_append", "gsrq_assign", "gsrq_update",
+EXPORTS = ["gsrq_cluster_workspace_bytes", "gsrq_cluster_fit", "gsrq_cluster_assign", "gsrq_cluster_metrics", "gsrq_workspace_bytes", "gsrq_fit_stage", "gsrq_encode", "gsrq_decode", "gsrq_encode_append", "gsrq_assign", "gsrq_update",
            "gsrq_init_ids", "gsrq_debug_scores", "gsrq_encode_host", "gsrq_decode_host", "gsrq_pipeline_host", "gsrq_release_host_pool", "gsrq_profile_enable",
            "gsrq_profile_read", "gsrq_launch_count", "gsrq_last_error", "gsrq_version"]
 
@@ -59,6 +59,7 @@ def lib():
             raise ImportError(f"{p} is not built: run `python -c 'import __graft_entry__ as g; g.build()'`")
         _lib = C.CDLL(str(p))
         _lib.gsrq_workspace_bytes.restype = C.c_size_t
+        _lib.gsrq_cluster_workspace_bytes.restype = C.c_size_t
         _lib.gsrq_last_error.restype = C.c_char_p
         _lib.gsrq_version.restype = C.c_char_p
         _lib.gsrq_launch_count.restype = C.c_int64
@@ -156,6 +157,36 @@ def gsrq_init_ids(kv, view, residual, fit_tokens, K, stage, seed, ids_out, ws):
     n_fit = 0 if fit_tokens is None else fit_tokens.shape[1]
     _check(lib().gsrq_init_ids(_ptr(kv), C.byref(view), _ptr(residual), _ptr(fit_tokens), C.c_int64(n_fit), K, stage,
                                C.c_uint64(seed), _ptr(ids_out), _ptr(ws), C.c_size_t(ws.numel()), _stream()))
+
+
+def cluster_workspace(N: int, d: int, K: int) -> torch.Tensor:
+    n = lib().gsrq_cluster_workspace_bytes(C.c_int64(N), d, K)
+    if n == 0:
+        raise GsrqError(-1, lib().gsrq_last_error().decode())
+    return torch.empty(n, dtype=torch.uint8, device="cuda")
+
+
+def gsrq_cluster_fit(x, w, K, iters, seed, method, shapes, gains, idx_out, ws, want_stats=True):
+    """x [N][d] fp32 CUDA rows; method 0 = GSKM, 1 = K-means; shapes [K][d], gains [K] fp32, idx_out [N] int16/uint16 storage."""
+    N, d = x.shape
+    stats = (gsrq_fit_stats * 1)() if want_stats else None
+    _check(lib().gsrq_cluster_fit(_ptr(x), _ptr(w), C.c_int64(N), d, K, iters, C.c_uint64(seed), method, _ptr(shapes), _ptr(gains),
+                                  _ptr(idx_out), stats, _ptr(ws), C.c_size_t(ws.numel()), _stream()))
+    return stats
+
+
+def gsrq_cluster_assign(x, K, method, shapes, gains, idx_out):
+    N, d = x.shape
+    _check(lib().gsrq_cluster_assign(_ptr(x), C.c_int64(N), d, K, method, _ptr(shapes), _ptr(gains), _ptr(idx_out), _stream()))
+
+
+def gsrq_cluster_metrics(x, K, method, shapes, gains, idx, ws):
+    """Returns dict(mse, gain_err, cosine, shrinkage) of the reconstruction by the assigned prototypes."""
+    N, d = x.shape
+    out = (C.c_double * 4)()
+    _check(lib().gsrq_cluster_metrics(_ptr(x), C.c_int64(N), d, K, method, _ptr(shapes), _ptr(gains), _ptr(idx), out, _ptr(ws),
+                                      C.c_size_t(ws.numel()), _stream()))
+    return dict(mse=out[0], gain_err=out[1], cosine=out[2], shrinkage=out[3])
 
 
 def gsrq_encode_host(kv_host: torch.Tensor, view, cb, codes_host: torch.Tensor):

@@ -734,6 +734,48 @@ static int decode_wide(const uint8_t *codes, const gsrq_codebook *cb, int n_stag
   return GSRQ_OK;
 }
 
+// ---- stand-alone clustering of fp32 rows: GSKM (Alg. 1) or textbook weighted K-means, one group, K <= 4096 ----
+struct CPlan { size_t off_st, off_rows, off_wt, off_wn, off_rnorm, off_idx, off_ids, off_epart, off_term, off_part, off_met, total; long long nE; };
+
+static CPlan make_cplan(long long N, int d, int K) {
+  CPlan p;
+  size_t o = 0;
+  p.nE = (N + 7) / 8;
+  p.off_st = o;    o += align_up(sizeof(DevStats));
+  p.off_rows = o;  o += align_up((size_t)N * d * sizeof(float));
+  p.off_wt = o;    o += align_up((size_t)N * sizeof(float));
+  p.off_wn = o;    o += align_up((size_t)N * sizeof(double));
+  p.off_rnorm = o; o += align_up((size_t)N * sizeof(float));
+  p.off_idx = o;   o += align_up((size_t)N * sizeof(uint16_t));
+  p.off_ids = o;   o += align_up((size_t)K * sizeof(long long));
+  p.off_epart = o; o += align_up((size_t)p.nE * sizeof(double));
+  p.off_term = o;  o += align_up((size_t)kTermStride * K * sizeof(double));
+  p.off_part = o;  o += align_up((size_t)K * kWideParts * (2 * d + 2) * sizeof(double));
+  p.off_met = o;   o += align_up((size_t)p.nE * 5 * sizeof(double) + 64);
+  p.total = o;
+  return p;
+}
+
+static int check_cluster(long long N, int d, int K) {
+  if (N <= 0 || d <= 0 || d > wide::kMaxD || (d & 3) || K <= 0 || K > wide::kMaxK) {
+    set_error("clustering: need N > 0, d a multiple of 4 in [4, %d], K in [1, %d] (got N=%lld d=%d K=%d)", wide::kMaxD, wide::kMaxK, N, d, K);
+    return GSRQ_EINVAL;
+  }
+  return GSRQ_OK;
+}
+
+static int cluster_assign(const float *rows, long long N, int d, int K, int mode, const float *shapes, const float *gains, uint16_t *idx, DevStats *st,
+                          int slot, cudaStream_t stream) {
+  wide::WAssignParams a{};
+  a.rows = rows; a.N = N; a.d = d; a.K = K; a.mode = mode; a.shapes = shapes; a.gains = gains; a.cb_stride_g = K; a.idx = idx; a.idx16 = 1;
+  a.st = st; a.slot = slot;
+  const size_t smem = wide::wide_assign_smem(d);
+  GSRQ_CUDA_CHECK(cudaFuncSetAttribute(wide::k_wide_assign, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  LAUNCH(kClsRefine, stream, (wide::k_wide_assign<<<dim3((unsigned)((N + wide::kWaRows - 1) / wide::kWaRows), 1), 256, smem, stream>>>(a)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  return GSRQ_OK;
+}
+
 }  // namespace gsrq
 
 using namespace gsrq;
@@ -1127,6 +1169,93 @@ int gsrq_init_ids(const void *kv, const gsrq_view *view, const float *residual, 
                                                                                      stage, seed, (long long *)ids_out, st, nullptr,
                                                                                      nullptr, 0, nullptr))));
   GSRQ_CUDA_CHECK(cudaGetLastError());
+  return GSRQ_OK;
+}
+
+
+size_t gsrq_cluster_workspace_bytes(int64_t N, int d, int K) {
+  if (check_cluster(N, d, K) != GSRQ_OK) return 0;
+  return make_cplan(N, d, K).total;
+}
+
+int gsrq_cluster_fit(const float *x, const float *w, int64_t N, int d, int K, int iters, uint64_t seed, int method, float *shapes, float *gains,
+                     uint16_t *idx_out, gsrq_fit_stats *stats, void *workspace, size_t workspace_bytes, gsrq_stream_t stream_) {
+  cudaStream_t stream = (cudaStream_t)stream_;
+  if (!x || !shapes || !gains || !idx_out) { set_error("NULL input"); return GSRQ_EINVAL; }
+  int rc = check_cluster(N, d, K);
+  if (rc) return rc;
+  if (method != 0 && method != 1) { set_error("method must be 0 (GSKM) or 1 (K-means)"); return GSRQ_EINVAL; }
+  if (iters < 0 || iters > GSRQ_MAX_ITERS) { set_error("iters must be in [0, %d]", GSRQ_MAX_ITERS); return GSRQ_EINVAL; }
+  if ((rc = check_align16(x, "x"))) return rc;
+  if (N < K) { set_error("fewer rows (%lld) than centroids (%d)", (long long)N, K); return GSRQ_EDEGENERATE; }
+  const CPlan pl = make_cplan(N, d, K);
+  rc = check_ws(workspace, workspace_bytes, pl.total);
+  if (rc) return rc;
+  char *ws = (char *)workspace;
+  DevStats *st = (DevStats *)(ws + pl.off_st);
+  float *Rf = (float *)(ws + pl.off_rows);
+  GSRQ_CUDA_CHECK(cudaMemsetAsync(st, 0, sizeof(DevStats), stream));
+  GSRQ_CUDA_CHECK(cudaMemsetAsync(idx_out, 0, (size_t)N * sizeof(uint16_t), stream));
+  wide::WPrepParams q{};
+  q.src.kv = nullptr; q.src.rows = x; q.src.dtype = GSRQ_F32; q.src.M = 1; q.src.d = d; q.src.stride_g = 0; q.src.stride_t = 0; q.src.rows_per_group = N;
+  q.w = w; q.w_stride_g = 0; q.fit_tokens = nullptr; q.nf_tok = N; q.Rf = Rf; q.wt = (float *)(ws + pl.off_wt); q.wn = (double *)(ws + pl.off_wn);
+  q.rnorm = (float *)(ws + pl.off_rnorm); q.epart = (double *)(ws + pl.off_epart); q.ahi = nullptr; q.alo = nullptr;
+  LAUNCH(kClsPrep, stream, (wide::k_wide_prep<<<dim3((unsigned)pl.nE, 1), 256, 0, stream>>>(q)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  LAUNCH(kClsPrep, stream, (wide::k_wide_init<<<1, 512, (size_t)K * sizeof(long long), stream>>>(Rf, N, d, K, 1, 0, seed, (long long *)(ws + pl.off_ids), st, shapes, gains,
+                                                                                                (long long)K, method)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  wide::WUpdateParams u{};
+  u.rows = Rf; u.wn = (const double *)(ws + pl.off_wn); u.wt = (const float *)(ws + pl.off_wt); u.nf_tok = N; u.M = 1; u.idx = idx_out; u.idx16 = 1;
+  u.N = N; u.d = d; u.K = K; u.shapes = shapes; u.gains = gains; u.cb_stride_g = K; u.st = st; u.term = (double *)(ws + pl.off_term);
+  u.term_stride = kTermStride; u.term_k = K; u.gmax = nullptr; u.nparts = (N >= 8192) ? kWideParts : 1; u.part = (double *)(ws + pl.off_part);
+  for (int t = (method == 1 ? 1 : 0); t <= iters; ++t) {   // GSKM: t = 0 is Alg. 1 l.2 (gains under the max-projection assignment)
+    const int mode = (method == 1) ? wide::kModeKm : (t == 0 ? wide::kModeProj : wide::kModeGskm);
+    rc = cluster_assign(Rf, N, d, K, mode, shapes, gains, idx_out, st, t, stream);
+    if (rc) return rc;
+    u.mode = (method == 1) ? 2 : (t > 0 ? 1 : 0); u.t = t;
+    const dim3 ugrid((unsigned)K, 1, (unsigned)u.nparts);
+    if (d > 128) LAUNCH(kClsUpdate, stream, (wide::k_wide_update<2><<<ugrid, 256, 0, stream>>>(u)));
+    else LAUNCH(kClsUpdate, stream, (wide::k_wide_update<1><<<ugrid, 256, 0, stream>>>(u)));
+    GSRQ_CUDA_CHECK(cudaGetLastError());
+    if (u.nparts > 1) {
+      LAUNCH(kClsUpdate, stream, (wide::k_wide_update_finish<<<dim3((unsigned)K, 1), 256, 0, stream>>>(u)));
+      GSRQ_CUDA_CHECK(cudaGetLastError());
+    }
+    LAUNCH(kClsMisc, stream, (wide::k_wide_converged<<<1, 32, 0, stream>>>(st, 1, t)));
+    GSRQ_CUDA_CHECK(cudaGetLastError());
+  }
+  if (!stats) return GSRQ_OK;
+  LAUNCH(kClsMisc, stream, (k_finish<<<1, 160, 0, stream>>>(st, (const double *)(ws + pl.off_term), kTermStride, K, (const double *)(ws + pl.off_epart), (int)pl.nE, iters, K)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  return copy_fit_stats(st, 1, stats, stream);
+}
+
+int gsrq_cluster_assign(const float *x, int64_t N, int d, int K, int method, const float *shapes, const float *gains, uint16_t *idx_out,
+                        gsrq_stream_t stream_) {
+  if (!x || !shapes || !gains || !idx_out) { set_error("NULL input"); return GSRQ_EINVAL; }
+  int rc = check_cluster(N, d, K);
+  if (rc) return rc;
+  return cluster_assign(x, N, d, K, method == 1 ? wide::kModeKm : wide::kModeGskm, shapes, gains, idx_out, nullptr, 0, (cudaStream_t)stream_);
+}
+
+int gsrq_cluster_metrics(const float *x, int64_t N, int d, int K, int method, const float *shapes, const float *gains, const uint16_t *idx,
+                         double *out_host, void *workspace, size_t workspace_bytes, gsrq_stream_t stream_) {
+  cudaStream_t stream = (cudaStream_t)stream_;
+  if (!x || !shapes || !gains || !idx || !out_host) { set_error("NULL input"); return GSRQ_EINVAL; }
+  int rc = check_cluster(N, d, K);
+  if (rc) return rc;
+  const CPlan pl = make_cplan(N, d, K);
+  rc = check_ws(workspace, workspace_bytes, pl.total);
+  if (rc) return rc;
+  double *part = (double *)((char *)workspace + pl.off_met);
+  double *res = part + (size_t)pl.nE * 5;
+  LAUNCH(kClsMisc, stream, (wide::k_cluster_metrics<<<(unsigned)pl.nE, 256, 0, stream>>>(x, N, d, shapes, gains, idx, method == 1, part)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  LAUNCH(kClsMisc, stream, (wide::k_cluster_metrics_finish<<<1, 160, 0, stream>>>(part, pl.nE, N, res)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  GSRQ_CUDA_CHECK(cudaMemcpyAsync(out_host, res, 4 * sizeof(double), cudaMemcpyDeviceToHost, stream));
+  GSRQ_CUDA_CHECK(cudaStreamSynchronize(stream));
   return GSRQ_OK;
 }
 

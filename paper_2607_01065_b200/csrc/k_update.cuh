@@ -442,7 +442,7 @@ __global__ void __launch_bounds__(kUpdThreads, 1) k_update(UpdParams p) {
 // Per-group wrap-up of a fit: iters_run, Etot = sum of the energy partials (fixed order) and
 // J_t = Etot - sum_k term_t[k] (Eq. 4 summed over rows; k in ascending order).  grid = G, block = 160.
 __global__ void __launch_bounds__(160) k_finish(DevStats *__restrict__ st, const double *__restrict__ term, int term_stride,
-                                                int K, const double *__restrict__ epart, int n_epart, int iters) {
+                                                int K, const double *__restrict__ epart, int n_epart, int iters, int term_k = 256) {
   __shared__ double etot;
   const int g = blockIdx.x, t = threadIdx.x;
   if (t == 0) {
@@ -454,7 +454,7 @@ __global__ void __launch_bounds__(160) k_finish(DevStats *__restrict__ st, const
   __syncthreads();
   const int n = st[g].done_iter ? st[g].done_iter : iters;
   if (t >= 1 && t <= n) {
-    const double *tm = term + ((long long)g * term_stride + t) * 256;
+    const double *tm = term + ((long long)g * term_stride + t) * term_k;
     double sum = 0.0;
     for (int k = 0; k < K; ++k) sum += tm[k];
     st[g].J[t] = etot - sum;

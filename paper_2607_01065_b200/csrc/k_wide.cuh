@@ -684,5 +684,54 @@ __global__ void __launch_bounds__(256) k_wide_gather(RowSrc src, long long N, fl
   }
 }
 
+// ---------------------------------------------------------------------------------------------------- quality metrics
+// PAPER.md:202 / :85: per row e2 = ||x - xhat||^2, | ||x|| - ||xhat|| |, cos(x, xhat), ||xhat||^2, ||x||^2 with xhat = the row's prototype
+// (KM: the centroid; GSKM: fl32(g_k s_k)); fp64, element order; warp per row, the CTA's 8 rows added in warp order.
+// out: [gridDim.x][5] partial sums.  grid = ceil(N / 8), block = 256.
+__global__ void __launch_bounds__(256) k_cluster_metrics(const float *__restrict__ x, long long N, int d, const float *__restrict__ shapes,
+                                                         const float *__restrict__ gains, const uint16_t *__restrict__ idx, int km,
+                                                         double *__restrict__ out) {
+  __shared__ double sh[8][5];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const long long i = (long long)blockIdx.x * 8 + warp;
+  double v[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+  if (i < N) {
+    const int k = idx[i];
+    const float gk = km ? 1.0f : gains[k];
+    double e2 = 0.0, nx2 = 0.0, np2 = 0.0, dot = 0.0;
+    for (int j = lane; j < d; j += 32) {
+      const double a = (double)x[i * d + j];
+      const double b = (double)(km ? shapes[(long long)k * d + j] : __fmul_rn(gk, shapes[(long long)k * d + j]));
+      e2 += (a - b) * (a - b); nx2 += a * a; np2 += b * b; dot += a * b;
+    }
+    for (int off = 16; off; off >>= 1) {
+      e2 += __shfl_xor_sync(0xffffffffu, e2, off); nx2 += __shfl_xor_sync(0xffffffffu, nx2, off);
+      np2 += __shfl_xor_sync(0xffffffffu, np2, off); dot += __shfl_xor_sync(0xffffffffu, dot, off);
+    }
+    const double nx = sqrt(nx2), np = sqrt(np2);
+    v[0] = e2; v[1] = fabs(nx - np); v[2] = (nx > 0.0 && np > 0.0) ? dot / (nx * np) : 0.0; v[3] = np2; v[4] = nx2;
+  }
+  if (lane == 0)
+    for (int q = 0; q < 5; ++q) sh[warp][q] = v[q];
+  __syncthreads();
+  if (threadIdx.x < 5) {
+    double s = 0.0;
+    for (int w8 = 0; w8 < 8; ++w8) s += sh[w8][threadIdx.x];
+    out[(long long)blockIdx.x * 5 + threadIdx.x] = s;
+  }
+}
+
+// partial sums [n][5] -> res[4] = {MSE, gain error, cosine, shrinkage ratio}; one block of 5 x 32 threads, fixed order
+__global__ void __launch_bounds__(160) k_cluster_metrics_finish(const double *__restrict__ part, long long n, long long N, double *__restrict__ res) {
+  __shared__ double tot[5];
+  const int q = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  double s = 0.0;
+  for (long long c = lane; c < n; c += 32) s += part[c * 5 + q];
+  for (int off = 16; off; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
+  if (lane == 0) tot[q] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) { res[0] = tot[0] / (double)N; res[1] = tot[1] / (double)N; res[2] = tot[2] / (double)N; res[3] = tot[3] / tot[4]; }
+}
+
 }  // namespace wide
 }  // namespace gsrq

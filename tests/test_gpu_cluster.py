@@ -1,0 +1,87 @@
+"""GSKM against the K-means baseline on the GPU (gsrq_cluster_fit / _assign / _metrics; section 6.1, :200-212) versus the
+CPU oracle (oracle/km_oracle.c, oracle/gsrq_oracle.c), and the trend of the paper's random-normal sweeps (Fig. 4).
+Run with `-m gpu` on a B200."""
+import numpy as np
+import pytest
+import torch
+
+from _harness import stats_np
+from oracle import gsrq_oracle as o
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    import __graft_entry__ as ge
+    ge.build()
+    from paper_2607_01065_b200 import binding
+    return binding
+
+
+def _gpu_fit(B, x_np, w_np, K, iters, seed, method):
+    x = torch.from_numpy(x_np).cuda()
+    w = None if w_np is None else torch.from_numpy(w_np).cuda()
+    N, d = x_np.shape
+    shapes = torch.zeros(K, d, device="cuda"); gains = torch.zeros(K, device="cuda")
+    idx = torch.zeros(N, dtype=torch.int16, device="cuda")
+    ws = B.cluster_workspace(N, d, K)
+    stats = B.gsrq_cluster_fit(x, w, K, iters, seed, method, shapes, gains, idx, ws)
+    fin = torch.zeros(N, dtype=torch.int16, device="cuda")
+    B.gsrq_cluster_assign(x, K, method, shapes, gains, fin)
+    met = B.gsrq_cluster_metrics(x, K, method, shapes, gains, fin, ws)
+    torch.cuda.synchronize()
+    return dict(shapes=shapes.cpu().numpy(), gains=gains.cpu().numpy(), idx_last=idx.cpu().numpy().view(np.uint16).astype(np.int32),
+                idx_final=fin.cpu().numpy().view(np.uint16).astype(np.int32), stats=stats_np(stats, 0), metrics=met)
+
+
+@pytest.mark.parametrize("N,d,K,iters,weighted", [(3000, 32, 300, 12, True), (2500, 256, 64, 8, False), (4000, 20, 1500, 6, True)])
+def test_kmeans_matches_oracle(B, N, d, K, iters, weighted):
+    rng = np.random.default_rng(50 + d)
+    x = (rng.standard_normal((N, d)) * np.exp(0.4 * rng.standard_normal(N))[:, None]).astype(np.float32)
+    w = np.exp(rng.standard_normal(N)).astype(np.float32) if weighted else None
+    ref = o.km_fit(x, w, K, iters, 3)
+    got = _gpu_fit(B, x, w, K, iters, 3, method=1)
+    assert np.abs(got["shapes"] - ref["mu"]).max() <= 1e-4 and np.abs(got["shapes"] - ref["mu"]).max() <= 1e-6
+    assert np.array_equal(got["idx_last"], ref["idx_last"])
+    assert got["stats"]["iters_run"] == ref["iters_run"] and np.array_equal(got["stats"]["changed"], ref["changed"])
+    np.testing.assert_allclose(got["stats"]["J"], ref["J_assign"], rtol=1e-6)
+    a, _ = o.km_assign(x, ref["mu"])
+    assert np.array_equal(got["idx_final"], a)
+    m = o.metrics(x, ref["mu"], a)
+    for k in ("mse", "gain_err", "cosine", "shrinkage"):
+        assert got["metrics"][k] == pytest.approx(m[k], rel=1e-9), k
+
+
+@pytest.mark.parametrize("N,d,K,iters", [(3000, 64, 512, 10), (2000, 12, 40, 15)])
+def test_gskm_cluster_fit_matches_oracle(B, N, d, K, iters):
+    rng = np.random.default_rng(60 + d)
+    x = (rng.standard_normal((N, d)) * np.exp(0.4 * rng.standard_normal(N))[:, None]).astype(np.float32)
+    w = np.exp(rng.standard_normal(N)).astype(np.float32)
+    ref = o.fit_stage(x, w, K, iters, 5)
+    got = _gpu_fit(B, x, w, K, iters, 5, method=0)
+    assert np.abs(got["shapes"] - ref["shapes"]).max() <= 1e-6 and np.abs(got["gains"] - ref["gains"]).max() <= 1e-5
+    assert np.array_equal(got["idx_last"], ref["idx_last"])
+    assert got["stats"]["iters_run"] == ref["iters_run"] and np.array_equal(got["stats"]["changed"], ref["changed"])
+    np.testing.assert_allclose(got["stats"]["J"], ref["J_assign"], rtol=1e-6)
+    a, _, _ = o.assign(x, ref["shapes"], ref["gains"])
+    assert np.array_equal(got["idx_final"], a)
+    m = o.metrics(x, ref["gains"][:, None] * ref["shapes"], a)
+    for k in ("mse", "gain_err", "cosine", "shrinkage"):
+        assert got["metrics"][k] == pytest.approx(m[k], rel=1e-9), k
+
+
+def test_fig4_trend_under_capacity(B):
+    """on x ~ N(0, I_D), N = 10,000, in the under-capacity regime (D = 256, small K) GSKM has a higher cosine
+    similarity and a lower gain error than KM; with ample capacity (D = 8, K = 2048) the two are close.  Only the trend is stated
+    in the paper (the figure's values are not in the text)."""
+    from paper_2607_01065_b200 import fig4_sweep
+    rows = fig4_sweep.sweep(settings=[(256, 64), (256, 512), (8, 2048)], iters=15)
+    for r in rows:
+        print(r)
+    for r in rows[:2]:
+        assert r["gskm"]["cosine"] > r["km"]["cosine"] and r["gskm"]["gain_err"] < r["km"]["gain_err"]
+        assert r["km"]["shrinkage"] < 0.5                                    # centroid shrinkage, Eq. 2
+    assert abs(rows[2]["gskm"]["cosine"] - rows[2]["km"]["cosine"]) < 0.02
+    gap_small_k = rows[0]["gskm"]["cosine"] - rows[0]["km"]["cosine"]
+    assert gap_small_k > 0.0
