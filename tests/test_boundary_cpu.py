@@ -50,9 +50,16 @@ def test_workspace_bytes_and_argument_errors(B):
     with pytest.raises(B.GsrqError):
         B.gsrq_workspace_bytes(v, 257, 2, 0)
     lib = B.lib()
-    v64 = B.gsrq_view(B.GSRQ_BF16, 8, 4096, 128, 64, 4096 * 128, 128)
-    assert lib.gsrq_workspace_bytes(C.byref(v64), 256, 2, C.c_int64(0)) == 0
-    assert b"d = 64" in lib.gsrq_last_error()
+    v4 = B.gsrq_view(B.GSRQ_BF16, 8, 4096, 128, 4, 4096 * 128, 128)      # d = 4: no kernel (GSRQ_EUNSUPPORTED)
+    assert lib.gsrq_workspace_bytes(C.byref(v4), 256, 2, C.c_int64(0)) == 0
+    assert b"d = 4" in lib.gsrq_last_error()
+    for d_wide in (64, 128):                                             # the paper's operating points are served
+        vw = B.gsrq_view(B.GSRQ_BF16, 8, 4096, 128, d_wide, 4096 * 128, 128)
+        assert lib.gsrq_workspace_bytes(C.byref(vw), 256, 12, C.c_int64(0)) > 0
+    # stand-alone clustering (KM baseline / GSKM): argument checks
+    assert B.lib().gsrq_cluster_workspace_bytes(C.c_int64(10000), 256, 2048) > 0
+    assert B.lib().gsrq_cluster_workspace_bytes(C.c_int64(10000), 258, 2048) == 0     # d not a multiple of 4
+    assert B.lib().gsrq_cluster_workspace_bytes(C.c_int64(10000), 256, 5000) == 0     # K > 4096
     # compute entry points validate before any CUDA call: NULL pointers -> GSRQ_EINVAL
     cb = B.gsrq_codebook(256, 2, None, None)
     rc = lib.gsrq_encode(None, C.byref(v), C.byref(cb), 0, 2, None, None, None, C.c_size_t(0), None)
