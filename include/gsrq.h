@@ -193,6 +193,31 @@ int gsrq_init_ids(const void *kv, const gsrq_view *view, const float *residual,
                   const int64_t *fit_tokens, int64_t n_fit, int K, int stage, uint64_t seed,
                   int64_t *ids_out, void *workspace, size_t workspace_bytes, gsrq_stream_t stream);
 
+/* ---- decode fused into attention (PAPER.md:443 (ii), :445) ---- */
+
+/* Scratch of gsrq_attention_decode for B sequences of at most max_len tokens (host function, no CUDA calls). */
+size_t gsrq_attention_workspace_bytes(int B, int Hq, int G, int64_t max_len);
+
+/*
+ * One decoding step of grouped-query attention computed straight from the GSRQ codes of the K and V cache, without writing the
+ * dequantised cache (PAPER.md:443 (ii): "bit-unpacking, dequantization, RoPE, and attention computation ... without materializing
+ * intermediate FP16 tensors"): for sequence b and query head h (KV head g = h / (Hq / G)), over the tokens t of the sequence,
+ *     out[b][h] = sum_t softmax_t(scale * q[b][h] . k_t) * vhat_t,
+ *     khat_t = sum_{s < k_stages} cK^(s)[codes], vhat_t = sum_{s < v_stages} cV^(s)[codes]  (fp32, stage order, as gsrq_decode; no cast),
+ *     k_t = khat_t (rope_theta == 0: keys were quantised after the rotary embedding) or RoPE(khat_t, t) (rope_theta > 0: rotate-half
+ *     convention, angle = t * rope_theta^(-2 i / hd), t counted from the sequence's first token; q is given already rotated).
+ * q        : [B][Hq][hd] fp32.            out: [B][Hq][hd] fp32 (zeros for an empty sequence).
+ * k_codes / v_codes: the cache's code planes as gsrq_encode / gsrq_encode_append write them, [S][G][plane_rows], row = token * M + m
+ *            (8-byte aligned); k_cb / v_cb their codebooks; k_stages / v_stages: prefix of stages used.
+ * seq_start, seq_len: device [B] int64: first token and number of tokens of each sequence inside the planes; max_len >= every seq_len
+ *            (host value, sizes the split of the token range over CTAs).
+ * This build serves hd = 128, d = 16, K <= 256, 1..4 stages, Hq / G <= 8.  fp32 arithmetic, no atomics: bit-reproducible.
+ */
+int gsrq_attention_decode(const float *q, const uint8_t *k_codes, const gsrq_codebook *k_cb, int k_stages, const uint8_t *v_codes,
+                          const gsrq_codebook *v_cb, int v_stages, int64_t plane_rows, const int64_t *seq_start, const int64_t *seq_len,
+                          int64_t max_len, int B, int Hq, int G, int hd, int d, float scale, float rope_theta, float *out,
+                          void *workspace, size_t workspace_bytes, gsrq_stream_t stream);
+
 /* ---- stand-alone clustering of fp32 rows: GSKM against the K-means baseline (section 6.1, :200-212; section 4, :60-85) ---- */
 
 /* Scratch for the three calls below (host function, no CUDA calls); 0 on bad arguments. */

@@ -41,7 +41,7 @@ class gsrq_fit_stats(C.Structure):
 
 
 _lib = None
-EXPORTS = ["gsrq_cluster_workspace_bytes", "gsrq_cluster_fit", "gsrq_cluster_assign", "gsrq_cluster_metrics", "gsrq_workspace_bytes", "gsrq_fit_stage", "gsrq_encode", "gsrq_decode", "gsrq_encode_append", "gsrq_assign", "gsrq_update",
+EXPORTS = ["gsrq_attention_workspace_bytes", "gsrq_attention_decode", "gsrq_cluster_workspace_bytes", "gsrq_cluster_fit", "gsrq_cluster_assign", "gsrq_cluster_metrics", "gsrq_workspace_bytes", "gsrq_fit_stage", "gsrq_encode", "gsrq_decode", "gsrq_encode_append", "gsrq_assign", "gsrq_update",
            "gsrq_init_ids", "gsrq_debug_scores", "gsrq_encode_host", "gsrq_decode_host", "gsrq_pipeline_host", "gsrq_release_host_pool", "gsrq_profile_enable",
            "gsrq_profile_read", "gsrq_launch_count", "gsrq_last_error", "gsrq_version"]
 
@@ -60,6 +60,7 @@ def lib():
         _lib = C.CDLL(str(p))
         _lib.gsrq_workspace_bytes.restype = C.c_size_t
         _lib.gsrq_cluster_workspace_bytes.restype = C.c_size_t
+        _lib.gsrq_attention_workspace_bytes.restype = C.c_size_t
         _lib.gsrq_last_error.restype = C.c_char_p
         _lib.gsrq_version.restype = C.c_char_p
         _lib.gsrq_launch_count.restype = C.c_int64
@@ -157,6 +158,21 @@ def gsrq_init_ids(kv, view, residual, fit_tokens, K, stage, seed, ids_out, ws):
     n_fit = 0 if fit_tokens is None else fit_tokens.shape[1]
     _check(lib().gsrq_init_ids(_ptr(kv), C.byref(view), _ptr(residual), _ptr(fit_tokens), C.c_int64(n_fit), K, stage,
                                C.c_uint64(seed), _ptr(ids_out), _ptr(ws), C.c_size_t(ws.numel()), _stream()))
+
+
+def gsrq_attention_decode(q, k_codes, k_cb, k_stages, v_codes, v_cb, v_stages, plane_rows, seq_start, seq_len, max_len, G, d, scale,
+                          rope_theta, out, ws=None):
+    """q [B][Hq][hd] fp32, codes [S][G][plane_rows] uint8, seq_start / seq_len int64 [B] CUDA tensors; out [B][Hq][hd] fp32."""
+    Bq, Hq, hd = q.shape
+    if ws is None:
+        n = lib().gsrq_attention_workspace_bytes(Bq, Hq, G, C.c_int64(max_len))
+        if n == 0:
+            raise GsrqError(-1, lib().gsrq_last_error().decode())
+        ws = torch.empty(n, dtype=torch.uint8, device="cuda")
+    _check(lib().gsrq_attention_decode(_ptr(q), _ptr(k_codes), C.byref(k_cb), k_stages, _ptr(v_codes), C.byref(v_cb), v_stages,
+                                       C.c_int64(plane_rows), _ptr(seq_start), _ptr(seq_len), C.c_int64(max_len), Bq, Hq, G, hd, d,
+                                       C.c_float(scale), C.c_float(rope_theta), _ptr(out), _ptr(ws), C.c_size_t(ws.numel()), _stream()))
+    return ws
 
 
 def cluster_workspace(N: int, d: int, K: int) -> torch.Tensor:

@@ -17,6 +17,7 @@
 #include "k_encode_tc.cuh"
 #include "k_wide.cuh"
 #include "k_score_tc_wide.cuh"
+#include "k_attn.cuh"
 
 namespace gsrq {
 
@@ -1256,6 +1257,66 @@ int gsrq_cluster_metrics(const float *x, int64_t N, int d, int K, int method, co
   GSRQ_CUDA_CHECK(cudaGetLastError());
   GSRQ_CUDA_CHECK(cudaMemcpyAsync(out_host, res, 4 * sizeof(double), cudaMemcpyDeviceToHost, stream));
   GSRQ_CUDA_CHECK(cudaStreamSynchronize(stream));
+  return GSRQ_OK;
+}
+
+static int attn_splits(int B, int G, long long max_len) {
+  long long want = 4LL * sm_count() / ((long long)B * G);   // two CTAs fit on an SM: at most two full waves, no partial third one
+  const long long cap = (max_len + 2047) / 2048;   // at least 2048 tokens per split: the per-CTA tables have to amortise
+  if (want > cap) want = cap;
+  if (want < 1) want = 1;
+  if (want > 256) want = 256;
+  return (int)want;
+}
+
+size_t gsrq_attention_workspace_bytes(int B, int Hq, int G, int64_t max_len) {
+  if (B <= 0 || G <= 0 || Hq <= 0 || Hq % G || Hq / G > 8 || max_len < 0) { set_error("attention: bad B / Hq / G / max_len"); return 0; }
+  return align_up((size_t)B * G * attn_splits(B, G, max_len) * (Hq / G) * attn::kPartStride * sizeof(float)) + 256;
+}
+
+int gsrq_attention_decode(const float *q, const uint8_t *k_codes, const gsrq_codebook *k_cb, int k_stages, const uint8_t *v_codes,
+                          const gsrq_codebook *v_cb, int v_stages, int64_t plane_rows, const int64_t *seq_start, const int64_t *seq_len,
+                          int64_t max_len, int B, int Hq, int G, int hd, int d, float scale, float rope_theta, float *out, void *workspace,
+                          size_t workspace_bytes, gsrq_stream_t stream_) {
+  cudaStream_t stream = (cudaStream_t)stream_;
+  if (!q || !k_codes || !v_codes || !k_cb || !v_cb || !k_cb->shapes || !k_cb->gains || !v_cb->shapes || !v_cb->gains || !seq_start || !seq_len || !out) {
+    set_error("NULL input"); return GSRQ_EINVAL;
+  }
+  if (hd != attn::kHd || d != attn::kD) { set_error("attention: this build serves head_dim 128 with d = 16 (got %d, %d)", hd, d); return GSRQ_EUNSUPPORTED; }
+  if (B <= 0 || G <= 0 || Hq <= 0 || Hq % G || Hq / G > 8) { set_error("attention: need Hq a multiple of G with at most 8 query heads per KV head"); return GSRQ_EINVAL; }
+  if (k_cb->K < 1 || k_cb->K > 256 || v_cb->K < 1 || v_cb->K > 256 || k_stages < 1 || k_stages > 4 || k_stages > k_cb->S || v_stages < 1 || v_stages > 4 ||
+      v_stages > v_cb->S) { set_error("attention: K in [1, 256] and 1..4 stages (<= S) for keys and values"); return GSRQ_EINVAL; }
+  if (plane_rows <= 0 || plane_rows % attn::kM || max_len < 0 || rope_theta < 0.0f) { set_error("attention: bad plane_rows / max_len / rope_theta"); return GSRQ_EINVAL; }
+  if (((uintptr_t)k_codes & 7) || ((uintptr_t)v_codes & 7)) { set_error("code planes must be 8-byte aligned"); return GSRQ_EINVAL; }
+  const size_t need = gsrq_attention_workspace_bytes(B, Hq, G, max_len);
+  int rc = check_ws(workspace, workspace_bytes, need);
+  if (rc) return rc;
+  attn::AttnParams p{};
+  p.q = q; p.kc = k_codes; p.vc = v_codes; p.k_shapes = k_cb->shapes; p.k_gains = k_cb->gains; p.v_shapes = v_cb->shapes; p.v_gains = v_cb->gains;
+  p.kS = k_cb->S; p.kK = k_cb->K; p.vS = v_cb->S; p.vK = v_cb->K; p.k_stages = k_stages; p.v_stages = v_stages; p.plane_rows = plane_rows;
+  p.seq_start = (const long long *)seq_start; p.seq_len = (const long long *)seq_len; p.B = B; p.Hq = Hq; p.G = G; p.n_rep = Hq / G;
+  p.n_split = attn_splits(B, G, max_len); p.scale = scale; p.rope_theta = rope_theta; p.part = (float *)workspace; p.out = out;
+  const bool rope = rope_theta > 0.0f;
+  const size_t smem = attn::attn_smem_bytes(k_stages, v_stages, p.n_rep, rope);
+  if (smem > 227 * 1024) { set_error("attention: %d key stages x %d query heads per KV head do not fit in shared memory", k_stages, p.n_rep); return GSRQ_EUNSUPPORTED; }
+  const dim3 grid((unsigned)p.n_split, (unsigned)G, (unsigned)B);
+#define GSRQ_ATTN(ROPE, NREP, NS)                                                                                                       \
+  do {                                                                                                                                  \
+    GSRQ_CUDA_CHECK(cudaFuncSetAttribute(attn::k_attn_decode<ROPE, NREP, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+    LAUNCH(kClsDecode, stream, (attn::k_attn_decode<ROPE, NREP, NS><<<grid, attn::kThreads, smem, stream>>>(p)));                       \
+  } while (0)
+  // compile-time head ratio / stage count for the common shapes (LLaMA-3-8B: 4 query heads per KV head); else the generic kernel
+  const int ns = (k_stages == v_stages) ? k_stages : 0;
+  if (p.n_rep == 4 && ns == 1) { if (rope) GSRQ_ATTN(true, 4, 1); else GSRQ_ATTN(false, 4, 1); }
+  else if (p.n_rep == 4 && ns == 2) { if (rope) GSRQ_ATTN(true, 4, 2); else GSRQ_ATTN(false, 4, 2); }
+  else if (p.n_rep == 4 && ns == 4) { if (rope) GSRQ_ATTN(true, 4, 4); else GSRQ_ATTN(false, 4, 4); }
+  else if (p.n_rep == 1 && ns == 2) { if (rope) GSRQ_ATTN(true, 1, 2); else GSRQ_ATTN(false, 1, 2); }
+  else if (p.n_rep == 8 && ns == 2) { if (rope) GSRQ_ATTN(true, 8, 2); else GSRQ_ATTN(false, 8, 2); }
+  else { if (rope) GSRQ_ATTN(true, 0, 0); else GSRQ_ATTN(false, 0, 0); }
+#undef GSRQ_ATTN
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  LAUNCH(kClsDecode, stream, (attn::k_attn_combine<<<dim3((unsigned)Hq, (unsigned)B), 128, 0, stream>>>(p)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
   return GSRQ_OK;
 }
 

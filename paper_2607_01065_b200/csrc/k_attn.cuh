@@ -1,0 +1,314 @@
+// k_attn.cuh -- decode-attention straight from the GSRQ codes (PAPER.md:443 (ii): "on-the-fly bit-unpacking, dequantization,
+// RoPE, and attention computation during decoding without materializing intermediate FP16 tensors"; the step is
+// bound by memory traffic, and the codes are 16x smaller than the bf16 cache at 1 bit per element).
+//
+// For sequence b, KV head g and its n_rep = Hq / G query heads (grouped-query attention; LLaMA-3-8B: 32 / 8), over the
+// sequence's tokens t:      out_h = sum_t softmax_t(scale q_h . k_t) vhat_t,
+//     khat_t = sum_s cK^(s)[aK^(s)_t],  vhat_t = sum_s cV^(s)[aV^(s)_t]   (fp32 sums in stage order, never written to memory),
+//     k_t = khat_t                               keys stored after the rotary embedding (rope_theta == 0), or
+//     k_t = RoPE(khat_t, t)                      keys quantised before it (rotate-half convention, angle = t theta^(-2i/hd)).
+// Without RoPE the keys are never even dequantised: q_h . khat_t = sum_s sum_m (q_h[m] . cK^(s)_k[.])[k = aK^(s)_{t,m}], so one table
+// QT[h][s][m][k] of n_rep x S x 8 x 256 dot products per (sequence, KV head) turns a token's logit into S x 8 shared-memory
+// lookups per query head.  With RoPE the two sub-vectors of a rotary pair (elements i and i + 64) are dequantised in registers,
+// rotated with cos / sin((base + off) theta_i) = angle addition of a per-chunk base (double precision) and a per-CTA offset
+// table, and multiplied with q.  Values: thread = output element, the chunk's probabilities are broadcast from shared memory.
+// Split-K over the tokens (flash-decoding): CTA (split, g, b) keeps a running max / sum per head, k_attn_combine merges the
+// splits in split order.  d = 16, hd = 128, K <= 256, up to 4 stages each; fp32 arithmetic, no atomics (bit-reproducible).
+#pragma once
+#include "gsrq_common.cuh"
+
+namespace gsrq {
+namespace attn {
+
+constexpr int kHd = 128, kD = 16, kM = 8, kThreads = 256;
+constexpr int kPartStride = kHd + 2;   // m, l, acc[128]
+
+struct AttnParams {
+  const float *q;             // [B][Hq][128] fp32 (already rotated when rope_theta > 0)
+  const uint8_t *kc, *vc;     // code planes: stage s, head g, row t*8 + m at codes[(s*G + g)*plane_rows + t*8 + m]
+  const float *k_shapes, *k_gains, *v_shapes, *v_gains;   // [G][S][K][16], [G][S][K]
+  int kS, kK, vS, vK;         // codebook dimensions (S = stages in the arrays)
+  int k_stages, v_stages;     // stages used
+  long long plane_rows;
+  const long long *seq_start, *seq_len;   // [B] first token / number of tokens of each sequence in the planes
+  int B, Hq, G, n_rep, n_split;
+  float scale, rope_theta;
+  float *part;                // [B][G][n_split][n_rep][130]
+  float *out;                 // [B][Hq][128]
+};
+
+__host__ __device__ inline size_t attn_smem_bytes(int k_stages, int v_stages, int n_rep, bool rope) {
+  const int ch = rope ? 64 : 256;
+  size_t b = (size_t)v_stages * 256 * kD * 4;                                 // value codeword table
+  b += rope ? ((size_t)k_stages * 256 * kD * 4 + (size_t)n_rep * kHd * 4 + 64 * 64 * 8 + 64 * 8)   // key table, q, offset / base rotations
+            : (size_t)((n_rep + 3) & ~3) * k_stages * kM * 256 * 4;           // q . codeword tables (heads innermost, padded to 4)
+  b += (size_t)(n_rep * ch > kHd ? n_rep * ch : kHd) * 4;                     // logits / probabilities of the chunk (also the final exchange buffer)
+  b += (size_t)ch * kM * (size_t)v_stages;                                    // the chunk's value codes
+  b += 3 * 8 * 4 + 16;                                                        // running max, sum, rescale per head
+  return (b + 15) & ~(size_t)15;
+}
+
+// NREP / NS > 0: query heads per KV head and stages (keys = values) fixed at compile time, every loop over them unrolled;
+// NREP == 0 && NS == 0: the generic kernel (any n_rep <= 8, 1..4 stages each).
+template <bool ROPE, int NREP, int NS>
+__global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
+  extern __shared__ __align__(16) uint8_t asm_raw[];
+  constexpr int CH = ROPE ? 64 : 256;
+  constexpr int HMAX = NREP > 0 ? NREP : 8;
+  const int sp = blockIdx.x, g = blockIdx.y, b = blockIdx.z, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int n_rep = NREP > 0 ? NREP : p.n_rep, SK = NS > 0 ? NS : p.k_stages, SV = NS > 0 ? NS : p.v_stages;
+  float *vtab = reinterpret_cast<float *>(asm_raw);
+  float *ktab = vtab + SV * 256 * kD;                                   // ROPE: key table; else the q . codeword tables
+  float *qs = ktab + SK * 256 * kD;                                     // ROPE only
+  float2 *cs_off = reinterpret_cast<float2 *>(qs + n_rep * kHd);        // [64 offsets][64 frequencies]
+  float2 *cs_base = cs_off + 64 * 64;                                   // [64]
+  const int HP = (n_rep + 3) & ~3;                                      // heads padded to a multiple of 4
+  float *qt = ktab;                                                     // [SK][8][256][HP]
+  float *lg = ROPE ? reinterpret_cast<float *>(cs_base + 64) : qt + HP * SK * kM * 256;
+  uint8_t *vcodes = reinterpret_cast<uint8_t *>(lg + (n_rep * CH > kHd ? n_rep * CH : kHd));   // [SV][CH][8]
+  float *m_run = reinterpret_cast<float *>(vcodes + ((CH * kM * SV + 15) & ~15));
+  float *l_run = m_run + 8, *sc_h = l_run + 8;
+
+  const long long t_seq0 = p.seq_start[b], len = p.seq_len[b];
+  long long per = (len + p.n_split - 1) / p.n_split;
+  per = (per + CH - 1) / CH * CH;
+  const long long tb = (long long)sp * per, te = min(len, tb + per);
+  const float *qg = p.q + ((long long)b * p.Hq + (long long)g * n_rep) * kHd;
+
+  // ---- tables ----
+#pragma unroll 8
+  for (int e = tid; e < SV * 256 * kD; e += kThreads) {
+    const int s = e / (256 * kD), r = e - s * 256 * kD, k = r >> 4;
+    const long long cb = ((long long)g * p.vS + s) * p.vK + k;
+    vtab[e] = (k < p.vK) ? __fmul_rn(p.v_gains[cb], p.v_shapes[cb * kD + (r & 15)]) : 0.0f;
+  }
+  if (ROPE) {
+#pragma unroll 8
+    for (int e = tid; e < SK * 256 * kD; e += kThreads) {
+      const int s = e / (256 * kD), r = e - s * 256 * kD, k = r >> 4;
+      const long long cb = ((long long)g * p.kS + s) * p.kK + k;
+      ktab[e] = (k < p.kK) ? __fmul_rn(p.k_gains[cb], p.k_shapes[cb * kD + (r & 15)]) : 0.0f;
+    }
+    for (int e = tid; e < n_rep * kHd; e += kThreads) qs[e] = qg[e];
+    for (int e = tid; e < 64 * 64; e += kThreads) {   // rotation by (offset within the chunk) x theta_i, in double
+      const int off = e >> 6, i = e & 63;
+      double sn, cs;
+      sincos((double)off * pow((double)p.rope_theta, -(double)i / 64.0), &sn, &cs);
+      cs_off[e] = make_float2((float)cs, (float)sn);
+    }
+  } else {
+    // QT[h][s][m][k] = sum_j q_h[16 m + j] cK^(s)_k[j]: thread per codeword (s, k), every (h, m); q staged in the (still unused) logits buffer
+    for (int e = tid; e < n_rep * kHd; e += kThreads) lg[e] = qg[e];
+    __syncthreads();
+    for (int e = tid; e < SK * 256; e += kThreads) {
+      const int s = e >> 8, k = e & 255;
+      float c[kD];
+      const long long cb = ((long long)g * p.kS + s) * p.kK + k;
+      const float gk = (k < p.kK) ? p.k_gains[cb] : 0.0f;
+#pragma unroll
+      for (int j = 0; j < kD; ++j) c[j] = (k < p.kK) ? __fmul_rn(gk, p.k_shapes[cb * kD + j]) : 0.0f;
+      for (int h = 0; h < n_rep; ++h)
+#pragma unroll
+        for (int m = 0; m < kM; ++m) {
+          float a = 0.0f;
+#pragma unroll
+          for (int j = 0; j < kD; ++j) a = fmaf(lg[h * kHd + m * kD + j], c[j], a);
+          qt[((s * kM + m) * 256 + k) * HP + h] = a;
+        }
+    }
+  }
+  if (tid < 8) { m_run[tid] = -INFINITY; l_run[tid] = 0.0f; sc_h[tid] = 0.0f; }
+  // values: warp w takes the tokens t = w (mod 8) of a chunk, lane l the output elements 4 l .. 4 l + 3
+  float acc[HMAX][4];
+#pragma unroll
+  for (int h = 0; h < HMAX; ++h) { acc[h][0] = 0.0f; acc[h][1] = 0.0f; acc[h][2] = 0.0f; acc[h][3] = 0.0f; }
+  const int m_out = lane >> 2, j_out = (lane & 3) * 4;
+  __syncthreads();
+
+  for (long long t0 = tb; t0 < te; t0 += CH) {
+    const int nv = (int)min((long long)CH, te - t0);   // valid tokens of the chunk
+    // the chunk's value codes -> shared memory (coalesced 8-byte loads)
+    for (int e = tid; e < SV * CH; e += kThreads) {
+      const int s = e / CH, t = e - s * CH;
+      uint2 v = make_uint2(0u, 0u);
+      if (t < nv) v = *reinterpret_cast<const uint2 *>(p.vc + ((long long)s * p.G + g) * p.plane_rows + (t_seq0 + t0 + t) * kM);
+      reinterpret_cast<uint2 *>(vcodes)[e] = v;
+    }
+    // ---- logits ----
+    if (!ROPE) {
+      const int t = tid;
+      if (t < nv) {
+        float sum[(HMAX + 3) & ~3];
+#pragma unroll
+        for (int h = 0; h < ((HMAX + 3) & ~3); ++h) sum[h] = 0.0f;
+#pragma unroll
+        for (int s = 0; s < (NS > 0 ? NS : 4); ++s) {
+          if (s >= SK) break;
+          const uint2 cw = *reinterpret_cast<const uint2 *>(p.kc + ((long long)s * p.G + g) * p.plane_rows + (t_seq0 + t0 + t) * kM);
+#pragma unroll
+          for (int m = 0; m < kM; ++m) {
+            const int k = (int)(((m < 4 ? cw.x : cw.y) >> (8 * (m & 3))) & 255u);
+            const float4 *q4 = reinterpret_cast<const float4 *>(qt + ((s * kM + m) * 256 + k) * HP);
+#pragma unroll
+            for (int h4 = 0; h4 < (HMAX + 3) / 4; ++h4) {
+              if (4 * h4 >= n_rep) break;
+              const float4 v = q4[h4];
+              sum[4 * h4] += v.x;
+              if (4 * h4 + 1 < HMAX) sum[4 * h4 + 1] += v.y;
+              if (4 * h4 + 2 < HMAX) sum[4 * h4 + 2] += v.z;
+              if (4 * h4 + 3 < HMAX) sum[4 * h4 + 3] += v.w;
+            }
+          }
+        }
+#pragma unroll
+        for (int h = 0; h < HMAX; ++h)
+          if (h < n_rep) lg[h * CH + t] = sum[h] * p.scale;
+      }
+    } else {
+      if (tid < 64) {   // rotation by (first position of the chunk) x theta_i, in double
+        double sn, cs;
+        sincos((double)t0 * pow((double)p.rope_theta, -(double)tid / 64.0), &sn, &cs);
+        cs_base[tid] = make_float2((float)cs, (float)sn);
+      }
+      __syncthreads();
+      const int t = tid >> 2, mq = tid & 3;   // token of the chunk, rotary pair of sub-vectors (mq, mq + 4)
+      float part[HMAX];
+#pragma unroll
+      for (int h = 0; h < HMAX; ++h) part[h] = 0.0f;
+      if (t < nv) {
+        float a[kD], bb[kD];
+#pragma unroll
+        for (int j = 0; j < kD; ++j) { a[j] = 0.0f; bb[j] = 0.0f; }
+#pragma unroll
+        for (int s = 0; s < (NS > 0 ? NS : 4); ++s) {
+          if (s >= SK) break;
+          const uint8_t *cp = p.kc + ((long long)s * p.G + g) * p.plane_rows + (t_seq0 + t0 + t) * kM;
+          const float4 *ra = reinterpret_cast<const float4 *>(ktab + (s * 256 + cp[mq]) * kD);
+          const float4 *rb = reinterpret_cast<const float4 *>(ktab + (s * 256 + cp[mq + 4]) * kD);
+#pragma unroll
+          for (int q4 = 0; q4 < 4; ++q4) {
+            const float4 va = ra[q4], vb = rb[q4];
+            if (s == 0) { a[4 * q4] = va.x; a[4 * q4 + 1] = va.y; a[4 * q4 + 2] = va.z; a[4 * q4 + 3] = va.w;
+                          bb[4 * q4] = vb.x; bb[4 * q4 + 1] = vb.y; bb[4 * q4 + 2] = vb.z; bb[4 * q4 + 3] = vb.w; }
+            else { a[4 * q4] = __fadd_rn(a[4 * q4], va.x); a[4 * q4 + 1] = __fadd_rn(a[4 * q4 + 1], va.y); a[4 * q4 + 2] = __fadd_rn(a[4 * q4 + 2], va.z); a[4 * q4 + 3] = __fadd_rn(a[4 * q4 + 3], va.w);
+                   bb[4 * q4] = __fadd_rn(bb[4 * q4], vb.x); bb[4 * q4 + 1] = __fadd_rn(bb[4 * q4 + 1], vb.y); bb[4 * q4 + 2] = __fadd_rn(bb[4 * q4 + 2], vb.z); bb[4 * q4 + 3] = __fadd_rn(bb[4 * q4 + 3], vb.w); }
+          }
+        }
+#pragma unroll
+        for (int j = 0; j < kD; ++j) {
+          const int i = mq * kD + j;
+          const float2 cb = cs_base[i], co = cs_off[t * 64 + i];
+          const float c = cb.x * co.x - cb.y * co.y, sn = cb.y * co.x + cb.x * co.y;
+          const float ar = a[j] * c - bb[j] * sn, br = bb[j] * c + a[j] * sn;
+#pragma unroll
+          for (int h = 0; h < HMAX; ++h)
+            if (h < n_rep) part[h] = fmaf(qs[h * kHd + i], ar, fmaf(qs[h * kHd + 64 + i], br, part[h]));
+        }
+      }
+#pragma unroll
+      for (int h = 0; h < HMAX; ++h) {
+        if (h < n_rep) {
+          float v = part[h];
+          v += __shfl_xor_sync(0xffffffffu, v, 1);
+          v += __shfl_xor_sync(0xffffffffu, v, 2);
+          if (mq == 0 && t < nv) lg[h * CH + t] = v * p.scale;
+        }
+      }
+    }
+    __syncthreads();
+    // ---- running softmax: warp h handles head h ----
+    if (warp < n_rep) {
+      const int h = warp;
+      float mx = -INFINITY;
+      for (int t = lane; t < nv; t += 32) mx = fmaxf(mx, lg[h * CH + t]);
+      for (int off = 16; off; off >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, off));
+      const float m_old = m_run[h], m_new = fmaxf(m_old, mx);
+      float sum = 0.0f;
+      for (int t = lane; t < CH; t += 32) {
+        const float pr = (t < nv) ? expf(lg[h * CH + t] - m_new) : 0.0f;
+        lg[h * CH + t] = pr;
+        sum += pr;
+      }
+      for (int off = 16; off; off >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, off);
+      if (lane == 0) {
+        const float sc = (m_old == -INFINITY) ? 0.0f : expf(m_old - m_new);
+        sc_h[h] = sc;
+        l_run[h] = l_run[h] * sc + sum;
+        m_run[h] = m_new;
+      }
+    }
+    __syncthreads();
+    // ---- values: thread = output element (two threads per element, even / odd tokens) ----
+#pragma unroll
+    for (int h = 0; h < HMAX; ++h)
+      if (h < n_rep) { const float sc = sc_h[h]; acc[h][0] *= sc; acc[h][1] *= sc; acc[h][2] *= sc; acc[h][3] *= sc; }
+    auto value_of = [&](int t) -> float4 {   // vhat_t[4 lane .. 4 lane + 3] = sum over the stages, fp32, stage order
+      float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+      for (int s = 0; s < (NS > 0 ? NS : 4); ++s) {
+        if (s >= SV) break;
+        const float4 c = *reinterpret_cast<const float4 *>(vtab + (s * 256 + vcodes[(s * CH + t) * kM + m_out]) * kD + j_out);
+        if (s == 0) v = c;
+        else { v.x = __fadd_rn(v.x, c.x); v.y = __fadd_rn(v.y, c.y); v.z = __fadd_rn(v.z, c.z); v.w = __fadd_rn(v.w, c.w); }
+      }
+      return v;
+    };
+    int t = warp;
+    for (; t + 8 < nv; t += 16) {   // two tokens in flight
+      const float4 v0 = value_of(t), v1 = value_of(t + 8);
+#pragma unroll
+      for (int h = 0; h < HMAX; ++h)
+        if (h < n_rep) {
+          const float p0 = lg[h * CH + t], p1 = lg[h * CH + t + 8];
+          acc[h][0] = fmaf(p1, v1.x, fmaf(p0, v0.x, acc[h][0])); acc[h][1] = fmaf(p1, v1.y, fmaf(p0, v0.y, acc[h][1]));
+          acc[h][2] = fmaf(p1, v1.z, fmaf(p0, v0.z, acc[h][2])); acc[h][3] = fmaf(p1, v1.w, fmaf(p0, v0.w, acc[h][3]));
+        }
+    }
+    for (; t < nv; t += 8) {
+      const float4 v = value_of(t);
+#pragma unroll
+      for (int h = 0; h < HMAX; ++h)
+        if (h < n_rep) {
+          const float p0 = lg[h * CH + t];
+          acc[h][0] = fmaf(p0, v.x, acc[h][0]); acc[h][1] = fmaf(p0, v.y, acc[h][1]);
+          acc[h][2] = fmaf(p0, v.z, acc[h][2]); acc[h][3] = fmaf(p0, v.w, acc[h][3]);
+        }
+    }
+    __syncthreads();
+  }
+  // ---- this split's result: m, l, acc = the eight warps' partial sums added in warp order ----
+  float *ex = reinterpret_cast<float *>(asm_raw);   // [8 warps][n_rep][128]: the codeword tables are no longer needed
+  float *pp = p.part + (((long long)b * p.G + g) * p.n_split + sp) * n_rep * kPartStride;
+#pragma unroll
+  for (int h = 0; h < HMAX; ++h)
+    if (h < n_rep) *reinterpret_cast<float4 *>(ex + ((warp * n_rep + h) * kHd) + 4 * lane) = make_float4(acc[h][0], acc[h][1], acc[h][2], acc[h][3]);
+  __syncthreads();
+  for (int e = tid; e < n_rep * kHd; e += kThreads) {
+    float sum = 0.0f;
+#pragma unroll
+    for (int w8 = 0; w8 < 8; ++w8) sum += ex[w8 * n_rep * kHd + e];
+    pp[(e >> 7) * kPartStride + 2 + (e & 127)] = sum;
+  }
+  if (tid < n_rep) { pp[tid * kPartStride] = m_run[tid]; pp[tid * kPartStride + 1] = l_run[tid]; }
+}
+
+// Merge the splits of one (sequence, query head) in split order.  grid = (Hq, B), block = 128.
+__global__ void __launch_bounds__(128) k_attn_combine(AttnParams p) {
+  const int hq = blockIdx.x, b = blockIdx.y, e = threadIdx.x;
+  const int g = hq / p.n_rep, h = hq - g * p.n_rep;
+  const float *pp = p.part + (((long long)b * p.G + g) * p.n_split) * p.n_rep * kPartStride + h * kPartStride;
+  const long long st = (long long)p.n_rep * kPartStride;
+  float M = -INFINITY;
+  for (int s = 0; s < p.n_split; ++s) M = fmaxf(M, pp[s * st]);
+  float L = 0.0f, o = 0.0f;
+  for (int s = 0; s < p.n_split; ++s) {
+    const float ms = pp[s * st];
+    const float w = (ms == -INFINITY) ? 0.0f : expf(ms - M);
+    L += pp[s * st + 1] * w;
+    o += pp[s * st + 2 + e] * w;
+  }
+  p.out[((long long)b * p.Hq + hq) * kHd + e] = (L > 0.0f) ? o / L : 0.0f;
+}
+
+}  // namespace attn
+}  // namespace gsrq
