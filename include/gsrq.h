@@ -193,6 +193,35 @@ int gsrq_init_ids(const void *kv, const gsrq_view *view, const float *residual,
                   const int64_t *fit_tokens, int64_t n_fit, int K, int stage, uint64_t seed,
                   int64_t *ids_out, void *workspace, size_t workspace_bytes, gsrq_stream_t stream);
 
+/* ---- variants ---- */
+
+/* Log-smoothed gradient weights (PAPER.md:192 Eq. 9; :434 Eq. 10): grad is a tensor laid out like the KV tensor it belongs to
+ * (view: dtype, G, T, hd, strides; d is ignored); per head g and token t  w = ||grad[g][t][:]||_2 (stored as fp32),
+ * lambda = tau / (median_t w + eps) (median per head; the mean of the two middle values for an even count),
+ * w_out[g][t] = log(1 + lambda w).  w_out: device [G][T] fp32 -- pass it to gsrq_fit_stage with w_stride_g = T. */
+int gsrq_log_weights(const void *grad, const gsrq_view *view, float tau, float eps, float *w_out, gsrq_stream_t stream);
+
+/* Per-vector gain codes (the alternative reading of "a codeword index plus a gain", reading c-G; BASELINE.json config 0):
+ * for each stage s < n_stages:  k = argmax_k r . s_k (lowest index on ties), gamma = fp16(max(0, r . s_k)),
+ * r <- fl32(r - fl32(fl32(gamma) s_k)).  Only the shapes of cb are used.  codes [S][G][T*M] uint8 and gains16 [S][G][T*M] IEEE half
+ * (as uint16) are written for the stages; residual [G][T*M][d] fp32 is a REQUIRED working buffer and holds the final residual.
+ * d in {8, 16, 32}.  workspace as for gsrq_assign (gsrq_workspace_bytes(view, K, S, 0)).  16/d extra bits per element per stage. */
+int gsrq_encode_pervector_gain(const void *kv, const gsrq_view *view, const gsrq_codebook *cb, int n_stages, uint8_t *codes,
+                               uint16_t *gains16, float *residual, void *workspace, size_t workspace_bytes, gsrq_stream_t stream);
+
+/* xhat = sum_{s < n_stages} fl32(gamma^(s) s^(s)_k), fp32 in stage order, one round-to-nearest-even cast to out_view->dtype. */
+int gsrq_decode_pervector_gain(const uint8_t *codes, const uint16_t *gains16, const gsrq_codebook *cb, int n_stages, void *kv_out,
+                               const gsrq_view *out_view, gsrq_stream_t stream);
+
+/* Nibble packing for K <= 16 (BASELINE.json config 0 "Codes are 4-bit indices"; "bit-packing"): each of the n_planes
+ * rows of N codes becomes ceil(N / 2) bytes, code 2i in the low nibble, code 2i + 1 in the high nibble.  Storage-side only. */
+int gsrq_pack_nibbles(const uint8_t *codes, int64_t n_planes, int64_t N, uint8_t *packed, gsrq_stream_t stream);
+int gsrq_unpack_nibbles(const uint8_t *packed, int64_t n_planes, int64_t N, uint8_t *codes, gsrq_stream_t stream);
+
+/* Per-subspace codebooks ("an independent codebook per subspace"): no separate entry point -- subspace m of a
+ * [G][T][hd] tensor is the view {G, T, hd' = d, d, stride_g, stride_t} on the pointer kv + m * d elements, and a head-inner
+ * [T][G][hd] tensor is ONE view with G' = G * M groups, hd' = d, stride_g' = d (tests/test_gpu_variants.py). */
+
 /* ---- decode fused into attention (PAPER.md:443 (ii), :445) ---- */
 
 /* Scratch of gsrq_attention_decode for B sequences of at most max_len tokens (host function, no CUDA calls). */

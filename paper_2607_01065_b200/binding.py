@@ -41,7 +41,8 @@ class gsrq_fit_stats(C.Structure):
 
 
 _lib = None
-EXPORTS = ["gsrq_attention_workspace_bytes", "gsrq_attention_decode", "gsrq_cluster_workspace_bytes", "gsrq_cluster_fit", "gsrq_cluster_assign", "gsrq_cluster_metrics", "gsrq_workspace_bytes", "gsrq_fit_stage", "gsrq_encode", "gsrq_decode", "gsrq_encode_append", "gsrq_assign", "gsrq_update",
+EXPORTS = ["gsrq_log_weights", "gsrq_encode_pervector_gain", "gsrq_decode_pervector_gain", "gsrq_pack_nibbles", "gsrq_unpack_nibbles",
+           "gsrq_attention_workspace_bytes", "gsrq_attention_decode", "gsrq_cluster_workspace_bytes", "gsrq_cluster_fit", "gsrq_cluster_assign", "gsrq_cluster_metrics", "gsrq_workspace_bytes", "gsrq_fit_stage", "gsrq_encode", "gsrq_decode", "gsrq_encode_append", "gsrq_assign", "gsrq_update",
            "gsrq_init_ids", "gsrq_debug_scores", "gsrq_encode_host", "gsrq_decode_host", "gsrq_pipeline_host", "gsrq_release_host_pool", "gsrq_profile_enable",
            "gsrq_profile_read", "gsrq_launch_count", "gsrq_last_error", "gsrq_version"]
 
@@ -173,6 +174,27 @@ def gsrq_attention_decode(q, k_codes, k_cb, k_stages, v_codes, v_cb, v_stages, p
                                        C.c_int64(plane_rows), _ptr(seq_start), _ptr(seq_len), C.c_int64(max_len), Bq, Hq, G, hd, d,
                                        C.c_float(scale), C.c_float(rope_theta), _ptr(out), _ptr(ws), C.c_size_t(ws.numel()), _stream()))
     return ws
+
+
+def gsrq_log_weights(grad, view, tau, eps, w_out):
+    _check(lib().gsrq_log_weights(_ptr(grad), C.byref(view), C.c_float(tau), C.c_float(eps), _ptr(w_out), _stream()))
+
+
+def gsrq_encode_pervector_gain(kv, view, cb, n_stages, codes, gains16, residual, ws):
+    _check(lib().gsrq_encode_pervector_gain(_ptr(kv), C.byref(view), C.byref(cb), n_stages, _ptr(codes), _ptr(gains16), _ptr(residual),
+                                            _ptr(ws), C.c_size_t(ws.numel()), _stream()))
+
+
+def gsrq_decode_pervector_gain(codes, gains16, cb, n_stages, kv_out, out_view):
+    _check(lib().gsrq_decode_pervector_gain(_ptr(codes), _ptr(gains16), C.byref(cb), n_stages, _ptr(kv_out), C.byref(out_view), _stream()))
+
+
+def gsrq_pack_nibbles(codes, n_planes, N, packed):
+    _check(lib().gsrq_pack_nibbles(_ptr(codes), C.c_int64(n_planes), C.c_int64(N), _ptr(packed), _stream()))
+
+
+def gsrq_unpack_nibbles(packed, n_planes, N, codes):
+    _check(lib().gsrq_unpack_nibbles(_ptr(packed), C.c_int64(n_planes), C.c_int64(N), _ptr(codes), _stream()))
 
 
 def cluster_workspace(N: int, d: int, K: int) -> torch.Tensor:

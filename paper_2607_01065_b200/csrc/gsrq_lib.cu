@@ -18,6 +18,7 @@
 #include "k_wide.cuh"
 #include "k_score_tc_wide.cuh"
 #include "k_attn.cuh"
+#include "k_variants.cuh"
 
 namespace gsrq {
 
@@ -1316,6 +1317,80 @@ int gsrq_attention_decode(const float *q, const uint8_t *k_codes, const gsrq_cod
 #undef GSRQ_ATTN
   GSRQ_CUDA_CHECK(cudaGetLastError());
   LAUNCH(kClsDecode, stream, (attn::k_attn_combine<<<dim3((unsigned)Hq, (unsigned)B), 128, 0, stream>>>(p)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  return GSRQ_OK;
+}
+
+int gsrq_log_weights(const void *grad, const gsrq_view *view, float tau, float eps, float *w_out, gsrq_stream_t stream_) {
+  cudaStream_t stream = (cudaStream_t)stream_;
+  if (!grad || !view || !w_out) { set_error("NULL input"); return GSRQ_EINVAL; }
+  if ((view->dtype != GSRQ_F32 && view->dtype != GSRQ_BF16) || view->G <= 0 || view->T <= 0 || view->hd <= 0) { set_error("bad view"); return GSRQ_EINVAL; }
+  if (!(tau > 0.0f) || eps < 0.0f) { set_error("tau must be > 0 and eps >= 0"); return GSRQ_EINVAL; }
+  dim3 grid((unsigned)((view->T + 7) / 8), (unsigned)view->G);
+  LAUNCH(kClsPrep, stream, (var::k_grad_norms<<<grid, 256, 0, stream>>>(grad, view->dtype, view->hd, view->T, view->stride_g, view->stride_t, w_out)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  LAUNCH(kClsPrep, stream, (var::k_log_weights<<<view->G, 1024, 0, stream>>>(w_out, view->T, (double)tau, (double)eps)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  return GSRQ_OK;
+}
+
+int gsrq_encode_pervector_gain(const void *kv, const gsrq_view *view, const gsrq_codebook *cb, int n_stages, uint8_t *codes, uint16_t *gains16,
+                               float *residual, void *workspace, size_t workspace_bytes, gsrq_stream_t stream_) {
+  cudaStream_t stream = (cudaStream_t)stream_;
+  if (!kv || !cb || !cb->shapes || !cb->gains || !codes || !gains16 || !residual) { set_error("NULL input (the fp32 residual buffer is required)"); return GSRQ_EINVAL; }
+  int rc = check_view(view, cb->K, cb->S);
+  if (rc) return rc;
+  if (is_wide(view->d)) { set_error("per-vector gain codes: d in {8, 16, 32}"); return GSRQ_EUNSUPPORTED; }
+  if (n_stages < 1 || n_stages > cb->S) { set_error("n_stages %d out of [1, %d]", n_stages, cb->S); return GSRQ_EINVAL; }
+  if ((rc = check_align16(kv, "kv")) || (rc = check_align16(residual, "residual"))) return rc;
+  const int G = view->G, d = view->d, M = view->hd / d;
+  const long long N = view->T * M;
+  for (int s = 0; s < n_stages; ++s) {
+    uint8_t *plane = codes + (size_t)s * G * N;
+    // shape of the stage: arg-max of the plain projection r . s_k (exact, lowest index on ties)
+    rc = gsrq_assign(kv, view, s ? residual : nullptr, cb, s, 1, plane, workspace, workspace_bytes, stream_);
+    if (rc) return rc;
+    var::PvgParams p{};
+    p.src = make_src(kv, view, s ? residual : nullptr, N); p.N = N; p.shapes = cb->shapes + (size_t)s * cb->K * d; p.cb_stride_g = (long long)cb->S * cb->K;
+    p.codes = plane; p.gains = reinterpret_cast<__half *>(gains16) + (size_t)s * G * N; p.res_out = residual;
+    dim3 grid((unsigned)((N + 255) / 256), (unsigned)G);
+    LAUNCH(kClsEncode, stream, DISPATCH_D(d, (var::k_pvg_finish<D><<<grid, 256, 0, stream>>>(p))));
+    GSRQ_CUDA_CHECK(cudaGetLastError());
+  }
+  return GSRQ_OK;
+}
+
+int gsrq_decode_pervector_gain(const uint8_t *codes, const uint16_t *gains16, const gsrq_codebook *cb, int n_stages, void *kv_out,
+                               const gsrq_view *out_view, gsrq_stream_t stream_) {
+  cudaStream_t stream = (cudaStream_t)stream_;
+  if (!codes || !gains16 || !cb || !cb->shapes || !kv_out) { set_error("NULL input"); return GSRQ_EINVAL; }
+  int rc = check_view(out_view, cb->K, cb->S);
+  if (rc) return rc;
+  if (is_wide(out_view->d)) { set_error("per-vector gain codes: d in {8, 16, 32}"); return GSRQ_EUNSUPPORTED; }
+  if (n_stages < 0 || n_stages > cb->S) { set_error("n_stages %d out of [0, %d]", n_stages, cb->S); return GSRQ_EINVAL; }
+  var::PvgDecParams p{};
+  p.codes = codes; p.gains = reinterpret_cast<const __half *>(gains16); p.shapes = cb->shapes; p.S = cb->S; p.K = cb->K; p.G = out_view->G;
+  p.n_stages = n_stages; p.M = out_view->hd / out_view->d; p.N = out_view->T * p.M; p.out = kv_out; p.dtype = out_view->dtype;
+  p.stride_g = out_view->stride_g; p.stride_t = out_view->stride_t;
+  dim3 grid((unsigned)((p.N + 255) / 256), (unsigned)out_view->G);
+  const int d = out_view->d;
+  LAUNCH(kClsDecode, stream, DISPATCH_D(d, (var::k_pvg_decode<D><<<grid, 256, 0, stream>>>(p))));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  return GSRQ_OK;
+}
+
+int gsrq_pack_nibbles(const uint8_t *codes, int64_t n_planes, int64_t N, uint8_t *packed, gsrq_stream_t stream_) {
+  cudaStream_t stream = (cudaStream_t)stream_;
+  if (!codes || !packed || n_planes <= 0 || N <= 0) { set_error("bad arguments"); return GSRQ_EINVAL; }
+  LAUNCH(kClsMisc, stream, (var::k_pack_nibbles<<<1184, 256, 0, stream>>>(codes, n_planes, N, packed)));
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  return GSRQ_OK;
+}
+
+int gsrq_unpack_nibbles(const uint8_t *packed, int64_t n_planes, int64_t N, uint8_t *codes, gsrq_stream_t stream_) {
+  cudaStream_t stream = (cudaStream_t)stream_;
+  if (!codes || !packed || n_planes <= 0 || N <= 0) { set_error("bad arguments"); return GSRQ_EINVAL; }
+  LAUNCH(kClsMisc, stream, (var::k_unpack_nibbles<<<1184, 256, 0, stream>>>(packed, n_planes, N, codes)));
   GSRQ_CUDA_CHECK(cudaGetLastError());
   return GSRQ_OK;
 }
