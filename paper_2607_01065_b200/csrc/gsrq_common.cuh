@@ -11,7 +11,6 @@ namespace gsrq {
 
 constexpr double kEps = 1e-12;   // y = r / (||r|| + eps)            PAPER.md:178, reading c-E
 constexpr double kDelta = 1e-8;  // "numerically close to zero"      PAPER.md:178, reading c-E
-constexpr int kChunkRows = 2048; // rows per reduction chunk (one CTA)
 constexpr uint64_t kGamma = 0x9E3779B97F4A7C15ULL;
 
 // Device-side statistics of one group (mirrors gsrq_fit_stats; slot 0 of changed[] is the

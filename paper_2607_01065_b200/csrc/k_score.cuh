@@ -3,7 +3,7 @@
 // Assignment (Eq. 5):  k_i = argmax_k (2 g_k r_i.s_k - g_k^2), lowest k on ties.
 // Strategy "filter + exact refine": a fast filter computes every score
 // with a rigorous per-row error bound E_i and keeps the top two; a row whose top-2 gap is
-// <= 2 E_i is appended to a list and re-scored by k_refine in fp64 with the operation order
+// <= 2 E_i is appended to a list and re-scored by k_encode_exact in fp64 with the operation order
 // of the definition.  The assignment therefore equals the exact-arithmetic arg-max and the
 // near-tie exemption of the parity protocol is never needed.
 #pragma once
