@@ -260,6 +260,85 @@ def run_append(B):
     return app
 
 
+def run_d128(B, pk):
+    """The paper's own operating point: D = 128, K = 256, R = 12 stages (0.75 bits per element) on a K-like
+    8 x 32768 x 128 bf16 layer: 12 fits (10 iterations, each followed by the prefix encode that feeds the next fit), the 12-stage
+    encode, the decode, and the tcgen05 scoring pass alone (per-class CUDA-event time of one encode)."""
+    G, T, hd, d, K, S, iters = 8, 32768, 128, 128, 256, 12, 10
+    x = torch.from_numpy(inputs.k_like(G, T, hd, inputs.seed_of(3, "k"))).to(torch.bfloat16).cuda()
+    w = torch.from_numpy(inputs.token_weights(T, inputs.seed_of(3, "w"))).cuda()
+    view = B.view_of(x, d)
+    sh = torch.zeros(G, S, K, d, device="cuda"); ga = torch.zeros(G, S, K, device="cuda")
+    cb = B.codebook_of(sh, ga); ws = B.workspace(view, K, S, 0)
+    codes = torch.zeros(S, G, T, dtype=torch.uint8, device="cuda")
+    res = torch.zeros(G, T, d, device="cuda"); out = torch.empty_like(x)
+
+    def fit_all():
+        for s in range(S):
+            B.gsrq_fit_stage(x, view, w, 0, None, cb, s, res if s else None, iters, 0, ws, want_stats=False)
+            B.gsrq_encode(x, view, cb, 0, s + 1, codes, res, ws)
+
+    fit_ms, fit_min = timed(fit_all, reps=3, warm=1)
+    enc_ms, enc_min = timed(lambda: B.gsrq_encode(x, view, cb, 0, S, codes, None, ws), reps=20)
+    dec_ms, dec_min = timed(lambda: B.gsrq_decode(codes, cb, S, out, view), reps=20)
+    B.gsrq_profile_enable(True)
+    B.gsrq_encode(x, view, cb, 0, S, codes, None, ws)
+    torch.cuda.synchronize()
+    prof = B.gsrq_profile_read()
+    B.gsrq_profile_enable(False)
+    rows = G * T
+    score_ms = prof["score"][0] / max(prof["score"][1], 1)
+    flops = 2.0 * K * d * rows
+    rel = float(((out.float() - x.float()) ** 2).sum() / (x.float() ** 2).sum())
+    return dict(workload="d128: k-cache-8x32768x128, D=128, K=256, R=12 (0.75 bit/element), 10 iterations, fit on all tokens",
+                fit_12_stages_with_prefix_encodes_ms=fit_ms, fit_ms_min=fit_min, encode_12_stages_ms=enc_ms, encode_ms_min=enc_min,
+                encode_kv_vectors_per_s=G * T / (enc_ms * 1e-3), encode_algorithmic_tflops=flops * S / (enc_ms * 1e-3) / 1e12,
+                decode_ms=dec_ms, decode_ms_min=dec_min, decode_gb_per_s=rows * (S + 2 * d) / (dec_ms * 1e-3) / 1e9,
+                scoring_pass=dict(kernel="tc::k_score_tc_wide<2> (tcgen05, SWIZZLE_128B operands)", ms_per_launch=score_ms,
+                                  algorithmic_tflops=flops / (score_ms * 1e-3) / 1e12,
+                                  frac_of_sustained_bf16_peak=flops / (score_ms * 1e-3) / 1e12 / pk["bf16_tflops_sustained"],
+                                  note="17 (stage 0, bf16-exact rows) or 25 (residual stages) M128xN256xK16 MMAs per 128-row tile for 8 "
+                                       "algorithmic ones: ncu tensor-pipe utilisation in profiles/r2_ncu_summaries.md"),
+                encode_ms_by_class={k: v[0] for k, v in prof.items() if v[1]}, rel_residual_energy=rel)
+
+
+def run_attention(B, pk):
+    """Decode fused into attention (PAPER.md:443 (ii)): one decoding step of LLaMA-3-8B-shaped GQA (32 query / 8 KV heads, head_dim 128)
+    straight from S = 2 GSRQ codes, for the batch / context pairs of the paper's latency tables."""
+    G, Hq, hd, d, K, S = 8, 32, 128, 16, 256, 2
+    outl = []
+    for Bq, ctx in ((8, 1024), (32, 1024), (1, 131072), (8, 131072)):
+        T = Bq * ctx
+        gen = torch.Generator(device="cuda"); gen.manual_seed(0)
+        kc = torch.randint(0, 256, (S, G, T * 8), dtype=torch.uint8, device="cuda", generator=gen)
+        vc = torch.randint(0, 256, (S, G, T * 8), dtype=torch.uint8, device="cuda", generator=gen)
+        sh = torch.nn.functional.normalize(torch.randn(G, S, K, d, device="cuda", generator=gen), dim=-1).contiguous()
+        ga = torch.rand(G, S, K, device="cuda", generator=gen).contiguous()
+        cb = B.codebook_of(sh, ga)
+        q = torch.randn(Bq, Hq, hd, device="cuda", generator=gen)
+        start = (torch.arange(Bq, device="cuda") * ctx).to(torch.int64)
+        length = torch.full((Bq,), ctx, dtype=torch.int64, device="cuda")
+        o_ = torch.zeros(Bq, Hq, hd, device="cuda")
+        for theta in (0.0, 500000.0):
+            ws = B.gsrq_attention_decode(q, kc, cb, S, vc, cb, S, T * 8, start, length, ctx, G, d, hd ** -0.5, theta, o_)
+            md, mn = timed(lambda: B.gsrq_attention_decode(q, kc, cb, S, vc, cb, S, T * 8, start, length, ctx, G, d, hd ** -0.5, theta, o_, ws), reps=20)
+            code_bytes = 2 * S * G * T * 8
+            outl.append(dict(batch=Bq, context=ctx, rope=theta > 0, us=md * 1e3, us_min=mn * 1e3, code_bytes=code_bytes,
+                             codes_gb_per_s=code_bytes / (md * 1e-3) / 1e9, frac_of_copy_bw_on_code_bytes=code_bytes / (md * 1e-3) / 1e9 / pk["hbm_gbs"],
+                             bf16_cache_bytes=2 * G * T * hd * 2, us_to_read_bf16_cache_at_copy_bw=2 * G * T * hd * 2 / (pk["hbm_gbs"] * 1e9) * 1e6))
+        del kc, vc
+        torch.cuda.empty_cache()
+    return outl
+
+
+def run_cluster(B):
+    """GSKM against the K-means baseline on x ~ N(0, I_D), N = 10,000 (Fig. 4): two points of each sweep."""
+    from paper_2607_01065_b200 import fig4_sweep
+    t0 = time.perf_counter()
+    rows = fig4_sweep.sweep(settings=[(128, 2048), (256, 2048), (256, 256)], iters=25)
+    return dict(seconds=time.perf_counter() - t0, rows=rows)
+
+
 # ------------------------------------------------------------------------------------------------ main
 def main():
     ap = argparse.ArgumentParser()
@@ -468,6 +547,10 @@ def main():
                 extras[f"cfg{cfg}_{kind}"] = run_small_cfg(B, pk, cfg, kind, flush)
                 torch.cuda.empty_cache()
         extras["append"] = run_append(B)
+        extras["d128"] = run_d128(B, pk)
+        torch.cuda.empty_cache()
+        extras["attention_decode"] = run_attention(B, pk)
+        extras["fig4_sweep_excerpt"] = run_cluster(B)
         line["extras"] = extras
     if not args.no_cpu_baseline:
         val, step_s, desc, cores = oracle_value(1)
