@@ -960,30 +960,26 @@ int gsrq_decode(const uint8_t *codes, const gsrq_codebook *cb, int n_stages, voi
     const long long need = (n_chunks + kDecThreads / 32 - 1) / (kDecThreads / 32);
     if (ctas > need) ctas = need;
     dim3 grid((unsigned)ctas, (unsigned)out_view->G);
-#define GSRQ_DEC_FAST(NS, DENSE)                                                                                          \
-  do {                                                                                                                    \
-    GSRQ_CUDA_CHECK(cudaFuncSetAttribute(k_decode_fast<NS, DENSE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-    LAUNCH(kClsDecode, stream, (k_decode_fast<NS, DENSE><<<grid, kDecThreads, smem, stream>>>(p, n_chunks)));                \
+    // output addressing: dense rows, or a (head, token) slice of 8 rows = 128 contiguous elements (head_dim 128), or anything else
+    const int layout = dense ? 1 : ((p.M == 8 && out_view->stride_t % 4 == 0) ? 2 : 0);
+    const bool bf16 = out_view->dtype == GSRQ_BF16;
+#define GSRQ_DEC_LAUNCH(NS, LAY, BF, DUPF)                                                                                          \
+  do {                                                                                                                              \
+    GSRQ_CUDA_CHECK(cudaFuncSetAttribute(k_decode_fast<NS, LAY, BF, DUPF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+    LAUNCH(kClsDecode, stream, (k_decode_fast<NS, LAY, BF, DUPF><<<grid, kDecThreads, smem, stream>>>(p, n_chunks)));                \
   } while (0)
-    if (deep) {
-      if (dense) {
-        GSRQ_CUDA_CHECK(cudaFuncSetAttribute(k_decode_fast<kDecDeep, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        LAUNCH(kClsDecode, stream, (k_decode_fast<kDecDeep, true, false><<<grid, kDecThreads, smem, stream>>>(p, n_chunks)));
-      } else {
-        GSRQ_CUDA_CHECK(cudaFuncSetAttribute(k_decode_fast<kDecDeep, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        LAUNCH(kClsDecode, stream, (k_decode_fast<kDecDeep, false, false><<<grid, kDecThreads, smem, stream>>>(p, n_chunks)));
-      }
-    } else
-    switch (n_stages * 2 + (dense ? 1 : 0)) {
-      case 2: GSRQ_DEC_FAST(1, false); break;
-      case 3: GSRQ_DEC_FAST(1, true); break;
-      case 4: GSRQ_DEC_FAST(2, false); break;
-      case 5: GSRQ_DEC_FAST(2, true); break;
-      case 6: GSRQ_DEC_FAST(3, false); break;
-      case 7: GSRQ_DEC_FAST(3, true); break;
-      case 8: GSRQ_DEC_FAST(4, false); break;
-      default: GSRQ_DEC_FAST(4, true); break;
-    }
+#define GSRQ_DEC_FAST(NS, DUPF)                                                                 \
+  do {                                                                                          \
+    if (layout == 1) { if (bf16) GSRQ_DEC_LAUNCH(NS, 1, true, DUPF); else GSRQ_DEC_LAUNCH(NS, 1, false, DUPF); }      \
+    else if (layout == 2) { if (bf16) GSRQ_DEC_LAUNCH(NS, 2, true, DUPF); else GSRQ_DEC_LAUNCH(NS, 2, false, DUPF); } \
+    else { if (bf16) GSRQ_DEC_LAUNCH(NS, 0, true, DUPF); else GSRQ_DEC_LAUNCH(NS, 0, false, DUPF); }                  \
+  } while (0)
+    if (deep) GSRQ_DEC_FAST(kDecDeep, false);
+    else if (n_stages == 1) GSRQ_DEC_FAST(1, true);
+    else if (n_stages == 2) GSRQ_DEC_FAST(2, true);
+    else if (n_stages == 3) GSRQ_DEC_FAST(3, true);
+    else GSRQ_DEC_FAST(4, true);
+#undef GSRQ_DEC_LAUNCH
 #undef GSRQ_DEC_FAST
     GSRQ_CUDA_CHECK(cudaGetLastError());
     p.row_begin = n_chunks * 256;

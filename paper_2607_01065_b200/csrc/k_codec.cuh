@@ -115,7 +115,10 @@ constexpr int kDecDeep = 12;             // stages of the single-copy variant (2
 // DUP = true : NS = number of stages (1..4), duplicated table rows (128 bytes), conflict-free.
 // DUP = false: NS = kDecDeep = upper bound, p.n_stages (5..kDecDeep) stages decoded; single-copy table rows (64 bytes:
 //              two codewords of equal parity in one LDS phase conflict 2-way) so that 12 stages fit in shared memory.
-template <int NS, bool DENSE, bool DUP = true>
+// LAYOUT: 0 = any strided view; 1 = dense ([G][N][16] contiguous per group); 2 = M == 8 (a (head, token) slice is 8 rows = 128
+// contiguous elements, e.g. head_dim 128 in either tensor layout): the warp's 8 rows of an iteration are one token.
+// BF16: output dtype fixed at compile time (bf16 / fp32) so that the inner loop carries no dtype branch.
+template <int NS, int LAYOUT, bool BF16, bool DUP = true>
 __global__ void __launch_bounds__(kDecThreads) k_decode_fast(DecParams p, long long n_chunks) {
   extern __shared__ __align__(16) float tab[];
   constexpr int RS = DUP ? 32 : 16;  // floats per table row
@@ -135,15 +138,18 @@ __global__ void __launch_bounds__(kDecThreads) k_decode_fast(DecParams p, long l
   const float *tl = tab + (DUP ? (lane & 7) : (lane & 3)) * 4;
   const int msh = ((p.M & (p.M - 1)) == 0) ? (31 - __clz(p.M)) : -1;
   const long long ch0 = (long long)blockIdx.x * (kDecThreads / 32) + warp, chs = (long long)gridDim.x * (kDecThreads / 32);
-  // lane l holds the 8 code bytes of rows 8l..8l+7 of the chunk (one coalesced 256-byte load per stage),
-  // loaded one chunk ahead; iteration u decodes rows 8u..8u+7 (slot = row within the 8), whose codes
-  // sit in lane u: two shuffles per stage.  Every store instruction writes 256 contiguous bytes (bf16).
+  // lane l holds the 8 code bytes of rows 8l..8l+7 of the chunk (one coalesced 256-byte load per stage), loaded one chunk ahead;
+  // iteration u decodes rows 8u..8u+7 (slot = row within the 8), whose codes sit in lane u: two shuffles and a byte permute per
+  // stage (a shared-memory strip of the code bytes instead of the shuffles was measured: no faster).  Every store instruction
+  // writes 256 contiguous bytes (bf16).
   uint2 nx[NS];
   if (ch0 < n_chunks) {
 #pragma unroll
     for (int s = 0; s < NS; ++s)
       if (s < ns) nx[s] = __ldcs(reinterpret_cast<const uint2 *>(p.codes + ((long long)s * p.G + g) * p.N + ch0 * 256) + lane);
   }
+  uint16_t *out16 = reinterpret_cast<uint16_t *>(p.out) + (long long)g * p.stride_g;
+  float *out32 = reinterpret_cast<float *>(p.out) + (long long)g * p.stride_g;
   for (long long ch = ch0; ch < n_chunks; ch += chs) {
     uint2 cw[NS];
 #pragma unroll
@@ -153,14 +159,17 @@ __global__ void __launch_bounds__(kDecThreads) k_decode_fast(DecParams p, long l
       for (int s = 0; s < NS; ++s)
         if (s < ns) nx[s] = __ldcs(reinterpret_cast<const uint2 *>(p.codes + ((long long)s * p.G + g) * p.N + (ch + chs) * 256) + lane);
     }
+    // element offset of this lane's 4 values in iteration 0 and the step per iteration (LAYOUT 1 / 2: both warp-uniform + 4 lane)
+    long long off0 = 0, step = 0;
+    if (LAYOUT == 1) { off0 = ch * 4096 + lane * 4; step = 128; }
+    if (LAYOUT == 2) { off0 = ch * 32 * p.stride_t + lane * 4; step = p.stride_t; }
 #pragma unroll 8
     for (int u = 0; u < 32; ++u) {
       float4 acc;
 #pragma unroll
       for (int s = 0; s < NS; ++s) {
         if (s >= ns) break;
-        const uint32_t lo = __shfl_sync(0xffffffffu, cw[s].x, u), hi = __shfl_sync(0xffffffffu, cw[s].y, u);
-        const uint32_t k = (((slot & 4) ? hi : lo) >> (8 * (slot & 3))) & 0xFFu;
+        const uint32_t k = __byte_perm(__shfl_sync(0xffffffffu, cw[s].x, u), __shfl_sync(0xffffffffu, cw[s].y, u), slot) & 0xFFu;
         const float4 c = *reinterpret_cast<const float4 *>(tl + ((size_t)s * 256 + k) * RS);
         if (s == 0) acc = c;
         else {
@@ -168,20 +177,16 @@ __global__ void __launch_bounds__(kDecThreads) k_decode_fast(DecParams p, long l
           acc.z = __fadd_rn(acc.z, c.z); acc.w = __fadd_rn(acc.w, c.w);
         }
       }
-      const long long i = ch * 256 + u * 8 + slot;
       long long off;
-      if (DENSE) {
-        off = (long long)g * p.stride_g + i * 16 + c4 * 4;
-      } else {
+      if (LAYOUT == 0) {
+        const long long i = ch * 256 + u * 8 + slot;
         const long long tok = (msh >= 0) ? (i >> msh) : (i / p.M);
-        off = (long long)g * p.stride_g + tok * p.stride_t + (i - tok * p.M) * 16 + c4 * 4;
-      }
-      if (p.dtype == GSRQ_BF16) {
-        __stcs(reinterpret_cast<uint2 *>(reinterpret_cast<uint16_t *>(p.out) + off),
-               make_uint2(pack_bf16x2(acc.x, acc.y), pack_bf16x2(acc.z, acc.w)));
+        off = tok * p.stride_t + (i - tok * p.M) * 16 + c4 * 4;
       } else {
-        __stcs(reinterpret_cast<float4 *>(reinterpret_cast<float *>(p.out) + off), acc);
+        off = off0 + u * step;
       }
+      if (BF16) __stcs(reinterpret_cast<uint2 *>(out16 + off), make_uint2(pack_bf16x2(acc.x, acc.y), pack_bf16x2(acc.z, acc.w)));
+      else __stcs(reinterpret_cast<float4 *>(out32 + off), acc);
     }
   }
 }
