@@ -29,7 +29,10 @@ constexpr uint32_t kEncSmemOnes = kEncMaxS * 3 * kBImgBytes;                 // 
 constexpr uint32_t kEncSmemA = kEncSmemOnes + kPlaneBytes;                   // ring of kEncStages tiles
 constexpr uint32_t kEncSmemP = kEncSmemA + kEncStages * kPlaneBytes;         // residual planes [2 buffers][hi, lo]
 constexpr uint32_t kEncSmemBar = kEncSmemP + 4 * kPlaneBytes;
-constexpr uint32_t kEncSmemTotal = kEncSmemBar + 256 + 1024;                 // + alignment slack
+constexpr uint32_t kEncSmemCb = kEncSmemBar + 256;                           // fp32 codebook of the pass's stages: [stage]{shapes [256][16], gains [256]}
+constexpr uint32_t kEncCbStage = kN * kD * 4 + kN * 4;
+constexpr uint32_t kEncSmemTotal = kEncSmemCb + kEncMaxS * kEncCbStage + 1024;   // + alignment slack
+static_assert(kEncSmemTotal <= 227 * 1024, "shared-memory budget");
 
 struct EncTcParams {
   const uint8_t *bimg;     // [G][n_stages][3][8192] operand images (mode 0)
@@ -155,6 +158,19 @@ __global__ void __launch_bounds__(kThreads, 1) k_encode_tc(const __grid_constant
     const int r_in_tile = q * 32 + lane;
     uint8_t *planes = sgen + kEncSmemP + (2 * wg) * kPlaneBytes;
     const uint32_t sw = ((uint32_t)(r_in_tile >> 2) & 1u) << 4;  // SWIZZLE_32B: the two 16-byte chunks of a row swap
+    // the fp32 codebook of the pass's stages -> shared memory: the gain (decision margin) and the codeword (subtraction) of a row's
+    // winner sit on the critical path between a tile's stages, and a global load there costs ten times a shared-memory one
+    {
+      const int et = threadIdx.x - 64;  // 0..255
+      for (int s = 0; s < S; ++s) {
+        float *cbs = reinterpret_cast<float *>(sgen + kEncSmemCb + s * kEncCbStage);
+        const long long c0 = ((long long)g * p.S + p.s0 + s) * p.K;
+        const float4 *src = reinterpret_cast<const float4 *>(p.shapes + c0 * kD);
+        for (int e = et; e < p.K * (kD / 4); e += 256) reinterpret_cast<float4 *>(cbs)[e] = __ldg(src + e);
+        if (et < p.K) cbs[kN * kD + et] = __ldg(p.gains + c0 + et);
+      }
+      asm volatile("bar.sync 1, 256;" ::: "memory");
+    }
     for (int it = wg; it < n_my; it += 2) {
       const int pr = it >> 1;
       const int st = it % kEncStages, ph = (it / kEncStages) & 1;
@@ -227,8 +243,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_encode_tc(const __grid_constant
           }
         });
         const int k = gi * 16 + ji;
-        const long long cw = ((long long)g * p.S + p.s0 + s) * p.K + min(k, p.K - 1);
-        const float gk = __ldg(p.gains + cw);
+        const float *cbs = reinterpret_cast<const float *>(sgen + kEncSmemCb + s * kEncCbStage);
+        const int kc = min(k, p.K - 1);
+        const float gk = cbs[kN * kD + kc];
         const float E2 = decision_margin(best, rn, gk, gm, rho17, 0);
         if (alive && best - second <= E2) {  // ambiguous: the exact path takes the row over from this stage
           const uint32_t gmask = candidate_groups(gmA, best, E2);  // groups of 16 columns within the margin: the only candidates
@@ -239,11 +256,11 @@ __global__ void __launch_bounds__(kThreads, 1) k_encode_tc(const __grid_constant
           alive = false;
         }
         if (alive && p.codes) p.codes[(long long)(p.s0 + s) * p.code_stride_s + gr] = (uint8_t)k;
-        // r <- fl32(r - fl32(g_k s_k)): the codeword comes from the fp32 codebook (L1-resident)
-        const float4 *sp = reinterpret_cast<const float4 *>(p.shapes + cw * kD);
+        // r <- fl32(r - fl32(g_k s_k)): the codeword comes from the fp32 codebook in shared memory
+        const float4 *sp = reinterpret_cast<const float4 *>(cbs + kc * kD);
 #pragma unroll
         for (int v = 0; v < 4; ++v) {
-          const float4 sv = __ldg(sp + v);
+          const float4 sv = sp[v];
           r[4 * v] = __fsub_rn(r[4 * v], __fmul_rn(gk, sv.x));
           r[4 * v + 1] = __fsub_rn(r[4 * v + 1], __fmul_rn(gk, sv.y));
           r[4 * v + 2] = __fsub_rn(r[4 * v + 2], __fmul_rn(gk, sv.z));
