@@ -42,8 +42,9 @@ __host__ __device__ inline size_t attn_smem_bytes(int k_stages, int v_stages, in
   size_t b = (size_t)v_stages * 256 * kD * 4;                                 // value codeword table
   b += rope ? ((size_t)k_stages * 256 * kD * 4 + (size_t)n_rep * kHd * 4 + 64 * 64 * 8 + 64 * 8)   // key table, q, offset / base rotations
             : (size_t)((n_rep + 3) & ~3) * k_stages * kM * 256 * 4;           // q . codeword tables (heads innermost, padded to 4)
-  b += (size_t)(n_rep * ch > kHd ? n_rep * ch : kHd) * 4;                     // logits / probabilities of the chunk (also the final exchange buffer)
-  b += (size_t)ch * kM * (size_t)v_stages;                                    // the chunk's value codes
+  const int hp = (n_rep + 3) & ~3;
+  b += (size_t)(hp * ch > n_rep * kHd ? hp * ch : n_rep * kHd) * 4;           // logits / probabilities of the chunk [token][head], first the staged q
+  b += (size_t)ch * kM * (size_t)(v_stages == 3 ? 4 : v_stages);              // the chunk's value codes [token][m][stage]
   b += 3 * 8 * 4 + 16;                                                        // running max, sum, rescale per head
   return (b + 15) & ~(size_t)15;
 }
@@ -65,8 +66,9 @@ __global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
   const int HP = (n_rep + 3) & ~3;                                      // heads padded to a multiple of 4
   float *qt = ktab;                                                     // [SK][8][256][HP]
   float *lg = ROPE ? reinterpret_cast<float *>(cs_base + 64) : qt + HP * SK * kM * 256;
-  uint8_t *vcodes = reinterpret_cast<uint8_t *>(lg + (n_rep * CH > kHd ? n_rep * CH : kHd));   // [SV][CH][8]
-  float *m_run = reinterpret_cast<float *>(vcodes + ((CH * kM * SV + 15) & ~15));
+  const int SVP = SV == 3 ? 4 : SV;                                     // stages of one (token, m) side by side, padded to 1 / 2 / 4 bytes
+  uint8_t *vcodes = reinterpret_cast<uint8_t *>(lg + (HP * CH > n_rep * kHd ? HP * CH : n_rep * kHd));   // [CH][8][SVP]
+  float *m_run = reinterpret_cast<float *>(vcodes + ((CH * kM * SVP + 15) & ~15));
   float *l_run = m_run + 8, *sc_h = l_run + 8;
 
   const long long t_seq0 = p.seq_start[b], len = p.seq_len[b];
@@ -127,12 +129,27 @@ __global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
 
   for (long long t0 = tb; t0 < te; t0 += CH) {
     const int nv = (int)min((long long)CH, te - t0);   // valid tokens of the chunk
-    // the chunk's value codes -> shared memory (coalesced 8-byte loads)
-    for (int e = tid; e < SV * CH; e += kThreads) {
-      const int s = e / CH, t = e - s * CH;
-      uint2 v = make_uint2(0u, 0u);
-      if (t < nv) v = *reinterpret_cast<const uint2 *>(p.vc + ((long long)s * p.G + g) * p.plane_rows + (t_seq0 + t0 + t) * kM);
-      reinterpret_cast<uint2 *>(vcodes)[e] = v;
+    // the chunk's value codes -> shared memory (coalesced 8-byte loads), the stages of one sub-vector side by side
+    if (NS == 2) {
+      for (int t = tid; t < CH; t += kThreads) {
+        uint2 a = make_uint2(0u, 0u), c = make_uint2(0u, 0u);
+        if (t < nv) {
+          a = *reinterpret_cast<const uint2 *>(p.vc + ((long long)g) * p.plane_rows + (t_seq0 + t0 + t) * kM);
+          c = *reinterpret_cast<const uint2 *>(p.vc + ((long long)p.G + g) * p.plane_rows + (t_seq0 + t0 + t) * kM);
+        }
+        reinterpret_cast<uint4 *>(vcodes)[t] = make_uint4(__byte_perm(a.x, c.x, 0x5140), __byte_perm(a.x, c.x, 0x7362),
+                                                          __byte_perm(a.y, c.y, 0x5140), __byte_perm(a.y, c.y, 0x7362));
+      }
+    } else {
+      for (int e = tid; e < SV * CH; e += kThreads) {
+        const int s = e / CH, t = e - s * CH;
+        uint2 v = make_uint2(0u, 0u);
+        if (t < nv) v = *reinterpret_cast<const uint2 *>(p.vc + ((long long)s * p.G + g) * p.plane_rows + (t_seq0 + t0 + t) * kM);
+        if (SVP == 1) reinterpret_cast<uint2 *>(vcodes)[t] = v;
+        else
+#pragma unroll
+          for (int m = 0; m < kM; ++m) vcodes[(t * kM + m) * SVP + s] = (uint8_t)(((m < 4 ? v.x : v.y) >> (8 * (m & 3))) & 255u);
+      }
     }
     // ---- logits ----
     if (!ROPE) {
@@ -161,8 +178,10 @@ __global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
           }
         }
 #pragma unroll
-        for (int h = 0; h < HMAX; ++h)
-          if (h < n_rep) lg[h * CH + t] = sum[h] * p.scale;
+        for (int h4 = 0; h4 < (HMAX + 3) / 4; ++h4)
+          if (4 * h4 < n_rep)
+            *reinterpret_cast<float4 *>(lg + t * HP + 4 * h4) =
+                make_float4(sum[4 * h4] * p.scale, sum[4 * h4 + 1] * p.scale, sum[4 * h4 + 2] * p.scale, sum[4 * h4 + 3] * p.scale);
       }
     } else {
       if (tid < 64) {   // rotation by (first position of the chunk) x theta_i, in double
@@ -211,7 +230,7 @@ __global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
           float v = part[h];
           v += __shfl_xor_sync(0xffffffffu, v, 1);
           v += __shfl_xor_sync(0xffffffffu, v, 2);
-          if (mq == 0 && t < nv) lg[h * CH + t] = v * p.scale;
+          if (mq == 0 && t < nv) lg[t * HP + h] = v * p.scale;
         }
       }
     }
@@ -220,13 +239,13 @@ __global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
     if (warp < n_rep) {
       const int h = warp;
       float mx = -INFINITY;
-      for (int t = lane; t < nv; t += 32) mx = fmaxf(mx, lg[h * CH + t]);
+      for (int t = lane; t < nv; t += 32) mx = fmaxf(mx, lg[t * HP + h]);
       for (int off = 16; off; off >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, off));
       const float m_old = m_run[h], m_new = fmaxf(m_old, mx);
       float sum = 0.0f;
       for (int t = lane; t < CH; t += 32) {
-        const float pr = (t < nv) ? expf(lg[h * CH + t] - m_new) : 0.0f;
-        lg[h * CH + t] = pr;
+        const float pr = (t < nv) ? expf(lg[t * HP + h] - m_new) : 0.0f;
+        lg[t * HP + h] = pr;
         sum += pr;
       }
       for (int off = 16; off; off >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, off);
@@ -244,36 +263,45 @@ __global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
       if (h < n_rep) { const float sc = sc_h[h]; acc[h][0] *= sc; acc[h][1] *= sc; acc[h][2] *= sc; acc[h][3] *= sc; }
     auto value_of = [&](int t) -> float4 {   // vhat_t[4 lane .. 4 lane + 3] = sum over the stages, fp32, stage order
       float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+      const uint8_t *cp = vcodes + (t * kM + m_out) * SVP;
+      unsigned cw;                            // the stages' code bytes of this lane's sub-vector, one load
+      if (NS == 1) cw = *cp;
+      else if (NS == 2) cw = *reinterpret_cast<const unsigned short *>(cp);
+      else if (SVP == 4) cw = *reinterpret_cast<const unsigned *>(cp);
+      else if (SVP == 2) cw = *reinterpret_cast<const unsigned short *>(cp);
+      else cw = *cp;
 #pragma unroll
       for (int s = 0; s < (NS > 0 ? NS : 4); ++s) {
         if (s >= SV) break;
-        const float4 c = *reinterpret_cast<const float4 *>(vtab + (s * 256 + vcodes[(s * CH + t) * kM + m_out]) * kD + j_out);
+        const float4 c = *reinterpret_cast<const float4 *>(vtab + (s * 256 + ((cw >> (8 * s)) & 255u)) * kD + j_out);
         if (s == 0) v = c;
         else { v.x = __fadd_rn(v.x, c.x); v.y = __fadd_rn(v.y, c.y); v.z = __fadd_rn(v.z, c.z); v.w = __fadd_rn(v.w, c.w); }
       }
       return v;
     };
+    auto add_token = [&](int t, const float4 &v) {   // acc_h += p_h(t) vhat_t: the token's probabilities as float4 broadcasts
+#pragma unroll
+      for (int h4 = 0; h4 < (HMAX + 3) / 4; ++h4) {
+        if (4 * h4 >= n_rep) break;
+        const float4 pr = *reinterpret_cast<const float4 *>(lg + t * HP + 4 * h4);
+        const float pv[4] = {pr.x, pr.y, pr.z, pr.w};
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const int h = 4 * h4 + i;
+          if (h < HMAX && h < n_rep) {
+            acc[h][0] = fmaf(pv[i], v.x, acc[h][0]); acc[h][1] = fmaf(pv[i], v.y, acc[h][1]);
+            acc[h][2] = fmaf(pv[i], v.z, acc[h][2]); acc[h][3] = fmaf(pv[i], v.w, acc[h][3]);
+          }
+        }
+      }
+    };
     int t = warp;
     for (; t + 8 < nv; t += 16) {   // two tokens in flight
       const float4 v0 = value_of(t), v1 = value_of(t + 8);
-#pragma unroll
-      for (int h = 0; h < HMAX; ++h)
-        if (h < n_rep) {
-          const float p0 = lg[h * CH + t], p1 = lg[h * CH + t + 8];
-          acc[h][0] = fmaf(p1, v1.x, fmaf(p0, v0.x, acc[h][0])); acc[h][1] = fmaf(p1, v1.y, fmaf(p0, v0.y, acc[h][1]));
-          acc[h][2] = fmaf(p1, v1.z, fmaf(p0, v0.z, acc[h][2])); acc[h][3] = fmaf(p1, v1.w, fmaf(p0, v0.w, acc[h][3]));
-        }
+      add_token(t, v0);
+      add_token(t + 8, v1);
     }
-    for (; t < nv; t += 8) {
-      const float4 v = value_of(t);
-#pragma unroll
-      for (int h = 0; h < HMAX; ++h)
-        if (h < n_rep) {
-          const float p0 = lg[h * CH + t];
-          acc[h][0] = fmaf(p0, v.x, acc[h][0]); acc[h][1] = fmaf(p0, v.y, acc[h][1]);
-          acc[h][2] = fmaf(p0, v.z, acc[h][2]); acc[h][3] = fmaf(p0, v.w, acc[h][3]);
-        }
-    }
+    for (; t < nv; t += 8) add_token(t, value_of(t));
     __syncthreads();
   }
   // ---- this split's result: m, l, acc = the eight warps' partial sums added in warp order ----
