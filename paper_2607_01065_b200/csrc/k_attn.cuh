@@ -38,7 +38,7 @@ struct AttnParams {
 };
 
 __host__ __device__ inline size_t attn_smem_bytes(int k_stages, int v_stages, int n_rep, bool rope) {
-  const int ch = rope ? 64 : 256;
+  const int ch = rope ? 64 : 512;
   size_t b = (size_t)v_stages * 256 * kD * 4;                                 // value codeword table
   b += rope ? ((size_t)k_stages * 256 * kD * 4 + (size_t)n_rep * kHd * 4 + 64 * 64 * 8 + 64 * 8)   // key table, q, offset / base rotations
             : (size_t)((n_rep + 3) & ~3) * k_stages * kM * 256 * 4;           // q . codeword tables (heads innermost, padded to 4)
@@ -54,7 +54,7 @@ __host__ __device__ inline size_t attn_smem_bytes(int k_stages, int v_stages, in
 template <bool ROPE, int NREP, int NS>
 __global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
   extern __shared__ __align__(16) uint8_t asm_raw[];
-  constexpr int CH = ROPE ? 64 : 256;
+  constexpr int CH = ROPE ? 64 : 512;
   constexpr int HMAX = NREP > 0 ? NREP : 8;
   const int sp = blockIdx.x, g = blockIdx.y, b = blockIdx.z, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int n_rep = NREP > 0 ? NREP : p.n_rep, SK = NS > 0 ? NS : p.k_stages, SV = NS > 0 ? NS : p.v_stages;
@@ -153,8 +153,7 @@ __global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
     }
     // ---- logits ----
     if (!ROPE) {
-      const int t = tid;
-      if (t < nv) {
+      for (int t = tid; t < nv; t += kThreads) {
         float sum[(HMAX + 3) & ~3];
 #pragma unroll
         for (int h = 0; h < ((HMAX + 3) & ~3); ++h) sum[h] = 0.0f;
