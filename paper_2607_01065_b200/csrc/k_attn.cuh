@@ -38,13 +38,14 @@ struct AttnParams {
 };
 
 __host__ __device__ inline size_t attn_smem_bytes(int k_stages, int v_stages, int n_rep, bool rope) {
-  const int ch = rope ? 64 : 512;
+  const int ch = rope ? 256 : 512;
   size_t b = (size_t)v_stages * 256 * kD * 4;                                 // value codeword table
-  b += rope ? ((size_t)k_stages * 256 * kD * 4 + (size_t)n_rep * kHd * 4 + 64 * 64 * 8 + 64 * 8)   // key table, q, offset / base rotations
+  b += rope ? ((size_t)k_stages * 256 * kD * 4 + 64 * 64 * 8 + 4 * 64 * 8)    // key table, offset / base rotations
             : (size_t)((n_rep + 3) & ~3) * k_stages * kM * 256 * 4;           // q . codeword tables (heads innermost, padded to 4)
   const int hp = (n_rep + 3) & ~3;
   b += (size_t)(hp * ch > n_rep * kHd ? hp * ch : n_rep * kHd) * 4;           // logits / probabilities of the chunk [token][head], first the staged q
   b += (size_t)ch * kM * (size_t)(v_stages == 3 ? 4 : v_stages);              // the chunk's value codes [token][m][stage]
+  if (rope) b += (size_t)ch * kM * (size_t)k_stages;                          // and key codes [stage][token][m]
   b += 3 * 8 * 4 + 16;                                                        // running max, sum, rescale per head
   return (b + 15) & ~(size_t)15;
 }
@@ -54,21 +55,21 @@ __host__ __device__ inline size_t attn_smem_bytes(int k_stages, int v_stages, in
 template <bool ROPE, int NREP, int NS>
 __global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
   extern __shared__ __align__(16) uint8_t asm_raw[];
-  constexpr int CH = ROPE ? 64 : 512;
+  constexpr int CH = ROPE ? 256 : 512;
   constexpr int HMAX = NREP > 0 ? NREP : 8;
   const int sp = blockIdx.x, g = blockIdx.y, b = blockIdx.z, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int n_rep = NREP > 0 ? NREP : p.n_rep, SK = NS > 0 ? NS : p.k_stages, SV = NS > 0 ? NS : p.v_stages;
   float *vtab = reinterpret_cast<float *>(asm_raw);
   float *ktab = vtab + SV * 256 * kD;                                   // ROPE: key table; else the q . codeword tables
-  float *qs = ktab + SK * 256 * kD;                                     // ROPE only
-  float2 *cs_off = reinterpret_cast<float2 *>(qs + n_rep * kHd);        // [64 offsets][64 frequencies]
-  float2 *cs_base = cs_off + 64 * 64;                                   // [64]
+  float2 *cs_off = reinterpret_cast<float2 *>(ktab + SK * 256 * kD);    // ROPE only: [64 offsets][64 frequencies]
+  float2 *cs_base = cs_off + 64 * 64;                                   // [4 sub-chunks of 64 tokens][64]
   const int HP = (n_rep + 3) & ~3;                                      // heads padded to a multiple of 4
   float *qt = ktab;                                                     // [SK][8][256][HP]
-  float *lg = ROPE ? reinterpret_cast<float *>(cs_base + 64) : qt + HP * SK * kM * 256;
+  float *lg = ROPE ? reinterpret_cast<float *>(cs_base + 4 * 64) : qt + HP * SK * kM * 256;
   const int SVP = SV == 3 ? 4 : SV;                                     // stages of one (token, m) side by side, padded to 1 / 2 / 4 bytes
   uint8_t *vcodes = reinterpret_cast<uint8_t *>(lg + (HP * CH > n_rep * kHd ? HP * CH : n_rep * kHd));   // [CH][8][SVP]
-  float *m_run = reinterpret_cast<float *>(vcodes + ((CH * kM * SVP + 15) & ~15));
+  uint2 *kcodes = reinterpret_cast<uint2 *>(vcodes + ((CH * kM * SVP + 15) & ~15));   // ROPE only: [SK][CH]
+  float *m_run = reinterpret_cast<float *>(reinterpret_cast<uint8_t *>(kcodes) + (ROPE ? CH * kM * SK : 0));
   float *l_run = m_run + 8, *sc_h = l_run + 8;
 
   const long long t_seq0 = p.seq_start[b], len = p.seq_len[b];
@@ -91,7 +92,6 @@ __global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
       const long long cb = ((long long)g * p.kS + s) * p.kK + k;
       ktab[e] = (k < p.kK) ? __fmul_rn(p.k_gains[cb], p.k_shapes[cb * kD + (r & 15)]) : 0.0f;
     }
-    for (int e = tid; e < n_rep * kHd; e += kThreads) qs[e] = qg[e];
     for (int e = tid; e < 64 * 64; e += kThreads) {   // rotation by (offset within the chunk) x theta_i, in double
       const int off = e >> 6, i = e & 63;
       double sn, cs;
@@ -118,6 +118,17 @@ __global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
           qt[((s * kM + m) * 256 + k) * HP + h] = a;
         }
     }
+  }
+  float qa[ROPE ? HMAX : 1][4], qb[ROPE ? HMAX : 1][4];   // ROPE: this thread's q elements (pairs i, i + 64) of every head
+  if (ROPE) {
+    const int i0 = ((tid & 15) >> 2) * kD + (tid & 3) * 4;
+#pragma unroll
+    for (int h = 0; h < HMAX; ++h)
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        qa[ROPE ? h : 0][e] = (h < n_rep) ? qg[h * kHd + i0 + e] : 0.0f;
+        qb[ROPE ? h : 0][e] = (h < n_rep) ? qg[h * kHd + 64 + i0 + e] : 0.0f;
+      }
   }
   if (tid < 8) { m_run[tid] = -INFINITY; l_run[tid] = 0.0f; sc_h[tid] = 0.0f; }
   // values: warp w takes the tokens t = w (mod 8) of a chunk, lane l the output elements 4 l .. 4 l + 3
@@ -151,6 +162,13 @@ __global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
           for (int m = 0; m < kM; ++m) vcodes[(t * kM + m) * SVP + s] = (uint8_t)(((m < 4 ? v.x : v.y) >> (8 * (m & 3))) & 255u);
       }
     }
+    if (ROPE)
+      for (int e = tid; e < SK * CH; e += kThreads) {
+        const int s = e / CH, t = e - s * CH;
+        uint2 v = make_uint2(0u, 0u);
+        if (t < nv) v = *reinterpret_cast<const uint2 *>(p.kc + ((long long)s * p.G + g) * p.plane_rows + (t_seq0 + t0 + t) * kM);
+        kcodes[e] = v;
+      }
     // ---- logits ----
     if (!ROPE) {
       for (int t = tid; t < nv; t += kThreads) {
@@ -183,53 +201,77 @@ __global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
                 make_float4(sum[4 * h4] * p.scale, sum[4 * h4 + 1] * p.scale, sum[4 * h4 + 2] * p.scale, sum[4 * h4 + 3] * p.scale);
       }
     } else {
-      if (tid < 64) {   // rotation by (first position of the chunk) x theta_i, in double
+      // Thread = (token slot tid / 16, rotary sub-vector pair mq, quad jq): the pairs i = 16 mq + 4 jq + e and i + 64, e < 4, of the
+      // tokens slot, slot + 16, ... of each 64-token sub-chunk; its 8 q elements per head stay in registers for the whole CTA.
+      {   // rotation by (first position of each sub-chunk) x theta_i, in double
+        const int sub = tid >> 6, i = tid & 63;
         double sn, cs;
-        sincos((double)t0 * pow((double)p.rope_theta, -(double)tid / 64.0), &sn, &cs);
+        sincos((double)(t0 + 64 * sub) * pow((double)p.rope_theta, -(double)i / 64.0), &sn, &cs);
         cs_base[tid] = make_float2((float)cs, (float)sn);
       }
       __syncthreads();
-      const int t = tid >> 2, mq = tid & 3;   // token of the chunk, rotary pair of sub-vectors (mq, mq + 4)
-      float part[HMAX];
+      const int l16 = tid & 15, slot = tid >> 4, mq = l16 >> 2, i0 = mq * kD + (l16 & 3) * 4;
+#pragma unroll 1
+      for (int sub = 0; sub < CH / 64; ++sub) {
+        if (sub * 64 >= nv) break;
+        float2 cb[4];
+        {
+          const float4 b0 = *reinterpret_cast<const float4 *>(cs_base + sub * 64 + i0), b1 = *reinterpret_cast<const float4 *>(cs_base + sub * 64 + i0 + 2);
+          cb[0] = make_float2(b0.x, b0.y); cb[1] = make_float2(b0.z, b0.w); cb[2] = make_float2(b1.x, b1.y); cb[3] = make_float2(b1.z, b1.w);
+        }
 #pragma unroll
-      for (int h = 0; h < HMAX; ++h) part[h] = 0.0f;
-      if (t < nv) {
-        float a[kD], bb[kD];
+        for (int it = 0; it < 4; ++it) {
+          const int off = it * 16 + slot, t = sub * 64 + off;
+          const bool ok = t < nv;
+          float a[4] = {0.f, 0.f, 0.f, 0.f}, bb[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-        for (int j = 0; j < kD; ++j) { a[j] = 0.0f; bb[j] = 0.0f; }
-#pragma unroll
-        for (int s = 0; s < (NS > 0 ? NS : 4); ++s) {
-          if (s >= SK) break;
-          const uint8_t *cp = p.kc + ((long long)s * p.G + g) * p.plane_rows + (t_seq0 + t0 + t) * kM;
-          const float4 *ra = reinterpret_cast<const float4 *>(ktab + (s * 256 + cp[mq]) * kD);
-          const float4 *rb = reinterpret_cast<const float4 *>(ktab + (s * 256 + cp[mq + 4]) * kD);
-#pragma unroll
-          for (int q4 = 0; q4 < 4; ++q4) {
-            const float4 va = ra[q4], vb = rb[q4];
-            if (s == 0) { a[4 * q4] = va.x; a[4 * q4 + 1] = va.y; a[4 * q4 + 2] = va.z; a[4 * q4 + 3] = va.w;
-                          bb[4 * q4] = vb.x; bb[4 * q4 + 1] = vb.y; bb[4 * q4 + 2] = vb.z; bb[4 * q4 + 3] = vb.w; }
-            else { a[4 * q4] = __fadd_rn(a[4 * q4], va.x); a[4 * q4 + 1] = __fadd_rn(a[4 * q4 + 1], va.y); a[4 * q4 + 2] = __fadd_rn(a[4 * q4 + 2], va.z); a[4 * q4 + 3] = __fadd_rn(a[4 * q4 + 3], va.w);
-                   bb[4 * q4] = __fadd_rn(bb[4 * q4], vb.x); bb[4 * q4 + 1] = __fadd_rn(bb[4 * q4 + 1], vb.y); bb[4 * q4 + 2] = __fadd_rn(bb[4 * q4 + 2], vb.z); bb[4 * q4 + 3] = __fadd_rn(bb[4 * q4 + 3], vb.w); }
+          for (int s = 0; s < (NS > 0 ? NS : 4); ++s) {
+            if (s >= SK) break;
+            const uint2 cw = kcodes[s * CH + t];
+            const float4 va = *reinterpret_cast<const float4 *>(ktab + (s * 256 + ((cw.x >> (8 * mq)) & 255u)) * kD + (l16 & 3) * 4);
+            const float4 vb = *reinterpret_cast<const float4 *>(ktab + (s * 256 + ((cw.y >> (8 * mq)) & 255u)) * kD + (l16 & 3) * 4);
+            if (s == 0) { a[0] = va.x; a[1] = va.y; a[2] = va.z; a[3] = va.w; bb[0] = vb.x; bb[1] = vb.y; bb[2] = vb.z; bb[3] = vb.w; }
+            else { a[0] = __fadd_rn(a[0], va.x); a[1] = __fadd_rn(a[1], va.y); a[2] = __fadd_rn(a[2], va.z); a[3] = __fadd_rn(a[3], va.w);
+                   bb[0] = __fadd_rn(bb[0], vb.x); bb[1] = __fadd_rn(bb[1], vb.y); bb[2] = __fadd_rn(bb[2], vb.z); bb[3] = __fadd_rn(bb[3], vb.w); }
           }
-        }
+          float2 co[4];
+          {
+            const float4 o0 = *reinterpret_cast<const float4 *>(cs_off + off * 64 + i0), o1 = *reinterpret_cast<const float4 *>(cs_off + off * 64 + i0 + 2);
+            co[0] = make_float2(o0.x, o0.y); co[1] = make_float2(o0.z, o0.w); co[2] = make_float2(o1.x, o1.y); co[3] = make_float2(o1.z, o1.w);
+          }
+          float part[HMAX];
 #pragma unroll
-        for (int j = 0; j < kD; ++j) {
-          const int i = mq * kD + j;
-          const float2 cb = cs_base[i], co = cs_off[t * 64 + i];
-          const float c = cb.x * co.x - cb.y * co.y, sn = cb.y * co.x + cb.x * co.y;
-          const float ar = a[j] * c - bb[j] * sn, br = bb[j] * c + a[j] * sn;
+          for (int h = 0; h < HMAX; ++h) part[h] = 0.0f;
 #pragma unroll
-          for (int h = 0; h < HMAX; ++h)
-            if (h < n_rep) part[h] = fmaf(qs[h * kHd + i], ar, fmaf(qs[h * kHd + 64 + i], br, part[h]));
-        }
-      }
+          for (int e = 0; e < 4; ++e) {
+            const float c = cb[e].x * co[e].x - cb[e].y * co[e].y, sn = cb[e].y * co[e].x + cb[e].x * co[e].y;
+            const float ar = a[e] * c - bb[e] * sn, br = bb[e] * c + a[e] * sn;
 #pragma unroll
-      for (int h = 0; h < HMAX; ++h) {
-        if (h < n_rep) {
-          float v = part[h];
-          v += __shfl_xor_sync(0xffffffffu, v, 1);
-          v += __shfl_xor_sync(0xffffffffu, v, 2);
-          if (mq == 0 && t < nv) lg[t * HP + h] = v * p.scale;
+            for (int h = 0; h < HMAX; ++h)
+              if (h < n_rep) part[h] = fmaf(qa[h][e], ar, fmaf(qb[h][e], br, part[h]));
+          }
+          // sum over the token's 16 threads
+          if (HMAX == 4) {   // 4 heads: exchange halves first (5 shuffles instead of 16); lane l16 < 4 ends with head 2 (l16 & 1) + (l16 >> 1)
+            const bool b0 = l16 & 1, b1 = l16 & 2;
+            float v0 = (b0 ? part[2] : part[0]) + __shfl_xor_sync(0xffffffffu, b0 ? part[0] : part[2], 1);
+            float v1 = (b0 ? part[3] : part[1]) + __shfl_xor_sync(0xffffffffu, b0 ? part[1] : part[3], 1);
+            float r = (b1 ? v1 : v0) + __shfl_xor_sync(0xffffffffu, b1 ? v0 : v1, 2);
+            r += __shfl_xor_sync(0xffffffffu, r, 4);
+            r += __shfl_xor_sync(0xffffffffu, r, 8);
+            if (l16 < 4 && ok) lg[t * HP + 2 * (l16 & 1) + (l16 >> 1)] = r * p.scale;
+          } else {
+#pragma unroll
+            for (int h = 0; h < HMAX; ++h) {
+              if (h < n_rep) {
+                float v = part[h];
+                v += __shfl_xor_sync(0xffffffffu, v, 1);
+                v += __shfl_xor_sync(0xffffffffu, v, 2);
+                v += __shfl_xor_sync(0xffffffffu, v, 4);
+                v += __shfl_xor_sync(0xffffffffu, v, 8);
+                if (l16 == 0 && ok) lg[t * HP + h] = v * p.scale;
+              }
+            }
+          }
         }
       }
     }
