@@ -138,47 +138,67 @@ __global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
   const int m_out = lane >> 2, j_out = (lane & 3) * 4;
   __syncthreads();
 
-  for (long long t0 = tb; t0 < te; t0 += CH) {
-    const int nv = (int)min((long long)CH, te - t0);   // valid tokens of the chunk
-    // the chunk's value codes -> shared memory (coalesced 8-byte loads), the stages of one sub-vector side by side
-    if (NS == 2) {
-      for (int t = tid; t < CH; t += kThreads) {
-        uint2 a = make_uint2(0u, 0u), c = make_uint2(0u, 0u);
-        if (t < nv) {
-          a = *reinterpret_cast<const uint2 *>(p.vc + ((long long)g) * p.plane_rows + (t_seq0 + t0 + t) * kM);
-          c = *reinterpret_cast<const uint2 *>(p.vc + ((long long)p.G + g) * p.plane_rows + (t_seq0 + t0 + t) * kM);
-        }
-        reinterpret_cast<uint4 *>(vcodes)[t] = make_uint4(__byte_perm(a.x, c.x, 0x5140), __byte_perm(a.x, c.x, 0x7362),
-                                                          __byte_perm(a.y, c.y, 0x5140), __byte_perm(a.y, c.y, 0x7362));
-      }
-    } else {
-      for (int e = tid; e < SV * CH; e += kThreads) {
-        const int s = e / CH, t = e - s * CH;
-        uint2 v = make_uint2(0u, 0u);
-        if (t < nv) v = *reinterpret_cast<const uint2 *>(p.vc + ((long long)s * p.G + g) * p.plane_rows + (t_seq0 + t0 + t) * kM);
-        if (SVP == 1) reinterpret_cast<uint2 *>(vcodes)[t] = v;
-        else
+  // Code bytes of this thread's tokens (tid, tid + 256, ...) of a chunk, every stage: fetched one chunk ahead, so that the
+  // loads of chunk n + 1 are in flight while chunk n is computed.
+  constexpr int TPT = CH / kThreads, SMAX = NS > 0 ? NS : 4;
+  uint2 nk[TPT][SMAX], nvc[TPT][SMAX];
+  auto fetch = [&](long long t0c) {
 #pragma unroll
-          for (int m = 0; m < kM; ++m) vcodes[(t * kM + m) * SVP + s] = (uint8_t)(((m < 4 ? v.x : v.y) >> (8 * (m & 3))) & 255u);
+    for (int i = 0; i < TPT; ++i) {
+      const long long t = t0c + tid + i * kThreads;
+#pragma unroll
+      for (int s = 0; s < SMAX; ++s) {
+        nk[i][s] = make_uint2(0u, 0u); nvc[i][s] = make_uint2(0u, 0u);
+        if (t < te && s < SK) nk[i][s] = *reinterpret_cast<const uint2 *>(p.kc + ((long long)s * p.G + g) * p.plane_rows + (t_seq0 + t) * kM);
+        if (t < te && s < SV) nvc[i][s] = *reinterpret_cast<const uint2 *>(p.vc + ((long long)s * p.G + g) * p.plane_rows + (t_seq0 + t) * kM);
       }
     }
-    if (ROPE)
-      for (int e = tid; e < SK * CH; e += kThreads) {
-        const int s = e / CH, t = e - s * CH;
-        uint2 v = make_uint2(0u, 0u);
-        if (t < nv) v = *reinterpret_cast<const uint2 *>(p.kc + ((long long)s * p.G + g) * p.plane_rows + (t_seq0 + t0 + t) * kM);
-        kcodes[e] = v;
+  };
+  fetch(tb);
+
+  for (long long t0 = tb; t0 < te; t0 += CH) {
+    const int nv = (int)min((long long)CH, te - t0);   // valid tokens of the chunk
+    // the chunk's value codes -> shared memory, the stages of one sub-vector side by side; key codes: shared memory (RoPE: any
+    // thread needs any token) or this thread's registers
+    uint2 ck[TPT][SMAX];
+#pragma unroll
+    for (int i = 0; i < TPT; ++i) {
+      const int t = tid + i * kThreads;
+      if (NS == 2) {
+        const uint2 a = nvc[i][0], c = nvc[i][1];
+        reinterpret_cast<uint4 *>(vcodes)[t] = make_uint4(__byte_perm(a.x, c.x, 0x5140), __byte_perm(a.x, c.x, 0x7362),
+                                                          __byte_perm(a.y, c.y, 0x5140), __byte_perm(a.y, c.y, 0x7362));
+      } else {
+#pragma unroll
+        for (int s = 0; s < SMAX; ++s) {
+          if (s >= SV) break;
+          const uint2 v = nvc[i][s];
+          if (SVP == 1) reinterpret_cast<uint2 *>(vcodes)[t] = v;
+          else
+#pragma unroll
+            for (int m = 0; m < kM; ++m) vcodes[(t * kM + m) * SVP + s] = (uint8_t)(((m < 4 ? v.x : v.y) >> (8 * (m & 3))) & 255u);
+        }
       }
+#pragma unroll
+      for (int s = 0; s < SMAX; ++s) {
+        ck[i][s] = nk[i][s];
+        if (ROPE && s < SK) kcodes[s * CH + t] = nk[i][s];
+      }
+    }
+    if (t0 + CH < te) fetch(t0 + CH);
     // ---- logits ----
     if (!ROPE) {
-      for (int t = tid; t < nv; t += kThreads) {
+#pragma unroll
+      for (int i = 0; i < TPT; ++i) {
+        const int t = tid + i * kThreads;
+        if (t >= nv) break;
         float sum[(HMAX + 3) & ~3];
 #pragma unroll
         for (int h = 0; h < ((HMAX + 3) & ~3); ++h) sum[h] = 0.0f;
 #pragma unroll
         for (int s = 0; s < (NS > 0 ? NS : 4); ++s) {
           if (s >= SK) break;
-          const uint2 cw = *reinterpret_cast<const uint2 *>(p.kc + ((long long)s * p.G + g) * p.plane_rows + (t_seq0 + t0 + t) * kM);
+          const uint2 cw = ck[i][s];
 #pragma unroll
           for (int m = 0; m < kM; ++m) {
             const int k = (int)(((m < 4 ? cw.x : cw.y) >> (8 * (m & 3))) & 255u);
