@@ -10,8 +10,9 @@
 // Without RoPE the keys are never even dequantised: q_h . khat_t = sum_s sum_m (q_h[m] . cK^(s)_k[.])[k = aK^(s)_{t,m}], so one table
 // QT[h][s][m][k] of n_rep x S x 8 x 256 dot products per (sequence, KV head) turns a token's logit into S x 8 shared-memory
 // lookups per query head.  With RoPE the two sub-vectors of a rotary pair (elements i and i + 64) are dequantised in registers,
-// rotated with cos / sin((base + off) theta_i) = angle addition of a per-chunk base (double precision) and a per-CTA offset
-// table, and multiplied with q.  Values: thread = output element, the chunk's probabilities are broadcast from shared memory.
+// rotated with cos / sin((base + off) theta_i) = angle addition of a base per 64 tokens (double precision) and a per-CTA offset
+// table, and multiplied with q (held in registers: a thread owns four rotary pairs of every 16th token).  Values: warp = token,
+// lane = four output elements; the token's probabilities of all heads are one float4 broadcast from shared memory.
 // Split-K over the tokens (flash-decoding): CTA (split, g, b) keeps a running max / sum per head, k_attn_combine merges the
 // splits in split order.  d = 16, hd = 128, K <= 256, up to 4 stages each; fp32 arithmetic, no atomics (bit-reproducible).
 #pragma once
@@ -318,7 +319,7 @@ __global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
       }
     }
     __syncthreads();
-    // ---- values: thread = output element (two threads per element, even / odd tokens) ----
+    // ---- values: warp = token (t = warp, warp + 8, ...), lane = output elements 4 lane .. 4 lane + 3 ----
 #pragma unroll
     for (int h = 0; h < HMAX; ++h)
       if (h < n_rep) { const float sc = sc_h[h]; acc[h][0] *= sc; acc[h][1] *= sc; acc[h][2] *= sc; acc[h][3] *= sc; }
