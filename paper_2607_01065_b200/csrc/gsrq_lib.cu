@@ -474,9 +474,21 @@ struct WPlan {
   long long nf_tok, Nf, Nall, R, nE;   // R = rows the row-sized buffers hold
   int M;
   size_t off_st, off_cnt, off_rows, off_wt, off_wn, off_rnorm, off_idx, off_ids, off_epart, off_term, off_ahi, off_alo, off_bimg, off_gmax,
-      off_list, off_part, total;
+      off_list, off_part, off_starts, off_items, total;
 };
 constexpr int kWideParts = 4;   // row ranges per group in the wide update (k_wide.cuh)
+
+// Sub-ranges of a group's rows for the stable counting sort in front of the wide update (k_wide_bucket): about 2048 rows each, at
+// most 32 (larger ones for more rows); 0 = too many rows for that path, the update scans the assignment itself.
+static int wide_nsub(long long N) {
+  long long sub = 2048;
+  while (sub < 32768 && (N + sub - 1) / sub > wide::kMaxSub) sub *= 2;
+  const long long n = (N + sub - 1) / sub;
+  if (n > wide::kMaxSub || N >= (1LL << 31)) return 0;
+  return (int)n;
+}
+static long long wide_max_items(long long N, int K) { return N / wide::kItemRows + K + 1; }
+static int wide_parts(long long N) { return (N >= 8192) ? kWideParts : 1; }
 
 static bool wide_tc(int d) { return (d == 64 || d == 128) && use_tc(tc::kD); }
 
@@ -506,7 +518,12 @@ static WPlan make_wplan(const gsrq_view *v, long long n_fit_tokens) {
   p.off_bimg = o;  o += align_up(tcp ? G * (size_t)tc::wide_bimg_bytes<2>() : 0);
   p.off_gmax = o;  o += align_up(G * sizeof(int));
   p.off_list = o;  o += align_up(G * R * sizeof(uint2));
-  p.off_part = o;  o += align_up(G * GSRQ_MAX_K * (size_t)kWideParts * (2 * d + 2) * sizeof(double));
+  {
+    const size_t scan_parts = (size_t)GSRQ_MAX_K * kWideParts, items = (size_t)wide_max_items(p.R, GSRQ_MAX_K);
+    p.off_part = o;  o += align_up(G * (scan_parts > items ? scan_parts : items) * (2 * d + 2) * sizeof(double));
+  }
+  p.off_starts = o; o += align_up(G * (size_t)wide::kMaxSub * (GSRQ_MAX_K + 1) * sizeof(int));
+  p.off_items = o;  o += align_up(G * (size_t)(GSRQ_MAX_K + 1) * sizeof(int));
   p.total = o;
   return p;
 }
@@ -611,10 +628,32 @@ static int wide_update(const WPlan &pl, const gsrq_view *v, char *ws, const floa
   u.rows = rows; u.wn = (const double *)(ws + pl.off_wn); u.wt = (const float *)(ws + pl.off_wt); u.nf_tok = nf_tok; u.M = pl.M;
   u.idx = idx; u.idx16 = 0; u.N = N; u.d = v->d; u.K = K; u.shapes = shapes_st; u.gains = gains_st; u.cb_stride_g = cb_stride_g; u.mode = mode;
   u.st = st; u.term = st ? (double *)(ws + pl.off_term) : nullptr; u.term_stride = kTermStride; u.term_k = 256; u.t = t; u.gmax = nullptr;
-  u.nparts = (N >= 8192) ? kWideParts : 1; u.part = (double *)(ws + pl.off_part);
+  u.part = (double *)(ws + pl.off_part);
+  u.nsub = wide_nsub(N);
+  if (u.nsub > 0) {
+    // rows sorted by cluster (the undecided-row list of the assignment is free by now and holds the order), then balanced items
+    wide::WBucketParams b{};
+    b.idx = idx; b.N = N; b.K = K; b.nsub = u.nsub; b.order = (int *)(ws + pl.off_list); b.starts = (int *)(ws + pl.off_starts); b.st = st; b.t = t;
+    const size_t bsmem = (size_t)256 * K * sizeof(uint16_t);
+    GSRQ_CUDA_CHECK(cudaFuncSetAttribute(wide::k_wide_bucket, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bsmem));
+    LAUNCH(kClsUpdate, stream, (wide::k_wide_bucket<<<dim3((unsigned)u.nsub, (unsigned)v->G), 256, bsmem, stream>>>(b)));
+    GSRQ_CUDA_CHECK(cudaGetLastError());
+    u.order = b.order; u.starts = b.starts; u.item_first = (int *)(ws + pl.off_items); u.max_items = (int)wide_max_items(N, K); u.nparts = 1;
+    LAUNCH(kClsUpdate, stream, (wide::k_wide_items<<<(unsigned)v->G, 256, 0, stream>>>(u)));
+    GSRQ_CUDA_CHECK(cudaGetLastError());
+    const dim3 igrid((unsigned)((u.max_items + 7) / 8), (unsigned)v->G);
+    if (v->d > 128) LAUNCH(kClsUpdate, stream, (wide::k_wide_update_items<2><<<igrid, 256, 0, stream>>>(u)));
+    else LAUNCH(kClsUpdate, stream, (wide::k_wide_update_items<1><<<igrid, 256, 0, stream>>>(u)));
+    GSRQ_CUDA_CHECK(cudaGetLastError());
+    LAUNCH(kClsUpdate, stream, (wide::k_wide_update_items_finish<<<dim3((unsigned)K, (unsigned)v->G), 256, 0, stream>>>(u)));
+    GSRQ_CUDA_CHECK(cudaGetLastError());
+    return GSRQ_OK;
+  }
+  u.nparts = wide_parts(N);
   const dim3 ugrid((unsigned)K, (unsigned)v->G, (unsigned)u.nparts);
-  if (v->d > 128) LAUNCH(kClsUpdate, stream, (wide::k_wide_update<2><<<ugrid, 256, 0, stream>>>(u)));
-  else LAUNCH(kClsUpdate, stream, (wide::k_wide_update<1><<<ugrid, 256, 0, stream>>>(u)));
+  const size_t usmem = wide::wide_update_smem();
+  if (v->d > 128) LAUNCH(kClsUpdate, stream, (wide::k_wide_update<2><<<ugrid, 256, usmem, stream>>>(u)));
+  else LAUNCH(kClsUpdate, stream, (wide::k_wide_update<1><<<ugrid, 256, usmem, stream>>>(u)));
   GSRQ_CUDA_CHECK(cudaGetLastError());
   if (u.nparts > 1) {
     LAUNCH(kClsUpdate, stream, (wide::k_wide_update_finish<<<dim3((unsigned)K, (unsigned)v->G), 256, 0, stream>>>(u)));
@@ -1213,8 +1252,8 @@ int gsrq_cluster_fit(const float *x, const float *w, int64_t N, int d, int K, in
     if (rc) return rc;
     u.mode = (method == 1) ? 2 : (t > 0 ? 1 : 0); u.t = t;
     const dim3 ugrid((unsigned)K, 1, (unsigned)u.nparts);
-    if (d > 128) LAUNCH(kClsUpdate, stream, (wide::k_wide_update<2><<<ugrid, 256, 0, stream>>>(u)));
-    else LAUNCH(kClsUpdate, stream, (wide::k_wide_update<1><<<ugrid, 256, 0, stream>>>(u)));
+    if (d > 128) LAUNCH(kClsUpdate, stream, (wide::k_wide_update<2><<<ugrid, 256, wide::wide_update_smem(), stream>>>(u)));
+    else LAUNCH(kClsUpdate, stream, (wide::k_wide_update<1><<<ugrid, 256, wide::wide_update_smem(), stream>>>(u)));
     GSRQ_CUDA_CHECK(cudaGetLastError());
     if (u.nparts > 1) {
       LAUNCH(kClsUpdate, stream, (wide::k_wide_update_finish<<<dim3((unsigned)K, 1), 256, 0, stream>>>(u)));

@@ -380,7 +380,67 @@ struct WUpdateParams {
   int *gmax;              // optional [G]: bit pattern of max_k g_k after this update (atomicMax on an int), for the tensor-core filter
   int nparts;             // the rows of a group are split in nparts contiguous ranges (gridDim.z), one CTA each
   double *part;           // nparts > 1: [G][K][nparts][2d + 2] partial sums, merged in range order by k_wide_update_finish
+  // sorted mode (K <= 256, uint8 assignment; k_wide_bucket -> k_wide_items -> k_wide_update_items -> k_wide_update_items_finish):
+  const int *order;       // [G][N] row indices, sub-range by sub-range, cluster by cluster, ascending (stable counting sort)
+  const int *starts;      // [G][nsub][K + 1] first position of each cluster within its sub-range's part of order
+  int nsub;               // <= 32
+  int *item_first;        // [G][K + 1] first work item of each cluster; an item = up to kItemRows consecutive rows of one cluster's list
+  int max_items;          // bound of the items of a group: N / kItemRows + K; part is [G][max_items][2d + 2] in this mode
 };
+
+constexpr int kMaxSub = 32;      // sub-ranges per group in sorted mode (one per lane in k_wide_update_items)
+constexpr int kItemRows = 64;
+inline size_t wide_update_smem() { return (size_t)2048 * 16; }
+// first row of sub-range sp of nsub (16-row aligned; sub-range nsub starts at N)
+__host__ __device__ inline long long wide_sub_begin(long long N, int sp, int nsub) { return sp >= nsub ? N : ((N * (long long)sp / nsub) & ~15LL); }
+
+// Stable counting sort of the rows of one sub-range by cluster.  Thread t owns the rows [t per, (t + 1) per) of the sub-range and its
+// own row of a [256][K] table of uint16 counters: count, exclusive scan over (cluster, thread), scatter.  Rows of a cluster come
+// out in ascending order.  grid = (nsub, G), block = 256, dynamic shared memory 256 K uint16.
+struct WBucketParams {
+  const uint8_t *idx;     // [G][N]
+  long long N;
+  int K, nsub;
+  int *order, *starts;
+  const DevStats *st;
+  int t;
+};
+
+__global__ void __launch_bounds__(256) k_wide_bucket(WBucketParams p) {
+  extern __shared__ __align__(16) uint16_t btab[];   // [256][K]
+  __shared__ int start[257];
+  __shared__ int wtot[8];
+  const int sp = blockIdx.x, g = blockIdx.y, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, K = p.K;
+  if (group_done(p.st, g, p.t)) return;
+  const long long rb = wide_sub_begin(p.N, sp, p.nsub), re = wide_sub_begin(p.N, sp + 1, p.nsub);
+  const int n = (int)(re - rb), per = (n + 255) / 256;
+  const int b = min(n, tid * per), e = min(n, b + per);
+  const uint8_t *ix = p.idx + (long long)g * p.N + rb;
+  for (int q = tid; q < 128 * K; q += 256) reinterpret_cast<uint32_t *>(btab)[q] = 0u;
+  __syncthreads();
+  uint16_t *mine = btab + tid * K;
+  for (int i = b; i < e; ++i) { const int k = ix[i]; if (k < K) ++mine[k]; }   // a byte >= K (caller's assignment) belongs to no cluster
+  __syncthreads();
+  int run = 0;
+  if (tid < K)
+    for (int t = 0; t < 256; ++t) { const int c = btab[t * K + tid]; btab[t * K + tid] = (uint16_t)run; run += c; }
+  int incl = run;
+  for (int off = 1; off < 32; off <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, off); if (lane >= off) incl += v; }
+  if (lane == 31) wtot[warp] = incl;
+  __syncthreads();
+  int base = 0;
+  for (int w8 = 0; w8 < warp; ++w8) base += wtot[w8];
+  start[tid] = base + incl - run;
+  if (tid == 255) start[256] = base + incl;
+  __syncthreads();
+  int *ord = p.order + (long long)g * p.N + rb;
+  for (int i = b; i < e; ++i) {
+    const int k = ix[i];
+    if (k < K) ord[start[k] + (int)(mine[k]++)] = (int)(rb + i);
+  }
+  int *so = p.starts + ((long long)g * p.nsub + sp) * (K + 1);
+  for (int k = tid; k <= K; k += 256) so[k] = start[k];
+}
 
 // Eq. 7 / Eq. 8 (or the KM centroid) for cluster k of group g from its sums fin = A[d] | B[d] | W | cnt; all 256 threads.
 __device__ __forceinline__ void wide_finish_cluster(const WUpdateParams &p, int g, int k, const double *fin, double *red);
@@ -389,13 +449,14 @@ __device__ __forceinline__ void wide_finish_cluster(const WUpdateParams &p, int 
 // up in fp64 in that order (thread = element: A_e for e < d, B_e for the next d values); with one range per group the CTA goes
 // on to Eq. 7 / Eq. 8, else the partial sums go to global memory for k_wide_update_finish (heavy-tailed cluster sizes: a
 // cluster with thousands of rows would otherwise keep one CTA busy long after the others have finished).
-// grid = (K, G, nparts), block = 256.  NQ = values per thread = ceil(2 d / 256).
+// grid = (K, G, nparts), block = 256, dynamic shared memory wide_update_smem().  NQ = float4 per lane and row = ceil(d / 128).
 template <int NQ>
 __global__ void __launch_bounds__(256) k_wide_update(WUpdateParams p) {
-  constexpr int kChunk = 2048;              // rows scanned per round (8 per thread)
-  __shared__ int rowq[kChunk];              // matching rows of the round (offset from the round's first row), ascending
-  __shared__ float wq[kChunk];              // their weights w_i
-  __shared__ double wnq[kChunk];            // and w_i / (||r_i|| + eps)
+  constexpr int kScanChunk = 2048, kChunk = kScanChunk;   // rows scanned per round (8 per thread)
+  extern __shared__ __align__(16) uint8_t upd_raw[];
+  double *wnq = reinterpret_cast<double *>(upd_raw);           // [kChunk] w_i / (||r_i|| + eps) of the round's matching rows, ascending
+  int *rowq = reinterpret_cast<int *>(wnq + kChunk);           // their row (offset from the round's first row / index in the group)
+  float *wq = reinterpret_cast<float *>(rowq + kChunk);        // their weights w_i
   __shared__ int wcnt[8];
   __shared__ double fin[2 * kMaxD + 2];
   __shared__ double red[256];
@@ -405,19 +466,47 @@ __global__ void __launch_bounds__(256) k_wide_update(WUpdateParams p) {
   const long long re = (blockIdx.z + 1 == (unsigned)p.nparts) ? p.N : ((p.N * (long long)(blockIdx.z + 1) / p.nparts) & ~15LL);
   const int d = p.d;
   const int msh = ((p.M & (p.M - 1)) == 0) ? (31 - __clz(p.M)) : -1;
-  double acc[NQ];
+  // warp w adds the list entries w, w + 8, ... (ascending), lane l the elements 4 l .. 4 l + 3 (+ 128 q): A (coefficient w) and
+  // B (coefficient w / (||r|| + eps)) of the same elements, so a row is widened to fp64 once
+  double accA[NQ][4], accB[NQ][4];
 #pragma unroll
-  for (int q = 0; q < NQ; ++q) acc[q] = 0.0;
+  for (int q = 0; q < NQ; ++q)
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { accA[q][j] = 0.0; accB[q][j] = 0.0; }
   double accW = 0.0;
   long long cnt = 0;
   const float *rows_g = p.rows + (long long)g * p.N * d;
-  // element this thread reads and whether it belongs to A (coefficient w) or B (coefficient w / (||r|| + eps))
-  int el[NQ];
-  bool isA[NQ], live[NQ];
+  bool live[NQ];
 #pragma unroll
-  for (int q = 0; q < NQ; ++q) { const int v = tid + 256 * q; live[q] = v < 2 * d; isA[q] = v < d; el[q] = (v < d) ? v : v - d; if (!live[q]) el[q] = 0; }
-  for (long long c0 = rb; c0 < re; c0 += kChunk) {
-    // ordered compaction of the matching rows of [c0, c0 + kChunk): thread t looks at rows c0 + 8 t .. + 7
+  for (int q = 0; q < NQ; ++q) live[q] = 4 * lane + 128 * q < d;
+  auto add_rows = [&](const float *rows_c, int total) {
+    constexpr int kDepth = 4;   // rows in flight per warp
+    for (int r0 = warp; r0 < total; r0 += 8 * kDepth) {
+      float4 x[kDepth][NQ];
+#pragma unroll
+      for (int u = 0; u < kDepth; ++u)
+#pragma unroll
+        for (int q = 0; q < NQ; ++q)
+          x[u][q] = (r0 + 8 * u < total && live[q]) ? __ldg(reinterpret_cast<const float4 *>(rows_c + (long long)rowq[r0 + 8 * u] * d + 4 * lane + 128 * q))
+                                                     : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+      for (int u = 0; u < kDepth; ++u) {
+        if (r0 + 8 * u < total) {
+          const double wv = (double)wq[r0 + 8 * u], wnv = wnq[r0 + 8 * u];
+#pragma unroll
+          for (int q = 0; q < NQ; ++q) {
+            const double v[4] = {(double)x[u][q].x, (double)x[u][q].y, (double)x[u][q].z, (double)x[u][q].w};
+#pragma unroll
+            for (int j = 0; j < 4; ++j) { accA[q][j] = fma(wv, v[j], accA[q][j]); accB[q][j] = fma(wnv, v[j], accB[q][j]); }
+          }
+          if (lane == 0) accW += wv;
+        }
+      }
+    }
+    cnt += total;
+  };
+  for (long long c0 = rb; c0 < re; c0 += kScanChunk) {
+    // ordered compaction of the matching rows of [c0, c0 + kScanChunk): thread t looks at rows c0 + 8 t .. + 7
     int my[8], nm = 0;
     const long long b0 = c0 + 8LL * tid;
     if (!p.idx16 && b0 + 8 <= re && (((long long)g * p.N + b0) & 7) == 0) {   // 8 assignment bytes in one load
@@ -451,39 +540,26 @@ __global__ void __launch_bounds__(256) k_wide_update(WUpdateParams p) {
         ++pos;
       }
     __syncthreads();
-    // add the rows in list order, 4 per trip, the next trip's loads in flight while this trip is added
-    const float *rows_c = rows_g + c0 * d;
-    float xa[4][NQ], xb[4][NQ];
-    auto ld = [&](float (&x)[4][NQ], int r0) {
-#pragma unroll
-      for (int u = 0; u < 4; ++u)
-#pragma unroll
-        for (int q = 0; q < NQ; ++q) x[u][q] = (r0 + u < total && live[q]) ? __ldg(rows_c + (long long)rowq[r0 + u] * d + el[q]) : 0.0f;
-    };
-    auto fm = [&](const float (&x)[4][NQ], int r0) {
-#pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        if (r0 + u < total) {
-          const double wv = (double)wq[r0 + u], wnv = wnq[r0 + u];
-#pragma unroll
-          for (int q = 0; q < NQ; ++q) acc[q] = fma(isA[q] ? wv : wnv, (double)x[u][q], acc[q]);
-          if (tid == 0) accW += wv;
-        }
-      }
-    };
-    ld(xa, 0);
-    for (int r0 = 0; r0 < total; r0 += 8) {
-      ld(xb, r0 + 4);
-      fm(xa, r0);
-      ld(xa, r0 + 8);
-      fm(xb, r0 + 4);
-    }
-    cnt += total;
+    add_rows(rows_g + c0 * d, total);
     __syncthreads();
   }
+  // the eight warps' sums, added in warp order
+  for (int w8 = 0; w8 < 8; ++w8) {
+    if (warp == w8) {
 #pragma unroll
-  for (int q = 0; q < NQ; ++q) { const int v = tid + 256 * q; if (live[q]) fin[v] = acc[q]; }
-  if (tid == 0) { fin[2 * d] = accW; fin[2 * d + 1] = (double)cnt; }
+      for (int q = 0; q < NQ; ++q)
+        if (live[q])
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const int e = 4 * lane + 128 * q + j;
+            fin[e] = (w8 ? fin[e] : 0.0) + accA[q][j];
+            fin[d + e] = (w8 ? fin[d + e] : 0.0) + accB[q][j];
+          }
+      if (lane == 0) fin[2 * d] = (w8 ? fin[2 * d] : 0.0) + accW;
+    }
+    __syncthreads();
+  }
+  if (tid == 0) fin[2 * d + 1] = (double)cnt;
   __syncthreads();
   if (p.nparts > 1) {
     double *out = p.part + (((long long)g * p.K + k) * p.nparts + blockIdx.z) * (2 * d + 2);
@@ -504,6 +580,146 @@ __global__ void __launch_bounds__(256) k_wide_update_finish(WUpdateParams p) {
   for (int v = tid; v < 2 * d + 2; v += 256) {
     double sum = 0.0;
     for (int q = 0; q < p.nparts; ++q) sum += in[(long long)q * (2 * d + 2) + v];
+    fin[v] = sum;
+  }
+  __syncthreads();
+  wide_finish_cluster(p, g, k, fin, red);
+}
+
+// ---- sorted mode ----
+// Work items of a group from the sorted lists: cluster k with n_k rows gets ceil(n_k / kItemRows) items.  grid = G, block = 256.
+__global__ void __launch_bounds__(256) k_wide_items(WUpdateParams p) {
+  __shared__ int wtot[8];
+  const int g = blockIdx.x, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  if (group_done(p.st, g, p.t)) return;
+  int n = 0;
+  if (tid < p.K)
+    for (int sp = 0; sp < p.nsub; ++sp) {
+      const int *stp = p.starts + ((long long)g * p.nsub + sp) * (p.K + 1);
+      n += stp[tid + 1] - stp[tid];
+    }
+  const int items = (n + kItemRows - 1) / kItemRows;
+  int incl = items;
+  for (int off = 1; off < 32; off <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, off); if (lane >= off) incl += v; }
+  if (lane == 31) wtot[warp] = incl;
+  __syncthreads();
+  int base = 0;
+  for (int w8 = 0; w8 < warp; ++w8) base += wtot[w8];
+  int *out = p.item_first + (long long)g * (p.K + 1);
+  if (tid < p.K) out[tid] = base + incl - items;
+  if (tid == p.K - 1) out[p.K] = base + incl;
+}
+
+// One warp per work item: up to kItemRows rows of one cluster, added in ascending order in fp64 (lane l: the elements 4 l .. 4 l + 3
+// (+ 128 q) of A and of B), eight rows in flight; the item's sums go to part[g][item].  No block-wide barrier after the table load.
+// grid = (ceil(max_items / 8), G), block = 256.
+template <int NQ>
+__global__ void __launch_bounds__(256) k_wide_update_items(WUpdateParams p) {
+  __shared__ int first[257];
+  const int g = blockIdx.y, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, d = p.d, K = p.K;
+  if (group_done(p.st, g, p.t)) return;
+  for (int q = tid; q <= K; q += 256) first[q] = p.item_first[(long long)g * (K + 1) + q];
+  __syncthreads();
+  const int item = blockIdx.x * 8 + warp;
+  if (item >= first[K]) return;
+  int lo = 0, hi = K - 1;                       // the cluster k with first[k] <= item < first[k + 1]
+  while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (first[mid] <= item) lo = mid; else hi = mid - 1; }
+  const int k = lo, seg = item - first[k];
+  // cluster k's piece of every sub-range list: lane sp holds its length and first position
+  int c_sp = 0, pos_sp = 0;
+  if (lane < p.nsub) {
+    const int *stp = p.starts + ((long long)g * p.nsub + lane) * (K + 1);
+    const int s0 = stp[k];
+    c_sp = stp[k + 1] - s0;
+    pos_sp = (int)wide_sub_begin(p.N, lane, p.nsub) + s0;
+  }
+  int incl = c_sp;
+  for (int off = 1; off < 32; off <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, off); if (lane >= off) incl += v; }
+  const int n_k = __shfl_sync(0xffffffffu, incl, 31);
+  const int e0 = seg * kItemRows, n_it = min(kItemRows, n_k - e0);
+  // entries e0 + lane and e0 + 32 + lane of the cluster's concatenated list
+  const int msh = ((p.M & (p.M - 1)) == 0) ? (31 - __clz(p.M)) : -1;
+  int row[2] = {0, 0};
+  float wv[2] = {0.f, 0.f};
+  double wnv[2] = {0.0, 0.0};
+  const int *ord = p.order + (long long)g * p.N;
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    const int e = e0 + 32 * h + lane;
+    int src = -1;
+    for (int sp = 0; sp < p.nsub; ++sp) {
+      const int in_sp = __shfl_sync(0xffffffffu, incl, sp), c = __shfl_sync(0xffffffffu, c_sp, sp), ps = __shfl_sync(0xffffffffu, pos_sp, sp);
+      if (src < 0 && e < in_sp) src = ps + (e - (in_sp - c));
+    }
+    if (32 * h + lane < n_it) {
+      const int i = ord[src];
+      row[h] = i;
+      wv[h] = __ldg(p.wt + (long long)g * p.nf_tok + ((msh >= 0) ? (i >> msh) : (i / p.M)));
+      wnv[h] = __ldg(p.wn + (long long)g * p.N + i);
+    }
+  }
+  double accA[NQ][4], accB[NQ][4], accW = 0.0;
+#pragma unroll
+  for (int q = 0; q < NQ; ++q)
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { accA[q][j] = 0.0; accB[q][j] = 0.0; }
+  bool live[NQ];
+#pragma unroll
+  for (int q = 0; q < NQ; ++q) live[q] = 4 * lane + 128 * q < d;
+  const float *rows_g = p.rows + (long long)g * p.N * d;
+  constexpr int kDepth = 8;
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    for (int u0 = 0; u0 < 32 && 32 * h + u0 < n_it; u0 += kDepth) {
+      float4 x[kDepth][NQ];
+#pragma unroll
+      for (int u = 0; u < kDepth; ++u) {
+        const int i = __shfl_sync(0xffffffffu, row[h], u0 + u);
+#pragma unroll
+        for (int q = 0; q < NQ; ++q)
+          x[u][q] = (32 * h + u0 + u < n_it && live[q]) ? __ldg(reinterpret_cast<const float4 *>(rows_g + (long long)i * d + 4 * lane + 128 * q))
+                                                          : make_float4(0.f, 0.f, 0.f, 0.f);
+      }
+#pragma unroll
+      for (int u = 0; u < kDepth; ++u) {
+        const double w_ = (double)__shfl_sync(0xffffffffu, wv[h], u0 + u), wn_ = __shfl_sync(0xffffffffu, wnv[h], u0 + u);
+        if (32 * h + u0 + u < n_it) {
+#pragma unroll
+          for (int q = 0; q < NQ; ++q) {
+            const double v[4] = {(double)x[u][q].x, (double)x[u][q].y, (double)x[u][q].z, (double)x[u][q].w};
+#pragma unroll
+            for (int j = 0; j < 4; ++j) { accA[q][j] = fma(w_, v[j], accA[q][j]); accB[q][j] = fma(wn_, v[j], accB[q][j]); }
+          }
+          accW += w_;
+        }
+      }
+    }
+  }
+  double *out = p.part + ((long long)g * p.max_items + item) * (2 * d + 2);
+#pragma unroll
+  for (int q = 0; q < NQ; ++q)
+    if (live[q]) {
+      const int e = 4 * lane + 128 * q;
+      *reinterpret_cast<double2 *>(out + e) = make_double2(accA[q][0], accA[q][1]);
+      *reinterpret_cast<double2 *>(out + e + 2) = make_double2(accA[q][2], accA[q][3]);
+      *reinterpret_cast<double2 *>(out + d + e) = make_double2(accB[q][0], accB[q][1]);
+      *reinterpret_cast<double2 *>(out + d + e + 2) = make_double2(accB[q][2], accB[q][3]);
+    }
+  if (lane == 0) { out[2 * d] = accW; out[2 * d + 1] = (double)n_it; }
+}
+
+// A cluster's items merged in item order (= ascending rows), then Eq. 7 / Eq. 8.  grid = (K, G), block = 256.
+__global__ void __launch_bounds__(256) k_wide_update_items_finish(WUpdateParams p) {
+  __shared__ double fin[2 * kMaxD + 2];
+  __shared__ double red[256];
+  const int k = blockIdx.x, g = blockIdx.y, tid = threadIdx.x;
+  if (group_done(p.st, g, p.t)) return;
+  const int d = p.d;
+  const int i0 = p.item_first[(long long)g * (p.K + 1) + k], i1 = p.item_first[(long long)g * (p.K + 1) + k + 1];
+  const double *in = p.part + ((long long)g * p.max_items + i0) * (2 * d + 2);
+  for (int v = tid; v < 2 * d + 2; v += 256) {
+    double sum = 0.0;
+    for (int q = 0; q < i1 - i0; ++q) sum += in[(long long)q * (2 * d + 2) + v];
     fin[v] = sum;
   }
   __syncthreads();
