@@ -84,7 +84,8 @@ __global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
   for (int e = tid; e < SV * 256 * kD; e += kThreads) {
     const int s = e / (256 * kD), r = e - s * 256 * kD, k = r >> 4;
     const long long cb = ((long long)g * p.vS + s) * p.vK + k;
-    vtab[e] = (k < p.vK) ? __fmul_rn(p.v_gains[cb], p.v_shapes[cb * kD + (r & 15)]) : 0.0f;
+    // two stages: codeword k of stage s at float (2 k + s) 16, so that a stage-0 row and a stage-1 row never share a bank
+    vtab[NS == 2 ? ((2 * k + s) * kD + (r & 15)) : e] = (k < p.vK) ? __fmul_rn(p.v_gains[cb], p.v_shapes[cb * kD + (r & 15)]) : 0.0f;
   }
   if (ROPE) {
 #pragma unroll 8
@@ -132,11 +133,19 @@ __global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
       }
   }
   if (tid < 8) { m_run[tid] = -INFINITY; l_run[tid] = 0.0f; sc_h[tid] = 0.0f; }
-  // values: warp w takes the tokens t = w (mod 8) of a chunk, lane l the output elements 4 l .. 4 l + 3
-  float acc[HMAX][4];
+  // values: warp w takes the tokens t = w (mod 8) of a chunk.  Lane l: the output elements 4 l .. 4 l + 3 of vhat_t (sum of the
+  // stages in registers); with two stages (PAIR) instead the stage (l / 4) % 2 part of the sub-vectors 2 (l / 8), 2 (l / 8) + 1,
+  // elements 4 (l % 4) .. + 3 -- a quarter-warp then reads one stage-0 and one stage-1 row per instruction, which the table
+  // layout keeps in opposite bank halves (conflict-free), and the two stages' sums are added once at the end.
+  constexpr bool PAIR = (NS == 2);
+  constexpr int NA = PAIR ? 8 : 4;
+  float acc[HMAX][NA];
 #pragma unroll
-  for (int h = 0; h < HMAX; ++h) { acc[h][0] = 0.0f; acc[h][1] = 0.0f; acc[h][2] = 0.0f; acc[h][3] = 0.0f; }
+  for (int h = 0; h < HMAX; ++h)
+#pragma unroll
+    for (int i = 0; i < NA; ++i) acc[h][i] = 0.0f;
   const int m_out = lane >> 2, j_out = (lane & 3) * 4;
+  const int pq = lane >> 3, ph = (lane >> 2) & 1;
   __syncthreads();
 
   // Code bytes of this thread's tokens (tid, tid + 256, ...) of a chunk, every stage: fetched one chunk ahead, so that the
@@ -322,7 +331,11 @@ __global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
     // ---- values: warp = token (t = warp, warp + 8, ...), lane = output elements 4 lane .. 4 lane + 3 ----
 #pragma unroll
     for (int h = 0; h < HMAX; ++h)
-      if (h < n_rep) { const float sc = sc_h[h]; acc[h][0] *= sc; acc[h][1] *= sc; acc[h][2] *= sc; acc[h][3] *= sc; }
+      if (h < n_rep) {
+        const float sc = sc_h[h];
+#pragma unroll
+        for (int i = 0; i < NA; ++i) acc[h][i] *= sc;
+      }
     auto value_of = [&](int t) -> float4 {   // vhat_t[4 lane .. 4 lane + 3] = sum over the stages, fp32, stage order
       float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
       const uint8_t *cp = vcodes + (t * kM + m_out) * SVP;
@@ -357,13 +370,49 @@ __global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
         }
       }
     };
-    int t = warp;
-    for (; t + 8 < nv; t += 16) {   // two tokens in flight
-      const float4 v0 = value_of(t), v1 = value_of(t + 8);
-      add_token(t, v0);
-      add_token(t + 8, v1);
+    if (PAIR) {
+      auto rows_of = [&](int t, float4 &va, float4 &vb) {   // this lane's stage: codeword rows of the sub-vectors 2 pq and 2 pq + 1
+        const unsigned cw = *reinterpret_cast<const unsigned *>(vcodes + (t * kM + 2 * pq) * 2);   // bytes (m, s): (2pq, 0) (2pq, 1) (2pq+1, 0) (2pq+1, 1)
+        va = *reinterpret_cast<const float4 *>(vtab + (2 * ((cw >> (8 * ph)) & 255u) + ph) * kD + j_out);
+        vb = *reinterpret_cast<const float4 *>(vtab + (2 * ((cw >> (16 + 8 * ph)) & 255u) + ph) * kD + j_out);
+      };
+      auto add_pair = [&](int t, const float4 &va, const float4 &vb) {
+#pragma unroll
+        for (int h4 = 0; h4 < (HMAX + 3) / 4; ++h4) {
+          if (4 * h4 >= n_rep) break;
+          const float4 pr = *reinterpret_cast<const float4 *>(lg + t * HP + 4 * h4);
+          const float pv[4] = {pr.x, pr.y, pr.z, pr.w};
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const int h = 4 * h4 + i;
+            if (h < HMAX && h < n_rep) {
+              acc[h][0] = fmaf(pv[i], va.x, acc[h][0]); acc[h][1] = fmaf(pv[i], va.y, acc[h][1]);
+              acc[h][2] = fmaf(pv[i], va.z, acc[h][2]); acc[h][3] = fmaf(pv[i], va.w, acc[h][3]);
+              acc[h][NA - 4] = fmaf(pv[i], vb.x, acc[h][NA - 4]); acc[h][NA - 3] = fmaf(pv[i], vb.y, acc[h][NA - 3]);
+              acc[h][NA - 2] = fmaf(pv[i], vb.z, acc[h][NA - 2]); acc[h][NA - 1] = fmaf(pv[i], vb.w, acc[h][NA - 1]);
+            }
+          }
+        }
+      };
+      int t = warp;
+      for (; t + 24 < nv; t += 32) {   // four tokens in flight
+        float4 a0, b0, a1, b1, a2, b2, a3, b3;
+        rows_of(t, a0, b0); rows_of(t + 8, a1, b1); rows_of(t + 16, a2, b2); rows_of(t + 24, a3, b3);
+        add_pair(t, a0, b0);
+        add_pair(t + 8, a1, b1);
+        add_pair(t + 16, a2, b2);
+        add_pair(t + 24, a3, b3);
+      }
+      for (; t < nv; t += 8) { float4 a0, b0; rows_of(t, a0, b0); add_pair(t, a0, b0); }
+    } else {
+      int t = warp;
+      for (; t + 8 < nv; t += 16) {   // two tokens in flight
+        const float4 v0 = value_of(t), v1 = value_of(t + 8);
+        add_token(t, v0);
+        add_token(t + 8, v1);
+      }
+      for (; t < nv; t += 8) add_token(t, value_of(t));
     }
-    for (; t < nv; t += 8) add_token(t, value_of(t));
     __syncthreads();
   }
   // ---- this split's result: m, l, acc = the eight warps' partial sums added in warp order ----
@@ -371,7 +420,17 @@ __global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
   float *pp = p.part + (((long long)b * p.G + g) * p.n_split + sp) * n_rep * kPartStride;
 #pragma unroll
   for (int h = 0; h < HMAX; ++h)
-    if (h < n_rep) *reinterpret_cast<float4 *>(ex + ((warp * n_rep + h) * kHd) + 4 * lane) = make_float4(acc[h][0], acc[h][1], acc[h][2], acc[h][3]);
+    if (h < n_rep) {
+      if (PAIR) {   // stage 0 + stage 1 (lane ^ 4); the stage-0 lane stores sub-vector 2 pq, the stage-1 lane 2 pq + 1
+        float tot[NA];
+#pragma unroll
+        for (int i = 0; i < NA; ++i) { const float o = __shfl_xor_sync(0xffffffffu, acc[h][i], 4); tot[i] = ph ? o + acc[h][i] : acc[h][i] + o; }
+        *reinterpret_cast<float4 *>(ex + ((warp * n_rep + h) * kHd) + (2 * pq + ph) * kD + j_out) =
+            ph ? make_float4(tot[NA - 4], tot[NA - 3], tot[NA - 2], tot[NA - 1]) : make_float4(tot[0], tot[1], tot[2], tot[3]);
+      } else {
+        *reinterpret_cast<float4 *>(ex + ((warp * n_rep + h) * kHd) + 4 * lane) = make_float4(acc[h][0], acc[h][1], acc[h][2], acc[h][3]);
+      }
+    }
   __syncthreads();
   for (int e = tid; e < n_rep * kHd; e += kThreads) {
     float sum = 0.0f;
