@@ -65,7 +65,7 @@ __global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
   float2 *cs_off = reinterpret_cast<float2 *>(ktab + SK * 256 * kD);    // ROPE only: [64 offsets][64 frequencies]
   float2 *cs_base = cs_off + 64 * 64;                                   // [4 sub-chunks of 64 tokens][64]
   const int HP = (n_rep + 3) & ~3;                                      // heads padded to a multiple of 4
-  float *qt = ktab;                                                     // [SK][8][256][HP]
+  float *qt = ktab;                                                     // [SK][256][8][HP]
   float *lg = ROPE ? reinterpret_cast<float *>(cs_base + 4 * 64) : qt + HP * SK * kM * 256;
   const int SVP = SV == 3 ? 4 : SV;                                     // stages of one (token, m) side by side, padded to 1 / 2 / 4 bytes
   uint8_t *vcodes = reinterpret_cast<uint8_t *>(lg + (HP * CH > n_rep * kHd ? HP * CH : n_rep * kHd));   // [CH][8][SVP]
@@ -101,24 +101,39 @@ __global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
       cs_off[e] = make_float2((float)cs, (float)sn);
     }
   } else {
-    // QT[h][s][m][k] = sum_j q_h[16 m + j] cK^(s)_k[j]: thread per codeword (s, k), every (h, m); q staged in the (still unused) logits buffer
+    // QT[s][k][m][h] = sum_j q_h[16 m + j] cK^(s)_k[j]; q staged in the (still unused) logits buffer
     for (int e = tid; e < n_rep * kHd; e += kThreads) lg[e] = qg[e];
     __syncthreads();
-    for (int e = tid; e < SK * 256; e += kThreads) {
-      const int s = e >> 8, k = e & 255;
+    // thread per (codeword, sub-vector): consecutive lanes write consecutive entries; a thread's sub-vector m = tid % 8 is the same
+    // for all its entries, so its q elements stay in registers (up to 4 heads)
+    constexpr bool QREG = HMAX <= 4;
+    float qr[QREG ? HMAX : 1][kD];
+    if (QREG)
+#pragma unroll
+      for (int h = 0; h < HMAX; ++h)
+#pragma unroll
+        for (int j = 0; j < kD; ++j) qr[QREG ? h : 0][j] = (h < n_rep) ? lg[h * kHd + (tid & 7) * kD + j] : 0.0f;
+    for (int e = tid; e < SK * 256 * kM; e += kThreads) {
+      const int m = e & 7, k = (e >> 3) & 255, s = e >> 11;
       float c[kD];
       const long long cb = ((long long)g * p.kS + s) * p.kK + k;
       const float gk = (k < p.kK) ? p.k_gains[cb] : 0.0f;
 #pragma unroll
-      for (int j = 0; j < kD; ++j) c[j] = (k < p.kK) ? __fmul_rn(gk, p.k_shapes[cb * kD + j]) : 0.0f;
-      for (int h = 0; h < n_rep; ++h)
+      for (int j4 = 0; j4 < kD / 4; ++j4) {
+        const float4 v = (k < p.kK) ? *reinterpret_cast<const float4 *>(p.k_shapes + cb * kD + 4 * j4) : make_float4(0.f, 0.f, 0.f, 0.f);
+        c[4 * j4] = __fmul_rn(gk, v.x); c[4 * j4 + 1] = __fmul_rn(gk, v.y); c[4 * j4 + 2] = __fmul_rn(gk, v.z); c[4 * j4 + 3] = __fmul_rn(gk, v.w);
+      }
+      float a[(HMAX + 3) & ~3];
 #pragma unroll
-        for (int m = 0; m < kM; ++m) {
-          float a = 0.0f;
+      for (int h = 0; h < ((HMAX + 3) & ~3); ++h) {
+        a[h] = 0.0f;
+        if (h < HMAX && h < n_rep)
 #pragma unroll
-          for (int j = 0; j < kD; ++j) a = fmaf(lg[h * kHd + m * kD + j], c[j], a);
-          qt[((s * kM + m) * 256 + k) * HP + h] = a;
-        }
+          for (int j = 0; j < kD; ++j) a[h] = fmaf(QREG ? qr[QREG ? h : 0][j] : lg[h * kHd + m * kD + j], c[j], a[h]);
+      }
+#pragma unroll
+      for (int h4 = 0; h4 < (HMAX + 3) / 4; ++h4)
+        if (4 * h4 < HP) *reinterpret_cast<float4 *>(qt + (long long)e * HP + 4 * h4) = make_float4(a[4 * h4], a[4 * h4 + 1], a[4 * h4 + 2], a[4 * h4 + 3]);
     }
   }
   float qa[ROPE ? HMAX : 1][4], qb[ROPE ? HMAX : 1][4];   // ROPE: this thread's q elements (pairs i, i + 64) of every head
@@ -210,9 +225,12 @@ __global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
           if (s >= SK) break;
           const uint2 cw = ck[i][s];
 #pragma unroll
-          for (int m = 0; m < kM; ++m) {
-            const int k = (int)(((m < 4 ? cw.x : cw.y) >> (8 * (m & 3))) & 255u);
-            const float4 *q4 = reinterpret_cast<const float4 *>(qt + ((s * kM + m) * 256 + k) * HP);
+          for (int j = 0; j < kM; ++j) {
+            // lane l takes sub-vector (l + j) % 8 at step j: the eight lanes of a quarter-warp read eight different sub-vectors'
+            // entries, which the table layout puts in eight different 16-byte bank groups (no conflicts whatever the codes are)
+            const int m = (lane + j) & 7;
+            const int k = (int)(__byte_perm(cw.x, cw.y, m) & 255u);
+            const float4 *q4 = reinterpret_cast<const float4 *>(qt + ((s * 256 + k) * kM + m) * HP);
 #pragma unroll
             for (int h4 = 0; h4 < (HMAX + 3) / 4; ++h4) {
               if (4 * h4 >= n_rep) break;
