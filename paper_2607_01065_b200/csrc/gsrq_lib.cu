@@ -1336,19 +1336,24 @@ int gsrq_attention_decode(const float *q, const uint8_t *k_codes, const gsrq_cod
   const size_t smem = attn::attn_smem_bytes(k_stages, v_stages, p.n_rep, rope);
   if (smem > 227 * 1024) { set_error("attention: %d key stages x %d query heads per KV head do not fit in shared memory", k_stages, p.n_rep); return GSRQ_EUNSUPPORTED; }
   const dim3 grid((unsigned)p.n_split, (unsigned)G, (unsigned)B);
-#define GSRQ_ATTN(ROPE, NREP, NS)                                                                                                       \
-  do {                                                                                                                                  \
-    GSRQ_CUDA_CHECK(cudaFuncSetAttribute(attn::k_attn_decode<ROPE, NREP, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-    LAUNCH(kClsDecode, stream, (attn::k_attn_decode<ROPE, NREP, NS><<<grid, attn::kThreads, smem, stream>>>(p)));                       \
+#define GSRQ_ATTN_K(KERNEL)                                                                                            \
+  do {                                                                                                                \
+    GSRQ_CUDA_CHECK(cudaFuncSetAttribute(KERNEL, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));            \
+    LAUNCH(kClsDecode, stream, (KERNEL<<<grid, attn::kThreads, smem, stream>>>(p)));                                  \
+  } while (0)
+#define GSRQ_ATTN(NREP, NS)                                                                                           \
+  do {                                                                                                                \
+    if (rope) GSRQ_ATTN_K((attn::k_attn_decode_rope<NREP, NS>)); else GSRQ_ATTN_K((attn::k_attn_decode<false, NREP, NS>)); \
   } while (0)
   // compile-time head ratio / stage count for the common shapes (LLaMA-3-8B: 4 query heads per KV head); else the generic kernel
   const int ns = (k_stages == v_stages) ? k_stages : 0;
-  if (p.n_rep == 4 && ns == 1) { if (rope) GSRQ_ATTN(true, 4, 1); else GSRQ_ATTN(false, 4, 1); }
-  else if (p.n_rep == 4 && ns == 2) { if (rope) GSRQ_ATTN(true, 4, 2); else GSRQ_ATTN(false, 4, 2); }
-  else if (p.n_rep == 4 && ns == 4) { if (rope) GSRQ_ATTN(true, 4, 4); else GSRQ_ATTN(false, 4, 4); }
-  else if (p.n_rep == 1 && ns == 2) { if (rope) GSRQ_ATTN(true, 1, 2); else GSRQ_ATTN(false, 1, 2); }
-  else if (p.n_rep == 8 && ns == 2) { if (rope) GSRQ_ATTN(true, 8, 2); else GSRQ_ATTN(false, 8, 2); }
-  else { if (rope) GSRQ_ATTN(true, 0, 0); else GSRQ_ATTN(false, 0, 0); }
+  if (p.n_rep == 4 && ns == 1) GSRQ_ATTN(4, 1);
+  else if (p.n_rep == 4 && ns == 2) GSRQ_ATTN(4, 2);
+  else if (p.n_rep == 4 && ns == 4) GSRQ_ATTN(4, 4);
+  else if (p.n_rep == 1 && ns == 2) GSRQ_ATTN(1, 2);
+  else if (p.n_rep == 8 && ns == 2) GSRQ_ATTN(8, 2);
+  else GSRQ_ATTN(0, 0);
+#undef GSRQ_ATTN_K
 #undef GSRQ_ATTN
   GSRQ_CUDA_CHECK(cudaGetLastError());
   LAUNCH(kClsDecode, stream, (attn::k_attn_combine<<<dim3((unsigned)Hq, (unsigned)B), 128, 0, stream>>>(p)));

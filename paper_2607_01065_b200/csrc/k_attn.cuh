@@ -54,7 +54,7 @@ __host__ __device__ inline size_t attn_smem_bytes(int k_stages, int v_stages, in
 // NREP / NS > 0: query heads per KV head and stages (keys = values) fixed at compile time, every loop over them unrolled;
 // NREP == 0 && NS == 0: the generic kernel (any n_rep <= 8, 1..4 stages each).
 template <bool ROPE, int NREP, int NS>
-__global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
+__device__ __forceinline__ void attn_decode_body(const AttnParams &p) {
   extern __shared__ __align__(16) uint8_t asm_raw[];
   constexpr int CH = ROPE ? 256 : 512;
   constexpr int HMAX = NREP > 0 ? NREP : 8;
@@ -92,7 +92,7 @@ __global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
     for (int e = tid; e < SK * 256 * kD; e += kThreads) {
       const int s = e / (256 * kD), r = e - s * 256 * kD, k = r >> 4;
       const long long cb = ((long long)g * p.kS + s) * p.kK + k;
-      ktab[e] = (k < p.kK) ? __fmul_rn(p.k_gains[cb], p.k_shapes[cb * kD + (r & 15)]) : 0.0f;
+      ktab[NS == 2 ? ((2 * k + s) * kD + (r & 15)) : e] = (k < p.kK) ? __fmul_rn(p.k_gains[cb], p.k_shapes[cb * kD + (r & 15)]) : 0.0f;   // two stages: as the value table
     }
     for (int e = tid; e < 64 * 64; e += kThreads) {   // rotation by (offset within the chunk) x theta_i, in double
       const int off = e >> 6, i = e & 63;
@@ -273,18 +273,26 @@ __global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
           const bool ok = t < nv;
           float a[4] = {0.f, 0.f, 0.f, 0.f}, bb[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-          for (int s = 0; s < (NS > 0 ? NS : 4); ++s) {
-            if (s >= SK) break;
+          for (int st = 0; st < (NS > 0 ? NS : 4); ++st) {
+            if (st >= SK) break;
+            // two stages: the odd sub-vector pairs take stage 1 first, so that the two rows a quarter-warp reads per instruction lie in
+            // opposite bank halves (a two-term fp32 sum does not depend on the order)
+            const int s = (NS == 2) ? (st ^ (mq & 1)) : st;
             const uint2 cw = kcodes[s * CH + t];
-            const float4 va = *reinterpret_cast<const float4 *>(ktab + (s * 256 + ((cw.x >> (8 * mq)) & 255u)) * kD + (l16 & 3) * 4);
-            const float4 vb = *reinterpret_cast<const float4 *>(ktab + (s * 256 + ((cw.y >> (8 * mq)) & 255u)) * kD + (l16 & 3) * 4);
-            if (s == 0) { a[0] = va.x; a[1] = va.y; a[2] = va.z; a[3] = va.w; bb[0] = vb.x; bb[1] = vb.y; bb[2] = vb.z; bb[3] = vb.w; }
+            const int ra = (NS == 2) ? (2 * ((cw.x >> (8 * mq)) & 255u) + s) : (s * 256 + ((cw.x >> (8 * mq)) & 255u));
+            const int rb = (NS == 2) ? (2 * ((cw.y >> (8 * mq)) & 255u) + s) : (s * 256 + ((cw.y >> (8 * mq)) & 255u));
+            const float4 va = *reinterpret_cast<const float4 *>(ktab + ra * kD + (l16 & 3) * 4);
+            const float4 vb = *reinterpret_cast<const float4 *>(ktab + rb * kD + (l16 & 3) * 4);
+            if (st == 0) { a[0] = va.x; a[1] = va.y; a[2] = va.z; a[3] = va.w; bb[0] = vb.x; bb[1] = vb.y; bb[2] = vb.z; bb[3] = vb.w; }
             else { a[0] = __fadd_rn(a[0], va.x); a[1] = __fadd_rn(a[1], va.y); a[2] = __fadd_rn(a[2], va.z); a[3] = __fadd_rn(a[3], va.w);
                    bb[0] = __fadd_rn(bb[0], vb.x); bb[1] = __fadd_rn(bb[1], vb.y); bb[2] = __fadd_rn(bb[2], vb.z); bb[3] = __fadd_rn(bb[3], vb.w); }
           }
           float2 co[4];
           {
-            const float4 o0 = *reinterpret_cast<const float4 *>(cs_off + off * 64 + i0), o1 = *reinterpret_cast<const float4 *>(cs_off + off * 64 + i0 + 2);
+            // this lane's 32 bytes in two loads, the halves in the order that gives the eight lanes of a quarter-warp eight different bank groups
+            const int sw = ((l16 & 3) + mq) & 1;
+            const float4 f0 = *reinterpret_cast<const float4 *>(cs_off + off * 64 + i0 + 2 * sw), f1 = *reinterpret_cast<const float4 *>(cs_off + off * 64 + i0 + 2 * (1 - sw));
+            const float4 o0 = sw ? f1 : f0, o1 = sw ? f0 : f1;
             co[0] = make_float2(o0.x, o0.y); co[1] = make_float2(o0.z, o0.w); co[2] = make_float2(o1.x, o1.y); co[3] = make_float2(o1.z, o1.w);
           }
           float part[HMAX];
@@ -458,6 +466,13 @@ __global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) {
   }
   if (tid < n_rep) { pp[tid * kPartStride] = m_run[tid]; pp[tid * kPartStride + 1] = l_run[tid]; }
 }
+
+// Two entry points so that the register budgets differ: the RoPE body is held to 128 registers (two CTAs per SM, which shared
+// memory allows), the table-lookup body is left to the compiler (about 100).
+template <bool ROPE, int NREP, int NS>
+__global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) { attn_decode_body<ROPE, NREP, NS>(p); }
+template <int NREP, int NS>
+__global__ void __launch_bounds__(kThreads, 2) k_attn_decode_rope(AttnParams p) { attn_decode_body<true, NREP, NS>(p); }
 
 // Merge the splits of one (sequence, query head) in split order.  grid = (Hq, B), block = 128.
 __global__ void __launch_bounds__(128) k_attn_combine(AttnParams p) {
