@@ -8,7 +8,7 @@ A "step" is that whole hot path for both tensors:
     for X in (K, V): for s in 0..S-1: gsrq_fit_stage(X, stage s, fit sample) ; gsrq_encode(X, stages [0,S)) ; gsrq_decode(X)
 value = KV vectors (token x head, 2 x 8 x 1,048,576 per step) through the whole step per second, summed over ranks
 (replicas: every rank works on its own layer).  Inputs are resident in HBM and far larger than L2 (no flush needed).
-e2e is the same through gsrq_pipeline_host on pinned HOST buffers (H2D of the tensors, D2H of codes, codebooks and
+e2e is the same through gsrq_pipeline_host_batch on pinned HOST buffers (H2D of the tensors, D2H of codes, codebooks and
 the decoded tensors inside the timed region).  Rank 0 also times BASELINE configs 1-3 and the encode-on-append
 latency as extras (>= 20 repetitions each, median and min), and the CPU oracle on a bounded sample.
 
@@ -456,16 +456,16 @@ def main():
     if not args.no_e2e:
         host = {kind: dict(x=tens[kind]["x"].cpu().pin_memory(), w=tens[kind]["w"].cpu().pin_memory(),
                            fit=tens[kind]["fit_tokens"].cpu().pin_memory()) for kind in ("k", "v")}
-        sh_h = torch.empty(G, S, K, d).pin_memory(); ga_h = torch.empty(G, S, K).pin_memory()
-        co_h = torch.empty(S, G, T * M, dtype=torch.uint8).pin_memory()
-        out_h = torch.empty(T, G, hd, dtype=torch.bfloat16).pin_memory()
+        kinds = ("k", "v")
+        sh_h = [torch.empty(G, S, K, d).pin_memory() for _ in kinds]; ga_h = [torch.empty(G, S, K).pin_memory() for _ in kinds]
+        co_h = [torch.empty(S, G, T * M, dtype=torch.uint8).pin_memory() for _ in kinds]
+        out_h = [torch.empty(T, G, hd, dtype=torch.bfloat16).pin_memory() for _ in kinds]
         del out, codes
         torch.cuda.empty_cache()
 
-        def e2e_step():
-            for kind in ("k", "v"):
-                h = host[kind]
-                B.gsrq_pipeline_host(h["x"], view, h["w"], h["fit"], K, S, iters, 0, sh_h, ga_h, co_h, out_h)
+        def e2e_step():   # one call for the layer's K and V cache: V uploads while K is fitted, encoded, decoded and downloaded
+            B.gsrq_pipeline_host_batch([host[k_]["x"] for k_ in kinds], view, [host[k_]["w"] for k_ in kinds], [host[k_]["fit"] for k_ in kinds],
+                                       K, S, iters, 0, sh_h, ga_h, co_h, out_h)
 
         e2e_step()
         barrier()
@@ -477,9 +477,9 @@ def main():
         e2e_s = (time.perf_counter() - t0) / n_e2e
         e2e_val, _ = whole_job_value(e2e_s, units, world, "cuda")
         h2d = sum(h["x"].numel() * 2 + h["w"].numel() * 4 + h["fit"].numel() * 8 for h in host.values())
-        d2h = 2 * (sh_h.numel() * 4 + ga_h.numel() * 4 + co_h.numel() + out_h.numel() * 2)
+        d2h = sum(sh_h[i].numel() * 4 + ga_h[i].numel() * 4 + co_h[i].numel() + out_h[i].numel() * 2 for i in range(len(kinds)))
         e2e = dict(value=e2e_val, unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h, ms_per_step=e2e_s * 1e3,
-                   steps=n_e2e, call="gsrq_pipeline_host (pinned host buffers, fit_tokens given)")
+                   steps=n_e2e, call="gsrq_pipeline_host_batch (K and V in one call, pinned host buffers, fit_tokens given)")
         B.gsrq_release_host_pool()
         del host, sh_h, ga_h, co_h, out_h
     if world > 1:

@@ -300,6 +300,17 @@ int gsrq_pipeline_host(const void *kv_host, const gsrq_view *view, const float *
                        int64_t n_fit, int K, int S, int iters, uint64_t seed, float *shapes_host, float *gains_host,
                        uint8_t *codes_host, void *kv_out_host);
 
+/* gsrq_pipeline_host for n tensors of the same view (a layer's K and V cache, several layers, ...), pipelined: the tensors
+ * alternate between two streams, so that tensor i + 1 is uploaded while tensor i is fitted, encoded, decoded and downloaded (both
+ * copy directions and the SMs busy at once; uploads follow one another, each at full link speed).  Every array has n entries:
+ * kv_host[i], shapes_host[i], gains_host[i], codes_host[i] as in gsrq_pipeline_host; w_host, fit_tokens_host, kv_out_host may be
+ * NULL or hold NULL entries (no weights / fit on all tokens / no decode); n_fit, K, S, iters, seed are shared.  The host
+ * buffers should be pinned: a copy from or to pageable memory blocks the calling thread and serialises the tensors.  Results
+ * are identical to n calls of gsrq_pipeline_host.  Returns the first tensor's error, if any; synchronises. */
+int gsrq_pipeline_host_batch(int n, const void *const *kv_host, const gsrq_view *view, const float *const *w_host,
+                             const int64_t *const *fit_tokens_host, int64_t n_fit, int K, int S, int iters, uint64_t seed,
+                             float *const *shapes_host, float *const *gains_host, uint8_t *const *codes_host, void *const *kv_out_host);
+
 /* Free the device memory the *_host entry points keep between calls (current device). */
 void gsrq_release_host_pool(void);
 

@@ -43,7 +43,7 @@ class gsrq_fit_stats(C.Structure):
 _lib = None
 EXPORTS = ["gsrq_log_weights", "gsrq_encode_pervector_gain", "gsrq_decode_pervector_gain", "gsrq_pack_nibbles", "gsrq_unpack_nibbles",
            "gsrq_attention_workspace_bytes", "gsrq_attention_decode", "gsrq_cluster_workspace_bytes", "gsrq_cluster_fit", "gsrq_cluster_assign", "gsrq_cluster_metrics", "gsrq_workspace_bytes", "gsrq_fit_stage", "gsrq_encode", "gsrq_decode", "gsrq_encode_append", "gsrq_assign", "gsrq_update",
-           "gsrq_init_ids", "gsrq_debug_scores", "gsrq_encode_host", "gsrq_decode_host", "gsrq_pipeline_host", "gsrq_release_host_pool", "gsrq_profile_enable",
+           "gsrq_init_ids", "gsrq_debug_scores", "gsrq_encode_host", "gsrq_decode_host", "gsrq_pipeline_host", "gsrq_pipeline_host_batch", "gsrq_release_host_pool", "gsrq_profile_enable",
            "gsrq_profile_read", "gsrq_launch_count", "gsrq_last_error", "gsrq_version"]
 
 
@@ -245,6 +245,26 @@ def gsrq_pipeline_host(kv_host, view, w_host, fit_tokens_host, K, S, iters, seed
     n_fit = 0 if fit_tokens_host is None else fit_tokens_host.shape[1]
     _check(lib().gsrq_pipeline_host(_ptr(kv_host), C.byref(view), _ptr(w_host), _ptr(fit_tokens_host), C.c_int64(n_fit), K, S, iters,
                                     C.c_uint64(seed), _ptr(shapes_host), _ptr(gains_host), _ptr(codes_host), _ptr(kv_out_host)))
+
+
+def gsrq_pipeline_host_batch(kv_hosts, view, w_hosts, fit_tokens_hosts, K, S, iters, seed, shapes_hosts, gains_hosts, codes_hosts, kv_out_hosts):
+    """gsrq_pipeline_host for a list of HOST tensors of the same view (e.g. a layer's K and V cache), pipelined over two streams.
+    w_hosts / fit_tokens_hosts / kv_out_hosts: lists (entries may be None) or None."""
+    n = len(kv_hosts)
+    def arr(ts):
+        if ts is None:
+            return None
+        assert len(ts) == n
+        for t in ts:
+            assert t is None or not t.is_cuda
+        return (C.c_void_p * n)(*[(t.data_ptr() if t is not None else None) for t in ts])
+    n_fit = 0
+    if fit_tokens_hosts is not None:
+        shp = {t.shape[1] for t in fit_tokens_hosts if t is not None}
+        assert len(shp) <= 1, "the tensors of a batch share n_fit"
+        n_fit = shp.pop() if shp else 0
+    _check(lib().gsrq_pipeline_host_batch(n, arr(kv_hosts), C.byref(view), arr(w_hosts), arr(fit_tokens_hosts), C.c_int64(n_fit), K, S, iters,
+                                          C.c_uint64(seed), arr(shapes_hosts), arr(gains_hosts), arr(codes_hosts), arr(kv_out_hosts)))
 
 
 def gsrq_release_host_pool():

@@ -1513,13 +1513,20 @@ __global__ void k_collect_err(const DevStats *__restrict__ st, int G, int *__res
     if (st[g].err) atomicMin(err_accum, st[g].err);   // error codes are negative: keep the lowest
 }
 
-int gsrq_pipeline_host(const void *kv_host, const gsrq_view *view, const float *w_host, const int64_t *fit_tokens_host,
-                       int64_t n_fit, int K, int S, int iters, uint64_t seed, float *shapes_host, float *gains_host,
-                       uint8_t *codes_host, void *kv_out_host) {
-  if (!kv_host || !shapes_host || !gains_host || !codes_host) { set_error("NULL input"); return GSRQ_EINVAL; }
-  int rc = check_view(view, K, S);
-  if (rc) return rc;
-  if (fit_tokens_host && (n_fit <= 0 || n_fit > view->T)) { set_error("n_fit out of range"); return GSRQ_EINVAL; }
+// One tensor's chain of the host pipeline, enqueued on `stream` (nothing here waits for the device).  h2d_after: the upload
+// waits for this event (the previous tensor's upload, so that uploads run one after the other at full link speed instead of
+// sharing it); h2d_done is recorded after this tensor's upload.
+struct PipeJob {
+  char *base = nullptr;
+  cudaStream_t stream = nullptr;
+  int *h_err = nullptr;   // pinned: a download into pageable memory would block the enqueueing thread until the chain is done
+  int rc = GSRQ_OK;
+  cudaError_t e = cudaSuccess;
+};
+
+static void pipeline_enqueue(PipeJob &jb, cudaMemPool_t pool, const void *kv_host, const gsrq_view *view, const float *w_host,
+                             const int64_t *fit_tokens_host, int64_t n_fit, int K, int S, int iters, uint64_t seed, float *shapes_host,
+                             float *gains_host, uint8_t *codes_host, void *kv_out_host, cudaEvent_t h2d_after, cudaEvent_t h2d_done) {
   const int G = view->G, d = view->d, M = view->hd / d;
   const size_t esz = view->dtype == GSRQ_BF16 ? 2 : 4;
   const size_t kv_bytes = (size_t)G * view->T * view->hd * esz;
@@ -1528,16 +1535,16 @@ int gsrq_pipeline_host(const void *kv_host, const gsrq_view *view, const float *
   const size_t ft_bytes = fit_tokens_host ? (size_t)G * n_fit * sizeof(int64_t) : 0;
   const size_t wsb = gsrq_workspace_bytes(view, K, S, fit_tokens_host ? n_fit : 0);
   const bool per_stage = !fit_tokens_host;   // fit on all tokens: encode each stage after its fit, its residual feeds the next fit
-  cudaStream_t stream = nullptr;
-  cudaMemPool_t pool = host_pool();
-  if (!pool) { set_error("gsrq_pipeline_host: could not create the device memory pool"); return GSRQ_ECUDA; }
-  char *base = nullptr;
+  cudaStream_t stream = jb.stream;
   size_t off[10], o = 0;
   const size_t sizes[10] = {kv_bytes, (size_t)view->T * 4, sh_bytes, ga_bytes, n_rows * S, per_stage ? n_rows * d * 4 : 0, wsb,
                             kv_out_host ? kv_bytes : 0, ft_bytes, 256};
   for (int i = 0; i < 10; ++i) { off[i] = o; o += align_up(sizes[i]); }
-  cudaError_t e = cudaMallocFromPoolAsync((void **)&base, o, pool, stream);
-  if (e != cudaSuccess) { set_error("gsrq_pipeline_host: %s", cudaGetErrorString(e)); return GSRQ_ECUDA; }
+  cudaError_t &e = jb.e;
+  int &rc = jb.rc;
+  e = cudaMallocFromPoolAsync((void **)&jb.base, o, pool, stream);
+  if (e != cudaSuccess) { jb.base = nullptr; return; }
+  char *base = jb.base;
   void *d_kv = base + off[0];
   float *d_w = w_host ? (float *)(base + off[1]) : nullptr;
   gsrq_codebook cb{K, S, (float *)(base + off[2]), (float *)(base + off[3])};
@@ -1547,7 +1554,9 @@ int gsrq_pipeline_host(const void *kv_host, const gsrq_view *view, const float *
   int64_t *d_ft = fit_tokens_host ? (int64_t *)(base + off[8]) : nullptr;
   int *d_err = (int *)(base + off[9]);
   const Plan pl = make_plan(view, K, S, fit_tokens_host ? n_fit : 0);
-  e = cudaMemcpyAsync(d_kv, kv_host, kv_bytes, cudaMemcpyHostToDevice, stream);
+  if (h2d_after) e = cudaStreamWaitEvent(stream, h2d_after, 0);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(d_kv, kv_host, kv_bytes, cudaMemcpyHostToDevice, stream);
+  if (e == cudaSuccess && h2d_done) e = cudaEventRecord(h2d_done, stream);
   if (e == cudaSuccess && w_host) e = cudaMemcpyAsync(d_w, w_host, (size_t)view->T * 4, cudaMemcpyHostToDevice, stream);
   if (e == cudaSuccess && d_ft) e = cudaMemcpyAsync(d_ft, fit_tokens_host, ft_bytes, cudaMemcpyHostToDevice, stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(d_err, 0, sizeof(int), stream);
@@ -1569,18 +1578,75 @@ int gsrq_pipeline_host(const void *kv_host, const gsrq_view *view, const float *
     rc = gsrq_decode(d_codes, &cb, S, d_out, view, stream);
     if (rc == GSRQ_OK) e = cudaMemcpyAsync(kv_out_host, d_out, kv_bytes, cudaMemcpyDeviceToHost, stream);
   }
-  int h_err = 0;
   if (rc == GSRQ_OK && e == cudaSuccess) e = cudaMemcpyAsync(shapes_host, cb.shapes, sh_bytes, cudaMemcpyDeviceToHost, stream);
   if (rc == GSRQ_OK && e == cudaSuccess) e = cudaMemcpyAsync(gains_host, cb.gains, ga_bytes, cudaMemcpyDeviceToHost, stream);
   if (rc == GSRQ_OK && e == cudaSuccess) e = cudaMemcpyAsync(codes_host, d_codes, n_rows * S, cudaMemcpyDeviceToHost, stream);
-  if (rc == GSRQ_OK && e == cudaSuccess) e = cudaMemcpyAsync(&h_err, d_err, sizeof(int), cudaMemcpyDeviceToHost, stream);
-  cudaFreeAsync(base, stream);
-  cudaError_t e2 = cudaStreamSynchronize(stream);
-  if (e == cudaSuccess) e = e2;
+  if (rc == GSRQ_OK && e == cudaSuccess) e = cudaMemcpyAsync(jb.h_err, d_err, sizeof(int), cudaMemcpyDeviceToHost, stream);
+}
+
+// Waits for the job's stream, returns its memory to the pool; the job's status.
+static int pipeline_finish(PipeJob &jb) {
+  if (jb.base) cudaFreeAsync(jb.base, jb.stream);
+  const cudaError_t e2 = cudaStreamSynchronize(jb.stream);
+  if (jb.e == cudaSuccess) jb.e = e2;
+  if (jb.e != cudaSuccess) { set_error("gsrq_pipeline_host: %s", cudaGetErrorString(jb.e)); cudaGetLastError(); return GSRQ_ECUDA; }
+  if (jb.rc == GSRQ_OK && *jb.h_err == GSRQ_EDEGENERATE) { set_error("a group has fewer than K distinct non-zero fit rows"); return GSRQ_EDEGENERATE; }
+  if (jb.rc == GSRQ_OK && *jb.h_err != 0) { set_error("the fit kernel's group barrier timed out"); return GSRQ_ECUDA; }
+  return jb.rc;
+}
+
+int gsrq_pipeline_host_batch(int n, const void *const *kv_host, const gsrq_view *view, const float *const *w_host,
+                             const int64_t *const *fit_tokens_host, int64_t n_fit, int K, int S, int iters, uint64_t seed,
+                             float *const *shapes_host, float *const *gains_host, uint8_t *const *codes_host, void *const *kv_out_host) {
+  if (n <= 0 || n > 64 || !kv_host || !shapes_host || !gains_host || !codes_host) { set_error("gsrq_pipeline_host_batch: need 1..64 tensors and non-NULL pointer arrays"); return GSRQ_EINVAL; }
+  int rc = check_view(view, K, S);
+  if (rc) return rc;
+  for (int i = 0; i < n; ++i) {
+    if (!kv_host[i] || !shapes_host[i] || !gains_host[i] || !codes_host[i]) { set_error("NULL input (tensor %d)", i); return GSRQ_EINVAL; }
+    const int64_t *ft = fit_tokens_host ? fit_tokens_host[i] : nullptr;
+    if (ft && (n_fit <= 0 || n_fit > view->T)) { set_error("n_fit out of range"); return GSRQ_EINVAL; }
+  }
+  cudaMemPool_t pool = host_pool();
+  if (!pool) { set_error("gsrq_pipeline_host: could not create the device memory pool"); return GSRQ_ECUDA; }
+  // two streams, tensors alternate between them: tensor i + 1 uploads while tensor i computes and downloads (the two copy
+  // directions and the SMs work at the same time); a stream's next tensor starts when its previous one is done
+  cudaStream_t st[2] = {nullptr, nullptr};
+  cudaEvent_t up[2] = {nullptr, nullptr};
+  const int ns = n > 1 ? 2 : 1;
+  cudaError_t e = cudaSuccess;
+  for (int q = 0; q < ns && e == cudaSuccess; ++q) {
+    e = cudaStreamCreateWithFlags(&st[q], cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&up[q], cudaEventDisableTiming);
+  }
+  std::vector<PipeJob> jobs((size_t)n);
+  int first_bad = GSRQ_OK;
+  int *h_errs = nullptr;
+  if (e == cudaSuccess) e = cudaHostAlloc((void **)&h_errs, (size_t)n * sizeof(int), cudaHostAllocDefault);
+  if (e == cudaSuccess) {
+    for (int i = 0; i < n; ++i) {
+      PipeJob &jb = jobs[(size_t)i];
+      jb.stream = st[i % ns];
+      jb.h_err = h_errs + i;
+      *jb.h_err = 0;
+      if (i >= ns) { const int r = pipeline_finish(jobs[(size_t)(i - ns)]); if (r != GSRQ_OK && first_bad == GSRQ_OK) first_bad = r; }   // its stream (and event) are free again
+      pipeline_enqueue(jb, pool, kv_host[i], view, w_host ? w_host[i] : nullptr, fit_tokens_host ? fit_tokens_host[i] : nullptr, n_fit, K, S, iters, seed,
+                       shapes_host[i], gains_host[i], codes_host[i], kv_out_host ? kv_out_host[i] : nullptr, (i > 0 && ns > 1) ? up[(i - 1) % ns] : nullptr,
+                       ns > 1 ? up[i % ns] : nullptr);
+    }
+    for (int i = (n > ns ? n - ns : 0); i < n; ++i) { const int r = pipeline_finish(jobs[(size_t)i]); if (r != GSRQ_OK && first_bad == GSRQ_OK) first_bad = r; }
+  }
+  for (int q = 0; q < ns; ++q) { if (up[q]) cudaEventDestroy(up[q]); if (st[q]) cudaStreamDestroy(st[q]); }
+  if (h_errs) cudaFreeHost(h_errs);
   if (e != cudaSuccess) { set_error("gsrq_pipeline_host: %s", cudaGetErrorString(e)); return GSRQ_ECUDA; }
-  if (rc == GSRQ_OK && h_err == GSRQ_EDEGENERATE) { set_error("a group has fewer than K distinct non-zero fit rows"); return GSRQ_EDEGENERATE; }
-  if (rc == GSRQ_OK && h_err != 0) { set_error("the fit kernel's group barrier timed out"); return GSRQ_ECUDA; }
-  return rc;
+  return first_bad;
+}
+
+int gsrq_pipeline_host(const void *kv_host, const gsrq_view *view, const float *w_host, const int64_t *fit_tokens_host,
+                       int64_t n_fit, int K, int S, int iters, uint64_t seed, float *shapes_host, float *gains_host,
+                       uint8_t *codes_host, void *kv_out_host) {
+  if (!kv_host || !shapes_host || !gains_host || !codes_host) { set_error("NULL input"); return GSRQ_EINVAL; }
+  return gsrq_pipeline_host_batch(1, &kv_host, view, &w_host, &fit_tokens_host, n_fit, K, S, iters, seed, &shapes_host, &gains_host, &codes_host,
+                                  &kv_out_host);
 }
 
 void gsrq_release_host_pool(void) {

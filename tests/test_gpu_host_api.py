@@ -53,6 +53,39 @@ def test_pipeline_host_reports_a_degenerate_group(B):
     assert e.value.code == -5
 
 
+def test_pipeline_host_batch_equals_single_calls(B):
+    """Three tensors (K-like, V-like, K-like) in one pipelined call over two streams: bit-identical to three gsrq_pipeline_host calls;
+    the third tensor reuses the first one's stream.  One of them without decode output."""
+    c = inputs.CONFIGS[1]
+    T, K, S, iters = 1024, 256, 2, 4
+    xs = [inputs.k_like(c.G, T, c.hd, 901), inputs.v_like(c.G, T, c.hd, 902), inputs.k_like(c.G, T, c.hd, 903)]
+    w = inputs.token_weights(T, 904)
+    fit = inputs.fit_sample(c.G, T, 300, 905)
+    M = c.hd // c.d
+    x_h = [torch.from_numpy(x).to(torch.bfloat16).pin_memory() for x in xs]
+    w_h = torch.from_numpy(w).pin_memory(); fit_h = torch.from_numpy(fit).pin_memory()
+    view = B.view_of(x_h[0], c.d)
+    mk = lambda: (torch.empty(c.G, S, K, c.d).pin_memory(), torch.empty(c.G, S, K).pin_memory(),
+                  torch.empty(S, c.G, T * M, dtype=torch.uint8).pin_memory(), torch.empty(c.G, T, c.hd, dtype=torch.bfloat16).pin_memory())
+    single = [mk() for _ in xs]
+    for x, (sh, ga, co, out) in zip(x_h, single):
+        B.gsrq_pipeline_host(x, view, w_h, fit_h, K, S, iters, 0, sh, ga, co, out)
+    batch = [mk() for _ in xs]
+    B.gsrq_pipeline_host_batch(x_h, view, [w_h] * 3, [fit_h] * 3, K, S, iters, 0, [b[0] for b in batch], [b[1] for b in batch], [b[2] for b in batch],
+                               [batch[0][3], None, batch[2][3]])
+    for i, (s_, b_) in enumerate(zip(single, batch)):
+        assert torch.equal(s_[0], b_[0]) and torch.equal(s_[1], b_[1]) and torch.equal(s_[2], b_[2]), i
+        if i != 1:
+            assert torch.equal(s_[3], b_[3]), i
+    # a degenerate tensor in the middle is reported, the others are still processed
+    bad = torch.zeros_like(x_h[1])
+    with pytest.raises(B.GsrqError) as e:
+        B.gsrq_pipeline_host_batch([x_h[0], bad, x_h[2]], view, None, None, K, S, 2, 0, [b[0] for b in batch], [b[1] for b in batch],
+                                   [b[2] for b in batch], None)
+    assert e.value.code == -5
+    B.gsrq_release_host_pool()
+
+
 def test_misaligned_tensor_pointer_is_an_error_not_a_fault(B):
     buf = torch.zeros(2 * 64 * 128 + 8, dtype=torch.bfloat16, device="cuda")
     x = buf[4:4 + 2 * 64 * 128].view(2, 64, 128)            # base offset by 8 bytes
