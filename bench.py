@@ -491,13 +491,26 @@ def main():
     # ---- rooflines: algorithmic work per launch / live launch duration ----
     tot_ms = sum(v[0] for v in prof.values())
 
+    def ncu_traffic(cls):
+        """dram__bytes_read.sum + dram__bytes_write.sum per launch of the class (average over its launches per tensor), from the committed
+        ncu --set full capture of this command (profiles/r2_traffic.csv; not measured in this run); None without the file."""
+        try:
+            import csv
+            with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "profiles", "r2_traffic.csv")) as f:
+                rws = [r for r in csv.DictReader(f) if r["class"] == cls]
+            n_l = sum(int(r["launches_per_tensor"]) for r in rws)
+            return sum((int(r["dram_bytes_read"]) + int(r["dram_bytes_write"])) * int(r["launches_per_tensor"]) for r in rws) / n_l if n_l else None
+        except (OSError, KeyError, ValueError):
+            return None
+
     def kern(name, cls, bound, work_per_launch, unit, note):
         ms_c, n = prof[cls]
         per = ms_c / max(n, 1)
         peak = pk["bf16_tflops_sustained"] if bound == "tensor" else pk["hbm_gbs"]
         ach = work_per_launch / (per * 1e-3) / (1e12 if bound == "tensor" else 1e9) if per > 0 else 0.0
-        return dict(bound=bound, kernel=name, achieved=ach, peak=peak, unit=unit, frac=ach / peak, traffic=None,
-                    traffic_note="dram__bytes of this kernel: see the ncu --set full summaries under profiles/ (not measured in this run)",
+        return dict(bound=bound, kernel=name, achieved=ach, peak=peak, unit=unit, frac=ach / peak, traffic=ncu_traffic(cls),
+                    traffic_note="bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum, class average) from the committed ncu --set full capture "
+                                 "of this command: profiles/r2_traffic.csv, profiles/r2_ncu_summaries.md; not measured in this run",
                     algorithmic_per_launch=work_per_launch, ms_per_launch=per, launches=n,
                     share_of_step=ms_c / tot_ms if tot_ms else None, note=note)
 
