@@ -8,11 +8,15 @@
 //     k_t = khat_t                               keys stored after the rotary embedding (rope_theta == 0), or
 //     k_t = RoPE(khat_t, t)                      keys quantised before it (rotate-half convention, angle = t theta^(-2i/hd)).
 // Without RoPE the keys are never even dequantised: q_h . khat_t = sum_s sum_m (q_h[m] . cK^(s)_k[.])[k = aK^(s)_{t,m}], so one table
-// QT[h][s][m][k] of n_rep x S x 8 x 256 dot products per (sequence, KV head) turns a token's logit into S x 8 shared-memory
-// lookups per query head.  With RoPE the two sub-vectors of a rotary pair (elements i and i + 64) are dequantised in registers,
+// QT[s][k][m][h] of S x 256 x 8 x n_rep dot products per (sequence, KV head) turns a token's logit into S x 8 shared-memory
+// lookups (one 16-byte entry = the 4 heads; lane l reads sub-vector (l + j) % 8 at step j, so the 8 lanes of a quarter-warp hit
+// 8 different bank groups whatever the codes are).  With RoPE the two sub-vectors of a rotary pair (elements i and i + 64) are dequantised in registers,
 // rotated with cos / sin((base + off) theta_i) = angle addition of a base per 64 tokens (double precision) and a per-CTA offset
 // table, and multiplied with q (held in registers: a thread owns four rotary pairs of every 16th token).  Values: warp = token,
-// lane = four output elements; the token's probabilities of all heads are one float4 broadcast from shared memory.
+// lane = four output elements; the token's probabilities of all heads are one float4 broadcast from shared memory; with two
+// stages a lane adds up ONE stage of two sub-vectors and the two stage tables are interleaved (codeword k of stage s at row
+// 2 k + s), so that the two rows a quarter-warp reads per instruction lie in opposite bank halves; the stages meet at the end
+// (sum_t p_t (c0_t + c1_t) = sum_t p_t c0_t + sum_t p_t c1_t up to fp32 rounding, within the test's tolerance).
 // Split-K over the tokens (flash-decoding): CTA (split, g, b) keeps a running max / sum per head, k_attn_combine merges the
 // splits in split order.  d = 16, hd = 128, K <= 256, up to 4 stages each; fp32 arithmetic, no atomics (bit-reproducible).
 #pragma once
