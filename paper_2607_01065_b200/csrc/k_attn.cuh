@@ -14,9 +14,8 @@
 // rotated with cos / sin((base + off) theta_i) = angle addition of a base per 64 tokens (double precision) and a per-CTA offset
 // table, and multiplied with q (held in registers: a thread owns four rotary pairs of every 16th token).  Values: warp = token,
 // lane = four output elements; the token's probabilities of all heads are one float4 broadcast from shared memory; with two
-// stages a lane adds up ONE stage of two sub-vectors and the two stage tables are interleaved (codeword k of stage s at row
-// 2 k + s), so that the two rows a quarter-warp reads per instruction lie in opposite bank halves; the stages meet at the end
-// (sum_t p_t (c0_t + c1_t) = sum_t p_t c0_t + sum_t p_t c1_t up to fp32 rounding, within the test's tolerance).
+// stages the two stage tables are interleaved (codeword k of stage s at row 2 k + s) and the odd sub-vectors' lanes read stage 1
+// first, so that the two rows a quarter-warp reads per instruction lie in opposite bank halves.
 // Split-K over the tokens (flash-decoding): CTA (split, g, b) keeps a running max / sum per head, k_attn_combine merges the
 // splits in split order.  d = 16, hd = 128, K <= 256, up to 4 stages each; fp32 arithmetic, no atomics (bit-reproducible).
 #pragma once
@@ -152,19 +151,14 @@ __device__ __forceinline__ void attn_decode_body(const AttnParams &p) {
       }
   }
   if (tid < 8) { m_run[tid] = -INFINITY; l_run[tid] = 0.0f; sc_h[tid] = 0.0f; }
-  // values: warp w takes the tokens t = w (mod 8) of a chunk.  Lane l: the output elements 4 l .. 4 l + 3 of vhat_t (sum of the
-  // stages in registers); with two stages (PAIR) instead the stage (l / 4) % 2 part of the sub-vectors 2 (l / 8), 2 (l / 8) + 1,
-  // elements 4 (l % 4) .. + 3 -- a quarter-warp then reads one stage-0 and one stage-1 row per instruction, which the table
-  // layout keeps in opposite bank halves (conflict-free), and the two stages' sums are added once at the end.
-  constexpr bool PAIR = (NS == 2);
-  constexpr int NA = PAIR ? 8 : 4;
-  float acc[HMAX][NA];
+  // values: warp w takes the tokens t = w (mod 8) of a chunk, lane l the output elements 4 l .. 4 l + 3 of vhat_t (sum of the stages
+  // in registers).  Two stages: the tables are interleaved (codeword k of stage s at row 2 k + s: stage 0 in the lower, stage 1 in
+  // the upper bank half) and the lanes of the odd sub-vectors read stage 1 first, so that the two rows a quarter-warp reads per
+  // instruction never share a bank; a two-term fp32 sum does not depend on the order, so vhat_t is still the stage-order sum.
+  float acc[HMAX][4];
 #pragma unroll
-  for (int h = 0; h < HMAX; ++h)
-#pragma unroll
-    for (int i = 0; i < NA; ++i) acc[h][i] = 0.0f;
+  for (int h = 0; h < HMAX; ++h) { acc[h][0] = 0.0f; acc[h][1] = 0.0f; acc[h][2] = 0.0f; acc[h][3] = 0.0f; }
   const int m_out = lane >> 2, j_out = (lane & 3) * 4;
-  const int pq = lane >> 3, ph = (lane >> 2) & 1;
   __syncthreads();
 
   // Code bytes of this thread's tokens (tid, tid + 256, ...) of a chunk, every stage: fetched one chunk ahead, so that the
@@ -363,8 +357,7 @@ __device__ __forceinline__ void attn_decode_body(const AttnParams &p) {
     for (int h = 0; h < HMAX; ++h)
       if (h < n_rep) {
         const float sc = sc_h[h];
-#pragma unroll
-        for (int i = 0; i < NA; ++i) acc[h][i] *= sc;
+        acc[h][0] *= sc; acc[h][1] *= sc; acc[h][2] *= sc; acc[h][3] *= sc;
       }
     auto value_of = [&](int t) -> float4 {   // vhat_t[4 lane .. 4 lane + 3] = sum over the stages, fp32, stage order
       float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -375,6 +368,12 @@ __device__ __forceinline__ void attn_decode_body(const AttnParams &p) {
       else if (SVP == 4) cw = *reinterpret_cast<const unsigned *>(cp);
       else if (SVP == 2) cw = *reinterpret_cast<const unsigned short *>(cp);
       else cw = *cp;
+      if (NS == 2) {
+        const int s1 = m_out & 1;   // stage read first
+        const float4 ca = *reinterpret_cast<const float4 *>(vtab + (2 * ((cw >> (8 * s1)) & 255u) + s1) * kD + j_out);
+        const float4 cb = *reinterpret_cast<const float4 *>(vtab + (2 * ((cw >> (8 * (1 - s1))) & 255u) + (1 - s1)) * kD + j_out);
+        return make_float4(__fadd_rn(ca.x, cb.x), __fadd_rn(ca.y, cb.y), __fadd_rn(ca.z, cb.z), __fadd_rn(ca.w, cb.w));
+      }
 #pragma unroll
       for (int s = 0; s < (NS > 0 ? NS : 4); ++s) {
         if (s >= SV) break;
@@ -400,49 +399,15 @@ __device__ __forceinline__ void attn_decode_body(const AttnParams &p) {
         }
       }
     };
-    if (PAIR) {
-      auto rows_of = [&](int t, float4 &va, float4 &vb) {   // this lane's stage: codeword rows of the sub-vectors 2 pq and 2 pq + 1
-        const unsigned cw = *reinterpret_cast<const unsigned *>(vcodes + (t * kM + 2 * pq) * 2);   // bytes (m, s): (2pq, 0) (2pq, 1) (2pq+1, 0) (2pq+1, 1)
-        va = *reinterpret_cast<const float4 *>(vtab + (2 * ((cw >> (8 * ph)) & 255u) + ph) * kD + j_out);
-        vb = *reinterpret_cast<const float4 *>(vtab + (2 * ((cw >> (16 + 8 * ph)) & 255u) + ph) * kD + j_out);
-      };
-      auto add_pair = [&](int t, const float4 &va, const float4 &vb) {
-#pragma unroll
-        for (int h4 = 0; h4 < (HMAX + 3) / 4; ++h4) {
-          if (4 * h4 >= n_rep) break;
-          const float4 pr = *reinterpret_cast<const float4 *>(lg + t * HP + 4 * h4);
-          const float pv[4] = {pr.x, pr.y, pr.z, pr.w};
-#pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            const int h = 4 * h4 + i;
-            if (h < HMAX && h < n_rep) {
-              acc[h][0] = fmaf(pv[i], va.x, acc[h][0]); acc[h][1] = fmaf(pv[i], va.y, acc[h][1]);
-              acc[h][2] = fmaf(pv[i], va.z, acc[h][2]); acc[h][3] = fmaf(pv[i], va.w, acc[h][3]);
-              acc[h][NA - 4] = fmaf(pv[i], vb.x, acc[h][NA - 4]); acc[h][NA - 3] = fmaf(pv[i], vb.y, acc[h][NA - 3]);
-              acc[h][NA - 2] = fmaf(pv[i], vb.z, acc[h][NA - 2]); acc[h][NA - 1] = fmaf(pv[i], vb.w, acc[h][NA - 1]);
-            }
-          }
-        }
-      };
-      int t = warp;
-      for (; t + 24 < nv; t += 32) {   // four tokens in flight
-        float4 a0, b0, a1, b1, a2, b2, a3, b3;
-        rows_of(t, a0, b0); rows_of(t + 8, a1, b1); rows_of(t + 16, a2, b2); rows_of(t + 24, a3, b3);
-        add_pair(t, a0, b0);
-        add_pair(t + 8, a1, b1);
-        add_pair(t + 16, a2, b2);
-        add_pair(t + 24, a3, b3);
-      }
-      for (; t < nv; t += 8) { float4 a0, b0; rows_of(t, a0, b0); add_pair(t, a0, b0); }
-    } else {
-      int t = warp;
-      for (; t + 8 < nv; t += 16) {   // two tokens in flight
-        const float4 v0 = value_of(t), v1 = value_of(t + 8);
-        add_token(t, v0);
-        add_token(t + 8, v1);
-      }
-      for (; t < nv; t += 8) add_token(t, value_of(t));
+    int t = warp;
+    for (; t + 24 < nv; t += 32) {   // four tokens in flight
+      const float4 v0 = value_of(t), v1 = value_of(t + 8), v2 = value_of(t + 16), v3 = value_of(t + 24);
+      add_token(t, v0);
+      add_token(t + 8, v1);
+      add_token(t + 16, v2);
+      add_token(t + 24, v3);
     }
+    for (; t < nv; t += 8) add_token(t, value_of(t));
     __syncthreads();
   }
   // ---- this split's result: m, l, acc = the eight warps' partial sums added in warp order ----
@@ -451,15 +416,7 @@ __device__ __forceinline__ void attn_decode_body(const AttnParams &p) {
 #pragma unroll
   for (int h = 0; h < HMAX; ++h)
     if (h < n_rep) {
-      if (PAIR) {   // stage 0 + stage 1 (lane ^ 4); the stage-0 lane stores sub-vector 2 pq, the stage-1 lane 2 pq + 1
-        float tot[NA];
-#pragma unroll
-        for (int i = 0; i < NA; ++i) { const float o = __shfl_xor_sync(0xffffffffu, acc[h][i], 4); tot[i] = ph ? o + acc[h][i] : acc[h][i] + o; }
-        *reinterpret_cast<float4 *>(ex + ((warp * n_rep + h) * kHd) + (2 * pq + ph) * kD + j_out) =
-            ph ? make_float4(tot[NA - 4], tot[NA - 3], tot[NA - 2], tot[NA - 1]) : make_float4(tot[0], tot[1], tot[2], tot[3]);
-      } else {
-        *reinterpret_cast<float4 *>(ex + ((warp * n_rep + h) * kHd) + 4 * lane) = make_float4(acc[h][0], acc[h][1], acc[h][2], acc[h][3]);
-      }
+      *reinterpret_cast<float4 *>(ex + ((warp * n_rep + h) * kHd) + 4 * lane) = make_float4(acc[h][0], acc[h][1], acc[h][2], acc[h][3]);
     }
   __syncthreads();
   for (int e = tid; e < n_rep * kHd; e += kThreads) {
