@@ -247,6 +247,43 @@ int gsrq_attention_decode(const float *q, const uint8_t *k_codes, const gsrq_cod
                           int64_t max_len, int B, int Hq, int G, int hd, int d, float scale, float rope_theta, float *out,
                           void *workspace, size_t workspace_bytes, gsrq_stream_t stream);
 
+/*
+ * gsrq_attention_decode for callers that cannot provide scratch memory.
+ *
+ * Who this is for: code that runs where device memory can no longer be obtained, so that it has no workspace to pass to
+ * gsrq_attention_decode -- a serving loop whose memory manager has claimed the whole GPU for the KV cache and hands nothing back;
+ * a plug-in called from inside somebody else's stream capture or latency-critical section, where cudaMalloc / cudaFree are not
+ * permitted (they synchronise the device, and are not allowed while a stream is capturing); a host that forbids allocation after
+ * start-up.  This call, and everything under it, calls no cudaMalloc, no cudaFree, no memory pool and no other allocating routine:
+ * the per-split partial results go to a fixed buffer of GSRQ_ATTENTION_STATIC_SCRATCH_BYTES that is part of the library image.
+ * Every GPU on which the library's kernels are loaded holds that buffer from then until the process exits, used or not.
+ *
+ * Arguments, arithmetic, shapes served and results are those of gsrq_attention_decode (bit-identical: same kernels, same split of
+ * the token range), without `workspace` / `workspace_bytes`.  The caller still owns and passes q, the code planes, the codebooks,
+ * seq_start / seq_len and out (device pointers).
+ *
+ * Limit: B * G * n_split * (Hq / G) * 130 * 4 bytes must fit in the buffer, n_split being the library's split of the token range
+ * (at most 4 * SM count / (B * G), at most one per 2048 tokens of max_len, at least 1).  With LLaMA-3-8B's 8 KV heads and 4 query
+ * heads per KV head that is every batch up to 252 sequences (batch 8 x 131072 tokens needs 1.2 MiB).  A larger request returns
+ * GSRQ_EWORKSPACE with the needed and available sizes in gsrq_last_error(), and launches nothing; use gsrq_attention_decode then.
+ *
+ * First call on each device: looks up the buffer's device address (cudaGetSymbolAddress, with the caller's current device), which
+ * can make the CUDA runtime load the library's device code.  Make this first call at start-up on every device that will be used,
+ * outside any stream capture; later calls only read the cached address.
+ *
+ * One buffer per device, shared by every call in the process, and not cleared between calls (no entry has to start at zero:
+ * each call overwrites every entry it later reads).  Two calls that can run at the same time on one GPU -- issued to different
+ * streams without an ordering between them, or from two threads -- overwrite each other's partial results and return garbage:
+ * order them (same stream, or an event).  Calls on different GPUs are independent.  The launches of this entry point are counted by
+ * gsrq_launch_count() but are never event-timed by gsrq_profile_enable().
+ */
+#define GSRQ_ATTENTION_STATIC_SCRATCH_BYTES (4u << 20)
+size_t gsrq_attention_static_scratch_bytes(void); /* == GSRQ_ATTENTION_STATIC_SCRATCH_BYTES; host function, no CUDA calls */
+int gsrq_attention_decode_static(const float *q, const uint8_t *k_codes, const gsrq_codebook *k_cb, int k_stages, const uint8_t *v_codes,
+                                 const gsrq_codebook *v_cb, int v_stages, int64_t plane_rows, const int64_t *seq_start,
+                                 const int64_t *seq_len, int64_t max_len, int B, int Hq, int G, int hd, int d, float scale,
+                                 float rope_theta, float *out, gsrq_stream_t stream);
+
 /* ---- stand-alone clustering of fp32 rows: GSKM against the K-means baseline (section 6.1, :200-212; section 4, :60-85) ---- */
 
 /* Scratch for the three calls below (host function, no CUDA calls); 0 on bad arguments. */

@@ -42,7 +42,7 @@ class gsrq_fit_stats(C.Structure):
 
 _lib = None
 EXPORTS = ["gsrq_log_weights", "gsrq_encode_pervector_gain", "gsrq_decode_pervector_gain", "gsrq_pack_nibbles", "gsrq_unpack_nibbles",
-           "gsrq_attention_workspace_bytes", "gsrq_attention_decode", "gsrq_cluster_workspace_bytes", "gsrq_cluster_fit", "gsrq_cluster_assign", "gsrq_cluster_metrics", "gsrq_workspace_bytes", "gsrq_fit_stage", "gsrq_encode", "gsrq_decode", "gsrq_encode_append", "gsrq_assign", "gsrq_update",
+           "gsrq_attention_workspace_bytes", "gsrq_attention_decode", "gsrq_attention_static_scratch_bytes", "gsrq_attention_decode_static", "gsrq_cluster_workspace_bytes", "gsrq_cluster_fit", "gsrq_cluster_assign", "gsrq_cluster_metrics", "gsrq_workspace_bytes", "gsrq_fit_stage", "gsrq_encode", "gsrq_decode", "gsrq_encode_append", "gsrq_assign", "gsrq_update",
            "gsrq_init_ids", "gsrq_debug_scores", "gsrq_encode_host", "gsrq_decode_host", "gsrq_pipeline_host", "gsrq_pipeline_host_batch", "gsrq_release_host_pool", "gsrq_profile_enable",
            "gsrq_profile_read", "gsrq_launch_count", "gsrq_last_error", "gsrq_version"]
 
@@ -62,6 +62,7 @@ def lib():
         _lib.gsrq_workspace_bytes.restype = C.c_size_t
         _lib.gsrq_cluster_workspace_bytes.restype = C.c_size_t
         _lib.gsrq_attention_workspace_bytes.restype = C.c_size_t
+        _lib.gsrq_attention_static_scratch_bytes.restype = C.c_size_t
         _lib.gsrq_last_error.restype = C.c_char_p
         _lib.gsrq_version.restype = C.c_char_p
         _lib.gsrq_launch_count.restype = C.c_int64
@@ -174,6 +175,22 @@ def gsrq_attention_decode(q, k_codes, k_cb, k_stages, v_codes, v_cb, v_stages, p
                                        C.c_int64(plane_rows), _ptr(seq_start), _ptr(seq_len), C.c_int64(max_len), Bq, Hq, G, hd, d,
                                        C.c_float(scale), C.c_float(rope_theta), _ptr(out), _ptr(ws), C.c_size_t(ws.numel()), _stream()))
     return ws
+
+
+def gsrq_attention_static_scratch_bytes():
+    return int(lib().gsrq_attention_static_scratch_bytes())
+
+
+def gsrq_attention_decode_static(q, k_codes, k_cb, k_stages, v_codes, v_cb, v_stages, plane_rows, seq_start, seq_len, max_len, G, d, scale,
+                                 rope_theta, out):
+    """gsrq_attention_decode without a workspace: for callers that cannot obtain device memory (an engine that has given the whole
+    GPU to its KV cache, code running inside a stream capture, a no-allocation-after-start-up host).  The partial results go to a
+    fixed 4 MiB buffer inside the library; larger requests raise GSRQ_EWORKSPACE.  Same tensors and results as gsrq_attention_decode;
+    calls that overlap on one GPU race on the shared buffer (include/gsrq.h)."""
+    Bq, Hq, hd = q.shape
+    _check(lib().gsrq_attention_decode_static(_ptr(q), _ptr(k_codes), C.byref(k_cb), k_stages, _ptr(v_codes), C.byref(v_cb), v_stages,
+                                              C.c_int64(plane_rows), _ptr(seq_start), _ptr(seq_len), C.c_int64(max_len), Bq, Hq, G, hd, d,
+                                              C.c_float(scale), C.c_float(rope_theta), _ptr(out), _stream()))
 
 
 def gsrq_log_weights(grad, view, tau, eps, w_out):

@@ -1361,6 +1361,110 @@ int gsrq_attention_decode(const float *q, const uint8_t *k_codes, const gsrq_cod
   return GSRQ_OK;
 }
 
+// ---- gsrq_attention_decode_static: the attention step for callers that have no way to hand over scratch memory ----
+//
+// The attention kernels leave one partial result (running max, sum, 128 accumulators) per (sequence, KV head, split, query head) in
+// global memory and a second kernel merges the splits.  gsrq_attention_decode takes that buffer from the caller's workspace.  Here
+// it lives in the library image instead: a fixed array in device global memory that the CUDA runtime places when it loads this
+// module on a GPU, and that stays there until the process exits (every GPU this library is used on pays the 4 MiB once).
+//
+// g_attn_static_part, as host code sees it, is only a handle for the runtime; it is NOT the array's device address and must never
+// be given to a kernel.  The address is asked for once per device (cudaGetSymbolAddress, with that device current) and kept in
+// g_attn_static_ptr[device].
+static __device__ __align__(256) float g_attn_static_part[GSRQ_ATTENTION_STATIC_SCRATCH_BYTES / sizeof(float)];
+static float *g_attn_static_ptr[64] = {nullptr};
+static std::mutex g_attn_static_mu;
+
+// Device address of the static partial buffer on the CURRENT device (set-up on the first call per device, then a table lookup).
+static int attn_static_scratch(float **out) {
+  int dev = 0;
+  GSRQ_CUDA_CHECK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) { set_error("attention (static scratch): device ordinal %d out of range", dev); return GSRQ_ECUDA; }
+  std::lock_guard<std::mutex> lk(g_attn_static_mu);
+  if (!g_attn_static_ptr[dev]) {
+    float *ptr = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress((void **)&ptr, g_attn_static_part);
+    if (e != cudaSuccess || !ptr) {
+      set_error("attention (static scratch): cudaGetSymbolAddress failed on device %d: %s", dev, cudaGetErrorString(e));
+      return GSRQ_ECUDA;
+    }
+    g_attn_static_ptr[dev] = ptr;
+  }
+  *out = g_attn_static_ptr[dev];
+  return GSRQ_OK;
+}
+
+size_t gsrq_attention_static_scratch_bytes(void) { return sizeof(g_attn_static_part); }
+
+int gsrq_attention_decode_static(const float *q, const uint8_t *k_codes, const gsrq_codebook *k_cb, int k_stages, const uint8_t *v_codes,
+                                 const gsrq_codebook *v_cb, int v_stages, int64_t plane_rows, const int64_t *seq_start,
+                                 const int64_t *seq_len, int64_t max_len, int B, int Hq, int G, int hd, int d, float scale,
+                                 float rope_theta, float *out, gsrq_stream_t stream_) {
+  cudaStream_t stream = (cudaStream_t)stream_;
+  if (!q || !k_codes || !v_codes || !k_cb || !v_cb || !k_cb->shapes || !k_cb->gains || !v_cb->shapes || !v_cb->gains || !seq_start || !seq_len || !out) {
+    set_error("NULL input"); return GSRQ_EINVAL;
+  }
+  if (hd != attn::kHd || d != attn::kD) { set_error("attention: this build serves head_dim 128 with d = 16 (got %d, %d)", hd, d); return GSRQ_EUNSUPPORTED; }
+  if (B <= 0 || B > 65535 || G <= 0 || G > 65535 || Hq <= 0 || Hq % G || Hq / G > 8) {
+    set_error("attention: need B, G <= 65535 and Hq a multiple of G with at most 8 query heads per KV head"); return GSRQ_EINVAL;
+  }
+  if (k_cb->K < 1 || k_cb->K > 256 || v_cb->K < 1 || v_cb->K > 256 || k_stages < 1 || k_stages > 4 || k_stages > k_cb->S || v_stages < 1 || v_stages > 4 ||
+      v_stages > v_cb->S) { set_error("attention: K in [1, 256] and 1..4 stages (<= S) for keys and values"); return GSRQ_EINVAL; }
+  if (plane_rows <= 0 || plane_rows % attn::kM || max_len < 0 || rope_theta < 0.0f) { set_error("attention: bad plane_rows / max_len / rope_theta"); return GSRQ_EINVAL; }
+  if (((uintptr_t)k_codes & 7) || ((uintptr_t)v_codes & 7)) { set_error("code planes must be 8-byte aligned"); return GSRQ_EINVAL; }
+  if (((uintptr_t)k_cb->shapes & 15) || ((uintptr_t)v_cb->shapes & 15)) { set_error("codebook shapes must be 16-byte aligned"); return GSRQ_EINVAL; }
+  // the same split of the token range as gsrq_attention_decode (so the two paths add in the same order and agree bit for bit)
+  const int n_split = attn_splits(B, G, max_len), n_rep = Hq / G;
+  const size_t need = (size_t)B * G * n_split * n_rep * attn::kPartStride * sizeof(float);
+  if (need > sizeof(g_attn_static_part)) {
+    set_error("attention (static scratch): B = %d sequences x G = %d KV heads x %d splits x %d query heads per KV head need %zu bytes of "
+              "partial results, the built-in buffer holds %zu; use gsrq_attention_decode with a workspace", B, G, n_split, n_rep, need,
+              sizeof(g_attn_static_part));
+    return GSRQ_EWORKSPACE;
+  }
+  float *part = nullptr;
+  int rc = attn_static_scratch(&part);
+  if (rc) return rc;
+  attn::AttnParams p{};
+  p.q = q; p.kc = k_codes; p.vc = v_codes; p.k_shapes = k_cb->shapes; p.k_gains = k_cb->gains; p.v_shapes = v_cb->shapes; p.v_gains = v_cb->gains;
+  p.kS = k_cb->S; p.kK = k_cb->K; p.vS = v_cb->S; p.vK = v_cb->K; p.k_stages = k_stages; p.v_stages = v_stages; p.plane_rows = plane_rows;
+  p.seq_start = (const long long *)seq_start; p.seq_len = (const long long *)seq_len; p.B = B; p.Hq = Hq; p.G = G; p.n_rep = n_rep;
+  p.n_split = n_split; p.scale = scale; p.rope_theta = rope_theta; p.part = part; p.out = out;
+  const bool rope = rope_theta > 0.0f;
+  const size_t smem = attn::attn_smem_bytes(k_stages, v_stages, n_rep, rope);
+  if (smem > 227 * 1024) { set_error("attention: %d key stages x %d query heads per KV head do not fit in shared memory", k_stages, n_rep); return GSRQ_EUNSUPPORTED; }
+  const dim3 grid((unsigned)n_split, (unsigned)G, (unsigned)B);
+  // Plain launches: no event pair around them even when gsrq_profile_enable is on (creating events is an allocation of its own).
+  // Nothing in the buffer has to start at zero: every split's CTA stores all of its n_rep x 130 floats before the merge kernel,
+  // which follows on the same stream, reads exactly the B x G x n_split x n_rep entries of THIS call.
+#define GSRQ_ATTN_K(KERNEL)                                                                                            \
+  do {                                                                                                                \
+    GSRQ_CUDA_CHECK(cudaFuncSetAttribute(KERNEL, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));            \
+    KERNEL<<<grid, attn::kThreads, smem, stream>>>(p);                                                                \
+  } while (0)
+#define GSRQ_ATTN(NREP, NS)                                                                                           \
+  do {                                                                                                                \
+    if (rope) GSRQ_ATTN_K((attn::k_attn_decode_rope<NREP, NS>)); else GSRQ_ATTN_K((attn::k_attn_decode<false, NREP, NS>)); \
+  } while (0)
+  const int ns = (k_stages == v_stages) ? k_stages : 0;
+  if (n_rep == 4 && ns == 1) GSRQ_ATTN(4, 1);
+  else if (n_rep == 4 && ns == 2) GSRQ_ATTN(4, 2);
+  else if (n_rep == 4 && ns == 4) GSRQ_ATTN(4, 4);
+  else if (n_rep == 1 && ns == 2) GSRQ_ATTN(1, 2);
+  else if (n_rep == 8 && ns == 2) GSRQ_ATTN(8, 2);
+  else GSRQ_ATTN(0, 0);
+#undef GSRQ_ATTN_K
+#undef GSRQ_ATTN
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  attn::k_attn_combine<<<dim3((unsigned)Hq, (unsigned)B), 128, 0, stream>>>(p);
+  GSRQ_CUDA_CHECK(cudaGetLastError());
+  {
+    std::lock_guard<std::mutex> lk(g_prof_mu);
+    g_launches[kClsDecode] += 2;
+  }
+  return GSRQ_OK;
+}
+
 int gsrq_log_weights(const void *grad, const gsrq_view *view, float tau, float eps, float *w_out, gsrq_stream_t stream_) {
   cudaStream_t stream = (cudaStream_t)stream_;
   if (!grad || !view || !w_out) { set_error("NULL input"); return GSRQ_EINVAL; }
