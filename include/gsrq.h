@@ -214,8 +214,9 @@ int gsrq_decode_pervector_gain(const uint8_t *codes, const uint16_t *gains16, co
                                const gsrq_view *out_view, gsrq_stream_t stream);
 
 /* Nibble packing for K <= 16 (BASELINE.json config 0 "Codes are 4-bit indices"; "bit-packing"): each of the n_planes
- * rows of N codes becomes ceil(N / 2) bytes, code 2i in the low nibble, code 2i + 1 in the high nibble.  Storage-side only. */
-int gsrq_pack_nibbles(const uint8_t *codes, int64_t n_planes, int64_t N, uint8_t *packed, gsrq_stream_t stream);
+ * rows of N codes becomes ceil(N / 2) bytes, code 2i in the low nibble, code 2i + 1 in the high nibble.  Storage-side only.
+ * K is the codebook size the codes were produced with: K > 16 (a code would lose its high bits) returns GSRQ_EINVAL. */
+int gsrq_pack_nibbles(const uint8_t *codes, int K, int64_t n_planes, int64_t N, uint8_t *packed, gsrq_stream_t stream);
 int gsrq_unpack_nibbles(const uint8_t *packed, int64_t n_planes, int64_t N, uint8_t *codes, gsrq_stream_t stream);
 
 /* Per-subspace codebooks ("an independent codebook per subspace"): no separate entry point -- subspace m of a
@@ -239,7 +240,10 @@ size_t gsrq_attention_workspace_bytes(int B, int Hq, int G, int64_t max_len);
  * k_codes / v_codes: the cache's code planes as gsrq_encode / gsrq_encode_append write them, [S][G][plane_rows], row = token * M + m
  *            (8-byte aligned); k_cb / v_cb their codebooks; k_stages / v_stages: prefix of stages used.
  * seq_start, seq_len: device [B] int64: first token and number of tokens of each sequence inside the planes; max_len >= every seq_len
- *            (host value, sizes the split of the token range over CTAs).
+ *            (host value, sizes the split of the token range over CTAs).  A sequence with a negative start or length, or one that
+ *            reaches beyond plane_rows / 8 tokens, is not read: it is served as an empty sequence (zeros).
+ * B, G <= 65535; the codebooks' shapes arrays must be 16-byte aligned (GSRQ_EINVAL otherwise).  Code bytes >= K select a zero
+ *            codeword here; the stand-alone decodes clamp them to K - 1 (cold paths) -- either way nothing outside the codebook is read.
  * This build serves hd = 128, d = 16, K <= 256, 1..4 stages, Hq / G <= 8.  fp32 arithmetic, no atomics: bit-reproducible.
  */
 int gsrq_attention_decode(const float *q, const uint8_t *k_codes, const gsrq_codebook *k_cb, int k_stages, const uint8_t *v_codes,

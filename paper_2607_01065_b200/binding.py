@@ -206,8 +206,8 @@ def gsrq_decode_pervector_gain(codes, gains16, cb, n_stages, kv_out, out_view):
     _check(lib().gsrq_decode_pervector_gain(_ptr(codes), _ptr(gains16), C.byref(cb), n_stages, _ptr(kv_out), C.byref(out_view), _stream()))
 
 
-def gsrq_pack_nibbles(codes, n_planes, N, packed):
-    _check(lib().gsrq_pack_nibbles(_ptr(codes), C.c_int64(n_planes), C.c_int64(N), _ptr(packed), _stream()))
+def gsrq_pack_nibbles(codes, K, n_planes, N, packed):
+    _check(lib().gsrq_pack_nibbles(_ptr(codes), K, C.c_int64(n_planes), C.c_int64(N), _ptr(packed), _stream()))
 
 
 def gsrq_unpack_nibbles(packed, n_planes, N, codes):

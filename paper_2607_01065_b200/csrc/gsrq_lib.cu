@@ -1273,6 +1273,7 @@ int gsrq_cluster_assign(const float *x, int64_t N, int d, int K, int method, con
   if (!x || !shapes || !gains || !idx_out) { set_error("NULL input"); return GSRQ_EINVAL; }
   int rc = check_cluster(N, d, K);
   if (rc) return rc;
+  if ((rc = check_align16(x, "x")) || (rc = check_align16(shapes, "shapes"))) return rc;
   return cluster_assign(x, N, d, K, method == 1 ? wide::kModeKm : wide::kModeGskm, shapes, gains, idx_out, nullptr, 0, (cudaStream_t)stream_);
 }
 
@@ -1287,7 +1288,7 @@ int gsrq_cluster_metrics(const float *x, int64_t N, int d, int K, int method, co
   if (rc) return rc;
   double *part = (double *)((char *)workspace + pl.off_met);
   double *res = part + (size_t)pl.nE * 5;
-  LAUNCH(kClsMisc, stream, (wide::k_cluster_metrics<<<(unsigned)pl.nE, 256, 0, stream>>>(x, N, d, shapes, gains, idx, method == 1, part)));
+  LAUNCH(kClsMisc, stream, (wide::k_cluster_metrics<<<(unsigned)pl.nE, 256, 0, stream>>>(x, N, d, shapes, gains, idx, method == 1, K, part)));
   GSRQ_CUDA_CHECK(cudaGetLastError());
   LAUNCH(kClsMisc, stream, (wide::k_cluster_metrics_finish<<<1, 160, 0, stream>>>(part, pl.nE, N, res)));
   GSRQ_CUDA_CHECK(cudaGetLastError());
@@ -1320,6 +1321,8 @@ int gsrq_attention_decode(const float *q, const uint8_t *k_codes, const gsrq_cod
   }
   if (hd != attn::kHd || d != attn::kD) { set_error("attention: this build serves head_dim 128 with d = 16 (got %d, %d)", hd, d); return GSRQ_EUNSUPPORTED; }
   if (B <= 0 || G <= 0 || Hq <= 0 || Hq % G || Hq / G > 8) { set_error("attention: need Hq a multiple of G with at most 8 query heads per KV head"); return GSRQ_EINVAL; }
+  if (B > 65535 || G > 65535) { set_error("attention: at most 65535 sequences and KV heads per call (grid limits), got B = %d, G = %d", B, G); return GSRQ_EINVAL; }
+  if (((uintptr_t)k_cb->shapes & 15) || ((uintptr_t)v_cb->shapes & 15)) { set_error("codebook shapes must be 16-byte aligned"); return GSRQ_EINVAL; }
   if (k_cb->K < 1 || k_cb->K > 256 || v_cb->K < 1 || v_cb->K > 256 || k_stages < 1 || k_stages > 4 || k_stages > k_cb->S || v_stages < 1 || v_stages > 4 ||
       v_stages > v_cb->S) { set_error("attention: K in [1, 256] and 1..4 stages (<= S) for keys and values"); return GSRQ_EINVAL; }
   if (plane_rows <= 0 || plane_rows % attn::kM || max_len < 0 || rope_theta < 0.0f) { set_error("attention: bad plane_rows / max_len / rope_theta"); return GSRQ_EINVAL; }
@@ -1523,9 +1526,10 @@ int gsrq_decode_pervector_gain(const uint8_t *codes, const uint16_t *gains16, co
   return GSRQ_OK;
 }
 
-int gsrq_pack_nibbles(const uint8_t *codes, int64_t n_planes, int64_t N, uint8_t *packed, gsrq_stream_t stream_) {
+int gsrq_pack_nibbles(const uint8_t *codes, int K, int64_t n_planes, int64_t N, uint8_t *packed, gsrq_stream_t stream_) {
   cudaStream_t stream = (cudaStream_t)stream_;
   if (!codes || !packed || n_planes <= 0 || N <= 0) { set_error("bad arguments"); return GSRQ_EINVAL; }
+  if (K < 1 || K > 16) { set_error("nibble packing holds codes of K <= 16 codewords, got K = %d", K); return GSRQ_EINVAL; }
   LAUNCH(kClsMisc, stream, (var::k_pack_nibbles<<<1184, 256, 0, stream>>>(codes, n_planes, N, packed)));
   GSRQ_CUDA_CHECK(cudaGetLastError());
   return GSRQ_OK;

@@ -76,7 +76,9 @@ __device__ __forceinline__ void attn_decode_body(const AttnParams &p) {
   float *m_run = reinterpret_cast<float *>(reinterpret_cast<uint8_t *>(kcodes) + (ROPE ? CH * kM * SK : 0));
   float *l_run = m_run + 8, *sc_h = l_run + 8;
 
-  const long long t_seq0 = p.seq_start[b], len = p.seq_len[b];
+  const long long t_seq0 = p.seq_start[b];
+  long long len = p.seq_len[b];
+  if (t_seq0 < 0 || len < 0 || t_seq0 + len > p.plane_rows / kM) len = 0;   // a sequence that leaves the code planes is served as empty (zeros), never read
   long long per = (len + p.n_split - 1) / p.n_split;
   per = (per + CH - 1) / CH * CH;
   const long long tb = (long long)sp * per, te = min(len, tb + per);

@@ -58,7 +58,7 @@ __global__ void __launch_bounds__(256) k_decode(DecParams p) {
         const long long i = ib + (long long)u * RPI;
 #pragma unroll
         for (int s = 0; s < 8; ++s)
-          code[u][s] = (s < ns && i < r1) ? p.codes[((long long)(s0 + s) * p.G + g) * p.N + i] : 0;
+          code[u][s] = (s < ns && i < r1) ? min((int)p.codes[((long long)(s0 + s) * p.G + g) * p.N + i], p.K - 1) : 0;   // a byte >= K (K < 256) stays inside the table
       }
 #pragma unroll
       for (int s = 0; s < 8; ++s) {

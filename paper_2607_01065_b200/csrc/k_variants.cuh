@@ -133,7 +133,7 @@ __global__ void __launch_bounds__(256) k_pvg_decode(PvgDecParams p) {
   for (int st = 0; st < p.n_stages; ++st) {
     const long long ci = ((long long)st * p.G + g) * p.N + i;
     const float gf = __half2float(p.gains[ci]);
-    const float *s = p.shapes + (((long long)g * p.S + st) * p.K + p.codes[ci]) * D;
+    const float *s = p.shapes + (((long long)g * p.S + st) * p.K + min((int)p.codes[ci], p.K - 1)) * D;
 #pragma unroll
     for (int j = 0; j < D; ++j) {
       const float c = __fmul_rn(gf, s[j]);

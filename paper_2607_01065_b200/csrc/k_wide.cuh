@@ -805,7 +805,7 @@ __global__ void __launch_bounds__(256) k_wide_subtract(WSubParams p) {
   const long long i = (long long)blockIdx.x * 8 + warp;
   if (i >= p.N) return;
   const long long gi = (long long)g * p.N + i;
-  const int k = p.idx[gi];
+  const int k = min((int)p.idx[gi], p.K - 1);   // a caller-supplied code >= K must not index past the codebook
   if (p.codes && lane == 0) p.codes[gi] = (uint8_t)k;
   const float gk = p.gains[(long long)g * p.cb_stride_g + k];
   const float *s = p.shapes + ((long long)g * p.cb_stride_g + k) * p.d;
@@ -861,7 +861,7 @@ __global__ void __launch_bounds__(256) k_wide_decode(WDecParams p) {
   for (int e0 = lane * 4; e0 < p.d; e0 += 128) {
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
     for (int s = 0; s < p.n_stages; ++s) {
-      const int k = p.codes[((long long)s * p.G + g) * p.N + i];
+      const int k = min((int)p.codes[((long long)s * p.G + g) * p.N + i], p.K - 1);
       const long long cb = ((long long)g * p.S + s) * p.K + k;
       const float gk = __ldg(p.gains + cb);
       const float4 sv = __ldg(reinterpret_cast<const float4 *>(p.shapes + cb * p.d + e0));
@@ -906,13 +906,13 @@ __global__ void __launch_bounds__(256) k_wide_gather(RowSrc src, long long N, fl
 // out: [gridDim.x][5] partial sums.  grid = ceil(N / 8), block = 256.
 __global__ void __launch_bounds__(256) k_cluster_metrics(const float *__restrict__ x, long long N, int d, const float *__restrict__ shapes,
                                                          const float *__restrict__ gains, const uint16_t *__restrict__ idx, int km,
-                                                         double *__restrict__ out) {
+                                                         int K, double *__restrict__ out) {
   __shared__ double sh[8][5];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const long long i = (long long)blockIdx.x * 8 + warp;
   double v[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
   if (i < N) {
-    const int k = idx[i];
+    const int k = min((int)idx[i], K - 1);   // caller-supplied labels: clamped, never read past the codebook
     const float gk = km ? 1.0f : gains[k];
     double e2 = 0.0, nx2 = 0.0, np2 = 0.0, dot = 0.0;
     for (int j = lane; j < d; j += 32) {

@@ -66,6 +66,19 @@ def test_workspace_bytes_and_argument_errors(B):
     assert rc == -1
     rc = lib.gsrq_decode(None, C.byref(cb), 2, None, C.byref(v), None)
     assert rc == -1
+    # argument checks that come before any CUDA call (fake, never dereferenced addresses)
+    p = lambda a: C.c_void_p(a)
+    assert lib.gsrq_pack_nibbles(p(0x1000), 17, C.c_int64(1), C.c_int64(8), p(0x2000), None) == -1 and b"K = 17" in lib.gsrq_last_error()
+    cb_ok = B.gsrq_codebook(256, 2, 0x10000, 0x20000)
+    cb_odd = B.gsrq_codebook(256, 2, 0x10004, 0x20000)   # shapes are read as float4
+    attn = lambda fn, kcb, Bq, tail: fn(p(0x1000), p(0x2000), C.byref(kcb), 2, p(0x3000), C.byref(cb_ok), 2, C.c_int64(8 * 64), p(0x4000), p(0x5000),
+                                         C.c_int64(64), Bq, 32, 8, 128, 16, C.c_float(0.1), C.c_float(0.0), p(0x6000), *tail)
+    ws = (p(0x7000), C.c_size_t(1 << 30), None)
+    assert attn(lib.gsrq_attention_decode, cb_odd, 2, ws) == -1 and b"16-byte" in lib.gsrq_last_error()
+    assert attn(lib.gsrq_attention_decode, cb_ok, 70000, ws) == -1 and b"65535" in lib.gsrq_last_error()
+    assert attn(lib.gsrq_attention_decode_static, cb_odd, 2, (None,)) == -1
+    assert attn(lib.gsrq_attention_decode_static, cb_ok, 70000, (None,)) == -1
+    assert lib.gsrq_cluster_assign(p(0x1004), C.c_int64(100), 16, 8, 0, p(0x2000), p(0x3000), p(0x4000), None) == -1
 
 
 def test_product_path_does_not_reach_the_oracle():

@@ -84,3 +84,21 @@ def test_attention_on_an_encoded_cache_equals_attention_on_the_decoded_tensor(B)
     B.gsrq_decode(gv["codes_dev"], gv["cb"], S, vd, B.view_of(vd, d))
     want = torch.nn.functional.scaled_dot_product_attention(q.double().view(1, G, 4, hd), kd.double()[None], vd.double()[None]).view(1, 8, hd)
     assert (out.double() - want).abs().max() <= 2e-4 * want.abs().max()
+
+
+def test_attention_sequence_outside_the_code_planes_is_served_as_empty(B):
+    """A (seq_start, seq_len) pair that reaches beyond plane_rows / 8 tokens is never read: its output rows are zeros, the other
+    sequences of the call are unaffected (include/gsrq.h)."""
+    G, Tc, K, S, Hq = 2, 300, 256, 2, 8
+    c = _case(91, G, Tc, K, S, S, 3, Hq)
+    start = np.array([0, 200, -1], dtype=np.int64); length = np.array([300, 200, 10], dtype=np.int64)
+    want = ao.attention_decode(c["q"][:1], c["kc"], c["ks"], c["kg"], c["vc"], c["vs"], c["vg"], c["hd"], start[:1], length[:1], rope_theta=0.0)
+    dev = lambda a: torch.from_numpy(a).cuda()
+    ks, kg, vs, vg = dev(c["ks"]), dev(c["kg"]), dev(c["vs"]), dev(c["vg"])
+    for fn in (B.gsrq_attention_decode, B.gsrq_attention_decode_static):
+        out = torch.full((3, Hq, c["hd"]), 7.0, device="cuda")
+        fn(dev(c["q"]), dev(c["kc"]), B.codebook_of(ks, kg), S, dev(c["vc"]), B.codebook_of(vs, vg), S, Tc * c["M"], dev(start), dev(length),
+           300, G, c["d"], 1.0 / np.sqrt(c["hd"]), 0.0, out)
+        got = out.cpu().numpy().astype(np.float64)
+        assert np.abs(got[0] - want[0]).max() <= 2e-4 * np.abs(want).max()
+        assert not got[1:].any()

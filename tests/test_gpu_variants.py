@@ -81,7 +81,10 @@ def test_nibble_packing(B):
     c = rng.integers(0, 16, (6, 4097)).astype(np.uint8)
     cd = torch.from_numpy(c).cuda()
     packed = torch.zeros(6, 2049, dtype=torch.uint8, device="cuda")
-    B.gsrq_pack_nibbles(cd, 6, 4097, packed)
+    B.gsrq_pack_nibbles(cd, 16, 6, 4097, packed)
+    with pytest.raises(B.GsrqError) as e:   # K > 16: a code would lose its high bits
+        B.gsrq_pack_nibbles(cd, 17, 6, 4097, packed)
+    assert e.value.code == -1
     assert np.array_equal(packed.cpu().numpy(), vo.pack_nibbles(c))
     back = torch.zeros_like(cd)
     B.gsrq_unpack_nibbles(packed, 6, 4097, back)
@@ -92,7 +95,7 @@ def test_nibble_packing(B):
     got = gpu_gsrq(dd["x"], dd["w"], cfg.d, cfg.K, cfg.S, cfg.iters, seed=0, dtype="f32")
     n = got["codes"].shape[-1]
     pk = torch.zeros(cfg.S * cfg.G, (n + 1) // 2, dtype=torch.uint8, device="cuda")
-    B.gsrq_pack_nibbles(got["codes_dev"], cfg.S * cfg.G, n, pk)
+    B.gsrq_pack_nibbles(got["codes_dev"], cfg.K, cfg.S * cfg.G, n, pk)
     un = torch.zeros_like(got["codes_dev"])
     B.gsrq_unpack_nibbles(pk, cfg.S * cfg.G, n, un)
     assert torch.equal(un, got["codes_dev"]) and pk.numel() * 2 == got["codes_dev"].numel()
@@ -132,3 +135,27 @@ def test_per_subspace_codebooks(B):
     flat = np.ascontiguousarray(x_np.reshape(G, T, M, d).transpose(0, 2, 1, 3).reshape(G * M, T, d))
     ref = o.gsrq_fit_encode(flat, w_np, d, K, 1, iters, seed=0, encode=False)
     assert np.abs(shapes.cpu().numpy() - ref["shapes"]).max() <= 1e-6 and np.abs(gains.cpu().numpy() - ref["gains"]).max() <= 1e-5
+
+
+def test_code_bytes_beyond_K_are_clamped_not_followed(B):
+    """Caller-supplied code bytes >= K (possible when K < 256) must not index past the codebook: the cold decode paths clamp them
+    to K - 1 (d = 8 generic kernel, d = 64 wide kernel, per-vector-gain decode)."""
+    rng = np.random.default_rng(17)
+    for d, hd in ((8, 32), (64, 128)):
+        G, T, K, S = 2, 37, 5, 2
+        M = hd // d
+        sh = rng.standard_normal((G, S, K, d)).astype(np.float32); sh /= np.linalg.norm(sh, axis=-1, keepdims=True)
+        gn = np.abs(rng.standard_normal((G, S, K))).astype(np.float32)
+        codes = rng.integers(0, K, (S, G, T * M)).astype(np.uint8)
+        wild = codes.copy(); wild[codes == K - 1] = 255
+        shd, gnd = torch.from_numpy(sh).cuda(), torch.from_numpy(gn).cuda()
+        cb = B.codebook_of(shd, gnd)
+        a = torch.zeros(G, T, hd, device="cuda"); b = torch.full_like(a, 3.0)
+        B.gsrq_decode(torch.from_numpy(codes).cuda(), cb, S, a, B.view_of(a, d))
+        B.gsrq_decode(torch.from_numpy(wild).cuda(), cb, S, b, B.view_of(b, d))
+        assert torch.equal(a, b)
+        if d == 8:
+            g16 = torch.from_numpy(np.abs(rng.standard_normal((S, G, T * M))).astype(np.float16)).cuda()
+            B.gsrq_decode_pervector_gain(torch.from_numpy(codes).cuda(), g16, cb, S, a, B.view_of(a, d))
+            B.gsrq_decode_pervector_gain(torch.from_numpy(wild).cuda(), g16, cb, S, b, B.view_of(b, d))
+            assert torch.equal(a, b)
