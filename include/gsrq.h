@@ -116,7 +116,8 @@ size_t gsrq_workspace_bytes(const gsrq_view *view, int K, int S, int64_t n_fit_t
  * seed     : selects the initial rows (splitmix64 stream, reading c-I).
  * stats    : HOST array of G structs or NULL.  When given, the call synchronises `stream`
  *            and returns GSRQ_EDEGENERATE if any group could not be initialised; the per-iteration
- *            distortions are only computed in that case.
+ *            distortions are only computed in that case.  With stats == NULL the call is asynchronous and
+ *            detection of those errors is deferred to gsrq_fit_status (below).
  * Kernels  : d == 16: ONE persistent cooperative kernel runs all passes (tcgen05 filter with an fp64 re-score of
  *            the ambiguous rows, per-CTA fp64 reduction, merge + Eq. 7-8, two group barriers per pass) and
  *            leaves the loop when a group's assignments stop changing (Alg. 1 l.15-16).  Other d: two
@@ -127,6 +128,18 @@ int gsrq_fit_stage(const void *kv, const gsrq_view *view, const float *w, int64_
                    const int64_t *fit_tokens, int64_t n_fit, gsrq_codebook *cb, int stage,
                    const float *residual, int iters, uint64_t seed, gsrq_fit_stats *stats,
                    void *workspace, size_t workspace_bytes, gsrq_stream_t stream);
+
+/*
+ * Outcome of the last gsrq_fit_stage call that used `workspace` (same view, K, S and fit-subset size as that call; n_fit_tokens:
+ * 0 = it fitted on all T tokens).  gsrq_fit_stage(stats = NULL) returns before the GPU has run, so it cannot report what only the
+ * kernels find out; this call synchronises `stream` (the fit's stream), reads the per-group error words from the workspace and
+ * returns GSRQ_OK, GSRQ_EDEGENERATE (a group had fewer than K distinct non-zero fit rows: its codebook is unspecified) or
+ * GSRQ_ECUDA (a CTA of the persistent fit kernel never reached a group barrier within the spin bound; the kernel then stops
+ * updating that group's codebook and every CTA of the group leaves the loop).  Each fit clears the words at its start and other
+ * gsrq calls may overwrite them, so callers that pass stats == NULL and care call this after each fit, before the next call
+ * that is given the same workspace.
+ */
+int gsrq_fit_status(const void *workspace, const gsrq_view *view, int K, int S, int64_t n_fit_tokens, gsrq_stream_t stream);
 
 /*
  * Encode stages [stage_begin, stage_end) with fixed codebooks (RQ):

@@ -42,7 +42,7 @@ class gsrq_fit_stats(C.Structure):
 
 _lib = None
 EXPORTS = ["gsrq_log_weights", "gsrq_encode_pervector_gain", "gsrq_decode_pervector_gain", "gsrq_pack_nibbles", "gsrq_unpack_nibbles",
-           "gsrq_attention_workspace_bytes", "gsrq_attention_decode", "gsrq_attention_static_scratch_bytes", "gsrq_attention_decode_static", "gsrq_cluster_workspace_bytes", "gsrq_cluster_fit", "gsrq_cluster_assign", "gsrq_cluster_metrics", "gsrq_workspace_bytes", "gsrq_fit_stage", "gsrq_encode", "gsrq_decode", "gsrq_encode_append", "gsrq_assign", "gsrq_update",
+           "gsrq_attention_workspace_bytes", "gsrq_attention_decode", "gsrq_attention_static_scratch_bytes", "gsrq_attention_decode_static", "gsrq_cluster_workspace_bytes", "gsrq_cluster_fit", "gsrq_cluster_assign", "gsrq_cluster_metrics", "gsrq_workspace_bytes", "gsrq_fit_stage", "gsrq_fit_status", "gsrq_encode", "gsrq_decode", "gsrq_encode_append", "gsrq_assign", "gsrq_update",
            "gsrq_init_ids", "gsrq_debug_scores", "gsrq_encode_host", "gsrq_decode_host", "gsrq_pipeline_host", "gsrq_pipeline_host_batch", "gsrq_release_host_pool", "gsrq_profile_enable",
            "gsrq_profile_read", "gsrq_launch_count", "gsrq_last_error", "gsrq_version"]
 
@@ -125,6 +125,11 @@ def gsrq_fit_stage(kv, view, w, w_stride_g, fit_tokens, cb, stage, residual, ite
                               stats, _ptr(ws), C.c_size_t(ws.numel()), _stream())
     _check(rc)
     return stats
+
+
+def gsrq_fit_status(ws, view, K, S, n_fit_tokens=0):
+    """Raise GsrqError if the last gsrq_fit_stage on this workspace hit a degenerate group or a barrier timeout (synchronises)."""
+    _check(lib().gsrq_fit_status(_ptr(ws), C.byref(view), K, S, C.c_int64(n_fit_tokens), _stream()))
 
 
 def gsrq_encode(kv, view, cb, stage_begin, stage_end, codes, residual_out, ws):

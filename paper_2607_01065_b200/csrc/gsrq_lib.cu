@@ -939,6 +939,27 @@ int gsrq_fit_stage(const void *kv, const gsrq_view *view, const float *w, int64_
   return GSRQ_OK;
 }
 
+int gsrq_fit_status(const void *workspace, const gsrq_view *view, int K, int S, int64_t n_fit_tokens, gsrq_stream_t stream_) {
+  cudaStream_t stream = (cudaStream_t)stream_;
+  if (!workspace) { set_error("workspace is NULL"); return GSRQ_EINVAL; }
+  int rc = check_view(view, K, S);
+  if (rc) return rc;
+  if (n_fit_tokens < 0 || n_fit_tokens > view->T) { set_error("n_fit_tokens out of [0, T]"); return GSRQ_EINVAL; }
+  const size_t off = is_wide(view->d) ? make_wplan(view, n_fit_tokens).off_st : make_plan(view, K, S, n_fit_tokens).off_st;
+  const DevStats *st = (const DevStats *)((const char *)workspace + off);
+  std::vector<int> err((size_t)view->G, 0);
+  // the G error words, one per DevStats record
+  GSRQ_CUDA_CHECK(cudaMemcpy2DAsync(err.data(), sizeof(int), &st[0].err, sizeof(DevStats), sizeof(int), (size_t)view->G, cudaMemcpyDeviceToHost, stream));
+  GSRQ_CUDA_CHECK(cudaStreamSynchronize(stream));
+  bool degenerate = false;
+  for (int g = 0; g < view->G; ++g) {
+    if (err[g] == GSRQ_EDEGENERATE) degenerate = true;
+    else if (err[g] != 0) { set_error("the fit kernel's group barrier timed out (group %d): the codebook of this stage is not valid", g); return GSRQ_ECUDA; }
+  }
+  if (degenerate) { set_error("a group has fewer than K distinct non-zero fit rows"); return GSRQ_EDEGENERATE; }
+  return GSRQ_OK;
+}
+
 
 int gsrq_encode(const void *kv, const gsrq_view *view, const gsrq_codebook *cb, int stage_begin, int stage_end,
                 uint8_t *codes, float *residual_out, void *workspace, size_t workspace_bytes, gsrq_stream_t stream_) {

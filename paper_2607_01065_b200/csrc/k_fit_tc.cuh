@@ -75,9 +75,18 @@ struct FitTcParams {
   long long *clk;          // debug: [G][nx][16] cycles per phase (GSRQ_FIT_CLOCKS), or nullptr
 };
 
+// The group's "a barrier wait timed out" flag, read from global memory (never from a stale cache line).
+__device__ __forceinline__ bool fit_lost(const DevStats *st) {
+  int e = 0;
+  if (st) asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(e) : "l"(&st->err) : "memory");
+  return e == GSRQ_ECUDA;
+}
+
 // Barrier among the CTAs of one group: arrive on an integer counter in global memory, spin until `target` arrivals.
 // The CTAs are co-resident (cooperative launch, one per SM).  A bounded spin: a lost CTA ends the wait (and flags the
-// fit as failed) instead of hanging the device.
+// fit as failed) instead of hanging the device.  Once the flag is up, the group's other CTAs stop waiting as well (they poll it
+// every 4096 spins) and every CTA leaves the pass loop at its next check without touching the codebook again: the caller sees
+// GSRQ_ECUDA through `stats` or gsrq_fit_status, never a silently half-updated codebook reported as GSRQ_OK.
 __device__ __forceinline__ void group_barrier(unsigned int *ctr, unsigned int target, DevStats *st) {
   __syncthreads();   // every thread's writes happen-before thread 0's release below (cumulativity)
   if (threadIdx.x == 0) {
@@ -87,7 +96,8 @@ __device__ __forceinline__ void group_barrier(unsigned int *ctr, unsigned int ta
     for (;;) {
       asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(ctr) : "memory");
       if (v >= target) break;
-      if (++spins > (1LL << 26)) { if (st) st->err = GSRQ_ECUDA; break; }
+      if (++spins > (1LL << 26)) { if (st) st->err = GSRQ_ECUDA; __threadfence(); break; }
+      if ((spins & 4095) == 0 && fit_lost(st)) break;
     }
   }
   __syncthreads();
@@ -451,7 +461,12 @@ k_fit_tc(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CUte
     // ---------------- (d) every CTA of the group has published its partials ----------------
     ++epoch;
     group_barrier(p.bar + g, epoch * (unsigned int)nx, stg);
-    if (tid == 0) misc[0] = (stg && !p.skip_scoring) ? __ldcg(&stg->changed[t]) : 1;
+    if (tid == 0) {
+      misc[0] = (stg && !p.skip_scoring) ? __ldcg(&stg->changed[t]) : 1;
+      misc[1] = fit_lost(stg) ? 1 : 0;
+    }
+    __syncthreads();
+    if (misc[1]) break;   // a CTA of the group was lost: the partials are incomplete, leave the codebook as it is
     clk_mark(3);
 
     // ---------------- (e) merge + Eq. 7 / Eq. 8 for my clusters k = bx, bx + nx, ... ----------------
@@ -538,6 +553,9 @@ k_fit_tc(const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CUte
     // ---------------- (f) the new codebook is complete; Alg. 1 l.15-16 ----------------
     ++epoch;
     group_barrier(p.bar + g, epoch * (unsigned int)nx, stg);
+    if (tid == 0) misc[1] = fit_lost(stg) ? 1 : 0;
+    __syncthreads();
+    if (misc[1]) break;
     clk_mark(5);
     if (lloyd && t > 1 && !p.skip_scoring && misc[0] == 0) {  // assignments unchanged: this was the last iteration
       if (bx == 0 && tid == 0 && stg) stg->done_iter = t;

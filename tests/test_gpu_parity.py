@@ -227,3 +227,25 @@ def test_degenerate_and_edge_inputs(B):
     ref = o.gsrq_fit_encode(xn, None, 8, 1, 1, 3)
     assert np.array_equal(got["codes"], ref["codes"]) and np.abs(got["shapes"] - ref["shapes"]).max() < 1e-6
     assert stats_np(got["stats"][0], 0)["iters_run"] == ref["stats"][0][0]["iters_run"] == 2
+
+
+@pytest.mark.parametrize("d,hd", [(8, 16), (16, 128), (128, 128)])
+def test_fit_status_reports_what_an_asynchronous_fit_cannot(B, d, hd):
+    """gsrq_fit_stage(stats = NULL) returns GSRQ_OK before the kernels have run; gsrq_fit_status reads the per-group error words
+    afterwards (include/gsrq.h): a group of all-zero rows is degenerate (GSRQ_EDEGENERATE), a healthy fit reports GSRQ_OK."""
+    G, T, K = 2, 512, 16
+    x = torch.randn(G, T, hd, device="cuda", generator=torch.Generator(device="cuda").manual_seed(3))
+    if d == 16:
+        x = x.bfloat16()   # the persistent tensor-core fit kernel
+    shapes = torch.zeros(G, 1, K, d, device="cuda"); gains = torch.zeros(G, 1, K, device="cuda")
+    cb = B.codebook_of(shapes, gains)
+    view = B.view_of(x, d)
+    ws = B.workspace(view, K, 1)
+    B.gsrq_fit_stage(x, view, None, 0, None, cb, 0, None, 3, 0, ws, want_stats=False)
+    B.gsrq_fit_status(ws, view, K, 1)          # healthy: no error
+    assert torch.isfinite(shapes).all() and (shapes.norm(dim=-1) - 1).abs().max() < 1e-5
+    x[1].zero_()                               # group 1 has no non-zero row
+    B.gsrq_fit_stage(x, view, None, 0, None, cb, 0, None, 3, 0, ws, want_stats=False)   # asynchronous: cannot know yet
+    with pytest.raises(B.GsrqError) as e:
+        B.gsrq_fit_status(ws, view, K, 1)
+    assert e.value.code == -5
