@@ -74,10 +74,15 @@ def test_wide_fused_encode_many_stages_and_prefix_decode(B):
         assert np.array_equal(dec, want), n
 
 
+def _rho(d, n_planes):
+    """The filter's rho (k_score_tc_wide.cuh): accumulation budgeted at 2^-23 per step."""
+    return ((9.0 if n_planes == 2 else 8.0) if d == 128 else (6.5 if n_planes == 2 else 5.5)) * 2.0 ** -17
+
+
 @pytest.mark.parametrize("d,use_residual", [(128, False), (128, True), (64, True)])
 def test_wide_tc_scores_within_bound(B, d, use_residual):
     """Raw tcgen05 scores at d = 64 / 128 against fp64, relative to the bound the kernel uses:
-    E(g) = rho 2^-17 (2 g ||r||) + 2^-18 g^2, rho = 4 / 5 (d = 64), 5 / 6 (d = 128) for one / two operand planes."""
+    E(g) = rho 2^-17 (2 g ||r||) + 2^-18 g^2, rho = 5.5 / 6.5 (d = 64), 8 / 9 (d = 128) for one / two operand planes."""
     G, T, hd, K = 2, 300, 128, 256
     x_np, _ = _data("k", G, T, hd, 4400 + d)
     rows = o.rows_of(x_np, d)
@@ -112,7 +117,7 @@ def test_wide_tc_scores_within_bound(B, d, use_residual):
             err = np.abs(sc[g_][:, :K] - exact)
             nrm = np.linalg.norm(r64, axis=1)
             gk = g64[None] if mode == 0 else np.ones((1, K))
-            rho = ((6.0 if use_residual else 5.0) if d == 128 else (5.0 if use_residual else 4.0)) * 2.0 ** -17
+            rho = _rho(d, 2 if use_residual else 1)
             E = rho * 2 * gk * nrm[:, None] + (2.0 ** -18 * gk * gk if mode == 0 else 0.0)
             ratio = (err / np.maximum(E, 1e-30)).max()
             print(f"wide tc filter error / bound: {ratio:.3f} (d={d} residual={use_residual} mode={mode} g={g_})")
@@ -148,3 +153,49 @@ def test_wide_lockstep_update_and_init(B):
     B.gsrq_update(x, view, None, w, 0, torch.from_numpy(a_np).cuda(), cb, 0, True, ws)
     torch.cuda.synchronize()
     assert np.abs(shapes.cpu().numpy() - s_want).max() <= 1e-7 and np.abs(gains.cpu().numpy() - g_want).max() <= 1e-6
+
+
+@pytest.mark.parametrize("d", [64, 128])
+def test_wide_tc_scores_within_bound_under_cancellation(B, d):
+    """Adversarial input for the filter's error bound: every row is made (nearly) orthogonal to a chosen codeword, and the elements of
+    rows and codewords spread over twelve binades, so that the products of a dot product are large and cancel -- the case where a
+    tensor core that truncates or aligns its partial sums loses most.  The raw scores must still be within half of the bound
+    E(g) (two operand planes: fp32 rows), and the arg-max must equal the exact one."""
+    rng = np.random.default_rng(900 + d)
+    G, T, hd, K = 2, 200, 128, 256
+    M = hd // d
+    N = T * M
+    mag = lambda shape: np.exp2(rng.uniform(-6, 6, shape)) * rng.choice([-1.0, 1.0], shape)
+    s_np = mag((G, 1, K, d))
+    s_np /= np.linalg.norm(s_np, axis=-1, keepdims=True)
+    s_np = s_np.astype(np.float32)
+    g_np = (0.5 + np.abs(rng.standard_normal((G, 1, K)))).astype(np.float32)
+    rows = mag((G, N, d))
+    for g_ in range(G):   # remove the component along one codeword per row: that score is pure cancellation
+        pick = s_np[g_, 0][rng.integers(0, K, N)].astype(np.float64)
+        pick /= np.linalg.norm(pick, axis=1, keepdims=True)
+        rows[g_] -= (rows[g_] * pick).sum(1, keepdims=True) * pick
+    rows = rows.astype(np.float32)
+    x = torch.zeros(G, T, hd, dtype=torch.bfloat16, device="cuda")   # the rows come in through the fp32 residual (hi + lo planes)
+    view = B.view_of(x, d)
+    res = torch.from_numpy(rows).cuda()
+    shapes, gains = torch.from_numpy(s_np).cuda(), torch.from_numpy(g_np).cuda()
+    cb = B.codebook_of(shapes, gains)
+    ws = B.workspace(view, K, 1, 0)
+    for mode in (0, 1):
+        scores = torch.zeros(G, N, 256, device="cuda")
+        idx = torch.zeros(G, N, dtype=torch.uint8, device="cuda")
+        B.gsrq_debug_scores(x, view, res, cb, 0, mode, scores, idx, ws)
+        torch.cuda.synchronize()
+        sc = scores.cpu().numpy().astype(np.float64)
+        for g_ in range(G):
+            r64, s64, g64 = rows[g_].astype(np.float64), s_np[g_, 0].astype(np.float64), g_np[g_, 0].astype(np.float64)
+            dots = r64 @ s64.T
+            exact = 2 * g64[None] * dots - g64[None] ** 2 if mode == 0 else 2 * dots
+            gk = g64[None] if mode == 0 else np.ones((1, K))
+            E = _rho(d, 2) * 2 * gk * np.linalg.norm(r64, axis=1)[:, None] + (2.0 ** -18 * gk * gk if mode == 0 else 0.0)
+            ratio = (np.abs(sc[g_][:, :K] - exact) / E).max()
+            print(f"wide tc filter error / bound under cancellation: {ratio:.3f} (d={d} mode={mode} g={g_})")
+            assert ratio <= 0.5, f"filter error reaches {ratio:.3f} of the bound (d={d}, mode {mode}, group {g_})"
+            a, _, _ = o.assign(rows[g_], s_np[g_, 0], g_np[g_, 0] if mode == 0 else None)
+            assert np.array_equal(idx[g_].cpu().numpy(), a)
