@@ -78,3 +78,43 @@ def test_rope_attention_equals_attention_on_rotated_keys_and_empty_sequence():
     p = np.exp(lg - lg.max()); p /= p.sum()
     np.testing.assert_allclose(out[0, 1], p @ vhat[1, 5:35], rtol=1e-12)
     assert not out[1].any()
+
+
+def test_rope_frequency_schedule_hand_values():
+    """Pins the inverse frequencies of ao.rope for i >= 1 (reading a-R of DESIGN.md: rotate-half convention of the LLaMA family,
+    angle_i = position * theta^(-2 i / hd)).  Hand values for hd = 8, theta = 10000, position 3: pair (i, i + 4) turns by
+    3 * 10000^(-2 i / 8) = 3, 0.3, 0.03, 0.003 radians for i = 0..3.  A schedule of theta^(-i / hd) (angles 3, 0.949, 0.3, 0.0949)
+    or any other exponent fails."""
+    x = np.array([[1.0, 2.0, -3.0, 0.5, 0.25, -1.5, 4.0, 2.5]])
+    r = ao.rope(x, np.array([3]), 10000.0)[0]
+    for i, ang in enumerate([3.0, 0.3, 0.03, 0.003]):
+        a, b = x[0, i], x[0, i + 4]
+        assert r[i] == pytest.approx(a * np.cos(ang) - b * np.sin(ang), rel=1e-12, abs=1e-14), i
+        assert r[i + 4] == pytest.approx(b * np.cos(ang) + a * np.sin(ang), rel=1e-12, abs=1e-14), i
+    # literal numbers (cos / sin of 0.3 and 0.03 typed in, not computed): element 1 and 5, element 2 and 6
+    assert r[1] == pytest.approx(2.0 * 0.955336489125606 + 1.5 * 0.29552020666133955, rel=1e-12)
+    assert r[5] == pytest.approx(-1.5 * 0.955336489125606 + 2.0 * 0.29552020666133955, rel=1e-12)
+    assert r[2] == pytest.approx(-3.0 * 0.9995500337489875 - 4.0 * 0.02999550020249566, rel=1e-12)
+    assert r[6] == pytest.approx(4.0 * 0.9995500337489875 - 3.0 * 0.02999550020249566, rel=1e-12)
+
+
+def test_rope_equals_the_llama_rotary_embedding_of_transformers():
+    """The same pin against a library: transformers' LLaMA rotary embedding (inverse frequencies and apply_rotary_pos_emb's
+    rotate-half pairing) at LLaMA-3's head_dim 128 / theta 500000 (the model family of PAPER.md:216)."""
+    pytest.importorskip("transformers")
+    from transformers import LlamaConfig
+    from transformers.models.llama.modeling_llama import LlamaRotaryEmbedding, apply_rotary_pos_emb
+    hd, nh, theta = 128, 2, 500000.0
+    rot = LlamaRotaryEmbedding(config=LlamaConfig(hidden_size=hd * nh, num_attention_heads=nh, num_key_value_heads=nh, rope_theta=theta,
+                                                  max_position_embeddings=4096))
+    # the oracle's inverse frequencies, read off its output: e_i at position 1 turns by inv_i
+    eye = np.eye(hd)[: hd // 2]
+    r = ao.rope(eye, np.ones(hd // 2), theta)
+    inv = np.arctan2(r[np.arange(hd // 2), np.arange(hd // 2) + hd // 2], r[np.arange(hd // 2), np.arange(hd // 2)])
+    np.testing.assert_allclose(inv, rot.inv_freq.double().numpy(), rtol=2e-6)   # the library stores them in fp32
+    x = torch.randn(1, nh, 4, hd, dtype=torch.float64, generator=torch.Generator().manual_seed(5))
+    pos = torch.tensor([[0, 1, 7, 100]])
+    cos, sin = rot(x, pos)
+    want, _ = apply_rotary_pos_emb(x, x, cos.double(), sin.double())
+    got = ao.rope(x[0].numpy(), np.broadcast_to(pos.numpy(), (nh, 4)), theta)
+    np.testing.assert_allclose(got, want[0].numpy(), atol=2e-5)
