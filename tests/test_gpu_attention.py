@@ -19,9 +19,10 @@ def B():
     return binding
 
 
-def _case(seed, G, Tc, K, SK, SV, Bq, Hq):
+def _case(seed, G, Tc, K, SK, SV, Bq, Hq, d=16):
     rng = np.random.default_rng(seed)
-    hd, d, M = 128, 16, 8
+    hd = 128
+    M = hd // d
     def cb(S, gain):
         s = rng.standard_normal((G, S, K, d)); s /= np.linalg.norm(s, axis=-1, keepdims=True)
         g = (gain * np.abs(rng.standard_normal((G, S, K))) * (0.5 ** np.arange(S))[None, :, None])
@@ -68,7 +69,7 @@ def test_attention_decode_matches_oracle(B, rope_theta, G, Tc, K, SK, SV, Hq, le
 def test_attention_on_an_encoded_cache_equals_attention_on_the_decoded_tensor(B):
     """End to end on the library's own codes: fit + encode a K-like and a V-like cache, then attention from the codes equals
     plain attention on gsrq_decode's fp32 output."""
-    from _harness import gpu_gsrq
+    from paper_2607_01065_b200.pipeline import gpu_gsrq
     from paper_2607_01065_b200 import inputs
     G, T, hd, d, K, S = 2, 1024, 128, 16, 256, 2
     xk = inputs.k_like(G, T, hd, 777); xv = inputs.v_like(G, T, hd, 778)
@@ -102,3 +103,34 @@ def test_attention_sequence_outside_the_code_planes_is_served_as_empty(B):
         got = out.cpu().numpy().astype(np.float64)
         assert np.abs(got[0] - want[0]).max() <= 2e-4 * np.abs(want).max()
         assert not got[1:].any()
+
+
+@pytest.mark.parametrize("rope_theta", [0.0, 500000.0])
+@pytest.mark.parametrize("G,Tc,K,SK,SV,Hq,lens", [
+    (2, 2500, 256, 12, 12, 8, [1500, 0, 999, 1]),    # the paper's point: D = 128, R = 12 (0.75 bits per element), GQA 4:1
+    (1, 700, 100, 16, 32, 8, [700]),                 # R = 16 keys, R = 32 values, K < 256, 8 query heads on one KV head
+    (2, 300, 256, 1, 3, 2, [120, 180]),              # one query head per KV head, few stages
+])
+def test_attention_decode_at_the_papers_operating_point_matches_oracle(B, rope_theta, G, Tc, K, SK, SV, Hq, lens):
+    """d = head_dim = 128 (one sub-vector per token and head), up to 32 stages: the configuration the paper's latency tables are
+    measured at, against the same fp64 oracle and with the same 2e-4 tolerance (reading a-T) as d = 16."""
+    Bq = len(lens)
+    c = _case(300 + Tc, G, Tc, K, SK, SV, Bq, Hq, d=128)
+    start = np.concatenate([[0], np.cumsum(lens)[:-1]]).astype(np.int64)
+    length = np.array(lens, dtype=np.int64)
+    want = ao.attention_decode(c["q"], c["kc"], c["ks"], c["kg"], c["vc"], c["vs"], c["vg"], c["hd"], start, length, rope_theta=rope_theta)
+    dev = lambda a: torch.from_numpy(a).cuda()
+    ks, kg, vs, vg = dev(c["ks"]), dev(c["kg"]), dev(c["vs"]), dev(c["vg"])
+    outs = []
+    for _ in range(2):
+        out = torch.full((Bq, Hq, c["hd"]), 7.0, device="cuda")
+        B.gsrq_attention_decode(dev(c["q"]), dev(c["kc"]), B.codebook_of(ks, kg), SK, dev(c["vc"]), B.codebook_of(vs, vg), SV, Tc * c["M"],
+                                dev(start), dev(length), int(max(lens)), G, c["d"], 1.0 / np.sqrt(c["hd"]), rope_theta, out)
+        outs.append(out)
+    got = outs[0].cpu().numpy().astype(np.float64)
+    scale = np.abs(want).max()
+    assert np.abs(got - want).max() <= 2e-4 * scale, np.abs(got - want).max() / scale
+    for b, n in enumerate(lens):
+        if n == 0:
+            assert not got[b].any()
+    assert torch.equal(outs[0], outs[1])   # run-to-run bit identity

@@ -5,7 +5,7 @@ import numpy as np
 import pytest
 import torch
 
-from _harness import stats_np
+from paper_2607_01065_b200.pipeline import stats_np
 from oracle import gsrq_oracle as o
 
 pytestmark = pytest.mark.gpu

@@ -4,7 +4,7 @@ accepts, at sizes the oracle finishes in a fraction of a second.  BASELINE.json'
 import numpy as np
 import pytest
 
-from _harness import gpu_decode, gpu_gsrq
+from paper_2607_01065_b200.pipeline import gpu_decode, gpu_gsrq
 from oracle import gsrq_oracle as o
 from paper_2607_01065_b200 import inputs
 

@@ -5,7 +5,7 @@ import numpy as np
 import pytest
 import torch
 
-from _harness import gpu_decode, gpu_gsrq
+from paper_2607_01065_b200.pipeline import gpu_decode, gpu_gsrq
 from paper_2607_01065_b200 import inputs
 
 pytestmark = pytest.mark.gpu

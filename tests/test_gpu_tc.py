@@ -4,7 +4,7 @@ import numpy as np
 import pytest
 import torch
 
-from _harness import to_device
+from paper_2607_01065_b200.pipeline import to_device
 from oracle import gsrq_oracle as o
 from paper_2607_01065_b200 import inputs
 

@@ -5,7 +5,7 @@ import numpy as np
 import pytest
 import torch
 
-from _harness import gpu_gsrq, to_device
+from paper_2607_01065_b200.pipeline import gpu_gsrq, to_device
 from oracle import gsrq_oracle as o
 from oracle import variants_oracle as vo
 from paper_2607_01065_b200 import inputs

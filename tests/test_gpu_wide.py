@@ -5,7 +5,7 @@ import numpy as np
 import pytest
 import torch
 
-from _harness import gpu_decode, gpu_gsrq, stats_np, to_device
+from paper_2607_01065_b200.pipeline import gpu_decode, gpu_gsrq, stats_np, to_device
 from oracle import gsrq_oracle as o
 from paper_2607_01065_b200 import inputs
 
