@@ -336,32 +336,37 @@ def bf16_attention_baseline(Bq, ctx, G, Hq, hd, gen):
 
 def run_attention(B, pk):
     """Decode fused into attention (PAPER.md:443 (ii)): one decoding step of LLaMA-3-8B-shaped GQA (32 query / 8 KV heads, head_dim 128)
-    straight from S = 2 GSRQ codes, for the batch / context pairs of the paper's latency tables."""
-    G, Hq, hd, d, K, S = 8, 32, 128, 16, 256, 2
+    straight from the GSRQ codes, for the batch / context pairs of the paper's latency tables: the d = 16, S = 2 codes
+    of the headline config (table-lookup kernels) and the paper's own operating point D = 128, R = 12 (0.75 bits per element; the
+    dequantising kernel).  Each leg sits beside MEASURED library attention on a bf16 cache of the same shape."""
+    G, Hq, hd, K = 8, 32, 128, 256
     outl = []
     for Bq, ctx in ((8, 1024), (32, 1024), (1, 131072), (8, 131072)):
         T = Bq * ctx
         gen = torch.Generator(device="cuda"); gen.manual_seed(0)
-        kc = torch.randint(0, 256, (S, G, T * 8), dtype=torch.uint8, device="cuda", generator=gen)
-        vc = torch.randint(0, 256, (S, G, T * 8), dtype=torch.uint8, device="cuda", generator=gen)
-        sh = torch.nn.functional.normalize(torch.randn(G, S, K, d, device="cuda", generator=gen), dim=-1).contiguous()
-        ga = torch.rand(G, S, K, device="cuda", generator=gen).contiguous()
-        cb = B.codebook_of(sh, ga)
         q = torch.randn(Bq, Hq, hd, device="cuda", generator=gen)
         start = (torch.arange(Bq, device="cuda") * ctx).to(torch.int64)
         length = torch.full((Bq,), ctx, dtype=torch.int64, device="cuda")
         o_ = torch.zeros(Bq, Hq, hd, device="cuda")
         base = bf16_attention_baseline(Bq, ctx, G, Hq, hd, gen)
-        for theta in (0.0, 500000.0):
-            ws = B.gsrq_attention_decode(q, kc, cb, S, vc, cb, S, T * 8, start, length, ctx, G, d, hd ** -0.5, theta, o_)
-            md, mn = timed(lambda: B.gsrq_attention_decode(q, kc, cb, S, vc, cb, S, T * 8, start, length, ctx, G, d, hd ** -0.5, theta, o_, ws), reps=20)
-            code_bytes = 2 * S * G * T * 8
-            outl.append(dict(batch=Bq, context=ctx, rope=theta > 0, us=md * 1e3, us_min=mn * 1e3, code_bytes=code_bytes,
-                             codes_gb_per_s=code_bytes / (md * 1e-3) / 1e9, frac_of_copy_bw_on_code_bytes=code_bytes / (md * 1e-3) / 1e9 / pk["hbm_gbs"],
-                             bf16_cache_bytes=2 * G * T * hd * 2, us_to_read_bf16_cache_at_copy_bw=2 * G * T * hd * 2 / (pk["hbm_gbs"] * 1e9) * 1e6,
-                             bf16_attention_measured=base,
-                             speedup_over_measured_bf16_attention={k: v["us"] / (md * 1e3) for k, v in base.items() if "us" in v}))
-        del kc, vc
+        for d, S in ((16, 2), (128, 12)):
+            M = hd // d
+            kc = torch.randint(0, 256, (S, G, T * M), dtype=torch.uint8, device="cuda", generator=gen)
+            vc = torch.randint(0, 256, (S, G, T * M), dtype=torch.uint8, device="cuda", generator=gen)
+            sh = torch.nn.functional.normalize(torch.randn(G, S, K, d, device="cuda", generator=gen), dim=-1).contiguous()
+            ga = torch.rand(G, S, K, device="cuda", generator=gen).contiguous()
+            cb = B.codebook_of(sh, ga)
+            for theta in (0.0, 500000.0):
+                ws = B.gsrq_attention_decode(q, kc, cb, S, vc, cb, S, T * M, start, length, ctx, G, d, hd ** -0.5, theta, o_)
+                md, mn = timed(lambda: B.gsrq_attention_decode(q, kc, cb, S, vc, cb, S, T * M, start, length, ctx, G, d, hd ** -0.5, theta, o_, ws),
+                               reps=20 if d == 16 else 5)
+                code_bytes = 2 * S * G * T * M
+                outl.append(dict(batch=Bq, context=ctx, d=d, stages=S, rope=theta > 0, us=md * 1e3, us_min=mn * 1e3, code_bytes=code_bytes,
+                                 codes_gb_per_s=code_bytes / (md * 1e-3) / 1e9, frac_of_copy_bw_on_code_bytes=code_bytes / (md * 1e-3) / 1e9 / pk["hbm_gbs"],
+                                 bf16_cache_bytes=2 * G * T * hd * 2, us_to_read_bf16_cache_at_copy_bw=2 * G * T * hd * 2 / (pk["hbm_gbs"] * 1e9) * 1e6,
+                                 bf16_attention_measured=base,
+                                 speedup_over_measured_bf16_attention={k: v["us"] / (md * 1e3) for k, v in base.items() if "us" in v}))
+            del kc, vc
         torch.cuda.empty_cache()
     return outl
 

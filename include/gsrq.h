@@ -257,7 +257,10 @@ size_t gsrq_attention_workspace_bytes(int B, int Hq, int G, int64_t max_len);
  *            reaches beyond plane_rows / 8 tokens, is not read: it is served as an empty sequence (zeros).
  * B, G <= 65535; the codebooks' shapes arrays must be 16-byte aligned (GSRQ_EINVAL otherwise).  Code bytes >= K select a zero
  *            codeword here; the stand-alone decodes clamp them to K - 1 (cold paths) -- either way nothing outside the codebook is read.
- * This build serves hd = 128, d = 16, K <= 256, 1..4 stages, Hq / G <= 8.  fp32 arithmetic, no atomics: bit-reproducible.
+ * This build serves hd = 128, K <= 256, Hq / G <= 8, with d = 16 and 1..4 stages (table-lookup kernels, shared-memory codeword tables)
+ * or d = 128 and 1..32 stages (the paper's operating point: D = 128, R = 12 / 16 / 32; row = token, plane_rows =
+ * tokens in the planes; a dequantising kernel that reads the codeword rows from L2 -- functional, far from the d = 16 kernels'
+ * speed).  q must be 16-byte aligned.  fp32 arithmetic, no atomics: bit-reproducible.
  */
 int gsrq_attention_decode(const float *q, const uint8_t *k_codes, const gsrq_codebook *k_cb, int k_stages, const uint8_t *v_codes,
                           const gsrq_codebook *v_cb, int v_stages, int64_t plane_rows, const int64_t *seq_start, const int64_t *seq_len,
@@ -275,8 +278,8 @@ int gsrq_attention_decode(const float *q, const uint8_t *k_codes, const gsrq_cod
  * the per-split partial results go to a fixed buffer of GSRQ_ATTENTION_STATIC_SCRATCH_BYTES that is part of the library image.
  * Every GPU on which the library's kernels are loaded holds that buffer from then until the process exits, used or not.
  *
- * Arguments, arithmetic, shapes served and results are those of gsrq_attention_decode (bit-identical: same kernels, same split of
- * the token range), without `workspace` / `workspace_bytes`.  The caller still owns and passes q, the code planes, the codebooks,
+ * Arguments, arithmetic and results are those of gsrq_attention_decode (bit-identical: same kernels, same split of the token range),
+ * without `workspace` / `workspace_bytes`; it serves the d = 16 shapes (1..4 stages) only.  The caller still owns and passes q, the code planes, the codebooks,
  * seq_start / seq_len and out (device pointers).
  *
  * Limit: B * G * n_split * (Hq / G) * 130 * 4 bytes must fit in the buffer, n_split being the library's split of the token range

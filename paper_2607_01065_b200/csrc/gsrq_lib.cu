@@ -1327,9 +1327,20 @@ static int attn_splits(int B, int G, long long max_len) {
   return (int)want;
 }
 
+// d = 128: the dequantising kernel has no per-CTA table to amortise, so a split may be as short as 64 tokens (never fewer splits
+// than attn_splits gives: the workspace is sized for this count).
+static int attn_splits_wide(int B, int G, long long max_len) {
+  long long want = 4LL * sm_count() / ((long long)B * G);
+  const long long cap = (max_len + 63) / 64;
+  if (want > cap) want = cap;
+  if (want < 1) want = 1;
+  if (want > 256) want = 256;
+  return (int)want;
+}
+
 size_t gsrq_attention_workspace_bytes(int B, int Hq, int G, int64_t max_len) {
   if (B <= 0 || G <= 0 || Hq <= 0 || Hq % G || Hq / G > 8 || max_len < 0) { set_error("attention: bad B / Hq / G / max_len"); return 0; }
-  return align_up((size_t)B * G * attn_splits(B, G, max_len) * (Hq / G) * attn::kPartStride * sizeof(float)) + 256;
+  return align_up((size_t)B * G * attn_splits_wide(B, G, max_len) * (Hq / G) * attn::kPartStride * sizeof(float)) + 256;
 }
 
 int gsrq_attention_decode(const float *q, const uint8_t *k_codes, const gsrq_codebook *k_cb, int k_stages, const uint8_t *v_codes,
@@ -1340,14 +1351,19 @@ int gsrq_attention_decode(const float *q, const uint8_t *k_codes, const gsrq_cod
   if (!q || !k_codes || !v_codes || !k_cb || !v_cb || !k_cb->shapes || !k_cb->gains || !v_cb->shapes || !v_cb->gains || !seq_start || !seq_len || !out) {
     set_error("NULL input"); return GSRQ_EINVAL;
   }
-  if (hd != attn::kHd || d != attn::kD) { set_error("attention: this build serves head_dim 128 with d = 16 (got %d, %d)", hd, d); return GSRQ_EUNSUPPORTED; }
+  const bool wide_pt = (hd == attn::kHd && d == attn::kHd);   // the paper's operating point: one 128-wide sub-vector per token and head
+  if (hd != attn::kHd || (d != attn::kD && !wide_pt)) { set_error("attention: this build serves head_dim 128 with d = 16 or d = 128 (got %d, %d)", hd, d); return GSRQ_EUNSUPPORTED; }
+  const int max_stages = wide_pt ? GSRQ_MAX_STAGES : 4, rows_per_tok = wide_pt ? 1 : attn::kM;
   if (B <= 0 || G <= 0 || Hq <= 0 || Hq % G || Hq / G > 8) { set_error("attention: need Hq a multiple of G with at most 8 query heads per KV head"); return GSRQ_EINVAL; }
   if (B > 65535 || G > 65535) { set_error("attention: at most 65535 sequences and KV heads per call (grid limits), got B = %d, G = %d", B, G); return GSRQ_EINVAL; }
   if (((uintptr_t)k_cb->shapes & 15) || ((uintptr_t)v_cb->shapes & 15)) { set_error("codebook shapes must be 16-byte aligned"); return GSRQ_EINVAL; }
-  if (k_cb->K < 1 || k_cb->K > 256 || v_cb->K < 1 || v_cb->K > 256 || k_stages < 1 || k_stages > 4 || k_stages > k_cb->S || v_stages < 1 || v_stages > 4 ||
-      v_stages > v_cb->S) { set_error("attention: K in [1, 256] and 1..4 stages (<= S) for keys and values"); return GSRQ_EINVAL; }
-  if (plane_rows <= 0 || plane_rows % attn::kM || max_len < 0 || rope_theta < 0.0f) { set_error("attention: bad plane_rows / max_len / rope_theta"); return GSRQ_EINVAL; }
-  if (((uintptr_t)k_codes & 7) || ((uintptr_t)v_codes & 7)) { set_error("code planes must be 8-byte aligned"); return GSRQ_EINVAL; }
+  if (k_cb->K < 1 || k_cb->K > 256 || v_cb->K < 1 || v_cb->K > 256 || k_stages < 1 || k_stages > max_stages || k_stages > k_cb->S || v_stages < 1 ||
+      v_stages > max_stages || v_stages > v_cb->S) {
+    set_error("attention: K in [1, 256] and 1..%d stages (<= S) for keys and values at d = %d", max_stages, d); return GSRQ_EINVAL;
+  }
+  if (plane_rows <= 0 || plane_rows % rows_per_tok || max_len < 0 || rope_theta < 0.0f) { set_error("attention: bad plane_rows / max_len / rope_theta"); return GSRQ_EINVAL; }
+  if (!wide_pt && (((uintptr_t)k_codes & 7) || ((uintptr_t)v_codes & 7))) { set_error("code planes must be 8-byte aligned"); return GSRQ_EINVAL; }
+  if ((uintptr_t)q & 15) { set_error("q must be 16-byte aligned"); return GSRQ_EINVAL; }
   const size_t need = gsrq_attention_workspace_bytes(B, Hq, G, max_len);
   int rc = check_ws(workspace, workspace_bytes, need);
   if (rc) return rc;
@@ -1355,8 +1371,18 @@ int gsrq_attention_decode(const float *q, const uint8_t *k_codes, const gsrq_cod
   p.q = q; p.kc = k_codes; p.vc = v_codes; p.k_shapes = k_cb->shapes; p.k_gains = k_cb->gains; p.v_shapes = v_cb->shapes; p.v_gains = v_cb->gains;
   p.kS = k_cb->S; p.kK = k_cb->K; p.vS = v_cb->S; p.vK = v_cb->K; p.k_stages = k_stages; p.v_stages = v_stages; p.plane_rows = plane_rows;
   p.seq_start = (const long long *)seq_start; p.seq_len = (const long long *)seq_len; p.B = B; p.Hq = Hq; p.G = G; p.n_rep = Hq / G;
-  p.n_split = attn_splits(B, G, max_len); p.scale = scale; p.rope_theta = rope_theta; p.part = (float *)workspace; p.out = out;
+  p.n_split = wide_pt ? attn_splits_wide(B, G, max_len) : attn_splits(B, G, max_len);
+  p.scale = scale; p.rope_theta = rope_theta; p.part = (float *)workspace; p.out = out;
   const bool rope = rope_theta > 0.0f;
+  if (wide_pt) {   // d = 128: dequantising kernel (codeword rows from L2), then the same merge of the splits
+    const dim3 wgrid((unsigned)p.n_split, (unsigned)G, (unsigned)B);
+    if (rope) LAUNCH(kClsDecode, stream, (attn::k_attn_decode_wide<true><<<wgrid, attn::kThreads, 0, stream>>>(p)));
+    else LAUNCH(kClsDecode, stream, (attn::k_attn_decode_wide<false><<<wgrid, attn::kThreads, 0, stream>>>(p)));
+    GSRQ_CUDA_CHECK(cudaGetLastError());
+    LAUNCH(kClsDecode, stream, (attn::k_attn_combine<<<dim3((unsigned)Hq, (unsigned)B), 128, 0, stream>>>(p)));
+    GSRQ_CUDA_CHECK(cudaGetLastError());
+    return GSRQ_OK;
+  }
   const size_t smem = attn::attn_smem_bytes(k_stages, v_stages, p.n_rep, rope);
   if (smem > 227 * 1024) { set_error("attention: %d key stages x %d query heads per KV head do not fit in shared memory", k_stages, p.n_rep); return GSRQ_EUNSUPPORTED; }
   const dim3 grid((unsigned)p.n_split, (unsigned)G, (unsigned)B);

@@ -437,6 +437,121 @@ __global__ void __launch_bounds__(kThreads) k_attn_decode(AttnParams p) { attn_d
 template <int NREP, int NS>
 __global__ void __launch_bounds__(kThreads, 2) k_attn_decode_rope(AttnParams p) { attn_decode_body<true, NREP, NS>(p); }
 
+// ---- the paper's own operating point: d = head_dim = 128 (one sub-vector per token and head), up to 32 stages ----
+// The codeword tables of that point (stages x 256 x 128 fp32 = 1.5 MB per head at R = 12) do not fit in shared memory, so this
+// kernel dequantises from the codebooks as they lie in global memory (L2-resident: every CTA of a KV head reads the same rows):
+// a warp owns every 8th token of the split; lane l holds channels 4l .. 4l + 3 of khat_t and vhat_t (fp32 sums in stage order,
+// c = fl32(g_k s_k), exactly gsrq_decode's), rotates the key when rope_theta > 0 (pair (i, i + 64): lanes l and l ^ 16; angle in
+// double), reduces the n_rep logits over the warp and keeps a running max / sum / accumulator per query head.  The 8 warps are
+// merged in warp order into the same partial record the d = 16 kernels write (k_attn_combine merges the splits).  No atomics.
+// Functional first: per token it reads 2 x stages x 512 bytes of codeword rows from L2, which bounds it far below the HBM rate
+// of the codes.  grid = (n_split, G, B), block = 256, static shared memory only.
+template <bool ROPE>
+__global__ void __launch_bounds__(kThreads, 2) k_attn_decode_wide(AttnParams p) {
+  __shared__ float sm_m[8][8], sm_l[8][8];
+  __shared__ __align__(16) float sm_acc[8][8][kHd];   // [warp][head][channel]
+  const int sp = blockIdx.x, g = blockIdx.y, b = blockIdx.z, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int n_rep = p.n_rep;
+  const long long t_seq0 = p.seq_start[b];
+  long long len = p.seq_len[b];
+  if (t_seq0 < 0 || len < 0 || t_seq0 + len > p.plane_rows) len = 0;   // M = 1: plane_rows is the number of tokens in the planes
+  const long long per = (len + p.n_split - 1) / p.n_split;
+  const long long tb = (long long)sp * per, te = min(len, tb + per);
+  float q[8][4], acc[8][4], m_run[8], l_run[8];
+#pragma unroll
+  for (int h = 0; h < 8; ++h) {
+    const float4 v = (h < n_rep) ? *reinterpret_cast<const float4 *>(p.q + ((long long)b * p.Hq + (long long)g * n_rep + h) * kHd + 4 * lane)
+                                 : make_float4(0.f, 0.f, 0.f, 0.f);
+    q[h][0] = v.x; q[h][1] = v.y; q[h][2] = v.z; q[h][3] = v.w;
+    acc[h][0] = acc[h][1] = acc[h][2] = acc[h][3] = 0.0f;
+    m_run[h] = -INFINITY; l_run[h] = 0.0f;
+  }
+  double inv_freq[4] = {0.0, 0.0, 0.0, 0.0};
+  if (ROPE)
+#pragma unroll
+    for (int j = 0; j < 4; ++j) inv_freq[j] = pow((double)p.rope_theta, -(double)(4 * (lane & 15) + j) / 64.0);
+  const float *ksh = p.k_shapes + (long long)g * p.kS * p.kK * kHd, *kga = p.k_gains + (long long)g * p.kS * p.kK;
+  const float *vsh = p.v_shapes + (long long)g * p.vS * p.vK * kHd, *vga = p.v_gains + (long long)g * p.vS * p.vK;
+  // xhat = ((c_0 + c_1) + ...) in fp32, stage order; four stages' gain and row loads are issued together (latency), then added in order
+  auto dequant = [&](int code_l, int ns, const float *sh, const float *ga, int Kc, float (&x)[4]) {
+    for (int s0 = 0; s0 < ns; s0 += 4) {
+      float gk[4];
+      float4 sv[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int s = min(s0 + u, ns - 1);   // past the last stage: a valid (repeated) load that is not added
+        const long long cbi = (long long)s * Kc + __shfl_sync(0xffffffffu, code_l, s);
+        gk[u] = __ldg(ga + cbi);
+        sv[u] = __ldg(reinterpret_cast<const float4 *>(sh + cbi * kHd) + lane);
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        if (s0 + u >= ns) break;
+        const float c0 = __fmul_rn(gk[u], sv[u].x), c1 = __fmul_rn(gk[u], sv[u].y), c2 = __fmul_rn(gk[u], sv[u].z), c3 = __fmul_rn(gk[u], sv[u].w);
+        if (s0 + u == 0) { x[0] = c0; x[1] = c1; x[2] = c2; x[3] = c3; }
+        else { x[0] = __fadd_rn(x[0], c0); x[1] = __fadd_rn(x[1], c1); x[2] = __fadd_rn(x[2], c2); x[3] = __fadd_rn(x[3], c3); }
+      }
+    }
+  };
+  for (long long t = tb + warp; t < te; t += 8) {
+    // lane s holds the code byte of stage s (keys and values)
+    const long long tok = t_seq0 + t;
+    const int kcode = (lane < p.k_stages) ? min((int)p.kc[((long long)lane * p.G + g) * p.plane_rows + tok], p.kK - 1) : 0;
+    const int vcode = (lane < p.v_stages) ? min((int)p.vc[((long long)lane * p.G + g) * p.plane_rows + tok], p.vK - 1) : 0;
+    float kh[4], vh[4];
+    dequant(kcode, p.k_stages, ksh, kga, p.kK, kh);
+    dequant(vcode, p.v_stages, vsh, vga, p.vK, vh);
+    if (ROPE) {   // rotate-half: (a, b) = (x_i, x_{i + 64}) -> (a cos - b sin, b cos + a sin), angle = t * theta^(-2 i / 128)
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        double sn, cs;
+        sincos((double)t * inv_freq[j], &sn, &cs);
+        const float mine = kh[j], other = __shfl_xor_sync(0xffffffffu, mine, 16);
+        kh[j] = (lane < 16) ? fmaf(mine, (float)cs, -other * (float)sn) : fmaf(mine, (float)cs, other * (float)sn);
+      }
+    }
+#pragma unroll
+    for (int h = 0; h < 8; ++h) {
+      if (h >= n_rep) break;
+      float dot = fmaf(q[h][0], kh[0], fmaf(q[h][1], kh[1], fmaf(q[h][2], kh[2], q[h][3] * kh[3])));
+#pragma unroll
+      for (int off = 16; off; off >>= 1) dot += __shfl_xor_sync(0xffffffffu, dot, off);
+      const float lg = dot * p.scale;
+      const float m_new = fmaxf(m_run[h], lg);
+      const float resc = (m_run[h] == -INFINITY) ? 0.0f : expf(m_run[h] - m_new);
+      const float pr = expf(lg - m_new);
+      l_run[h] = fmaf(l_run[h], resc, pr);
+#pragma unroll
+      for (int j = 0; j < 4; ++j) acc[h][j] = fmaf(acc[h][j], resc, pr * vh[j]);
+      m_run[h] = m_new;
+    }
+  }
+  // ---- the split's record: the eight warps merged in warp order ----
+#pragma unroll
+  for (int h = 0; h < 8; ++h) {
+    if (h >= n_rep) break;
+    if (lane == 0) { sm_m[warp][h] = m_run[h]; sm_l[warp][h] = l_run[h]; }
+    *reinterpret_cast<float4 *>(&sm_acc[warp][h][4 * lane]) = make_float4(acc[h][0], acc[h][1], acc[h][2], acc[h][3]);
+  }
+  __syncthreads();
+  float *pp = p.part + (((long long)b * p.G + g) * p.n_split + sp) * n_rep * kPartStride;
+  for (int e = tid; e < n_rep * kHd; e += kThreads) {
+    const int h = e >> 7, c = e & 127;
+    float M = -INFINITY;
+#pragma unroll
+    for (int w8 = 0; w8 < 8; ++w8) M = fmaxf(M, sm_m[w8][h]);
+    float L = 0.0f, o = 0.0f;
+#pragma unroll
+    for (int w8 = 0; w8 < 8; ++w8) {
+      const float wgt = (sm_m[w8][h] == -INFINITY) ? 0.0f : expf(sm_m[w8][h] - M);
+      L = fmaf(sm_l[w8][h], wgt, L);
+      o = fmaf(sm_acc[w8][h][c], wgt, o);
+    }
+    pp[h * kPartStride + 2 + c] = o;
+    if (c == 0) { pp[h * kPartStride] = M; pp[h * kPartStride + 1] = L; }
+  }
+}
+
 // Merge the splits of one (sequence, query head) in split order.  grid = (Hq, B), block = 128.
 __global__ void __launch_bounds__(128) k_attn_combine(AttnParams p) {
   const int hq = blockIdx.x, b = blockIdx.y, e = threadIdx.x;
