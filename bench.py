@@ -48,6 +48,15 @@ def peaks():
     return dict(hbm_gbs=6650.0, bf16_tflops=1590.0, bf16_tflops_sustained=1400.0, source="fallback (B200_PROFILING.md)")
 
 
+def csrc_hash() -> str:
+    """sha256 over the library's kernel sources (names and contents, sorted): ties a committed ncu capture to the code it measured."""
+    import hashlib
+    h = hashlib.sha256()
+    for p in sorted((ROOT / "paper_2607_01065_b200" / "csrc").glob("*.cu*")):
+        h.update(p.name.encode()); h.update(p.read_bytes())
+    return h.hexdigest()
+
+
 def workload_config():
     """The `config` object of the JSON line: identical for both arms."""
     c = inputs.CONFIGS[4]
@@ -531,13 +540,20 @@ def main():
     # ---- rooflines: algorithmic work per launch / live launch duration ----
     tot_ms = sum(v[0] for v in prof.values())
 
+    traffic_file = "profiles/r3_traffic.csv"
+    traffic_stale = [None]
+
     def ncu_traffic(cls):
         """dram__bytes_read.sum + dram__bytes_write.sum per launch of the class (average over its launches per tensor), from the committed
-        ncu --set full capture of this command (profiles/r2_traffic.csv; not measured in this run); None without the file."""
+        ncu --set full capture of this command (not measured in this run).  The capture names the kernel sources it was taken on
+        (column csrc_sha256 = csrc_hash()); when they have changed since, the figure is stale and None is reported instead."""
         try:
             import csv
-            with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "profiles", "r2_traffic.csv")) as f:
+            with open(ROOT / traffic_file) as f:
                 rws = [r for r in csv.DictReader(f) if r["class"] == cls]
+            if not rws or any(r.get("csrc_sha256") != csrc_hash() for r in rws):
+                traffic_stale[0] = True
+                return None
             n_l = sum(int(r["launches_per_tensor"]) for r in rws)
             return sum((int(r["dram_bytes_read"]) + int(r["dram_bytes_write"])) * int(r["launches_per_tensor"]) for r in rws) / n_l if n_l else None
         except (OSError, KeyError, ValueError):
@@ -549,8 +565,9 @@ def main():
         peak = pk["bf16_tflops_sustained"] if bound == "tensor" else pk["hbm_gbs"]
         ach = work_per_launch / (per * 1e-3) / (1e12 if bound == "tensor" else 1e9) if per > 0 else 0.0
         return dict(bound=bound, kernel=name, achieved=ach, peak=peak, unit=unit, frac=ach / peak, traffic=ncu_traffic(cls),
-                    traffic_note="bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum, class average) from the committed ncu --set full capture "
-                                 "of this command: profiles/r2_traffic.csv, profiles/r2_ncu_summaries.md; not measured in this run",
+                    traffic_note=f"bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum, class average) from the committed ncu --set full capture "
+                                 f"of this command ({traffic_file}); not measured in this run; null when there is no capture of the current kernel "
+                                 f"sources (csrc hash {csrc_hash()[:12]})",
                     algorithmic_per_launch=work_per_launch, ms_per_launch=per, launches=n,
                     share_of_step=ms_c / tot_ms if tot_ms else None, note=note)
 

@@ -58,17 +58,20 @@ def test_wide_free_running_fit_encode_decode(B, kind, hd, d, G, T, K, S, iters):
     assert np.array_equal(got["residual"], ref["residual"])
 
 
-def test_wide_fused_encode_many_stages_and_prefix_decode(B):
-    """R = 12 stages at D = 128 (0.75 bits per element): one gsrq_encode of all stages with given codebooks equals
-    the oracle stage by stage; every prefix decodes alone; fits that re-derive their residual agree too."""
-    G, T, hd, d, K, S = 2, 640, 128, 128, 256, 12
-    x, w = _data("k", G, T, hd, 4300)
+@pytest.mark.parametrize("S,T,prefixes", [(12, 640, (1, 5, 12)),                   # R = 12: 0.75 bits per element
+                                          (16, 520, (4, 8, 12, 16)),               # R = 16: 1 bit per element
+                                          (32, 2048, (4, 8, 12, 16, 20, 24, 28, 32))])   # R = 32: 2 bits per element (GSRQ_MAX_STAGES); enough rows that no stage is degenerate
+def test_wide_fused_encode_many_stages_and_prefix_decode(B, S, T, prefixes):
+    """R = 12 / 16 / 32 stages at D = 128 (the paper's three bit rates): one gsrq_encode of all stages with given
+    codebooks equals the oracle stage by stage; prefixes decode alone; fits that re-derive their residual agree too."""
+    G, hd, d, K = 2, 128, 128, 256
+    x, w = _data("k", G, T, hd, 4300 + S)
     ref = o.gsrq_fit_encode(x, w, d, K, S, 2, seed=0)
     got = gpu_gsrq(x, w, d, K, S, 2, seed=0, dtype="bf16", pass_residual=False)   # fits re-derive the residual; one encode of [0, S)
     assert np.array_equal(got["codes"], ref["codes"])
     assert np.abs(got["shapes"] - ref["shapes"]).max() <= 1e-6 and np.abs(got["gains"] - ref["gains"]).max() <= 1e-5
     assert np.array_equal(got["residual"], ref["residual"])
-    for n in (1, 5, 12):
+    for n in prefixes:
         dec = gpu_decode(got["codes_dev"], got["cb"], n, G, T, hd, d, dtype="bf16")
         want, _ = o.decode(got["codes"][:n], got["shapes"][:, :n], got["gains"][:, :n], hd, bf16=True)
         assert np.array_equal(dec, want), n
